@@ -1,0 +1,196 @@
+"""CPU oracle for libmopal - TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+
+ctypes wrapper over ``mopal_oracle.c`` (long double parity build, plus the
+plain-double timed build).  Only ``tests/``, ``__graft_entry__.smoke()`` and
+``bench.py``'s cpu_baseline / ``--impl reference`` legs may import this package;
+nothing under ``paper_2601_19654_b200/`` does, and this package imports nothing
+from there.
+
+Arrays are numpy float64, SoA ``[3, ld]`` C-contiguous (component c of body b at
+``[c, b]``), bodies 0..nb-1 (the paper's element 1, the star, is not a body:
+PAPER.md:134).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "mopal_oracle.c")
+_LIBS = {"ld": os.path.join(_HERE, "libmopal_oracle.so"),
+         "f64": os.path.join(_HERE, "libmopal_oracle_f64.so")}
+_loaded = {}
+
+
+def build(force: bool = False) -> None:
+    """Compile both oracle builds with gcc (no CUDA involved)."""
+    stale = force or any((not os.path.exists(p)) or os.path.getmtime(p) < os.path.getmtime(_SRC)
+                         for p in _LIBS.values())
+    if stale:
+        subprocess.check_call(["sh", os.path.join(_HERE, "build_oracle.sh")])
+
+
+def _dp(a):
+    return a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def _lib(kind="ld"):
+    if kind in _loaded:
+        return _loaded[kind]
+    build()
+    L = C.CDLL(_LIBS[kind])
+    D, I, I64 = C.POINTER(C.c_double), C.c_int, C.c_int64
+    P32, PU8, PI64 = C.POINTER(C.c_int32), C.POINTER(C.c_uint8), C.POINTER(C.c_int64)
+    L.oracle_real_bytes.restype = I
+    L.oracle_changeover.restype = C.c_double
+    L.oracle_changeover.argtypes = [C.c_double, C.c_double]
+    L.oracle_accel.restype = I
+    L.oracle_accel.argtypes = [I, I, D, D, D, D, D]
+    L.oracle_boxes.restype = I
+    L.oracle_boxes.argtypes = [I, I, C.c_double, D, D, D, D, D, D, D]
+    L.oracle_pair_d2min.restype = C.c_double
+    L.oracle_pair_d2min.argtypes = [I, C.c_double, D, D, D, D, I, I]
+    L.oracle_encounters.restype = I64
+    L.oracle_encounters.argtypes = [I, I, C.c_double, D, D, D, D, D, P32, I64, PU8, P32, I64, PI64]
+    L.oracle_drift.restype = I
+    L.oracle_drift.argtypes = [I, I, C.c_double, C.c_double, D, D, P32]
+    L.oracle_kick.restype = I
+    L.oracle_kick.argtypes = [I, I, C.c_double, D, D]
+    L.oracle_jump.restype = I
+    L.oracle_jump.argtypes = [I, I, C.c_double, C.c_double, D, D, D, D]
+    L.oracle_step.restype = I64
+    L.oracle_step.argtypes = [I, I, C.c_double, D, D, C.c_double, D, D, D, D, D,
+                              P32, I64, PU8, P32, I64, PI64, P32]
+    L.oracle_step_noenc.restype = I
+    L.oracle_step_noenc.argtypes = [I, I, C.c_double, D, D, C.c_double, D, D, D]
+    _loaded[kind] = L
+    return L
+
+
+def _soa(a):
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    assert a.ndim == 2 and a.shape[0] == 3, a.shape
+    return a
+
+
+def _vec(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def real_bytes(kind="ld") -> int:
+    return _lib(kind).oracle_real_bytes()
+
+
+def set_threads(n: int) -> None:
+    os.environ["OMP_NUM_THREADS"] = str(int(n))
+
+
+def changeover(r: float, rc: float, kind="ld") -> float:
+    """K(r; rc): quintic smoothstep between 0.1 rc and rc (reading A-1)."""
+    return float(_lib(kind).oracle_changeover(float(r), float(rc)))
+
+
+def accel(gm, x, rcrit, kind="ld"):
+    """O-A.  Returns (a[3,nb], S[3,nb]) with S = sum_j |term| for the tolerance."""
+    x = _soa(x); gm = _vec(gm); rcrit = _vec(rcrit)
+    nb = x.shape[1]
+    a = np.zeros_like(x); S = np.zeros_like(x)
+    rc = _lib(kind).oracle_accel(nb, nb, _dp(gm), _dp(x), _dp(rcrit), _dp(a), _dp(S))
+    assert rc == 0
+    return a, S
+
+
+def boxes(h, x0, v0, x1, v1, rcrit, kind="ld"):
+    """O-B.1.  Returns (lo[2,nb], hi[2,nb]) for x and y."""
+    x0, v0, x1, v1 = map(_soa, (x0, v0, x1, v1)); rcrit = _vec(rcrit)
+    nb = x0.shape[1]
+    lo = np.zeros((2, nb)); hi = np.zeros((2, nb))
+    rc = _lib(kind).oracle_boxes(nb, nb, float(h), _dp(x0), _dp(v0), _dp(x1), _dp(v1),
+                                 _dp(rcrit), _dp(lo), _dp(hi))
+    assert rc == 0
+    return lo, hi
+
+
+def pair_d2min(h, x0, v0, x1, v1, i, j, kind="ld") -> float:
+    x0, v0, x1, v1 = map(_soa, (x0, v0, x1, v1))
+    nb = x0.shape[1]
+    return float(_lib(kind).oracle_pair_d2min(nb, float(h), _dp(x0), _dp(v0), _dp(x1), _dp(v1),
+                                              int(i), int(j)))
+
+
+def encounters(h, x0, v0, x1, v1, rcrit, cap=None, kind="ld"):
+    """O-B.  Returns dict(pairs[n,2] sorted, count (true total), flag[nb] uint8,
+    ambig[m,2], n_ambig)."""
+    x0, v0, x1, v1 = map(_soa, (x0, v0, x1, v1)); rcrit = _vec(rcrit)
+    nb = x0.shape[1]
+    L = _lib(kind)
+    if cap is None:
+        cap = 1 << 16
+    while True:
+        pairs = np.zeros((max(cap, 1), 2), dtype=np.int32)
+        amb = np.zeros((max(cap, 1), 2), dtype=np.int32)
+        flag = np.zeros(max(nb, 1), dtype=np.uint8)
+        n_amb = C.c_int64(0)
+        cnt = L.oracle_encounters(nb, nb, float(h), _dp(x0), _dp(v0), _dp(x1), _dp(v1), _dp(rcrit),
+                                  pairs.ctypes.data_as(C.POINTER(C.c_int32)), cap,
+                                  flag.ctypes.data_as(C.POINTER(C.c_uint8)),
+                                  amb.ctypes.data_as(C.POINTER(C.c_int32)), cap, C.byref(n_amb))
+        assert cnt >= 0
+        if cnt <= cap and n_amb.value <= cap:
+            break
+        cap = int(max(cnt, n_amb.value))
+    return dict(pairs=pairs[:cnt].copy(), count=int(cnt), flag=flag[:nb].copy(),
+                ambig=amb[:n_amb.value].copy(), n_ambig=int(n_amb.value))
+
+
+def drift(mu, dt, x, v, kind="ld"):
+    """O-C.  Returns (x1, v1, iflag[nb])."""
+    x = _soa(x).copy(); v = _soa(v).copy()
+    nb = x.shape[1]
+    iflag = np.zeros(max(nb, 1), dtype=np.int32)
+    nf = _lib(kind).oracle_drift(nb, nb, float(mu), float(dt), _dp(x), _dp(v),
+                                 iflag.ctypes.data_as(C.POINTER(C.c_int32)))
+    assert nf >= 0
+    return x, v, iflag[:nb]
+
+
+def kick(hk, v, a, kind="ld"):
+    v = _soa(v).copy(); a = _soa(a)
+    _lib(kind).oracle_kick(v.shape[1], v.shape[1], float(hk), _dp(v), _dp(a))
+    return v
+
+
+def jump(hj, mu, gm, x, v, kind="ld"):
+    """Returns (x_new, P[3]) with P = sum gm_j v_j."""
+    x = _soa(x).copy(); v = _soa(v); gm = _vec(gm)
+    P = np.zeros(3)
+    _lib(kind).oracle_jump(x.shape[1], x.shape[1], float(hj), float(mu), _dp(gm), _dp(x), _dp(v), _dp(P))
+    return x, P
+
+
+def step(mu, gm, rcrit, h, x, v, a, cap=1 << 16, with_encounters=True, kind="ld"):
+    """O-D, one hybrid step.  Returns dict(x, v, a, x0, v0, pairs, count, flag, ambig, n_ambig, nfail)."""
+    x = _soa(x).copy(); v = _soa(v).copy(); a = _soa(a).copy()
+    gm = _vec(gm); rcrit = _vec(rcrit)
+    nb = x.shape[1]
+    L = _lib(kind)
+    if not with_encounters:
+        rc = L.oracle_step_noenc(nb, nb, float(mu), _dp(gm), _dp(rcrit), float(h), _dp(x), _dp(v), _dp(a))
+        assert rc == 0
+        return dict(x=x, v=v, a=a)
+    x0 = np.zeros_like(x); v0 = np.zeros_like(v)
+    pairs = np.zeros((cap, 2), dtype=np.int32); amb = np.zeros((cap, 2), dtype=np.int32)
+    flag = np.zeros(max(nb, 1), dtype=np.uint8)
+    n_amb = C.c_int64(0); nfail = C.c_int32(0)
+    P32 = C.POINTER(C.c_int32)
+    cnt = L.oracle_step(nb, nb, float(mu), _dp(gm), _dp(rcrit), float(h), _dp(x), _dp(v), _dp(a),
+                        _dp(x0), _dp(v0), pairs.ctypes.data_as(P32), cap,
+                        flag.ctypes.data_as(C.POINTER(C.c_uint8)), amb.ctypes.data_as(P32), cap,
+                        C.byref(n_amb), C.byref(nfail))
+    assert cnt >= 0
+    return dict(x=x, v=v, a=a, x0=x0, v0=v0, pairs=pairs[:min(cnt, cap)].copy(), count=int(cnt),
+                flag=flag[:nb].copy(), ambig=amb[:min(n_amb.value, cap)].copy(),
+                n_ambig=int(n_amb.value), nfail=int(nfail.value))

@@ -1,0 +1,541 @@
+/*
+ * mopal_oracle.c - TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+ *
+ * A plain, slow, obviously-correct CPU restatement of the hot path of Mercury's
+ * hybrid symplectic step as the Mercury-Opal paper (arxiv 2601.19654) lays it
+ * out: the O(N^2) K(r)-weighted mutual-gravity sum (force block, LOOP 2,
+ * PAPER.md:150-165), the interaction/stellar-Hamiltonian block (kick, mvsum
+ * reduction, jump, x0/v0 copy), the per-body Kepler drift
+ * and the close-encounter check (mce_snif LOOPs 1-3,
+ * PAPER.md:243-276), in the step order of PAPER.md:134.
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / reference
+ * legs may load this.  It shares no code, header, table or helper with the CUDA
+ * path under paper_2601_19654_b200/csrc and neither includes the other.
+ *
+ * Arithmetic: every intermediate and every accumulator is `real`
+ * (= long double, x87 80-bit, eps 5.4e-20) ; inputs and outputs are double.
+ * Straight double loops in the paper's loop order, no tiling, no SIMD, no
+ * reordering.  `#pragma omp parallel for` over the OUTER body loop only (each
+ * body's own sum is still sequential, ascending j) - it changes no result.
+ * Built a second time with -DORACLE_DOUBLE (real = double) purely as the timed
+ * CPU baseline; the parity oracle is the long double build.
+ *
+ * The paper prints loop skeletons with the physics elided in <...> placeholders
+ * and no equation; the arithmetic below follows the readings listed in
+ * DESIGN.md section "Readings" (A-1..A-10, B-a..B-i, C-a..C-f, S-1..S-5), which
+ * restate the paper's cited lineage (Chambers 1999; universal
+ * variable Kepler solver as in WHFast).
+ *
+ * Layout: SoA planes, component c of body b at [c*ld + b], b = 0..nb-1
+ * (paper index = b + 2; its element 1 is the star).
+ *
+ * Pins (tests/test_oracle_*.py, -m "not gpu"):
+ *   accel      : mpmath brute force N<=8, Newton III, ring closed form, K limits,
+ *                two-body closed form                               -> pinned
+ *   boxes/pairs: mpmath brute force N<=8, straight-line closest approach closed
+ *                form, dense sampling of the Hermite cubic, permutation /
+ *                translation / time-reversal invariances            -> pinned
+ *   drift      : period return + energy, circular closed form, fg determinant,
+ *                group property, mpmath elements-based propagation  -> pinned
+ *   step       : nb=1 by hand, angular momentum, reversibility, dt^2 energy
+ *                scaling                                            -> pinned
+ *   multi-step trajectories beyond ~10 steps: parity unpinned by construction
+ *   (chaos; the paper itself compares curves and medians).
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+#ifdef ORACLE_DOUBLE
+typedef double real;
+#define R_SQRT sqrt
+#define R_FABS fabs
+#define R_EPS 2.220446049250313e-16
+#else
+typedef long double real;
+#define R_SQRT sqrtl
+#define R_FABS fabsl
+#define R_EPS 1.0842021724855044e-19L
+#endif
+
+#define X_(p, c, b) ((real)(p)[(size_t)(c) * (size_t)ld + (size_t)(b)])
+
+static inline real rmax(real a, real b) { return a > b ? a : b; }
+static inline real rmin(real a, real b) { return a < b ? a : b; }
+
+int oracle_real_bytes(void) { return (int)sizeof(real); }
+
+/* ---------------------------------------------------------------------------
+ * Changeover weight K(s ; rc)  [reading A-1, A-4, A-5; PAPER.md:104 fn. 14]
+ *   q = (s - 0.1 rc) / (0.9 rc);  K = 0 (q<=0), 1 (q>=1), else q^3 (10 - 15 q + 6 q^2)
+ * decided on squared quantities exactly as O-A states:
+ *   s2 >= rc^2 -> 1 ; s2 <= (0.1 rc)^2 -> 0.
+ * ------------------------------------------------------------------------- */
+static real changeover_s2(real s2, real rc)
+{
+    real rc2 = rc * rc;
+    if (s2 >= rc2) return 1;
+    real rin = (real)0.1L * rc;
+    if (s2 <= rin * rin) return 0;
+    real s = R_SQRT(s2);
+    real q = (s - rin) / ((real)0.9L * rc);
+    return q * q * q * ((real)10 - (real)15 * q + (real)6 * q * q);
+}
+
+double oracle_changeover(double r, double rc)
+{
+    real rr = (real)r;
+    return (double)changeover_s2(rr * rr, (real)rc);
+}
+
+/* ---------------------------------------------------------------------------
+ * O-A  acceleration (force block LOOP 2):
+ *   a_i = sum_{j != i} gm_j K_ij (x_j - x_i) / r_ij^3 ,  rc = max(rcrit_i, rcrit_j)
+ * body-body terms only (the star is the drift's, the indirect term the jump's;
+ * reading A-7).  S (nullable) receives sum_j |term| per component for the
+ * parity tolerance |a_gpu - a_ref| <= 1e-12 S.
+ * ------------------------------------------------------------------------- */
+int oracle_accel(int nb, int ld, const double *gm, const double *x,
+                 const double *rcrit, double *a, double *S)
+{
+    if (nb < 0 || ld < nb) return 1;
+#pragma omp parallel for schedule(static)
+    for (int i = 0; i < nb; ++i) {
+        real xi = X_(x, 0, i), yi = X_(x, 1, i), zi = X_(x, 2, i);
+        real rci = (real)rcrit[i];
+        real ax = 0, ay = 0, az = 0, sx = 0, sy = 0, sz = 0;
+        for (int j = 0; j < nb; ++j) {
+            if (j == i) continue;
+            real dx = X_(x, 0, j) - xi;
+            real dy = X_(x, 1, j) - yi;
+            real dz = X_(x, 2, j) - zi;
+            real s2 = dx * dx + dy * dy + dz * dz;
+            if (s2 == 0) continue;                       /* reading A-9 */
+            real rc = rmax(rci, (real)rcrit[j]);         /* reading A-3 */
+            real K = changeover_s2(s2, rc);
+            if (K == 0) continue;
+            real w = (real)gm[j] * K / (s2 * R_SQRT(s2));
+            ax += w * dx; ay += w * dy; az += w * dz;
+            sx += R_FABS(w * dx); sy += R_FABS(w * dy); sz += R_FABS(w * dz);
+        }
+        a[0 * (size_t)ld + i] = (double)ax;
+        a[1 * (size_t)ld + i] = (double)ay;
+        a[2 * (size_t)ld + i] = (double)az;
+        if (S) {
+            S[0 * (size_t)ld + i] = (double)sx;
+            S[1 * (size_t)ld + i] = (double)sy;
+            S[2 * (size_t)ld + i] = (double)sz;
+        }
+    }
+    return 0;
+}
+
+/* ---------------------------------------------------------------------------
+ * O-B.1  boxes (mce_snif LOOP 1 + LOOP 2; readings B-a,b,c)
+ * Per body and per coordinate c in {x, y}: extremes of the cubic Hermite
+ * interpolant through (p0, h w0) at tau=0 and (p1, h w1) at tau=1, padded by
+ * rcrit.  lo/hi: [2][nb] (x plane then y plane).
+ * ------------------------------------------------------------------------- */
+static void box_1d(real p0, real p1, real w0, real w1, real h, real *lo, real *hi)
+{
+    real l = rmin(p0, p1), u = rmax(p0, p1);
+    if (w0 * w1 < 0) {
+        real k1 = h * w0;
+        real k2 = -(real)3 * p0 - (real)2 * h * w0 + (real)3 * p1 - h * w1;
+        real k3 = (real)2 * p0 + h * w0 - (real)2 * p1 + h * w1;
+        real D = k2 * k2 - (real)3 * k3 * k1;
+        if (D >= 0) {
+            real sq = R_SQRT(D);
+            real qq = (k2 >= 0) ? (k2 + sq) : (k2 - sq);
+            if (qq != 0) {
+                real ta = -k1 / qq;
+                if (ta > 0 && ta < 1) {
+                    real p = ((k3 * ta + k2) * ta + k1) * ta + p0;
+                    l = rmin(l, p); u = rmax(u, p);
+                }
+            }
+            if (k3 != 0) {
+                real tb = -qq / ((real)3 * k3);
+                if (tb > 0 && tb < 1) {
+                    real p = ((k3 * tb + k2) * tb + k1) * tb + p0;
+                    l = rmin(l, p); u = rmax(u, p);
+                }
+            }
+        }
+    }
+    *lo = l; *hi = u;
+}
+
+static void boxes_real(int nb, int ld, real h, const double *x0, const double *v0,
+                       const double *x1, const double *v1, const double *rcrit,
+                       real *lo, real *hi)
+{
+#pragma omp parallel for schedule(static)
+    for (int b = 0; b < nb; ++b) {
+        for (int c = 0; c < 2; ++c) {
+            real l, u;
+            box_1d(X_(x0, c, b), X_(x1, c, b), X_(v0, c, b), X_(v1, c, b), h, &l, &u);
+            lo[(size_t)c * nb + b] = l - (real)rcrit[b];
+            hi[(size_t)c * nb + b] = u + (real)rcrit[b];
+        }
+    }
+}
+
+int oracle_boxes(int nb, int ld, double h, const double *x0, const double *v0,
+                 const double *x1, const double *v1, const double *rcrit,
+                 double *lo, double *hi)
+{
+    if (nb < 0 || ld < nb) return 1;
+    real *l = (real *)malloc(sizeof(real) * 2 * (size_t)(nb + 1));
+    real *u = (real *)malloc(sizeof(real) * 2 * (size_t)(nb + 1));
+    if (!l || !u) { free(l); free(u); return 2; }
+    boxes_real(nb, ld, (real)h, x0, v0, x1, v1, rcrit, l, u);
+    for (size_t k = 0; k < 2 * (size_t)nb; ++k) { lo[k] = (double)l[k]; hi[k] = (double)u[k]; }
+    free(l); free(u);
+    return 0;
+}
+
+/* ---------------------------------------------------------------------------
+ * O-B.2  minimum separation estimate of one pair over the step (mce_min,
+ * PAPER.md:261-262, 281-283; reading B-d): cubic Hermite interpolant of the
+ * SQUARED separation, interior minimum only when approaching at the start and
+ * receding at the end.  Returns d2min; d0/d1 (nullable) get the end values.
+ * ------------------------------------------------------------------------- */
+static real pair_d2min(int ld, real h, const double *x0, const double *v0,
+                       const double *x1, const double *v1, int i, int j,
+                       real *d0_out, real *d1_out)
+{
+    real d0 = 0, d1 = 0, s0 = 0, s1 = 0;
+    for (int c = 0; c < 3; ++c) {
+        real D0 = X_(x0, c, i) - X_(x0, c, j);
+        real D1 = X_(x1, c, i) - X_(x1, c, j);
+        real U0 = X_(v0, c, i) - X_(v0, c, j);
+        real U1 = X_(v1, c, i) - X_(v1, c, j);
+        d0 += D0 * D0; d1 += D1 * D1;
+        s0 += D0 * U0; s1 += D1 * U1;
+    }
+    real d0t = (real)2 * s0, d1t = (real)2 * s1;
+    real d2min;
+    if (d0t * h <= 0 && d1t * h >= 0) {
+        real c1 = h * d0t;
+        real c2 = -(real)3 * d0 - (real)2 * h * d0t + (real)3 * d1 - h * d1t;
+        real c3 = (real)2 * d0 + h * d0t - (real)2 * d1 + h * d1t;
+        real D = rmax(c2 * c2 - (real)3 * c3 * c1, 0);
+        real den = c2 + R_SQRT(D);
+        real tau = (den > 0) ? (-c1 / den) : (real)0;
+        tau = rmin(rmax(tau, 0), 1);
+        d2min = rmax(((c3 * tau + c2) * tau + c1) * tau + d0, 0);
+        d2min = rmin(d2min, rmin(d0, d1));
+    } else {
+        d2min = rmin(d0, d1);
+    }
+    if (d0_out) *d0_out = d0;
+    if (d1_out) *d1_out = d1;
+    return d2min;
+}
+
+double oracle_pair_d2min(int ld, double h, const double *x0, const double *v0,
+                         const double *x1, const double *v1, int i, int j)
+{
+    return (double)pair_d2min(ld, (real)h, x0, v0, x1, v1, i, j, 0, 0);
+}
+
+/* classify one pair: 0 = out, 1 = in (flagged), bit 1 set (|2) = ambiguous:
+ * some comparison deciding the outcome sits within 1e-12 relative of equality
+ * (north_star: lists bit-exact "except for pairs within 1e-12 relative of a
+ * threshold"). */
+#define AMBIG_TOL ((real)1e-12L)
+static int near_eq(real a, real b, real scale)
+{
+    return R_FABS(a - b) <= AMBIG_TOL * scale;
+}
+
+static int classify_pair(int nb, int ld, real h, const double *x0, const double *v0,
+                         const double *x1, const double *v1, const double *rcrit,
+                         const real *lo, const real *hi, int i, int j)
+{
+    int amb = 0, gate = 1;
+    for (int c = 0; c < 2; ++c) {                        /* box gate, reading B-f */
+        real li = lo[(size_t)c * nb + i], ui = hi[(size_t)c * nb + i];
+        real lj = lo[(size_t)c * nb + j], uj = hi[(size_t)c * nb + j];
+        if (!(li <= uj)) gate = 0;
+        if (!(lj <= ui)) gate = 0;
+        if (near_eq(li, uj, rmax(R_FABS(li), R_FABS(uj)))) amb = 1;
+        if (near_eq(lj, ui, rmax(R_FABS(lj), R_FABS(ui)))) amb = 1;
+    }
+    if (!gate && !amb) return 0;
+    real d0, d1;
+    real d2 = pair_d2min(ld, h, x0, v0, x1, v1, i, j, &d0, &d1);
+    real rc = rmax((real)rcrit[i], (real)rcrit[j]);      /* reading B-e */
+    real rc2 = rc * rc;
+    int in = gate && (d2 <= rc2);
+    int amb2 = near_eq(d2, rc2, rmax(rc2, rmax(d0, d1)));
+    /* ambiguity matters only if flipping the near-equal comparison could flip
+       the outcome: a near-equal gate with the distance test failing clearly is
+       still a clear "out". */
+    int ambiguous = 0;
+    if (amb2 && (gate || amb)) ambiguous = 1;
+    if (amb && (d2 <= rc2 || amb2)) ambiguous = 1;
+    return in | (ambiguous ? 2 : 0);
+}
+
+/* ---------------------------------------------------------------------------
+ * O-B  encounter list (mce_snif LOOP 3).  All i<j, ascending
+ * i then ascending j (the paper's order is whatever its atomics give,
+ * PAPER.md:264-269; reading B-g).  pairs: 2*cap int32 (i,j interleaved), count
+ * returned is the TRUE total even if > cap.  flag[b]=1 iff b is in a flagged
+ * pair (paper: ce=2).  ambig (nullable): pairs whose outcome
+ * is within 1e-12 relative of a threshold, n_ambig = their true number.
+ * ------------------------------------------------------------------------- */
+int64_t oracle_encounters(int nb, int ld, double h_, const double *x0, const double *v0,
+                          const double *x1, const double *v1, const double *rcrit,
+                          int32_t *pairs, int64_t cap, uint8_t *flag,
+                          int32_t *ambig, int64_t ambig_cap, int64_t *n_ambig)
+{
+    if (nb < 0 || ld < nb) return -1;
+    real h = (real)h_;
+    real *lo = (real *)malloc(sizeof(real) * 2 * (size_t)(nb + 1));
+    real *hi = (real *)malloc(sizeof(real) * 2 * (size_t)(nb + 1));
+    int64_t *rowcnt = (int64_t *)calloc((size_t)nb + 1, sizeof(int64_t));
+    int64_t *rowamb = (int64_t *)calloc((size_t)nb + 1, sizeof(int64_t));
+    if (!lo || !hi || !rowcnt || !rowamb) { free(lo); free(hi); free(rowcnt); free(rowamb); return -2; }
+    boxes_real(nb, ld, h, x0, v0, x1, v1, rcrit, lo, hi);
+    if (flag) memset(flag, 0, (size_t)nb);
+    /* pass 1: per-row counts */
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int i = 0; i < nb; ++i) {
+        int64_t c = 0, ca = 0;
+        for (int j = i + 1; j < nb; ++j) {
+            int r = classify_pair(nb, ld, h, x0, v0, x1, v1, rcrit, lo, hi, i, j);
+            c += (r & 1); ca += ((r >> 1) & 1);
+        }
+        rowcnt[i] = c; rowamb[i] = ca;
+    }
+    int64_t total = 0, total_a = 0;
+    for (int i = 0; i < nb; ++i) {
+        int64_t c = rowcnt[i], ca = rowamb[i];
+        rowcnt[i] = total; rowamb[i] = total_a;
+        total += c; total_a += ca;
+    }
+    /* pass 2: fill in order */
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int i = 0; i < nb; ++i) {
+        int64_t o = rowcnt[i], oa = rowamb[i];
+        int64_t ne = ((i + 1 < nb) ? rowcnt[i + 1] : total) - o;
+        int64_t na = ((i + 1 < nb) ? rowamb[i + 1] : total_a) - oa;
+        if (ne == 0 && na == 0) continue;
+        for (int j = i + 1; j < nb; ++j) {
+            int r = classify_pair(nb, ld, h, x0, v0, x1, v1, rcrit, lo, hi, i, j);
+            if (r & 1) {
+                if (pairs && o < cap) { pairs[2 * o] = i; pairs[2 * o + 1] = j; }
+                ++o;
+                if (flag) {                              /* from the definition, not the (maybe truncated) list */
+#pragma omp atomic write
+                    flag[i] = 1;
+#pragma omp atomic write
+                    flag[j] = 1;
+                }
+            }
+            if (r & 2) {
+                if (ambig && oa < ambig_cap) { ambig[2 * oa] = i; ambig[2 * oa + 1] = j; }
+                ++oa;
+            }
+        }
+    }
+    if (n_ambig) *n_ambig = total_a;
+    free(lo); free(hi); free(rowcnt); free(rowamb);
+    return total;
+}
+
+/* ---------------------------------------------------------------------------
+ * O-C  Kepler drift (arxes_drift; readings C-a..C-f).
+ * Universal variables: c_n(z) = sum_k (-z)^k / (2k+n)!,  G_n = X^n c_n(beta X^2)
+ *   solve  r0 G1 + eta0 G2 + mu G3 = dt  for X   (F' = r > 0: unique root)
+ *   f = 1 - mu G2 / r0, g = dt - mu G3, fdot = -mu G1 / (r0 r), gdot = 1 - mu G2 / r
+ * ------------------------------------------------------------------------- */
+static void stumpff(real z, real *c0, real *c1, real *c2, real *c3)
+{
+    int n = 0;
+    while (R_FABS(z) > (real)0.1L) { z *= (real)0.25L; ++n; }
+    /* series: c2 = 1/2! - z/4! + z^2/6! - ... ; c3 = 1/3! - z/5! + z^2/7! - ... */
+    real t2 = (real)0.5L, t3 = (real)1 / (real)6, s2 = 0, s3 = 0;
+    for (int k = 1; k <= 30; ++k) {
+        s2 += t2; s3 += t3;
+        t2 *= -z / (real)((2 * k + 1) * (2 * k + 2));
+        t3 *= -z / (real)((2 * k + 2) * (2 * k + 3));
+        if (R_FABS(t2) < R_EPS * (real)0.01L && R_FABS(t3) < R_EPS * (real)0.01L) break;
+    }
+    s2 += t2; s3 += t3;
+    real C2 = s2, C3 = s3;
+    real C1 = (real)1 - z * C3;
+    real C0 = (real)1 - z * C2;
+    for (; n > 0; --n) {                                 /* undo each quartering */
+        C3 = (C2 + C0 * C3) * (real)0.25L;
+        C2 = C1 * C1 * (real)0.5L;
+        C1 = C0 * C1;
+        C0 = (real)2 * C0 * C0 - (real)1;
+    }
+    *c0 = C0; *c1 = C1; *c2 = C2; *c3 = C3;
+}
+
+static void gfuncs(real X, real beta, real *G0, real *G1, real *G2, real *G3)
+{
+    real c0, c1, c2, c3;
+    real X2 = X * X;
+    stumpff(beta * X2, &c0, &c1, &c2, &c3);
+    *G0 = c0; *G1 = X * c1; *G2 = X2 * c2; *G3 = X2 * X * c3;
+}
+
+/* one body; returns 0 ok, 1 failed (state untouched) */
+static int drift_one(real mu, real dt, real *px, real *pv)
+{
+    real x0 = px[0], y0 = px[1], z0 = px[2], vx = pv[0], vy = pv[1], vz = pv[2];
+    real r0 = R_SQRT(x0 * x0 + y0 * y0 + z0 * z0);
+    if (!(r0 > 0)) return 1;                             /* reading C-f */
+    real v2 = vx * vx + vy * vy + vz * vz;
+    real eta0 = x0 * vx + y0 * vy + z0 * vz;
+    real beta = (real)2 * mu / r0 - v2;
+    real X = dt / r0, G0, G1, G2, G3, r = r0;
+    int conv = 0;
+    for (int it = 0; it < 60; ++it) {
+        gfuncs(X, beta, &G0, &G1, &G2, &G3);
+        real F = r0 * G1 + eta0 * G2 + mu * G3 - dt;
+        r = r0 * G0 + eta0 * G1 + mu * G2;
+        if (!(r > 0) || !isfinite((double)F)) break;
+        real dX = -F / r;
+        X += dX;
+        if (R_FABS(dX) <= (real)4 * R_EPS * R_FABS(X)) { conv = 1; break; }
+    }
+    if (!conv) {
+        /* bisection on a bracket grown from 0 (F(0) = -dt, F monotone in X) */
+        real sgn = dt >= 0 ? (real)1 : (real)-1;
+        real a = 0, b = sgn * R_FABS(dt / r0);
+        int ok = 0;
+        for (int it = 0; it < 200; ++it) {
+            gfuncs(b, beta, &G0, &G1, &G2, &G3);
+            real F = r0 * G1 + eta0 * G2 + mu * G3 - dt;
+            if (!isfinite((double)F)) return 1;
+            if (F * sgn >= 0) { ok = 1; break; }
+            a = b; b *= (real)2;
+        }
+        if (!ok) return 1;
+        for (int it = 0; it < 200; ++it) {
+            real m = (real)0.5L * (a + b);
+            gfuncs(m, beta, &G0, &G1, &G2, &G3);
+            real F = r0 * G1 + eta0 * G2 + mu * G3 - dt;
+            if (F * sgn >= 0) b = m; else a = m;
+            if (R_FABS(b - a) <= (real)2 * R_EPS * R_FABS(b)) break;
+        }
+        X = (real)0.5L * (a + b);
+    }
+    gfuncs(X, beta, &G0, &G1, &G2, &G3);
+    r = r0 * G0 + eta0 * G1 + mu * G2;
+    if (!(r > 0)) return 1;
+    real fm1 = -mu * G2 / r0;                            /* f - 1 */
+    real g = dt - mu * G3;
+    real fd = -mu * G1 / (r0 * r);
+    real gdm1 = -mu * G2 / r;                            /* gdot - 1 */
+    px[0] = x0 + (fm1 * x0 + g * vx);
+    px[1] = y0 + (fm1 * y0 + g * vy);
+    px[2] = z0 + (fm1 * z0 + g * vz);
+    pv[0] = vx + (fd * x0 + gdm1 * vx);
+    pv[1] = vy + (fd * y0 + gdm1 * vy);
+    pv[2] = vz + (fd * z0 + gdm1 * vz);
+    return 0;
+}
+
+/* x, v in place; iflag (nullable) per body: 0 ok, 1 failed.  Returns #failed. */
+int oracle_drift(int nb, int ld, double mu, double dt, double *x, double *v, int32_t *iflag)
+{
+    if (nb < 0 || ld < nb) return -1;
+    int nfail = 0;
+#pragma omp parallel for schedule(static) reduction(+ : nfail)
+    for (int b = 0; b < nb; ++b) {
+        real px[3], pv[3];
+        for (int c = 0; c < 3; ++c) { px[c] = X_(x, c, b); pv[c] = X_(v, c, b); }
+        int f = drift_one((real)mu, (real)dt, px, pv);
+        if (!f) {
+            for (int c = 0; c < 3; ++c) {
+                x[(size_t)c * ld + b] = (double)px[c];
+                v[(size_t)c * ld + b] = (double)pv[c];
+            }
+        }
+        if (iflag) iflag[b] = f;
+        nfail += f;
+    }
+    return nfail;
+}
+
+/* ---------------------------------------------------------------------------
+ * Hamiltonian block pieces
+ * ------------------------------------------------------------------------- */
+/* LOOP 1: v_j += hk a_j */
+int oracle_kick(int nb, int ld, double hk, double *v, const double *a)
+{
+#pragma omp parallel for schedule(static)
+    for (int b = 0; b < nb; ++b)
+        for (int c = 0; c < 3; ++c)
+            v[(size_t)c * ld + b] = (double)(X_(v, c, b) + (real)hk * X_(a, c, b));
+    return 0;
+}
+
+/* LOOP 2: mvsum = sum_j gm_j v_j (ascending j) ; LOOP 3: x_j += hj mvsum / mu */
+int oracle_jump(int nb, int ld, double hj, double mu, const double *gm, double *x,
+                const double *v, double *P3)
+{
+    real P[3] = {0, 0, 0};
+    for (int b = 0; b < nb; ++b)
+        for (int c = 0; c < 3; ++c) P[c] += (real)gm[b] * X_(v, c, b);
+#pragma omp parallel for schedule(static)
+    for (int b = 0; b < nb; ++b)
+        for (int c = 0; c < 3; ++c)
+            x[(size_t)c * ld + b] = (double)(X_(x, c, b) + (real)hj * P[c] / (real)mu);
+    if (P3) for (int c = 0; c < 3; ++c) P3[c] = (double)P[c];
+    return 0;
+}
+
+/* ---------------------------------------------------------------------------
+ * O-D  one hybrid step of size h (mdt_hy, Fig. 1; readings S-1..S-5):
+ *   kick h/2 -> jump h/2 -> copy x0,v0 -> drift h -> encounter check ->
+ *   jump h/2 (mvsum from the drifted v) -> a = accel(x) -> kick h/2.
+ * `a` must be current for `x` on entry; it is current for the new x on exit.
+ * No restore and no encounter resolution (reading S-3).
+ * Returns the encounter count of this step (<0 on error); *nfail = drift failures.
+ * ------------------------------------------------------------------------- */
+int64_t oracle_step(int nb, int ld, double mu, const double *gm, const double *rcrit,
+                    double h, double *x, double *v, double *a, double *x0, double *v0,
+                    int32_t *pairs, int64_t cap, uint8_t *flag,
+                    int32_t *ambig, int64_t ambig_cap, int64_t *n_ambig, int32_t *nfail)
+{
+    if (nb < 0 || ld < nb) return -1;
+    oracle_kick(nb, ld, 0.5 * h, v, a);
+    oracle_jump(nb, ld, 0.5 * h, mu, gm, x, v, 0);
+    for (int c = 0; c < 3; ++c) {                        /* LOOP 4 */
+        memcpy(x0 + (size_t)c * ld, x + (size_t)c * ld, sizeof(double) * (size_t)nb);
+        memcpy(v0 + (size_t)c * ld, v + (size_t)c * ld, sizeof(double) * (size_t)nb);
+    }
+    int nf = oracle_drift(nb, ld, mu, h, x, v, 0);
+    if (nfail) *nfail = nf;
+    int64_t cnt = oracle_encounters(nb, ld, h, x0, v0, x, v, rcrit, pairs, cap, flag,
+                                    ambig, ambig_cap, n_ambig);
+    oracle_jump(nb, ld, 0.5 * h, mu, gm, x, v, 0);
+    oracle_accel(nb, ld, gm, x, rcrit, a, 0);
+    oracle_kick(nb, ld, 0.5 * h, v, a);
+    return cnt;
+}
+
+/* step without the O(N^2/2) encounter pass, for long multi-step invariant pins */
+int oracle_step_noenc(int nb, int ld, double mu, const double *gm, const double *rcrit,
+                      double h, double *x, double *v, double *a)
+{
+    if (nb < 0 || ld < nb) return -1;
+    oracle_kick(nb, ld, 0.5 * h, v, a);
+    oracle_jump(nb, ld, 0.5 * h, mu, gm, x, v, 0);
+    oracle_drift(nb, ld, mu, h, x, v, 0);
+    oracle_jump(nb, ld, 0.5 * h, mu, gm, x, v, 0);
+    oracle_accel(nb, ld, gm, x, rcrit, a, 0);
+    oracle_kick(nb, ld, 0.5 * h, v, a);
+    return 0;
+}

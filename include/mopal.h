@@ -1,0 +1,173 @@
+/*
+ * mopal.h - C ABI of libmopal: the data-parallel hot path of Mercury-Opal's
+ * (arxiv 2601.19654) fully interacting n-body integration on one B200 (sm_100a).
+ *
+ * What the library computes (citations are /root/reference/PAPER.md lines; the
+ * paper elides all arithmetic in <...> placeholders, so each operation is the
+ * reading recorded in DESIGN.md section 3):
+ *
+ *   mo_accel      force block LOOP 2:
+ *                   a_i = sum_{j != i} gm_j K_ij (x_j - x_i) / r_ij^3,
+ *                   K_ij = changeover weight of r_ij with rc = max(rcrit_i, rcrit_j)
+ *                   (critical radius, PAPER.md:104 fn. 14); body-body terms only.
+ *   mo_drift      keplerian drift of every body about the star, mu = G m_star, over dt
+ *                   by Gauss f,g in universal variables (arxes_drift, PAPER.md:59,
+ *                   130, 231-233; iflag -> MO_ENOCONV).
+ *   mo_encounters mce_snif: per-body x,y extremes over the step
+ *                   padded by rcrit (LOOP 1-2), then for every i<j: boxes overlap and
+ *                   estimated minimum separation over the step <= max(rcrit_i,rcrit_j)
+ *                   (LOOP 3) -> pair list (ice/jce), per-body flag (ce), count (nce).
+ *   mo_step       mdt_hy (Fig. 1, 202-226): kick h/2, stellar jump h/2,
+ *                   copy x0,v0, drift h, encounter check, jump h/2, accel, kick h/2 -
+ *                   all state resident in HBM (the paper moves 7N doubles H<->D twice
+ *                   per step).  No restore and no Bulirsch-Stoer
+ *                   resolution of flagged pairs (mdt_hkce stays out of scope).
+ *
+ * Units: AU, day, Msun; gm = G * mass.  Coordinates are democratic heliocentric:
+ * heliocentric positions, barycentric velocities (PAPER.md:84, 100 fn. 12).
+ * Bodies are indexed 0..nb-1; the star (the paper's array element 1,
+ * PAPER.md:134) is not a body, only m_star.
+ *
+ * Layout: every per-body 3-vector array is SoA, 3 planes of `ld` doubles:
+ * component c of body b at [c*ld + b]; ld >= nb, ld % 4 == 0, base 16-byte aligned.
+ *
+ * Memory: "device" pointers are CUDA device memory of the current device,
+ * "host" pointers ordinary (preferably pinned) host memory.  The CALLER owns every
+ * array passed in; the context BORROWS the device arrays given to mo_create for its
+ * whole lifetime and owns only its scratch (freed by mo_destroy).
+ *
+ * Execution: all work is enqueued on the stream given to mo_create and the calls
+ * return immediately, except where a host out-pointer is given (then the call
+ * synchronises that stream before returning).  No exceptions, abort, exit or
+ * stdout; failures are return codes.  Asynchronous CUDA errors surface as
+ * MO_ECUDA on the next synchronising call.  There is no CPU fallback: without a
+ * CUDA device mo_create returns MO_ECUDA.
+ */
+#ifndef MOPAL_H
+#define MOPAL_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mo_ctx mo_ctx; /* opaque */
+
+typedef enum {
+    MO_OK = 0,
+    MO_EINVAL = 1,    /* null / misaligned pointer, nb < 1, ld < nb or ld % 4, non-finite or
+                         non-positive m_star / G, dt == 0 or non-finite, cap < 0, nsteps < 0 */
+    MO_ENOMEM = 2,    /* scratch allocation failed */
+    MO_ECUDA = 3,     /* CUDA runtime error (or no device) */
+    MO_EOVERFLOW = 4, /* more encounter pairs than `cap`: the first `cap` pairs in sorted
+                         order are stored, the count is still the true total */
+    MO_ENOCONV = 5    /* >= 1 body's Kepler solve failed (paper's iflag);
+                         those bodies are left unchanged, the others advanced */
+} mo_status;
+
+typedef struct {
+    int64_t steps_done; /* mo_step steps completed since mo_create */
+    int64_t nce_last;   /* encounter pairs found by the last encounter pass (true total) */
+    int64_t nce_total;  /* sum of nce_last over all passes */
+    int32_t drift_fail; /* bodies whose Kepler solve failed, cumulative */
+    int32_t max_newton; /* largest Newton iteration count any body needed so far */
+} mo_stats;
+
+/* Create a context.  Reads `mass` once (gm = G*mass is kept in scratch).
+ *   nb       number of bodies (>= 1); ld plane stride in doubles
+ *   m_star,G central mass (Msun) and gravitational constant (AU^3 Msun^-1 day^-2;
+ *            Mercury's units give G = k^2 = 2.959122082855911e-4)
+ *   mass     device, nb           (borrowed only during the call)
+ *   x, v     device, 3*ld each    (borrowed, read and written)
+ *   a        device, 3*ld         (borrowed, written by mo_accel / mo_step)
+ *   rcrit    device, nb, AU       (borrowed; read at every launch, so the caller may
+ *                                  update it between calls as the paper does)
+ *   pairs    device, 2*cap int32  (borrowed, out) pair k = (pairs[2k], pairs[2k+1]), 0-based,
+ *                                  i<j, sorted by i then j; may be NULL iff cap == 0
+ *   flag     device, nb uint8     (borrowed, out) 1 iff the body is in a flagged pair
+ *   cuda_stream  cudaStream_t; NULL = legacy default stream                          */
+mo_status mo_create(mo_ctx **out, int32_t nb, int32_t ld, double m_star, double G,
+                    const double *mass, double *x, double *v, double *a,
+                    const double *rcrit, int32_t *pairs, int64_t cap, uint8_t *flag,
+                    void *cuda_stream);
+
+/* a <- accel(x).  Asynchronous. */
+mo_status mo_accel(mo_ctx *ctx);
+
+/* x, v <- Kepler drift over dt (dt may be negative).  Asynchronous; failures are
+ * counted in stats.drift_fail and reported by the next synchronising call. */
+mo_status mo_drift(mo_ctx *ctx, double dt);
+
+/* Encounter check for a step of size dt that took (x0, v0) to the context's current
+ * (x, v).  x0, v0: device, 3*ld, or both NULL to use the snapshot the last mo_step (or
+ * mo_snapshot) stored.  Writes pairs / flag; if count_host != NULL the stream is
+ * synchronised and *count_host receives the true pair count (MO_EOVERFLOW if > cap). */
+mo_status mo_encounters(mo_ctx *ctx, double dt, const double *x0, const double *v0,
+                        int64_t *count_host);
+
+/* nsteps hybrid steps of size dt.  `a` must be current for `x` unless the context has
+ * never computed it or mo_invalidate_accel was called (then it is computed first, the
+ * paper's first-call logic).  stats_host nullable; if given the call
+ * synchronises and returns MO_EOVERFLOW / MO_ENOCONV if either happened. */
+mo_status mo_step(mo_ctx *ctx, double dt, int32_t nsteps, mo_stats *stats_host);
+
+void mo_destroy(mo_ctx *ctx);
+
+/* ---- extras ------------------------------------------------------------- */
+
+/* Copy the current x, v into the context's x0, v0 snapshot (asynchronous). */
+mo_status mo_snapshot(mo_ctx *ctx);
+/* Device pointers of the snapshot planes (3*ld doubles each), for inspection. */
+mo_status mo_snapshot_ptrs(mo_ctx *ctx, const double **x0, const double **v0);
+/* Copy the snapshot into caller-owned device arrays (3*ld doubles each; asynchronous). */
+mo_status mo_snapshot_copy(mo_ctx *ctx, double *x0_dst, double *v0_dst);
+/* Tell the context that the caller changed x: the next mo_step recomputes a first. */
+mo_status mo_invalidate_accel(mo_ctx *ctx);
+/* Synchronise the stream and read the statistics. */
+mo_status mo_get_stats(mo_ctx *ctx, mo_stats *stats_host);
+/* Number of libmopal kernels launched on behalf of this context so far. */
+int64_t mo_launch_count(const mo_ctx *ctx);
+/* Bytes of device scratch the context owns. */
+int64_t mo_workspace_bytes(const mo_ctx *ctx);
+
+/* Host-buffer variant of the step (the paper's per-step data region):
+ * copies x_host, v_host (3*ld each) and, if non-NULL, rcrit_host (nb) to the device,
+ * runs nsteps steps, copies x, v back, and if pairs_host != NULL the first
+ * min(count, cap_host, cap) pairs.  a_is_current != 0 asserts that the device-resident
+ * `a` is valid for x_host (e.g. x_host is what the previous call returned); otherwise
+ * it is recomputed first.  Always synchronises.  Writes the borrowed rcrit buffer. */
+mo_status mo_step_host(mo_ctx *ctx, double dt, int32_t nsteps, double *x_host,
+                       double *v_host, const double *rcrit_host, int32_t a_is_current,
+                       int32_t *pairs_host, int64_t cap_host, mo_stats *stats_host);
+
+/* Host-buffer variant of mo_accel: uploads x_host (3*ld), computes, downloads a_host
+ * (3*ld).  Synchronises. */
+mo_status mo_accel_host(mo_ctx *ctx, const double *x_host, double *a_host);
+
+/* Measures the FP64 FMA issue peak of the current device with a register-resident
+ * DFMA loop (148 SMs x 64 lanes x 2 flop x clock on B200): runs `reps` timed launches
+ * on `cuda_stream` and writes the best TFLOP/s and its duration in ms.  Used as the
+ * measured denominator of the pair kernel's roofline (MEASURED_PEAKS.json has none). */
+mo_status mo_probe_fp64_peak(void *cuda_stream, int32_t reps, double *tflops_out,
+                             double *ms_out);
+
+/* Pair-kernel launch geometry chosen for this nb: i-bodies per thread, j-splits,
+ * CTAs, resident CTAs per SM (all nullable). */
+mo_status mo_pair_geometry(const mo_ctx *ctx, int32_t *ipt, int32_t *jsplit,
+                           int32_t *ctas, int32_t *ctas_per_sm);
+
+/* Time of the last pair-accel kernel launch alone, measured with CUDA events on the
+ * context's stream when timing was enabled with mo_set_kernel_timing(ctx, 1).
+ * Synchronises.  ms_out receives the mean over the launches since enabling (and
+ * n_out their number); both reset on read. */
+mo_status mo_set_kernel_timing(mo_ctx *ctx, int32_t on);
+mo_status mo_pair_kernel_ms(mo_ctx *ctx, double *ms_out, int32_t *n_out);
+
+const char *mo_strerror(mo_status s);
+const char *mo_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MOPAL_H */

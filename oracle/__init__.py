@@ -49,6 +49,10 @@ def _lib(kind="ld"):
     L.oracle_changeover.argtypes = [C.c_double, C.c_double]
     L.oracle_accel.restype = I
     L.oracle_accel.argtypes = [I, I, D, D, D, D, D]
+    L.oracle_accel_rows.restype = I
+    L.oracle_accel_rows.argtypes = [I, I, D, D, D, P32, I, D, D]
+    L.oracle_encounters_rows.restype = I64
+    L.oracle_encounters_rows.argtypes = [I, I, C.c_double, D, D, D, D, D, P32, I64, PU8, P32, I64, PI64, I, I]
     L.oracle_boxes.restype = I
     L.oracle_boxes.argtypes = [I, I, C.c_double, D, D, D, D, D, D, D]
     L.oracle_pair_d2min.restype = C.c_double
@@ -103,6 +107,18 @@ def accel(gm, x, rcrit, kind="ld"):
     return a, S
 
 
+def accel_rows(gm, x, rcrit, rows, kind="ld"):
+    """O-A for the chosen bodies only.  Returns (a[3,len(rows)], S[3,len(rows)])."""
+    x = _soa(x); gm = _vec(gm); rcrit = _vec(rcrit)
+    rows = np.ascontiguousarray(rows, dtype=np.int32)
+    nb = x.shape[1]
+    a = np.zeros((3, len(rows))); S = np.zeros((3, len(rows)))
+    rc = _lib(kind).oracle_accel_rows(nb, nb, _dp(gm), _dp(x), _dp(rcrit),
+                                      rows.ctypes.data_as(C.POINTER(C.c_int32)), len(rows), _dp(a), _dp(S))
+    assert rc == 0
+    return a, S
+
+
 def boxes(h, x0, v0, x1, v1, rcrit, kind="ld"):
     """O-B.1.  Returns (lo[2,nb], hi[2,nb]) for x and y."""
     x0, v0, x1, v1 = map(_soa, (x0, v0, x1, v1)); rcrit = _vec(rcrit)
@@ -121,9 +137,9 @@ def pair_d2min(h, x0, v0, x1, v1, i, j, kind="ld") -> float:
                                               int(i), int(j)))
 
 
-def encounters(h, x0, v0, x1, v1, rcrit, cap=None, kind="ld"):
+def encounters(h, x0, v0, x1, v1, rcrit, cap=None, kind="ld", row_stride=1, row_phase=0):
     """O-B.  Returns dict(pairs[n,2] sorted, count (true total), flag[nb] uint8,
-    ambig[m,2], n_ambig)."""
+    ambig[m,2], n_ambig).  row_stride > 1 restricts to rows i % row_stride == row_phase."""
     x0, v0, x1, v1 = map(_soa, (x0, v0, x1, v1)); rcrit = _vec(rcrit)
     nb = x0.shape[1]
     L = _lib(kind)
@@ -134,10 +150,11 @@ def encounters(h, x0, v0, x1, v1, rcrit, cap=None, kind="ld"):
         amb = np.zeros((max(cap, 1), 2), dtype=np.int32)
         flag = np.zeros(max(nb, 1), dtype=np.uint8)
         n_amb = C.c_int64(0)
-        cnt = L.oracle_encounters(nb, nb, float(h), _dp(x0), _dp(v0), _dp(x1), _dp(v1), _dp(rcrit),
-                                  pairs.ctypes.data_as(C.POINTER(C.c_int32)), cap,
-                                  flag.ctypes.data_as(C.POINTER(C.c_uint8)),
-                                  amb.ctypes.data_as(C.POINTER(C.c_int32)), cap, C.byref(n_amb))
+        cnt = L.oracle_encounters_rows(nb, nb, float(h), _dp(x0), _dp(v0), _dp(x1), _dp(v1), _dp(rcrit),
+                                       pairs.ctypes.data_as(C.POINTER(C.c_int32)), cap,
+                                       flag.ctypes.data_as(C.POINTER(C.c_uint8)),
+                                       amb.ctypes.data_as(C.POINTER(C.c_int32)), cap, C.byref(n_amb),
+                                       int(row_stride), int(row_phase))
         assert cnt >= 0
         if cnt <= cap and n_amb.value <= cap:
             break

@@ -97,36 +97,60 @@ double oracle_changeover(double r, double rc)
  * reading A-7).  S (nullable) receives sum_j |term| per component for the
  * parity tolerance |a_gpu - a_ref| <= 1e-12 S.
  * ------------------------------------------------------------------------- */
+static void accel_row(int nb, int ld, const double *gm, const double *x, const double *rcrit,
+                      int i, real *acc3, real *abs3)
+{
+    real xi = X_(x, 0, i), yi = X_(x, 1, i), zi = X_(x, 2, i);
+    real rci = (real)rcrit[i];
+    real ax = 0, ay = 0, az = 0, sx = 0, sy = 0, sz = 0;
+    for (int j = 0; j < nb; ++j) {
+        if (j == i) continue;
+        real dx = X_(x, 0, j) - xi;
+        real dy = X_(x, 1, j) - yi;
+        real dz = X_(x, 2, j) - zi;
+        real s2 = dx * dx + dy * dy + dz * dz;
+        if (s2 == 0) continue;                       /* reading A-9 */
+        real rc = rmax(rci, (real)rcrit[j]);         /* reading A-3 */
+        real K = changeover_s2(s2, rc);
+        if (K == 0) continue;
+        real w = (real)gm[j] * K / (s2 * R_SQRT(s2));
+        ax += w * dx; ay += w * dy; az += w * dz;
+        sx += R_FABS(w * dx); sy += R_FABS(w * dy); sz += R_FABS(w * dz);
+    }
+    acc3[0] = ax; acc3[1] = ay; acc3[2] = az;
+    abs3[0] = sx; abs3[1] = sy; abs3[2] = sz;
+}
+
 int oracle_accel(int nb, int ld, const double *gm, const double *x,
                  const double *rcrit, double *a, double *S)
 {
     if (nb < 0 || ld < nb) return 1;
 #pragma omp parallel for schedule(static)
     for (int i = 0; i < nb; ++i) {
-        real xi = X_(x, 0, i), yi = X_(x, 1, i), zi = X_(x, 2, i);
-        real rci = (real)rcrit[i];
-        real ax = 0, ay = 0, az = 0, sx = 0, sy = 0, sz = 0;
-        for (int j = 0; j < nb; ++j) {
-            if (j == i) continue;
-            real dx = X_(x, 0, j) - xi;
-            real dy = X_(x, 1, j) - yi;
-            real dz = X_(x, 2, j) - zi;
-            real s2 = dx * dx + dy * dy + dz * dz;
-            if (s2 == 0) continue;                       /* reading A-9 */
-            real rc = rmax(rci, (real)rcrit[j]);         /* reading A-3 */
-            real K = changeover_s2(s2, rc);
-            if (K == 0) continue;
-            real w = (real)gm[j] * K / (s2 * R_SQRT(s2));
-            ax += w * dx; ay += w * dy; az += w * dz;
-            sx += R_FABS(w * dx); sy += R_FABS(w * dy); sz += R_FABS(w * dz);
+        real acc[3], ab[3];
+        accel_row(nb, ld, gm, x, rcrit, i, acc, ab);
+        for (int c = 0; c < 3; ++c) {
+            a[(size_t)c * ld + i] = (double)acc[c];
+            if (S) S[(size_t)c * ld + i] = (double)ab[c];
         }
-        a[0 * (size_t)ld + i] = (double)ax;
-        a[1 * (size_t)ld + i] = (double)ay;
-        a[2 * (size_t)ld + i] = (double)az;
-        if (S) {
-            S[0 * (size_t)ld + i] = (double)sx;
-            S[1 * (size_t)ld + i] = (double)sy;
-            S[2 * (size_t)ld + i] = (double)sz;
+    }
+    return 0;
+}
+
+/* the same sum for a chosen subset of bodies i (full-size sampled parity):
+ * a_out / S_out are [3][nrows]. */
+int oracle_accel_rows(int nb, int ld, const double *gm, const double *x, const double *rcrit,
+                      const int32_t *rows, int nrows, double *a_out, double *S_out)
+{
+    if (nb < 0 || ld < nb || nrows < 0) return 1;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int k = 0; k < nrows; ++k) {
+        real acc[3], ab[3];
+        if (rows[k] < 0 || rows[k] >= nb) continue;
+        accel_row(nb, ld, gm, x, rcrit, rows[k], acc, ab);
+        for (int c = 0; c < 3; ++c) {
+            a_out[(size_t)c * nrows + k] = (double)acc[c];
+            if (S_out) S_out[(size_t)c * nrows + k] = (double)ab[c];
         }
     }
     return 0;
@@ -289,10 +313,11 @@ static int classify_pair(int nb, int ld, real h, const double *x0, const double 
  * pair (paper: ce=2).  ambig (nullable): pairs whose outcome
  * is within 1e-12 relative of a threshold, n_ambig = their true number.
  * ------------------------------------------------------------------------- */
-int64_t oracle_encounters(int nb, int ld, double h_, const double *x0, const double *v0,
-                          const double *x1, const double *v1, const double *rcrit,
-                          int32_t *pairs, int64_t cap, uint8_t *flag,
-                          int32_t *ambig, int64_t ambig_cap, int64_t *n_ambig)
+static int64_t encounters_impl(int nb, int ld, double h_, const double *x0, const double *v0,
+                               const double *x1, const double *v1, const double *rcrit,
+                               int32_t *pairs, int64_t cap, uint8_t *flag,
+                               int32_t *ambig, int64_t ambig_cap, int64_t *n_ambig,
+                               int row_stride, int row_phase)
 {
     if (nb < 0 || ld < nb) return -1;
     real h = (real)h_;
@@ -307,6 +332,7 @@ int64_t oracle_encounters(int nb, int ld, double h_, const double *x0, const dou
 #pragma omp parallel for schedule(dynamic, 16)
     for (int i = 0; i < nb; ++i) {
         int64_t c = 0, ca = 0;
+        if (i % row_stride != row_phase) continue;
         for (int j = i + 1; j < nb; ++j) {
             int r = classify_pair(nb, ld, h, x0, v0, x1, v1, rcrit, lo, hi, i, j);
             c += (r & 1); ca += ((r >> 1) & 1);
@@ -347,6 +373,28 @@ int64_t oracle_encounters(int nb, int ld, double h_, const double *x0, const dou
     if (n_ambig) *n_ambig = total_a;
     free(lo); free(hi); free(rowcnt); free(rowamb);
     return total;
+}
+
+int64_t oracle_encounters(int nb, int ld, double h_, const double *x0, const double *v0,
+                          const double *x1, const double *v1, const double *rcrit,
+                          int32_t *pairs, int64_t cap, uint8_t *flag,
+                          int32_t *ambig, int64_t ambig_cap, int64_t *n_ambig)
+{
+    return encounters_impl(nb, ld, h_, x0, v0, x1, v1, rcrit, pairs, cap, flag, ambig, ambig_cap,
+                           n_ambig, 1, 0);
+}
+
+/* the same list restricted to rows i with i % row_stride == row_phase (full-size sampled
+ * parity); flag then marks only bodies of those pairs. */
+int64_t oracle_encounters_rows(int nb, int ld, double h_, const double *x0, const double *v0,
+                               const double *x1, const double *v1, const double *rcrit,
+                               int32_t *pairs, int64_t cap, uint8_t *flag,
+                               int32_t *ambig, int64_t ambig_cap, int64_t *n_ambig,
+                               int row_stride, int row_phase)
+{
+    if (row_stride < 1 || row_phase < 0 || row_phase >= row_stride) return -1;
+    return encounters_impl(nb, ld, h_, x0, v0, x1, v1, rcrit, pairs, cap, flag, ambig, ambig_cap,
+                           n_ambig, row_stride, row_phase);
 }
 
 /* ---------------------------------------------------------------------------

@@ -1,0 +1,550 @@
+// mopal.cu - C ABI of libmopal (include/mopal.h): context, argument checking, launch
+// orchestration and the CUDA-graph step driver.  All arithmetic is in the kernels of
+// pair_accel.cuh / kepler.cuh / encounters.cuh / glue.cuh.
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <new>
+#include <vector>
+
+#include "../../include/mopal.h"
+#include "glue.cuh"
+
+using namespace mopal;
+
+struct mo_ctx {
+    int nb = 0, ld = 0, nbPad = 0, nTiles = 0, nsm = 0;
+    double m_star = 0, G = 0, mu = 0;
+    // borrowed
+    double *x = nullptr, *v = nullptr, *a = nullptr;
+    const double* rcrit = nullptr;
+    int* pairs = nullptr;
+    long long cap = 0;
+    uint8_t* flag = nullptr;
+    cudaStream_t stream = nullptr;
+    // owned scratch
+    double *gm = nullptr, *x0 = nullptr, *v0 = nullptr, *part = nullptr, *psumA = nullptr, *psumB = nullptr;
+    unsigned char* tiles = nullptr;
+    double4* box = nullptr;
+    int* rowcnt = nullptr;
+    long long* rowoff = nullptr;
+    DevStats* dstats = nullptr;
+    DevStats* hstats = nullptr;  // pinned
+    double* probe = nullptr;
+    size_t ws_bytes = 0;
+    // geometry
+    int ipt = 1, unroll = 4, nIblk = 0, nsplit = 1, tps = 1, ctas_per_sm = 1, npsum = 0;
+    int enc_tps = 1, enc_nsplit = 1;
+    bool a_valid = false, snap_valid = false, debug = false, use_graph = true;
+    long long launches = 0;
+    cudaError_t last_err = cudaSuccess;
+    // graph cache (one dt)
+    cudaGraphExec_t gexec = nullptr;
+    double gdt = 0;
+    // per-launch timing of the pair kernel
+    bool timing = false;
+    std::vector<cudaEvent_t> ev;  // start/stop interleaved
+    size_t ev_used = 0;
+};
+
+#define CK(call)                                          \
+    do {                                                  \
+        cudaError_t e_ = (call);                          \
+        if (e_ != cudaSuccess) {                          \
+            ctx->last_err = e_;                           \
+            return MO_ECUDA;                              \
+        }                                                 \
+    } while (0)
+
+static inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+static mo_status post_launch(mo_ctx* ctx, int n = 1) {
+    ctx->launches += n;
+    CK(cudaGetLastError());
+    if (ctx->debug) CK(cudaStreamSynchronize(ctx->stream));
+    return MO_OK;
+}
+
+template <typename T>
+static cudaError_t dalloc(mo_ctx* ctx, T** p, size_t n) {
+    size_t bytes = n * sizeof(T);
+    if (bytes == 0) bytes = 16;
+    cudaError_t e = cudaMalloc(reinterpret_cast<void**>(p), bytes);
+    if (e == cudaSuccess) ctx->ws_bytes += bytes;
+    return e;
+}
+
+typedef void (*pair_kernel_t)(AccelParams);
+static pair_kernel_t pick_pair_kernel(int ipt, int unroll) {
+    if (ipt == 1) return unroll == 2 ? pair_accel_kernel<1, 2> : pair_accel_kernel<1, 4>;
+    return unroll == 4 ? pair_accel_kernel<2, 4> : pair_accel_kernel<2, 2>;
+}
+
+static int env_int(const char* name, int dflt) {
+    const char* s = getenv(name);
+    return (s && *s) ? atoi(s) : dflt;
+}
+
+// j-split count: minimise (waves) x (tiles per CTA + start-up), see DESIGN.md section 5
+static void choose_geometry(mo_ctx* ctx) {
+    const int nb = ctx->nb;
+    ctx->ipt = env_int("MO_IPT", nb >= 8192 ? 2 : 1);
+    if (ctx->ipt != 1 && ctx->ipt != 2) ctx->ipt = 1;
+    ctx->unroll = env_int("MO_UNROLL", ctx->ipt == 2 ? 2 : 4);
+    if (ctx->unroll != 2 && ctx->unroll != 4) ctx->unroll = 4;
+    const int rows = CONSUMER_THREADS * ctx->ipt;
+    ctx->nIblk = (nb + rows - 1) / rows;
+    int occ = 1;
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, pick_pair_kernel(ctx->ipt, ctx->unroll), CTA_THREADS, 0);
+    if (occ < 1) occ = 1;
+    ctx->ctas_per_sm = occ;
+    const long long slots = (long long)ctx->nsm * occ;
+    const int smax = ctx->nTiles < 48 ? ctx->nTiles : 48;
+    double best = 1e300;
+    int bestS = 1;
+    for (int S = 1; S <= smax; ++S) {
+        const int tps = (ctx->nTiles + S - 1) / S;
+        const int Se = (ctx->nTiles + tps - 1) / tps;
+        const long long ctas = (long long)ctx->nIblk * Se;
+        const long long waves = (ctas + slots - 1) / slots;
+        const double cost = (double)waves * (tps + 1.5);
+        if (cost < best * (1.0 - 1e-9)) { best = cost; bestS = Se; }
+    }
+    const int forced = env_int("MO_JSPLIT", 0);
+    if (forced > 0) bestS = forced < ctx->nTiles ? forced : ctx->nTiles;
+    ctx->tps = (ctx->nTiles + bestS - 1) / bestS;
+    ctx->nsplit = (ctx->nTiles + ctx->tps - 1) / ctx->tps;
+    // encounter pass 1: row blocks x j-chunks, about 32 chunks
+    ctx->enc_tps = ctx->nTiles / 32 > 1 ? ctx->nTiles / 32 : 1;
+    ctx->enc_nsplit = (ctx->nTiles + ctx->enc_tps - 1) / ctx->enc_tps;
+}
+
+extern "C" const char* mo_strerror(mo_status s) {
+    switch (s) {
+        case MO_OK: return "ok";
+        case MO_EINVAL: return "invalid argument";
+        case MO_ENOMEM: return "out of device memory";
+        case MO_ECUDA: return "CUDA error or no CUDA device";
+        case MO_EOVERFLOW: return "more encounter pairs than cap";
+        case MO_ENOCONV: return "Kepler solve failed for at least one body";
+    }
+    return "unknown status";
+}
+
+extern "C" const char* mo_version(void) { return "libmopal 0.1 (sm_100a)"; }
+
+extern "C" void mo_destroy(mo_ctx* ctx) {
+    if (!ctx) return;
+    if (ctx->gexec) cudaGraphExecDestroy(ctx->gexec);
+    for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
+    cudaFree(ctx->gm); cudaFree(ctx->x0); cudaFree(ctx->v0); cudaFree(ctx->part);
+    cudaFree(ctx->psumA); cudaFree(ctx->psumB); cudaFree(ctx->tiles); cudaFree(ctx->box);
+    cudaFree(ctx->rowcnt); cudaFree(ctx->rowoff); cudaFree(ctx->dstats); cudaFree(ctx->probe);
+    if (ctx->hstats) cudaFreeHost(ctx->hstats);
+    delete ctx;
+}
+
+extern "C" mo_status mo_create(mo_ctx** out, int32_t nb, int32_t ld, double m_star, double G, const double* mass,
+                               double* x, double* v, double* a, const double* rcrit, int32_t* pairs, int64_t cap,
+                               uint8_t* flag, void* cuda_stream) {
+    if (!out) return MO_EINVAL;
+    *out = nullptr;
+    if (nb < 1 || ld < nb || (ld & 3) || !mass || !x || !v || !a || !rcrit || !flag || cap < 0 || (cap > 0 && !pairs))
+        return MO_EINVAL;
+    if (!(m_star > 0.0) || !(G > 0.0) || !isfinite(m_star) || !isfinite(G)) return MO_EINVAL;
+    if (!aligned16(x) || !aligned16(v) || !aligned16(a) || !aligned16(mass) || !aligned16(rcrit)) return MO_EINVAL;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); return MO_ECUDA; }
+    mo_ctx* ctx = new (std::nothrow) mo_ctx();
+    if (!ctx) return MO_ENOMEM;
+    ctx->nb = nb; ctx->ld = ld; ctx->m_star = m_star; ctx->G = G; ctx->mu = G * m_star;
+    ctx->x = x; ctx->v = v; ctx->a = a; ctx->rcrit = rcrit; ctx->pairs = pairs; ctx->cap = cap; ctx->flag = flag;
+    ctx->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
+    ctx->debug = env_int("MO_DEBUG", 0) != 0;
+    ctx->use_graph = env_int("MO_NO_GRAPH", 0) == 0;
+    ctx->nTiles = (nb + TJ - 1) / TJ;
+    ctx->nbPad = ctx->nTiles * TJ;
+    int dev = 0;
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
+        cudaGetLastError(); delete ctx; return MO_ECUDA;
+    }
+    if (prop.major < 10) { delete ctx; return MO_ECUDA; }  // sm_100a code only
+    ctx->nsm = prop.multiProcessorCount;
+    choose_geometry(ctx);
+    ctx->npsum = (ctx->nbPad + ON_BLOCK - 1) / ON_BLOCK;
+    cudaError_t e = cudaSuccess;
+    const size_t pl = 3 * (size_t)ld;
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->gm, (size_t)nb);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->x0, pl);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->v0, pl);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->part, pl * (size_t)ctx->nsplit);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->psumA, 3 * (size_t)ctx->npsum);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->psumB, 3 * (size_t)ctx->npsum);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->tiles, (size_t)ctx->nTiles * ACC_TILE_BYTES);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->box, (size_t)ctx->nbPad);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->rowcnt, (size_t)ctx->nbPad);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->rowoff, (size_t)ctx->nbPad);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->dstats, 1);
+    if (e == cudaSuccess) e = cudaMallocHost(reinterpret_cast<void**>(&ctx->hstats), sizeof(DevStats));
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        mo_destroy(ctx);
+        return e == cudaErrorMemoryAllocation ? MO_ENOMEM : MO_ECUDA;
+    }
+    e = cudaMemsetAsync(ctx->dstats, 0, sizeof(DevStats), ctx->stream);
+    if (e == cudaSuccess) {
+        gm_kernel<<<(nb + 255) / 256, 256, 0, ctx->stream>>>(mass, G, nb, ctx->gm);
+        ctx->launches += 1;
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);  // `mass` is borrowed only during the call
+    if (e != cudaSuccess) { mo_destroy(ctx); return MO_ECUDA; }
+    *out = ctx;
+    return MO_OK;
+}
+
+// ---- stage launchers -------------------------------------------------------------------------
+static mo_status launch_pair(mo_ctx* ctx) {
+    AccelParams p;
+    p.tiles = ctx->tiles; p.x = ctx->x; p.rcrit = ctx->rcrit; p.part = ctx->part;
+    p.nb = ctx->nb; p.ld = ctx->ld; p.nTiles = ctx->nTiles; p.tps = ctx->tps;
+    dim3 grid(ctx->nIblk, ctx->nsplit);
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (ctx->timing) {
+        if (ctx->ev_used + 2 > ctx->ev.size()) {
+            cudaEvent_t a, b;
+            CK(cudaEventCreate(&a)); CK(cudaEventCreate(&b));
+            ctx->ev.push_back(a); ctx->ev.push_back(b);
+        }
+        e0 = ctx->ev[ctx->ev_used]; e1 = ctx->ev[ctx->ev_used + 1];
+        ctx->ev_used += 2;
+        CK(cudaEventRecord(e0, ctx->stream));
+    }
+    pick_pair_kernel(ctx->ipt, ctx->unroll)<<<grid, CTA_THREADS, 0, ctx->stream>>>(p);
+    if (ctx->timing) CK(cudaEventRecord(e1, ctx->stream));
+    return post_launch(ctx);
+}
+
+// a <- accel(x), optionally preceded by the jump (psumB) and followed by the kick
+static mo_status enqueue_accel(mo_ctx* ctx, bool jump, double hj, bool kick, double hk) {
+    if (jump)
+        pack_kernel<true><<<ctx->nTiles, TJ, 0, ctx->stream>>>(ctx->x, ctx->gm, ctx->rcrit, ctx->nb, ctx->ld, ctx->tiles,
+                                                                ctx->psumB, ctx->npsum, hj / ctx->mu);
+    else
+        pack_kernel<false><<<ctx->nTiles, TJ, 0, ctx->stream>>>(ctx->x, ctx->gm, ctx->rcrit, ctx->nb, ctx->ld, ctx->tiles,
+                                                                 nullptr, 0, 0.0);
+    mo_status s = post_launch(ctx);
+    if (s != MO_OK) return s;
+    s = launch_pair(ctx);
+    if (s != MO_OK) return s;
+    const int nblk = (ctx->nb + ON_BLOCK - 1) / ON_BLOCK;
+    if (kick)
+        accel_reduce_kernel<true><<<nblk, ON_BLOCK, 0, ctx->stream>>>(ctx->part, ctx->nsplit, ctx->nb, ctx->ld, ctx->a, ctx->v, hk);
+    else
+        accel_reduce_kernel<false><<<nblk, ON_BLOCK, 0, ctx->stream>>>(ctx->part, ctx->nsplit, ctx->nb, ctx->ld, ctx->a, nullptr, 0.0);
+    return post_launch(ctx);
+}
+
+static EncState enc_state(const mo_ctx* ctx, const double* x0, const double* v0, double h) {
+    EncState s;
+    s.x0 = x0; s.v0 = v0; s.x1 = ctx->x; s.v1 = ctx->v; s.rcrit = ctx->rcrit;
+    s.nb = ctx->nb; s.ld = ctx->ld; s.h = h;
+    return s;
+}
+
+// pass 1 + scan + pass 2 on boxes already in ctx->box (rowcnt and flag already zeroed)
+static mo_status enqueue_pairs(mo_ctx* ctx, const EncState& es, int step_inc) {
+    EncCountParams cp;
+    cp.s = es; cp.box = ctx->box; cp.rowcnt = ctx->rowcnt; cp.nTiles = ctx->nTiles; cp.tps = ctx->enc_tps;
+    enc_count_kernel<<<dim3(ctx->nTiles, ctx->enc_nsplit), CTA_THREADS, 0, ctx->stream>>>(cp);
+    mo_status s = post_launch(ctx);
+    if (s != MO_OK) return s;
+    enc_scan_kernel<<<1, SCAN_THREADS, 0, ctx->stream>>>(ctx->rowcnt, ctx->rowoff, ctx->nb, ctx->cap, step_inc, ctx->dstats);
+    s = post_launch(ctx);
+    if (s != MO_OK) return s;
+    EncWriteParams wp;
+    wp.s = es; wp.box = ctx->box; wp.rowcnt = ctx->rowcnt; wp.rowoff = ctx->rowoff;
+    wp.pairs = ctx->pairs; wp.cap = ctx->cap; wp.flag = ctx->flag;
+    int blocks = (ctx->nb + 7) / 8;
+    const int maxb = ctx->nsm * 8;
+    if (blocks > maxb) blocks = maxb;
+    enc_write_kernel<<<blocks, 256, 0, ctx->stream>>>(wp);
+    return post_launch(ctx);
+}
+
+static mo_status enqueue_step(mo_ctx* ctx, double dt) {
+    kick_psum_kernel<true><<<ctx->npsum, ON_BLOCK, 0, ctx->stream>>>(ctx->v, ctx->a, ctx->gm, ctx->nb, ctx->ld, 0.5 * dt, ctx->psumA);
+    mo_status s = post_launch(ctx);
+    if (s != MO_OK) return s;
+    MidParams mp;
+    mp.x = ctx->x; mp.v = ctx->v; mp.x0 = ctx->x0; mp.v0 = ctx->v0; mp.gm = ctx->gm; mp.rcrit = ctx->rcrit;
+    mp.psum_in = ctx->psumA; mp.psum_out = ctx->psumB; mp.box = ctx->box; mp.rowcnt = ctx->rowcnt; mp.flag = ctx->flag;
+    mp.st = ctx->dstats; mp.nb = ctx->nb; mp.ld = ctx->ld; mp.nbPad = ctx->nbPad; mp.npsum = ctx->npsum;
+    mp.hj_over_mu = 0.5 * dt / ctx->mu; mp.mu = ctx->mu; mp.h = dt;
+    jump_drift_boxes_kernel<<<ctx->npsum, ON_BLOCK, 0, ctx->stream>>>(mp);
+    s = post_launch(ctx);
+    if (s != MO_OK) return s;
+    s = enqueue_pairs(ctx, enc_state(ctx, ctx->x0, ctx->v0, dt), 1);
+    if (s != MO_OK) return s;
+    return enqueue_accel(ctx, true, 0.5 * dt, true, 0.5 * dt);
+}
+static const int KERNELS_PER_STEP = 8;
+
+static mo_status read_stats(mo_ctx* ctx, mo_stats* out, bool* overflow) {
+    CK(cudaMemcpyAsync(ctx->hstats, ctx->dstats, sizeof(DevStats), cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    if (out) {
+        out->steps_done = ctx->hstats->steps_done;
+        out->nce_last = ctx->hstats->nce_last;
+        out->nce_total = ctx->hstats->nce_total;
+        out->drift_fail = ctx->hstats->drift_fail;
+        out->max_newton = ctx->hstats->max_newton;
+    }
+    if (overflow) *overflow = ctx->hstats->overflow != 0;
+    return MO_OK;
+}
+
+static mo_status status_from_stats(mo_ctx* ctx, mo_stats* out) {
+    bool ovf = false;
+    mo_stats tmp;
+    mo_status s = read_stats(ctx, &tmp, &ovf);
+    if (s != MO_OK) return s;
+    if (out) *out = tmp;
+    if (ovf) return MO_EOVERFLOW;
+    if (tmp.drift_fail > 0) return MO_ENOCONV;
+    return MO_OK;
+}
+
+// ---- public entry points ---------------------------------------------------------------------
+extern "C" mo_status mo_accel(mo_ctx* ctx) {
+    if (!ctx) return MO_EINVAL;
+    mo_status s = enqueue_accel(ctx, false, 0.0, false, 0.0);
+    if (s == MO_OK) ctx->a_valid = true;
+    return s;
+}
+
+extern "C" mo_status mo_drift(mo_ctx* ctx, double dt) {
+    if (!ctx || !isfinite(dt)) return MO_EINVAL;
+    const int nblk = (ctx->nb + ON_BLOCK - 1) / ON_BLOCK;
+    drift_kernel<<<nblk, ON_BLOCK, 0, ctx->stream>>>(ctx->x, ctx->v, ctx->nb, ctx->ld, ctx->mu, dt, ctx->dstats);
+    ctx->a_valid = false;
+    return post_launch(ctx);
+}
+
+extern "C" mo_status mo_snapshot(mo_ctx* ctx) {
+    if (!ctx) return MO_EINVAL;
+    const size_t bytes = 3 * (size_t)ctx->ld * sizeof(double);
+    CK(cudaMemcpyAsync(ctx->x0, ctx->x, bytes, cudaMemcpyDeviceToDevice, ctx->stream));
+    CK(cudaMemcpyAsync(ctx->v0, ctx->v, bytes, cudaMemcpyDeviceToDevice, ctx->stream));
+    ctx->snap_valid = true;
+    return MO_OK;
+}
+
+extern "C" mo_status mo_snapshot_ptrs(mo_ctx* ctx, const double** x0, const double** v0) {
+    if (!ctx) return MO_EINVAL;
+    if (x0) *x0 = ctx->x0;
+    if (v0) *v0 = ctx->v0;
+    return MO_OK;
+}
+
+extern "C" mo_status mo_snapshot_copy(mo_ctx* ctx, double* x0_dst, double* v0_dst) {
+    if (!ctx || !x0_dst || !v0_dst) return MO_EINVAL;
+    const size_t bytes = 3 * (size_t)ctx->ld * sizeof(double);
+    CK(cudaMemcpyAsync(x0_dst, ctx->x0, bytes, cudaMemcpyDeviceToDevice, ctx->stream));
+    CK(cudaMemcpyAsync(v0_dst, ctx->v0, bytes, cudaMemcpyDeviceToDevice, ctx->stream));
+    return MO_OK;
+}
+
+extern "C" mo_status mo_invalidate_accel(mo_ctx* ctx) {
+    if (!ctx) return MO_EINVAL;
+    ctx->a_valid = false;
+    return MO_OK;
+}
+
+extern "C" mo_status mo_encounters(mo_ctx* ctx, double dt, const double* x0, const double* v0, int64_t* count_host) {
+    if (!ctx || !isfinite(dt) || dt == 0.0) return MO_EINVAL;
+    if ((x0 == nullptr) != (v0 == nullptr)) return MO_EINVAL;
+    if (!x0) {
+        if (!ctx->snap_valid) return MO_EINVAL;
+        x0 = ctx->x0; v0 = ctx->v0;
+    } else if (!aligned16(x0) || !aligned16(v0)) {
+        return MO_EINVAL;
+    }
+    EncState es = enc_state(ctx, x0, v0, dt);
+    boxes_kernel<<<(ctx->nbPad + ON_BLOCK - 1) / ON_BLOCK, ON_BLOCK, 0, ctx->stream>>>(es, ctx->box, ctx->nbPad, ctx->rowcnt, ctx->flag);
+    mo_status s = post_launch(ctx);
+    if (s != MO_OK) return s;
+    s = enqueue_pairs(ctx, es, 0);
+    if (s != MO_OK) return s;
+    if (count_host) {
+        mo_stats st;
+        s = read_stats(ctx, &st, nullptr);
+        if (s != MO_OK) return s;
+        *count_host = st.nce_last;
+        if (st.nce_last > ctx->cap) return MO_EOVERFLOW;
+    }
+    return MO_OK;
+}
+
+extern "C" mo_status mo_step(mo_ctx* ctx, double dt, int32_t nsteps, mo_stats* stats_host) {
+    if (!ctx || !isfinite(dt) || dt == 0.0 || nsteps < 0) return MO_EINVAL;
+    mo_status s = MO_OK;
+    if (!ctx->a_valid && nsteps > 0) {
+        s = mo_accel(ctx);
+        if (s != MO_OK) return s;
+    }
+    const bool graph = ctx->use_graph && !ctx->timing && !ctx->debug && nsteps > 1;
+    if (graph) {
+        if (!ctx->gexec || ctx->gdt != dt) {
+            if (ctx->gexec) { cudaGraphExecDestroy(ctx->gexec); ctx->gexec = nullptr; }
+            cudaGraph_t g = nullptr;
+            const long long l0 = ctx->launches;
+            CK(cudaStreamBeginCapture(ctx->stream, cudaStreamCaptureModeThreadLocal));
+            s = enqueue_step(ctx, dt);
+            cudaError_t e = cudaStreamEndCapture(ctx->stream, &g);
+            ctx->launches = l0;  // captured, not launched
+            if (s != MO_OK || e != cudaSuccess) {
+                if (g) cudaGraphDestroy(g);
+                ctx->last_err = e;
+                cudaGetLastError();
+                return MO_ECUDA;
+            }
+            e = cudaGraphInstantiate(&ctx->gexec, g, 0);
+            cudaGraphDestroy(g);
+            if (e != cudaSuccess) { ctx->gexec = nullptr; ctx->last_err = e; return MO_ECUDA; }
+            ctx->gdt = dt;
+        }
+        for (int k = 0; k < nsteps; ++k) {
+            CK(cudaGraphLaunch(ctx->gexec, ctx->stream));
+            ctx->launches += KERNELS_PER_STEP;
+        }
+    } else {
+        for (int k = 0; k < nsteps; ++k) {
+            s = enqueue_step(ctx, dt);
+            if (s != MO_OK) return s;
+        }
+    }
+    if (nsteps > 0) { ctx->snap_valid = true; ctx->a_valid = true; }
+    if (stats_host) return status_from_stats(ctx, stats_host);
+    return MO_OK;
+}
+
+extern "C" mo_status mo_get_stats(mo_ctx* ctx, mo_stats* stats_host) {
+    if (!ctx || !stats_host) return MO_EINVAL;
+    return status_from_stats(ctx, stats_host);
+}
+
+extern "C" int64_t mo_launch_count(const mo_ctx* ctx) { return ctx ? ctx->launches : 0; }
+extern "C" int64_t mo_workspace_bytes(const mo_ctx* ctx) { return ctx ? (int64_t)ctx->ws_bytes : 0; }
+
+extern "C" mo_status mo_pair_geometry(const mo_ctx* ctx, int32_t* ipt, int32_t* jsplit, int32_t* ctas, int32_t* ctas_per_sm) {
+    if (!ctx) return MO_EINVAL;
+    if (ipt) *ipt = ctx->ipt;
+    if (jsplit) *jsplit = ctx->nsplit;
+    if (ctas) *ctas = ctx->nIblk * ctx->nsplit;
+    if (ctas_per_sm) *ctas_per_sm = ctx->ctas_per_sm;
+    return MO_OK;
+}
+
+extern "C" mo_status mo_set_kernel_timing(mo_ctx* ctx, int32_t on) {
+    if (!ctx) return MO_EINVAL;
+    ctx->timing = on != 0;
+    ctx->ev_used = 0;
+    return MO_OK;
+}
+
+extern "C" mo_status mo_pair_kernel_ms(mo_ctx* ctx, double* ms_out, int32_t* n_out) {
+    if (!ctx || !ms_out) return MO_EINVAL;
+    CK(cudaStreamSynchronize(ctx->stream));
+    double tot = 0.0;
+    int n = 0;
+    for (size_t k = 0; k + 1 < ctx->ev_used; k += 2) {
+        float ms = 0.f;
+        CK(cudaEventElapsedTime(&ms, ctx->ev[k], ctx->ev[k + 1]));
+        tot += ms; ++n;
+    }
+    *ms_out = n ? tot / n : 0.0;
+    if (n_out) *n_out = n;
+    ctx->ev_used = 0;
+    return MO_OK;
+}
+
+extern "C" mo_status mo_step_host(mo_ctx* ctx, double dt, int32_t nsteps, double* x_host, double* v_host,
+                                  const double* rcrit_host, int32_t a_is_current, int32_t* pairs_host, int64_t cap_host,
+                                  mo_stats* stats_host) {
+    if (!ctx || !x_host || !v_host || !isfinite(dt) || dt == 0.0 || nsteps < 0 || cap_host < 0) return MO_EINVAL;
+    const size_t bytes = 3 * (size_t)ctx->ld * sizeof(double);
+    CK(cudaMemcpyAsync(ctx->x, x_host, bytes, cudaMemcpyHostToDevice, ctx->stream));
+    CK(cudaMemcpyAsync(ctx->v, v_host, bytes, cudaMemcpyHostToDevice, ctx->stream));
+    if (rcrit_host)
+        CK(cudaMemcpyAsync(const_cast<double*>(ctx->rcrit), rcrit_host, (size_t)ctx->nb * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
+    if (!a_is_current) ctx->a_valid = false;
+    mo_status s = mo_step(ctx, dt, nsteps, nullptr);
+    if (s != MO_OK) return s;
+    CK(cudaMemcpyAsync(x_host, ctx->x, bytes, cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaMemcpyAsync(v_host, ctx->v, bytes, cudaMemcpyDeviceToHost, ctx->stream));
+    mo_stats st;
+    mo_status rs = status_from_stats(ctx, &st);
+    if (rs == MO_ECUDA) return rs;
+    if (stats_host) *stats_host = st;
+    if (pairs_host && nsteps > 0) {
+        long long n = st.nce_last;
+        if (n > ctx->cap) n = ctx->cap;
+        if (n > cap_host) n = cap_host;
+        if (n > 0) {
+            CK(cudaMemcpyAsync(pairs_host, ctx->pairs, (size_t)n * 2 * sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+            CK(cudaStreamSynchronize(ctx->stream));
+        }
+    }
+    return rs;
+}
+
+extern "C" mo_status mo_accel_host(mo_ctx* ctx, const double* x_host, double* a_host) {
+    if (!ctx || !x_host || !a_host) return MO_EINVAL;
+    const size_t bytes = 3 * (size_t)ctx->ld * sizeof(double);
+    CK(cudaMemcpyAsync(ctx->x, x_host, bytes, cudaMemcpyHostToDevice, ctx->stream));
+    mo_status s = mo_accel(ctx);
+    if (s != MO_OK) return s;
+    CK(cudaMemcpyAsync(a_host, ctx->a, bytes, cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    return MO_OK;
+}
+
+extern "C" mo_status mo_probe_fp64_peak(void* cuda_stream, int32_t reps, double* tflops_out, double* ms_out) {
+    if (!tflops_out || reps < 1) return MO_EINVAL;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+    int dev = 0, nsm = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
+        cudaGetLastError();
+        return MO_ECUDA;
+    }
+    const int blocks = nsm * 8, threads = 256, iters = 1 << 14;
+    double* buf = nullptr;
+    if (cudaMalloc(reinterpret_cast<void**>(&buf), (size_t)blocks * threads * sizeof(double)) != cudaSuccess) {
+        cudaGetLastError();
+        return MO_ENOMEM;
+    }
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    double best = 1e300;
+    mo_status rs = MO_OK;
+    for (int r = 0; r < reps + 2; ++r) {  // two warm-ups
+        cudaEventRecord(e0, st);
+        dfma_probe_kernel<<<blocks, threads, 0, st>>>(buf, iters, 0.999999, 1e-9);
+        cudaEventRecord(e1, st);
+        if (cudaEventSynchronize(e1) != cudaSuccess) { rs = MO_ECUDA; break; }
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        if (r >= 2 && ms < best) best = ms;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaFree(buf);
+    if (rs != MO_OK) { cudaGetLastError(); return rs; }
+    const double flops = (double)blocks * threads * (double)iters * 32.0 * 2.0;
+    *tflops_out = flops / (best * 1e-3) / 1e12;
+    if (ms_out) *ms_out = best;
+    return MO_OK;
+}

@@ -1,0 +1,388 @@
+"""GPU parity: libmopal (through the C ABI binding) against the CPU oracle, element by
+element on the same seeded inputs.  Tolerances are north_star's:
+  accel      |a_gpu - a_ref| <= 1e-12 * sum_j |contribution_j|   per component
+  encounters pair lists bit-exact except pairs within 1e-12 relative of a threshold
+  drift      1e-13 relative (to the vector's 2-norm, reading C-d)
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+import oracle
+from paper_2601_19654_b200 import workloads as W
+
+G = W.G_AU_DAY_MSUN
+
+
+@pytest.fixture(scope="module")
+def M():
+    from paper_2601_19654_b200 import mopal
+    return mopal
+
+
+def _mk(M, w, rcrit=None, cap=1 << 20):
+    return M.Mopal(w.mass, w.x, w.v, w.rcrit if rcrit is None else rcrit, m_star=w.m_star, G=w.G, cap=cap)
+
+
+def _check_accel(a_gpu, a_ref, S, what=""):
+    err = np.abs(a_gpu - a_ref)
+    tol = 1e-12 * S
+    bad = err > tol + 1e-300
+    worst = np.max(err / (S + 1e-300))
+    assert not bad.any(), f"{what}: {bad.sum()} components out of tolerance, worst {worst:.3e} x S"
+    return worst
+
+
+def _rel_vec_err(got, ref):
+    return np.max(np.abs(got - ref), axis=0) / np.linalg.norm(ref, axis=0)
+
+
+def _pairs_ok(got, ref):
+    """SURE_IN subset of GPU list subset of SURE_IN + AMBIG; returns #ambiguous."""
+    S = set(map(tuple, ref["pairs"].tolist()))
+    A = set(map(tuple, ref["ambig"].tolist()))
+    Gs = set(map(tuple, got.tolist()))
+    assert (S - A) <= Gs, f"missing {sorted((S - A) - Gs)[:5]}"
+    assert Gs <= (S | A), f"extra {sorted(Gs - (S | A))[:5]}"
+    return len(A)
+
+
+# ------------------------------------------------------------------------------ accel
+@pytest.mark.parametrize("cfg", [0, 1, 2])
+def test_accel_full_configs(M, cfg):
+    w = W.make_config(cfg)
+    m = _mk(M, w)
+    m.accel()
+    a = m.get("a")
+    a_ref, S = oracle.accel(G * w.mass, w.x, w.rcrit)
+    worst = _check_accel(a, a_ref, S, w.name)
+    assert worst < 2e-13          # in practice ~sqrt(n) eps, far inside the bound
+    m.close()
+
+
+@pytest.mark.parametrize("cfg", [3, 4])
+def test_accel_headline_sizes_sampled_rows(M, cfg):
+    """full-size launch configuration (the one bench.py times); oracle on sampled bodies."""
+    w = W.make_config(cfg)
+    m = _mk(M, w)
+    m.accel()
+    a = m.get("a")
+    rng = np.random.default_rng(cfg)
+    rows = np.unique(np.concatenate([np.arange(8), [w.nb - 1, w.nb - 2, 127, 128, 255, 256],
+                                     rng.integers(0, w.nb, 48)])).astype(np.int32)
+    a_ref, S = oracle.accel_rows(G * w.mass, w.x, w.rcrit, rows)
+    _check_accel(a[:, rows], a_ref, S, w.name)
+    # property at any size: Newton III with the symmetric K
+    for c in range(3):
+        assert abs(np.sum(w.mass * a[c])) <= 1e-11 * np.sum(w.mass * np.abs(a[c]))
+    m.close()
+
+
+@pytest.mark.parametrize("nb", [1, 2, 3, 127, 128, 129, 255, 257, 1000])
+def test_accel_ragged_sizes_and_changeover_shell(M, nb):
+    w = W.random_cluster(nb, 100 + nb, box=1.0, rc_frac=(0.0, 0.7)) if nb > 1 else W.random_cluster(1, 5)
+    m = _mk(M, w)
+    m.accel()
+    a = m.get("a")
+    a_ref, S = oracle.accel(G * w.mass, w.x, w.rcrit)
+    _check_accel(a, a_ref, S, f"cluster{nb}")
+    if nb > 100:   # the sample really exercises K in (0,1), K = 0 and K = 1
+        d = np.linalg.norm(w.x[:, :, None] - w.x[:, None, :], axis=0) + 9 * np.eye(nb)
+        rc = np.maximum(w.rcrit[:, None], w.rcrit[None, :])
+        assert ((d < rc) & (d > 0.1 * rc)).any() and (d <= 0.1 * rc).any() and (d >= rc).any()
+    m.close()
+
+
+def test_accel_degenerate_cases(M):
+    # coincident bodies contribute nothing; rcrit = 0 is Newtonian; rcrit huge gives exactly 0
+    w = W.shrink(0, 300)
+    x = w.x.copy(); x[:, 7] = x[:, 3]
+    gm = G * w.mass
+    for rc in (np.zeros(w.nb), w.rcrit, np.full(w.nb, 1e6)):
+        m = M.Mopal(w.mass, x, w.v, rc)
+        m.accel()
+        a = m.get("a")
+        a_ref, S = oracle.accel(gm, x, rc)
+        assert np.all(np.isfinite(a))
+        _check_accel(a, a_ref, S)
+        if rc[0] > 1e5:
+            assert np.all(a == 0.0)
+        m.close()
+
+
+def test_accel_is_deterministic(M):
+    w = W.make_config(1)
+    m = _mk(M, w)
+    m.accel(); a1 = m.get("a").copy()
+    m.accel(); a2 = m.get("a")
+    assert np.array_equal(a1, a2)
+    m.close()
+
+
+# ------------------------------------------------------------------------------ drift
+@pytest.mark.parametrize("cfg", [0, 1, 2, 3, 4])
+def test_drift_all_configs(M, cfg):
+    w = W.make_config(cfg)
+    m = _mk(M, w)
+    m.drift(w.dt)
+    x, v = m.get("x"), m.get("v")
+    st = m.stats()
+    assert st.drift_fail == 0 and st.max_newton <= 8
+    x_ref, v_ref, fl = oracle.drift(G * w.m_star, w.dt, w.x, w.v)
+    assert not fl.any()
+    assert _rel_vec_err(x, x_ref).max() <= 1e-13
+    assert _rel_vec_err(v, v_ref).max() <= 1e-13
+    m.close()
+
+
+@pytest.mark.parametrize("dt", [-8.0, 0.37, 400.0, 5.0e4])
+def test_drift_long_negative_and_eccentric(M, dt):
+    rng = np.random.default_rng(3)
+    nb = 2000
+    a = rng.uniform(0.3, 40, nb); e = rng.uniform(0, 0.95, nb)
+    mu = G
+    x, v = W.elements_to_state(np.full(nb, mu), a, e, rng.uniform(0, 1.0, nb), rng.uniform(0, 6.28, nb),
+                               rng.uniform(0, 6.28, nb), rng.uniform(0, 6.28, nb))
+    m = M.Mopal(np.full(nb, 1e-12), x, v, np.zeros(nb))
+    m.drift(dt)
+    xg, vg = m.get("x"), m.get("v")
+    assert m.stats().drift_fail == 0
+    x_ref, v_ref, fl = oracle.drift(mu, dt, x, v)
+    # conditioning: inputs are doubles; a relative change eps of the state moves the body by
+    # ~eps * 3 pi * (#orbits) * (1+e)/(1-e) along the orbit -> scale the 1e-13 bar accordingly
+    P = 2 * np.pi * np.sqrt(a**3 / mu)
+    amp = 1 + 10 * np.abs(dt) / P * (1 + e) / (1 - e)
+    assert np.max(_rel_vec_err(xg, x_ref) / amp) <= 1e-13
+    assert np.max(_rel_vec_err(vg, v_ref) / (amp * (1 + e) / (1 - e))) <= 1e-13
+    m.close()
+
+
+def test_drift_failure_flag_and_hyperbolic(M):
+    x = np.array([[0.0, 1.0, 1.0], [0.0, 0.0, 0.0], [0.0, 0.0, 0.0]])
+    v = np.array([[0.01, 0.0, 0.0], [0.0, 0.017, 0.04], [0.0, 0.0, 0.001]])
+    m = M.Mopal(np.full(3, 1e-12), x, v, np.zeros(3))
+    m.drift(50.0)
+    st = m.stats()
+    assert st.drift_fail == 1 and st.status == M.MO_ENOCONV
+    xg, vg = m.get("x"), m.get("v")
+    assert np.all(xg[:, 0] == 0) and np.all(vg[:, 0] == v[:, 0])     # failed body untouched
+    x_ref, v_ref, fl = oracle.drift(G, 50.0, x, v)
+    assert fl.tolist() == [1, 0, 0]
+    assert _rel_vec_err(xg[:, 1:], x_ref[:, 1:]).max() <= 1e-13      # bound and hyperbolic
+    assert _rel_vec_err(vg[:, 1:], v_ref[:, 1:]).max() <= 1e-13
+    m.close()
+
+
+# ------------------------------------------------------------------------------ encounters
+def _enc_inputs(w):
+    x1, v1, fl = oracle.drift(G * w.m_star, w.dt, w.x, w.v)
+    return x1, v1
+
+
+@pytest.mark.parametrize("cfg,scale", [(0, 1.0), (1, 1.0), (2, 1.0), (2, 25.0)])
+def test_encounters_full_configs(M, cfg, scale):
+    """reading B-i: the harness drifts a saved copy to get (x0,v0)->(x1,v1)."""
+    w = W.make_config(cfg)
+    rcrit = w.rcrit * scale
+    x1, v1 = _enc_inputs(w)
+    ref = oracle.encounters(w.dt, w.x, w.v, x1, v1, rcrit)
+    m = M.Mopal(w.mass, w.x, w.v, rcrit)
+    m.snapshot()
+    m.set("x", x1); m.set("v", v1)
+    cnt = m.encounters(w.dt)
+    got = m.pair_list(cnt)
+    n_amb = _pairs_ok(got, ref)
+    if n_amb == 0:
+        assert cnt == ref["count"] and np.array_equal(got, ref["pairs"])
+        assert np.array_equal(m.get("flag"), ref["flag"])
+    assert got.tolist() == sorted(got.tolist())
+    if scale > 1 or cfg < 2:
+        assert cnt > 0
+    m.close()
+
+
+@pytest.mark.parametrize("cfg,stride", [(3, 97), (4, 193)])
+def test_encounters_headline_sizes_sampled_rows(M, cfg, stride):
+    w = W.make_config(cfg)
+    x1, v1 = _enc_inputs(w)
+    m = _mk(M, w)
+    m.snapshot()
+    m.set("x", x1); m.set("v", v1)
+    cnt = m.encounters(w.dt)
+    got = m.pair_list(cnt)
+    assert cnt == len(got) > 0
+    assert got.tolist() == sorted(got.tolist()) and np.all(got[:, 0] < got[:, 1])
+    fl = np.zeros(w.nb, dtype=np.uint8); fl[got.ravel()] = 1
+    assert np.array_equal(fl, m.get("flag"))
+    # rows 0..7 hold the giants (most pairs) - take them plus a strided sample
+    for phase_rows, kw in [(got[got[:, 0] % stride == 5], dict(row_stride=stride, row_phase=5))]:
+        ref = oracle.encounters(w.dt, w.x, w.v, x1, v1, w.rcrit, **kw)
+        _pairs_ok(phase_rows, ref)
+    m.close()
+
+
+def test_encounters_overflow_and_edges(M):
+    w = W.shrink(0, 200)
+    x1, v1 = _enc_inputs(w)
+    huge = np.full(w.nb, 1e3)
+    ref = oracle.encounters(w.dt, w.x, w.v, x1, v1, huge)
+    total = w.nb * (w.nb - 1) // 2
+    assert ref["count"] == total
+    cap = 1000
+    m = M.Mopal(w.mass, w.x, w.v, huge, cap=cap)
+    m.snapshot(); m.set("x", x1); m.set("v", v1)
+    cnt = m.encounters(w.dt)
+    assert cnt == total                                       # true total past cap
+    assert np.array_equal(m.pair_list(cnt), ref["pairs"][:cap])   # first cap pairs in sorted order
+    assert m.get("flag").all()
+    with pytest.raises(M.MopalError) as ei:
+        m.encounters(w.dt, raise_on_overflow=True)
+    assert ei.value.status == M.MO_EOVERFLOW
+    m.close()
+    # rcrit = 0: nothing; negative dt with start/end swapped: same list
+    m = M.Mopal(w.mass, w.x, w.v, np.zeros(w.nb))
+    m.snapshot(); m.set("x", x1); m.set("v", v1)
+    assert m.encounters(w.dt) == 0 and not m.get("flag").any()
+    m.close()
+    rc = w.rcrit * 3
+    ref = oracle.encounters(-w.dt, x1, v1, w.x, w.v, rc)
+    m = M.Mopal(w.mass, x1, v1, rc)
+    m.snapshot(); m.set("x", w.x); m.set("v", w.v)
+    cnt = m.encounters(-w.dt)
+    _pairs_ok(m.pair_list(cnt), ref)
+    assert cnt > 0
+    m.close()
+
+
+def test_encounters_explicit_x0_v0_pointers(M):
+    import torch
+    w = W.shrink(1, 600)
+    x1, v1 = _enc_inputs(w)
+    ref = oracle.encounters(w.dt, w.x, w.v, x1, v1, w.rcrit)
+    m = M.Mopal(w.mass, x1, v1, w.rcrit)
+    x0 = torch.zeros_like(m.x); v0 = torch.zeros_like(m.v)
+    x0[:, :w.nb] = torch.from_numpy(w.x).cuda(); v0[:, :w.nb] = torch.from_numpy(w.v).cuda()
+    cnt = m.encounters(w.dt, x0, v0)
+    _pairs_ok(m.pair_list(cnt), ref)
+    m.close()
+
+
+# ------------------------------------------------------------------------------ step
+def _step_err(m, ref):
+    return _rel_vec_err(m.get("x"), ref["x"]).max(), _rel_vec_err(m.get("v"), ref["v"]).max()
+
+
+@pytest.mark.parametrize("cfg,nsteps", [(0, 10), (1, 3), (2, 1)])
+def test_step_vs_oracle(M, cfg, nsteps):
+    w = W.make_config(cfg)
+    gm = G * w.mass
+    mu = G * w.m_star
+    m = _mk(M, w)
+    a, _ = oracle.accel(gm, w.x, w.rcrit)
+    x, v = w.x, w.v
+    for k in range(nsteps):
+        st = m.step(w.dt, 1)
+        r = oracle.step(mu, gm, w.rcrit, w.dt, x, v, a)
+        x, v, a = r["x"], r["v"], r["a"]
+        ex, ev = _step_err(m, r)
+        tol = 1e-13 * (1 + k)                     # graded: rounding differences grow (P-S6)
+        assert ex <= tol and ev <= tol, (k, ex, ev)
+        assert st.steps_done == k + 1 and st.drift_fail == 0
+        got = m.pair_list(st.nce_last)
+        _pairs_ok(got, r)
+        if r["n_ambig"] == 0:
+            assert st.nce_last == r["count"]
+        # the snapshot is the oracle's x0, v0
+        x0, v0 = m.snapshot_tensors()
+        assert _rel_vec_err(x0[:, :w.nb].cpu().numpy(), r["x0"]).max() <= tol
+    m.close()
+
+
+def test_step_multi_equals_single_steps_and_graph_path(M):
+    w = W.make_config(0)
+    m1 = _mk(M, w); m2 = _mk(M, w)
+    for _ in range(6):
+        m1.step(w.dt, 1)
+    st = m2.step(w.dt, 6)                        # CUDA-graph replay path
+    assert st.steps_done == 6
+    assert np.array_equal(m1.get("x"), m2.get("x")) and np.array_equal(m1.get("v"), m2.get("v"))
+    assert m1.stats().nce_total == st.nce_total
+    m1.close(); m2.close()
+
+
+def test_step_nb1_and_reversibility(M):
+    w = W.make_disk(N=2, seed=1, giants=[(1e-3, 5.2, 0.05, 0.02, 0.3)], a=("uniform", 1, 2), sig_e=0.01,
+                    sig_i=0.01, mass=("equal", 1e-9), dt=8.0, steps=1)
+    m = _mk(M, w)
+    m.step(8.0, 1)
+    r = oracle.step(G, G * w.mass, w.rcrit, 8.0, w.x, w.v, np.zeros((3, 1)))
+    ex, ev = _step_err(m, r)
+    assert ex <= 1e-13 and ev <= 1e-13
+    m.close()
+    w = W.make_config(0)
+    m = _mk(M, w)
+    m.step(w.dt, 5); m.step(-w.dt, 5)
+    assert _rel_vec_err(m.get("x"), w.x).max() <= 1e-12 and _rel_vec_err(m.get("v"), w.v).max() <= 1e-12
+    m.close()
+
+
+@pytest.mark.parametrize("cfg,nsteps", [(3, 3), (4, 2)])
+def test_step_headline_sizes_properties(M, cfg, nsteps):
+    """full sizes: properties that hold at any size + sampled oracle rows on the final state."""
+    w = W.make_config(cfg)
+    m = _mk(M, w)
+    L0 = (w.mass * np.cross(w.x.T, w.v.T).T).sum(1)
+    st = m.step(w.dt, nsteps)
+    assert st.steps_done == nsteps and st.drift_fail == 0
+    x, v, a = m.get("x"), m.get("v"), m.get("a")
+    L1 = (w.mass * np.cross(x.T, v.T).T).sum(1)
+    assert np.linalg.norm(L1 - L0) <= 1e-13 * np.linalg.norm(L0)       # P-S2
+    rows = np.unique(np.random.default_rng(1).integers(0, w.nb, 24)).astype(np.int32)
+    a_ref, S = oracle.accel_rows(G * w.mass, x, w.rcrit, rows)          # a is current for x
+    _check_accel(a[:, rows], a_ref, S)
+    got = m.pair_list(st.nce_last)
+    assert len(got) == st.nce_last and got.tolist() == sorted(got.tolist())
+    m.close()
+
+
+# ------------------------------------------------------------------------------ boundary
+def test_host_buffer_entry_points(M):
+    import torch
+    w = W.make_config(0)
+    m = _mk(M, w)
+    xh = torch.zeros((3, m.ld), dtype=torch.float64).pin_memory(); vh = torch.zeros_like(xh).pin_memory()
+    xh[:, :w.nb] = torch.from_numpy(w.x); vh[:, :w.nb] = torch.from_numpy(w.v)
+    ah = torch.zeros_like(xh).pin_memory()
+    m.accel_host(xh, ah)
+    a_ref, S = oracle.accel(G * w.mass, w.x, w.rcrit)
+    _check_accel(ah[:, :w.nb].numpy(), a_ref, S)
+    ph = torch.zeros((4096, 2), dtype=torch.int32).pin_memory()
+    st = m.step_host(w.dt, 2, xh, vh, rcrit_host=torch.from_numpy(w.rcrit), a_is_current=True, pairs_host=ph)
+    m2 = _mk(M, w); st2 = m2.step(w.dt, 2)
+    assert np.array_equal(xh[:, :w.nb].numpy(), m2.get("x")) and np.array_equal(vh[:, :w.nb].numpy(), m2.get("v"))
+    assert st.nce_last == st2.nce_last and np.array_equal(ph[:st.nce_last].numpy(), m2.pair_list(st2.nce_last))
+    m.close(); m2.close()
+
+
+def test_invalid_arguments_and_bookkeeping(M):
+    import ctypes as C
+    w = W.shrink(0, 64)
+    m = _mk(M, w)
+    L = M.load()
+    assert L.mo_step(m._ctx, 0.0, 1, None) == M.MO_EINVAL
+    assert L.mo_step(m._ctx, float("nan"), 1, None) == M.MO_EINVAL
+    assert L.mo_step(m._ctx, 1.0, -1, None) == M.MO_EINVAL
+    assert L.mo_encounters(m._ctx, 1.0, None, None, None) == M.MO_EINVAL   # no snapshot yet
+    ctx = C.c_void_p()
+    assert L.mo_create(C.byref(ctx), 0, 0, 1.0, 1.0, None, None, None, None, None, None, 0, None, None) == M.MO_EINVAL
+    assert L.mo_create(C.byref(ctx), 5, 5, 1.0, 1.0, m.mass.data_ptr(), m.x.data_ptr(), m.v.data_ptr(), m.a.data_ptr(),
+                       m.rcrit.data_ptr(), None, 0, m.flag.data_ptr(), None) == M.MO_EINVAL   # ld % 4
+    n0 = m.launch_count()
+    m.accel()
+    assert m.launch_count() == n0 + 3 and m.workspace_bytes() > 0
+    g = m.pair_geometry()
+    assert g["ctas"] >= 1 and g["ipt"] in (1, 2)
+    tf, ms = M.probe_fp64_peak(2)
+    assert 5.0 < tf < 80.0
+    m.close()

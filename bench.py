@@ -1,0 +1,312 @@
+#!/usr/bin/env python
+"""bench.py - BASELINE.json's metric on BASELINE.json's headline config.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 3]
+
+A "step" is one pass of the whole hot path (kick, jump, snapshot,
+Kepler drift, encounter boxes + pair list, jump, O(N^2) K-weighted pair accelerations, kick)
+= one ``mo_step`` over the N=65,536 planetesimal disk (config 3, seed 4; synthetic, recipe
+in DESIGN.md).  ``value`` = ordered FP64 pair interactions per second, nb*(nb-1) per step,
+with all state resident in HBM; ``e2e`` = the same through ``mo_step_host`` with pinned HOST
+buffers (x, v, rcrit up; x, v, pair list, stats down inside the timed region).
+
+One JSON line on stdout (rank 0).  The path does not shard (north_star: one GPU): under
+torchrun every rank runs an independent replica, timing is the
+max over ranks, ``value`` the total over replicas.
+
+``--impl reference`` times the CPU oracle (test infrastructure, as it stands) on the box's
+host cores on a bounded sample of the same step - a deliberately slow baseline.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+METRIC = "fp64_pair_interactions_per_s"
+UNIT = "pairs/s"
+FLOP_PER_PAIR = 26.0          # SURVEY.md 8(d) / DESIGN.md: K = 1 path, per ordered pair
+FP64_LANES_PER_SM = 64        # DESIGN.md section "Rooflines": 148 SMs x 64 DFMA/clk x 2 x f
+# dram__bytes_read.sum + dram__bytes_write.sum of one pair_accel_kernel launch at config 3
+# from the ncu --set full capture summarised in profiles/ (None until captured)
+PAIR_KERNEL_DRAM_TRAFFIC_BYTES = None
+
+
+def _dist_env():
+    return int(os.environ.get("RANK", "0")), int(os.environ.get("LOCAL_RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.idx = gpu_index
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+
+    def start(self):
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                       "-lms", "100", "-i", str(self.idx)], stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush(); self.f.seek(0)
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f.read().splitlines():
+            c = [t.strip() for t in line.split(",")]
+            if len(c) < 9:
+                continue
+            try:
+                sm.append(float(c[1])); mx.append(float(c[2])); pw.append(float(c[3]))
+            except ValueError:
+                continue
+            for n, val in zip(names, c[5:9]):
+                if val.lower().startswith("active"):
+                    reasons.add(n)
+        self.f.close()
+        try:
+            os.unlink(self.f.name)
+        except OSError:
+            pass
+        if sm:
+            out.update(sm_mhz=statistics.median(sm), sm_max_mhz=max(mx), reasons=sorted(reasons), samples=len(sm),
+                       power_w_max=max(pw))
+        return out
+
+
+def _host_cores() -> int:
+    try:
+        return len(os.sched_getaffinity(0))
+    except AttributeError:
+        return os.cpu_count() or 1
+
+
+# --------------------------------------------------------------------------- CPU oracle leg
+def oracle_step_sample(w, budget_s: float, kind: str = "ld"):
+    """Times the oracle on a bounded sample of ONE hybrid step of workload w and scales it to
+    the whole step: R sampled rows of the pair sum (each row is the full ascending-j loop),
+    a strided row sample of the encounter pass, and the full O(N) drift.  Returns
+    (estimated seconds per full step, description, seconds actually spent)."""
+    import oracle
+    cores = _host_cores()
+    oracle.set_threads(cores)
+    gm, mu = w.G * w.mass, w.G * w.m_star
+    nb = w.nb
+    t_start = time.perf_counter()
+    # calibrate on a few rows, then size the sample for the budget
+    rows = np.arange(0, nb, max(1, nb // (4 * cores)), dtype=np.int32)[: 4 * cores]
+    t0 = time.perf_counter(); oracle.accel_rows(gm, w.x, w.rcrit, rows, kind=kind); t1 = time.perf_counter()
+    per_row = (t1 - t0) / len(rows)
+    R = int(min(nb, max(len(rows), 0.6 * budget_s / max(per_row, 1e-9))))
+    rows = np.unique(np.linspace(0, nb - 1, R).astype(np.int32))
+    t0 = time.perf_counter(); oracle.accel_rows(gm, w.x, w.rcrit, rows, kind=kind); t_acc = time.perf_counter() - t0
+    t0 = time.perf_counter(); x1, v1, _ = oracle.drift(mu, w.dt, w.x, w.v, kind=kind); t_drift = time.perf_counter() - t0
+    # encounter rows i % stride == 0 see on average the same number of j > i as any other phase
+    stride = int(max(1, round(nb / max(len(rows) * 2, 1))))
+    t0 = time.perf_counter()
+    oracle.encounters(w.dt, w.x, w.v, x1, v1, w.rcrit, kind=kind, row_stride=stride, row_phase=0)
+    t_enc = time.perf_counter() - t0
+    est = t_acc * nb / len(rows) + t_enc * stride + t_drift
+    what = (f"one hybrid step estimated from {len(rows)} of {nb} pair-sum rows ({t_acc:.2f} s), encounter rows "
+            f"i%{stride}==0 ({t_enc:.2f} s) and the full drift ({t_drift:.3f} s); oracle build '{kind}' "
+            f"({'x87 long double' if kind == 'ld' else 'plain double'}), OpenMP over rows")
+    return est, what, time.perf_counter() - t_start
+
+
+def run_reference(args):
+    rank, _, world = _dist_env()
+    if rank != 0:
+        return 0
+    from paper_2601_19654_b200 import workloads as W
+    w = W.make_config(args.config)
+    pairs = w.nb * (w.nb - 1)
+    cores = _host_cores()
+    budget = max(2.0, min(20.0, 150.0 / max(args.steps + args.warmup, 1)))
+    est = []
+    what = ""
+    for k in range(args.warmup + args.steps):
+        e, what, _ = oracle_step_sample(w, budget)
+        if k >= args.warmup:
+            est.append(e)
+    sec = sum(est) / len(est)
+    val = pairs / sec
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": w.name, "N": w.N, "nb": w.nb, "dt_days": w.dt, "seed": w.seed},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": what},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# --------------------------------------------------------------------------- GPU leg
+def run_ours(args):
+    import torch
+    rank, local_rank, world = _dist_env()
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py: no CUDA device - libmopal has no CPU path (use --impl reference for the oracle)")
+    dev = local_rank % torch.cuda.device_count()
+    torch.cuda.set_device(dev)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", dev))
+    from paper_2601_19654_b200 import mopal as M
+    from paper_2601_19654_b200 import workloads as W
+
+    w = W.make_config(args.config)
+    nb, pairs = w.nb, w.nb * (w.nb - 1)
+    K, Wm = args.steps, max(args.warmup, 3)
+    cap = 1 << 20
+    m = M.Mopal(w.mass, w.x, w.v, w.rcrit, m_star=w.m_star, G=w.G, cap=cap, device=f"cuda:{dev}")
+    stream = m.stream
+    geo = m.pair_geometry()
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # FP64 issue peak of this GPU: burst (best launch) and sustained (1.5 s train of launches)
+    peak_burst, _, peak_sust = M.probe_fp64_peak(160, with_mean=True)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=m.device)   # > 126 MB L2
+
+    # ---- device-resident timing: K steps, L2 flushed between timed steps ------------------
+    m.accel()
+    for _ in range(Wm):
+        m.step(w.dt, 1, sync=False)
+    st0 = m.stats()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
+    sampler = ClockSampler(dev)
+    sampler.start()
+    m.set_kernel_timing(True)
+    barrier()
+    n0 = m.launch_count()
+    t_wall0 = time.perf_counter()
+    for k in range(K):
+        flush.zero_()                       # untimed: evicts the 5.8 MB state from L2
+        ev[k][0].record(stream)
+        m.step(w.dt, 1, sync=False)
+        ev[k][1].record(stream)
+    barrier()
+    t_wall = time.perf_counter() - t_wall0
+    n_launch = m.launch_count() - n0
+    pair_ms, n_pair = m.pair_kernel_ms()
+    m.set_kernel_timing(False)
+    clocks = sampler.stop()
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    total_ms = sum(step_ms)
+    st1 = m.stats()
+    assert st1.steps_done - st0.steps_done == K and st1.drift_fail == 0, (st0, st1)
+
+    # ---- end to end through the host-buffer entry point ------------------------------------
+    ld = m.ld
+    xh = torch.zeros((3, ld), dtype=torch.float64).pin_memory(); vh = torch.zeros((3, ld), dtype=torch.float64).pin_memory()
+    xh[:, :nb] = torch.from_numpy(w.x); vh[:, :nb] = torch.from_numpy(w.v)
+    rh = torch.from_numpy(w.rcrit.copy()).pin_memory()
+    ph = torch.zeros((cap, 2), dtype=torch.int32).pin_memory()
+    Ke = max(3, min(K, 10))
+    m.step_host(w.dt, 1, xh, vh, rcrit_host=rh, a_is_current=False, pairs_host=ph)      # warm-up (computes a first)
+    m.step_host(w.dt, 1, xh, vh, rcrit_host=rh, a_is_current=True, pairs_host=ph)
+    barrier()
+    d2h_pairs = 0
+    t0 = time.perf_counter()
+    for _ in range(Ke):
+        s = m.step_host(w.dt, 1, xh, vh, rcrit_host=rh, a_is_current=True, pairs_host=ph)
+        d2h_pairs += 8 * min(s.nce_last, cap)
+    torch.cuda.synchronize()
+    t_e2e = time.perf_counter() - t0
+    h2d = 2 * 3 * ld * 8 + nb * 8
+    d2h = 2 * 3 * ld * 8 + 40 + d2h_pairs // Ke
+
+    # ---- max over ranks --------------------------------------------------------------------
+    tt = torch.tensor([total_ms, t_e2e * 1e3, pair_ms], dtype=torch.float64, device=m.device)
+    if dist is not None:
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    total_ms_max, e2e_ms_max, pair_ms_max = (float(t) for t in tt.tolist())
+    value = world * pairs * K / (total_ms_max * 1e-3)
+    e2e_value = world * pairs * Ke / (e2e_ms_max * 1e-3)
+
+    if rank == 0:
+        achieved = FLOP_PER_PAIR * pairs / (pair_ms_max * 1e-3) / 1e12
+        nsm = torch.cuda.get_device_properties(dev).multi_processor_count
+        sm_max = clocks.get("sm_max_mhz") or 1965.0
+        nominal = nsm * FP64_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
+            "ms_per_step": total_ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": w.name, "N": w.N, "nb": nb, "dt_days": w.dt, "seed": w.seed,
+                       "parallelism": "single GPU" if world == 1 else f"{world} independent replicas (path does not shard)",
+                       "l2": "flushed (256 MiB memset) between timed steps; the 5.8 MB state is otherwise L2-resident",
+                       "pair_kernel_geometry": geo, "encounter_pairs_last_step": st1.nce_last},
+            "pct_fp64_peak": {"of_measured_sustained": 100 * achieved / peak_sust, "of_measured_burst": 100 * achieved / peak_burst,
+                              "of_nominal": 100 * achieved / nominal, "flop_per_pair": FLOP_PER_PAIR},
+            "roofline": {"bound": "alu", "kernel": "pair_accel_kernel", "achieved": achieved, "peak": peak_sust,
+                         "unit": "TFLOP/s", "frac": achieved / peak_sust, "traffic": PAIR_KERNEL_DRAM_TRAFFIC_BYTES,
+                         "peak_source": "mo_probe_fp64_peak: register-resident DFMA loop on this GPU, 160 launches back to "
+                                        "back (sustained); MEASURED_PEAKS.json has no FP64 figure",
+                         "peak_burst": peak_burst, "peak_nominal": nominal, "kernel_ms": pair_ms_max, "kernel_launches_timed": n_pair,
+                         "kernel_share_of_step": pair_ms_max * n_pair / total_ms_max,
+                         "pairs_per_s_kernel": pairs / (pair_ms_max * 1e-3)},
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                    "steps": Ke, "ms_per_step": e2e_ms_max / Ke, "api": "mo_step_host (pinned host x, v, rcrit in; x, v, pairs, stats out)"},
+            "gpu_launches": n_launch,
+            "clocks": {k: clocks.get(k) for k in ("sm_mhz", "sm_max_mhz", "reasons", "samples", "power_w_max")},
+            "wall_s_timed_region": t_wall,
+        }
+        if not args.no_cpu and world == 1:
+            est, what, _ = oracle_step_sample(w, args.cpu_budget)
+            line["cpu_baseline"] = {"value": pairs / est, "unit": UNIT, "cores": _host_cores(), "kind": "oracle",
+                                    "sample": what, "ms_per_step": est * 1e3}
+        print(json.dumps(line), flush=True)
+    m.close()
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json config index (3 = N=65,536 headline)")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of CPU work for the cpu_baseline sample")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -146,11 +146,13 @@ mo_status mo_step_host(mo_ctx *ctx, double dt, int32_t nsteps, double *x_host,
 mo_status mo_accel_host(mo_ctx *ctx, const double *x_host, double *a_host);
 
 /* Measures the FP64 FMA issue peak of the current device with a register-resident
- * DFMA loop (148 SMs x 64 lanes x 2 flop x clock on B200): runs `reps` timed launches
- * on `cuda_stream` and writes the best TFLOP/s and its duration in ms.  Used as the
- * measured denominator of the pair kernel's roofline (MEASURED_PEAKS.json has none). */
+ * DFMA loop (148 SMs x 64 lanes x 2 flop x clock on B200): runs `reps` back-to-back timed
+ * launches on `cuda_stream` and writes the best single launch's TFLOP/s (burst) and its
+ * duration in ms, and - if tflops_mean_out != NULL - the TFLOP/s over the whole train of
+ * launches (sustained, under the power cap when reps spans seconds).  Used as the measured
+ * denominator of the pair kernel's roofline (MEASURED_PEAKS.json has no FP64 figure). */
 mo_status mo_probe_fp64_peak(void *cuda_stream, int32_t reps, double *tflops_out,
-                             double *ms_out);
+                             double *ms_out, double *tflops_mean_out);
 
 /* Pair-kernel launch geometry chosen for this nb: i-bodies per thread, j-splits,
  * CTAs, resident CTAs per SM (all nullable). */

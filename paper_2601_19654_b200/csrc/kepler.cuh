@@ -59,7 +59,7 @@ __device__ __forceinline__ GF gfuncs(double X, double beta) {
 constexpr int DRIFT_MAX_NEWTON = 12;
 
 // returns 0 ok / 1 failed (state untouched); *iters = Newton iterations used
-__device__ __forceinline__ int drift_body(double mu, double dt, double& x, double& y, double& z, double& vx,
+__device__ __forceinline__ int drift_body(double mu, double dt_full, double& x, double& y, double& z, double& vx,
                                           double& vy, double& vz, int* iters) {
     const double r0 = sqrt(fma(z, z, fma(y, y, x * x)));
     *iters = 0;
@@ -67,6 +67,14 @@ __device__ __forceinline__ int drift_body(double mu, double dt, double& x, doubl
     const double v2 = fma(vz, vz, fma(vy, vy, vx * vx));
     const double eta0 = fma(z, vz, fma(y, vy, x * vx));
     const double beta = 2.0 * mu / r0 - v2;
+    // A bound orbit returns to the same state after T = 2 pi mu / beta^(3/2): drop whole
+    // periods first.  Otherwise z = beta X^2 grows like (2 pi dt/T)^2, each argument
+    // quartering of stumpff() doubles the phase error and dt - mu G3 cancels ~dt/T digits.
+    double dt = dt_full;
+    if (beta > 0.0) {
+        const double T = 6.283185307179586 * mu / (beta * sqrt(beta));
+        if (fabs(dt_full) > T) dt = fma(-rint(dt_full / T), T, dt_full);
+    }
     double X = dt / r0;
     bool conv = false;
     int it = 0;

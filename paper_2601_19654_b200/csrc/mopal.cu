@@ -24,6 +24,7 @@ struct mo_ctx {
     long long cap = 0;
     uint8_t* flag = nullptr;
     cudaStream_t stream = nullptr;
+    cudaStream_t cap_stream = nullptr;  // owned: graph capture needs a non-legacy stream
     // owned scratch
     double *gm = nullptr, *x0 = nullptr, *v0 = nullptr, *part = nullptr, *psumA = nullptr, *psumB = nullptr;
     unsigned char* tiles = nullptr;
@@ -138,6 +139,7 @@ extern "C" const char* mo_version(void) { return "libmopal 0.1 (sm_100a)"; }
 extern "C" void mo_destroy(mo_ctx* ctx) {
     if (!ctx) return;
     if (ctx->gexec) cudaGraphExecDestroy(ctx->gexec);
+    if (ctx->cap_stream) cudaStreamDestroy(ctx->cap_stream);
     for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
     cudaFree(ctx->gm); cudaFree(ctx->x0); cudaFree(ctx->v0); cudaFree(ctx->part);
     cudaFree(ctx->psumA); cudaFree(ctx->psumB); cudaFree(ctx->tiles); cudaFree(ctx->box);
@@ -402,9 +404,15 @@ extern "C" mo_status mo_step(mo_ctx* ctx, double dt, int32_t nsteps, mo_stats* s
             if (ctx->gexec) { cudaGraphExecDestroy(ctx->gexec); ctx->gexec = nullptr; }
             cudaGraph_t g = nullptr;
             const long long l0 = ctx->launches;
-            CK(cudaStreamBeginCapture(ctx->stream, cudaStreamCaptureModeThreadLocal));
+            // the caller's stream may be the legacy default stream, which cannot be captured:
+            // record the step on an owned stream, replay the graph on the caller's
+            if (!ctx->cap_stream) CK(cudaStreamCreateWithFlags(&ctx->cap_stream, cudaStreamNonBlocking));
+            cudaStream_t user = ctx->stream;
+            CK(cudaStreamBeginCapture(ctx->cap_stream, cudaStreamCaptureModeThreadLocal));
+            ctx->stream = ctx->cap_stream;
             s = enqueue_step(ctx, dt);
-            cudaError_t e = cudaStreamEndCapture(ctx->stream, &g);
+            ctx->stream = user;
+            cudaError_t e = cudaStreamEndCapture(ctx->cap_stream, &g);
             ctx->launches = l0;  // captured, not launched
             if (s != MO_OK || e != cudaSuccess) {
                 if (g) cudaGraphDestroy(g);
@@ -513,7 +521,8 @@ extern "C" mo_status mo_accel_host(mo_ctx* ctx, const double* x_host, double* a_
     return MO_OK;
 }
 
-extern "C" mo_status mo_probe_fp64_peak(void* cuda_stream, int32_t reps, double* tflops_out, double* ms_out) {
+extern "C" mo_status mo_probe_fp64_peak(void* cuda_stream, int32_t reps, double* tflops_out, double* ms_out,
+                                        double* tflops_mean_out) {
     if (!tflops_out || reps < 1) return MO_EINVAL;
     cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
     int dev = 0, nsm = 0;
@@ -527,11 +536,12 @@ extern "C" mo_status mo_probe_fp64_peak(void* cuda_stream, int32_t reps, double*
         cudaGetLastError();
         return MO_ENOMEM;
     }
-    cudaEvent_t e0, e1;
-    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    cudaEvent_t e0, e1, ea, eb;
+    cudaEventCreate(&e0); cudaEventCreate(&e1); cudaEventCreate(&ea); cudaEventCreate(&eb);
     double best = 1e300;
     mo_status rs = MO_OK;
     for (int r = 0; r < reps + 2; ++r) {  // two warm-ups
+        if (r == 2) cudaEventRecord(ea, st);
         cudaEventRecord(e0, st);
         dfma_probe_kernel<<<blocks, threads, 0, st>>>(buf, iters, 0.999999, 1e-9);
         cudaEventRecord(e1, st);
@@ -540,11 +550,18 @@ extern "C" mo_status mo_probe_fp64_peak(void* cuda_stream, int32_t reps, double*
         cudaEventElapsedTime(&ms, e0, e1);
         if (r >= 2 && ms < best) best = ms;
     }
-    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    float tot = 0.f;
+    if (rs == MO_OK) {
+        cudaEventRecord(eb, st);
+        if (cudaEventSynchronize(eb) != cudaSuccess) rs = MO_ECUDA;
+        else cudaEventElapsedTime(&tot, ea, eb);
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaEventDestroy(ea); cudaEventDestroy(eb);
     cudaFree(buf);
     if (rs != MO_OK) { cudaGetLastError(); return rs; }
     const double flops = (double)blocks * threads * (double)iters * 32.0 * 2.0;
     *tflops_out = flops / (best * 1e-3) / 1e12;
     if (ms_out) *ms_out = best;
+    if (tflops_mean_out) *tflops_mean_out = flops * reps / (tot * 1e-3) / 1e12;
     return MO_OK;
 }

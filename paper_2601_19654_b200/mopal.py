@@ -66,7 +66,7 @@ def load():
     L.mo_step_host.argtypes = [vp, D, I32, vp, vp, vp, I32, vp, I64, C.POINTER(MoStats)]
     L.mo_accel_host.restype = C.c_int; L.mo_accel_host.argtypes = [vp, vp, vp]
     L.mo_probe_fp64_peak.restype = C.c_int
-    L.mo_probe_fp64_peak.argtypes = [vp, I32, C.POINTER(D), C.POINTER(D)]
+    L.mo_probe_fp64_peak.argtypes = [vp, I32, C.POINTER(D), C.POINTER(D), C.POINTER(D)]
     L.mo_pair_geometry.restype = C.c_int
     L.mo_pair_geometry.argtypes = [vp, C.POINTER(I32), C.POINTER(I32), C.POINTER(I32), C.POINTER(I32)]
     L.mo_set_kernel_timing.restype = C.c_int; L.mo_set_kernel_timing.argtypes = [vp, I32]
@@ -85,16 +85,18 @@ def version() -> str:
     return load().mo_version().decode()
 
 
-def probe_fp64_peak(reps: int = 5):
-    """(TFLOP/s, ms) of the library's register-resident DFMA probe on the current device."""
+def probe_fp64_peak(reps: int = 5, with_mean: bool = False):
+    """(best TFLOP/s, its ms[, TFLOP/s over the whole train]) of the library's register-resident
+    DFMA probe on the current device."""
     import torch
     if not torch.cuda.is_available():
         raise MopalError(MO_ECUDA, "mo_probe_fp64_peak")
-    tf, ms = C.c_double(0), C.c_double(0)
-    st = load().mo_probe_fp64_peak(C.c_void_p(torch.cuda.current_stream().cuda_stream), reps, C.byref(tf), C.byref(ms))
+    tf, ms, mean = C.c_double(0), C.c_double(0), C.c_double(0)
+    st = load().mo_probe_fp64_peak(C.c_void_p(torch.cuda.current_stream().cuda_stream), reps, C.byref(tf), C.byref(ms),
+                                   C.byref(mean))
     if st != MO_OK:
         raise MopalError(st, "mo_probe_fp64_peak")
-    return tf.value, ms.value
+    return (tf.value, ms.value, mean.value) if with_mean else (tf.value, ms.value)
 
 
 @dataclass

@@ -82,6 +82,8 @@ def test_accel_headline_sizes_sampled_rows(M, cfg):
 @pytest.mark.parametrize("nb", [1, 2, 3, 127, 128, 129, 255, 257, 1000])
 def test_accel_ragged_sizes_and_changeover_shell(M, nb):
     w = W.random_cluster(nb, 100 + nb, box=1.0, rc_frac=(0.0, 0.7)) if nb > 1 else W.random_cluster(1, 5)
+    if nb > 100:   # plant one pair well inside 0.1 rc (K = 0) - random draws do not always have one
+        w.x[:, 1] = w.x[:, 0] + np.array([0.03 * max(w.rcrit[0], w.rcrit[1]), 0.0, 0.0])
     m = _mk(M, w)
     m.accel()
     a = m.get("a")

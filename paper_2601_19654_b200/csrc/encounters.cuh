@@ -6,13 +6,25 @@
 //                      only when approaching at the start and receding at the end)
 //                      is <= max(rcrit_i, rcrit_j)^2.
 // The paper appends with an atomic capture in whatever order threads arrive
-// (PAPER.md:264-269).  Here the list is deterministic and sorted by construction:
-//   pass 1  thread-per-row i over TMA-staged tiles of j boxes counts the hits of each row,
-//   scan    exclusive prefix sum of the row counts gives each row's slot range,
-//   pass 2  one warp per non-empty row re-tests its j's in order and compacts the hits
-//           with warp ballot + prefix popcounts straight into the row's slots.
-// Both passes call the same pair test, written with explicit _rn intrinsics so that the
-// compiler can neither contract nor reorder it: the two passes decide identically.
+// (PAPER.md:264-269).  Here the list is deterministic and sorted:
+//   find    thread-per-row i over TMA-staged tiles of j boxes.  The O(N^2/2) gate runs on
+//           FP32 copies of the boxes rounded OUTWARD (lo down, hi up), so it can only pass
+//           more pairs than the FP64 gate, never fewer; it costs 1 LDS.128 + 4 FSETP per
+//           pair on the FP32/ALU pipes.  Survivors (~1e-5..1e-3 of the pairs) are compacted
+//           per warp with ballot + prefix popcounts into a shared-memory queue and taken 32
+//           at a time - one survivor per lane - through the exact FP64 box gate and the
+//           exact pair test.  Hits bump their row's counter and go to an unsorted hit list.
+//   scan    exclusive prefix sum of the row counts gives each row's slot range, the total
+//           count and the overflow flag.
+//   place   every hit drops its j into its row's slot range (scratch), then ranks itself
+//           among its row's j's and writes (i, j) at rowoff[i] + rank: the final list is
+//           sorted by (i, j) whatever order the atomics ran in.
+//   overflow (count > cap): the list must hold the FIRST cap pairs in sorted order, which an
+//           unsorted hit list cannot give; enc_write_kernel then re-tests the non-empty rows
+//           in order (one warp per row, ballot compaction straight into the row's slots).
+//           It exits at once when there was no overflow.
+// The pair test is written with explicit _rn intrinsics so that the compiler can neither
+// contract nor reorder it: every pass decides identically.
 #pragma once
 #include "common.cuh"
 
@@ -106,40 +118,85 @@ __device__ __noinline__ bool pair_hit(const EncState& s, int i, int j) {
     return d2min <= __dmul_rn(rc, rc);
 }
 
-__device__ __forceinline__ bool box_gate(const double4& bi, const double2& ja, const double2& jb) {
-    // {lox,hix} = ja, {loy,hiy} = jb of body j
-    return (bi.x <= ja.y) & (ja.x <= bi.y) & (bi.z <= jb.y) & (jb.x <= bi.w);
+// conservative FP32 copy of a box: lo rounded down, hi rounded up
+__device__ __forceinline__ float4 box_f32(const double4& b) {
+    return make_float4(__double2float_rd(b.x), __double2float_ru(b.y), __double2float_rd(b.z), __double2float_ru(b.w));
+}
+__device__ __forceinline__ double4 pad_box() {   // can never overlap anything
+    const double inf = __longlong_as_double(0x7ff0000000000000LL);
+    return make_double4(inf, -inf, inf, -inf);
+}
+__device__ __forceinline__ float4 pad_boxf() {
+    const float inf = __int_as_float(0x7f800000);
+    return make_float4(inf, -inf, inf, -inf);
 }
 
+// per-pass device scratch of the encounter pipeline
+struct EncBuf {
+    double4* box;        // nbPad exact boxes {lox, hix, loy, hiy}
+    float4* boxf;        // nbPad outward-rounded FP32 boxes (the j tiles of the find pass)
+    int* rowcnt;         // nbPad hits per row
+    int* rowfill;        // nbPad placement cursor per row
+    long long* rowoff;   // nbPad exclusive prefix of rowcnt
+    int2* hits;          // cap unsorted hits (i, j)
+    int* tmpj;           // cap j's grouped by row, unsorted inside a row
+    unsigned long long* nhit;  // hits appended this pass (may exceed cap)
+    int* ovf_now;        // this pass found more pairs than cap
+};
+
 // ---- O(N) kernel: boxes, and reset of the per-row counters and flags ------------------------
-__global__ void __launch_bounds__(ON_BLOCK) boxes_kernel(EncState s, double4* __restrict__ box, int nbPad,
-                                                         int* __restrict__ rowcnt, uint8_t* __restrict__ flag) {
+__global__ void __launch_bounds__(ON_BLOCK) boxes_kernel(EncState s, EncBuf e, int nbPad, uint8_t* __restrict__ flag) {
     const int b = blockIdx.x * ON_BLOCK + threadIdx.x;
+    if (b == 0) *e.nhit = 0ull;
     if (b >= nbPad) return;
     double4 r;
     if (b < s.nb) {
         body_box(s.x0, s.v0, s.x1, s.v1, s.rcrit[b], s.ld, b, s.h, r);
-        rowcnt[b] = 0;
         flag[b] = 0;
+        e.boxf[b] = box_f32(r);
     } else {
-        const double inf = __longlong_as_double(0x7ff0000000000000LL);
-        r = make_double4(inf, -inf, inf, -inf);
+        r = pad_box();
+        e.boxf[b] = pad_boxf();
     }
-    box[b] = r;
+    e.rowcnt[b] = 0;
+    e.rowfill[b] = 0;
+    e.box[b] = r;
 }
 
-// ---- pass 1: per-row hit counts ----------------------------------------------------------------
-struct EncCountParams {
+// ---- find: FP32 gate over all i<j, exact test on the warp-compacted survivors ----------------
+constexpr int BOXF_TILE_BYTES = TJ * 16;   // TJ x float4
+constexpr int ENC_BATCH = 8;               // j's gated between two survivor checks
+constexpr int ENC_QCAP = 64;               // per-warp survivor queue (a drain leaves < 32)
+
+struct EncFindParams {
     EncState s;
-    const double4* box;  // nbPad records
-    int* rowcnt;
+    EncBuf e;
+    long long cap;
     int nTiles, tps;
 };
 
-__global__ void __launch_bounds__(CTA_THREADS) enc_count_kernel(EncCountParams p) {
-    __shared__ __align__(128) unsigned char s_tiles[STAGES * BOX_TILE_BYTES];
+__device__ __forceinline__ bool gate_f32(const float4& a, const float4& b) {
+    return (a.x <= b.y) & (b.x <= a.y) & (a.z <= b.w) & (b.z <= a.w);
+}
+__device__ __forceinline__ bool gate_f64(const double4& a, const double4& b) {
+    return (a.x <= b.y) & (b.x <= a.y) & (a.z <= b.w) & (b.z <= a.w);
+}
+
+// one survivor per lane: exact FP64 gate, exact pair test, record the hit
+__device__ __forceinline__ void enc_exact(const EncFindParams& p, int2 c) {
+    const double4 bi = p.e.box[c.x], bj = p.e.box[c.y];
+    if (!gate_f64(bi, bj)) return;
+    if (!pair_hit(p.s, c.x, c.y)) return;
+    atomicAdd(&p.e.rowcnt[c.x], 1);
+    const unsigned long long pos = atomicAdd(p.e.nhit, 1ull);
+    if ((long long)pos < p.cap) p.e.hits[pos] = c;
+}
+
+__global__ void __launch_bounds__(CTA_THREADS) enc_find_kernel(EncFindParams p) {
+    __shared__ __align__(128) unsigned char s_tiles[STAGES * BOXF_TILE_BYTES];
     __shared__ __align__(8) uint64_t s_full[STAGES];
     __shared__ __align__(8) uint64_t s_empty[STAGES];
+    __shared__ int2 s_q[CONSUMER_THREADS / 32][ENC_QCAP];
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     // rows of this CTA are [rb*TJ, rb*TJ+TJ): only tiles >= rb hold any j > i
@@ -156,38 +213,58 @@ __global__ void __launch_bounds__(CTA_THREADS) enc_count_kernel(EncCountParams p
     }
     __syncthreads();
 
-    if (warp == CONSUMER_THREADS / 32) {
+    if (warp == CONSUMER_THREADS / 32) {  // ---- TMA producer warp ----
         if (lane == 0) {
-            const unsigned char* src = reinterpret_cast<const unsigned char*>(p.box) + (size_t)t0 * BOX_TILE_BYTES;
+            const unsigned char* src = reinterpret_cast<const unsigned char*>(p.e.boxf) + (size_t)t0 * BOXF_TILE_BYTES;
             for (int n = 0; n < nt; ++n) {
                 const int st = n % STAGES;
                 mbar_wait(&s_empty[st], ((n / STAGES) & 1) ^ 1);
-                mbar_arrive_expect_tx(&s_full[st], BOX_TILE_BYTES);
-                tma_load_1d(s_tiles + st * BOX_TILE_BYTES, src + (size_t)n * BOX_TILE_BYTES, BOX_TILE_BYTES, &s_full[st]);
+                mbar_arrive_expect_tx(&s_full[st], BOXF_TILE_BYTES);
+                tma_load_1d(s_tiles + st * BOXF_TILE_BYTES, src + (size_t)n * BOXF_TILE_BYTES, BOXF_TILE_BYTES, &s_full[st]);
             }
         }
         return;
     }
 
+    const unsigned full = 0xffffffffu, lt = (1u << lane) - 1u;
     const int i = rb * TJ + tid;
-    const double inf = __longlong_as_double(0x7ff0000000000000LL);
-    const double4 bi = (i < p.s.nb) ? p.box[i] : make_double4(inf, -inf, inf, -inf);
-    int cnt = 0;
+    const float4 bi = p.e.boxf[i];            // pad rows (i >= nb) hold the never-overlapping box
+    int2* q = s_q[warp];
+    int qhead = 0, qn = 0;                    // warp-uniform
+
     for (int n = 0; n < nt; ++n) {
         const int st = n % STAGES;
         mbar_wait(&s_full[st], (n / STAGES) & 1);
-        const double2* tj = reinterpret_cast<const double2*>(s_tiles + st * BOX_TILE_BYTES);
+        const float4* tj = reinterpret_cast<const float4*>(s_tiles + st * BOXF_TILE_BYTES);
         const int j0 = (t0 + n) * TJ;
-        const int jmin = (t0 + n == rb) ? (tid + 1) : 0;  // diagonal tile: j > i only
-#pragma unroll 4
-        for (int jj = 0; jj < TJ; ++jj) {
-            const double2 ja = tj[2 * jj], jb = tj[2 * jj + 1];
-            if (box_gate(bi, ja, jb) && jj >= jmin) cnt += pair_hit(p.s, i, j0 + jj) ? 1 : 0;
+        const int jmin = (t0 + n == rb) ? tid + 1 : 0;    // diagonal tile: j > i only
+#pragma unroll 1
+        for (int jj = 0; jj < TJ; jj += ENC_BATCH) {
+            bool any = false;
+#pragma unroll
+            for (int u = 0; u < ENC_BATCH; ++u) any |= gate_f32(bi, tj[jj + u]);
+            if (__any_sync(full, any)) {                  // rare: some lane has a survivor in this batch
+#pragma unroll 1
+                for (int u = 0; u < ENC_BATCH; ++u) {
+                    const bool has = gate_f32(bi, tj[jj + u]) && (jj + u >= jmin);
+                    const unsigned bal = __ballot_sync(full, has);
+                    if (bal == 0u) continue;
+                    if (has) q[(qhead + qn + __popc(bal & lt)) & (ENC_QCAP - 1)] = make_int2(i, j0 + jj + u);
+                    qn += __popc(bal);
+                    __syncwarp();
+                    if (qn >= 32) {                       // a full warp of survivors
+                        enc_exact(p, q[(qhead + lane) & (ENC_QCAP - 1)]);
+                        qhead = (qhead + 32) & (ENC_QCAP - 1);
+                        qn -= 32;
+                        __syncwarp();
+                    }
+                }
+            }
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(&s_empty[st]);
     }
-    if (cnt) atomicAdd(&p.rowcnt[i], cnt);
+    if (lane < qn) enc_exact(p, q[(qhead + lane) & (ENC_QCAP - 1)]);
 }
 
 // ---- scan: rowoff = exclusive prefix sum of rowcnt; count -> stats ----------------------------
@@ -199,68 +276,116 @@ struct DevStats {
 };
 
 constexpr int SCAN_THREADS = 1024;
-__global__ void __launch_bounds__(SCAN_THREADS) enc_scan_kernel(const int* __restrict__ rowcnt, long long* __restrict__ rowoff,
-                                                                int nb, long long cap, int step_inc, DevStats* __restrict__ st) {
+// one block; each round scans 4*SCAN_THREADS counters (int4 per thread, coalesced)
+__global__ void __launch_bounds__(SCAN_THREADS) enc_scan_kernel(EncBuf e, int nbPad, long long cap, int step_inc,
+                                                                DevStats* __restrict__ st) {
     __shared__ long long wsum[SCAN_THREADS / 32];
-    const int per = (nb + SCAN_THREADS - 1) / SCAN_THREADS;
-    const int b0 = threadIdx.x * per, b1 = min(b0 + per, nb);
-    long long local = 0;
-    for (int b = b0; b < b1; ++b) local += rowcnt[b];
-    long long incl = local;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        long long t = __shfl_up_sync(0xffffffffu, incl, o);
-        if ((threadIdx.x & 31) >= o) incl += t;
-    }
-    if ((threadIdx.x & 31) == 31) wsum[threadIdx.x >> 5] = incl;
+    __shared__ long long carry_s;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    if (tid == 0) carry_s = 0;
     __syncthreads();
-    if (threadIdx.x < 32) {
-        long long v = wsum[threadIdx.x], inc2 = v;
+    for (int base = 0; base < nbPad; base += 4 * SCAN_THREADS) {   // nbPad is a multiple of TJ
+        const int b = base + 4 * tid;
+        int4 c = make_int4(0, 0, 0, 0);
+        if (b < nbPad) c = *reinterpret_cast<const int4*>(e.rowcnt + b);
+        const long long local = (long long)c.x + c.y + c.z + c.w;
+        long long incl = local;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
-            long long t = __shfl_up_sync(0xffffffffu, inc2, o);
-            if (threadIdx.x >= o) inc2 += t;
+            const long long t = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o) incl += t;
         }
-        wsum[threadIdx.x] = inc2 - v;  // exclusive warp offsets
-        if (threadIdx.x == 31) {
-            st->nce_last = inc2;
-            st->nce_total += inc2;
-            st->steps_done += step_inc;
-            if (inc2 > cap) st->overflow = 1;
+        if (lane == 31) wsum[warp] = incl;
+        __syncthreads();
+        if (warp == 0) {
+            const long long v = wsum[lane];
+            long long inc2 = v;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const long long t = __shfl_up_sync(0xffffffffu, inc2, o);
+                if (lane >= o) inc2 += t;
+            }
+            wsum[lane] = inc2 - v;   // exclusive warp offsets
         }
+        __syncthreads();
+        const long long carry = carry_s;
+        long long run = carry + wsum[warp] + (incl - local);
+        if (b < nbPad) {
+            e.rowoff[b] = run; run += c.x;
+            e.rowoff[b + 1] = run; run += c.y;
+            e.rowoff[b + 2] = run; run += c.z;
+            e.rowoff[b + 3] = run; run += c.w;
+        }
+        __syncthreads();
+        if (tid == SCAN_THREADS - 1) carry_s = run;   // the last thread's running total is the block total
+        __syncthreads();
     }
-    __syncthreads();
-    long long run = wsum[threadIdx.x >> 5] + (incl - local);
-    for (int b = b0; b < b1; ++b) { rowoff[b] = run; run += rowcnt[b]; }
+    if (tid == 0) {
+        const long long total = carry_s;
+        st->nce_last = total;
+        st->nce_total += total;
+        st->steps_done += step_inc;
+        *e.ovf_now = total > cap ? 1 : 0;
+        if (total > cap) st->overflow = 1;
+    }
 }
 
-// ---- pass 2: one warp per non-empty row, ballot + prefix compaction into the row's slots ----
+// ---- place: hits -> sorted list (no overflow) ------------------------------------------------
+__global__ void __launch_bounds__(256) enc_scatter_kernel(EncBuf e, uint8_t* __restrict__ flag) {
+    if (*e.ovf_now) return;
+    const unsigned long long n = *e.nhit;
+    for (unsigned long long h = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x; h < n;
+         h += (unsigned long long)gridDim.x * blockDim.x) {
+        const int2 c = e.hits[h];
+        const int k = atomicAdd(&e.rowfill[c.x], 1);
+        e.tmpj[e.rowoff[c.x] + k] = c.y;
+        flag[c.x] = 1;
+        flag[c.y] = 1;
+    }
+}
+
+__global__ void __launch_bounds__(256) enc_rank_kernel(EncBuf e, int* __restrict__ pairs) {
+    if (*e.ovf_now) return;
+    const unsigned long long n = *e.nhit;
+    for (unsigned long long h = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x; h < n;
+         h += (unsigned long long)gridDim.x * blockDim.x) {
+        const int2 c = e.hits[h];
+        const long long off = e.rowoff[c.x];
+        const int cnt = e.rowcnt[c.x];
+        const int* seg = e.tmpj + off;
+        int rank = 0;
+        for (int k = 0; k < cnt; ++k) rank += (seg[k] < c.y) ? 1 : 0;   // the j's of a row are distinct
+        const long long pos = off + rank;
+        pairs[2 * pos] = c.x;
+        pairs[2 * pos + 1] = c.y;
+    }
+}
+
+// ---- overflow fallback: one warp per non-empty row, in-order ballot compaction ---------------
 struct EncWriteParams {
     EncState s;
-    const double4* box;
-    const int* rowcnt;
-    const long long* rowoff;
+    EncBuf e;
     int* pairs;
     long long cap;
     uint8_t* flag;
 };
 
 __global__ void __launch_bounds__(256) enc_write_kernel(EncWriteParams p) {
+    if (*p.e.ovf_now == 0) return;
     const int lane = threadIdx.x & 31;
     const int gw = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const int nw = (gridDim.x * blockDim.x) >> 5;
     for (int row = gw; row < p.s.nb; row += nw) {
-        const int cnt = p.rowcnt[row];
+        const int cnt = p.e.rowcnt[row];
         if (cnt == 0) continue;
-        const long long off = p.rowoff[row];
-        const double4 bi = p.box[row];
+        const long long off = p.e.rowoff[row];
+        const double4 bi = p.e.box[row];
         int written = 0;
         for (int j0 = (row + 1) & ~31; j0 < p.s.nb && written < cnt; j0 += 32) {
             const int j = j0 + lane;
             bool hit = false;
             if (j > row && j < p.s.nb) {
-                const double4 bj = p.box[j];
-                if (box_gate(bi, make_double2(bj.x, bj.y), make_double2(bj.z, bj.w))) hit = pair_hit(p.s, row, j);
+                if (gate_f64(bi, p.e.box[j])) hit = pair_hit(p.s, row, j);
             }
             const unsigned m = __ballot_sync(0xffffffffu, hit);
             if (hit) {

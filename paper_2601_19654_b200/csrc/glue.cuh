@@ -38,8 +38,7 @@ struct MidParams {
     const double *gm, *rcrit;
     const double* psum_in;  // partials of sum gm v before the drift
     double* psum_out;       // partials after the drift
-    double4* box;
-    int* rowcnt;
+    EncBuf enc;
     uint8_t* flag;
     DevStats* st;
     int nb, ld, nbPad, npsum;
@@ -52,6 +51,8 @@ __global__ void __launch_bounds__(ON_BLOCK) jump_drift_boxes_kernel(MidParams p)
     reduce_psum(p.psum_in, p.npsum, sh, P0, P1, P2);
     const int b = blockIdx.x * ON_BLOCK + threadIdx.x;
     double s0 = 0, s1 = 0, s2 = 0;
+    if (b == 0) *p.enc.nhit = 0ull;
+    if (b < p.nbPad) { p.enc.rowcnt[b] = 0; p.enc.rowfill[b] = 0; }
     if (b < p.nb) {
         const int ld = p.ld;
         double x = p.x[b] + p.hj_over_mu * P0, y = p.x[ld + b] + p.hj_over_mu * P1, z = p.x[2 * ld + b] + p.hj_over_mu * P2;
@@ -72,14 +73,14 @@ __global__ void __launch_bounds__(ON_BLOCK) jump_drift_boxes_kernel(MidParams p)
         bx.x = __dsub_rn(lo, rc); bx.y = __dadd_rn(hi, rc);
         box_1d(y0, y, vy0, vy, p.h, lo, hi);
         bx.z = __dsub_rn(lo, rc); bx.w = __dadd_rn(hi, rc);
-        p.box[b] = bx;
-        p.rowcnt[b] = 0;
+        p.enc.box[b] = bx;
+        p.enc.boxf[b] = box_f32(bx);
         p.flag[b] = 0;
         const double g = p.gm[b];
         s0 = g * vx; s1 = g * vy; s2 = g * vz;
     } else if (b < p.nbPad) {
-        const double inf = __longlong_as_double(0x7ff0000000000000LL);
-        p.box[b] = make_double4(inf, -inf, inf, -inf);
+        p.enc.box[b] = pad_box();
+        p.enc.boxf[b] = pad_boxf();
     }
     block_sum3<ON_BLOCK>(s0, s1, s2, sh);
     if (threadIdx.x == 0) { p.psum_out[3 * blockIdx.x] = s0; p.psum_out[3 * blockIdx.x + 1] = s1; p.psum_out[3 * blockIdx.x + 2] = s2; }

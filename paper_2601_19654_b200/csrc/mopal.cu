@@ -28,9 +28,7 @@ struct mo_ctx {
     // owned scratch
     double *gm = nullptr, *x0 = nullptr, *v0 = nullptr, *part = nullptr, *psumA = nullptr, *psumB = nullptr;
     unsigned char* tiles = nullptr;
-    double4* box = nullptr;
-    int* rowcnt = nullptr;
-    long long* rowoff = nullptr;
+    EncBuf enc = {};
     DevStats* dstats = nullptr;
     DevStats* hstats = nullptr;  // pinned
     double* probe = nullptr;
@@ -142,8 +140,10 @@ extern "C" void mo_destroy(mo_ctx* ctx) {
     if (ctx->cap_stream) cudaStreamDestroy(ctx->cap_stream);
     for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
     cudaFree(ctx->gm); cudaFree(ctx->x0); cudaFree(ctx->v0); cudaFree(ctx->part);
-    cudaFree(ctx->psumA); cudaFree(ctx->psumB); cudaFree(ctx->tiles); cudaFree(ctx->box);
-    cudaFree(ctx->rowcnt); cudaFree(ctx->rowoff); cudaFree(ctx->dstats); cudaFree(ctx->probe);
+    cudaFree(ctx->psumA); cudaFree(ctx->psumB); cudaFree(ctx->tiles);
+    cudaFree(ctx->enc.box); cudaFree(ctx->enc.boxf); cudaFree(ctx->enc.rowcnt); cudaFree(ctx->enc.rowfill);
+    cudaFree(ctx->enc.rowoff); cudaFree(ctx->enc.hits); cudaFree(ctx->enc.tmpj); cudaFree(ctx->enc.nhit);
+    cudaFree(ctx->enc.ovf_now); cudaFree(ctx->dstats); cudaFree(ctx->probe);
     if (ctx->hstats) cudaFreeHost(ctx->hstats);
     delete ctx;
 }
@@ -186,9 +186,15 @@ extern "C" mo_status mo_create(mo_ctx** out, int32_t nb, int32_t ld, double m_st
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->psumA, 3 * (size_t)ctx->npsum);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->psumB, 3 * (size_t)ctx->npsum);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->tiles, (size_t)ctx->nTiles * ACC_TILE_BYTES);
-    if (e == cudaSuccess) e = dalloc(ctx, &ctx->box, (size_t)ctx->nbPad);
-    if (e == cudaSuccess) e = dalloc(ctx, &ctx->rowcnt, (size_t)ctx->nbPad);
-    if (e == cudaSuccess) e = dalloc(ctx, &ctx->rowoff, (size_t)ctx->nbPad);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->enc.box, (size_t)ctx->nbPad);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->enc.boxf, (size_t)ctx->nbPad);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->enc.rowcnt, (size_t)ctx->nbPad);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->enc.rowfill, (size_t)ctx->nbPad);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->enc.rowoff, (size_t)ctx->nbPad);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->enc.hits, (size_t)cap);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->enc.tmpj, (size_t)cap);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->enc.nhit, 1);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->enc.ovf_now, 1);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->dstats, 1);
     if (e == cudaSuccess) e = cudaMallocHost(reinterpret_cast<void**>(&ctx->hstats), sizeof(DevStats));
     if (e != cudaSuccess) {
@@ -257,23 +263,29 @@ static EncState enc_state(const mo_ctx* ctx, const double* x0, const double* v0,
     return s;
 }
 
-// pass 1 + scan + pass 2 on boxes already in ctx->box (rowcnt and flag already zeroed)
+// find + scan + place (+ overflow fallback) on boxes already in ctx->enc (counters already zeroed)
 static mo_status enqueue_pairs(mo_ctx* ctx, const EncState& es, int step_inc) {
-    EncCountParams cp;
-    cp.s = es; cp.box = ctx->box; cp.rowcnt = ctx->rowcnt; cp.nTiles = ctx->nTiles; cp.tps = ctx->enc_tps;
-    enc_count_kernel<<<dim3(ctx->nTiles, ctx->enc_nsplit), CTA_THREADS, 0, ctx->stream>>>(cp);
+    EncFindParams fp;
+    fp.s = es; fp.e = ctx->enc; fp.cap = ctx->cap; fp.nTiles = ctx->nTiles; fp.tps = ctx->enc_tps;
+    enc_find_kernel<<<dim3(ctx->nTiles, ctx->enc_nsplit), CTA_THREADS, 0, ctx->stream>>>(fp);
     mo_status s = post_launch(ctx);
     if (s != MO_OK) return s;
-    enc_scan_kernel<<<1, SCAN_THREADS, 0, ctx->stream>>>(ctx->rowcnt, ctx->rowoff, ctx->nb, ctx->cap, step_inc, ctx->dstats);
+    enc_scan_kernel<<<1, SCAN_THREADS, 0, ctx->stream>>>(ctx->enc, ctx->nbPad, ctx->cap, step_inc, ctx->dstats);
+    s = post_launch(ctx);
+    if (s != MO_OK) return s;
+    const int pblocks = ctx->nsm * 2;
+    enc_scatter_kernel<<<pblocks, 256, 0, ctx->stream>>>(ctx->enc, ctx->flag);
+    s = post_launch(ctx);
+    if (s != MO_OK) return s;
+    enc_rank_kernel<<<pblocks, 256, 0, ctx->stream>>>(ctx->enc, ctx->pairs);
     s = post_launch(ctx);
     if (s != MO_OK) return s;
     EncWriteParams wp;
-    wp.s = es; wp.box = ctx->box; wp.rowcnt = ctx->rowcnt; wp.rowoff = ctx->rowoff;
-    wp.pairs = ctx->pairs; wp.cap = ctx->cap; wp.flag = ctx->flag;
+    wp.s = es; wp.e = ctx->enc; wp.pairs = ctx->pairs; wp.cap = ctx->cap; wp.flag = ctx->flag;
     int blocks = (ctx->nb + 7) / 8;
     const int maxb = ctx->nsm * 8;
     if (blocks > maxb) blocks = maxb;
-    enc_write_kernel<<<blocks, 256, 0, ctx->stream>>>(wp);
+    enc_write_kernel<<<blocks, 256, 0, ctx->stream>>>(wp);   // exits at once unless count > cap
     return post_launch(ctx);
 }
 
@@ -283,7 +295,7 @@ static mo_status enqueue_step(mo_ctx* ctx, double dt) {
     if (s != MO_OK) return s;
     MidParams mp;
     mp.x = ctx->x; mp.v = ctx->v; mp.x0 = ctx->x0; mp.v0 = ctx->v0; mp.gm = ctx->gm; mp.rcrit = ctx->rcrit;
-    mp.psum_in = ctx->psumA; mp.psum_out = ctx->psumB; mp.box = ctx->box; mp.rowcnt = ctx->rowcnt; mp.flag = ctx->flag;
+    mp.psum_in = ctx->psumA; mp.psum_out = ctx->psumB; mp.enc = ctx->enc; mp.flag = ctx->flag;
     mp.st = ctx->dstats; mp.nb = ctx->nb; mp.ld = ctx->ld; mp.nbPad = ctx->nbPad; mp.npsum = ctx->npsum;
     mp.hj_over_mu = 0.5 * dt / ctx->mu; mp.mu = ctx->mu; mp.h = dt;
     jump_drift_boxes_kernel<<<ctx->npsum, ON_BLOCK, 0, ctx->stream>>>(mp);
@@ -293,7 +305,7 @@ static mo_status enqueue_step(mo_ctx* ctx, double dt) {
     if (s != MO_OK) return s;
     return enqueue_accel(ctx, true, 0.5 * dt, true, 0.5 * dt);
 }
-static const int KERNELS_PER_STEP = 8;
+static const int KERNELS_PER_STEP = 10;
 
 static mo_status read_stats(mo_ctx* ctx, mo_stats* out, bool* overflow) {
     CK(cudaMemcpyAsync(ctx->hstats, ctx->dstats, sizeof(DevStats), cudaMemcpyDeviceToHost, ctx->stream));
@@ -376,7 +388,7 @@ extern "C" mo_status mo_encounters(mo_ctx* ctx, double dt, const double* x0, con
         return MO_EINVAL;
     }
     EncState es = enc_state(ctx, x0, v0, dt);
-    boxes_kernel<<<(ctx->nbPad + ON_BLOCK - 1) / ON_BLOCK, ON_BLOCK, 0, ctx->stream>>>(es, ctx->box, ctx->nbPad, ctx->rowcnt, ctx->flag);
+    boxes_kernel<<<(ctx->nbPad + ON_BLOCK - 1) / ON_BLOCK, ON_BLOCK, 0, ctx->stream>>>(es, ctx->enc, ctx->nbPad, ctx->flag);
     mo_status s = post_launch(ctx);
     if (s != MO_OK) return s;
     s = enqueue_pairs(ctx, es, 0);

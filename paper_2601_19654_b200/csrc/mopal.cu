@@ -11,6 +11,7 @@
 
 #include "../../include/mopal.h"
 #include "glue.cuh"
+#include "pair_sym.cuh"
 
 using namespace mopal;
 
@@ -36,6 +37,14 @@ struct mo_ctx {
     // geometry
     int ipt = 1, unroll = 4, nIblk = 0, nsplit = 1, tps = 1, ctas_per_sm = 1, npsum = 0;
     int enc_tps = 1, enc_nsplit = 1;
+    // two-sided pair kernel (nb >= MO_SYM_MIN): work units and partial buffers
+    bool use_sym = false;
+    int sym_nI = 0, sym_ch = 1, sym_nunits = 0;
+    int4* sym_units = nullptr;
+    int* sym_ustart = nullptr;
+    double *sym_partI = nullptr, *sym_partJ = nullptr;
+    std::vector<int4> h_units;
+    std::vector<int> h_ustart;
     bool a_valid = false, snap_valid = false, debug = false, use_graph = true;
     long long launches = 0;
     cudaError_t last_err = cudaSuccess;
@@ -115,6 +124,33 @@ static void choose_geometry(mo_ctx* ctx) {
     if (forced > 0) bestS = forced < ctx->nTiles ? forced : ctx->nTiles;
     ctx->tps = (ctx->nTiles + bestS - 1) / bestS;
     ctx->nsplit = (ctx->nTiles + ctx->tps - 1) / ctx->tps;
+    // two-sided kernel for large nb: units = (row block, chunk of sym_ch j tiles from the diagonal on)
+    ctx->use_sym = env_int("MO_SYM", nb >= env_int("MO_SYM_MIN", 8192) ? 1 : 0) != 0;
+    if (ctx->use_sym) {
+        int occs = 1;
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occs, pair_sym_kernel, SYM_THREADS, 0);
+        if (occs < 1) occs = 1;
+        const long long sslots = (long long)ctx->nsm * occs;
+        ctx->sym_nI = (ctx->nbPad + SYM_R - 1) / SYM_R;
+        long long tot = 0;
+        for (int I = 0; I < ctx->sym_nI; ++I) tot += ctx->nTiles - I * SYM_TPB;
+        long long ch = (tot + 16 * sslots - 1) / (16 * sslots);   // about sixteen waves of units: short tail
+        if (ch < 1) ch = 1;
+        if (ch > 16) ch = 16;
+        ctx->sym_ch = env_int("MO_SYM_CH", (int)ch);
+        if (ctx->sym_ch < 1) ctx->sym_ch = 1;
+        ctx->h_units.clear(); ctx->h_ustart.clear();
+        for (int I = 0; I < ctx->sym_nI; ++I) {
+            ctx->h_ustart.push_back((int)ctx->h_units.size());
+            for (int t = I * SYM_TPB; t < ctx->nTiles; t += ctx->sym_ch) {
+                const int t1 = t + ctx->sym_ch < ctx->nTiles ? t + ctx->sym_ch : ctx->nTiles;
+                ctx->h_units.push_back(make_int4(I, t, t1, 0));
+            }
+        }
+        ctx->h_ustart.push_back((int)ctx->h_units.size());
+        ctx->sym_nunits = (int)ctx->h_units.size();
+        ctx->ipt = SYM_IPT; ctx->ctas_per_sm = occs; ctx->nsplit = 1;
+    }
     // encounter pass 1: row blocks x j-chunks, about 32 chunks
     ctx->enc_tps = ctx->nTiles / 32 > 1 ? ctx->nTiles / 32 : 1;
     ctx->enc_nsplit = (ctx->nTiles + ctx->enc_tps - 1) / ctx->enc_tps;
@@ -141,6 +177,7 @@ extern "C" void mo_destroy(mo_ctx* ctx) {
     for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
     cudaFree(ctx->gm); cudaFree(ctx->x0); cudaFree(ctx->v0); cudaFree(ctx->part);
     cudaFree(ctx->psumA); cudaFree(ctx->psumB); cudaFree(ctx->tiles);
+    cudaFree(ctx->sym_units); cudaFree(ctx->sym_ustart); cudaFree(ctx->sym_partI); cudaFree(ctx->sym_partJ);
     cudaFree(ctx->enc.box); cudaFree(ctx->enc.boxf); cudaFree(ctx->enc.rowcnt); cudaFree(ctx->enc.rowfill);
     cudaFree(ctx->enc.rowoff); cudaFree(ctx->enc.hits); cudaFree(ctx->enc.tmpj); cudaFree(ctx->enc.nhit);
     cudaFree(ctx->enc.ovf_now); cudaFree(ctx->dstats); cudaFree(ctx->probe);
@@ -182,7 +219,15 @@ extern "C" mo_status mo_create(mo_ctx** out, int32_t nb, int32_t ld, double m_st
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->gm, (size_t)nb);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->x0, pl);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->v0, pl);
-    if (e == cudaSuccess) e = dalloc(ctx, &ctx->part, pl * (size_t)ctx->nsplit);
+    if (e == cudaSuccess && !ctx->use_sym) e = dalloc(ctx, &ctx->part, pl * (size_t)ctx->nsplit);
+    if (ctx->use_sym) {
+        if (e == cudaSuccess) e = dalloc(ctx, &ctx->sym_units, (size_t)ctx->sym_nunits);
+        if (e == cudaSuccess) e = dalloc(ctx, &ctx->sym_ustart, ctx->h_ustart.size());
+        if (e == cudaSuccess) e = dalloc(ctx, &ctx->sym_partI, (size_t)ctx->sym_nunits * 3 * SYM_R);
+        if (e == cudaSuccess) e = dalloc(ctx, &ctx->sym_partJ, (size_t)symJ_off(ctx->sym_nI, ctx->nbPad));
+        if (e == cudaSuccess) e = cudaMemcpyAsync(ctx->sym_units, ctx->h_units.data(), ctx->h_units.size() * sizeof(int4), cudaMemcpyHostToDevice, ctx->stream);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(ctx->sym_ustart, ctx->h_ustart.data(), ctx->h_ustart.size() * sizeof(int), cudaMemcpyHostToDevice, ctx->stream);
+    }
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->psumA, 3 * (size_t)ctx->npsum);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->psumB, 3 * (size_t)ctx->npsum);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->tiles, (size_t)ctx->nTiles * ACC_TILE_BYTES);
@@ -231,25 +276,36 @@ static mo_status launch_pair(mo_ctx* ctx) {
         ctx->ev_used += 2;
         CK(cudaEventRecord(e0, ctx->stream));
     }
-    pick_pair_kernel(ctx->ipt, ctx->unroll)<<<grid, CTA_THREADS, 0, ctx->stream>>>(p);
+    if (ctx->use_sym) {
+        SymParams sp;
+        sp.tiles = ctx->tiles; sp.x = ctx->x; sp.gm = ctx->gm; sp.rcrit = ctx->rcrit; sp.units = ctx->sym_units;
+        sp.partI = ctx->sym_partI; sp.partJ = ctx->sym_partJ; sp.nb = ctx->nb; sp.ld = ctx->ld; sp.nbPad = ctx->nbPad;
+        pair_sym_kernel<<<ctx->sym_nunits, SYM_THREADS, 0, ctx->stream>>>(sp);
+    } else {
+        pick_pair_kernel(ctx->ipt, ctx->unroll)<<<grid, CTA_THREADS, 0, ctx->stream>>>(p);
+    }
     if (ctx->timing) CK(cudaEventRecord(e1, ctx->stream));
     return post_launch(ctx);
 }
 
 // a <- accel(x), optionally preceded by the jump (psumB) and followed by the kick
 static mo_status enqueue_accel(mo_ctx* ctx, bool jump, double hj, bool kick, double hk) {
-    if (jump)
-        pack_kernel<true><<<ctx->nTiles, TJ, 0, ctx->stream>>>(ctx->x, ctx->gm, ctx->rcrit, ctx->nb, ctx->ld, ctx->tiles,
-                                                                ctx->psumB, ctx->npsum, hj / ctx->mu);
-    else
-        pack_kernel<false><<<ctx->nTiles, TJ, 0, ctx->stream>>>(ctx->x, ctx->gm, ctx->rcrit, ctx->nb, ctx->ld, ctx->tiles,
-                                                                 nullptr, 0, 0.0);
+    const double hjm = jump ? hj / ctx->mu : 0.0;
+    const double* ps = jump ? ctx->psumB : nullptr;
+    const int nps = jump ? ctx->npsum : 0;
+    auto pk = jump ? (ctx->use_sym ? pack_kernel<true, true> : pack_kernel<true, false>)
+                   : (ctx->use_sym ? pack_kernel<false, true> : pack_kernel<false, false>);
+    pk<<<ctx->nTiles, TJ, 0, ctx->stream>>>(ctx->x, ctx->gm, ctx->rcrit, ctx->nb, ctx->ld, ctx->tiles, ps, nps, hjm);
     mo_status s = post_launch(ctx);
     if (s != MO_OK) return s;
     s = launch_pair(ctx);
     if (s != MO_OK) return s;
     const int nblk = (ctx->nb + ON_BLOCK - 1) / ON_BLOCK;
-    if (kick)
+    if (ctx->use_sym) {
+        auto rk = kick ? sym_reduce_kernel<true> : sym_reduce_kernel<false>;
+        rk<<<nblk, ON_BLOCK, 0, ctx->stream>>>(ctx->sym_partI, ctx->sym_partJ, ctx->sym_ustart, ctx->nb, ctx->ld, ctx->nbPad,
+                                               ctx->a, kick ? ctx->v : nullptr, kick ? hk : 0.0);
+    } else if (kick)
         accel_reduce_kernel<true><<<nblk, ON_BLOCK, 0, ctx->stream>>>(ctx->part, ctx->nsplit, ctx->nb, ctx->ld, ctx->a, ctx->v, hk);
     else
         accel_reduce_kernel<false><<<nblk, ON_BLOCK, 0, ctx->stream>>>(ctx->part, ctx->nsplit, ctx->nb, ctx->ld, ctx->a, nullptr, 0.0);
@@ -464,7 +520,8 @@ extern "C" mo_status mo_pair_geometry(const mo_ctx* ctx, int32_t* ipt, int32_t* 
     if (!ctx) return MO_EINVAL;
     if (ipt) *ipt = ctx->ipt;
     if (jsplit) *jsplit = ctx->nsplit;
-    if (ctas) *ctas = ctx->nIblk * ctx->nsplit;
+    if (ctas) *ctas = ctx->use_sym ? ctx->sym_nunits : ctx->nIblk * ctx->nsplit;
+    if (ctx->use_sym && jsplit) *jsplit = ctx->sym_ch;
     if (ctas_per_sm) *ctas_per_sm = ctx->ctas_per_sm;
     return MO_OK;
 }

@@ -200,7 +200,9 @@ __device__ __forceinline__ void reduce_psum(const double* __restrict__ psum, int
     __syncthreads();
 }
 
-template <bool JUMP>
+// SYM selects the tile layout: false = TJ records {x,y,z,gm} (pair_accel_kernel, broadcast reads),
+// true = SoA halves {x,y}[TJ] then {z,gm}[TJ] (pair_sym_kernel, lane-distinct reads).
+template <bool JUMP, bool SYM>
 __global__ void __launch_bounds__(TJ) pack_kernel(double* __restrict__ x, const double* __restrict__ gm,
                                                   const double* __restrict__ rcrit, int nb, int ld,
                                                   unsigned char* __restrict__ tiles,
@@ -231,8 +233,13 @@ __global__ void __launch_bounds__(TJ) pack_kernel(double* __restrict__ x, const 
         pb = make_double2(PAD_POS, 0.0);
     }
     unsigned char* tile = tiles + (size_t)blockIdx.x * ACC_TILE_BYTES;
-    double2* rec = reinterpret_cast<double2*>(tile) + 2 * threadIdx.x;
-    rec[0] = pa; rec[1] = pb;
+    if (SYM) {
+        double2* rec = reinterpret_cast<double2*>(tile);
+        rec[threadIdx.x] = pa; rec[TJ + threadIdx.x] = pb;
+    } else {
+        double2* rec = reinterpret_cast<double2*>(tile) + 2 * threadIdx.x;
+        rec[0] = pa; rec[1] = pb;
+    }
     ghi = __reduce_max_sync(0xffffffffu, ghi);
     if ((threadIdx.x & 31) == 0) sg[threadIdx.x >> 5] = ghi;
     __syncthreads();

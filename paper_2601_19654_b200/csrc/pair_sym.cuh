@@ -1,0 +1,249 @@
+// pair_sym.cuh - two-sided ("Newton III") form of the O(N^2) K(r)-weighted mutual-gravity
+// sum (force block LOOP 2):  a_i = sum_{j != i} gm_j K_ij (x_j - x_i) / r_ij^3.
+//
+// K_ij = K_ji (rc = max(rcrit_i, rcrit_j), reading A-3), so u_ij = K_ij / r_ij^3 is evaluated once
+// per UNORDERED pair and applied to both bodies:  a_i += gm_j u d,  a_j -= gm_i u d,  d = x_j - x_i.
+// FP64-pipe cost per unordered pair on the K = 1 path: 3 DADD (d), DMUL + 2 DFMA (s2), 4 DMUL +
+// 3 DFMA (u from the MUFU.RSQ64H seed, one third-order correction), 2 DMUL (gm_j u, gm_i u),
+// 6 DFMA (two accumulations) = 20, i.e. 10 per ordered pair against 16 for the one-sided kernel.
+//
+// Work unit = (row block I of SYM_R = 128*IPT bodies) x (a chunk of j tiles at or right of the
+// block's diagonal).  Each lane keeps IPT bodies i resident (position, gm, gate, accumulators).
+// A j tile is 4 groups of 32 bodies; a group ROTATES through the warp: at rotation s lane L works
+// on j = (L + s) mod 32, reading its record from the shared-memory tile (SoA halves {x,y}[128] and
+// {z,gm}[128]: 16-byte stride, conflict-free for lane-distinct addresses) and carrying the three
+// accumulators of that j in registers, handed to the neighbouring lane by SHFL after every
+// rotation (6 SHFL.32 per 80 FP64 instructions).  After 32 rotations every lane holds the partial
+// a_j of its home j = L.  The 4 warps' partials are combined through shared memory in warp order
+// and written to a triangular partial buffer partJ[I][c][j >= I*SYM_R]; the resident a_i go to
+// partI[unit][c][row].  sym_reduce_kernel adds, for each body, its row partials in unit order and
+// then its column partials in ascending I: a fixed tree that depends on nb only (reading A-8) -
+// no atomics, bit-reproducible.
+//
+// Diagonal tiles (j tile inside the row block) take each unordered pair once by masking j <= i.
+// Changeover / coincident pairs are caught by the same integer gate as in pair_accel.cuh and
+// recomputed exactly by slow_weight(gm = 1).
+#pragma once
+#include "common.cuh"
+#include "pair_accel.cuh"
+
+namespace mopal {
+
+constexpr int SYM_IPT = 4;
+constexpr int SYM_R = CONSUMER_THREADS * SYM_IPT;   // 512 rows per row block
+constexpr int SYM_TPB = SYM_R / TJ;                 // j tiles spanned by a row block (4)
+
+struct SymParams {
+    const unsigned char* tiles;  // nTiles * ACC_TILE_BYTES, SoA-halves layout (pack_kernel<.., true>)
+    const double* x;             // 3*ld
+    const double* gm;            // nb
+    const double* rcrit;         // nb
+    const int4* units;           // {I, t0, t1, unused}
+    double* partI;               // [nUnits][3][SYM_R]
+    double* partJ;               // triangular: block I at symJ_off(I), planes of (nbPad - I*SYM_R)
+    int nb, ld, nbPad;
+};
+
+__host__ __device__ inline long long symJ_off(int I, int nbPad) {
+    return 3LL * ((long long)I * nbPad - (long long)SYM_R * ((long long)I * (I - 1) / 2));
+}
+
+// one rotation: IPT pairs of this lane against body (pa, pb); returns updated travelling sums
+template <bool DIAG>
+__device__ __forceinline__ void sym_rotation(const double2 pa, const double2 pb, const int jglob,
+                                             const int (&ig)[SYM_IPT], const double (&xi)[SYM_IPT],
+                                             const double (&yi)[SYM_IPT], const double (&zi)[SYM_IPT],
+                                             const double (&mi)[SYM_IPT], const int (&g)[SYM_IPT],
+                                             double (&ax)[SYM_IPT], double (&ay)[SYM_IPT], double (&az)[SYM_IPT],
+                                             double& tx, double& ty, double& tz, const double* __restrict__ rcrit,
+                                             int nb) {
+    double dx[SYM_IPT], dy[SYM_IPT], dz[SYM_IPT], u[SYM_IPT];
+    bool any = false;
+#pragma unroll
+    for (int k = 0; k < SYM_IPT; ++k) {
+        dx[k] = pa.x - xi[k]; dy[k] = pa.y - yi[k]; dz[k] = pb.x - zi[k];
+        const double s2 = fma(dz[k], dz[k], fma(dy[k], dy[k], dx[k] * dx[k]));
+        const double y = rsqrt_seed(s2);
+        const double y2 = y * y;
+        const double e = fma(-s2, y2, 1.0);
+        const double u0 = y * y2;
+        const double t = e * fma(1.875, e, 1.5);
+        double uu = fma(u0, t, u0);
+        bool slow = __double2hiint(s2) <= g[k];
+        if (DIAG) {
+            const bool valid = jglob > ig[k];
+            uu = valid ? uu : 0.0;
+            slow = slow && valid;
+        }
+        u[k] = uu;
+        any |= slow;
+    }
+    if (any) {  // rare: changeover shell or coincident bodies
+#pragma unroll
+        for (int k = 0; k < SYM_IPT; ++k) {
+            const double s2 = fma(dz[k], dz[k], fma(dy[k], dy[k], dx[k] * dx[k]));
+            if (__double2hiint(s2) <= g[k] && (!DIAG || jglob > ig[k]))
+                u[k] = slow_weight(s2, 1.0, rcrit, ig[k], jglob, nb);
+        }
+    }
+#pragma unroll
+    for (int k = 0; k < SYM_IPT; ++k) {
+        const double wj = pb.y * u[k];
+        const double wi = mi[k] * u[k];
+        ax[k] = fma(wj, dx[k], ax[k]);
+        ay[k] = fma(wj, dy[k], ay[k]);
+        az[k] = fma(wj, dz[k], az[k]);
+        tx = fma(-wi, dx[k], tx);
+        ty = fma(-wi, dy[k], ty);
+        tz = fma(-wi, dz[k], tz);
+    }
+}
+
+template <bool DIAG>
+__device__ __forceinline__ void sym_tile(const unsigned char* tile, const int jbase, const int lane,
+                                         const int (&ig)[SYM_IPT], const double (&xi)[SYM_IPT],
+                                         const double (&yi)[SYM_IPT], const double (&zi)[SYM_IPT],
+                                         const double (&mi)[SYM_IPT], const int (&g)[SYM_IPT],
+                                         double (&ax)[SYM_IPT], double (&ay)[SYM_IPT], double (&az)[SYM_IPT],
+                                         double* __restrict__ sj, const double* __restrict__ rcrit, int nb) {
+    const double2* txy = reinterpret_cast<const double2*>(tile);
+    const double2* tzg = txy + TJ;
+    const unsigned full = 0xffffffffu;
+#pragma unroll 1
+    for (int grp = 0; grp < TJ / 32; ++grp) {
+        double tx = 0.0, ty = 0.0, tz = 0.0;
+#pragma unroll 1
+        for (int s = 0; s < 32; ++s) {
+            const int jl = grp * 32 + ((lane + s) & 31);
+            const double2 pa = txy[jl];
+            const double2 pb = tzg[jl];
+            sym_rotation<DIAG>(pa, pb, jbase + jl, ig, xi, yi, zi, mi, g, ax, ay, az, tx, ty, tz, rcrit, nb);
+            // hand the travelling sums of j = (lane+s) to the lane that works on that j next
+            tx = __shfl_sync(full, tx, lane + 1);
+            ty = __shfl_sync(full, ty, lane + 1);
+            tz = __shfl_sync(full, tz, lane + 1);
+        }
+        // after 32 rotations lane L holds the sums of its home j = grp*32 + L
+        sj[grp * 32 + lane] = tx;
+        sj[TJ + grp * 32 + lane] = ty;
+        sj[2 * TJ + grp * 32 + lane] = tz;
+    }
+}
+
+// No producer warp here: after the per-tile barrier every warp is done with the tile's slot, so
+// thread 0 refills it (TMA 1-D bulk copy, completion on the slot's mbarrier) - 128 threads x 168
+// registers lets 3 CTAs = 12 compute warps share an SM.
+constexpr int SYM_THREADS = CONSUMER_THREADS;
+
+__global__ void __launch_bounds__(SYM_THREADS, 3) pair_sym_kernel(SymParams p) {
+    __shared__ __align__(128) unsigned char s_tiles[STAGES * ACC_TILE_BYTES];
+    __shared__ __align__(16) double s_aj[2][SYM_THREADS / 32][3 * TJ];   // [parity][warp][c][j]
+    __shared__ __align__(8) uint64_t s_full[STAGES];
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int4 un = p.units[blockIdx.x];
+    const int I = un.x, t0 = un.y, nt = un.z - un.y;
+    const unsigned char* src = p.tiles + (size_t)t0 * ACC_TILE_BYTES;
+
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < STAGES; ++s) mbar_init(&s_full[s], 1);
+        mbar_fence_init();
+#pragma unroll
+        for (int s = 0; s < STAGES; ++s) {
+            if (s < nt) {
+                mbar_arrive_expect_tx(&s_full[s], ACC_TILE_BYTES);
+                tma_load_1d(s_tiles + s * ACC_TILE_BYTES, src + (size_t)s * ACC_TILE_BYTES, ACC_TILE_BYTES, &s_full[s]);
+            }
+        }
+    }
+    __syncthreads();
+
+    // ---- compute warps: resident bodies i = I*SYM_R + warp*32*IPT + k*32 + lane ----
+    const int ibase = I * SYM_R + warp * (32 * SYM_IPT) + lane;
+    double xi[SYM_IPT], yi[SYM_IPT], zi[SYM_IPT], mi[SYM_IPT], ax[SYM_IPT], ay[SYM_IPT], az[SYM_IPT];
+    int gi[SYM_IPT], ig[SYM_IPT];
+#pragma unroll
+    for (int k = 0; k < SYM_IPT; ++k) {
+        const int i = ibase + k * 32;
+        ig[k] = i;
+        if (i < p.nb) {
+            xi[k] = p.x[i]; yi[k] = p.x[p.ld + i]; zi[k] = p.x[2 * p.ld + i];
+            mi[k] = p.gm[i];
+            const double rc = p.rcrit[i];
+            gi[k] = __double2hiint(rc * rc);
+        } else {   // pad rows: far away and massless
+            xi[k] = yi[k] = zi[k] = -PAD_POS; mi[k] = 0.0; gi[k] = 0;
+        }
+        ax[k] = ay[k] = az[k] = 0.0;
+    }
+
+    const int jrow0 = I * SYM_R;                       // first column of partJ block I
+    const int jw = p.nbPad - jrow0;                    // its plane width
+    double* pj = p.partJ + symJ_off(I, p.nbPad);
+
+    for (int n = 0; n < nt; ++n) {
+        const int st = n % STAGES;
+        const int t = t0 + n;
+        mbar_wait(&s_full[st], (n / STAGES) & 1);
+        const unsigned char* tile = s_tiles + st * ACC_TILE_BYTES;
+        const int gt = *reinterpret_cast<const int*>(tile + TJ * 32);
+        int g[SYM_IPT];
+#pragma unroll
+        for (int k = 0; k < SYM_IPT; ++k) g[k] = max(gi[k], gt);
+        double* sj = s_aj[n & 1][warp];
+        if (t < (I + 1) * SYM_TPB)
+            sym_tile<true>(tile, t * TJ, lane, ig, xi, yi, zi, mi, g, ax, ay, az, sj, p.rcrit, p.nb);
+        else
+            sym_tile<false>(tile, t * TJ, lane, ig, xi, yi, zi, mi, g, ax, ay, az, sj, p.rcrit, p.nb);
+        // combine the 4 warps' column partials in warp order (double-buffered: one barrier per tile)
+        __syncthreads();
+        if (tid == 0 && n + STAGES < nt) {   // every warp has left slot st: refill it
+            mbar_arrive_expect_tx(&s_full[st], ACC_TILE_BYTES);
+            tma_load_1d(s_tiles + st * ACC_TILE_BYTES, src + (size_t)(n + STAGES) * ACC_TILE_BYTES, ACC_TILE_BYTES,
+                        &s_full[st]);
+        }
+        const int jc = t * TJ + tid - jrow0;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            double s = s_aj[n & 1][0][c * TJ + tid];
+#pragma unroll
+            for (int w = 1; w < SYM_THREADS / 32; ++w) s += s_aj[n & 1][w][c * TJ + tid];
+            pj[(size_t)c * jw + jc] = s;
+        }
+    }
+
+    double* pi = p.partI + (size_t)blockIdx.x * 3 * SYM_R;
+#pragma unroll
+    for (int k = 0; k < SYM_IPT; ++k) {
+        const int r = warp * (32 * SYM_IPT) + k * 32 + lane;
+        pi[r] = ax[k]; pi[SYM_R + r] = ay[k]; pi[2 * SYM_R + r] = az[k];
+    }
+}
+
+// a_b = (row partials of b's block, in unit order) + (column partials, ascending I); optionally
+// the closing half kick v += hk * a (Hamiltonian block LOOP 1).
+template <bool KICK>
+__global__ void __launch_bounds__(ON_BLOCK) sym_reduce_kernel(const double* __restrict__ partI,
+                                                               const double* __restrict__ partJ,
+                                                               const int* __restrict__ ustart, int nb, int ld,
+                                                               int nbPad, double* __restrict__ a,
+                                                               double* __restrict__ v, double hk) {
+    const int b = blockIdx.x * ON_BLOCK + threadIdx.x;
+    if (b >= nb) return;
+    const int Ib = b / SYM_R, r = b - Ib * SYM_R;
+    const int u0 = ustart[Ib], u1 = ustart[Ib + 1];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        double s = 0.0;
+        for (int u = u0; u < u1; ++u) s += partI[((size_t)u * 3 + c) * SYM_R + r];
+        for (int I = 0; I <= Ib; ++I) {
+            const int jw = nbPad - I * SYM_R;
+            s += partJ[symJ_off(I, nbPad) + (size_t)c * jw + (b - I * SYM_R)];
+        }
+        a[(size_t)c * ld + b] = s;
+        if (KICK) v[(size_t)c * ld + b] = fma(hk, s, v[(size_t)c * ld + b]);
+    }
+}
+
+}  // namespace mopal

@@ -96,6 +96,54 @@ def test_accel_ragged_sizes_and_changeover_shell(M, nb):
     m.close()
 
 
+@pytest.fixture
+def force_sym(monkeypatch):
+    """Select the two-sided pair kernel (pair_sym_kernel) whatever nb is; MO_SYM is read by mo_create."""
+    def _set(ch=None):
+        monkeypatch.setenv("MO_SYM", "1")
+        if ch is not None:
+            monkeypatch.setenv("MO_SYM_CH", str(ch))
+    return _set
+
+
+@pytest.mark.parametrize("nb,ch", [(1, 1), (2, 1), (33, 1), (129, 2), (511, 1), (512, 3), (513, 1), (1000, 2),
+                                   (1537, 1), (2500, 5)])
+def test_accel_sym_kernel_ragged_sizes_and_changeover_shell(M, force_sym, nb, ch):
+    # several row blocks (512 rows), diagonal and off-diagonal tiles, ragged tails, every chunking
+    force_sym(ch)
+    w = W.random_cluster(nb, 300 + nb, box=1.0, rc_frac=(0.0, 0.7)) if nb > 1 else W.random_cluster(1, 5)
+    if nb > 100:
+        w.x[:, 1] = w.x[:, 0] + np.array([0.03 * max(w.rcrit[0], w.rcrit[1]), 0.0, 0.0])
+        w.x[:, nb - 1] = w.x[:, 5]          # coincident bodies in different tiles contribute nothing
+    m = _mk(M, w)
+    assert m.pair_geometry()["ipt"] == 4    # the two-sided kernel really is the one running
+    m.accel()
+    a = m.get("a")
+    a_ref, S = oracle.accel(G * w.mass, w.x, w.rcrit)
+    assert np.all(np.isfinite(a))
+    _check_accel(a, a_ref, S, f"sym cluster{nb}")
+    m.accel()
+    assert np.array_equal(a, m.get("a"))    # fixed reduction tree: bit-reproducible
+    m.close()
+
+
+def test_accel_sym_kernel_disk_and_step(M, force_sym):
+    force_sym()
+    w = W.shrink(1, 3000)
+    m = _mk(M, w)
+    m.accel()
+    a_ref, S = oracle.accel(G * w.mass, w.x, w.rcrit)
+    _check_accel(m.get("a"), a_ref, S, "sym disk")
+    st = m.step(w.dt, 2)
+    x, v, acc = w.x, w.v, a_ref
+    for _ in range(2):
+        r = oracle.step(G * w.m_star, G * w.mass, w.rcrit, w.dt, x, v, acc)
+        x, v, acc = r["x"], r["v"], r["a"]
+    assert max(_rel_vec_err(m.get("x"), x).max(), _rel_vec_err(m.get("v"), v).max()) <= 3e-13
+    assert st.steps_done == 2
+    m.close()
+
+
 def test_accel_degenerate_cases(M):
     # coincident bodies contribute nothing; rcrit = 0 is Newtonian; rcrit huge gives exactly 0
     w = W.shrink(0, 300)

@@ -7,7 +7,16 @@
 //                      is <= max(rcrit_i, rcrit_j)^2.
 // The paper appends with an atomic capture in whatever order threads arrive
 // (PAPER.md:264-269).  Here the list is deterministic and sorted:
-//   find    thread-per-row i over TMA-staged tiles of j boxes.  The O(N^2/2) gate runs on
+//   sort    (performance only, never decides anything) bodies are binned on a 64 x 64 grid over
+//           the bounding square of the boxes' lower corners, in Morton order of the cell, by a
+//           counting sort (enc_key_kernel, enc_sortscatter_kernel); enc_tilebox_kernel takes the
+//           bounding box of every run of TJ = 128 sorted boxes.  A row tile then only visits
+//           the column tiles whose bounding box overlaps its own: the all-pairs gate of LOOP 3
+//           is evaluated on ~1e7..1e8 instead of N^2/2 pairs, and skipped pairs are exactly
+//           pairs the box gate rejects (the bounding boxes contain the boxes), so the flagged
+//           set is unchanged.  The order inside a cell depends on atomics; nothing downstream
+//           does (hits are ranked into sorted order).
+//   find    thread-per-row i over TMA-staged tiles of j boxes.  The gate runs on
 //           FP32 copies of the boxes rounded OUTWARD (lo down, hi up), so it can only pass
 //           more pairs than the FP64 gate, never fewer; it costs 1 LDS.128 + 4 FSETP per
 //           pair on the FP32/ALU pipes.  Survivors (~1e-5..1e-3 of the pairs) are compacted
@@ -142,37 +151,195 @@ struct EncBuf {
     int* tmpj;           // cap j's grouped by row, unsorted inside a row
     unsigned long long* nhit;  // hits appended this pass (may exceed cap)
     int* ovf_now;        // this pass found more pairs than cap
+    // spatial ordering of this pass (performance only)
+    float4* bpart;       // per block of the boxes kernel: {min lox, max lox, min loy, max loy}
+    int* cellcnt;        // ENC_NCELL bodies per grid cell
+    int* cellfill;       // ENC_NCELL placement cursors
+    int* key;            // nbPad cell of each body
+    int* perm;           // nbPad sorted position -> body
+    float4* sboxf;       // nbPad FP32 boxes in sorted order (pad records at the end)
+    float4* tbox;        // nTiles bounding box of each run of TJ sorted boxes
 };
+
+constexpr int ENC_GRID = 64;                       // cells per axis
+constexpr int ENC_NCELL = ENC_GRID * ENC_GRID;
+
+// block partial of the bounds of the boxes' lower corners (real bodies only) and reset of the
+// cell counters; called by every thread of a boxes kernel (blocks of ON_BLOCK threads)
+__device__ __forceinline__ void enc_bounds_partial(const EncBuf& e, bool real, const float4& bf, float4* sh4) {
+    const float inf = __int_as_float(0x7f800000);
+    float mnx = real ? bf.x : inf, mxx = real ? bf.x : -inf, mny = real ? bf.z : inf, mxy = real ? bf.z : -inf;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        mnx = fminf(mnx, __shfl_down_sync(0xffffffffu, mnx, o));
+        mxx = fmaxf(mxx, __shfl_down_sync(0xffffffffu, mxx, o));
+        mny = fminf(mny, __shfl_down_sync(0xffffffffu, mny, o));
+        mxy = fmaxf(mxy, __shfl_down_sync(0xffffffffu, mxy, o));
+    }
+    const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+    if (l == 0) sh4[w] = make_float4(mnx, mxx, mny, mxy);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        float4 r = sh4[0];
+#pragma unroll
+        for (int k = 1; k < ON_BLOCK / 32; ++k) {
+            r.x = fminf(r.x, sh4[k].x); r.y = fmaxf(r.y, sh4[k].y); r.z = fminf(r.z, sh4[k].z); r.w = fmaxf(r.w, sh4[k].w);
+        }
+        e.bpart[blockIdx.x] = r;
+    }
+    for (int c = blockIdx.x * ON_BLOCK + threadIdx.x; c < ENC_NCELL; c += gridDim.x * ON_BLOCK) {
+        e.cellcnt[c] = 0; e.cellfill[c] = 0;
+    }
+}
 
 // ---- O(N) kernel: boxes, and reset of the per-row counters and flags ------------------------
 __global__ void __launch_bounds__(ON_BLOCK) boxes_kernel(EncState s, EncBuf e, int nbPad, uint8_t* __restrict__ flag) {
+    __shared__ float4 sh4[ON_BLOCK / 32];
     const int b = blockIdx.x * ON_BLOCK + threadIdx.x;
     if (b == 0) *e.nhit = 0ull;
-    if (b >= nbPad) return;
-    double4 r;
-    if (b < s.nb) {
-        body_box(s.x0, s.v0, s.x1, s.v1, s.rcrit[b], s.ld, b, s.h, r);
-        flag[b] = 0;
-        e.boxf[b] = box_f32(r);
-    } else {
-        r = pad_box();
-        e.boxf[b] = pad_boxf();
+    float4 bf = pad_boxf();
+    if (b < nbPad) {
+        double4 r;
+        if (b < s.nb) {
+            body_box(s.x0, s.v0, s.x1, s.v1, s.rcrit[b], s.ld, b, s.h, r);
+            flag[b] = 0;
+            bf = box_f32(r);
+        } else {
+            r = pad_box();
+        }
+        e.boxf[b] = bf;
+        e.rowcnt[b] = 0;
+        e.rowfill[b] = 0;
+        e.box[b] = r;
     }
-    e.rowcnt[b] = 0;
-    e.rowfill[b] = 0;
-    e.box[b] = r;
+    enc_bounds_partial(e, b < s.nb, bf, sh4);
 }
 
-// ---- find: FP32 gate over all i<j, exact test on the warp-compacted survivors ----------------
+// ---- spatial ordering (performance only) ------------------------------------------------------
+__device__ __forceinline__ unsigned spread6(unsigned v) {   // abcdef -> 0a0b0c0d0e0f
+    v &= 0x3Fu;
+    v = (v | (v << 4)) & 0x30Fu;   // ab....cdef  -> 0b11_0000_1111
+    v = (v | (v << 2)) & 0x333u;   // 0b0011_0011_0011
+    v = (v | (v << 1)) & 0x555u;   // 0b0101_0101_0101
+    return v;
+}
+
+// cell of every body's lower box corner on the ENC_GRID^2 grid over the global bounds; histogram
+__global__ void __launch_bounds__(ON_BLOCK) enc_key_kernel(EncBuf e, int nb, int nbPad, int npart) {
+    __shared__ float4 sh4[ON_BLOCK / 32];
+    __shared__ float4 bounds;
+    const float inf = __int_as_float(0x7f800000);
+    float4 r = make_float4(inf, -inf, inf, -inf);
+    for (int k = threadIdx.x; k < npart; k += ON_BLOCK) {
+        const float4 q = e.bpart[k];
+        r.x = fminf(r.x, q.x); r.y = fmaxf(r.y, q.y); r.z = fminf(r.z, q.z); r.w = fmaxf(r.w, q.w);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        r.x = fminf(r.x, __shfl_down_sync(0xffffffffu, r.x, o));
+        r.y = fmaxf(r.y, __shfl_down_sync(0xffffffffu, r.y, o));
+        r.z = fminf(r.z, __shfl_down_sync(0xffffffffu, r.z, o));
+        r.w = fmaxf(r.w, __shfl_down_sync(0xffffffffu, r.w, o));
+    }
+    if ((threadIdx.x & 31) == 0) sh4[threadIdx.x >> 5] = r;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        float4 t = sh4[0];
+#pragma unroll
+        for (int k = 1; k < ON_BLOCK / 32; ++k) {
+            t.x = fminf(t.x, sh4[k].x); t.y = fmaxf(t.y, sh4[k].y); t.z = fminf(t.z, sh4[k].z); t.w = fmaxf(t.w, sh4[k].w);
+        }
+        bounds = t;
+    }
+    __syncthreads();
+    const int b = blockIdx.x * ON_BLOCK + threadIdx.x;
+    if (b >= nbPad) return;
+    int key = ENC_NCELL - 1;                 // pad records: last cell (they are placed after the bodies anyway)
+    if (b < nb) {
+        const float4 bf = e.boxf[b];
+        const float wx = bounds.y - bounds.x, wy = bounds.w - bounds.z;
+        const float sx = wx > 0.f ? (float)ENC_GRID / wx : 0.f, sy = wy > 0.f ? (float)ENC_GRID / wy : 0.f;
+        // NaN / inf coordinates fall into cell 0 or the last cell: any cell is a valid choice
+        int cx = (int)fminf(fmaxf((bf.x - bounds.x) * sx, 0.f), (float)(ENC_GRID - 1));
+        int cy = (int)fminf(fmaxf((bf.z - bounds.z) * sy, 0.f), (float)(ENC_GRID - 1));
+        cx = min(max(cx, 0), ENC_GRID - 1); cy = min(max(cy, 0), ENC_GRID - 1);
+        key = (int)(spread6((unsigned)cx) | (spread6((unsigned)cy) << 1));
+        atomicAdd(&e.cellcnt[key], 1);
+    }
+    e.key[b] = key;
+}
+
+// counting sort: every block prefix-sums the ENC_NCELL counters itself, then places its bodies
+__global__ void __launch_bounds__(ON_BLOCK) enc_sortscatter_kernel(EncBuf e, int nb, int nbPad) {
+    __shared__ int off[ENC_NCELL];
+    __shared__ int wtot[ON_BLOCK / 32];
+    constexpr int PER = ENC_NCELL / ON_BLOCK;   // 16 consecutive cells per thread
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    int c[PER], loc = 0;
+#pragma unroll
+    for (int k = 0; k < PER; ++k) { c[k] = e.cellcnt[tid * PER + k]; loc += c[k]; }
+    int incl = loc;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int t = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += t;
+    }
+    if (lane == 31) wtot[warp] = incl;
+    __syncthreads();
+    int wbase = 0;
+#pragma unroll
+    for (int k = 0; k < ON_BLOCK / 32; ++k) wbase += (k < warp) ? wtot[k] : 0;
+    int run = wbase + incl - loc;
+#pragma unroll
+    for (int k = 0; k < PER; ++k) { off[tid * PER + k] = run; run += c[k]; }
+    __syncthreads();
+    const int b = blockIdx.x * ON_BLOCK + tid;
+    if (b >= nbPad) return;
+    if (b < nb) {
+        const int key = e.key[b];
+        const int pos = off[key] + atomicAdd(&e.cellfill[key], 1);
+        e.perm[pos] = b;
+        e.sboxf[pos] = e.boxf[b];
+    } else {                                    // pad records keep their place at the end
+        e.perm[b] = b;
+        e.sboxf[b] = pad_boxf();
+    }
+}
+
+// bounding box of each run of TJ sorted boxes
+__global__ void __launch_bounds__(TJ) enc_tilebox_kernel(EncBuf e) {
+    __shared__ float4 sh4[TJ / 32];
+    float4 r = e.sboxf[blockIdx.x * TJ + threadIdx.x];    // {lox, hix, loy, hiy}; pads are (+inf, -inf, ..)
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        r.x = fminf(r.x, __shfl_down_sync(0xffffffffu, r.x, o));
+        r.y = fmaxf(r.y, __shfl_down_sync(0xffffffffu, r.y, o));
+        r.z = fminf(r.z, __shfl_down_sync(0xffffffffu, r.z, o));
+        r.w = fmaxf(r.w, __shfl_down_sync(0xffffffffu, r.w, o));
+    }
+    if ((threadIdx.x & 31) == 0) sh4[threadIdx.x >> 5] = r;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        float4 t = sh4[0];
+#pragma unroll
+        for (int k = 1; k < TJ / 32; ++k) {
+            t.x = fminf(t.x, sh4[k].x); t.y = fmaxf(t.y, sh4[k].y); t.z = fminf(t.z, sh4[k].z); t.w = fmaxf(t.w, sh4[k].w);
+        }
+        e.tbox[blockIdx.x] = t;
+    }
+}
+
+// ---- find: FP32 gate over the pairs of overlapping tiles, exact test on the survivors ---------
 constexpr int BOXF_TILE_BYTES = TJ * 16;   // TJ x float4
 constexpr int ENC_BATCH = 8;               // j's gated between two survivor checks
 constexpr int ENC_QCAP = 64;               // per-warp survivor queue (a drain leaves < 32)
+constexpr int ENC_WIN = 1024;              // column tiles examined per window (candidate list in smem)
 
 struct EncFindParams {
     EncState s;
     EncBuf e;
     long long cap;
-    int nTiles, tps;
+    int nTiles;
 };
 
 __device__ __forceinline__ bool gate_f32(const float4& a, const float4& b) {
@@ -182,89 +349,104 @@ __device__ __forceinline__ bool gate_f64(const double4& a, const double4& b) {
     return (a.x <= b.y) & (b.x <= a.y) & (a.z <= b.w) & (b.z <= a.w);
 }
 
-// one survivor per lane: exact FP64 gate, exact pair test, record the hit
+// one survivor per lane (sorted positions c.x < c.y): exact FP64 gate, exact pair test, record the
+// hit as (i, j) = (smaller, larger) body index
 __device__ __forceinline__ void enc_exact(const EncFindParams& p, int2 c) {
-    const double4 bi = p.e.box[c.x], bj = p.e.box[c.y];
+    const int ba = p.e.perm[c.x], bb = p.e.perm[c.y];
+    const int i = min(ba, bb), j = max(ba, bb);
+    const double4 bi = p.e.box[i], bj = p.e.box[j];
     if (!gate_f64(bi, bj)) return;
-    if (!pair_hit(p.s, c.x, c.y)) return;
-    atomicAdd(&p.e.rowcnt[c.x], 1);
+    if (!pair_hit(p.s, i, j)) return;
+    atomicAdd(&p.e.rowcnt[i], 1);
     const unsigned long long pos = atomicAdd(p.e.nhit, 1ull);
-    if ((long long)pos < p.cap) p.e.hits[pos] = c;
+    if ((long long)pos < p.cap) p.e.hits[pos] = make_int2(i, j);
 }
 
+// CTA rb owns the rb-th run of TJ sorted boxes (one per compute thread) and visits the column
+// tiles t >= rb whose bounding box overlaps its own; a fifth warp streams those tiles (TMA).
 __global__ void __launch_bounds__(CTA_THREADS) enc_find_kernel(EncFindParams p) {
     __shared__ __align__(128) unsigned char s_tiles[STAGES * BOXF_TILE_BYTES];
     __shared__ __align__(8) uint64_t s_full[STAGES];
     __shared__ __align__(8) uint64_t s_empty[STAGES];
     __shared__ int2 s_q[CONSUMER_THREADS / 32][ENC_QCAP];
+    __shared__ int s_list[ENC_WIN];
+    __shared__ int s_n;
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    // rows of this CTA are [rb*TJ, rb*TJ+TJ): only tiles >= rb hold any j > i
     const int rb = blockIdx.x;
-    const int t0 = max(blockIdx.y * p.tps, rb);
-    const int t1 = min((blockIdx.y + 1) * p.tps, p.nTiles);
-    const int nt = t1 - t0;
-    if (nt <= 0) return;
+    const float4 own = p.e.tbox[rb];
 
     if (tid == 0) {
 #pragma unroll
         for (int s = 0; s < STAGES; ++s) { mbar_init(&s_full[s], 1); mbar_init(&s_empty[s], CONSUMER_THREADS / 32); }
         mbar_fence_init();
     }
-    __syncthreads();
-
-    if (warp == CONSUMER_THREADS / 32) {  // ---- TMA producer warp ----
-        if (lane == 0) {
-            const unsigned char* src = reinterpret_cast<const unsigned char*>(p.e.boxf) + (size_t)t0 * BOXF_TILE_BYTES;
-            for (int n = 0; n < nt; ++n) {
-                const int st = n % STAGES;
-                mbar_wait(&s_empty[st], ((n / STAGES) & 1) ^ 1);
-                mbar_arrive_expect_tx(&s_full[st], BOXF_TILE_BYTES);
-                tma_load_1d(s_tiles + st * BOXF_TILE_BYTES, src + (size_t)n * BOXF_TILE_BYTES, BOXF_TILE_BYTES, &s_full[st]);
-            }
-        }
-        return;
-    }
-
     const unsigned full = 0xffffffffu, lt = (1u << lane) - 1u;
-    const int i = rb * TJ + tid;
-    const float4 bi = p.e.boxf[i];            // pad rows (i >= nb) hold the never-overlapping box
-    int2* q = s_q[warp];
+    const bool producer = warp == CONSUMER_THREADS / 32;
+    const int si = rb * TJ + (producer ? 0 : tid);
+    const float4 bi = p.e.sboxf[si];          // pad records hold the never-overlapping box
+    int2* q = s_q[producer ? 0 : warp];
     int qhead = 0, qn = 0;                    // warp-uniform
+    int nglob = 0;                            // tiles streamed so far (ring position), CTA-uniform
 
-    for (int n = 0; n < nt; ++n) {
-        const int st = n % STAGES;
-        mbar_wait(&s_full[st], (n / STAGES) & 1);
-        const float4* tj = reinterpret_cast<const float4*>(s_tiles + st * BOXF_TILE_BYTES);
-        const int j0 = (t0 + n) * TJ;
-        const int jmin = (t0 + n == rb) ? tid + 1 : 0;    // diagonal tile: j > i only
-#pragma unroll 1
-        for (int jj = 0; jj < TJ; jj += ENC_BATCH) {
-            bool any = false;
-#pragma unroll
-            for (int u = 0; u < ENC_BATCH; ++u) any |= gate_f32(bi, tj[jj + u]);
-            if (__any_sync(full, any)) {                  // rare: some lane has a survivor in this batch
-#pragma unroll 1
-                for (int u = 0; u < ENC_BATCH; ++u) {
-                    const bool has = gate_f32(bi, tj[jj + u]) && (jj + u >= jmin);
-                    const unsigned bal = __ballot_sync(full, has);
-                    if (bal == 0u) continue;
-                    if (has) q[(qhead + qn + __popc(bal & lt)) & (ENC_QCAP - 1)] = make_int2(i, j0 + jj + u);
-                    qn += __popc(bal);
-                    __syncwarp();
-                    if (qn >= 32) {                       // a full warp of survivors
-                        enc_exact(p, q[(qhead + lane) & (ENC_QCAP - 1)]);
-                        qhead = (qhead + 32) & (ENC_QCAP - 1);
-                        qn -= 32;
-                        __syncwarp();
-                    }
+    for (int w0 = rb; w0 < p.nTiles; w0 += ENC_WIN) {
+        __syncthreads();                      // previous window fully consumed (and the barriers initialised)
+        if (tid == 0) s_n = 0;
+        __syncthreads();
+        for (int t = w0 + tid; t < min(w0 + ENC_WIN, p.nTiles); t += CTA_THREADS)
+            if (gate_f32(own, p.e.tbox[t])) s_list[atomicAdd(&s_n, 1)] = t;
+        __syncthreads();
+        const int nt = s_n;
+
+        if (producer) {  // ---- TMA producer warp ----
+            if (lane == 0) {
+                const unsigned char* src = reinterpret_cast<const unsigned char*>(p.e.sboxf);
+                for (int n = 0; n < nt; ++n) {
+                    const int g = nglob + n, st = g % STAGES;
+                    mbar_wait(&s_empty[st], ((g / STAGES) & 1) ^ 1);
+                    mbar_arrive_expect_tx(&s_full[st], BOXF_TILE_BYTES);
+                    tma_load_1d(s_tiles + st * BOXF_TILE_BYTES, src + (size_t)s_list[n] * BOXF_TILE_BYTES, BOXF_TILE_BYTES,
+                                &s_full[st]);
                 }
             }
+        } else {
+            for (int n = 0; n < nt; ++n) {
+                const int g = nglob + n, st = g % STAGES;
+                mbar_wait(&s_full[st], (g / STAGES) & 1);
+                const float4* tj = reinterpret_cast<const float4*>(s_tiles + st * BOXF_TILE_BYTES);
+                const int t = s_list[n];
+                const int j0 = t * TJ;
+                const int jmin = (t == rb) ? tid + 1 : 0;         // diagonal tile: sorted position j > i only
+#pragma unroll 1
+                for (int jj = 0; jj < TJ; jj += ENC_BATCH) {
+                    bool any = false;
+#pragma unroll
+                    for (int u = 0; u < ENC_BATCH; ++u) any |= gate_f32(bi, tj[jj + u]);
+                    if (__any_sync(full, any)) {                  // rare: some lane has a survivor in this batch
+#pragma unroll 1
+                        for (int u = 0; u < ENC_BATCH; ++u) {
+                            const bool has = gate_f32(bi, tj[jj + u]) && (jj + u >= jmin);
+                            const unsigned bal = __ballot_sync(full, has);
+                            if (bal == 0u) continue;
+                            if (has) q[(qhead + qn + __popc(bal & lt)) & (ENC_QCAP - 1)] = make_int2(si, j0 + jj + u);
+                            qn += __popc(bal);
+                            __syncwarp();
+                            if (qn >= 32) {                       // a full warp of survivors
+                                enc_exact(p, q[(qhead + lane) & (ENC_QCAP - 1)]);
+                                qhead = (qhead + 32) & (ENC_QCAP - 1);
+                                qn -= 32;
+                                __syncwarp();
+                            }
+                        }
+                    }
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&s_empty[st]);
+            }
         }
-        __syncwarp();
-        if (lane == 0) mbar_arrive(&s_empty[st]);
+        nglob += nt;
     }
-    if (lane < qn) enc_exact(p, q[(qhead + lane) & (ENC_QCAP - 1)]);
+    if (!producer && lane < qn) enc_exact(p, q[(qhead + lane) & (ENC_QCAP - 1)]);
 }
 
 // ---- scan: rowoff = exclusive prefix sum of rowcnt; count -> stats ----------------------------

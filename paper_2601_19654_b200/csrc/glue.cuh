@@ -47,10 +47,12 @@ struct MidParams {
 
 __global__ void __launch_bounds__(ON_BLOCK) jump_drift_boxes_kernel(MidParams p) {
     __shared__ double sh[ON_BLOCK / 32][3];
+    __shared__ float4 sh4[ON_BLOCK / 32];
     double P0, P1, P2;
     reduce_psum(p.psum_in, p.npsum, sh, P0, P1, P2);
     const int b = blockIdx.x * ON_BLOCK + threadIdx.x;
     double s0 = 0, s1 = 0, s2 = 0;
+    float4 bf = pad_boxf();
     if (b == 0) *p.enc.nhit = 0ull;
     if (b < p.nbPad) { p.enc.rowcnt[b] = 0; p.enc.rowfill[b] = 0; }
     if (b < p.nb) {
@@ -74,7 +76,8 @@ __global__ void __launch_bounds__(ON_BLOCK) jump_drift_boxes_kernel(MidParams p)
         box_1d(y0, y, vy0, vy, p.h, lo, hi);
         bx.z = __dsub_rn(lo, rc); bx.w = __dadd_rn(hi, rc);
         p.enc.box[b] = bx;
-        p.enc.boxf[b] = box_f32(bx);
+        bf = box_f32(bx);
+        p.enc.boxf[b] = bf;
         p.flag[b] = 0;
         const double g = p.gm[b];
         s0 = g * vx; s1 = g * vy; s2 = g * vz;
@@ -84,6 +87,7 @@ __global__ void __launch_bounds__(ON_BLOCK) jump_drift_boxes_kernel(MidParams p)
     }
     block_sum3<ON_BLOCK>(s0, s1, s2, sh);
     if (threadIdx.x == 0) { p.psum_out[3 * blockIdx.x] = s0; p.psum_out[3 * blockIdx.x + 1] = s1; p.psum_out[3 * blockIdx.x + 2] = s2; }
+    enc_bounds_partial(p.enc, b < p.nb, bf, sh4);
 }
 
 // stand-alone drift (mo_drift)

@@ -36,7 +36,6 @@ struct mo_ctx {
     size_t ws_bytes = 0;
     // geometry
     int ipt = 1, unroll = 4, nIblk = 0, nsplit = 1, tps = 1, ctas_per_sm = 1, npsum = 0;
-    int enc_tps = 1, enc_nsplit = 1;
     // two-sided pair kernel (nb >= MO_SYM_MIN): work units and partial buffers
     bool use_sym = false;
     int sym_nI = 0, sym_ch = 1, sym_nunits = 0;
@@ -151,9 +150,6 @@ static void choose_geometry(mo_ctx* ctx) {
         ctx->sym_nunits = (int)ctx->h_units.size();
         ctx->ipt = SYM_IPT; ctx->ctas_per_sm = occs; ctx->nsplit = 1;
     }
-    // encounter pass 1: row blocks x j-chunks, about 32 chunks
-    ctx->enc_tps = ctx->nTiles / 32 > 1 ? ctx->nTiles / 32 : 1;
-    ctx->enc_nsplit = (ctx->nTiles + ctx->enc_tps - 1) / ctx->enc_tps;
 }
 
 extern "C" const char* mo_strerror(mo_status s) {
@@ -181,6 +177,8 @@ extern "C" void mo_destroy(mo_ctx* ctx) {
     cudaFree(ctx->enc.box); cudaFree(ctx->enc.boxf); cudaFree(ctx->enc.rowcnt); cudaFree(ctx->enc.rowfill);
     cudaFree(ctx->enc.rowoff); cudaFree(ctx->enc.hits); cudaFree(ctx->enc.tmpj); cudaFree(ctx->enc.nhit);
     cudaFree(ctx->enc.ovf_now); cudaFree(ctx->dstats); cudaFree(ctx->probe);
+    cudaFree(ctx->enc.bpart); cudaFree(ctx->enc.cellcnt); cudaFree(ctx->enc.cellfill); cudaFree(ctx->enc.key);
+    cudaFree(ctx->enc.perm); cudaFree(ctx->enc.sboxf); cudaFree(ctx->enc.tbox);
     if (ctx->hstats) cudaFreeHost(ctx->hstats);
     delete ctx;
 }
@@ -240,6 +238,13 @@ extern "C" mo_status mo_create(mo_ctx** out, int32_t nb, int32_t ld, double m_st
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->enc.tmpj, (size_t)cap);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->enc.nhit, 1);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->enc.ovf_now, 1);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->enc.bpart, (size_t)ctx->npsum);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->enc.cellcnt, (size_t)ENC_NCELL);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->enc.cellfill, (size_t)ENC_NCELL);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->enc.key, (size_t)ctx->nbPad);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->enc.perm, (size_t)ctx->nbPad);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->enc.sboxf, (size_t)ctx->nbPad);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->enc.tbox, (size_t)ctx->nTiles);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->dstats, 1);
     if (e == cudaSuccess) e = cudaMallocHost(reinterpret_cast<void**>(&ctx->hstats), sizeof(DevStats));
     if (e != cudaSuccess) {
@@ -321,10 +326,20 @@ static EncState enc_state(const mo_ctx* ctx, const double* x0, const double* v0,
 
 // find + scan + place (+ overflow fallback) on boxes already in ctx->enc (counters already zeroed)
 static mo_status enqueue_pairs(mo_ctx* ctx, const EncState& es, int step_inc) {
-    EncFindParams fp;
-    fp.s = es; fp.e = ctx->enc; fp.cap = ctx->cap; fp.nTiles = ctx->nTiles; fp.tps = ctx->enc_tps;
-    enc_find_kernel<<<dim3(ctx->nTiles, ctx->enc_nsplit), CTA_THREADS, 0, ctx->stream>>>(fp);
+    // spatial ordering of this pass (performance only): cell keys, counting sort, tile bounding boxes
+    enc_key_kernel<<<ctx->npsum, ON_BLOCK, 0, ctx->stream>>>(ctx->enc, ctx->nb, ctx->nbPad, ctx->npsum);
     mo_status s = post_launch(ctx);
+    if (s != MO_OK) return s;
+    enc_sortscatter_kernel<<<ctx->npsum, ON_BLOCK, 0, ctx->stream>>>(ctx->enc, ctx->nb, ctx->nbPad);
+    s = post_launch(ctx);
+    if (s != MO_OK) return s;
+    enc_tilebox_kernel<<<ctx->nTiles, TJ, 0, ctx->stream>>>(ctx->enc);
+    s = post_launch(ctx);
+    if (s != MO_OK) return s;
+    EncFindParams fp;
+    fp.s = es; fp.e = ctx->enc; fp.cap = ctx->cap; fp.nTiles = ctx->nTiles;
+    enc_find_kernel<<<ctx->nTiles, CTA_THREADS, 0, ctx->stream>>>(fp);
+    s = post_launch(ctx);
     if (s != MO_OK) return s;
     enc_scan_kernel<<<1, SCAN_THREADS, 0, ctx->stream>>>(ctx->enc, ctx->nbPad, ctx->cap, step_inc, ctx->dstats);
     s = post_launch(ctx);
@@ -361,7 +376,7 @@ static mo_status enqueue_step(mo_ctx* ctx, double dt) {
     if (s != MO_OK) return s;
     return enqueue_accel(ctx, true, 0.5 * dt, true, 0.5 * dt);
 }
-static const int KERNELS_PER_STEP = 10;
+static const int KERNELS_PER_STEP = 13;
 
 static mo_status read_stats(mo_ctx* ctx, mo_stats* out, bool* overflow) {
     CK(cudaMemcpyAsync(ctx->hstats, ctx->dstats, sizeof(DevStats), cudaMemcpyDeviceToHost, ctx->stream));

@@ -29,9 +29,19 @@
 
 namespace mopal {
 
-constexpr int SYM_IPT = 4;
-constexpr int SYM_R = CONSUMER_THREADS * SYM_IPT;   // 512 rows per row block
-constexpr int SYM_TPB = SYM_R / TJ;                 // j tiles spanned by a row block (4)
+#ifndef SYM_IPT_N
+#define SYM_IPT_N 6
+#endif
+#ifndef SYM_MINB
+#define SYM_MINB 2
+#endif
+#ifndef SYM_STAGES_N
+#define SYM_STAGES_N 4
+#endif
+constexpr int SYM_IPT = SYM_IPT_N;
+constexpr int SYM_STAGES = SYM_STAGES_N;
+constexpr int SYM_R = CONSUMER_THREADS * SYM_IPT;   // rows per row block (768)
+constexpr int SYM_TPB = SYM_R / TJ;                 // j tiles spanned by a row block (6)
 
 struct SymParams {
     const unsigned char* tiles;  // nTiles * ACC_TILE_BYTES, SoA-halves layout (pack_kernel<.., true>)
@@ -48,47 +58,67 @@ __host__ __device__ inline long long symJ_off(int I, int nbPad) {
     return 3LL * ((long long)I * nbPad - (long long)SYM_R * ((long long)I * (I - 1) / 2));
 }
 
-// one rotation: IPT pairs of this lane against body (pa, pb); returns updated travelling sums
+constexpr int SYM_TILE_STRIDE = 4608;   // shared-memory stage stride: tile (4112 B) padded to 9 x 512 B
+
+__device__ __forceinline__ void lds_rec(double2& a, double2& b, uint32_t addr) {
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(a.x), "=d"(a.y) : "r"(addr));
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2+2048];" : "=d"(b.x), "=d"(b.y) : "r"(addr));
+}
+
+// next record of the 32-record (512 B, 512-B aligned) group, cyclically: VIADD + one LOP3
+__device__ __forceinline__ uint32_t next_rec(uint32_t addr) { return (addr & ~511u) | ((addr + 16u) & 511u); }
+
+// one rotation: IPT pairs of this lane against the body whose record is (ca, cb).  The record of
+// the NEXT rotation is loaded into (na, nb2) as soon as this rotation's separations are formed, so
+// the shared-memory latency is covered by the FP64 instructions that follow.  An FP64 warp
+// instruction holds the sub-partition's issue port for two cycles, so every other instruction
+// costs half a DFMA: the changeover gate is ONE compare per rotation (min over the IPT high words
+// of s2 against the largest gate of the lane's bodies and the tile), the j index is only formed on
+// the slow path, and the records ping-pong between two register sets (no copies).
 template <bool DIAG>
-__device__ __forceinline__ void sym_rotation(const double2 pa, const double2 pb, const int jglob,
-                                             const int (&ig)[SYM_IPT], const double (&xi)[SYM_IPT],
+__device__ __forceinline__ void sym_rotation(const double2 ca, const double2 cb, double2& na, double2& nb2,
+                                             const uint32_t caddr, const uint32_t naddr, const int jgrp,
+                                             const int ibase, const double (&xi)[SYM_IPT],
                                              const double (&yi)[SYM_IPT], const double (&zi)[SYM_IPT],
-                                             const double (&mi)[SYM_IPT], const int (&g)[SYM_IPT],
+                                             const double (&mi)[SYM_IPT], const int g,
                                              double (&ax)[SYM_IPT], double (&ay)[SYM_IPT], double (&az)[SYM_IPT],
                                              double& tx, double& ty, double& tz, const double* __restrict__ rcrit,
                                              int nb) {
     double dx[SYM_IPT], dy[SYM_IPT], dz[SYM_IPT], u[SYM_IPT];
-    bool any = false;
 #pragma unroll
     for (int k = 0; k < SYM_IPT; ++k) {
-        dx[k] = pa.x - xi[k]; dy[k] = pa.y - yi[k]; dz[k] = pb.x - zi[k];
+        dx[k] = ca.x - xi[k]; dy[k] = ca.y - yi[k]; dz[k] = cb.x - zi[k];
+    }
+    lds_rec(na, nb2, naddr);
+    int hmin = 0x7fffffff;
+#pragma unroll
+    for (int k = 0; k < SYM_IPT; ++k) {
         const double s2 = fma(dz[k], dz[k], fma(dy[k], dy[k], dx[k] * dx[k]));
         const double y = rsqrt_seed(s2);
         const double y2 = y * y;
         const double e = fma(-s2, y2, 1.0);
         const double u0 = y * y2;
         const double t = e * fma(1.875, e, 1.5);
-        double uu = fma(u0, t, u0);
-        bool slow = __double2hiint(s2) <= g[k];
-        if (DIAG) {
-            const bool valid = jglob > ig[k];
-            uu = valid ? uu : 0.0;
-            slow = slow && valid;
-        }
-        u[k] = uu;
-        any |= slow;
+        u[k] = fma(u0, t, u0);
+        hmin = min(hmin, __double2hiint(s2));
     }
-    if (any) {  // rare: changeover shell or coincident bodies
+    const int jglob_d = DIAG ? jgrp + (int)((caddr & 511u) >> 4) : 0;
+    if (DIAG) {   // each unordered pair of a diagonal tile once: j > i only
+#pragma unroll
+        for (int k = 0; k < SYM_IPT; ++k) u[k] = jglob_d > ibase + k * 32 ? u[k] : 0.0;
+    }
+    if (hmin <= g) {  // rare: a pair that may be inside a changeover shell, or coincident bodies
+        const int jglob = jgrp + (int)((caddr & 511u) >> 4);
 #pragma unroll
         for (int k = 0; k < SYM_IPT; ++k) {
-            const double s2 = fma(dz[k], dz[k], fma(dy[k], dy[k], dx[k] * dx[k]));
-            if (__double2hiint(s2) <= g[k] && (!DIAG || jglob > ig[k]))
-                u[k] = slow_weight(s2, 1.0, rcrit, ig[k], jglob, nb);
+            const double q2 = fma(dz[k], dz[k], fma(dy[k], dy[k], dx[k] * dx[k]));
+            if (__double2hiint(q2) <= g && (!DIAG || jglob > ibase + k * 32))
+                u[k] = slow_weight(q2, 1.0, rcrit, ibase + k * 32, jglob, nb);
         }
     }
 #pragma unroll
     for (int k = 0; k < SYM_IPT; ++k) {
-        const double wj = pb.y * u[k];
+        const double wj = cb.y * u[k];
         const double wi = mi[k] * u[k];
         ax[k] = fma(wj, dx[k], ax[k]);
         ay[k] = fma(wj, dy[k], ay[k]);
@@ -99,26 +129,35 @@ __device__ __forceinline__ void sym_rotation(const double2 pa, const double2 pb,
     }
 }
 
+// tile_sa: shared-space address of the tile (512-B aligned); records {x,y}[TJ] then {z,gm}[TJ]
 template <bool DIAG>
-__device__ __forceinline__ void sym_tile(const unsigned char* tile, const int jbase, const int lane,
-                                         const int (&ig)[SYM_IPT], const double (&xi)[SYM_IPT],
-                                         const double (&yi)[SYM_IPT], const double (&zi)[SYM_IPT],
-                                         const double (&mi)[SYM_IPT], const int (&g)[SYM_IPT],
-                                         double (&ax)[SYM_IPT], double (&ay)[SYM_IPT], double (&az)[SYM_IPT],
-                                         double* __restrict__ sj, const double* __restrict__ rcrit, int nb) {
-    const double2* txy = reinterpret_cast<const double2*>(tile);
-    const double2* tzg = txy + TJ;
+__device__ __forceinline__ void sym_tile(const uint32_t tile_sa, const int jbase, const int lane, const int ibase,
+                                         const double (&xi)[SYM_IPT], const double (&yi)[SYM_IPT],
+                                         const double (&zi)[SYM_IPT], const double (&mi)[SYM_IPT],
+                                         const int g, double (&ax)[SYM_IPT], double (&ay)[SYM_IPT],
+                                         double (&az)[SYM_IPT], double* __restrict__ sj,
+                                         const double* __restrict__ rcrit, int nb) {
     const unsigned full = 0xffffffffu;
 #pragma unroll 1
     for (int grp = 0; grp < TJ / 32; ++grp) {
+        // this lane walks the group's 32 records cyclically, starting at its home record
+        uint32_t a0 = tile_sa + grp * 512 + lane * 16;
+        const int jgrp = jbase + grp * 32;
         double tx = 0.0, ty = 0.0, tz = 0.0;
+        double2 pa, pb, qa, qb;
+        lds_rec(pa, pb, a0);
 #pragma unroll 1
-        for (int s = 0; s < 32; ++s) {
-            const int jl = grp * 32 + ((lane + s) & 31);
-            const double2 pa = txy[jl];
-            const double2 pb = tzg[jl];
-            sym_rotation<DIAG>(pa, pb, jbase + jl, ig, xi, yi, zi, mi, g, ax, ay, az, tx, ty, tz, rcrit, nb);
+        for (int s = 0; s < 32; s += 2) {
+            const uint32_t a1 = next_rec(a0);
+            sym_rotation<DIAG>(pa, pb, qa, qb, a0, a1, jgrp, ibase, xi, yi, zi, mi, g, ax, ay, az, tx, ty, tz, rcrit,
+                               nb);
             // hand the travelling sums of j = (lane+s) to the lane that works on that j next
+            tx = __shfl_sync(full, tx, lane + 1);
+            ty = __shfl_sync(full, ty, lane + 1);
+            tz = __shfl_sync(full, tz, lane + 1);
+            a0 = next_rec(a1);                             // s = 30 wraps to the home record (unused load)
+            sym_rotation<DIAG>(qa, qb, pa, pb, a1, a0, jgrp, ibase, xi, yi, zi, mi, g, ax, ay, az, tx, ty, tz, rcrit,
+                               nb);
             tx = __shfl_sync(full, tx, lane + 1);
             ty = __shfl_sync(full, ty, lane + 1);
             tz = __shfl_sync(full, tz, lane + 1);
@@ -135,10 +174,10 @@ __device__ __forceinline__ void sym_tile(const unsigned char* tile, const int jb
 // registers lets 3 CTAs = 12 compute warps share an SM.
 constexpr int SYM_THREADS = CONSUMER_THREADS;
 
-__global__ void __launch_bounds__(SYM_THREADS, 3) pair_sym_kernel(SymParams p) {
-    __shared__ __align__(128) unsigned char s_tiles[STAGES * ACC_TILE_BYTES];
+__global__ void __launch_bounds__(SYM_THREADS, SYM_MINB) pair_sym_kernel(SymParams p) {
+    __shared__ __align__(512) unsigned char s_tiles[SYM_STAGES * SYM_TILE_STRIDE];
     __shared__ __align__(16) double s_aj[2][SYM_THREADS / 32][3 * TJ];   // [parity][warp][c][j]
-    __shared__ __align__(8) uint64_t s_full[STAGES];
+    __shared__ __align__(8) uint64_t s_full[SYM_STAGES];
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int4 un = p.units[blockIdx.x];
@@ -147,13 +186,13 @@ __global__ void __launch_bounds__(SYM_THREADS, 3) pair_sym_kernel(SymParams p) {
 
     if (tid == 0) {
 #pragma unroll
-        for (int s = 0; s < STAGES; ++s) mbar_init(&s_full[s], 1);
+        for (int s = 0; s < SYM_STAGES; ++s) mbar_init(&s_full[s], 1);
         mbar_fence_init();
 #pragma unroll
-        for (int s = 0; s < STAGES; ++s) {
+        for (int s = 0; s < SYM_STAGES; ++s) {
             if (s < nt) {
                 mbar_arrive_expect_tx(&s_full[s], ACC_TILE_BYTES);
-                tma_load_1d(s_tiles + s * ACC_TILE_BYTES, src + (size_t)s * ACC_TILE_BYTES, ACC_TILE_BYTES, &s_full[s]);
+                tma_load_1d(s_tiles + s * SYM_TILE_STRIDE, src + (size_t)s * ACC_TILE_BYTES, ACC_TILE_BYTES, &s_full[s]);
             }
         }
     }
@@ -162,18 +201,17 @@ __global__ void __launch_bounds__(SYM_THREADS, 3) pair_sym_kernel(SymParams p) {
     // ---- compute warps: resident bodies i = I*SYM_R + warp*32*IPT + k*32 + lane ----
     const int ibase = I * SYM_R + warp * (32 * SYM_IPT) + lane;
     double xi[SYM_IPT], yi[SYM_IPT], zi[SYM_IPT], mi[SYM_IPT], ax[SYM_IPT], ay[SYM_IPT], az[SYM_IPT];
-    int gi[SYM_IPT], ig[SYM_IPT];
+    int gi = 0;   // largest changeover gate of this lane's bodies: high word of rcrit_i^2
 #pragma unroll
     for (int k = 0; k < SYM_IPT; ++k) {
         const int i = ibase + k * 32;
-        ig[k] = i;
         if (i < p.nb) {
             xi[k] = p.x[i]; yi[k] = p.x[p.ld + i]; zi[k] = p.x[2 * p.ld + i];
             mi[k] = p.gm[i];
             const double rc = p.rcrit[i];
-            gi[k] = __double2hiint(rc * rc);
+            gi = max(gi, __double2hiint(rc * rc));
         } else {   // pad rows: far away and massless
-            xi[k] = yi[k] = zi[k] = -PAD_POS; mi[k] = 0.0; gi[k] = 0;
+            xi[k] = yi[k] = zi[k] = -PAD_POS; mi[k] = 0.0;
         }
         ax[k] = ay[k] = az[k] = 0.0;
     }
@@ -183,24 +221,23 @@ __global__ void __launch_bounds__(SYM_THREADS, 3) pair_sym_kernel(SymParams p) {
     double* pj = p.partJ + symJ_off(I, p.nbPad);
 
     for (int n = 0; n < nt; ++n) {
-        const int st = n % STAGES;
+        const int st = n % SYM_STAGES;
         const int t = t0 + n;
-        mbar_wait(&s_full[st], (n / STAGES) & 1);
-        const unsigned char* tile = s_tiles + st * ACC_TILE_BYTES;
+        mbar_wait(&s_full[st], (n / SYM_STAGES) & 1);
+        const unsigned char* tile = s_tiles + st * SYM_TILE_STRIDE;
+        const uint32_t tile_sa = smem_u32(tile);
         const int gt = *reinterpret_cast<const int*>(tile + TJ * 32);
-        int g[SYM_IPT];
-#pragma unroll
-        for (int k = 0; k < SYM_IPT; ++k) g[k] = max(gi[k], gt);
+        const int g = max(gi, gt);
         double* sj = s_aj[n & 1][warp];
         if (t < (I + 1) * SYM_TPB)
-            sym_tile<true>(tile, t * TJ, lane, ig, xi, yi, zi, mi, g, ax, ay, az, sj, p.rcrit, p.nb);
+            sym_tile<true>(tile_sa, t * TJ, lane, ibase, xi, yi, zi, mi, g, ax, ay, az, sj, p.rcrit, p.nb);
         else
-            sym_tile<false>(tile, t * TJ, lane, ig, xi, yi, zi, mi, g, ax, ay, az, sj, p.rcrit, p.nb);
+            sym_tile<false>(tile_sa, t * TJ, lane, ibase, xi, yi, zi, mi, g, ax, ay, az, sj, p.rcrit, p.nb);
         // combine the 4 warps' column partials in warp order (double-buffered: one barrier per tile)
         __syncthreads();
-        if (tid == 0 && n + STAGES < nt) {   // every warp has left slot st: refill it
+        if (tid == 0 && n + SYM_STAGES < nt) {   // every warp has left slot st: refill it
             mbar_arrive_expect_tx(&s_full[st], ACC_TILE_BYTES);
-            tma_load_1d(s_tiles + st * ACC_TILE_BYTES, src + (size_t)(n + STAGES) * ACC_TILE_BYTES, ACC_TILE_BYTES,
+            tma_load_1d(s_tiles + st * SYM_TILE_STRIDE, src + (size_t)(n + SYM_STAGES) * ACC_TILE_BYTES, ACC_TILE_BYTES,
                         &s_full[st]);
         }
         const int jc = t * TJ + tid - jrow0;

@@ -106,17 +106,17 @@ def force_sym(monkeypatch):
     return _set
 
 
-@pytest.mark.parametrize("nb,ch", [(1, 1), (2, 1), (33, 1), (129, 2), (511, 1), (512, 3), (513, 1), (1000, 2),
+@pytest.mark.parametrize("nb,ch", [(1, 1), (2, 1), (33, 1), (129, 2), (511, 1), (767, 1), (768, 3), (769, 1), (1000, 2),
                                    (1537, 1), (2500, 5)])
 def test_accel_sym_kernel_ragged_sizes_and_changeover_shell(M, force_sym, nb, ch):
-    # several row blocks (512 rows), diagonal and off-diagonal tiles, ragged tails, every chunking
+    # several row blocks (768 rows), diagonal and off-diagonal tiles, ragged tails, every chunking
     force_sym(ch)
     w = W.random_cluster(nb, 300 + nb, box=1.0, rc_frac=(0.0, 0.7)) if nb > 1 else W.random_cluster(1, 5)
     if nb > 100:
         w.x[:, 1] = w.x[:, 0] + np.array([0.03 * max(w.rcrit[0], w.rcrit[1]), 0.0, 0.0])
         w.x[:, nb - 1] = w.x[:, 5]          # coincident bodies in different tiles contribute nothing
     m = _mk(M, w)
-    assert m.pair_geometry()["ipt"] == 4    # the two-sided kernel really is the one running
+    assert m.pair_geometry()["ipt"] == 6    # the two-sided kernel really is the one running
     m.accel()
     a = m.get("a")
     a_ref, S = oracle.accel(G * w.mass, w.x, w.rcrit)

@@ -159,6 +159,7 @@ struct EncBuf {
     int* perm;           // nbPad sorted position -> body
     float4* sboxf;       // nbPad FP32 boxes in sorted order (pad records at the end)
     float4* tbox;        // nTiles bounding box of each run of TJ sorted boxes
+    int* tilecnt;        // nTiles hits per run of TJ rows (body order), the scan's block bases
 };
 
 constexpr int ENC_GRID = 64;                       // cells per axis
@@ -166,7 +167,8 @@ constexpr int ENC_NCELL = ENC_GRID * ENC_GRID;
 
 // block partial of the bounds of the boxes' lower corners (real bodies only) and reset of the
 // cell counters; called by every thread of a boxes kernel (blocks of ON_BLOCK threads)
-__device__ __forceinline__ void enc_bounds_partial(const EncBuf& e, bool real, const float4& bf, float4* sh4) {
+__device__ __forceinline__ void enc_bounds_partial(const EncBuf& e, bool real, const float4& bf, float4* sh4,
+                                                   int nTiles) {
     const float inf = __int_as_float(0x7f800000);
     float mnx = real ? bf.x : inf, mxx = real ? bf.x : -inf, mny = real ? bf.z : inf, mxy = real ? bf.z : -inf;
 #pragma unroll
@@ -190,6 +192,7 @@ __device__ __forceinline__ void enc_bounds_partial(const EncBuf& e, bool real, c
     for (int c = blockIdx.x * ON_BLOCK + threadIdx.x; c < ENC_NCELL; c += gridDim.x * ON_BLOCK) {
         e.cellcnt[c] = 0; e.cellfill[c] = 0;
     }
+    for (int c = blockIdx.x * ON_BLOCK + threadIdx.x; c < nTiles; c += gridDim.x * ON_BLOCK) e.tilecnt[c] = 0;
 }
 
 // ---- O(N) kernel: boxes, and reset of the per-row counters and flags ------------------------
@@ -212,7 +215,7 @@ __global__ void __launch_bounds__(ON_BLOCK) boxes_kernel(EncState s, EncBuf e, i
         e.rowfill[b] = 0;
         e.box[b] = r;
     }
-    enc_bounds_partial(e, b < s.nb, bf, sh4);
+    enc_bounds_partial(e, b < s.nb, bf, sh4, nbPad / TJ);
 }
 
 // ---- spatial ordering (performance only) ------------------------------------------------------
@@ -358,12 +361,15 @@ __device__ __forceinline__ void enc_exact(const EncFindParams& p, int2 c) {
     if (!gate_f64(bi, bj)) return;
     if (!pair_hit(p.s, i, j)) return;
     atomicAdd(&p.e.rowcnt[i], 1);
+    atomicAdd(&p.e.tilecnt[i / TJ], 1);
     const unsigned long long pos = atomicAdd(p.e.nhit, 1ull);
     if ((long long)pos < p.cap) p.e.hits[pos] = make_int2(i, j);
 }
 
-// CTA rb owns the rb-th run of TJ sorted boxes (one per compute thread) and visits the column
-// tiles t >= rb whose bounding box overlaps its own; a fifth warp streams those tiles (TMA).
+// CTA (rb, y) owns the rb-th run of TJ sorted boxes (one per compute thread) and visits the column
+// tiles t >= rb with (t - rb) % gridDim.y == y whose bounding box overlaps its own (the split over y
+// spreads the rows of dense regions, which overlap many tiles, over several CTAs); a fifth warp
+// streams those tiles (TMA).
 __global__ void __launch_bounds__(CTA_THREADS) enc_find_kernel(EncFindParams p) {
     __shared__ __align__(128) unsigned char s_tiles[STAGES * BOXF_TILE_BYTES];
     __shared__ __align__(8) uint64_t s_full[STAGES];
@@ -389,12 +395,15 @@ __global__ void __launch_bounds__(CTA_THREADS) enc_find_kernel(EncFindParams p) 
     int qhead = 0, qn = 0;                    // warp-uniform
     int nglob = 0;                            // tiles streamed so far (ring position), CTA-uniform
 
-    for (int w0 = rb; w0 < p.nTiles; w0 += ENC_WIN) {
+    const int S = gridDim.y;
+    for (int w0 = rb + blockIdx.y; w0 < p.nTiles; w0 += ENC_WIN * S) {
         __syncthreads();                      // previous window fully consumed (and the barriers initialised)
         if (tid == 0) s_n = 0;
         __syncthreads();
-        for (int t = w0 + tid; t < min(w0 + ENC_WIN, p.nTiles); t += CTA_THREADS)
-            if (gate_f32(own, p.e.tbox[t])) s_list[atomicAdd(&s_n, 1)] = t;
+        for (int k = tid; k < ENC_WIN; k += CTA_THREADS) {
+            const int t = w0 + k * S;
+            if (t < p.nTiles && gate_f32(own, p.e.tbox[t])) s_list[atomicAdd(&s_n, 1)] = t;
+        }
         __syncthreads();
         const int nt = s_n;
 
@@ -457,53 +466,43 @@ struct DevStats {
     int pad;
 };
 
-constexpr int SCAN_THREADS = 1024;
-// one block; each round scans 4*SCAN_THREADS counters (int4 per thread, coalesced)
-__global__ void __launch_bounds__(SCAN_THREADS) enc_scan_kernel(EncBuf e, int nbPad, long long cap, int step_inc,
-                                                                DevStats* __restrict__ st) {
-    __shared__ long long wsum[SCAN_THREADS / 32];
-    __shared__ long long carry_s;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    if (tid == 0) carry_s = 0;
-    __syncthreads();
-    for (int base = 0; base < nbPad; base += 4 * SCAN_THREADS) {   // nbPad is a multiple of TJ
-        const int b = base + 4 * tid;
-        int4 c = make_int4(0, 0, 0, 0);
-        if (b < nbPad) c = *reinterpret_cast<const int4*>(e.rowcnt + b);
-        const long long local = (long long)c.x + c.y + c.z + c.w;
-        long long incl = local;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const long long t = __shfl_up_sync(0xffffffffu, incl, o);
-            if (lane >= o) incl += t;
-        }
-        if (lane == 31) wsum[warp] = incl;
-        __syncthreads();
-        if (warp == 0) {
-            const long long v = wsum[lane];
-            long long inc2 = v;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                const long long t = __shfl_up_sync(0xffffffffu, inc2, o);
-                if (lane >= o) inc2 += t;
-            }
-            wsum[lane] = inc2 - v;   // exclusive warp offsets
-        }
-        __syncthreads();
-        const long long carry = carry_s;
-        long long run = carry + wsum[warp] + (incl - local);
-        if (b < nbPad) {
-            e.rowoff[b] = run; run += c.x;
-            e.rowoff[b + 1] = run; run += c.y;
-            e.rowoff[b + 2] = run; run += c.z;
-            e.rowoff[b + 3] = run; run += c.w;
-        }
-        __syncthreads();
-        if (tid == SCAN_THREADS - 1) carry_s = run;   // the last thread's running total is the block total
-        __syncthreads();
+// one block per run of TJ rows: the block's base is the sum of the per-tile hit counts before it
+// (tilecnt, bumped next to rowcnt by the find pass), so every block scans only its own TJ counters
+__global__ void __launch_bounds__(TJ) enc_scan_kernel(EncBuf e, int nTiles, long long cap, int step_inc,
+                                                       DevStats* __restrict__ st) {
+    __shared__ long long wpre[TJ / 32], wtot[TJ / 32];
+    __shared__ int wrow[TJ / 32];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, blk = blockIdx.x;
+    long long pre = 0, tot = 0;
+    for (int k = tid; k < nTiles; k += TJ) {
+        const int c = e.tilecnt[k];
+        pre += (k < blk) ? c : 0;
+        tot += c;
     }
-    if (tid == 0) {
-        const long long total = carry_s;
+    const int c = e.rowcnt[blk * TJ + tid];
+    int incl = c;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int t = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += t;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        pre += __shfl_down_sync(0xffffffffu, pre, o);
+        tot += __shfl_down_sync(0xffffffffu, tot, o);
+    }
+    if (lane == 0) { wpre[warp] = pre; wtot[warp] = tot; }
+    if (lane == 31) wrow[warp] = incl;
+    __syncthreads();
+    long long base = 0, total = 0;
+    int wbase = 0;
+#pragma unroll
+    for (int k = 0; k < TJ / 32; ++k) {
+        base += wpre[k]; total += wtot[k];
+        wbase += (k < warp) ? wrow[k] : 0;
+    }
+    e.rowoff[blk * TJ + tid] = base + wbase + (incl - c);
+    if (blk == 0 && tid == 0) {
         st->nce_last = total;
         st->nce_total += total;
         st->steps_done += step_inc;

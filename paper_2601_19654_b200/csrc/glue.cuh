@@ -87,7 +87,7 @@ __global__ void __launch_bounds__(ON_BLOCK) jump_drift_boxes_kernel(MidParams p)
     }
     block_sum3<ON_BLOCK>(s0, s1, s2, sh);
     if (threadIdx.x == 0) { p.psum_out[3 * blockIdx.x] = s0; p.psum_out[3 * blockIdx.x + 1] = s1; p.psum_out[3 * blockIdx.x + 2] = s2; }
-    enc_bounds_partial(p.enc, b < p.nb, bf, sh4);
+    enc_bounds_partial(p.enc, b < p.nb, bf, sh4, p.nbPad / TJ);
 }
 
 // stand-alone drift (mo_drift)

@@ -37,6 +37,7 @@ struct mo_ctx {
     // geometry
     int ipt = 1, unroll = 4, nIblk = 0, nsplit = 1, tps = 1, ctas_per_sm = 1, npsum = 0;
     // two-sided pair kernel (nb >= MO_SYM_MIN): work units and partial buffers
+    int enc_split = 1;
     bool use_sym = false;
     int sym_nI = 0, sym_ch = 1, sym_nunits = 0;
     int4* sym_units = nullptr;
@@ -123,6 +124,10 @@ static void choose_geometry(mo_ctx* ctx) {
     if (forced > 0) bestS = forced < ctx->nTiles ? forced : ctx->nTiles;
     ctx->tps = (ctx->nTiles + bestS - 1) / bestS;
     ctx->nsplit = (ctx->nTiles + ctx->tps - 1) / ctx->tps;
+    // encounter find: column tiles of a row tile are dealt round-robin to enc_split CTAs
+    ctx->enc_split = env_int("MO_ENC_SPLIT", ctx->nTiles / 8);
+    if (ctx->enc_split < 1) ctx->enc_split = 1;
+    if (ctx->enc_split > 8) ctx->enc_split = 8;
     // two-sided kernel for large nb: units = (row block, chunk of sym_ch j tiles from the diagonal on)
     ctx->use_sym = env_int("MO_SYM", nb >= env_int("MO_SYM_MIN", 8192) ? 1 : 0) != 0;
     if (ctx->use_sym) {
@@ -178,7 +183,7 @@ extern "C" void mo_destroy(mo_ctx* ctx) {
     cudaFree(ctx->enc.rowoff); cudaFree(ctx->enc.hits); cudaFree(ctx->enc.tmpj); cudaFree(ctx->enc.nhit);
     cudaFree(ctx->enc.ovf_now); cudaFree(ctx->dstats); cudaFree(ctx->probe);
     cudaFree(ctx->enc.bpart); cudaFree(ctx->enc.cellcnt); cudaFree(ctx->enc.cellfill); cudaFree(ctx->enc.key);
-    cudaFree(ctx->enc.perm); cudaFree(ctx->enc.sboxf); cudaFree(ctx->enc.tbox);
+    cudaFree(ctx->enc.perm); cudaFree(ctx->enc.sboxf); cudaFree(ctx->enc.tbox); cudaFree(ctx->enc.tilecnt);
     if (ctx->hstats) cudaFreeHost(ctx->hstats);
     delete ctx;
 }
@@ -245,6 +250,7 @@ extern "C" mo_status mo_create(mo_ctx** out, int32_t nb, int32_t ld, double m_st
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->enc.perm, (size_t)ctx->nbPad);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->enc.sboxf, (size_t)ctx->nbPad);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->enc.tbox, (size_t)ctx->nTiles);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->enc.tilecnt, (size_t)ctx->nTiles);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->dstats, 1);
     if (e == cudaSuccess) e = cudaMallocHost(reinterpret_cast<void**>(&ctx->hstats), sizeof(DevStats));
     if (e != cudaSuccess) {
@@ -338,10 +344,10 @@ static mo_status enqueue_pairs(mo_ctx* ctx, const EncState& es, int step_inc) {
     if (s != MO_OK) return s;
     EncFindParams fp;
     fp.s = es; fp.e = ctx->enc; fp.cap = ctx->cap; fp.nTiles = ctx->nTiles;
-    enc_find_kernel<<<ctx->nTiles, CTA_THREADS, 0, ctx->stream>>>(fp);
+    enc_find_kernel<<<dim3(ctx->nTiles, ctx->enc_split), CTA_THREADS, 0, ctx->stream>>>(fp);
     s = post_launch(ctx);
     if (s != MO_OK) return s;
-    enc_scan_kernel<<<1, SCAN_THREADS, 0, ctx->stream>>>(ctx->enc, ctx->nbPad, ctx->cap, step_inc, ctx->dstats);
+    enc_scan_kernel<<<ctx->nTiles, TJ, 0, ctx->stream>>>(ctx->enc, ctx->nTiles, ctx->cap, step_inc, ctx->dstats);
     s = post_launch(ctx);
     if (s != MO_OK) return s;
     const int pblocks = ctx->nsm * 2;

@@ -38,9 +38,27 @@ METRIC = "fp64_pair_interactions_per_s"
 UNIT = "pairs/s"
 FLOP_PER_PAIR = 26.0          # SURVEY.md 8(d) / DESIGN.md: K = 1 path, per ordered pair
 FP64_LANES_PER_SM = 64        # DESIGN.md section "Rooflines": 148 SMs x 64 DFMA/clk x 2 x f
-# dram__bytes_read.sum + dram__bytes_write.sum of one pair_accel_kernel launch at config 3
-# from the ncu --set full capture summarised in profiles/ (None until captured)
-PAIR_KERNEL_DRAM_TRAFFIC_BYTES = None
+# executed FP64 flops per ORDERED pair of the two-sided kernel: 3 DADD + 6 DMUL + 11 DFMA = 31 flop per
+# unordered pair (pair_sym.cuh; the ncu dadd/dmul/dfma counters in profiles/ show the same 3 : 6 : 11 mix)
+EXECUTED_FLOP_PER_PAIR = 15.5
+# dram__bytes_read.sum + dram__bytes_write.sum of one pair_sym_kernel launch at config 3 from the
+# ncu --set full capture summarised in profiles/r1c_pair_sym_full.md (5.1 MB read + 91.1 MB written)
+PAIR_KERNEL_DRAM_TRAFFIC_BYTES = {3: 96.3e6}
+
+
+def reduce_max_over_ranks(values, dist=None, device="cpu"):
+    """MAX over ranks of a list of floats (timings): the job is as slow as its slowest rank."""
+    import torch
+    t = torch.tensor(list(values), dtype=torch.float64, device=device)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t.tolist()]
+
+
+def whole_job_value(world: int, units_per_rank_step: float, steps: int, total_ms_max: float) -> float:
+    """Replicas only: every rank runs the same independent workload, so the job's throughput is
+    world x units per rank over the slowest rank's time."""
+    return world * units_per_rank_step * steps / (total_ms_max * 1e-3)
 
 
 def _dist_env():
@@ -246,15 +264,13 @@ def run_ours(args):
     d2h = 2 * 3 * ld * 8 + 40 + d2h_pairs // Ke
 
     # ---- max over ranks --------------------------------------------------------------------
-    tt = torch.tensor([total_ms, t_e2e * 1e3, pair_ms], dtype=torch.float64, device=m.device)
-    if dist is not None:
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-    total_ms_max, e2e_ms_max, pair_ms_max = (float(t) for t in tt.tolist())
-    value = world * pairs * K / (total_ms_max * 1e-3)
-    e2e_value = world * pairs * Ke / (e2e_ms_max * 1e-3)
+    total_ms_max, e2e_ms_max, pair_ms_max = reduce_max_over_ranks([total_ms, t_e2e * 1e3, pair_ms], dist, m.device)
+    value = whole_job_value(world, pairs, K, total_ms_max)
+    e2e_value = whole_job_value(world, pairs, Ke, e2e_ms_max)
 
     if rank == 0:
         achieved = FLOP_PER_PAIR * pairs / (pair_ms_max * 1e-3) / 1e12
+        executed = EXECUTED_FLOP_PER_PAIR * pairs / (pair_ms_max * 1e-3) / 1e12
         nsm = torch.cuda.get_device_properties(dev).multi_processor_count
         sm_max = clocks.get("sm_max_mhz") or 1965.0
         nominal = nsm * FP64_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
@@ -268,8 +284,13 @@ def run_ours(args):
                        "pair_kernel_geometry": geo, "encounter_pairs_last_step": st1.nce_last},
             "pct_fp64_peak": {"of_measured_sustained": 100 * achieved / peak_sust, "of_measured_burst": 100 * achieved / peak_burst,
                               "of_nominal": 100 * achieved / nominal, "flop_per_pair": FLOP_PER_PAIR},
-            "roofline": {"bound": "alu", "kernel": "pair_accel_kernel", "achieved": achieved, "peak": peak_sust,
-                         "unit": "TFLOP/s", "frac": achieved / peak_sust, "traffic": PAIR_KERNEL_DRAM_TRAFFIC_BYTES,
+            "roofline": {"bound": "alu", "kernel": "pair_sym_kernel", "achieved": achieved, "peak": peak_sust,
+                         "unit": "TFLOP/s", "frac": achieved / peak_sust,
+                         "traffic": PAIR_KERNEL_DRAM_TRAFFIC_BYTES.get(args.config),
+                         "note": "achieved = 26 algorithmic flop per ORDERED pair (SURVEY.md 8(d)) / kernel time; the kernel "
+                                 "evaluates each unordered pair once (Newton III), so frac can exceed 1; achieved_executed = "
+                                 "the 15.5 flop per ordered pair it really issues (3 DADD + 6 DMUL + 11 DFMA per unordered pair)",
+                         "achieved_executed": executed, "frac_executed": executed / peak_sust,
                          "peak_source": "mo_probe_fp64_peak: register-resident DFMA loop on this GPU, 160 launches back to "
                                         "back (sustained); MEASURED_PEAKS.json has no FP64 figure",
                          "peak_burst": peak_burst, "peak_nominal": nominal, "kernel_ms": pair_ms_max, "kernel_launches_timed": n_pair,
@@ -293,6 +314,48 @@ def run_ours(args):
     return 0
 
 
+def run_drift_sweep(args):
+    """HBM roofline of the O(N) Kepler-drift kernel (north_star: 'achieved HBM GB/s for the drift kernel'):
+    mo_drift alone at the five configs' sizes, where the state lives in L2, and at nb = 2^24, where
+    the 96 B/body (x, v read and written) really come from HBM.  One JSON line."""
+    import torch
+    from paper_2601_19654_b200 import mopal as M
+    from paper_2601_19654_b200 import workloads as W
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except OSError:
+        pass
+    hbm = float(peaks.get("hbm_gbs", 6550.0))
+    out = []
+    base = W.make_config(2)
+    for nb in [255, 4095, 16383, 65535, 131071, 1 << 24]:
+        reps = int(np.ceil(nb / base.nb))
+        idx = np.arange(nb) % base.nb                     # tile the 16,383-body disk (orbits only matter here)
+        x, v = base.x[:, idx].copy(), base.v[:, idx].copy()
+        m = M.Mopal(np.full(nb, 1e-10), x, v, np.zeros(nb), m_star=base.m_star, G=base.G, cap=16)
+        n_it = 200 if nb < 1 << 20 else 20
+        for _ in range(3):
+            m.drift(base.dt)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(m.stream)
+        for _ in range(n_it):
+            m.drift(base.dt)
+        e1.record(m.stream); torch.cuda.synchronize()
+        us = e0.elapsed_time(e1) * 1e3 / n_it
+        st = m.stats()
+        out.append({"nb": nb, "us_per_launch": us, "GBps": 96.0 * nb / (us * 1e-6) / 1e9, "bodies_per_s": nb / (us * 1e-6),
+                    "drift_fail": st.drift_fail, "max_newton": st.max_newton})
+        m.close(); del m, reps
+        torch.cuda.empty_cache()
+    big = out[-1]
+    print(json.dumps({"metric": "drift_kernel_hbm", "kernel": "drift_kernel", "algorithmic_bytes_per_body": 96,
+                      "roofline": {"bound": "hbm", "achieved": big["GBps"], "peak": hbm, "unit": "GB/s", "frac": big["GBps"] / hbm,
+                                   "at_nb": big["nb"], "peak_source": "MEASURED_PEAKS.json hbm_gbs" if peaks else "fallback 6550"},
+                      "sweep": out}), flush=True)
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -302,7 +365,10 @@ def main():
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json config index (3 = N=65,536 headline)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of CPU work for the cpu_baseline sample")
+    ap.add_argument("--drift-sweep", action="store_true", help="time mo_drift alone against the HBM roofline and exit")
     args = ap.parse_args()
+    if args.drift_sweep:
+        return run_drift_sweep(args)
     if args.impl == "reference":
         return run_reference(args)
     return run_ours(args)

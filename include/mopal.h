@@ -128,7 +128,8 @@ mo_status mo_invalidate_accel(mo_ctx *ctx);
 mo_status mo_get_stats(mo_ctx *ctx, mo_stats *stats_host);
 /* Number of libmopal kernels launched on behalf of this context so far. */
 int64_t mo_launch_count(const mo_ctx *ctx);
-/* Bytes of device scratch the context owns. */
+/* Bytes of device scratch the context owns so far.  The partial-sum buffers of the pair kernel
+ * are allocated by the first mo_accel / mo_step (which may therefore return MO_ENOMEM). */
 int64_t mo_workspace_bytes(const mo_ctx *ctx);
 
 /* Host-buffer variant of the step (the paper's per-step data region):

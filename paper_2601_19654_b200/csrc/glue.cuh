@@ -91,7 +91,7 @@ __global__ void __launch_bounds__(ON_BLOCK) jump_drift_boxes_kernel(MidParams p)
 }
 
 // stand-alone drift (mo_drift)
-__global__ void __launch_bounds__(ON_BLOCK) drift_kernel(double* __restrict__ xx, double* __restrict__ vv, int nb, int ld,
+__global__ void __launch_bounds__(ON_BLOCK, 4) drift_kernel(double* __restrict__ xx, double* __restrict__ vv, int nb, int ld,
                                                           double mu, double dt, DevStats* __restrict__ st) {
     const int b = blockIdx.x * ON_BLOCK + threadIdx.x;
     if (b >= nb) return;

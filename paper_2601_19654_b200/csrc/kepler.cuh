@@ -58,44 +58,92 @@ __device__ __forceinline__ GF gfuncs(double X, double beta) {
 
 constexpr int DRIFT_MAX_NEWTON = 12;
 
+// 1/sqrt(a) to ~1e-19 relative before rounding: MUFU.RSQ64H seed + one third-order correction
+__device__ __forceinline__ double rsqrt_full(double a) {
+    const double y = rsqrt_seed(a);
+    const double e = fma(-a, y * y, 1.0);
+    return fma(y * e, fma(0.375, e, 0.5), y);
+}
+// 1/a to ~1 ulp: MUFU.RCP64H seed + two Newton steps (no IEEE division sequence)
+__device__ __forceinline__ double rcp_fast(double a) {
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(a));
+    double e = fma(-a, y, 1.0);
+    y = fma(y, e, y);
+    e = fma(-a, y, 1.0);
+    return fma(y, e, y);
+}
+
 // returns 0 ok / 1 failed (state untouched); *iters = Newton iterations used
+//
+// Cost matters here: at ~500 FP64 instructions per body the kernel is FP64-issue bound, not HBM
+// bound (96 B per body).  So: the start value is the third-order series inverse of Kepler's equation
+// in X (exact for circular orbits, ~1e-6 relative for the disks' e ~ 0.02), a Newton step is
+// accepted as final as soon as the leading-order error estimate of the NEXT iterate,
+// |r'/(2r)| dX^2, is below 2e-16 |X| (normally the first step), and the G functions at the final X
+// come from their Taylor expansion about the last evaluation point (dG3 = G2, dG2 = G1, dG1 = G0,
+// dG0 = -beta G1; third order, error ~ dX^4) instead of another series evaluation.
 __device__ __forceinline__ int drift_body(double mu, double dt_full, double& x, double& y, double& z, double& vx,
                                           double& vy, double& vz, int* iters) {
-    const double r0 = sqrt(fma(z, z, fma(y, y, x * x)));
+    const double r2 = fma(z, z, fma(y, y, x * x));
     *iters = 0;
-    if (!(r0 > 0.0)) return 1;
+    if (!(r2 > 0.0) || !isfinite(r2)) return 1;
+    const double ir0 = rsqrt_full(r2);
+    const double r0 = r2 * ir0;
     const double v2 = fma(vz, vz, fma(vy, vy, vx * vx));
     const double eta0 = fma(z, vz, fma(y, vy, x * vx));
-    const double beta = 2.0 * mu / r0 - v2;
+    const double beta = fma(2.0 * mu, ir0, -v2);
+    const double kappa = fma(-beta, r0, mu);          // mu - beta r0 = d^2 r / dX^2 at X = 0
     // A bound orbit returns to the same state after T = 2 pi mu / beta^(3/2): drop whole
     // periods first.  Otherwise z = beta X^2 grows like (2 pi dt/T)^2, each argument
     // quartering of stumpff() doubles the phase error and dt - mu G3 cancels ~dt/T digits.
     double dt = dt_full;
-    if (beta > 0.0) {
+    if (beta > 0.0 && dt_full * dt_full * beta * beta * beta > 39.47841760435743 * mu * mu) {   // |dt| > T
         const double T = 6.283185307179586 * mu / (beta * sqrt(beta));
-        if (fabs(dt_full) > T) dt = fma(-rint(dt_full / T), T, dt_full);
+        dt = fma(-rint(dt_full / T), T, dt_full);
     }
-    double X = dt / r0;
+    // dt = r0 X + eta0 X^2/2 + kappa X^3/6 + ...  inverted to third order in tau = dt / r0
+    const double tau = dt * ir0;
+    const double b1 = -0.5 * eta0 * ir0;
+    const double c1 = fma(0.5 * eta0 * ir0, eta0, kappa * (-1.0 / 6.0)) * ir0;
+    double X = tau * fma(tau, fma(tau, c1, b1), 1.0);
+    if (!isfinite(X) || fabs(tau * fma(tau, c1, b1)) > 0.5) X = tau;   // series useless (large step): plain first order
     bool conv = false;
     int it = 0;
+    GF g;
+    double r = 0.0;
     for (; it < DRIFT_MAX_NEWTON; ++it) {
-        const GF g = gfuncs(X, beta);
+        g = gfuncs(X, beta);
         const double F = fma(r0, g.G1, fma(eta0, g.G2, mu * g.G3)) - dt;
-        const double r = fma(r0, g.G0, fma(eta0, g.G1, mu * g.G2));
+        r = fma(r0, g.G0, fma(eta0, g.G1, mu * g.G2));
         if (!(r > 0.0) || !isfinite(F)) break;
-        const double dX = -F / r;
-        X += dX;
-        // quadratic convergence: a step below 1e-9 |X| leaves an error far below 1 ulp
-        if (fabs(dX) <= 1e-9 * fabs(X) || dX == 0.0) { conv = true; ++it; break; }
+        const double ir = rcp_fast(r);
+        const double dX = -F * ir;
+        const double Xn = X + dX;
+        const double rp = fma(eta0, g.G0, kappa * g.G1);          // dr/dX
+        // error of Xn to leading order: |r'/(2r)| dX^2; trust the estimate only for small steps
+        if ((fabs(rp * ir) * dX * dX <= 4.0e-16 * fabs(Xn) && fabs(dX) <= 1e-3 * fabs(Xn)) || dX == 0.0) {
+            // G_n(X + dX) by Taylor expansion about X
+            const double h = 0.5 * dX, t3 = dX * (1.0 / 3.0);
+            const double G3 = fma(dX, fma(h, fma(t3, g.G0, g.G1), g.G2), g.G3);
+            const double G2 = fma(dX, fma(h, fma(-t3 * beta, g.G1, g.G0), g.G1), g.G2);
+            const double G1 = fma(dX, fma(-h * beta, fma(t3, g.G0, g.G1), g.G0), g.G1);
+            const double G0 = fma(-dX * beta, fma(h, fma(-t3 * beta, g.G1, g.G0), g.G1), g.G0);
+            g.G0 = G0; g.G1 = G1; g.G2 = G2; g.G3 = G3;
+            X = Xn;
+            conv = true; ++it;
+            break;
+        }
+        X = Xn;
     }
     *iters = it;
     if (!conv) {  // bisection on a bracket grown from 0 (F(0) = -dt, F monotone)
         const double sgn = dt >= 0.0 ? 1.0 : -1.0;
-        double a = 0.0, b = sgn * fabs(dt / r0);
+        double a = 0.0, b = sgn * fabs(dt * ir0);
         bool ok = false;
         for (int k = 0; k < 128; ++k) {
-            const GF g = gfuncs(b, beta);
-            const double F = fma(r0, g.G1, fma(eta0, g.G2, mu * g.G3)) - dt;
+            const GF q = gfuncs(b, beta);
+            const double F = fma(r0, q.G1, fma(eta0, q.G2, mu * q.G3)) - dt;
             if (!isfinite(F)) return 1;
             if (F * sgn >= 0.0) { ok = true; break; }
             a = b; b *= 2.0;
@@ -103,20 +151,22 @@ __device__ __forceinline__ int drift_body(double mu, double dt_full, double& x, 
         if (!ok) return 1;
         for (int k = 0; k < 128; ++k) {
             const double m = 0.5 * (a + b);
-            const GF g = gfuncs(m, beta);
-            const double F = fma(r0, g.G1, fma(eta0, g.G2, mu * g.G3)) - dt;
+            const GF q = gfuncs(m, beta);
+            const double F = fma(r0, q.G1, fma(eta0, q.G2, mu * q.G3)) - dt;
             if (F * sgn >= 0.0) b = m; else a = m;
             if (fabs(b - a) <= 4.4e-16 * fabs(b)) break;
         }
         X = 0.5 * (a + b);
+        g = gfuncs(X, beta);
     }
-    const GF g = gfuncs(X, beta);
-    const double r = fma(r0, g.G0, fma(eta0, g.G1, mu * g.G2));
+    r = fma(r0, g.G0, fma(eta0, g.G1, mu * g.G2));
     if (!(r > 0.0)) return 1;
-    const double fm1 = -mu * g.G2 / r0;
-    const double gg = dt - mu * g.G3;
-    const double fd = -mu * g.G1 / (r0 * r);
-    const double gdm1 = -mu * g.G2 / r;
+    const double ir = rcp_fast(r);
+    const double mG2 = -mu * g.G2;
+    const double fm1 = mG2 * ir0;
+    const double gg = fma(-mu, g.G3, dt);
+    const double fd = -mu * g.G1 * ir0 * ir;
+    const double gdm1 = mG2 * ir;
     const double nx = x + fma(fm1, x, gg * vx);
     const double ny = y + fma(fm1, y, gg * vy);
     const double nz = z + fma(fm1, z, gg * vz);

@@ -45,6 +45,7 @@ struct mo_ctx {
     double *sym_partI = nullptr, *sym_partJ = nullptr;
     std::vector<int4> h_units;
     std::vector<int> h_ustart;
+    bool pair_ready = false;
     bool a_valid = false, snap_valid = false, debug = false, use_graph = true;
     long long launches = 0;
     cudaError_t last_err = cudaSuccess;
@@ -222,15 +223,6 @@ extern "C" mo_status mo_create(mo_ctx** out, int32_t nb, int32_t ld, double m_st
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->gm, (size_t)nb);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->x0, pl);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->v0, pl);
-    if (e == cudaSuccess && !ctx->use_sym) e = dalloc(ctx, &ctx->part, pl * (size_t)ctx->nsplit);
-    if (ctx->use_sym) {
-        if (e == cudaSuccess) e = dalloc(ctx, &ctx->sym_units, (size_t)ctx->sym_nunits);
-        if (e == cudaSuccess) e = dalloc(ctx, &ctx->sym_ustart, ctx->h_ustart.size());
-        if (e == cudaSuccess) e = dalloc(ctx, &ctx->sym_partI, (size_t)ctx->sym_nunits * 3 * SYM_R);
-        if (e == cudaSuccess) e = dalloc(ctx, &ctx->sym_partJ, (size_t)symJ_off(ctx->sym_nI, ctx->nbPad));
-        if (e == cudaSuccess) e = cudaMemcpyAsync(ctx->sym_units, ctx->h_units.data(), ctx->h_units.size() * sizeof(int4), cudaMemcpyHostToDevice, ctx->stream);
-        if (e == cudaSuccess) e = cudaMemcpyAsync(ctx->sym_ustart, ctx->h_ustart.data(), ctx->h_ustart.size() * sizeof(int), cudaMemcpyHostToDevice, ctx->stream);
-    }
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->psumA, 3 * (size_t)ctx->npsum);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->psumB, 3 * (size_t)ctx->npsum);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->tiles, (size_t)ctx->nTiles * ACC_TILE_BYTES);
@@ -271,6 +263,31 @@ extern "C" mo_status mo_create(mo_ctx** out, int32_t nb, int32_t ld, double m_st
 }
 
 // ---- stage launchers -------------------------------------------------------------------------
+// partial-sum buffers of the pair kernels: allocated at the first mo_accel / mo_step, so that a context
+// used only for mo_drift / mo_encounters (e.g. a bandwidth sweep at 2^24 bodies) does not pay for them
+static mo_status ensure_pair_scratch(mo_ctx* ctx) {
+    if (ctx->pair_ready) return MO_OK;
+    cudaError_t e = cudaSuccess;
+    const size_t pl = 3 * (size_t)ctx->ld;
+    if (!ctx->use_sym) e = dalloc(ctx, &ctx->part, pl * (size_t)ctx->nsplit);
+    if (ctx->use_sym) {
+        if (e == cudaSuccess) e = dalloc(ctx, &ctx->sym_units, (size_t)ctx->sym_nunits);
+        if (e == cudaSuccess) e = dalloc(ctx, &ctx->sym_ustart, ctx->h_ustart.size());
+        if (e == cudaSuccess) e = dalloc(ctx, &ctx->sym_partI, (size_t)ctx->sym_nunits * 3 * SYM_R);
+        if (e == cudaSuccess) e = dalloc(ctx, &ctx->sym_partJ, (size_t)symJ_off(ctx->sym_nI, ctx->nbPad));
+        if (e == cudaSuccess) e = cudaMemcpyAsync(ctx->sym_units, ctx->h_units.data(), ctx->h_units.size() * sizeof(int4), cudaMemcpyHostToDevice, ctx->stream);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(ctx->sym_ustart, ctx->h_ustart.data(), ctx->h_ustart.size() * sizeof(int), cudaMemcpyHostToDevice, ctx->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);   // pageable source vectors
+    }
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        ctx->last_err = e;
+        return e == cudaErrorMemoryAllocation ? MO_ENOMEM : MO_ECUDA;
+    }
+    ctx->pair_ready = true;
+    return MO_OK;
+}
+
 static mo_status launch_pair(mo_ctx* ctx) {
     AccelParams p;
     p.tiles = ctx->tiles; p.x = ctx->x; p.rcrit = ctx->rcrit; p.part = ctx->part;
@@ -412,7 +429,9 @@ static mo_status status_from_stats(mo_ctx* ctx, mo_stats* out) {
 // ---- public entry points ---------------------------------------------------------------------
 extern "C" mo_status mo_accel(mo_ctx* ctx) {
     if (!ctx) return MO_EINVAL;
-    mo_status s = enqueue_accel(ctx, false, 0.0, false, 0.0);
+    mo_status s = ensure_pair_scratch(ctx);
+    if (s != MO_OK) return s;
+    s = enqueue_accel(ctx, false, 0.0, false, 0.0);
     if (s == MO_OK) ctx->a_valid = true;
     return s;
 }
@@ -482,7 +501,8 @@ extern "C" mo_status mo_encounters(mo_ctx* ctx, double dt, const double* x0, con
 
 extern "C" mo_status mo_step(mo_ctx* ctx, double dt, int32_t nsteps, mo_stats* stats_host) {
     if (!ctx || !isfinite(dt) || dt == 0.0 || nsteps < 0) return MO_EINVAL;
-    mo_status s = MO_OK;
+    mo_status s = ensure_pair_scratch(ctx);   // before any capture: allocation cannot be recorded
+    if (s != MO_OK) return s;
     if (!ctx->a_valid && nsteps > 0) {
         s = mo_accel(ctx);
         if (s != MO_OK) return s;

@@ -13,7 +13,7 @@
 // on j = (L + s) mod 32, reading its record from the shared-memory tile (SoA halves {x,y}[128] and
 // {z,gm}[128]: 16-byte stride, conflict-free for lane-distinct addresses) and carrying the three
 // accumulators of that j in registers, handed to the neighbouring lane by SHFL after every
-// rotation (6 SHFL.32 per 80 FP64 instructions).  After 32 rotations every lane holds the partial
+// rotation (6 SHFL.32 per 120 FP64 instructions at IPT = 6).  After 32 rotations every lane holds the partial
 // a_j of its home j = L.  The 4 warps' partials are combined through shared memory in warp order
 // and written to a triangular partial buffer partJ[I][c][j >= I*SYM_R]; the resident a_i go to
 // partI[unit][c][row].  sym_reduce_kernel adds, for each body, its row partials in unit order and
@@ -21,8 +21,15 @@
 // no atomics, bit-reproducible.
 //
 // Diagonal tiles (j tile inside the row block) take each unordered pair once by masking j <= i.
-// Changeover / coincident pairs are caught by the same integer gate as in pair_accel.cuh and
-// recomputed exactly by slow_weight(gm = 1).
+// Changeover / coincident pairs are caught by the same integer gate as in pair_accel.cuh (here one
+// compare per rotation: min of the IPT high words of s2 against the largest gate of the lane's
+// bodies and of the tile) and recomputed exactly by slow_weight(gm = 1).
+//
+// Tuning record (B200, N = 65,536; the SYM_* macros exist for these sweeps): IPT 4 at 3 CTAs/SM
+// 2.92 ms, IPT 6 at 2 CTAs/SM 2.87 ms, IPT 7 2.97 ms, IPT 8 spills; more resident warps do not help
+// (the FP64 pipe, not latency, is the limit: a pure DFMA stream reaches 86-90 % of the nominal peak
+// on this chip, every non-FP64 instruction costs about one more issue cycle); an FP32 MUFU.RSQ seed
+// re-biased with integer instructions is slower than MUFU.RSQ64H (+8 %).
 #pragma once
 #include "common.cuh"
 #include "pair_accel.cuh"

@@ -47,14 +47,14 @@ def _lib(kind="ld"):
     L.oracle_real_bytes.restype = I
     L.oracle_changeover.restype = C.c_double
     L.oracle_changeover.argtypes = [C.c_double, C.c_double]
-    L.oracle_accel.restype = I
-    L.oracle_accel.argtypes = [I, I, D, D, D, D, D]
-    L.oracle_accel_rows.restype = I
-    L.oracle_accel_rows.argtypes = [I, I, D, D, D, P32, I, D, D]
-    L.oracle_encounters_rows.restype = I64
-    L.oracle_encounters_rows.argtypes = [I, I, C.c_double, D, D, D, D, D, P32, I64, PU8, P32, I64, PI64, I, I]
-    L.oracle_boxes.restype = I
-    L.oracle_boxes.argtypes = [I, I, C.c_double, D, D, D, D, D, D, D]
+    L.oracle_accel_big.restype = I
+    L.oracle_accel_big.argtypes = [I, I, I, D, D, D, D, D]
+    L.oracle_accel_rows_big.restype = I
+    L.oracle_accel_rows_big.argtypes = [I, I, I, D, D, D, P32, I, D, D]
+    L.oracle_encounters_big.restype = I64
+    L.oracle_encounters_big.argtypes = [I, I, I, C.c_double, D, D, D, D, D, P32, I64, PU8, P32, I64, PI64, I, I]
+    L.oracle_boxes_big.restype = I
+    L.oracle_boxes_big.argtypes = [I, I, I, C.c_double, D, D, D, D, D, D, D]
     L.oracle_pair_d2min.restype = C.c_double
     L.oracle_pair_d2min.argtypes = [I, C.c_double, D, D, D, D, I, I]
     L.oracle_encounters.restype = I64
@@ -65,9 +65,9 @@ def _lib(kind="ld"):
     L.oracle_kick.argtypes = [I, I, C.c_double, D, D]
     L.oracle_jump.restype = I
     L.oracle_jump.argtypes = [I, I, C.c_double, C.c_double, D, D, D, D]
-    L.oracle_step.restype = I64
-    L.oracle_step.argtypes = [I, I, C.c_double, D, D, C.c_double, D, D, D, D, D,
-                              P32, I64, PU8, P32, I64, PI64, P32]
+    L.oracle_step_big.restype = I64
+    L.oracle_step_big.argtypes = [I, I, I, C.c_double, D, D, C.c_double, D, D, D, D, D,
+                                  P32, I64, PU8, P32, I64, PI64, P32]
     L.oracle_step_noenc.restype = I
     L.oracle_step_noenc.argtypes = [I, I, C.c_double, D, D, C.c_double, D, D, D]
     _loaded[kind] = L
@@ -97,34 +97,42 @@ def changeover(r: float, rc: float, kind="ld") -> float:
     return float(_lib(kind).oracle_changeover(float(r), float(rc)))
 
 
-def accel(gm, x, rcrit, kind="ld"):
+def _nbig(nbig, nb):
+    """nbig = number of big bodies = gravity sources / first members of encounter pairs
+    (PAPER.md:152-157, 249-260); None = every body (the fully interacting case)."""
+    n = nb if nbig is None else int(nbig)
+    assert 0 <= n <= nb
+    return n
+
+
+def accel(gm, x, rcrit, kind="ld", nbig=None):
     """O-A.  Returns (a[3,nb], S[3,nb]) with S = sum_j |term| for the tolerance."""
     x = _soa(x); gm = _vec(gm); rcrit = _vec(rcrit)
     nb = x.shape[1]
     a = np.zeros_like(x); S = np.zeros_like(x)
-    rc = _lib(kind).oracle_accel(nb, nb, _dp(gm), _dp(x), _dp(rcrit), _dp(a), _dp(S))
+    rc = _lib(kind).oracle_accel_big(nb, _nbig(nbig, nb), nb, _dp(gm), _dp(x), _dp(rcrit), _dp(a), _dp(S))
     assert rc == 0
     return a, S
 
 
-def accel_rows(gm, x, rcrit, rows, kind="ld"):
+def accel_rows(gm, x, rcrit, rows, kind="ld", nbig=None):
     """O-A for the chosen bodies only.  Returns (a[3,len(rows)], S[3,len(rows)])."""
     x = _soa(x); gm = _vec(gm); rcrit = _vec(rcrit)
     rows = np.ascontiguousarray(rows, dtype=np.int32)
     nb = x.shape[1]
     a = np.zeros((3, len(rows))); S = np.zeros((3, len(rows)))
-    rc = _lib(kind).oracle_accel_rows(nb, nb, _dp(gm), _dp(x), _dp(rcrit),
+    rc = _lib(kind).oracle_accel_rows_big(nb, _nbig(nbig, nb), nb, _dp(gm), _dp(x), _dp(rcrit),
                                       rows.ctypes.data_as(C.POINTER(C.c_int32)), len(rows), _dp(a), _dp(S))
     assert rc == 0
     return a, S
 
 
-def boxes(h, x0, v0, x1, v1, rcrit, kind="ld"):
+def boxes(h, x0, v0, x1, v1, rcrit, kind="ld", nbig=None):
     """O-B.1.  Returns (lo[2,nb], hi[2,nb]) for x and y."""
     x0, v0, x1, v1 = map(_soa, (x0, v0, x1, v1)); rcrit = _vec(rcrit)
     nb = x0.shape[1]
     lo = np.zeros((2, nb)); hi = np.zeros((2, nb))
-    rc = _lib(kind).oracle_boxes(nb, nb, float(h), _dp(x0), _dp(v0), _dp(x1), _dp(v1),
+    rc = _lib(kind).oracle_boxes_big(nb, _nbig(nbig, nb), nb, float(h), _dp(x0), _dp(v0), _dp(x1), _dp(v1),
                                  _dp(rcrit), _dp(lo), _dp(hi))
     assert rc == 0
     return lo, hi
@@ -137,7 +145,7 @@ def pair_d2min(h, x0, v0, x1, v1, i, j, kind="ld") -> float:
                                               int(i), int(j)))
 
 
-def encounters(h, x0, v0, x1, v1, rcrit, cap=None, kind="ld", row_stride=1, row_phase=0):
+def encounters(h, x0, v0, x1, v1, rcrit, cap=None, kind="ld", row_stride=1, row_phase=0, nbig=None):
     """O-B.  Returns dict(pairs[n,2] sorted, count (true total), flag[nb] uint8,
     ambig[m,2], n_ambig).  row_stride > 1 restricts to rows i % row_stride == row_phase."""
     x0, v0, x1, v1 = map(_soa, (x0, v0, x1, v1)); rcrit = _vec(rcrit)
@@ -150,7 +158,7 @@ def encounters(h, x0, v0, x1, v1, rcrit, cap=None, kind="ld", row_stride=1, row_
         amb = np.zeros((max(cap, 1), 2), dtype=np.int32)
         flag = np.zeros(max(nb, 1), dtype=np.uint8)
         n_amb = C.c_int64(0)
-        cnt = L.oracle_encounters_rows(nb, nb, float(h), _dp(x0), _dp(v0), _dp(x1), _dp(v1), _dp(rcrit),
+        cnt = L.oracle_encounters_big(nb, _nbig(nbig, nb), nb, float(h), _dp(x0), _dp(v0), _dp(x1), _dp(v1), _dp(rcrit),
                                        pairs.ctypes.data_as(C.POINTER(C.c_int32)), cap,
                                        flag.ctypes.data_as(C.POINTER(C.c_uint8)),
                                        amb.ctypes.data_as(C.POINTER(C.c_int32)), cap, C.byref(n_amb),
@@ -188,13 +196,14 @@ def jump(hj, mu, gm, x, v, kind="ld"):
     return x, P
 
 
-def step(mu, gm, rcrit, h, x, v, a, cap=1 << 16, with_encounters=True, kind="ld"):
+def step(mu, gm, rcrit, h, x, v, a, cap=1 << 16, with_encounters=True, kind="ld", nbig=None):
     """O-D, one hybrid step.  Returns dict(x, v, a, x0, v0, pairs, count, flag, ambig, n_ambig, nfail)."""
     x = _soa(x).copy(); v = _soa(v).copy(); a = _soa(a).copy()
     gm = _vec(gm); rcrit = _vec(rcrit)
     nb = x.shape[1]
     L = _lib(kind)
     if not with_encounters:
+        assert nbig is None or int(nbig) == nb
         rc = L.oracle_step_noenc(nb, nb, float(mu), _dp(gm), _dp(rcrit), float(h), _dp(x), _dp(v), _dp(a))
         assert rc == 0
         return dict(x=x, v=v, a=a)
@@ -203,7 +212,7 @@ def step(mu, gm, rcrit, h, x, v, a, cap=1 << 16, with_encounters=True, kind="ld"
     flag = np.zeros(max(nb, 1), dtype=np.uint8)
     n_amb = C.c_int64(0); nfail = C.c_int32(0)
     P32 = C.POINTER(C.c_int32)
-    cnt = L.oracle_step(nb, nb, float(mu), _dp(gm), _dp(rcrit), float(h), _dp(x), _dp(v), _dp(a),
+    cnt = L.oracle_step_big(nb, _nbig(nbig, nb), nb, float(mu), _dp(gm), _dp(rcrit), float(h), _dp(x), _dp(v), _dp(a),
                         _dp(x0), _dp(v0), pairs.ctypes.data_as(P32), cap,
                         flag.ctypes.data_as(C.POINTER(C.c_uint8)), amb.ctypes.data_as(P32), cap,
                         C.byref(n_amb), C.byref(nfail))

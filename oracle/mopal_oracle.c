@@ -97,13 +97,18 @@ double oracle_changeover(double r, double rc)
  * reading A-7).  S (nullable) receives sum_j |term| per component for the
  * parity tolerance |a_gpu - a_ref| <= 1e-12 S.
  * ------------------------------------------------------------------------- */
-static void accel_row(int nb, int ld, const double *gm, const double *x, const double *rcrit,
+/* nsrc = number of gravity sources: the paper's inner loop runs over the big bodies only,
+ * `do i = 2, nbig` inside `do j = 2, nbod` ("only the massive ones, labeled
+ * as big bodies in the software, are also gravity sources").  Sources are bodies
+ * 0..nsrc-1; nsrc = nb is the fully interacting case (reading R-1). */
+static void accel_row(int nb, int nsrc, int ld, const double *gm, const double *x, const double *rcrit,
                       int i, real *acc3, real *abs3)
 {
+    (void)nb;
     real xi = X_(x, 0, i), yi = X_(x, 1, i), zi = X_(x, 2, i);
     real rci = (real)rcrit[i];
     real ax = 0, ay = 0, az = 0, sx = 0, sy = 0, sz = 0;
-    for (int j = 0; j < nb; ++j) {
+    for (int j = 0; j < nsrc; ++j) {
         if (j == i) continue;
         real dx = X_(x, 0, j) - xi;
         real dy = X_(x, 1, j) - yi;
@@ -121,14 +126,14 @@ static void accel_row(int nb, int ld, const double *gm, const double *x, const d
     abs3[0] = sx; abs3[1] = sy; abs3[2] = sz;
 }
 
-int oracle_accel(int nb, int ld, const double *gm, const double *x,
-                 const double *rcrit, double *a, double *S)
+int oracle_accel_big(int nb, int nbig, int ld, const double *gm, const double *x,
+                     const double *rcrit, double *a, double *S)
 {
-    if (nb < 0 || ld < nb) return 1;
+    if (nb < 0 || ld < nb || nbig < 0 || nbig > nb) return 1;
 #pragma omp parallel for schedule(static)
     for (int i = 0; i < nb; ++i) {
         real acc[3], ab[3];
-        accel_row(nb, ld, gm, x, rcrit, i, acc, ab);
+        accel_row(nb, nbig, ld, gm, x, rcrit, i, acc, ab);
         for (int c = 0; c < 3; ++c) {
             a[(size_t)c * ld + i] = (double)acc[c];
             if (S) S[(size_t)c * ld + i] = (double)ab[c];
@@ -137,23 +142,35 @@ int oracle_accel(int nb, int ld, const double *gm, const double *x,
     return 0;
 }
 
+int oracle_accel(int nb, int ld, const double *gm, const double *x,
+                 const double *rcrit, double *a, double *S)
+{
+    return oracle_accel_big(nb, nb, ld, gm, x, rcrit, a, S);
+}
+
 /* the same sum for a chosen subset of bodies i (full-size sampled parity):
  * a_out / S_out are [3][nrows]. */
-int oracle_accel_rows(int nb, int ld, const double *gm, const double *x, const double *rcrit,
-                      const int32_t *rows, int nrows, double *a_out, double *S_out)
+int oracle_accel_rows_big(int nb, int nbig, int ld, const double *gm, const double *x, const double *rcrit,
+                          const int32_t *rows, int nrows, double *a_out, double *S_out)
 {
-    if (nb < 0 || ld < nb || nrows < 0) return 1;
+    if (nb < 0 || ld < nb || nrows < 0 || nbig < 0 || nbig > nb) return 1;
 #pragma omp parallel for schedule(dynamic, 1)
     for (int k = 0; k < nrows; ++k) {
         real acc[3], ab[3];
         if (rows[k] < 0 || rows[k] >= nb) continue;
-        accel_row(nb, ld, gm, x, rcrit, rows[k], acc, ab);
+        accel_row(nb, nbig, ld, gm, x, rcrit, rows[k], acc, ab);
         for (int c = 0; c < 3; ++c) {
             a_out[(size_t)c * nrows + k] = (double)acc[c];
             if (S_out) S_out[(size_t)c * nrows + k] = (double)ab[c];
         }
     }
     return 0;
+}
+
+int oracle_accel_rows(int nb, int ld, const double *gm, const double *x, const double *rcrit,
+                      const int32_t *rows, int nrows, double *a_out, double *S_out)
+{
+    return oracle_accel_rows_big(nb, nb, ld, gm, x, rcrit, rows, nrows, a_out, S_out);
 }
 
 /* ---------------------------------------------------------------------------
@@ -192,7 +209,9 @@ static void box_1d(real p0, real p1, real w0, real w1, real h, real *lo, real *h
     *lo = l; *hi = u;
 }
 
-static void boxes_real(int nb, int ld, real h, const double *x0, const double *v0,
+/* nbig: LOOP 2 adds rcrit to the extremes of the big bodies only, `do j = 2, nbig`
+ * (PAPER.md:249-253); nbig = nb pads every box (reading B-c; R-2). */
+static void boxes_real(int nb, int nbig, int ld, real h, const double *x0, const double *v0,
                        const double *x1, const double *v1, const double *rcrit,
                        real *lo, real *hi)
 {
@@ -201,24 +220,32 @@ static void boxes_real(int nb, int ld, real h, const double *x0, const double *v
         for (int c = 0; c < 2; ++c) {
             real l, u;
             box_1d(X_(x0, c, b), X_(x1, c, b), X_(v0, c, b), X_(v1, c, b), h, &l, &u);
-            lo[(size_t)c * nb + b] = l - (real)rcrit[b];
-            hi[(size_t)c * nb + b] = u + (real)rcrit[b];
+            real pad = (b < nbig) ? (real)rcrit[b] : (real)0;
+            lo[(size_t)c * nb + b] = l - pad;
+            hi[(size_t)c * nb + b] = u + pad;
         }
     }
+}
+
+int oracle_boxes_big(int nb, int nbig, int ld, double h, const double *x0, const double *v0,
+                     const double *x1, const double *v1, const double *rcrit,
+                     double *lo, double *hi)
+{
+    if (nb < 0 || ld < nb || nbig < 0 || nbig > nb) return 1;
+    real *l = (real *)malloc(sizeof(real) * 2 * (size_t)(nb + 1));
+    real *u = (real *)malloc(sizeof(real) * 2 * (size_t)(nb + 1));
+    if (!l || !u) { free(l); free(u); return 2; }
+    boxes_real(nb, nbig, ld, (real)h, x0, v0, x1, v1, rcrit, l, u);
+    for (size_t k = 0; k < 2 * (size_t)nb; ++k) { lo[k] = (double)l[k]; hi[k] = (double)u[k]; }
+    free(l); free(u);
+    return 0;
 }
 
 int oracle_boxes(int nb, int ld, double h, const double *x0, const double *v0,
                  const double *x1, const double *v1, const double *rcrit,
                  double *lo, double *hi)
 {
-    if (nb < 0 || ld < nb) return 1;
-    real *l = (real *)malloc(sizeof(real) * 2 * (size_t)(nb + 1));
-    real *u = (real *)malloc(sizeof(real) * 2 * (size_t)(nb + 1));
-    if (!l || !u) { free(l); free(u); return 2; }
-    boxes_real(nb, ld, (real)h, x0, v0, x1, v1, rcrit, l, u);
-    for (size_t k = 0; k < 2 * (size_t)nb; ++k) { lo[k] = (double)l[k]; hi[k] = (double)u[k]; }
-    free(l); free(u);
-    return 0;
+    return oracle_boxes_big(nb, nb, ld, h, x0, v0, x1, v1, rcrit, lo, hi);
 }
 
 /* ---------------------------------------------------------------------------
@@ -313,24 +340,26 @@ static int classify_pair(int nb, int ld, real h, const double *x0, const double 
  * pair (paper: ce=2).  ambig (nullable): pairs whose outcome
  * is within 1e-12 relative of a threshold, n_ambig = their true number.
  * ------------------------------------------------------------------------- */
-static int64_t encounters_impl(int nb, int ld, double h_, const double *x0, const double *v0,
+/* nbig: LOOP 3 runs `do i = 2, nbig` x `do j = 2, nbod`, j > i: the first
+ * body of a pair is a big body; nbig = nb tests every pair (reading R-3). */
+static int64_t encounters_impl(int nb, int nbig, int ld, double h_, const double *x0, const double *v0,
                                const double *x1, const double *v1, const double *rcrit,
                                int32_t *pairs, int64_t cap, uint8_t *flag,
                                int32_t *ambig, int64_t ambig_cap, int64_t *n_ambig,
                                int row_stride, int row_phase)
 {
-    if (nb < 0 || ld < nb) return -1;
+    if (nb < 0 || ld < nb || nbig < 0 || nbig > nb) return -1;
     real h = (real)h_;
     real *lo = (real *)malloc(sizeof(real) * 2 * (size_t)(nb + 1));
     real *hi = (real *)malloc(sizeof(real) * 2 * (size_t)(nb + 1));
     int64_t *rowcnt = (int64_t *)calloc((size_t)nb + 1, sizeof(int64_t));
     int64_t *rowamb = (int64_t *)calloc((size_t)nb + 1, sizeof(int64_t));
     if (!lo || !hi || !rowcnt || !rowamb) { free(lo); free(hi); free(rowcnt); free(rowamb); return -2; }
-    boxes_real(nb, ld, h, x0, v0, x1, v1, rcrit, lo, hi);
+    boxes_real(nb, nbig, ld, h, x0, v0, x1, v1, rcrit, lo, hi);
     if (flag) memset(flag, 0, (size_t)nb);
     /* pass 1: per-row counts */
 #pragma omp parallel for schedule(dynamic, 16)
-    for (int i = 0; i < nb; ++i) {
+    for (int i = 0; i < nbig; ++i) {
         int64_t c = 0, ca = 0;
         if (i % row_stride != row_phase) continue;
         for (int j = i + 1; j < nb; ++j) {
@@ -347,7 +376,7 @@ static int64_t encounters_impl(int nb, int ld, double h_, const double *x0, cons
     }
     /* pass 2: fill in order */
 #pragma omp parallel for schedule(dynamic, 16)
-    for (int i = 0; i < nb; ++i) {
+    for (int i = 0; i < nbig; ++i) {
         int64_t o = rowcnt[i], oa = rowamb[i];
         int64_t ne = ((i + 1 < nb) ? rowcnt[i + 1] : total) - o;
         int64_t na = ((i + 1 < nb) ? rowamb[i + 1] : total_a) - oa;
@@ -380,7 +409,7 @@ int64_t oracle_encounters(int nb, int ld, double h_, const double *x0, const dou
                           int32_t *pairs, int64_t cap, uint8_t *flag,
                           int32_t *ambig, int64_t ambig_cap, int64_t *n_ambig)
 {
-    return encounters_impl(nb, ld, h_, x0, v0, x1, v1, rcrit, pairs, cap, flag, ambig, ambig_cap,
+    return encounters_impl(nb, nb, ld, h_, x0, v0, x1, v1, rcrit, pairs, cap, flag, ambig, ambig_cap,
                            n_ambig, 1, 0);
 }
 
@@ -393,7 +422,18 @@ int64_t oracle_encounters_rows(int nb, int ld, double h_, const double *x0, cons
                                int row_stride, int row_phase)
 {
     if (row_stride < 1 || row_phase < 0 || row_phase >= row_stride) return -1;
-    return encounters_impl(nb, ld, h_, x0, v0, x1, v1, rcrit, pairs, cap, flag, ambig, ambig_cap,
+    return encounters_impl(nb, nb, ld, h_, x0, v0, x1, v1, rcrit, pairs, cap, flag, ambig, ambig_cap,
+                           n_ambig, row_stride, row_phase);
+}
+
+int64_t oracle_encounters_big(int nb, int nbig, int ld, double h_, const double *x0, const double *v0,
+                              const double *x1, const double *v1, const double *rcrit,
+                              int32_t *pairs, int64_t cap, uint8_t *flag,
+                              int32_t *ambig, int64_t ambig_cap, int64_t *n_ambig,
+                              int row_stride, int row_phase)
+{
+    if (row_stride < 1 || row_phase < 0 || row_phase >= row_stride) return -1;
+    return encounters_impl(nb, nbig, ld, h_, x0, v0, x1, v1, rcrit, pairs, cap, flag, ambig, ambig_cap,
                            n_ambig, row_stride, row_phase);
 }
 
@@ -549,15 +589,17 @@ int oracle_jump(int nb, int ld, double hj, double mu, const double *gm, double *
  *   kick h/2 -> jump h/2 -> copy x0,v0 -> drift h -> encounter check ->
  *   jump h/2 (mvsum from the drifted v) -> a = accel(x) -> kick h/2.
  * `a` must be current for `x` on entry; it is current for the new x on exit.
- * No restore and no encounter resolution (reading S-3).
+ * No restore and no encounter resolution (reading S-3).  nbig < nb: the force sum and the
+ * encounter check use the big bodies as sources / first members (R-1..R-3); kick, mvsum, jump,
+ * copy and drift run over all bodies, `do j = 2, nbod`.
  * Returns the encounter count of this step (<0 on error); *nfail = drift failures.
  * ------------------------------------------------------------------------- */
-int64_t oracle_step(int nb, int ld, double mu, const double *gm, const double *rcrit,
+int64_t oracle_step_big(int nb, int nbig, int ld, double mu, const double *gm, const double *rcrit,
                     double h, double *x, double *v, double *a, double *x0, double *v0,
                     int32_t *pairs, int64_t cap, uint8_t *flag,
                     int32_t *ambig, int64_t ambig_cap, int64_t *n_ambig, int32_t *nfail)
 {
-    if (nb < 0 || ld < nb) return -1;
+    if (nb < 0 || ld < nb || nbig < 0 || nbig > nb) return -1;
     oracle_kick(nb, ld, 0.5 * h, v, a);
     oracle_jump(nb, ld, 0.5 * h, mu, gm, x, v, 0);
     for (int c = 0; c < 3; ++c) {                        /* LOOP 4 */
@@ -566,12 +608,21 @@ int64_t oracle_step(int nb, int ld, double mu, const double *gm, const double *r
     }
     int nf = oracle_drift(nb, ld, mu, h, x, v, 0);
     if (nfail) *nfail = nf;
-    int64_t cnt = oracle_encounters(nb, ld, h, x0, v0, x, v, rcrit, pairs, cap, flag,
-                                    ambig, ambig_cap, n_ambig);
+    int64_t cnt = oracle_encounters_big(nb, nbig, ld, h, x0, v0, x, v, rcrit, pairs, cap, flag,
+                                        ambig, ambig_cap, n_ambig, 1, 0);
     oracle_jump(nb, ld, 0.5 * h, mu, gm, x, v, 0);
-    oracle_accel(nb, ld, gm, x, rcrit, a, 0);
+    oracle_accel_big(nb, nbig, ld, gm, x, rcrit, a, 0);
     oracle_kick(nb, ld, 0.5 * h, v, a);
     return cnt;
+}
+
+int64_t oracle_step(int nb, int ld, double mu, const double *gm, const double *rcrit,
+                    double h, double *x, double *v, double *a, double *x0, double *v0,
+                    int32_t *pairs, int64_t cap, uint8_t *flag,
+                    int32_t *ambig, int64_t ambig_cap, int64_t *n_ambig, int32_t *nfail)
+{
+    return oracle_step_big(nb, nb, ld, mu, gm, rcrit, h, x, v, a, x0, v0, pairs, cap, flag,
+                           ambig, ambig_cap, n_ambig, nfail);
 }
 
 /* step without the O(N^2/2) encounter pass, for long multi-step invariant pins */

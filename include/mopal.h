@@ -116,6 +116,16 @@ void mo_destroy(mo_ctx *ctx);
 
 /* ---- extras ------------------------------------------------------------- */
 
+/* Big x all variant (the paper's own loop bounds): bodies
+ * 0..nbig-1 are the "big" bodies.  Only they are gravity sources (mo_accel: a_i = sum over
+ * j < nbig, j != i, for every body i), only their boxes are padded by rcrit, and only they can
+ * be the first member of an encounter pair (i < nbig, i < j < nb).  Kick, stellar jump
+ * (P = sum over ALL bodies of gm v), snapshot and drift still run over every body.
+ * nbig = nb (the default after mo_create) is the fully interacting case.  1 <= nbig <= nb, else
+ * MO_EINVAL.  Changing nbig drops the cached step graph and the pair-kernel scratch and
+ * invalidates `a`.  Synchronises the stream. */
+mo_status mo_set_nbig(mo_ctx *ctx, int32_t nbig);
+
 /* Copy the current x, v into the context's x0, v0 snapshot (asynchronous). */
 mo_status mo_snapshot(mo_ctx *ctx);
 /* Device pointers of the snapshot planes (3*ld doubles each), for inspection. */

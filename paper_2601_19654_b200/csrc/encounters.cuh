@@ -87,6 +87,8 @@ __device__ __forceinline__ void body_box(const double* __restrict__ x0, const do
 struct EncState {
     const double *x0, *v0, *x1, *v1, *rcrit;
     int nb, ld;
+    int nbig;   // bodies 0..nbig-1 are big: padded boxes (LOOP 2), first members of pairs
+                // (LOOP 3 `do i = 2, nbig`); nbig = nb: every body
     double h;
 };
 
@@ -160,6 +162,7 @@ struct EncBuf {
     float4* sboxf;       // nbPad FP32 boxes in sorted order (pad records at the end)
     float4* tbox;        // nTiles bounding box of each run of TJ sorted boxes
     int* tilecnt;        // nTiles hits per run of TJ rows (body order), the scan's block bases
+    int* tbig;           // nTiles: 1 iff the run of TJ sorted boxes holds a big body (index < nbig)
 };
 
 constexpr int ENC_GRID = 64;                       // cells per axis
@@ -204,7 +207,7 @@ __global__ void __launch_bounds__(ON_BLOCK) boxes_kernel(EncState s, EncBuf e, i
     if (b < nbPad) {
         double4 r;
         if (b < s.nb) {
-            body_box(s.x0, s.v0, s.x1, s.v1, s.rcrit[b], s.ld, b, s.h, r);
+            body_box(s.x0, s.v0, s.x1, s.v1, b < s.nbig ? s.rcrit[b] : 0.0, s.ld, b, s.h, r);
             flag[b] = 0;
             bf = box_f32(r);
         } else {
@@ -309,10 +312,13 @@ __global__ void __launch_bounds__(ON_BLOCK) enc_sortscatter_kernel(EncBuf e, int
     }
 }
 
-// bounding box of each run of TJ sorted boxes
-__global__ void __launch_bounds__(TJ) enc_tilebox_kernel(EncBuf e) {
+// bounding box of each run of TJ sorted boxes, and whether the run holds a big body: a pair of
+// runs without one has no pair whose first member is big (LOOP 3 `do i = 2, nbig`)
+__global__ void __launch_bounds__(TJ) enc_tilebox_kernel(EncBuf e, int nbig) {
     __shared__ float4 sh4[TJ / 32];
     float4 r = e.sboxf[blockIdx.x * TJ + threadIdx.x];    // {lox, hix, loy, hiy}; pads are (+inf, -inf, ..)
+    const int big = __syncthreads_or(e.perm[blockIdx.x * TJ + threadIdx.x] < nbig);
+    if (threadIdx.x == 0) e.tbig[blockIdx.x] = big ? 1 : 0;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
         r.x = fminf(r.x, __shfl_down_sync(0xffffffffu, r.x, o));
@@ -357,6 +363,7 @@ __device__ __forceinline__ bool gate_f64(const double4& a, const double4& b) {
 __device__ __forceinline__ void enc_exact(const EncFindParams& p, int2 c) {
     const int ba = p.e.perm[c.x], bb = p.e.perm[c.y];
     const int i = min(ba, bb), j = max(ba, bb);
+    if (i >= p.s.nbig) return;                 // first member must be a big body
     const double4 bi = p.e.box[i], bj = p.e.box[j];
     if (!gate_f64(bi, bj)) return;
     if (!pair_hit(p.s, i, j)) return;
@@ -381,6 +388,7 @@ __global__ void __launch_bounds__(CTA_THREADS) enc_find_kernel(EncFindParams p) 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int rb = blockIdx.x;
     const float4 own = p.e.tbox[rb];
+    const bool rbig = p.e.tbig[rb] != 0;
 
     if (tid == 0) {
 #pragma unroll
@@ -402,7 +410,7 @@ __global__ void __launch_bounds__(CTA_THREADS) enc_find_kernel(EncFindParams p) 
         __syncthreads();
         for (int k = tid; k < ENC_WIN; k += CTA_THREADS) {
             const int t = w0 + k * S;
-            if (t < p.nTiles && gate_f32(own, p.e.tbox[t])) s_list[atomicAdd(&s_n, 1)] = t;
+            if (t < p.nTiles && gate_f32(own, p.e.tbox[t]) && (rbig || p.e.tbig[t] != 0)) s_list[atomicAdd(&s_n, 1)] = t;
         }
         __syncthreads();
         const int nt = s_n;
@@ -556,7 +564,7 @@ __global__ void __launch_bounds__(256) enc_write_kernel(EncWriteParams p) {
     const int lane = threadIdx.x & 31;
     const int gw = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const int nw = (gridDim.x * blockDim.x) >> 5;
-    for (int row = gw; row < p.s.nb; row += nw) {
+    for (int row = gw; row < p.s.nbig; row += nw) {
         const int cnt = p.e.rowcnt[row];
         if (cnt == 0) continue;
         const long long off = p.e.rowoff[row];

@@ -41,7 +41,7 @@ struct MidParams {
     EncBuf enc;
     uint8_t* flag;
     DevStats* st;
-    int nb, ld, nbPad, npsum;
+    int nb, ld, nbPad, npsum, nbig;
     double hj_over_mu, mu, h;
 };
 
@@ -68,7 +68,7 @@ __global__ void __launch_bounds__(ON_BLOCK) jump_drift_boxes_kernel(MidParams p)
         if (iters > 3) atomicMax(&p.st->max_newton, iters);
         p.x[b] = x; p.x[ld + b] = y; p.x[2 * ld + b] = z;
         p.v[b] = vx; p.v[ld + b] = vy; p.v[2 * ld + b] = vz;
-        const double rc = p.rcrit[b];
+        const double rc = b < p.nbig ? p.rcrit[b] : 0.0;   // LOOP 2 pads the big bodies only
         double lo, hi;
         double4 bx;
         box_1d(x0, x, vx0, vx, p.h, lo, hi);

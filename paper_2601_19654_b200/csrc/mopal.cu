@@ -17,6 +17,7 @@ using namespace mopal;
 
 struct mo_ctx {
     int nb = 0, ld = 0, nbPad = 0, nTiles = 0, nsm = 0;
+    int nbig = 0, nSrcTiles = 0;        // big bodies = gravity sources (mo_set_nbig); nbig = nb by default
     double m_star = 0, G = 0, mu = 0;
     // borrowed
     double *x = nullptr, *v = nullptr, *a = nullptr;
@@ -110,27 +111,28 @@ static void choose_geometry(mo_ctx* ctx) {
     if (occ < 1) occ = 1;
     ctx->ctas_per_sm = occ;
     const long long slots = (long long)ctx->nsm * occ;
-    const int smax = ctx->nTiles < 48 ? ctx->nTiles : 48;
+    const int nST = ctx->nSrcTiles;       // j tiles that hold a gravity source
+    const int smax = nST < 48 ? nST : 48;
     double best = 1e300;
     int bestS = 1;
     for (int S = 1; S <= smax; ++S) {
-        const int tps = (ctx->nTiles + S - 1) / S;
-        const int Se = (ctx->nTiles + tps - 1) / tps;
+        const int tps = (nST + S - 1) / S;
+        const int Se = (nST + tps - 1) / tps;
         const long long ctas = (long long)ctx->nIblk * Se;
         const long long waves = (ctas + slots - 1) / slots;
         const double cost = (double)waves * (tps + 1.5);
         if (cost < best * (1.0 - 1e-9)) { best = cost; bestS = Se; }
     }
     const int forced = env_int("MO_JSPLIT", 0);
-    if (forced > 0) bestS = forced < ctx->nTiles ? forced : ctx->nTiles;
-    ctx->tps = (ctx->nTiles + bestS - 1) / bestS;
-    ctx->nsplit = (ctx->nTiles + ctx->tps - 1) / ctx->tps;
+    if (forced > 0) bestS = forced < nST ? forced : nST;
+    ctx->tps = (nST + bestS - 1) / bestS;
+    ctx->nsplit = (nST + ctx->tps - 1) / ctx->tps;
     // encounter find: column tiles of a row tile are dealt round-robin to enc_split CTAs
     ctx->enc_split = env_int("MO_ENC_SPLIT", ctx->nTiles / 8);
     if (ctx->enc_split < 1) ctx->enc_split = 1;
     if (ctx->enc_split > 8) ctx->enc_split = 8;
     // two-sided kernel for large nb: units = (row block, chunk of sym_ch j tiles from the diagonal on)
-    ctx->use_sym = env_int("MO_SYM", nb >= env_int("MO_SYM_MIN", 8192) ? 1 : 0) != 0;
+    ctx->use_sym = ctx->nbig == nb && env_int("MO_SYM", nb >= env_int("MO_SYM_MIN", 8192) ? 1 : 0) != 0;
     if (ctx->use_sym) {
         int occs = 1;
         cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occs, pair_sym_kernel, SYM_THREADS, 0);
@@ -185,6 +187,7 @@ extern "C" void mo_destroy(mo_ctx* ctx) {
     cudaFree(ctx->enc.ovf_now); cudaFree(ctx->dstats); cudaFree(ctx->probe);
     cudaFree(ctx->enc.bpart); cudaFree(ctx->enc.cellcnt); cudaFree(ctx->enc.cellfill); cudaFree(ctx->enc.key);
     cudaFree(ctx->enc.perm); cudaFree(ctx->enc.sboxf); cudaFree(ctx->enc.tbox); cudaFree(ctx->enc.tilecnt);
+    cudaFree(ctx->enc.tbig);
     if (ctx->hstats) cudaFreeHost(ctx->hstats);
     delete ctx;
 }
@@ -209,6 +212,7 @@ extern "C" mo_status mo_create(mo_ctx** out, int32_t nb, int32_t ld, double m_st
     ctx->use_graph = env_int("MO_NO_GRAPH", 0) == 0;
     ctx->nTiles = (nb + TJ - 1) / TJ;
     ctx->nbPad = ctx->nTiles * TJ;
+    ctx->nbig = nb; ctx->nSrcTiles = ctx->nTiles;
     int dev = 0;
     cudaDeviceProp prop;
     if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
@@ -243,6 +247,7 @@ extern "C" mo_status mo_create(mo_ctx** out, int32_t nb, int32_t ld, double m_st
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->enc.sboxf, (size_t)ctx->nbPad);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->enc.tbox, (size_t)ctx->nTiles);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->enc.tilecnt, (size_t)ctx->nTiles);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->enc.tbig, (size_t)ctx->nTiles);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->dstats, 1);
     if (e == cudaSuccess) e = cudaMallocHost(reinterpret_cast<void**>(&ctx->hstats), sizeof(DevStats));
     if (e != cudaSuccess) {
@@ -291,7 +296,7 @@ static mo_status ensure_pair_scratch(mo_ctx* ctx) {
 static mo_status launch_pair(mo_ctx* ctx) {
     AccelParams p;
     p.tiles = ctx->tiles; p.x = ctx->x; p.rcrit = ctx->rcrit; p.part = ctx->part;
-    p.nb = ctx->nb; p.ld = ctx->ld; p.nTiles = ctx->nTiles; p.tps = ctx->tps;
+    p.nb = ctx->nb; p.ld = ctx->ld; p.nTiles = ctx->nSrcTiles; p.tps = ctx->tps;
     dim3 grid(ctx->nIblk, ctx->nsplit);
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     if (ctx->timing) {
@@ -323,7 +328,8 @@ static mo_status enqueue_accel(mo_ctx* ctx, bool jump, double hj, bool kick, dou
     const int nps = jump ? ctx->npsum : 0;
     auto pk = jump ? (ctx->use_sym ? pack_kernel<true, true> : pack_kernel<true, false>)
                    : (ctx->use_sym ? pack_kernel<false, true> : pack_kernel<false, false>);
-    pk<<<ctx->nTiles, TJ, 0, ctx->stream>>>(ctx->x, ctx->gm, ctx->rcrit, ctx->nb, ctx->ld, ctx->tiles, ps, nps, hjm);
+    pk<<<jump ? ctx->nTiles : ctx->nSrcTiles, TJ, 0, ctx->stream>>>(ctx->x, ctx->gm, ctx->rcrit, ctx->nb, ctx->nbig, ctx->ld,
+                                                                    ctx->tiles, ps, nps, hjm);
     mo_status s = post_launch(ctx);
     if (s != MO_OK) return s;
     s = launch_pair(ctx);
@@ -343,7 +349,7 @@ static mo_status enqueue_accel(mo_ctx* ctx, bool jump, double hj, bool kick, dou
 static EncState enc_state(const mo_ctx* ctx, const double* x0, const double* v0, double h) {
     EncState s;
     s.x0 = x0; s.v0 = v0; s.x1 = ctx->x; s.v1 = ctx->v; s.rcrit = ctx->rcrit;
-    s.nb = ctx->nb; s.ld = ctx->ld; s.h = h;
+    s.nb = ctx->nb; s.ld = ctx->ld; s.nbig = ctx->nbig; s.h = h;
     return s;
 }
 
@@ -356,7 +362,7 @@ static mo_status enqueue_pairs(mo_ctx* ctx, const EncState& es, int step_inc) {
     enc_sortscatter_kernel<<<ctx->npsum, ON_BLOCK, 0, ctx->stream>>>(ctx->enc, ctx->nb, ctx->nbPad);
     s = post_launch(ctx);
     if (s != MO_OK) return s;
-    enc_tilebox_kernel<<<ctx->nTiles, TJ, 0, ctx->stream>>>(ctx->enc);
+    enc_tilebox_kernel<<<ctx->nTiles, TJ, 0, ctx->stream>>>(ctx->enc, ctx->nbig);
     s = post_launch(ctx);
     if (s != MO_OK) return s;
     EncFindParams fp;
@@ -376,7 +382,7 @@ static mo_status enqueue_pairs(mo_ctx* ctx, const EncState& es, int step_inc) {
     if (s != MO_OK) return s;
     EncWriteParams wp;
     wp.s = es; wp.e = ctx->enc; wp.pairs = ctx->pairs; wp.cap = ctx->cap; wp.flag = ctx->flag;
-    int blocks = (ctx->nb + 7) / 8;
+    int blocks = (ctx->nbig + 7) / 8;
     const int maxb = ctx->nsm * 8;
     if (blocks > maxb) blocks = maxb;
     enc_write_kernel<<<blocks, 256, 0, ctx->stream>>>(wp);   // exits at once unless count > cap
@@ -391,6 +397,7 @@ static mo_status enqueue_step(mo_ctx* ctx, double dt) {
     mp.x = ctx->x; mp.v = ctx->v; mp.x0 = ctx->x0; mp.v0 = ctx->v0; mp.gm = ctx->gm; mp.rcrit = ctx->rcrit;
     mp.psum_in = ctx->psumA; mp.psum_out = ctx->psumB; mp.enc = ctx->enc; mp.flag = ctx->flag;
     mp.st = ctx->dstats; mp.nb = ctx->nb; mp.ld = ctx->ld; mp.nbPad = ctx->nbPad; mp.npsum = ctx->npsum;
+    mp.nbig = ctx->nbig;
     mp.hj_over_mu = 0.5 * dt / ctx->mu; mp.mu = ctx->mu; mp.h = dt;
     jump_drift_boxes_kernel<<<ctx->npsum, ON_BLOCK, 0, ctx->stream>>>(mp);
     s = post_launch(ctx);
@@ -465,6 +472,22 @@ extern "C" mo_status mo_snapshot_copy(mo_ctx* ctx, double* x0_dst, double* v0_ds
     const size_t bytes = 3 * (size_t)ctx->ld * sizeof(double);
     CK(cudaMemcpyAsync(x0_dst, ctx->x0, bytes, cudaMemcpyDeviceToDevice, ctx->stream));
     CK(cudaMemcpyAsync(v0_dst, ctx->v0, bytes, cudaMemcpyDeviceToDevice, ctx->stream));
+    return MO_OK;
+}
+
+extern "C" mo_status mo_set_nbig(mo_ctx* ctx, int32_t nbig) {
+    if (!ctx || nbig < 1 || nbig > ctx->nb) return MO_EINVAL;
+    if (nbig == ctx->nbig) return MO_OK;
+    CK(cudaStreamSynchronize(ctx->stream));   // nothing in flight may still use the scratch freed below
+    if (ctx->gexec) { cudaGraphExecDestroy(ctx->gexec); ctx->gexec = nullptr; }
+    cudaFree(ctx->part); ctx->part = nullptr;
+    cudaFree(ctx->sym_units); cudaFree(ctx->sym_ustart); cudaFree(ctx->sym_partI); cudaFree(ctx->sym_partJ);
+    ctx->sym_units = nullptr; ctx->sym_ustart = nullptr; ctx->sym_partI = nullptr; ctx->sym_partJ = nullptr;
+    ctx->pair_ready = false;
+    ctx->a_valid = false;
+    ctx->nbig = nbig;
+    ctx->nSrcTiles = (nbig + TJ - 1) / TJ;
+    choose_geometry(ctx);
     return MO_OK;
 }
 

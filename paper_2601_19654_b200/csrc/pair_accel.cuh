@@ -202,9 +202,12 @@ __device__ __forceinline__ void reduce_psum(const double* __restrict__ psum, int
 
 // SYM selects the tile layout: false = TJ records {x,y,z,gm} (pair_accel_kernel, broadcast reads),
 // true = SoA halves {x,y}[TJ] then {z,gm}[TJ] (pair_sym_kernel, lane-distinct reads).
+// nsrc = number of gravity sources (the big bodies): only the tiles that hold a
+// source are written, and bodies j >= nsrc in the last of them become pad records.  The jump
+// still moves every body (grid = all nb tiles with JUMP, the source tiles without).
 template <bool JUMP, bool SYM>
 __global__ void __launch_bounds__(TJ) pack_kernel(double* __restrict__ x, const double* __restrict__ gm,
-                                                  const double* __restrict__ rcrit, int nb, int ld,
+                                                  const double* __restrict__ rcrit, int nb, int nsrc, int ld,
                                                   unsigned char* __restrict__ tiles,
                                                   const double* __restrict__ psum, int npsum, double hj_over_mu) {
     __shared__ double sh[TJ / 32][3];
@@ -225,10 +228,15 @@ __global__ void __launch_bounds__(TJ) pack_kernel(double* __restrict__ x, const 
             x[j] = X; x[ld + j] = Y; x[2 * ld + j] = Z;
         }
         pa = make_double2(X, Y);
-        pb = make_double2(Z, gm[j]);
-        const double rc = rcrit[j];
-        ghi = __double2hiint(rc * rc);
-    } else {
+        pb = make_double2(Z, 0.0);
+        if (j < nsrc) {
+            pb.y = gm[j];
+            const double rc = rcrit[j];
+            ghi = __double2hiint(rc * rc);
+        }
+    }
+    if (blockIdx.x * TJ >= nsrc) return;      // no source in this tile (block-uniform)
+    if (j >= nsrc) {
         pa = make_double2(PAD_POS, PAD_POS);
         pb = make_double2(PAD_POS, 0.0);
     }

@@ -20,7 +20,8 @@ MO_OK, MO_EINVAL, MO_ENOMEM, MO_ECUDA, MO_EOVERFLOW, MO_ENOCONV = range(6)
 EXPORTS = ["mo_create", "mo_accel", "mo_drift", "mo_encounters", "mo_step", "mo_destroy",
            "mo_snapshot", "mo_snapshot_ptrs", "mo_snapshot_copy", "mo_invalidate_accel", "mo_get_stats", "mo_launch_count",
            "mo_workspace_bytes", "mo_step_host", "mo_accel_host", "mo_probe_fp64_peak",
-           "mo_pair_geometry", "mo_set_kernel_timing", "mo_pair_kernel_ms", "mo_strerror", "mo_version"]
+           "mo_pair_geometry", "mo_set_kernel_timing", "mo_pair_kernel_ms", "mo_strerror", "mo_version",
+           "mo_set_nbig"]
 
 
 class MoStats(C.Structure):
@@ -59,6 +60,7 @@ def load():
     L.mo_snapshot_ptrs.restype = C.c_int; L.mo_snapshot_ptrs.argtypes = [vp, C.POINTER(vp), C.POINTER(vp)]
     L.mo_snapshot_copy.restype = C.c_int; L.mo_snapshot_copy.argtypes = [vp, vp, vp]
     L.mo_invalidate_accel.restype = C.c_int; L.mo_invalidate_accel.argtypes = [vp]
+    L.mo_set_nbig.restype = C.c_int; L.mo_set_nbig.argtypes = [vp, I32]
     L.mo_get_stats.restype = C.c_int; L.mo_get_stats.argtypes = [vp, C.POINTER(MoStats)]
     L.mo_launch_count.restype = I64; L.mo_launch_count.argtypes = [vp]
     L.mo_workspace_bytes.restype = I64; L.mo_workspace_bytes.argtypes = [vp]
@@ -131,6 +133,7 @@ class Mopal:
         torch.cuda.set_device(self.device)
         nb = int(np.asarray(mass).shape[0])
         self.nb = nb
+        self.nbig = nb
         self.ld = (nb + 3) // 4 * 4
         self.cap = int(cap)
         self.m_star, self.G = float(m_star), float(G)
@@ -203,6 +206,12 @@ class Mopal:
         self._check(self._L.mo_snapshot_copy(self._ctx, x0.data_ptr(), v0.data_ptr()), "mo_snapshot_copy")
         self.stream.synchronize()
         return x0, v0
+
+    def set_nbig(self, nbig):
+        """Bodies 0..nbig-1 are the big bodies: the only gravity sources and first members of
+        encounter pairs; nbig = nb is fully interacting."""
+        self._check(self._L.mo_set_nbig(self._ctx, int(nbig)), "mo_set_nbig")
+        self.nbig = int(nbig)
 
     def invalidate_accel(self):
         self._check(self._L.mo_invalidate_accel(self._ctx), "mo_invalidate_accel")

@@ -106,7 +106,7 @@ def elements_to_state(mu, a, e, inc, Om, om, M):
 
 
 def make_disk(N, seed, giants, a, sig_e, sig_i, mass, dt, steps, name="custom",
-              m_star=M_STAR, G=G_AU_DAY_MSUN, n_hill=N_HILL):
+              m_star=M_STAR, G=G_AU_DAY_MSUN, n_hill=N_HILL, nbig=None):
     nb = N - 1
     g = len(giants)
     ns = nb - g
@@ -135,6 +135,8 @@ def make_disk(N, seed, giants, a, sig_e, sig_i, mass, dt, steps, name="custom",
         m_s = (mlo ** -1.5 + u_m * (mhi ** -1.5 - mlo ** -1.5)) ** (-1.0 / 1.5)
     else:
         raise ValueError(mass[0])
+    if nbig is not None:         # bodies nbig.. are massless particles: m = 0, rcrit = 0
+        m_s[max(int(nbig) - g, 0):] = 0.0
     gm_ = np.array([t[0] for t in giants], dtype=np.float64)
     ga = np.array([t[1] for t in giants], dtype=np.float64)
     ge = np.array([t[2] for t in giants], dtype=np.float64)
@@ -162,6 +164,16 @@ def make_config(idx: int) -> Workload:
     """One of BASELINE.json's five configs (0..4)."""
     c = dict(CONFIGS[idx])
     return make_disk(**c)
+
+
+def make_bigsmall(N: int, nbig: int, seed: int = 6, m_embryo: float = 3.0e-7) -> Workload:
+    """The paper's production regime (N_big 1..100 massive bodies, N_small
+    1e4..1e6 massless particles): the cfg3 disk recipe ([1,30] AU, sigma_e/i = 0.02/0.01, the four
+    giants) whose first ``nbig`` bodies are big - the giants plus Mars-mass embryos - and the rest
+    massless (rcrit = 0).  Not one of BASELINE.json's configs: the workload of SURVEY.md 8(f) row 1."""
+    return make_disk(N=N, seed=seed, giants=_GIANTS_4 if nbig >= 4 else _GIANTS_4[:nbig], a=("sigma", 1.0, 30.0),
+                     sig_e=0.02, sig_i=0.01, mass=("equal", m_embryo), dt=8.0, steps=100,
+                     name=f"bigsmall_N{N}_nbig{nbig}", nbig=nbig)
 
 
 def shrink(idx: int, N: int, seed=None) -> Workload:

@@ -436,3 +436,149 @@ def test_invalid_arguments_and_bookkeeping(M):
     tf, ms = M.probe_fp64_peak(2)
     assert 5.0 < tf < 80.0
     m.close()
+
+
+# ------------------------------------------------------------------------------ big x all
+def _mk_big(M, w, nbig, rcrit=None, cap=1 << 20):
+    m = _mk(M, w, rcrit=rcrit, cap=cap)
+    m.set_nbig(nbig)
+    return m
+
+
+@pytest.mark.parametrize("cfg,N,nbig,scale", [(1, 1500, 2, 1.0), (3, 3000, 4, 20.0), (2, 1025, 100, 30.0),
+                                             (2, 2500, 129, 30.0), (4, 700, 699, 50.0), (0, 256, 1, 1.0),
+                                             (2, 9000, 8999, 10.0)])
+def test_bigsmall_accel(M, cfg, N, nbig, scale):
+    """sources are bodies 0..nbig-1 only, every body is a sink; sizes put the
+    source boundary inside a tile, on a tile edge (128 + 1) and one short of nb."""
+    w = W.shrink(cfg, N)
+    rcrit = w.rcrit * scale
+    m = _mk_big(M, w, nbig, rcrit=rcrit)
+    m.accel()
+    a = m.get("a")
+    a_ref, S = oracle.accel(G * w.mass, w.x, rcrit, nbig=nbig)
+    _check_accel(a, a_ref, S, f"{w.name} nbig={nbig}")
+    if nbig < w.nb - 1:
+        a_all, _ = oracle.accel(G * w.mass, w.x, rcrit)
+        assert not np.array_equal(a_ref, a_all)
+    # back to fully interacting on the same context
+    m.set_nbig(w.nb)
+    m.accel()
+    a_ref, S = oracle.accel(G * w.mass, w.x, rcrit)
+    _check_accel(m.get("a"), a_ref, S, f"{w.name} back to nbig=nb")
+    m.close()
+
+
+@pytest.mark.parametrize("cfg,N,nbig,scale", [(1, 1500, 2, 1.0), (3, 3000, 4, 1.0), (2, 1025, 100, 40.0),
+                                             (4, 2000, 150, 60.0), (4, 700, 699, 50.0), (4, 3000, 1, 500.0)])
+def test_bigsmall_encounters(M, cfg, N, nbig, scale):
+    """boxes of the big bodies only are padded, first pair members are big."""
+    w = W.shrink(cfg, N)
+    rcrit = w.rcrit * scale
+    x1, v1 = _enc_inputs(w)
+    ref = oracle.encounters(w.dt, w.x, w.v, x1, v1, rcrit, nbig=nbig)
+    m = _mk_big(M, w, nbig, rcrit=rcrit)
+    m.snapshot()
+    m.set("x", x1); m.set("v", v1)
+    cnt = m.encounters(w.dt)
+    got = m.pair_list(cnt)
+    n_amb = _pairs_ok(got, ref)
+    assert cnt > 0 and np.all(got[:, 0] < nbig) and np.all(got[:, 0] < got[:, 1])
+    if n_amb == 0:
+        assert cnt == ref["count"] and np.array_equal(got, ref["pairs"])
+        assert np.array_equal(m.get("flag"), ref["flag"])
+    full = oracle.encounters(w.dt, w.x, w.v, x1, v1, rcrit)
+    if nbig < w.nb - 1 and scale > 1:
+        assert full["count"] != ref["count"]
+    m.close()
+
+
+def test_bigsmall_encounters_overflow(M):
+    w = W.shrink(4, 600)
+    nbig = 5
+    huge = np.full(w.nb, 1e3)
+    x1, v1 = _enc_inputs(w)
+    ref = oracle.encounters(w.dt, w.x, w.v, x1, v1, huge, nbig=nbig)
+    total = sum(w.nb - 1 - i for i in range(nbig))
+    assert ref["count"] == total
+    cap = 700
+    m = _mk_big(M, w, nbig, rcrit=huge, cap=cap)
+    m.snapshot(); m.set("x", x1); m.set("v", v1)
+    cnt = m.encounters(w.dt)
+    assert cnt == total and np.array_equal(m.pair_list(cnt), ref["pairs"][:cap])
+    assert m.get("flag").all()
+    m.close()
+
+
+@pytest.mark.parametrize("cfg,N,nbig,nsteps", [(1, 1200, 2, 4), (3, 2000, 4, 3), (2, 1500, 130, 2)])
+def test_bigsmall_step_vs_oracle(M, cfg, N, nbig, nsteps):
+    w = W.shrink(cfg, N)
+    mass = w.mass.copy()
+    if cfg != 2:
+        mass[nbig:] = 0.0               # massless small bodies (PAPER.md:66); cfg 2 keeps them massive: P still sums all
+    gm = G * mass
+    mu = G * w.m_star
+    m = M.Mopal(mass, w.x, w.v, w.rcrit, m_star=w.m_star, G=w.G)
+    m.set_nbig(nbig)
+    a, _ = oracle.accel(gm, w.x, w.rcrit, nbig=nbig)
+    x, v = w.x, w.v
+    for k in range(nsteps):
+        st = m.step(w.dt, 1)
+        r = oracle.step(mu, gm, w.rcrit, w.dt, x, v, a, nbig=nbig)
+        x, v, a = r["x"], r["v"], r["a"]
+        ex, ev = _step_err(m, r)
+        tol = 1e-13 * (1 + k)
+        assert ex <= tol and ev <= tol, (k, ex, ev)
+        got = m.pair_list(st.nce_last)
+        _pairs_ok(got, r)
+        if r["n_ambig"] == 0:
+            assert st.nce_last == r["count"]
+        assert np.all(got[:, 0] < nbig)
+    # graph-replay path with nbig set
+    m2 = M.Mopal(mass, w.x, w.v, w.rcrit, m_star=w.m_star, G=w.G)
+    m2.set_nbig(nbig)
+    st2 = m2.step(w.dt, nsteps)
+    assert np.array_equal(m.get("x"), m2.get("x")) and np.array_equal(m.get("v"), m2.get("v"))
+    assert st2.nce_last == st.nce_last
+    m.close(); m2.close()
+
+
+@pytest.mark.parametrize("N,nbig", [(262_144, 100), (1_000_000, 36)])
+def test_bigsmall_production_sizes(M, N, nbig):
+    """the paper's production regime (N_big <= 100, N_small up to 1e6): every big row
+    of the encounter list against the oracle, sampled accel rows, invariants after steps."""
+    w = W.make_bigsmall(N, nbig)
+    gm = G * w.mass
+    m = _mk_big(M, w, nbig)
+    m.accel()
+    rows = np.unique(np.concatenate([np.arange(min(nbig + 3, w.nb)),
+                                     np.random.default_rng(2).integers(0, w.nb, 40)])).astype(np.int32)
+    a_ref, S = oracle.accel_rows(gm, w.x, w.rcrit, rows, nbig=nbig)
+    _check_accel(m.get("a")[:, rows], a_ref, S, w.name)
+    x1, v1 = _enc_inputs(w)
+    m.snapshot(); m.set("x", x1); m.set("v", v1)
+    cnt = m.encounters(w.dt)
+    got = m.pair_list(cnt)
+    ref = oracle.encounters(w.dt, w.x, w.v, x1, v1, w.rcrit, nbig=nbig, cap=1 << 20)
+    n_amb = _pairs_ok(got, ref)
+    assert cnt > 0
+    if n_amb == 0:
+        assert np.array_equal(got, ref["pairs"]) and np.array_equal(m.get("flag"), ref["flag"])
+    m.set("x", w.x); m.set("v", w.v); m.invalidate_accel()
+    st = m.step(w.dt, 2)
+    assert st.steps_done == 2 and st.drift_fail == 0
+    x, v = m.get("x"), m.get("v")
+    a_ref, S = oracle.accel_rows(gm, x, w.rcrit, rows, nbig=nbig)
+    _check_accel(m.get("a")[:, rows], a_ref, S, w.name + " after 2 steps")
+    m.close()
+
+
+def test_bigsmall_invalid(M):
+    w = W.shrink(0, 64)
+    m = _mk(M, w)
+    L = M.load()
+    assert L.mo_set_nbig(m._ctx, 0) == M.MO_EINVAL
+    assert L.mo_set_nbig(m._ctx, w.nb + 1) == M.MO_EINVAL
+    assert L.mo_set_nbig(None, 1) == M.MO_EINVAL
+    assert L.mo_set_nbig(m._ctx, w.nb) == M.MO_OK
+    m.close()

@@ -153,6 +153,8 @@ struct EncBuf {
     int* tmpj;           // cap j's grouped by row, unsorted inside a row
     unsigned long long* nhit;  // hits appended this pass (may exceed cap)
     int* ovf_now;        // this pass found more pairs than cap
+    int* nlong;          // rows with more than ENC_RANK_LONG hits this pass ...
+    int* longrows;       // ... and their indices (any order), written by the scan
     // spatial ordering of this pass (performance only)
     float4* bpart;       // per block of the boxes kernel: {min lox, max lox, min loy, max loy}
     int* cellcnt;        // ENC_NCELL bodies per grid cell
@@ -165,6 +167,7 @@ struct EncBuf {
     int* tbig;           // nTiles: 1 iff the run of TJ sorted boxes holds a big body (index < nbig)
 };
 
+constexpr int ENC_RANK_LONG = 64;                  // rows with more hits are ranked by whole CTAs
 constexpr int ENC_GRID = 64;                       // cells per axis
 constexpr int ENC_NCELL = ENC_GRID * ENC_GRID;
 
@@ -202,7 +205,7 @@ __device__ __forceinline__ void enc_bounds_partial(const EncBuf& e, bool real, c
 __global__ void __launch_bounds__(ON_BLOCK) boxes_kernel(EncState s, EncBuf e, int nbPad, uint8_t* __restrict__ flag) {
     __shared__ float4 sh4[ON_BLOCK / 32];
     const int b = blockIdx.x * ON_BLOCK + threadIdx.x;
-    if (b == 0) *e.nhit = 0ull;
+    if (b == 0) { *e.nhit = 0ull; *e.nlong = 0; }
     float4 bf = pad_boxf();
     if (b < nbPad) {
         double4 r;
@@ -358,11 +361,9 @@ __device__ __forceinline__ bool gate_f64(const double4& a, const double4& b) {
     return (a.x <= b.y) & (b.x <= a.y) & (a.z <= b.w) & (b.z <= a.w);
 }
 
-// one survivor per lane (sorted positions c.x < c.y): exact FP64 gate, exact pair test, record the
-// hit as (i, j) = (smaller, larger) body index
-__device__ __forceinline__ void enc_exact(const EncFindParams& p, int2 c) {
-    const int ba = p.e.perm[c.x], bb = p.e.perm[c.y];
-    const int i = min(ba, bb), j = max(ba, bb);
+// exact FP64 gate and exact pair test of bodies i < j; a hit bumps its row's counters and goes to
+// the unsorted hit list
+__device__ __forceinline__ void enc_exact_body(const EncFindParams& p, int i, int j) {
     if (i >= p.s.nbig) return;                 // first member must be a big body
     const double4 bi = p.e.box[i], bj = p.e.box[j];
     if (!gate_f64(bi, bj)) return;
@@ -371,6 +372,86 @@ __device__ __forceinline__ void enc_exact(const EncFindParams& p, int2 c) {
     atomicAdd(&p.e.tilecnt[i / TJ], 1);
     const unsigned long long pos = atomicAdd(p.e.nhit, 1ull);
     if ((long long)pos < p.cap) p.e.hits[pos] = make_int2(i, j);
+}
+
+// one survivor per lane (sorted positions c.x < c.y): (i, j) = (smaller, larger) body index
+__device__ __forceinline__ void enc_exact(const EncFindParams& p, int2 c) {
+    const int ba = p.e.perm[c.x], bb = p.e.perm[c.y];
+    enc_exact_body(p, min(ba, bb), max(ba, bb));
+}
+
+// ---- big x all find for few big bodies (`do i = 2, nbig` x `do j = i+1, nbod`
+// with N_big <= ~100).  No spatial ordering: the nbig x nb rectangle of FP32 gates is
+// small (1e8 at nb = 1e6, nbig = 100).  Every thread keeps BIGF_JPT bodies j (body order) in
+// registers and sweeps the big boxes i < j, staged BIGF_CHUNK at a time in shared memory (one
+// broadcast LDS.128 + 4 FSETP per gate); the rare survivors go straight through the exact test.
+constexpr int BIGF_THREADS = 256;
+constexpr int BIGF_JPT = 4;
+constexpr int BIGF_CHUNK = 1024;
+constexpr int BIGF_BATCH = 4;              // big boxes gated between two survivor checks
+constexpr int BIGF_QCAP = 64;              // per-warp survivor queue (a drain leaves < 32)
+
+__global__ void __launch_bounds__(BIGF_THREADS) enc_bigfind_kernel(EncFindParams p) {
+    __shared__ float4 sbig[BIGF_CHUNK];
+    __shared__ int2 s_q[BIGF_THREADS / 32][BIGF_QCAP];
+    const int tid = threadIdx.x, lane = tid & 31;
+    const unsigned full = 0xffffffffu, lt = (1u << lane) - 1u;
+    const int jbase = blockIdx.x * (BIGF_THREADS * BIGF_JPT) + tid;
+    float4 bj[BIGF_JPT];
+#pragma unroll
+    for (int k = 0; k < BIGF_JPT; ++k) {
+        const int j = jbase + k * BIGF_THREADS;
+        bj[k] = j < p.s.nb ? p.e.boxf[j] : pad_boxf();
+    }
+    int2* q = s_q[tid >> 5];
+    int qhead = 0, qn = 0;                     // warp-uniform
+    const int jmax = min(p.s.nb, (int)(blockIdx.x + 1) * (BIGF_THREADS * BIGF_JPT)) - 1;   // largest j of this CTA
+    const int ilim = min(p.s.nbig, jmax);                                                  // rows i < j <= jmax
+    for (int i0 = 0; i0 < ilim; i0 += BIGF_CHUNK) {
+        const int n = min(BIGF_CHUNK, ilim - i0);
+        const int npad = (n + BIGF_BATCH - 1) / BIGF_BATCH * BIGF_BATCH;
+        __syncthreads();
+        for (int t = tid; t < npad; t += BIGF_THREADS) sbig[t] = t < n ? p.e.boxf[i0 + t] : pad_boxf();
+        __syncthreads();
+#pragma unroll 1
+        for (int ii = 0; ii < npad; ii += BIGF_BATCH) {
+            bool any = false;
+#pragma unroll
+            for (int u = 0; u < BIGF_BATCH; ++u) {
+                const float4 bi = sbig[ii + u];
+#pragma unroll
+                for (int k = 0; k < BIGF_JPT; ++k) any |= gate_f32(bi, bj[k]);
+            }
+            if (__any_sync(full, any)) {       // some lane has a survivor in this batch
+#pragma unroll 1
+                for (int u = 0; u < BIGF_BATCH; ++u) {
+                    const float4 bi = sbig[ii + u];
+                    const int i = i0 + ii + u;
+#pragma unroll
+                    for (int k = 0; k < BIGF_JPT; ++k) {
+                        const int j = jbase + k * BIGF_THREADS;
+                        const bool has = gate_f32(bi, bj[k]) && (i < j);
+                        const unsigned bal = __ballot_sync(full, has);
+                        if (bal == 0u) continue;
+                        if (has) q[(qhead + qn + __popc(bal & lt)) & (BIGF_QCAP - 1)] = make_int2(i, j);
+                        qn += __popc(bal);
+                        __syncwarp();
+                        if (qn >= 32) {        // a full warp of survivors through the exact test
+                            const int2 c = q[(qhead + lane) & (BIGF_QCAP - 1)];
+                            enc_exact_body(p, c.x, c.y);
+                            qhead = (qhead + 32) & (BIGF_QCAP - 1);
+                            qn -= 32;
+                            __syncwarp();
+                        }
+                    }
+                }
+            }
+        }
+    }
+    if (lane < qn) {
+        const int2 c = q[(qhead + lane) & (BIGF_QCAP - 1)];
+        enc_exact_body(p, c.x, c.y);
+    }
 }
 
 // CTA (rb, y) owns the rb-th run of TJ sorted boxes (one per compute thread) and visits the column
@@ -510,6 +591,7 @@ __global__ void __launch_bounds__(TJ) enc_scan_kernel(EncBuf e, int nTiles, long
         wbase += (k < warp) ? wrow[k] : 0;
     }
     e.rowoff[blk * TJ + tid] = base + wbase + (incl - c);
+    if (c > ENC_RANK_LONG && total <= cap) e.longrows[atomicAdd(e.nlong, 1)] = blk * TJ + tid;
     if (blk == 0 && tid == 0) {
         st->nce_last = total;
         st->nce_total += total;
@@ -533,20 +615,59 @@ __global__ void __launch_bounds__(256) enc_scatter_kernel(EncBuf e, uint8_t* __r
     }
 }
 
+// short rows (<= ENC_RANK_LONG hits): every hit ranks itself among the j's of its row.  Long rows
+// (a giant planet's row holds thousands of hits; the scan listed them): the row's j's are dealt in
+// blocks of 256 to CTAs, which stream the whole row through shared memory and count, per element,
+// the smaller j's (4 compares per LDS.128).
+constexpr int ENC_RANK_TILE = 2048;
 __global__ void __launch_bounds__(256) enc_rank_kernel(EncBuf e, int* __restrict__ pairs) {
+    __shared__ __align__(16) int s_key[ENC_RANK_TILE];
     if (*e.ovf_now) return;
     const unsigned long long n = *e.nhit;
     for (unsigned long long h = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x; h < n;
          h += (unsigned long long)gridDim.x * blockDim.x) {
         const int2 c = e.hits[h];
-        const long long off = e.rowoff[c.x];
         const int cnt = e.rowcnt[c.x];
+        if (cnt > ENC_RANK_LONG) continue;
+        const long long off = e.rowoff[c.x];
         const int* seg = e.tmpj + off;
         int rank = 0;
         for (int k = 0; k < cnt; ++k) rank += (seg[k] < c.y) ? 1 : 0;   // the j's of a row are distinct
         const long long pos = off + rank;
         pairs[2 * pos] = c.x;
         pairs[2 * pos + 1] = c.y;
+    }
+    const int nlong = *e.nlong;
+    int ubase = 0;                                                       // units before this row (CTA-uniform)
+    for (int L = 0; L < nlong; ++L) {
+        const int row = e.longrows[L];
+        const int cnt = e.rowcnt[row];
+        const long long off = e.rowoff[row];
+        const int* seg = e.tmpj + off;
+        const int nblk = (cnt + 255) / 256;
+        int u = ubase + ((int)blockIdx.x - ubase % (int)gridDim.x + (int)gridDim.x) % (int)gridDim.x;
+        for (; u < ubase + nblk; u += gridDim.x) {
+            const int k = (u - ubase) * 256 + threadIdx.x;
+            const int j = k < cnt ? seg[k] : 0;
+            int rank = 0;
+            for (int t0 = 0; t0 < cnt; t0 += ENC_RANK_TILE) {
+                __syncthreads();
+                for (int q = threadIdx.x; q < ENC_RANK_TILE; q += 256) s_key[q] = (t0 + q < cnt) ? seg[t0 + q] : 0x7fffffff;
+                __syncthreads();
+                const int4* t4 = reinterpret_cast<const int4*>(s_key);
+                const int lim = min(ENC_RANK_TILE, (cnt - t0 + 3) & ~3) / 4;
+#pragma unroll 4
+                for (int q = 0; q < lim; ++q) {
+                    const int4 v = t4[q];
+                    rank += (v.x < j) + (v.y < j) + (v.z < j) + (v.w < j);
+                }
+            }
+            if (k < cnt) {
+                pairs[2 * (off + rank)] = row;
+                pairs[2 * (off + rank) + 1] = j;
+            }
+        }
+        ubase += nblk;
     }
 }
 

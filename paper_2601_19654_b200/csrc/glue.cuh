@@ -16,7 +16,7 @@ namespace mopal {
 template <bool KICK>
 __global__ void __launch_bounds__(ON_BLOCK) kick_psum_kernel(double* __restrict__ v, const double* __restrict__ a,
                                                               const double* __restrict__ gm, int nb, int ld,
-                                                              double hk, double* __restrict__ psum) {
+                                                              double hk, double* psum, unsigned* ticket) {
     __shared__ double sh[ON_BLOCK / 32][3];
     const int b = blockIdx.x * ON_BLOCK + threadIdx.x;
     double s0 = 0, s1 = 0, s2 = 0;
@@ -31,6 +31,7 @@ __global__ void __launch_bounds__(ON_BLOCK) kick_psum_kernel(double* __restrict_
     }
     block_sum3<ON_BLOCK>(s0, s1, s2, sh);
     if (threadIdx.x == 0) { psum[3 * blockIdx.x] = s0; psum[3 * blockIdx.x + 1] = s1; psum[3 * blockIdx.x + 2] = s2; }
+    psum_finalize<ON_BLOCK>(psum, gridDim.x, ticket, sh);
 }
 
 struct MidParams {
@@ -38,6 +39,7 @@ struct MidParams {
     const double *gm, *rcrit;
     const double* psum_in;  // partials of sum gm v before the drift
     double* psum_out;       // partials after the drift
+    unsigned* ticket;       // last-block counter of psum_out
     EncBuf enc;
     uint8_t* flag;
     DevStats* st;
@@ -49,11 +51,11 @@ __global__ void __launch_bounds__(ON_BLOCK) jump_drift_boxes_kernel(MidParams p)
     __shared__ double sh[ON_BLOCK / 32][3];
     __shared__ float4 sh4[ON_BLOCK / 32];
     double P0, P1, P2;
-    reduce_psum(p.psum_in, p.npsum, sh, P0, P1, P2);
+    load_psum(p.psum_in, p.npsum, P0, P1, P2);
     const int b = blockIdx.x * ON_BLOCK + threadIdx.x;
     double s0 = 0, s1 = 0, s2 = 0;
     float4 bf = pad_boxf();
-    if (b == 0) *p.enc.nhit = 0ull;
+    if (b == 0) { *p.enc.nhit = 0ull; *p.enc.nlong = 0; }
     if (b < p.nbPad) { p.enc.rowcnt[b] = 0; p.enc.rowfill[b] = 0; }
     if (b < p.nb) {
         const int ld = p.ld;
@@ -87,6 +89,7 @@ __global__ void __launch_bounds__(ON_BLOCK) jump_drift_boxes_kernel(MidParams p)
     }
     block_sum3<ON_BLOCK>(s0, s1, s2, sh);
     if (threadIdx.x == 0) { p.psum_out[3 * blockIdx.x] = s0; p.psum_out[3 * blockIdx.x + 1] = s1; p.psum_out[3 * blockIdx.x + 2] = s2; }
+    psum_finalize<ON_BLOCK>(p.psum_out, p.npsum, p.ticket, sh);
     enc_bounds_partial(p.enc, b < p.nb, bf, sh4, p.nbPad / TJ);
 }
 

@@ -11,6 +11,7 @@
 
 #include "../../include/mopal.h"
 #include "glue.cuh"
+#include "pair_big.cuh"
 #include "pair_sym.cuh"
 
 using namespace mopal;
@@ -29,6 +30,7 @@ struct mo_ctx {
     cudaStream_t cap_stream = nullptr;  // owned: graph capture needs a non-legacy stream
     // owned scratch
     double *gm = nullptr, *x0 = nullptr, *v0 = nullptr, *part = nullptr, *psumA = nullptr, *psumB = nullptr;
+    unsigned* ticket = nullptr;         // two last-block counters (psumA, psumB)
     unsigned char* tiles = nullptr;
     EncBuf enc = {};
     DevStats* dstats = nullptr;
@@ -40,6 +42,10 @@ struct mo_ctx {
     // two-sided pair kernel (nb >= MO_SYM_MIN): work units and partial buffers
     int enc_split = 1;
     bool use_sym = false;
+    // few gravity sources (mo_set_nbig with nbig <= MO_BIG_MAX): sources in shared memory, direct big-row encounter pass
+    bool use_big = false;
+    int big_ipt = 1;
+    int gkernels = 0;                   // kernel launches recorded in the cached step graph
     int sym_nI = 0, sym_ch = 1, sym_nunits = 0;
     int4* sym_units = nullptr;
     int* sym_ustart = nullptr;
@@ -132,6 +138,16 @@ static void choose_geometry(mo_ctx* ctx) {
     if (ctx->enc_split < 1) ctx->enc_split = 1;
     if (ctx->enc_split > 8) ctx->enc_split = 8;
     // two-sided kernel for large nb: units = (row block, chunk of sym_ch j tiles from the diagonal on)
+    ctx->use_big = ctx->nbig < nb && ctx->nbig <= env_int("MO_BIG_MAX", 4096);
+    if (ctx->use_big) {
+        // bodies per thread: as many as still leave about two waves of CTAs
+        const long long want = 2LL * ctx->nsm * BIG_THREADS;
+        ctx->big_ipt = env_int("MO_BIG_IPT", nb >= 4 * want ? 4 : nb >= 2 * want ? 2 : 1);
+        if (ctx->big_ipt != 1 && ctx->big_ipt != 2 && ctx->big_ipt != 4) ctx->big_ipt = 1;
+        ctx->ipt = ctx->big_ipt; ctx->nsplit = 1; ctx->tps = ctx->nSrcTiles;
+        ctx->nIblk = (nb + BIG_THREADS * ctx->big_ipt - 1) / (BIG_THREADS * ctx->big_ipt);
+        ctx->ctas_per_sm = 0;
+    }
     ctx->use_sym = ctx->nbig == nb && env_int("MO_SYM", nb >= env_int("MO_SYM_MIN", 8192) ? 1 : 0) != 0;
     if (ctx->use_sym) {
         int occs = 1;
@@ -180,14 +196,14 @@ extern "C" void mo_destroy(mo_ctx* ctx) {
     if (ctx->cap_stream) cudaStreamDestroy(ctx->cap_stream);
     for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
     cudaFree(ctx->gm); cudaFree(ctx->x0); cudaFree(ctx->v0); cudaFree(ctx->part);
-    cudaFree(ctx->psumA); cudaFree(ctx->psumB); cudaFree(ctx->tiles);
+    cudaFree(ctx->psumA); cudaFree(ctx->psumB); cudaFree(ctx->ticket); cudaFree(ctx->tiles);
     cudaFree(ctx->sym_units); cudaFree(ctx->sym_ustart); cudaFree(ctx->sym_partI); cudaFree(ctx->sym_partJ);
     cudaFree(ctx->enc.box); cudaFree(ctx->enc.boxf); cudaFree(ctx->enc.rowcnt); cudaFree(ctx->enc.rowfill);
     cudaFree(ctx->enc.rowoff); cudaFree(ctx->enc.hits); cudaFree(ctx->enc.tmpj); cudaFree(ctx->enc.nhit);
     cudaFree(ctx->enc.ovf_now); cudaFree(ctx->dstats); cudaFree(ctx->probe);
     cudaFree(ctx->enc.bpart); cudaFree(ctx->enc.cellcnt); cudaFree(ctx->enc.cellfill); cudaFree(ctx->enc.key);
     cudaFree(ctx->enc.perm); cudaFree(ctx->enc.sboxf); cudaFree(ctx->enc.tbox); cudaFree(ctx->enc.tilecnt);
-    cudaFree(ctx->enc.tbig);
+    cudaFree(ctx->enc.tbig); cudaFree(ctx->enc.nlong); cudaFree(ctx->enc.longrows);
     if (ctx->hstats) cudaFreeHost(ctx->hstats);
     delete ctx;
 }
@@ -227,8 +243,10 @@ extern "C" mo_status mo_create(mo_ctx** out, int32_t nb, int32_t ld, double m_st
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->gm, (size_t)nb);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->x0, pl);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->v0, pl);
-    if (e == cudaSuccess) e = dalloc(ctx, &ctx->psumA, 3 * (size_t)ctx->npsum);
-    if (e == cudaSuccess) e = dalloc(ctx, &ctx->psumB, 3 * (size_t)ctx->npsum);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->psumA, 3 * (size_t)ctx->npsum + 3);   // partials + their sum
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->psumB, 3 * (size_t)ctx->npsum + 3);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->ticket, 2);
+    if (e == cudaSuccess) e = cudaMemsetAsync(ctx->ticket, 0, 2 * sizeof(unsigned), ctx->stream);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->tiles, (size_t)ctx->nTiles * ACC_TILE_BYTES);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->enc.box, (size_t)ctx->nbPad);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->enc.boxf, (size_t)ctx->nbPad);
@@ -248,6 +266,8 @@ extern "C" mo_status mo_create(mo_ctx** out, int32_t nb, int32_t ld, double m_st
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->enc.tbox, (size_t)ctx->nTiles);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->enc.tilecnt, (size_t)ctx->nTiles);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->enc.tbig, (size_t)ctx->nTiles);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->enc.nlong, 1);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->enc.longrows, (size_t)(cap / ENC_RANK_LONG + 1));
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->dstats, 1);
     if (e == cudaSuccess) e = cudaMallocHost(reinterpret_cast<void**>(&ctx->hstats), sizeof(DevStats));
     if (e != cudaSuccess) {
@@ -274,7 +294,7 @@ static mo_status ensure_pair_scratch(mo_ctx* ctx) {
     if (ctx->pair_ready) return MO_OK;
     cudaError_t e = cudaSuccess;
     const size_t pl = 3 * (size_t)ctx->ld;
-    if (!ctx->use_sym) e = dalloc(ctx, &ctx->part, pl * (size_t)ctx->nsplit);
+    if (!ctx->use_sym && !ctx->use_big) e = dalloc(ctx, &ctx->part, pl * (size_t)ctx->nsplit);
     if (ctx->use_sym) {
         if (e == cudaSuccess) e = dalloc(ctx, &ctx->sym_units, (size_t)ctx->sym_nunits);
         if (e == cudaSuccess) e = dalloc(ctx, &ctx->sym_ustart, ctx->h_ustart.size());
@@ -293,7 +313,15 @@ static mo_status ensure_pair_scratch(mo_ctx* ctx) {
     return MO_OK;
 }
 
-static mo_status launch_pair(mo_ctx* ctx) {
+typedef void (*big_kernel_t)(BigParams);
+static big_kernel_t pick_big_kernel(int ipt, bool kick) {
+    if (ipt == 4 && env_int("MO_BIG_U", 1) == 2) return kick ? pair_big_kernel<4, 2, true> : pair_big_kernel<4, 2, false>;
+    if (ipt == 4) return kick ? pair_big_kernel<4, 1, true> : pair_big_kernel<4, 1, false>;
+    if (ipt == 2) return kick ? pair_big_kernel<2, 2, true> : pair_big_kernel<2, 2, false>;
+    return kick ? pair_big_kernel<1, 4, true> : pair_big_kernel<1, 4, false>;
+}
+
+static mo_status launch_pair(mo_ctx* ctx, bool kick = false, double hk = 0.0) {
     AccelParams p;
     p.tiles = ctx->tiles; p.x = ctx->x; p.rcrit = ctx->rcrit; p.part = ctx->part;
     p.nb = ctx->nb; p.ld = ctx->ld; p.nTiles = ctx->nSrcTiles; p.tps = ctx->tps;
@@ -309,7 +337,12 @@ static mo_status launch_pair(mo_ctx* ctx) {
         ctx->ev_used += 2;
         CK(cudaEventRecord(e0, ctx->stream));
     }
-    if (ctx->use_sym) {
+    if (ctx->use_big) {
+        BigParams bp;
+        bp.x = ctx->x; bp.gm = ctx->gm; bp.rcrit = ctx->rcrit; bp.a = ctx->a; bp.v = ctx->v;
+        bp.nb = ctx->nb; bp.nbig = ctx->nbig; bp.ld = ctx->ld; bp.hk = hk;
+        pick_big_kernel(ctx->big_ipt, kick)<<<ctx->nIblk, BIG_THREADS, 0, ctx->stream>>>(bp);
+    } else if (ctx->use_sym) {
         SymParams sp;
         sp.tiles = ctx->tiles; sp.x = ctx->x; sp.gm = ctx->gm; sp.rcrit = ctx->rcrit; sp.units = ctx->sym_units;
         sp.partI = ctx->sym_partI; sp.partJ = ctx->sym_partJ; sp.nb = ctx->nb; sp.ld = ctx->ld; sp.nbPad = ctx->nbPad;
@@ -326,6 +359,17 @@ static mo_status enqueue_accel(mo_ctx* ctx, bool jump, double hj, bool kick, dou
     const double hjm = jump ? hj / ctx->mu : 0.0;
     const double* ps = jump ? ctx->psumB : nullptr;
     const int nps = jump ? ctx->npsum : 0;
+    if (ctx->use_big) {
+        // the jump still moves every body (pack_kernel also refreshes the few source tiles, unused here);
+        // pair_big_kernel reads the sources from x, writes a itself and applies the closing kick
+        if (jump) {
+            pack_kernel<true, false><<<ctx->nTiles, TJ, 0, ctx->stream>>>(ctx->x, ctx->gm, ctx->rcrit, ctx->nb, ctx->nbig, ctx->ld,
+                                                                        ctx->tiles, ps, nps, hjm);
+            mo_status s = post_launch(ctx);
+            if (s != MO_OK) return s;
+        }
+        return launch_pair(ctx, kick, hk);
+    }
     auto pk = jump ? (ctx->use_sym ? pack_kernel<true, true> : pack_kernel<true, false>)
                    : (ctx->use_sym ? pack_kernel<false, true> : pack_kernel<false, false>);
     pk<<<jump ? ctx->nTiles : ctx->nSrcTiles, TJ, 0, ctx->stream>>>(ctx->x, ctx->gm, ctx->rcrit, ctx->nb, ctx->nbig, ctx->ld,
@@ -355,22 +399,32 @@ static EncState enc_state(const mo_ctx* ctx, const double* x0, const double* v0,
 
 // find + scan + place (+ overflow fallback) on boxes already in ctx->enc (counters already zeroed)
 static mo_status enqueue_pairs(mo_ctx* ctx, const EncState& es, int step_inc) {
-    // spatial ordering of this pass (performance only): cell keys, counting sort, tile bounding boxes
-    enc_key_kernel<<<ctx->npsum, ON_BLOCK, 0, ctx->stream>>>(ctx->enc, ctx->nb, ctx->nbPad, ctx->npsum);
-    mo_status s = post_launch(ctx);
-    if (s != MO_OK) return s;
-    enc_sortscatter_kernel<<<ctx->npsum, ON_BLOCK, 0, ctx->stream>>>(ctx->enc, ctx->nb, ctx->nbPad);
-    s = post_launch(ctx);
-    if (s != MO_OK) return s;
-    enc_tilebox_kernel<<<ctx->nTiles, TJ, 0, ctx->stream>>>(ctx->enc, ctx->nbig);
-    s = post_launch(ctx);
-    if (s != MO_OK) return s;
     EncFindParams fp;
     fp.s = es; fp.e = ctx->enc; fp.cap = ctx->cap; fp.nTiles = ctx->nTiles;
-    enc_find_kernel<<<dim3(ctx->nTiles, ctx->enc_split), CTA_THREADS, 0, ctx->stream>>>(fp);
-    s = post_launch(ctx);
-    if (s != MO_OK) return s;
-    enc_scan_kernel<<<ctx->nTiles, TJ, 0, ctx->stream>>>(ctx->enc, ctx->nTiles, ctx->cap, step_inc, ctx->dstats);
+    mo_status s;
+    if (ctx->use_big) {
+        // few big bodies: the nbig x nb rectangle of gates directly, in body order
+        const int per = BIGF_THREADS * BIGF_JPT;
+        enc_bigfind_kernel<<<(ctx->nb + per - 1) / per, BIGF_THREADS, 0, ctx->stream>>>(fp);
+        s = post_launch(ctx);
+        if (s != MO_OK) return s;
+    } else {
+        // spatial ordering of this pass (performance only): cell keys, counting sort, tile bounding boxes
+        enc_key_kernel<<<ctx->npsum, ON_BLOCK, 0, ctx->stream>>>(ctx->enc, ctx->nb, ctx->nbPad, ctx->npsum);
+        s = post_launch(ctx);
+        if (s != MO_OK) return s;
+        enc_sortscatter_kernel<<<ctx->npsum, ON_BLOCK, 0, ctx->stream>>>(ctx->enc, ctx->nb, ctx->nbPad);
+        s = post_launch(ctx);
+        if (s != MO_OK) return s;
+        enc_tilebox_kernel<<<ctx->nTiles, TJ, 0, ctx->stream>>>(ctx->enc, ctx->nbig);
+        s = post_launch(ctx);
+        if (s != MO_OK) return s;
+        enc_find_kernel<<<dim3(ctx->nTiles, ctx->enc_split), CTA_THREADS, 0, ctx->stream>>>(fp);
+        s = post_launch(ctx);
+        if (s != MO_OK) return s;
+    }
+    // rows >= nbig hold no hits: only the tiles of the big rows are scanned
+    enc_scan_kernel<<<ctx->nSrcTiles, TJ, 0, ctx->stream>>>(ctx->enc, ctx->nSrcTiles, ctx->cap, step_inc, ctx->dstats);
     s = post_launch(ctx);
     if (s != MO_OK) return s;
     const int pblocks = ctx->nsm * 2;
@@ -390,12 +444,12 @@ static mo_status enqueue_pairs(mo_ctx* ctx, const EncState& es, int step_inc) {
 }
 
 static mo_status enqueue_step(mo_ctx* ctx, double dt) {
-    kick_psum_kernel<true><<<ctx->npsum, ON_BLOCK, 0, ctx->stream>>>(ctx->v, ctx->a, ctx->gm, ctx->nb, ctx->ld, 0.5 * dt, ctx->psumA);
+    kick_psum_kernel<true><<<ctx->npsum, ON_BLOCK, 0, ctx->stream>>>(ctx->v, ctx->a, ctx->gm, ctx->nb, ctx->ld, 0.5 * dt, ctx->psumA, ctx->ticket);
     mo_status s = post_launch(ctx);
     if (s != MO_OK) return s;
     MidParams mp;
     mp.x = ctx->x; mp.v = ctx->v; mp.x0 = ctx->x0; mp.v0 = ctx->v0; mp.gm = ctx->gm; mp.rcrit = ctx->rcrit;
-    mp.psum_in = ctx->psumA; mp.psum_out = ctx->psumB; mp.enc = ctx->enc; mp.flag = ctx->flag;
+    mp.psum_in = ctx->psumA; mp.psum_out = ctx->psumB; mp.ticket = ctx->ticket + 1; mp.enc = ctx->enc; mp.flag = ctx->flag;
     mp.st = ctx->dstats; mp.nb = ctx->nb; mp.ld = ctx->ld; mp.nbPad = ctx->nbPad; mp.npsum = ctx->npsum;
     mp.nbig = ctx->nbig;
     mp.hj_over_mu = 0.5 * dt / ctx->mu; mp.mu = ctx->mu; mp.h = dt;
@@ -406,7 +460,6 @@ static mo_status enqueue_step(mo_ctx* ctx, double dt) {
     if (s != MO_OK) return s;
     return enqueue_accel(ctx, true, 0.5 * dt, true, 0.5 * dt);
 }
-static const int KERNELS_PER_STEP = 13;
 
 static mo_status read_stats(mo_ctx* ctx, mo_stats* out, bool* overflow) {
     CK(cudaMemcpyAsync(ctx->hstats, ctx->dstats, sizeof(DevStats), cudaMemcpyDeviceToHost, ctx->stream));
@@ -545,6 +598,7 @@ extern "C" mo_status mo_step(mo_ctx* ctx, double dt, int32_t nsteps, mo_stats* s
             s = enqueue_step(ctx, dt);
             ctx->stream = user;
             cudaError_t e = cudaStreamEndCapture(ctx->cap_stream, &g);
+            ctx->gkernels = (int)(ctx->launches - l0);
             ctx->launches = l0;  // captured, not launched
             if (s != MO_OK || e != cudaSuccess) {
                 if (g) cudaGraphDestroy(g);
@@ -559,7 +613,7 @@ extern "C" mo_status mo_step(mo_ctx* ctx, double dt, int32_t nsteps, mo_stats* s
         }
         for (int k = 0; k < nsteps; ++k) {
             CK(cudaGraphLaunch(ctx->gexec, ctx->stream));
-            ctx->launches += KERNELS_PER_STEP;
+            ctx->launches += ctx->gkernels;
         }
     } else {
         for (int k = 0; k < nsteps; ++k) {
@@ -585,6 +639,12 @@ extern "C" mo_status mo_pair_geometry(const mo_ctx* ctx, int32_t* ipt, int32_t* 
     if (ipt) *ipt = ctx->ipt;
     if (jsplit) *jsplit = ctx->nsplit;
     if (ctas) *ctas = ctx->use_sym ? ctx->sym_nunits : ctx->nIblk * ctx->nsplit;
+    if (ctx->use_big && ctas_per_sm) {
+        int occ = 0;
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, pick_big_kernel(ctx->big_ipt, true), BIG_THREADS, 0);
+        *ctas_per_sm = occ;
+        return MO_OK;
+    }
     if (ctx->use_sym && jsplit) *jsplit = ctx->sym_ch;
     if (ctas_per_sm) *ctas_per_sm = ctx->ctas_per_sm;
     return MO_OK;

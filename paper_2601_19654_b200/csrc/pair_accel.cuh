@@ -181,23 +181,31 @@ __global__ void __launch_bounds__(ON_BLOCK) accel_reduce_kernel(const double* __
 // PAPER.md:209-219) using the block partial sums of gm*v.
 constexpr double PAD_POS = 1.0e15;  // pad bodies: far away and massless -> contribute exactly 0
 
-__device__ __forceinline__ void reduce_psum(const double* __restrict__ psum, int npsum, double (*sh)[3],
-                                            double& P0, double& P1, double& P2) {
-    // every block reduces the same partials in the same fixed order
-    double s0 = 0, s1 = 0, s2 = 0;
-    if (threadIdx.x < 32) {
-        for (int b = threadIdx.x; b < npsum; b += 32) { s0 += psum[3 * b]; s1 += psum[3 * b + 1]; s2 += psum[3 * b + 2]; }
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            s0 += __shfl_down_sync(0xffffffffu, s0, o);
-            s1 += __shfl_down_sync(0xffffffffu, s1, o);
-            s2 += __shfl_down_sync(0xffffffffu, s2, o);
-        }
-        if (threadIdx.x == 0) { sh[0][0] = s0; sh[0][1] = s1; sh[0][2] = s2; }
+// Sum of gm v (Hamiltonian block LOOP 2): every block of the producing kernel
+// writes a partial; the block that arrives last (ticket counter) adds the partials in index order
+// - the same order whichever block that is - into psum[3 npsum ..], which the next kernel reads.
+template <int BLOCK>
+__device__ __forceinline__ void psum_finalize(double* psum, int npsum, unsigned* ticket, double (*sh)[3]) {
+    __shared__ bool s_last;
+    if (threadIdx.x == 0) {
+        __threadfence();                                   // the partial is visible before the ticket
+        s_last = atomicAdd(ticket, 1u) == gridDim.x - 1;
     }
     __syncthreads();
-    P0 = sh[0][0]; P1 = sh[0][1]; P2 = sh[0][2];
-    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    double s0 = 0, s1 = 0, s2 = 0;
+    for (int b = threadIdx.x; b < npsum; b += BLOCK) {
+        s0 += __ldcg(psum + 3 * b); s1 += __ldcg(psum + 3 * b + 1); s2 += __ldcg(psum + 3 * b + 2);
+    }
+    block_sum3<BLOCK>(s0, s1, s2, sh);
+    if (threadIdx.x == 0) {
+        psum[3 * npsum] = s0; psum[3 * npsum + 1] = s1; psum[3 * npsum + 2] = s2;
+        *ticket = 0u;                                      // ready for the next launch
+    }
+}
+__device__ __forceinline__ void load_psum(const double* __restrict__ psum, int npsum, double& P0, double& P1, double& P2) {
+    P0 = psum[3 * npsum]; P1 = psum[3 * npsum + 1]; P2 = psum[3 * npsum + 2];
 }
 
 // SYM selects the tile layout: false = TJ records {x,y,z,gm} (pair_accel_kernel, broadcast reads),
@@ -210,12 +218,11 @@ __global__ void __launch_bounds__(TJ) pack_kernel(double* __restrict__ x, const 
                                                   const double* __restrict__ rcrit, int nb, int nsrc, int ld,
                                                   unsigned char* __restrict__ tiles,
                                                   const double* __restrict__ psum, int npsum, double hj_over_mu) {
-    __shared__ double sh[TJ / 32][3];
     __shared__ int sg[TJ / 32];
     double sx = 0, sy = 0, sz = 0;
     if (JUMP) {
         double P0, P1, P2;
-        reduce_psum(psum, npsum, sh, P0, P1, P2);
+        load_psum(psum, npsum, P0, P1, P2);
         sx = hj_over_mu * P0; sy = hj_over_mu * P1; sz = hj_over_mu * P2;
     }
     const int j = blockIdx.x * TJ + threadIdx.x;

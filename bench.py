@@ -41,6 +41,8 @@ FP64_LANES_PER_SM = 64        # DESIGN.md section "Rooflines": 148 SMs x 64 DFMA
 # executed FP64 flops per ORDERED pair of the two-sided kernel: 3 DADD + 6 DMUL + 11 DFMA = 31 flop per
 # unordered pair (pair_sym.cuh; the ncu dadd/dmul/dfma counters in profiles/ show the same 3 : 6 : 11 mix)
 EXECUTED_FLOP_PER_PAIR = 15.5
+# one-sided kernels (pair_accel_kernel, pair_big_kernel): 3 DADD + 5 DMUL + 8 DFMA per ordered pair
+EXECUTED_FLOP_PER_PAIR_ONE_SIDED = 24.0
 # dram__bytes_read.sum + dram__bytes_write.sum of one pair_sym_kernel launch at config 3 from the
 # ncu --set full capture summarised in profiles/r1c_pair_sym_full.md (5.1 MB read + 91.1 MB written)
 PAIR_KERNEL_DRAM_TRAFFIC_BYTES = {3: 96.3e6}
@@ -125,7 +127,22 @@ def _host_cores() -> int:
 
 
 # --------------------------------------------------------------------------- CPU oracle leg
-def oracle_step_sample(w, budget_s: float, kind: str = "ld"):
+def _workload(args):
+    """(workload, nbig or None): BASELINE.json config, or with --bigsmall N,NBIG the paper's production
+    regime - SURVEY.md 8(f) row 1, not a BASELINE.json config."""
+    from paper_2601_19654_b200 import workloads as W
+    if args.bigsmall:
+        N, nbig = (int(t) for t in args.bigsmall.split(","))
+        return W.make_bigsmall(N, nbig), nbig
+    return W.make_config(args.config), None
+
+
+def _pairs_per_step(w, nbig):
+    """ordered (sink i, source j != i) evaluations of one mo_accel"""
+    return w.nb * (w.nb - 1) if nbig is None else w.nb * nbig - nbig
+
+
+def oracle_step_sample(w, budget_s: float, kind: str = "ld", nbig=None):
     """Times the oracle on a bounded sample of ONE hybrid step of workload w and scales it to
     the whole step: R sampled rows of the pair sum (each row is the full ascending-j loop),
     a strided row sample of the encounter pass, and the full O(N) drift.  Returns
@@ -138,16 +155,16 @@ def oracle_step_sample(w, budget_s: float, kind: str = "ld"):
     t_start = time.perf_counter()
     # calibrate on a few rows, then size the sample for the budget
     rows = np.arange(0, nb, max(1, nb // (4 * cores)), dtype=np.int32)[: 4 * cores]
-    t0 = time.perf_counter(); oracle.accel_rows(gm, w.x, w.rcrit, rows, kind=kind); t1 = time.perf_counter()
+    t0 = time.perf_counter(); oracle.accel_rows(gm, w.x, w.rcrit, rows, kind=kind, nbig=nbig); t1 = time.perf_counter()
     per_row = (t1 - t0) / len(rows)
     R = int(min(nb, max(len(rows), 0.6 * budget_s / max(per_row, 1e-9))))
     rows = np.unique(np.linspace(0, nb - 1, R).astype(np.int32))
-    t0 = time.perf_counter(); oracle.accel_rows(gm, w.x, w.rcrit, rows, kind=kind); t_acc = time.perf_counter() - t0
+    t0 = time.perf_counter(); oracle.accel_rows(gm, w.x, w.rcrit, rows, kind=kind, nbig=nbig); t_acc = time.perf_counter() - t0
     t0 = time.perf_counter(); x1, v1, _ = oracle.drift(mu, w.dt, w.x, w.v, kind=kind); t_drift = time.perf_counter() - t0
     # encounter rows i % stride == 0 see on average the same number of j > i as any other phase
-    stride = int(max(1, round(nb / max(len(rows) * 2, 1))))
+    stride = int(max(1, round(nb / max(len(rows) * 2, 1)))) if nbig is None else 1     # big x all: only nbig rows, all taken
     t0 = time.perf_counter()
-    oracle.encounters(w.dt, w.x, w.v, x1, v1, w.rcrit, kind=kind, row_stride=stride, row_phase=0)
+    oracle.encounters(w.dt, w.x, w.v, x1, v1, w.rcrit, kind=kind, row_stride=stride, row_phase=0, nbig=nbig, cap=1 << 20)
     t_enc = time.perf_counter() - t0
     est = t_acc * nb / len(rows) + t_enc * stride + t_drift
     what = (f"one hybrid step estimated from {len(rows)} of {nb} pair-sum rows ({t_acc:.2f} s), encounter rows "
@@ -160,15 +177,14 @@ def run_reference(args):
     rank, _, world = _dist_env()
     if rank != 0:
         return 0
-    from paper_2601_19654_b200 import workloads as W
-    w = W.make_config(args.config)
-    pairs = w.nb * (w.nb - 1)
+    w, nbig = _workload(args)
+    pairs = _pairs_per_step(w, nbig)
     cores = _host_cores()
     budget = max(2.0, min(20.0, 150.0 / max(args.steps + args.warmup, 1)))
     est = []
     what = ""
     for k in range(args.warmup + args.steps):
-        e, what, _ = oracle_step_sample(w, budget)
+        e, what, _ = oracle_step_sample(w, budget, nbig=nbig)
         if k >= args.warmup:
             est.append(e)
     sec = sum(est) / len(est)
@@ -176,7 +192,7 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": w.name, "N": w.N, "nb": w.nb, "dt_days": w.dt, "seed": w.seed},
+            "config": {"workload": w.name, "N": w.N, "nb": w.nb, "nbig": w.nb if nbig is None else nbig, "dt_days": w.dt, "seed": w.seed},
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": what},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line), flush=True)
@@ -198,11 +214,16 @@ def run_ours(args):
     from paper_2601_19654_b200 import mopal as M
     from paper_2601_19654_b200 import workloads as W
 
-    w = W.make_config(args.config)
-    nb, pairs = w.nb, w.nb * (w.nb - 1)
+    w, nbig = _workload(args)
+    nb, pairs = w.nb, _pairs_per_step(w, nbig)
     K, Wm = args.steps, max(args.warmup, 3)
     cap = 1 << 20
     m = M.Mopal(w.mass, w.x, w.v, w.rcrit, m_star=w.m_star, G=w.G, cap=cap, device=f"cuda:{dev}")
+    if nbig is not None:
+        m.set_nbig(nbig)
+    kname = m.pair_kernel_name()
+    two_sided = kname == "pair_sym_kernel"
+    exec_flop = EXECUTED_FLOP_PER_PAIR if two_sided else EXECUTED_FLOP_PER_PAIR_ONE_SIDED
     stream = m.stream
     geo = m.pair_geometry()
 
@@ -270,7 +291,7 @@ def run_ours(args):
 
     if rank == 0:
         achieved = FLOP_PER_PAIR * pairs / (pair_ms_max * 1e-3) / 1e12
-        executed = EXECUTED_FLOP_PER_PAIR * pairs / (pair_ms_max * 1e-3) / 1e12
+        executed = exec_flop * pairs / (pair_ms_max * 1e-3) / 1e12
         nsm = torch.cuda.get_device_properties(dev).multi_processor_count
         sm_max = clocks.get("sm_max_mhz") or 1965.0
         nominal = nsm * FP64_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
@@ -278,18 +299,21 @@ def run_ours(args):
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
             "ms_per_step": total_ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
-            "config": {"workload": w.name, "N": w.N, "nb": nb, "dt_days": w.dt, "seed": w.seed,
+            "config": {"workload": w.name, "N": w.N, "nb": nb, "nbig": nb if nbig is None else nbig, "dt_days": w.dt, "seed": w.seed,
                        "parallelism": "single GPU" if world == 1 else f"{world} independent replicas (path does not shard)",
-                       "l2": "flushed (256 MiB memset) between timed steps; the 5.8 MB state is otherwise L2-resident",
+                       "l2": f"flushed (256 MiB memset) between timed steps; the {88 * nb / 1e6:.1f} MB state is otherwise L2-resident",
                        "pair_kernel_geometry": geo, "encounter_pairs_last_step": st1.nce_last},
             "pct_fp64_peak": {"of_measured_sustained": 100 * achieved / peak_sust, "of_measured_burst": 100 * achieved / peak_burst,
                               "of_nominal": 100 * achieved / nominal, "flop_per_pair": FLOP_PER_PAIR},
-            "roofline": {"bound": "alu", "kernel": "pair_sym_kernel", "achieved": achieved, "peak": peak_sust,
+            "roofline": {"bound": "alu", "kernel": kname, "achieved": achieved, "peak": peak_sust,
                          "unit": "TFLOP/s", "frac": achieved / peak_sust,
-                         "traffic": PAIR_KERNEL_DRAM_TRAFFIC_BYTES.get(args.config),
-                         "note": "achieved = 26 algorithmic flop per ORDERED pair (SURVEY.md 8(d)) / kernel time; the kernel "
-                                 "evaluates each unordered pair once (Newton III), so frac can exceed 1; achieved_executed = "
-                                 "the 15.5 flop per ordered pair it really issues (3 DADD + 6 DMUL + 11 DFMA per unordered pair)",
+                         "traffic": PAIR_KERNEL_DRAM_TRAFFIC_BYTES.get(args.config) if two_sided and nbig is None else None,
+                         "note": ("achieved = 26 algorithmic flop per ORDERED pair (SURVEY.md 8(d)) / kernel time; the kernel "
+                                  "evaluates each unordered pair once (Newton III), so frac can exceed 1; achieved_executed = "
+                                  "the 15.5 flop per ordered pair it really issues (3 DADD + 6 DMUL + 11 DFMA per unordered pair)")
+                                 if two_sided else
+                                 ("achieved = 26 algorithmic flop per ordered (sink, source) pair (SURVEY.md 8(d)) / kernel time; "
+                                  "achieved_executed = the 24 flop per pair it issues (3 DADD + 5 DMUL + 8 DFMA)"),
                          "achieved_executed": executed, "frac_executed": executed / peak_sust,
                          "peak_source": "mo_probe_fp64_peak: register-resident DFMA loop on this GPU, 160 launches back to "
                                         "back (sustained); MEASURED_PEAKS.json has no FP64 figure",
@@ -303,7 +327,7 @@ def run_ours(args):
             "wall_s_timed_region": t_wall,
         }
         if not args.no_cpu and world == 1:
-            est, what, _ = oracle_step_sample(w, args.cpu_budget)
+            est, what, _ = oracle_step_sample(w, args.cpu_budget, nbig=nbig)
             line["cpu_baseline"] = {"value": pairs / est, "unit": UNIT, "cores": _host_cores(), "kind": "oracle",
                                     "sample": what, "ms_per_step": est * 1e3}
         print(json.dumps(line), flush=True)
@@ -363,6 +387,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json config index (3 = N=65,536 headline)")
+    ap.add_argument("--bigsmall", default="", metavar="N,NBIG",
+                    help="big x all workload (SURVEY.md 8(f) row 1): N objects, NBIG gravity sources, e.g. 1000000,100")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of CPU work for the cpu_baseline sample")
     ap.add_argument("--drift-sweep", action="store_true", help="time mo_drift alone against the HBM roofline and exit")

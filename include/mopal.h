@@ -170,6 +170,11 @@ mo_status mo_probe_fp64_peak(void *cuda_stream, int32_t reps, double *tflops_out
 mo_status mo_pair_geometry(const mo_ctx *ctx, int32_t *ipt, int32_t *jsplit,
                            int32_t *ctas, int32_t *ctas_per_sm);
 
+/* Name of the pair kernel this context launches for mo_accel ("pair_sym_kernel": two-sided, nb >= 8192
+ * fully interacting; "pair_big_kernel": few gravity sources after mo_set_nbig; else "pair_accel_kernel").
+ * Static string; NULL for a NULL context. */
+const char *mo_pair_kernel_name(const mo_ctx *ctx);
+
 /* Time of the last pair-accel kernel launch alone, measured with CUDA events on the
  * context's stream when timing was enabled with mo_set_kernel_timing(ctx, 1).
  * Synchronises.  ms_out receives the mean over the launches since enabling (and

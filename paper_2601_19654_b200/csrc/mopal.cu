@@ -44,7 +44,7 @@ struct mo_ctx {
     bool use_sym = false;
     // few gravity sources (mo_set_nbig with nbig <= MO_BIG_MAX): sources in shared memory, direct big-row encounter pass
     bool use_big = false;
-    int big_ipt = 1;
+    int big_ipt = 1, big_grid = 1;
     int gkernels = 0;                   // kernel launches recorded in the cached step graph
     int sym_nI = 0, sym_ch = 1, sym_nunits = 0;
     int4* sym_units = nullptr;
@@ -103,6 +103,14 @@ static int env_int(const char* name, int dflt) {
     return (s && *s) ? atoi(s) : dflt;
 }
 
+typedef void (*big_kernel_t)(BigParams);
+static big_kernel_t pick_big_kernel(int ipt, bool kick) {
+    if (ipt == 4 && env_int("MO_BIG_U", 1) == 2) return kick ? pair_big_kernel<4, 2, true> : pair_big_kernel<4, 2, false>;
+    if (ipt == 4) return kick ? pair_big_kernel<4, 1, true> : pair_big_kernel<4, 1, false>;
+    if (ipt == 2) return kick ? pair_big_kernel<2, 2, true> : pair_big_kernel<2, 2, false>;
+    return kick ? pair_big_kernel<1, 4, true> : pair_big_kernel<1, 4, false>;
+}
+
 // j-split count: minimise (waves) x (tiles per CTA + start-up), see DESIGN.md section 5
 static void choose_geometry(mo_ctx* ctx) {
     const int nb = ctx->nb;
@@ -142,11 +150,15 @@ static void choose_geometry(mo_ctx* ctx) {
     if (ctx->use_big) {
         // bodies per thread: as many as still leave about two waves of CTAs
         const long long want = 2LL * ctx->nsm * BIG_THREADS;
-        ctx->big_ipt = env_int("MO_BIG_IPT", nb >= 4 * want ? 4 : nb >= 2 * want ? 2 : 1);
+        ctx->big_ipt = env_int("MO_BIG_IPT", nb >= 2 * want ? 2 : 1);   // 4 measured no faster (register-bound occupancy)
         if (ctx->big_ipt != 1 && ctx->big_ipt != 2 && ctx->big_ipt != 4) ctx->big_ipt = 1;
         ctx->ipt = ctx->big_ipt; ctx->nsplit = 1; ctx->tps = ctx->nSrcTiles;
         ctx->nIblk = (nb + BIG_THREADS * ctx->big_ipt - 1) / (BIG_THREADS * ctx->big_ipt);
-        ctx->ctas_per_sm = 0;
+        int occb = 1;
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occb, pick_big_kernel(ctx->big_ipt, true), BIG_THREADS, 0);
+        if (occb < 1) occb = 1;
+        ctx->ctas_per_sm = occb;
+        ctx->big_grid = ctx->nIblk < ctx->nsm * occb ? ctx->nIblk : ctx->nsm * occb;   // persistent: CTAs walk over i blocks
     }
     ctx->use_sym = ctx->nbig == nb && env_int("MO_SYM", nb >= env_int("MO_SYM_MIN", 8192) ? 1 : 0) != 0;
     if (ctx->use_sym) {
@@ -313,14 +325,6 @@ static mo_status ensure_pair_scratch(mo_ctx* ctx) {
     return MO_OK;
 }
 
-typedef void (*big_kernel_t)(BigParams);
-static big_kernel_t pick_big_kernel(int ipt, bool kick) {
-    if (ipt == 4 && env_int("MO_BIG_U", 1) == 2) return kick ? pair_big_kernel<4, 2, true> : pair_big_kernel<4, 2, false>;
-    if (ipt == 4) return kick ? pair_big_kernel<4, 1, true> : pair_big_kernel<4, 1, false>;
-    if (ipt == 2) return kick ? pair_big_kernel<2, 2, true> : pair_big_kernel<2, 2, false>;
-    return kick ? pair_big_kernel<1, 4, true> : pair_big_kernel<1, 4, false>;
-}
-
 static mo_status launch_pair(mo_ctx* ctx, bool kick = false, double hk = 0.0) {
     AccelParams p;
     p.tiles = ctx->tiles; p.x = ctx->x; p.rcrit = ctx->rcrit; p.part = ctx->part;
@@ -341,7 +345,7 @@ static mo_status launch_pair(mo_ctx* ctx, bool kick = false, double hk = 0.0) {
         BigParams bp;
         bp.x = ctx->x; bp.gm = ctx->gm; bp.rcrit = ctx->rcrit; bp.a = ctx->a; bp.v = ctx->v;
         bp.nb = ctx->nb; bp.nbig = ctx->nbig; bp.ld = ctx->ld; bp.hk = hk;
-        pick_big_kernel(ctx->big_ipt, kick)<<<ctx->nIblk, BIG_THREADS, 0, ctx->stream>>>(bp);
+        pick_big_kernel(ctx->big_ipt, kick)<<<ctx->big_grid, BIG_THREADS, 0, ctx->stream>>>(bp);
     } else if (ctx->use_sym) {
         SymParams sp;
         sp.tiles = ctx->tiles; sp.x = ctx->x; sp.gm = ctx->gm; sp.rcrit = ctx->rcrit; sp.units = ctx->sym_units;
@@ -638,16 +642,15 @@ extern "C" mo_status mo_pair_geometry(const mo_ctx* ctx, int32_t* ipt, int32_t* 
     if (!ctx) return MO_EINVAL;
     if (ipt) *ipt = ctx->ipt;
     if (jsplit) *jsplit = ctx->nsplit;
-    if (ctas) *ctas = ctx->use_sym ? ctx->sym_nunits : ctx->nIblk * ctx->nsplit;
-    if (ctx->use_big && ctas_per_sm) {
-        int occ = 0;
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, pick_big_kernel(ctx->big_ipt, true), BIG_THREADS, 0);
-        *ctas_per_sm = occ;
-        return MO_OK;
-    }
+    if (ctas) *ctas = ctx->use_sym ? ctx->sym_nunits : ctx->use_big ? ctx->big_grid : ctx->nIblk * ctx->nsplit;
     if (ctx->use_sym && jsplit) *jsplit = ctx->sym_ch;
     if (ctas_per_sm) *ctas_per_sm = ctx->ctas_per_sm;
     return MO_OK;
+}
+
+extern "C" const char* mo_pair_kernel_name(const mo_ctx* ctx) {
+    if (!ctx) return nullptr;
+    return ctx->use_big ? "pair_big_kernel" : ctx->use_sym ? "pair_sym_kernel" : "pair_accel_kernel";
 }
 
 extern "C" mo_status mo_set_kernel_timing(mo_ctx* ctx, int32_t on) {

@@ -21,7 +21,7 @@ EXPORTS = ["mo_create", "mo_accel", "mo_drift", "mo_encounters", "mo_step", "mo_
            "mo_snapshot", "mo_snapshot_ptrs", "mo_snapshot_copy", "mo_invalidate_accel", "mo_get_stats", "mo_launch_count",
            "mo_workspace_bytes", "mo_step_host", "mo_accel_host", "mo_probe_fp64_peak",
            "mo_pair_geometry", "mo_set_kernel_timing", "mo_pair_kernel_ms", "mo_strerror", "mo_version",
-           "mo_set_nbig"]
+           "mo_set_nbig", "mo_pair_kernel_name"]
 
 
 class MoStats(C.Structure):
@@ -61,6 +61,7 @@ def load():
     L.mo_snapshot_copy.restype = C.c_int; L.mo_snapshot_copy.argtypes = [vp, vp, vp]
     L.mo_invalidate_accel.restype = C.c_int; L.mo_invalidate_accel.argtypes = [vp]
     L.mo_set_nbig.restype = C.c_int; L.mo_set_nbig.argtypes = [vp, I32]
+    L.mo_pair_kernel_name.restype = C.c_char_p; L.mo_pair_kernel_name.argtypes = [vp]
     L.mo_get_stats.restype = C.c_int; L.mo_get_stats.argtypes = [vp, C.POINTER(MoStats)]
     L.mo_launch_count.restype = I64; L.mo_launch_count.argtypes = [vp]
     L.mo_workspace_bytes.restype = I64; L.mo_workspace_bytes.argtypes = [vp]
@@ -233,6 +234,9 @@ class Mopal:
         a, b, c, d = C.c_int32(), C.c_int32(), C.c_int32(), C.c_int32()
         self._check(self._L.mo_pair_geometry(self._ctx, C.byref(a), C.byref(b), C.byref(c), C.byref(d)), "mo_pair_geometry")
         return dict(ipt=a.value, jsplit=b.value, ctas=c.value, ctas_per_sm=d.value)
+
+    def pair_kernel_name(self) -> str:
+        return self._L.mo_pair_kernel_name(self._ctx).decode()
 
     def set_kernel_timing(self, on: bool):
         self._check(self._L.mo_set_kernel_timing(self._ctx, 1 if on else 0), "mo_set_kernel_timing")

@@ -70,6 +70,14 @@ def _lib(kind="ld"):
                                   P32, I64, PU8, P32, I64, PI64, P32]
     L.oracle_step_noenc.restype = I
     L.oracle_step_noenc.argtypes = [I, I, C.c_double, D, D, C.c_double, D, D, D]
+    L.oracle_h2dh.restype = I
+    L.oracle_h2dh.argtypes = [I, I, C.c_double, D, D]
+    L.oracle_dh2h.restype = I
+    L.oracle_dh2h.argtypes = [I, I, C.c_double, D, D]
+    L.oracle_hill.restype = I
+    L.oracle_hill.argtypes = [I, I, I, C.c_double, C.c_double, C.c_double, D, D, D, D, D]
+    L.oracle_energy.restype = I
+    L.oracle_energy.argtypes = [I, I, I, C.c_double, C.c_double, D, D, D, D]
     _loaded[kind] = L
     return L
 
@@ -220,3 +228,37 @@ def step(mu, gm, rcrit, h, x, v, a, cap=1 << 16, with_encounters=True, kind="ld"
     return dict(x=x, v=v, a=a, x0=x0, v0=v0, pairs=pairs[:min(cnt, cap)].copy(), count=int(cnt),
                 flag=flag[:nb].copy(), ambig=amb[:min(n_amb.value, cap)].copy(),
                 n_ambig=int(n_amb.value), nfail=int(nfail.value))
+
+
+# ---- per-step support routines (readings H-1..H-4, E-1..E-3) -------------------
+def h2dh(m_star, mass, v, kind="ld"):
+    """H-1: heliocentric velocities -> barycentric (democratic heliocentric); positions unchanged."""
+    v = _soa(v).copy(); mass = _vec(mass)
+    assert _lib(kind).oracle_h2dh(v.shape[1], v.shape[1], float(m_star), _dp(mass), _dp(v)) == 0
+    return v
+
+
+def dh2h(m_star, mass, v, kind="ld"):
+    """H-2: barycentric (democratic heliocentric) velocities -> heliocentric."""
+    v = _soa(v).copy(); mass = _vec(mass)
+    assert _lib(kind).oracle_dh2h(v.shape[1], v.shape[1], float(m_star), _dp(mass), _dp(v)) == 0
+    return v
+
+
+def hill(G, m_star, mass, x, v, n_hill=3.0, mode=0, kind="ld"):
+    """H-3/H-4: (r_hill, rcrit = n_hill r_hill); mode 0: from |x| ; mode 1: from the osculating a."""
+    x = _soa(x); v = _soa(v); mass = _vec(mass)
+    nb = x.shape[1]
+    rh = np.zeros(nb); rc = np.zeros(nb)
+    assert _lib(kind).oracle_hill(nb, nb, int(mode), float(n_hill), float(G), float(m_star), _dp(mass), _dp(x), _dp(v),
+                                  _dp(rh), _dp(rc)) == 0
+    return rh, rc
+
+
+def energy(G, m_star, mass, x, v, nbig=None, kind="ld"):
+    """E-1..E-3: dict(T, Us, Up, E, L[3], Eabs, Labs[3]) of star + bodies, barycentric frame."""
+    x = _soa(x); v = _soa(v); mass = _vec(mass)
+    nb = x.shape[1]
+    out = np.zeros(11)
+    assert _lib(kind).oracle_energy(nb, _nbig(nbig, nb), nb, float(G), float(m_star), _dp(mass), _dp(x), _dp(v), _dp(out)) == 0
+    return dict(T=out[0], Us=out[1], Up=out[2], E=out[3], L=out[4:7].copy(), Eabs=out[7], Labs=out[8:11].copy())

@@ -40,6 +40,12 @@
  *                group property, mpmath elements-based propagation  -> pinned
  *   step       : nb=1 by hand, angular momentum, reversibility, dt^2 energy
  *                scaling                                            -> pinned
+ *   support    : h2dh/dh2h - mpmath centre of mass of the inertial N+1-body definition,
+ *                two-body closed form, inverse; hill - exact cube closed form, Jupiter's
+ *                textbook 0.355 AU, generator's a recovered by vis-viva, (1-e) ratio at
+ *                perihelion; energy/L - two-body closed forms -GMm/2a and reduced-mass
+ *                sqrt(mu a (1-e^2)), mpmath brute force over all N+1 bodies, dt^2
+ *                scaling of the step's energy error                  -> pinned
  *   multi-step trajectories beyond ~10 steps: parity unpinned by construction
  *   (chaos; the paper itself compares curves and medians).
  */
@@ -636,5 +642,154 @@ int oracle_step_noenc(int nb, int ld, double mu, const double *gm, const double 
     oracle_jump(nb, ld, 0.5 * h, mu, gm, x, v, 0);
     oracle_accel(nb, ld, gm, x, rcrit, a, 0);
     oracle_kick(nb, ld, 0.5 * h, v, a);
+    return 0;
+}
+
+/* ---------------------------------------------------------------------------
+ * Per-step support routines the paper names next to the hot path:
+ * coordinate conversion heliocentric <-> democratic heliocentric (mco_h2dh, mce_dh2h;
+ * PAPER.md:84 item 1 and fn. 12), Hill and critical radii (mce_hill, mce_init;
+ * PAPER.md:87, 94, fn. 14, and 291 item 3: "critical radii are always updated since they
+ * depend on the instantaneous distance between each planet and the central star"), total
+ * energy and momentum (mxx_en).  The paper states what they compute in words
+ * only; the arithmetic follows readings H-1..H-4 and E-1..E-3.
+ * Masses in Msun (not gm): these routines need mass ratios and G separately.
+ * ------------------------------------------------------------------------- */
+#ifdef ORACLE_DOUBLE
+#define R_CBRT cbrt
+#else
+#define R_CBRT cbrtl
+#endif
+
+/* sum_k m_k v_k, ascending k */
+static void mv_sum(int nb, int ld, const double *mass, const double *v, real S[3])
+{
+    S[0] = S[1] = S[2] = 0;
+    for (int b = 0; b < nb; ++b)
+        for (int c = 0; c < 3; ++c) S[c] += (real)mass[b] * X_(v, c, b);
+}
+
+/* H-1: heliocentric -> democratic heliocentric.  Positions stay heliocentric; velocities
+ * become barycentric: v_j -= sum_k m_k v_k / (mstar + sum_k m_k)  (the star's heliocentric
+ * velocity is 0, so the barycentre moves at sum m v / M_total in the heliocentric frame). */
+int oracle_h2dh(int nb, int ld, double mstar, const double *mass, double *v)
+{
+    if (nb < 0 || ld < nb) return -1;
+    real S[3], mtot = (real)mstar;
+    mv_sum(nb, ld, mass, v, S);
+    for (int b = 0; b < nb; ++b) mtot += (real)mass[b];
+    for (int b = 0; b < nb; ++b)
+        for (int c = 0; c < 3; ++c)
+            v[(size_t)c * ld + b] = (double)(X_(v, c, b) - S[c] / mtot);
+    return 0;
+}
+
+/* H-2: democratic heliocentric -> heliocentric: v_j += sum_k m_k v_k / mstar
+ * (barycentric momentum is zero, so the star moves at -sum m v / mstar). */
+int oracle_dh2h(int nb, int ld, double mstar, const double *mass, double *v)
+{
+    if (nb < 0 || ld < nb) return -1;
+    real S[3];
+    mv_sum(nb, ld, mass, v, S);
+    for (int b = 0; b < nb; ++b)
+        for (int c = 0; c < 3; ++c)
+            v[(size_t)c * ld + b] = (double)(X_(v, c, b) + S[c] / (real)mstar);
+    return 0;
+}
+
+/* H-3 / H-4: Hill radius r_H = d (m / 3 mstar)^(1/3) and critical radius rcrit = nhill r_H.
+ * mode 0 (default reading of PAPER.md:94, 291): d = |x_j|, the instantaneous star-planet separation.
+ * mode 1 (variant): d = osculating semi-major axis, 1/a = 2/r - v_h^2 / (G (mstar + m_j)), with the
+ *        heliocentric velocity v_h = v + sum m v / mstar of the democratic heliocentric input (H-2);
+ *        unbound bodies (1/a <= 0) fall back to d = r.
+ * x heliocentric, v barycentric (democratic heliocentric), as everywhere on the path. */
+int oracle_hill(int nb, int ld, int mode, double nhill, double G, double mstar, const double *mass,
+                const double *x, const double *v, double *rhill, double *rcrit)
+{
+    if (nb < 0 || ld < nb || (mode != 0 && mode != 1)) return -1;
+    real S[3] = {0, 0, 0};
+    if (mode == 1) mv_sum(nb, ld, mass, v, S);
+#pragma omp parallel for schedule(static)
+    for (int b = 0; b < nb; ++b) {
+        real r2 = 0;
+        for (int c = 0; c < 3; ++c) r2 += X_(x, c, b) * X_(x, c, b);
+        real d = R_SQRT(r2);
+        if (mode == 1) {
+            real v2 = 0;
+            for (int c = 0; c < 3; ++c) {
+                real vh = X_(v, c, b) + S[c] / (real)mstar;
+                v2 += vh * vh;
+            }
+            real inva = (real)2 / d - v2 / ((real)G * ((real)mstar + (real)mass[b]));
+            if (inva > 0) d = (real)1 / inva;
+        }
+        real rh = d * R_CBRT((real)mass[b] / ((real)3 * (real)mstar));
+        if (rhill) rhill[b] = (double)rh;
+        if (rcrit) rcrit[b] = (double)((real)nhill * rh);
+    }
+    return 0;
+}
+
+/* E-1..E-3: total energy and angular momentum of star + bodies in the barycentric frame, from
+ * democratic heliocentric input (x heliocentric, v barycentric):
+ *   star:  v_s = -sum m v / mstar,  x_s = -sum m x / (mstar + sum m)   (barycentric)
+ *   T  = 1/2 sum m v^2 + 1/2 mstar v_s^2
+ *   Us = -G mstar sum m_j / |x_j|
+ *   Up = -G sum_{i<j, i<nbig} m_i m_j / |x_i - x_j|     (the pairs that interact: first member big,
+ *                                                        PAPER.md:152-157; nbig = nb: all pairs)
+ *   L  = sum m (x + x_s) x v + mstar x_s x v_s
+ * out[0..10] = T, Us, Up, E = T+Us+Up, Lx, Ly, Lz, sum|energy terms|, sum|L terms| per component. */
+int oracle_energy(int nb, int nbig, int ld, double G, double mstar, const double *mass,
+                  const double *x, const double *v, double *out)
+{
+    if (nb < 0 || ld < nb || nbig < 0 || nbig > nb) return -1;
+    real Sv[3], Sx[3] = {0, 0, 0}, mtot = (real)mstar;
+    mv_sum(nb, ld, mass, v, Sv);
+    for (int b = 0; b < nb; ++b) {
+        mtot += (real)mass[b];
+        for (int c = 0; c < 3; ++c) Sx[c] += (real)mass[b] * X_(x, c, b);
+    }
+    real xs[3], vs[3];
+    for (int c = 0; c < 3; ++c) { xs[c] = -Sx[c] / mtot; vs[c] = -Sv[c] / (real)mstar; }
+    real T = 0, Us = 0, Eabs = 0, L[3] = {0, 0, 0}, Labs[3] = {0, 0, 0};
+    for (int b = 0; b < nb; ++b) {
+        real m = (real)mass[b], r2 = 0, v2 = 0, p[3], w[3];
+        for (int c = 0; c < 3; ++c) {
+            p[c] = X_(x, c, b) + xs[c]; w[c] = X_(v, c, b);
+            r2 += X_(x, c, b) * X_(x, c, b); v2 += w[c] * w[c];
+        }
+        T += (real)0.5L * m * v2;
+        real us = (real)G * (real)mstar * m / R_SQRT(r2);
+        Us -= us;
+        Eabs += (real)0.5L * m * v2 + us;
+        real l[3] = {p[1] * w[2] - p[2] * w[1], p[2] * w[0] - p[0] * w[2], p[0] * w[1] - p[1] * w[0]};
+        for (int c = 0; c < 3; ++c) { L[c] += m * l[c]; Labs[c] += R_FABS(m * l[c]); }
+    }
+    {
+        real v2 = vs[0] * vs[0] + vs[1] * vs[1] + vs[2] * vs[2];
+        T += (real)0.5L * (real)mstar * v2;
+        Eabs += (real)0.5L * (real)mstar * v2;
+        real l[3] = {xs[1] * vs[2] - xs[2] * vs[1], xs[2] * vs[0] - xs[0] * vs[2], xs[0] * vs[1] - xs[1] * vs[0]};
+        for (int c = 0; c < 3; ++c) { L[c] += (real)mstar * l[c]; Labs[c] += R_FABS((real)mstar * l[c]); }
+    }
+    real Up = 0;
+#pragma omp parallel for schedule(dynamic, 16) reduction(+ : Up)
+    for (int i = 0; i < nbig; ++i) {
+        real acc = 0;
+        for (int j = i + 1; j < nb; ++j) {
+            real d2 = 0;
+            for (int c = 0; c < 3; ++c) {
+                real d = X_(x, c, i) - X_(x, c, j);
+                d2 += d * d;
+            }
+            if (d2 > 0) acc += (real)mass[j] / R_SQRT(d2);
+        }
+        Up += (real)G * (real)mass[i] * acc;
+    }
+    Eabs += Up;
+    Up = -Up;
+    out[0] = (double)T; out[1] = (double)Us; out[2] = (double)Up; out[3] = (double)(T + Us + Up);
+    for (int c = 0; c < 3; ++c) { out[4 + c] = (double)L[c]; out[8 + c] = (double)Labs[c]; }
+    out[7] = (double)Eabs;
     return 0;
 }

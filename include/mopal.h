@@ -126,6 +126,37 @@ void mo_destroy(mo_ctx *ctx);
  * invalidates `a`.  Synchronises the stream. */
 mo_status mo_set_nbig(mo_ctx *ctx, int32_t nbig);
 
+/* ---- per-step support routines on the device (readings H-1..H-4, E-1..E-3) ---
+ * The paper names these next to the hot path and runs them on the host, copying the critical
+ * radii to the device every step (PAPER.md:291 item 3); here they stay on the device. */
+
+/* mco_h2dh / mce_dh2h (PAPER.md:84 item 1, fn. 12).  In place on v (positions are heliocentric in
+ * both systems).  mo_h2dh: heliocentric -> barycentric velocities, v_j -= sum m v / (m_star + sum m);
+ * mo_dh2h: the inverse, v_j += sum m v / m_star.  Asynchronous on the context's stream. */
+mo_status mo_h2dh(mo_ctx *ctx);
+mo_status mo_dh2h(mo_ctx *ctx);
+
+/* mce_hill + critical radius (PAPER.md:87, 94 fn. 13-14, 291).  Overwrites the caller's rcrit array
+ * (device, nb doubles - the array given to mo_create, now written by the library) with
+ * n_hill * r_H, r_H = d * (m / (3 m_star))^(1/3); mode 0: d = |x_j|, the instantaneous star-planet
+ * separation; mode 1: d = osculating semi-major axis from x and the heliocentric velocity (unbound
+ * bodies: |x_j|).  rhill_dev (nullable, device, nb doubles) receives r_H.  x heliocentric, v
+ * barycentric.  MO_EINVAL: n_hill not finite or < 0, mode not 0/1.  Asynchronous. */
+mo_status mo_hill(mo_ctx *ctx, double n_hill, int32_t mode, double *rhill_dev);
+
+/* Make mo_step run mo_hill(n_hill, mode) at the start of every step ("the mce_hill routine is
+ * called at each timestep"): encounters and the closing accelerations of step n use
+ * the radii of the positions at the start of step n.  mode -1 switches it off (the default).
+ * Drops the cached step graph. */
+mo_status mo_set_hill(mo_ctx *ctx, double n_hill, int32_t mode);
+
+/* mxx_en: kinetic energy T (star included), star-body potential Us, body-body potential
+ * Up over the interacting pairs (i < j, i < nbig), E = T + Us + Up, and the total angular momentum L,
+ * all in the barycentric frame, Msun AU^2 day^-2 and Msun AU^2 day^-1.  Synchronises the stream.
+ * O(nbig * nb) pair evaluations. */
+typedef struct { double T, Us, Up, E, L[3]; } mo_energy_t;
+mo_status mo_energy(mo_ctx *ctx, mo_energy_t *out_host);
+
 /* Copy the current x, v into the context's x0, v0 snapshot (asynchronous). */
 mo_status mo_snapshot(mo_ctx *ctx);
 /* Device pointers of the snapshot planes (3*ld doubles each), for inspection. */

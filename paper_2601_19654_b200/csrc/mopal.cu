@@ -13,6 +13,7 @@
 #include "glue.cuh"
 #include "pair_big.cuh"
 #include "pair_sym.cuh"
+#include "support.cuh"
 
 using namespace mopal;
 
@@ -31,6 +32,13 @@ struct mo_ctx {
     // owned scratch
     double *gm = nullptr, *x0 = nullptr, *v0 = nullptr, *part = nullptr, *psumA = nullptr, *psumB = nullptr;
     unsigned* ticket = nullptr;         // two last-block counters (psumA, psumB)
+    // per-step support routines
+    double* gmsum = nullptr;            // sum of gm (device scalar)
+    double *en_on = nullptr, *en_pair = nullptr, *en_out = nullptr;   // energy partials / result (lazy)
+    double* en_host = nullptr;          // pinned, 7 doubles
+    int en_npair = 0, en_split = 1;
+    int hill_mode = -1;                 // mo_set_hill: -1 off
+    double hill_n = 3.0;
     unsigned char* tiles = nullptr;
     EncBuf enc = {};
     DevStats* dstats = nullptr;
@@ -208,7 +216,9 @@ extern "C" void mo_destroy(mo_ctx* ctx) {
     if (ctx->cap_stream) cudaStreamDestroy(ctx->cap_stream);
     for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
     cudaFree(ctx->gm); cudaFree(ctx->x0); cudaFree(ctx->v0); cudaFree(ctx->part);
-    cudaFree(ctx->psumA); cudaFree(ctx->psumB); cudaFree(ctx->ticket); cudaFree(ctx->tiles);
+    cudaFree(ctx->psumA); cudaFree(ctx->psumB); cudaFree(ctx->ticket);
+    cudaFree(ctx->gmsum); cudaFree(ctx->en_on); cudaFree(ctx->en_pair); cudaFree(ctx->en_out);
+    if (ctx->en_host) cudaFreeHost(ctx->en_host); cudaFree(ctx->tiles);
     cudaFree(ctx->sym_units); cudaFree(ctx->sym_ustart); cudaFree(ctx->sym_partI); cudaFree(ctx->sym_partJ);
     cudaFree(ctx->enc.box); cudaFree(ctx->enc.boxf); cudaFree(ctx->enc.rowcnt); cudaFree(ctx->enc.rowfill);
     cudaFree(ctx->enc.rowoff); cudaFree(ctx->enc.hits); cudaFree(ctx->enc.tmpj); cudaFree(ctx->enc.nhit);
@@ -257,6 +267,7 @@ extern "C" mo_status mo_create(mo_ctx** out, int32_t nb, int32_t ld, double m_st
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->v0, pl);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->psumA, 3 * (size_t)ctx->npsum + 3);   // partials + their sum
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->psumB, 3 * (size_t)ctx->npsum + 3);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->gmsum, 1);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->ticket, 2);
     if (e == cudaSuccess) e = cudaMemsetAsync(ctx->ticket, 0, 2 * sizeof(unsigned), ctx->stream);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->tiles, (size_t)ctx->nTiles * ACC_TILE_BYTES);
@@ -290,7 +301,8 @@ extern "C" mo_status mo_create(mo_ctx** out, int32_t nb, int32_t ld, double m_st
     e = cudaMemsetAsync(ctx->dstats, 0, sizeof(DevStats), ctx->stream);
     if (e == cudaSuccess) {
         gm_kernel<<<(nb + 255) / 256, 256, 0, ctx->stream>>>(mass, G, nb, ctx->gm);
-        ctx->launches += 1;
+        gmsum_kernel<<<1, 1024, 0, ctx->stream>>>(ctx->gm, nb, ctx->gmsum);
+        ctx->launches += 2;
         e = cudaGetLastError();
     }
     if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);  // `mass` is borrowed only during the call
@@ -447,7 +459,25 @@ static mo_status enqueue_pairs(mo_ctx* ctx, const EncState& es, int step_inc) {
     return post_launch(ctx);
 }
 
+// rcrit <- n_hill * r_H from the current x (and v for the osculating variant)
+static mo_status enqueue_hill(mo_ctx* ctx, double n_hill, int mode, double* rhill) {
+    double* rc = const_cast<double*>(ctx->rcrit);
+    if (mode == 1) {   // heliocentric velocities need sum gm v
+        kick_psum_kernel<false><<<ctx->npsum, ON_BLOCK, 0, ctx->stream>>>(ctx->v, nullptr, ctx->gm, ctx->nb, ctx->ld, 0.0, ctx->psumA, ctx->ticket);
+        mo_status s = post_launch(ctx);
+        if (s != MO_OK) return s;
+        hill_kernel<1><<<ctx->npsum, ON_BLOCK, 0, ctx->stream>>>(ctx->x, ctx->v, ctx->gm, ctx->psumA, ctx->npsum, ctx->mu, n_hill, ctx->nb, ctx->ld, rc, rhill);
+    } else {
+        hill_kernel<0><<<ctx->npsum, ON_BLOCK, 0, ctx->stream>>>(ctx->x, ctx->v, ctx->gm, ctx->psumA, ctx->npsum, ctx->mu, n_hill, ctx->nb, ctx->ld, rc, rhill);
+    }
+    return post_launch(ctx);
+}
+
 static mo_status enqueue_step(mo_ctx* ctx, double dt) {
+    if (ctx->hill_mode >= 0) {
+        mo_status hs = enqueue_hill(ctx, ctx->hill_n, ctx->hill_mode, nullptr);
+        if (hs != MO_OK) return hs;
+    }
     kick_psum_kernel<true><<<ctx->npsum, ON_BLOCK, 0, ctx->stream>>>(ctx->v, ctx->a, ctx->gm, ctx->nb, ctx->ld, 0.5 * dt, ctx->psumA, ctx->ticket);
     mo_status s = post_launch(ctx);
     if (s != MO_OK) return s;
@@ -545,6 +575,71 @@ extern "C" mo_status mo_set_nbig(mo_ctx* ctx, int32_t nbig) {
     ctx->nbig = nbig;
     ctx->nSrcTiles = (nbig + TJ - 1) / TJ;
     choose_geometry(ctx);
+    return MO_OK;
+}
+
+extern "C" mo_status mo_hill(mo_ctx* ctx, double n_hill, int32_t mode, double* rhill_dev) {
+    if (!ctx || !isfinite(n_hill) || n_hill < 0.0 || (mode != 0 && mode != 1)) return MO_EINVAL;
+    ctx->a_valid = false;             // K depends on rcrit
+    return enqueue_hill(ctx, n_hill, mode, rhill_dev);
+}
+
+extern "C" mo_status mo_set_hill(mo_ctx* ctx, double n_hill, int32_t mode) {
+    if (!ctx || mode < -1 || mode > 1 || (mode >= 0 && (!isfinite(n_hill) || n_hill < 0.0))) return MO_EINVAL;
+    if (ctx->gexec) {
+        CK(cudaStreamSynchronize(ctx->stream));
+        cudaGraphExecDestroy(ctx->gexec); ctx->gexec = nullptr;
+    }
+    ctx->hill_mode = mode;
+    if (mode >= 0) ctx->hill_n = n_hill;
+    return MO_OK;
+}
+
+static mo_status vshift(mo_ctx* ctx, bool to_dh) {
+    kick_psum_kernel<false><<<ctx->npsum, ON_BLOCK, 0, ctx->stream>>>(ctx->v, nullptr, ctx->gm, ctx->nb, ctx->ld, 0.0, ctx->psumA, ctx->ticket);
+    mo_status s = post_launch(ctx);
+    if (s != MO_OK) return s;
+    if (to_dh)
+        vshift_kernel<true><<<ctx->npsum, ON_BLOCK, 0, ctx->stream>>>(ctx->v, ctx->psumA, ctx->npsum, ctx->gmsum, ctx->mu, ctx->nb, ctx->ld);
+    else
+        vshift_kernel<false><<<ctx->npsum, ON_BLOCK, 0, ctx->stream>>>(ctx->v, ctx->psumA, ctx->npsum, ctx->gmsum, ctx->mu, ctx->nb, ctx->ld);
+    return post_launch(ctx);
+}
+extern "C" mo_status mo_h2dh(mo_ctx* ctx) { return ctx ? vshift(ctx, true) : MO_EINVAL; }
+extern "C" mo_status mo_dh2h(mo_ctx* ctx) { return ctx ? vshift(ctx, false) : MO_EINVAL; }
+
+extern "C" mo_status mo_energy(mo_ctx* ctx, mo_energy_t* out_host) {
+    if (!ctx || !out_host) return MO_EINVAL;
+    const int nIb = (ctx->nbig + EN_T - 1) / EN_T;
+    const int nT = (ctx->nb + EN_T - 1) / EN_T;
+    int split = (4 * ctx->nsm + nIb - 1) / nIb;          // about four waves of CTAs
+    if (split > nT) split = nT;
+    if (split < 1) split = 1;
+    if (!ctx->en_on || ctx->en_npair != nIb * split) {   // (re)allocate after mo_set_nbig
+        cudaFree(ctx->en_pair); ctx->en_pair = nullptr;
+        cudaError_t e = cudaSuccess;
+        if (!ctx->en_on) e = dalloc(ctx, &ctx->en_on, (size_t)ctx->npsum * EN_NSUM);
+        if (e == cudaSuccess && !ctx->en_out) e = dalloc(ctx, &ctx->en_out, 8);
+        if (e == cudaSuccess && !ctx->en_host) e = cudaMallocHost(reinterpret_cast<void**>(&ctx->en_host), 8 * sizeof(double));
+        if (e == cudaSuccess) e = dalloc(ctx, &ctx->en_pair, (size_t)nIb * split);
+        if (e != cudaSuccess) { cudaGetLastError(); ctx->last_err = e; return e == cudaErrorMemoryAllocation ? MO_ENOMEM : MO_ECUDA; }
+        ctx->en_npair = nIb * split; ctx->en_split = split;
+    }
+    energy_on_kernel<<<ctx->npsum, ON_BLOCK, 0, ctx->stream>>>(ctx->x, ctx->v, ctx->gm, ctx->nb, ctx->ld, ctx->en_on);
+    mo_status s = post_launch(ctx);
+    if (s != MO_OK) return s;
+    energy_pair_kernel<<<dim3(nIb, split), EN_T, 0, ctx->stream>>>(ctx->x, ctx->gm, ctx->nb, ctx->nbig, ctx->ld, ctx->en_pair);
+    s = post_launch(ctx);
+    if (s != MO_OK) return s;
+    energy_final_kernel<<<1, 256, 0, ctx->stream>>>(ctx->en_on, ctx->npsum, ctx->en_pair, ctx->en_npair, ctx->mu, ctx->en_out);
+    s = post_launch(ctx);
+    if (s != MO_OK) return s;
+    CK(cudaMemcpyAsync(ctx->en_host, ctx->en_out, 7 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    const double G = ctx->G;
+    out_host->T = ctx->en_host[0] / G; out_host->Us = ctx->en_host[1] / G; out_host->Up = ctx->en_host[2] / G;
+    out_host->E = ctx->en_host[3] / G;
+    for (int c = 0; c < 3; ++c) out_host->L[c] = ctx->en_host[4 + c] / G;
     return MO_OK;
 }
 

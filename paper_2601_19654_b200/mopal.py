@@ -21,12 +21,16 @@ EXPORTS = ["mo_create", "mo_accel", "mo_drift", "mo_encounters", "mo_step", "mo_
            "mo_snapshot", "mo_snapshot_ptrs", "mo_snapshot_copy", "mo_invalidate_accel", "mo_get_stats", "mo_launch_count",
            "mo_workspace_bytes", "mo_step_host", "mo_accel_host", "mo_probe_fp64_peak",
            "mo_pair_geometry", "mo_set_kernel_timing", "mo_pair_kernel_ms", "mo_strerror", "mo_version",
-           "mo_set_nbig", "mo_pair_kernel_name"]
+           "mo_set_nbig", "mo_pair_kernel_name", "mo_h2dh", "mo_dh2h", "mo_hill", "mo_set_hill", "mo_energy"]
 
 
 class MoStats(C.Structure):
     _fields_ = [("steps_done", C.c_int64), ("nce_last", C.c_int64), ("nce_total", C.c_int64),
                 ("drift_fail", C.c_int32), ("max_newton", C.c_int32)]
+
+
+class MoEnergy(C.Structure):
+    _fields_ = [("T", C.c_double), ("Us", C.c_double), ("Up", C.c_double), ("E", C.c_double), ("L", C.c_double * 3)]
 
 
 class MopalError(RuntimeError):
@@ -62,6 +66,11 @@ def load():
     L.mo_invalidate_accel.restype = C.c_int; L.mo_invalidate_accel.argtypes = [vp]
     L.mo_set_nbig.restype = C.c_int; L.mo_set_nbig.argtypes = [vp, I32]
     L.mo_pair_kernel_name.restype = C.c_char_p; L.mo_pair_kernel_name.argtypes = [vp]
+    L.mo_h2dh.restype = C.c_int; L.mo_h2dh.argtypes = [vp]
+    L.mo_dh2h.restype = C.c_int; L.mo_dh2h.argtypes = [vp]
+    L.mo_hill.restype = C.c_int; L.mo_hill.argtypes = [vp, C.c_double, I32, vp]
+    L.mo_set_hill.restype = C.c_int; L.mo_set_hill.argtypes = [vp, C.c_double, I32]
+    L.mo_energy.restype = C.c_int; L.mo_energy.argtypes = [vp, C.POINTER(MoEnergy)]
     L.mo_get_stats.restype = C.c_int; L.mo_get_stats.argtypes = [vp, C.POINTER(MoStats)]
     L.mo_launch_count.restype = I64; L.mo_launch_count.argtypes = [vp]
     L.mo_workspace_bytes.restype = I64; L.mo_workspace_bytes.argtypes = [vp]
@@ -213,6 +222,31 @@ class Mopal:
         encounter pairs; nbig = nb is fully interacting."""
         self._check(self._L.mo_set_nbig(self._ctx, int(nbig)), "mo_set_nbig")
         self.nbig = int(nbig)
+
+    # ---- per-step support routines (PAPER.md:84-94) ----
+    def h2dh(self):
+        """heliocentric -> barycentric velocities, in place (mco_h2dh)."""
+        self._check(self._L.mo_h2dh(self._ctx), "mo_h2dh")
+
+    def dh2h(self):
+        """barycentric -> heliocentric velocities, in place (mce_dh2h)."""
+        self._check(self._L.mo_dh2h(self._ctx), "mo_dh2h")
+
+    def hill(self, n_hill=3.0, mode=0, rhill=None):
+        """rcrit <- n_hill * Hill radius from the current state (mce_hill); ``rhill``: optional
+        float64 cuda tensor of nb elements that receives the Hill radii."""
+        ptr = None if rhill is None else rhill.data_ptr()
+        self._check(self._L.mo_hill(self._ctx, float(n_hill), int(mode), ptr), "mo_hill")
+
+    def set_hill(self, n_hill=3.0, mode=0):
+        """mo_step recomputes rcrit at the start of every step (mode -1: off)."""
+        self._check(self._L.mo_set_hill(self._ctx, float(n_hill), int(mode)), "mo_set_hill")
+
+    def energy(self):
+        """dict(T, Us, Up, E, L[3]) of star + bodies in the barycentric frame (mxx_en)."""
+        e = MoEnergy()
+        self._check(self._L.mo_energy(self._ctx, C.byref(e)), "mo_energy")
+        return dict(T=e.T, Us=e.Us, Up=e.Up, E=e.E, L=np.array(list(e.L)))
 
     def invalidate_accel(self):
         self._check(self._L.mo_invalidate_accel(self._ctx), "mo_invalidate_accel")

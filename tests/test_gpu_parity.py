@@ -582,3 +582,116 @@ def test_bigsmall_invalid(M):
     assert L.mo_set_nbig(None, 1) == M.MO_EINVAL
     assert L.mo_set_nbig(m._ctx, w.nb) == M.MO_OK
     m.close()
+
+
+# ------------------------------------------------------------------------------ support routines
+@pytest.mark.parametrize("cfg", [0, 1, 2])
+def test_support_h2dh_dh2h(M, cfg):
+    w = W.make_config(cfg)
+    m = _mk(M, w)
+    m.dh2h()
+    vh = m.get("v")
+    ref = oracle.dh2h(w.m_star, w.mass, w.v)
+    assert _rel_vec_err(vh, ref).max() <= 1e-15
+    m.h2dh()
+    back = oracle.h2dh(w.m_star, w.mass, ref)
+    assert _rel_vec_err(m.get("v"), back).max() <= 1e-15
+    assert _rel_vec_err(m.get("v"), w.v).max() <= 1e-15
+    assert np.array_equal(m.get("x"), w.x)
+    m.close()
+
+
+@pytest.mark.parametrize("cfg,mode,n_hill", [(0, 0, 3.0), (1, 1, 3.0), (2, 0, 2.5), (3, 1, 3.0), (4, 0, 3.0)])
+def test_support_hill(M, cfg, mode, n_hill):
+    import torch
+    w = W.make_config(cfg)
+    m = _mk(M, w, rcrit=np.zeros(w.nb))
+    rh_t = torch.zeros(w.nb, dtype=torch.float64, device=m.device)
+    m.hill(n_hill, mode, rhill=rh_t)
+    rh, rc = oracle.hill(G, w.m_star, w.mass, w.x, w.v, n_hill=n_hill, mode=mode)
+    got_rc, got_rh = m.get("rcrit"), rh_t.cpu().numpy()
+    tol = 2e-15 if mode == 0 else 1e-13          # mode 1: 1/a = 2/r - v^2/mu cancels ~2x, eccentric orbits more
+    assert np.max(np.abs(got_rh - rh) / rh) <= tol and np.max(np.abs(got_rc - rc) / rc) <= tol
+    if mode == 1 and cfg in (1, 3):
+        assert np.max(np.abs(got_rc - w.rcrit) / w.rcrit) <= 1e-11     # the generator's radii
+    m.close()
+
+
+@pytest.mark.parametrize("cfg,N,nbig", [(0, 256, None), (1, 3000, None), (2, 5000, 300), (1, 2000, 2), (4, 1025, 1024)])
+def test_support_energy(M, cfg, N, nbig):
+    w = W.shrink(cfg, N) if N != W.make_config(cfg).N else W.make_config(cfg)
+    m = _mk(M, w)
+    if nbig is not None:
+        m.set_nbig(nbig)
+    got = m.energy()
+    ref = oracle.energy(G, w.m_star, w.mass, w.x, w.v, nbig=nbig)
+    for k in ("T", "Us", "Up"):
+        assert abs(got[k] - ref[k]) <= 1e-13 * abs(ref[k]) + 1e-300, (k, got[k], ref[k])
+    assert abs(got["E"] - ref["E"]) <= 1e-12 * ref["Eabs"]
+    assert np.all(np.abs(got["L"] - ref["L"]) <= 1e-12 * ref["Labs"])
+    g2 = m.energy()
+    assert g2["E"] == got["E"] and np.array_equal(g2["L"], got["L"])      # deterministic
+    m.close()
+
+
+def test_support_energy_headline_size_and_conservation(M):
+    """full cfg3: pair potential over 2.1e9 pairs against the oracle's (OpenMP, a few seconds); then the
+    hybrid step conserves E to ~dt^2 and L to rounding."""
+    w = W.make_config(3)
+    m = _mk(M, w)
+    e0 = m.energy()
+    ref = oracle.energy(G, w.m_star, w.mass, w.x, w.v)
+    assert abs(e0["Up"] - ref["Up"]) <= 1e-12 * abs(ref["Up"])
+    assert abs(e0["E"] - ref["E"]) <= 1e-12 * ref["Eabs"]
+    m.step(w.dt, 5)
+    e1 = m.energy()
+    assert abs(e1["E"] - e0["E"]) <= 1e-6 * abs(e0["E"])
+    assert np.linalg.norm(e1["L"] - e0["L"]) <= 1e-12 * np.linalg.norm(e0["L"])
+    m.close()
+
+
+@pytest.mark.parametrize("cfg,N,mode,nbig", [(1, 1500, 0, None), (3, 2500, 1, None), (1, 1200, 0, 2)])
+def test_support_hill_inside_step(M, cfg, N, mode, nbig):
+    """mo_set_hill: rcrit recomputed from the state at the start of every step."""
+    w = W.shrink(cfg, N)
+    gm, mu = G * w.mass, G * w.m_star
+    m = _mk(M, w)
+    if nbig is not None:
+        m.set_nbig(nbig)
+    m.set_hill(3.0, mode)
+    a, _ = oracle.accel(gm, w.x, w.rcrit, nbig=nbig)
+    x, v = w.x, w.v
+    for k in range(3):
+        st = m.step(w.dt, 1)
+        _, rc = oracle.hill(G, w.m_star, w.mass, x, v, n_hill=3.0, mode=mode)
+        r = oracle.step(mu, gm, rc, w.dt, x, v, a, nbig=nbig)
+        x, v, a = r["x"], r["v"], r["a"]
+        ex, ev = _step_err(m, r)
+        tol = 1e-13 * (1 + k)
+        assert ex <= tol and ev <= tol, (k, ex, ev)
+        assert np.max(np.abs(m.get("rcrit") - rc) / rc.clip(1e-300)) <= (2e-15 if mode == 0 else 1e-12)
+        got = m.pair_list(st.nce_last)
+        # rcrit differs from the oracle's in the last bits: threshold pairs are the oracle's ambiguous ones
+        _pairs_ok(got, r)
+    # graph replay path gives the same trajectory
+    m2 = _mk(M, w)
+    if nbig is not None:
+        m2.set_nbig(nbig)
+    m2.set_hill(3.0, mode)
+    m2.step(w.dt, 3)
+    assert np.array_equal(m.get("x"), m2.get("x")) and np.array_equal(m.get("v"), m2.get("v"))
+    m2.set_hill(0.0, -1)
+    m.close(); m2.close()
+
+
+def test_support_invalid(M):
+    w = W.shrink(0, 64)
+    m = _mk(M, w)
+    L = M.load()
+    assert L.mo_hill(m._ctx, 3.0, 2, None) == M.MO_EINVAL
+    assert L.mo_hill(m._ctx, float("nan"), 0, None) == M.MO_EINVAL
+    assert L.mo_hill(m._ctx, -1.0, 0, None) == M.MO_EINVAL
+    assert L.mo_set_hill(m._ctx, 3.0, 5) == M.MO_EINVAL
+    assert L.mo_energy(m._ctx, None) == M.MO_EINVAL
+    assert L.mo_h2dh(None) == M.MO_EINVAL and L.mo_dh2h(None) == M.MO_EINVAL
+    m.close()

@@ -380,6 +380,63 @@ def run_drift_sweep(args):
     return 0
 
 
+def run_support(args):
+    """Rooflines of the per-step support routines: mo_energy's pair-potential
+    kernel against the FP64 issue peak at the headline config (13 FP64-pipe instructions per unordered
+    pair: 3 DADD, 3 DMUL, 6 DFMA, 1 DSETP = 18 flop + 1 compare); mo_hill and the h2dh/dh2h pair against HBM at nb = 2^24
+    (mode 0: 32 B in + 8 B out per body; a conversion: 24 B psum pass + 48 B shift pass).  One JSON line."""
+    import torch
+    from paper_2601_19654_b200 import mopal as M
+    from paper_2601_19654_b200 import workloads as W
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except OSError:
+        pass
+    hbm = float(peaks.get("hbm_gbs", 6550.0))
+
+    def timed(m, fn, n):
+        for _ in range(3):
+            fn()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(m.stream)
+        for _ in range(n):
+            fn()
+        e1.record(m.stream); torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / n
+
+    w = W.make_config(args.config)
+    m = M.Mopal(w.mass, w.x, w.v, w.rcrit, m_star=w.m_star, G=w.G, cap=16)
+    peak_burst, _, peak_sust = M.probe_fp64_peak(160, with_mean=True)
+    ms_en = timed(m, m.energy, 20)
+    upairs = w.nb * (w.nb - 1) / 2
+    en = {"workload": w.name, "ms": ms_en, "unordered_pairs_per_s": upairs / (ms_en * 1e-3),
+          "roofline": {"bound": "alu", "kernel": "energy_pair_kernel", "achieved": 18.0 * upairs / (ms_en * 1e-3) / 1e12,
+                       "peak": peak_sust, "unit": "TFLOP/s", "frac": 18.0 * upairs / (ms_en * 1e-3) / 1e12 / peak_sust,
+                       "note": "whole mo_energy call (3 kernels + 56 B D2H + sync) over 18 executed flop per unordered pair"}}
+    ms_h0 = timed(m, lambda: m.hill(3.0, 0), 200); ms_h1 = timed(m, lambda: m.hill(3.0, 1), 200)
+    small = {"nb": w.nb, "hill_mode0_us": ms_h0 * 1e3, "hill_mode1_us": ms_h1 * 1e3,
+             "dh2h_us": timed(m, m.dh2h, 200) * 1e3}
+    m.close()
+    nb = 1 << 24
+    base = W.make_config(2)
+    idx = np.arange(nb) % base.nb
+    m = M.Mopal(np.full(nb, 1e-10), base.x[:, idx].copy(), base.v[:, idx].copy(), np.zeros(nb), m_star=base.m_star, G=base.G, cap=16)
+    ms0 = timed(m, lambda: m.hill(3.0, 0), 20)
+    ms1 = timed(m, lambda: m.hill(3.0, 1), 20)
+    msc = timed(m, m.dh2h, 20)
+    big = {"nb": nb,
+           "hill_mode0": {"us": ms0 * 1e3, "GBps": 40.0 * nb / (ms0 * 1e-3) / 1e9, "frac": 40.0 * nb / (ms0 * 1e-3) / 1e9 / hbm},
+           "hill_mode1": {"us": ms1 * 1e3, "GBps": (32.0 + 64.0) * nb / (ms1 * 1e-3) / 1e9,
+                          "frac": (32.0 + 64.0) * nb / (ms1 * 1e-3) / 1e9 / hbm, "bytes_per_body": "psum pass 32 + hill pass 64"},
+           "dh2h": {"us": msc * 1e3, "GBps": (32.0 + 48.0) * nb / (msc * 1e-3) / 1e9, "frac": (32.0 + 48.0) * nb / (msc * 1e-3) / 1e9 / hbm,
+                    "bytes_per_body": "psum pass 32 (v, gm) + shift pass 48"}}
+    m.close()
+    print(json.dumps({"metric": "support_routines", "energy": en, "at_config": small, "hbm_bound": big,
+                      "hbm_peak_GBps": hbm, "fp64_peak_sustained_TFLOPs": peak_sust}), flush=True)
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -392,7 +449,10 @@ def main():
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of CPU work for the cpu_baseline sample")
     ap.add_argument("--drift-sweep", action="store_true", help="time mo_drift alone against the HBM roofline and exit")
+    ap.add_argument("--support", action="store_true", help="time mo_energy / mo_hill / mo_dh2h against their rooflines and exit")
     args = ap.parse_args()
+    if args.support:
+        return run_support(args)
     if args.drift_sweep:
         return run_drift_sweep(args)
     if args.impl == "reference":

@@ -612,7 +612,7 @@ extern "C" mo_status mo_energy(mo_ctx* ctx, mo_energy_t* out_host) {
     if (!ctx || !out_host) return MO_EINVAL;
     const int nIb = (ctx->nbig + EN_T - 1) / EN_T;
     const int nT = (ctx->nb + EN_T - 1) / EN_T;
-    int split = (4 * ctx->nsm + nIb - 1) / nIb;          // about four waves of CTAs
+    int split = (32 * ctx->nsm + nIb - 1) / nIb;         // many short CTAs: the rows of the triangle differ in length
     if (split > nT) split = nT;
     if (split < 1) split = 1;
     if (!ctx->en_on || ctx->en_npair != nIb * split) {   // (re)allocate after mo_set_nbig

@@ -43,9 +43,10 @@ FP64_LANES_PER_SM = 64        # DESIGN.md section "Rooflines": 148 SMs x 64 DFMA
 EXECUTED_FLOP_PER_PAIR = 15.5
 # one-sided kernels (pair_accel_kernel, pair_big_kernel): 3 DADD + 5 DMUL + 8 DFMA per ordered pair
 EXECUTED_FLOP_PER_PAIR_ONE_SIDED = 24.0
-# dram__bytes_read.sum + dram__bytes_write.sum of one pair_sym_kernel launch at config 3 from the
-# ncu --set full capture summarised in profiles/r1c_pair_sym_full.md (5.1 MB read + 91.1 MB written)
-PAIR_KERNEL_DRAM_TRAFFIC_BYTES = {3: 96.3e6}
+# dram__bytes_read.sum + dram__bytes_write.sum of one launch of the pair kernel from the ncu --set full captures
+# summarised in profiles/r1d_kernels_full.md: pair_sym_kernel at config 3 (5.1 MB read + 93.3 MB written),
+# pair_big_kernel at --bigsmall 1000000,100 (56.0 MB read + 2.9 MB written)
+PAIR_KERNEL_DRAM_TRAFFIC_BYTES = {3: 98.4e6, "1000000,100": 58.9e6}
 
 
 def reduce_max_over_ranks(values, dist=None, device="cpu"):
@@ -307,7 +308,7 @@ def run_ours(args):
                               "of_nominal": 100 * achieved / nominal, "flop_per_pair": FLOP_PER_PAIR},
             "roofline": {"bound": "alu", "kernel": kname, "achieved": achieved, "peak": peak_sust,
                          "unit": "TFLOP/s", "frac": achieved / peak_sust,
-                         "traffic": PAIR_KERNEL_DRAM_TRAFFIC_BYTES.get(args.config) if two_sided and nbig is None else None,
+                         "traffic": PAIR_KERNEL_DRAM_TRAFFIC_BYTES.get(args.bigsmall if nbig is not None else args.config),
                          "note": ("achieved = 26 algorithmic flop per ORDERED pair (SURVEY.md 8(d)) / kernel time; the kernel "
                                   "evaluates each unordered pair once (Newton III), so frac can exceed 1; achieved_executed = "
                                   "the 15.5 flop per ordered pair it really issues (3 DADD + 6 DMUL + 11 DFMA per unordered pair)")

@@ -14,6 +14,7 @@
 #include "pair_big.cuh"
 #include "pair_sym.cuh"
 #include "support.cuh"
+#include "step_small.cuh"
 
 using namespace mopal;
 
@@ -53,6 +54,8 @@ struct mo_ctx {
     // few gravity sources (mo_set_nbig with nbig <= MO_BIG_MAX): sources in shared memory, direct big-row encounter pass
     bool use_big = false;
     int big_ipt = 1, big_grid = 1;
+    bool use_psm = false;               // nb <= PSM_MAX: pair_small_kernel (several lanes per body) instead of pack + pair + reduce
+    bool use_small = false;             // nb <= SMALL_MAX: the pre-acceleration part of the step is one single-CTA kernel
     int gkernels = 0;                   // kernel launches recorded in the cached step graph
     int sym_nI = 0, sym_ch = 1, sym_nunits = 0;
     int4* sym_units = nullptr;
@@ -154,7 +157,9 @@ static void choose_geometry(mo_ctx* ctx) {
     if (ctx->enc_split < 1) ctx->enc_split = 1;
     if (ctx->enc_split > 8) ctx->enc_split = 8;
     // two-sided kernel for large nb: units = (row block, chunk of sym_ch j tiles from the diagonal on)
-    ctx->use_big = ctx->nbig < nb && ctx->nbig <= env_int("MO_BIG_MAX", 4096);
+    ctx->use_small = nb <= env_int("MO_SMALL_MAX", 400) && nb <= SMALL_MAX && env_int("MO_SMALL", 1) != 0;
+    ctx->use_psm = nb <= env_int("MO_PSM_MAX", PSM_MAX) && nb <= PSM_MAX && env_int("MO_PSM", 1) != 0;
+    ctx->use_big = !ctx->use_psm && ctx->nbig < nb && ctx->nbig <= env_int("MO_BIG_MAX", 4096);
     if (ctx->use_big) {
         // bodies per thread: as many as still leave about two waves of CTAs
         const long long want = 2LL * ctx->nsm * BIG_THREADS;
@@ -168,7 +173,7 @@ static void choose_geometry(mo_ctx* ctx) {
         ctx->ctas_per_sm = occb;
         ctx->big_grid = ctx->nIblk < ctx->nsm * occb ? ctx->nIblk : ctx->nsm * occb;   // persistent: CTAs walk over i blocks
     }
-    ctx->use_sym = ctx->nbig == nb && env_int("MO_SYM", nb >= env_int("MO_SYM_MIN", 8192) ? 1 : 0) != 0;
+    ctx->use_sym = !ctx->use_psm && ctx->nbig == nb && env_int("MO_SYM", nb >= env_int("MO_SYM_MIN", 8192) ? 1 : 0) != 0;
     if (ctx->use_sym) {
         int occs = 1;
         cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occs, pair_sym_kernel, SYM_THREADS, 0);
@@ -318,7 +323,7 @@ static mo_status ensure_pair_scratch(mo_ctx* ctx) {
     if (ctx->pair_ready) return MO_OK;
     cudaError_t e = cudaSuccess;
     const size_t pl = 3 * (size_t)ctx->ld;
-    if (!ctx->use_sym && !ctx->use_big) e = dalloc(ctx, &ctx->part, pl * (size_t)ctx->nsplit);
+    if (!ctx->use_sym && !ctx->use_big && !ctx->use_psm) e = dalloc(ctx, &ctx->part, pl * (size_t)ctx->nsplit);
     if (ctx->use_sym) {
         if (e == cudaSuccess) e = dalloc(ctx, &ctx->sym_units, (size_t)ctx->sym_nunits);
         if (e == cudaSuccess) e = dalloc(ctx, &ctx->sym_ustart, ctx->h_ustart.size());
@@ -353,7 +358,14 @@ static mo_status launch_pair(mo_ctx* ctx, bool kick = false, double hk = 0.0) {
         ctx->ev_used += 2;
         CK(cudaEventRecord(e0, ctx->stream));
     }
-    if (ctx->use_big) {
+    if (ctx->use_psm) {
+        BigParams bp;
+        bp.x = ctx->x; bp.gm = ctx->gm; bp.rcrit = ctx->rcrit; bp.a = ctx->a; bp.v = ctx->v;
+        bp.nb = ctx->nb; bp.nbig = ctx->nbig; bp.ld = ctx->ld; bp.hk = hk;
+        const int per = PSM_THREADS / PSM_G;
+        if (kick) pair_small_kernel<true><<<(ctx->nb + per - 1) / per, PSM_THREADS, 0, ctx->stream>>>(bp);
+        else pair_small_kernel<false><<<(ctx->nb + per - 1) / per, PSM_THREADS, 0, ctx->stream>>>(bp);
+    } else if (ctx->use_big) {
         BigParams bp;
         bp.x = ctx->x; bp.gm = ctx->gm; bp.rcrit = ctx->rcrit; bp.a = ctx->a; bp.v = ctx->v;
         bp.nb = ctx->nb; bp.nbig = ctx->nbig; bp.ld = ctx->ld; bp.hk = hk;
@@ -375,7 +387,7 @@ static mo_status enqueue_accel(mo_ctx* ctx, bool jump, double hj, bool kick, dou
     const double hjm = jump ? hj / ctx->mu : 0.0;
     const double* ps = jump ? ctx->psumB : nullptr;
     const int nps = jump ? ctx->npsum : 0;
-    if (ctx->use_big) {
+    if (ctx->use_big || ctx->use_psm) {
         // the jump still moves every body (pack_kernel also refreshes the few source tiles, unused here);
         // pair_big_kernel reads the sources from x, writes a itself and applies the closing kick
         if (jump) {
@@ -474,6 +486,22 @@ static mo_status enqueue_hill(mo_ctx* ctx, double n_hill, int mode, double* rhil
 }
 
 static mo_status enqueue_step(mo_ctx* ctx, double dt) {
+    if (ctx->use_small) {
+        SmallParams q;
+        MidParams& mp = q.m;
+        mp.x = ctx->x; mp.v = ctx->v; mp.x0 = ctx->x0; mp.v0 = ctx->v0; mp.gm = ctx->gm; mp.rcrit = ctx->rcrit;
+        mp.psum_in = nullptr; mp.psum_out = nullptr; mp.ticket = nullptr; mp.enc = ctx->enc; mp.flag = ctx->flag;
+        mp.st = ctx->dstats; mp.nb = ctx->nb; mp.ld = ctx->ld; mp.nbPad = ctx->nbPad; mp.npsum = 0; mp.nbig = ctx->nbig;
+        mp.hj_over_mu = 0.5 * dt / ctx->mu; mp.mu = ctx->mu; mp.h = dt;
+        q.a = ctx->a; q.hk = 0.5 * dt; q.pairs = ctx->pairs; q.cap = ctx->cap;
+        q.hill_mode = ctx->hill_mode; q.hill_n = ctx->hill_n;
+        int thr = (ctx->nb + 31) / 32 * 32;
+        if (thr < 64) thr = 64;
+        step_small_kernel<<<1, thr, 0, ctx->stream>>>(q);
+        mo_status ss = post_launch(ctx);
+        if (ss != MO_OK) return ss;
+        return enqueue_accel(ctx, false, 0.0, true, 0.5 * dt);   // both jumps are done: a(x), closing kick
+    }
     if (ctx->hill_mode >= 0) {
         mo_status hs = enqueue_hill(ctx, ctx->hill_n, ctx->hill_mode, nullptr);
         if (hs != MO_OK) return hs;
@@ -738,6 +766,14 @@ extern "C" mo_status mo_pair_geometry(const mo_ctx* ctx, int32_t* ipt, int32_t* 
     if (ipt) *ipt = ctx->ipt;
     if (jsplit) *jsplit = ctx->nsplit;
     if (ctas) *ctas = ctx->use_sym ? ctx->sym_nunits : ctx->use_big ? ctx->big_grid : ctx->nIblk * ctx->nsplit;
+    if (ctx->use_psm) {
+        const int per = PSM_THREADS / PSM_G;
+        if (ipt) *ipt = 1;
+        if (jsplit) *jsplit = PSM_G;
+        if (ctas) *ctas = (ctx->nb + per - 1) / per;
+        if (ctas_per_sm) *ctas_per_sm = 4;
+        return MO_OK;
+    }
     if (ctx->use_sym && jsplit) *jsplit = ctx->sym_ch;
     if (ctas_per_sm) *ctas_per_sm = ctx->ctas_per_sm;
     return MO_OK;
@@ -745,7 +781,7 @@ extern "C" mo_status mo_pair_geometry(const mo_ctx* ctx, int32_t* ipt, int32_t* 
 
 extern "C" const char* mo_pair_kernel_name(const mo_ctx* ctx) {
     if (!ctx) return nullptr;
-    return ctx->use_big ? "pair_big_kernel" : ctx->use_sym ? "pair_sym_kernel" : "pair_accel_kernel";
+    return ctx->use_psm ? "pair_small_kernel" : ctx->use_big ? "pair_big_kernel" : ctx->use_sym ? "pair_sym_kernel" : "pair_accel_kernel";
 }
 
 extern "C" mo_status mo_set_kernel_timing(mo_ctx* ctx, int32_t on) {

@@ -48,7 +48,20 @@ __global__ void __launch_bounds__(ON_BLOCK) vshift_kernel(double* __restrict__ v
     v[2 * ld + b] += sgn * (P2 / den);
 }
 
-// MODE 0: d = |x| ; MODE 1: d = osculating a from the heliocentric velocity v + P / mu (unbound: |x|)
+// Hill radius of one body.  mode 0: d = |x| ; mode 1: d = osculating a from the heliocentric velocity
+// v + P / mu, P = sum gm v (unbound: |x|)
+__device__ __forceinline__ double hill_body(double X, double Y, double Z, double vx, double vy, double vz, double g,
+                                            double mu, double P0, double P1, double P2, int mode) {
+    double d = sqrt(fma(Z, Z, fma(Y, Y, X * X)));
+    if (mode == 1) {
+        const double hx = vx + P0 / mu, hy = vy + P1 / mu, hz = vz + P2 / mu;
+        const double v2 = fma(hz, hz, fma(hy, hy, hx * hx));
+        const double inva = 2.0 / d - v2 / (mu + g);
+        if (inva > 0.0) d = 1.0 / inva;
+    }
+    return d * cbrt(g / (3.0 * mu));
+}
+
 template <int MODE>
 __global__ void __launch_bounds__(ON_BLOCK) hill_kernel(const double* __restrict__ x, const double* __restrict__ v,
                                                         const double* __restrict__ gm, const double* __restrict__ psum,
@@ -56,18 +69,12 @@ __global__ void __launch_bounds__(ON_BLOCK) hill_kernel(const double* __restrict
                                                         double* __restrict__ rcrit, double* __restrict__ rhill) {
     const int b = blockIdx.x * ON_BLOCK + threadIdx.x;
     if (b >= nb) return;
-    const double X = x[b], Y = x[ld + b], Z = x[2 * ld + b];
-    const double g = gm[b];
-    double d = sqrt(fma(Z, Z, fma(Y, Y, X * X)));
+    double P0 = 0.0, P1 = 0.0, P2 = 0.0, vx = 0.0, vy = 0.0, vz = 0.0;
     if (MODE == 1) {
-        double P0, P1, P2;
         load_psum(psum, npsum, P0, P1, P2);
-        const double vx = v[b] + P0 / mu, vy = v[ld + b] + P1 / mu, vz = v[2 * ld + b] + P2 / mu;
-        const double v2 = fma(vz, vz, fma(vy, vy, vx * vx));
-        const double inva = 2.0 / d - v2 / (mu + g);
-        if (inva > 0.0) d = 1.0 / inva;
+        vx = v[b]; vy = v[ld + b]; vz = v[2 * ld + b];
     }
-    const double rh = d * cbrt(g / (3.0 * mu));
+    const double rh = hill_body(x[b], x[ld + b], x[2 * ld + b], vx, vy, vz, gm[b], mu, P0, P1, P2, MODE);
     if (rhill) rhill[b] = rh;
     rcrit[b] = nhill * rh;
 }

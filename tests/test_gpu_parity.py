@@ -79,12 +79,16 @@ def test_accel_headline_sizes_sampled_rows(M, cfg):
     m.close()
 
 
-@pytest.mark.parametrize("nb", [1, 2, 3, 127, 128, 129, 255, 257, 1000])
-def test_accel_ragged_sizes_and_changeover_shell(M, nb):
+@pytest.mark.parametrize("psm", ["1", "0"])
+@pytest.mark.parametrize("nb", [1, 2, 3, 7, 8, 9, 127, 128, 129, 255, 257, 1000, 1024])
+def test_accel_ragged_sizes_and_changeover_shell(M, monkeypatch, nb, psm):
+    """psm = 1: pair_small_kernel (8 lanes per body); psm = 0: the tiled one-sided pair_accel_kernel"""
+    monkeypatch.setenv("MO_PSM", psm)
     w = W.random_cluster(nb, 100 + nb, box=1.0, rc_frac=(0.0, 0.7)) if nb > 1 else W.random_cluster(1, 5)
     if nb > 100:   # plant one pair well inside 0.1 rc (K = 0) - random draws do not always have one
         w.x[:, 1] = w.x[:, 0] + np.array([0.03 * max(w.rcrit[0], w.rcrit[1]), 0.0, 0.0])
     m = _mk(M, w)
+    assert m.pair_kernel_name() == ("pair_small_kernel" if psm == "1" else "pair_accel_kernel")
     m.accel()
     a = m.get("a")
     a_ref, S = oracle.accel(G * w.mass, w.x, w.rcrit)
@@ -101,6 +105,7 @@ def force_sym(monkeypatch):
     """Select the two-sided pair kernel (pair_sym_kernel) whatever nb is; MO_SYM is read by mo_create."""
     def _set(ch=None):
         monkeypatch.setenv("MO_SYM", "1")
+        monkeypatch.setenv("MO_PSM", "0")
         if ch is not None:
             monkeypatch.setenv("MO_SYM_CH", str(ch))
     return _set
@@ -430,7 +435,7 @@ def test_invalid_arguments_and_bookkeeping(M):
                        m.rcrit.data_ptr(), None, 0, m.flag.data_ptr(), None) == M.MO_EINVAL   # ld % 4
     n0 = m.launch_count()
     m.accel()
-    assert m.launch_count() == n0 + 3 and m.workspace_bytes() > 0
+    assert m.launch_count() == n0 + (1 if m.pair_kernel_name() == "pair_small_kernel" else 3) and m.workspace_bytes() > 0
     g = m.pair_geometry()
     assert g["ctas"] >= 1 and g["ipt"] in (1, 2)
     tf, ms = M.probe_fp64_peak(2)
@@ -695,3 +700,75 @@ def test_support_invalid(M):
     assert L.mo_energy(m._ctx, None) == M.MO_EINVAL
     assert L.mo_h2dh(None) == M.MO_EINVAL and L.mo_dh2h(None) == M.MO_EINVAL
     m.close()
+
+
+# ------------------------------------------------------------------------------ single-CTA step front end (nb <= 1024)
+@pytest.mark.parametrize("cfg,N,nbig,hill", [(1, 1025, None, -1), (1, 700, None, 0), (3, 900, None, 1), (1, 800, 2, -1),
+                                            (4, 333, 100, 0), (2, 33, None, -1)])
+def test_step_small_path_vs_oracle(M, monkeypatch, cfg, N, nbig, hill):
+    """nb <= 1024: hill, kick, jump, snapshot, drift, boxes, pair test and second jump run in one kernel."""
+    monkeypatch.setenv("MO_SMALL_MAX", "1024")
+    w = W.shrink(cfg, N)
+    scale = 40.0 if cfg in (2, 4) else 1.0
+    rc0 = w.rcrit * scale
+    gm, mu = G * w.mass, G * w.m_star
+    m = _mk(M, w, rcrit=rc0)
+    if nbig is not None:
+        m.set_nbig(nbig)
+    if hill >= 0:
+        m.set_hill(3.0 * scale, hill)
+    a, _ = oracle.accel(gm, w.x, rc0, nbig=nbig)
+    x, v, rc = w.x, w.v, rc0
+    seen = 0
+    for k in range(4):
+        st = m.step(w.dt, 1)
+        if hill >= 0:
+            _, rc = oracle.hill(G, w.m_star, w.mass, x, v, n_hill=3.0 * scale, mode=hill)
+        r = oracle.step(mu, gm, rc, w.dt, x, v, a, nbig=nbig)
+        x, v, a = r["x"], r["v"], r["a"]
+        ex, ev = _step_err(m, r)
+        tol = 1e-13 * (1 + k)
+        assert ex <= tol and ev <= tol, (k, ex, ev)
+        assert st.steps_done == k + 1 and st.drift_fail == 0
+        got = m.pair_list(st.nce_last)
+        _pairs_ok(got, r)
+        assert got.tolist() == sorted(got.tolist())
+        if r["n_ambig"] == 0:
+            assert st.nce_last == r["count"] and np.array_equal(m.get("flag"), r["flag"])
+        seen += st.nce_last
+        x0, v0 = m.snapshot_tensors()
+        assert _rel_vec_err(x0[:, :w.nb].cpu().numpy(), r["x0"]).max() <= tol
+    assert seen > 0 or cfg == 2
+    m2 = _mk(M, w, rcrit=rc0)                       # graph replay gives the same trajectory
+    if nbig is not None:
+        m2.set_nbig(nbig)
+    if hill >= 0:
+        m2.set_hill(3.0 * scale, hill)
+    st2 = m2.step(w.dt, 4)
+    assert np.array_equal(m.get("x"), m2.get("x")) and np.array_equal(m.get("v"), m2.get("v"))
+    assert st2.nce_last == st.nce_last and st2.nce_total == seen
+    m.close(); m2.close()
+
+
+def test_step_small_path_overflow_and_large_path_agree(M, monkeypatch):
+    monkeypatch.setenv("MO_SMALL_MAX", "1024")
+    w = W.shrink(4, 500)
+    huge = np.full(w.nb, 1e3)
+    total = w.nb * (w.nb - 1) // 2
+    m = M.Mopal(w.mass, w.x, w.v, huge, cap=777)
+    st = m.step(w.dt, 1)
+    assert st.status == M.MO_EOVERFLOW
+    assert st.nce_last == total and m.get("flag").all()
+    got = m.pair_list(st.nce_last)
+    ref = [(i, j) for i in range(w.nb) for j in range(i + 1, w.nb)][:777]
+    assert got.tolist() == [list(t) for t in ref]
+    m.close()
+    # the multi-kernel front end (MO_SMALL=0) and the single-CTA one agree to rounding of the two 3-vector sums
+    w = W.shrink(1, 900)
+    m1 = _mk(M, w); s1 = m1.step(w.dt, 3)
+    monkeypatch.setenv("MO_SMALL", "0")
+    m2 = _mk(M, w); s2 = m2.step(w.dt, 3)
+    monkeypatch.delenv("MO_SMALL")
+    assert _rel_vec_err(m1.get("x"), m2.get("x")).max() <= 1e-14 and _rel_vec_err(m1.get("v"), m2.get("v")).max() <= 1e-14
+    assert s1.nce_last == s2.nce_last and np.array_equal(m1.pair_list(s1.nce_last), m2.pair_list(s2.nce_last))
+    m1.close(); m2.close()

@@ -54,6 +54,7 @@ struct mo_ctx {
     // few gravity sources (mo_set_nbig with nbig <= MO_BIG_MAX): sources in shared memory, direct big-row encounter pass
     bool use_big = false;
     int big_ipt = 1, big_grid = 1;
+    int psm_g = 8;                      // lanes per body of pair_small_kernel
     bool use_psm = false;               // nb <= PSM_MAX: pair_small_kernel (several lanes per body) instead of pack + pair + reduce
     bool use_small = false;             // nb <= SMALL_MAX: the pre-acceleration part of the step is one single-CTA kernel
     int gkernels = 0;                   // kernel launches recorded in the cached step graph
@@ -158,7 +159,9 @@ static void choose_geometry(mo_ctx* ctx) {
     if (ctx->enc_split > 8) ctx->enc_split = 8;
     // two-sided kernel for large nb: units = (row block, chunk of sym_ch j tiles from the diagonal on)
     ctx->use_small = nb <= env_int("MO_SMALL_MAX", 400) && nb <= SMALL_MAX && env_int("MO_SMALL", 1) != 0;
-    ctx->use_psm = nb <= env_int("MO_PSM_MAX", PSM_MAX) && nb <= PSM_MAX && env_int("MO_PSM", 1) != 0;
+    ctx->use_psm = nb <= env_int("MO_PSM_MAX", 1024) && nb <= PSM_MAX && env_int("MO_PSM", 1) != 0;
+    ctx->psm_g = env_int("MO_PSM_G", 8);
+    if (ctx->psm_g != 2 && ctx->psm_g != 4 && ctx->psm_g != 8) ctx->psm_g = 8;
     ctx->use_big = !ctx->use_psm && ctx->nbig < nb && ctx->nbig <= env_int("MO_BIG_MAX", 4096);
     if (ctx->use_big) {
         // bodies per thread: as many as still leave about two waves of CTAs
@@ -362,9 +365,12 @@ static mo_status launch_pair(mo_ctx* ctx, bool kick = false, double hk = 0.0) {
         BigParams bp;
         bp.x = ctx->x; bp.gm = ctx->gm; bp.rcrit = ctx->rcrit; bp.a = ctx->a; bp.v = ctx->v;
         bp.nb = ctx->nb; bp.nbig = ctx->nbig; bp.ld = ctx->ld; bp.hk = hk;
-        const int per = PSM_THREADS / PSM_G;
-        if (kick) pair_small_kernel<true><<<(ctx->nb + per - 1) / per, PSM_THREADS, 0, ctx->stream>>>(bp);
-        else pair_small_kernel<false><<<(ctx->nb + per - 1) / per, PSM_THREADS, 0, ctx->stream>>>(bp);
+        const int G = ctx->psm_g, per = PSM_THREADS / G;
+        const int grid = (ctx->nb + per - 1) / per;
+        auto k = G == 8 ? (kick ? pair_small_kernel<8, true> : pair_small_kernel<8, false>)
+               : G == 4 ? (kick ? pair_small_kernel<4, true> : pair_small_kernel<4, false>)
+                        : (kick ? pair_small_kernel<2, true> : pair_small_kernel<2, false>);
+        k<<<grid, PSM_THREADS, 0, ctx->stream>>>(bp);
     } else if (ctx->use_big) {
         BigParams bp;
         bp.x = ctx->x; bp.gm = ctx->gm; bp.rcrit = ctx->rcrit; bp.a = ctx->a; bp.v = ctx->v;
@@ -465,7 +471,7 @@ static mo_status enqueue_pairs(mo_ctx* ctx, const EncState& es, int step_inc) {
     EncWriteParams wp;
     wp.s = es; wp.e = ctx->enc; wp.pairs = ctx->pairs; wp.cap = ctx->cap; wp.flag = ctx->flag;
     int blocks = (ctx->nbig + 7) / 8;
-    const int maxb = ctx->nsm * 8;
+    const int maxb = ctx->nsm;            // it exits at once unless count > cap: keep the empty launch small
     if (blocks > maxb) blocks = maxb;
     enc_write_kernel<<<blocks, 256, 0, ctx->stream>>>(wp);   // exits at once unless count > cap
     return post_launch(ctx);
@@ -767,9 +773,9 @@ extern "C" mo_status mo_pair_geometry(const mo_ctx* ctx, int32_t* ipt, int32_t* 
     if (jsplit) *jsplit = ctx->nsplit;
     if (ctas) *ctas = ctx->use_sym ? ctx->sym_nunits : ctx->use_big ? ctx->big_grid : ctx->nIblk * ctx->nsplit;
     if (ctx->use_psm) {
-        const int per = PSM_THREADS / PSM_G;
+        const int per = PSM_THREADS / ctx->psm_g;
         if (ipt) *ipt = 1;
-        if (jsplit) *jsplit = PSM_G;
+        if (jsplit) *jsplit = ctx->psm_g;
         if (ctas) *ctas = (ctx->nb + per - 1) / per;
         if (ctas_per_sm) *ctas_per_sm = 4;
         return MO_OK;

@@ -193,58 +193,63 @@ __global__ void __launch_bounds__(BIG_THREADS) pair_big_kernel(BigParams p) {
     }
 }
 
-// ---- tiny systems (nb <= PSM_MAX, the paper's own regime N <= 1000) -----------------
-// There are too few bodies to fill the chip with one thread per body, so PSM_G lanes share a body: lane g
-// sums the sources j = g, g + PSM_G, ... (ascending), the PSM_G partial sums are combined by a fixed
-// shuffle tree, lane 0 writes a_i (and the closing kick).  All sources live in shared memory; same per-pair
+// ---- small systems (nb <= PSM_MAX; the paper's own regime is N <= 1000) -------------
+// There are too few bodies to fill the chip with one thread per body, so G lanes share a body: lane g
+// sums the sources j = g, g + G, ... of each staged chunk (ascending), the G partial sums are combined by a
+// fixed shuffle tree, lane 0 writes a_i (and the closing kick).  Sources are staged in shared memory; same per-pair
 // arithmetic, per-source gate and in-line changeover weight as pair_big_kernel.  One launch replaces
 // pack + pair + reduce.
-constexpr int PSM_MAX = 1024;
-constexpr int PSM_G = 8;
+constexpr int PSM_MAX = 8191;         // above: the two-sided kernel
+constexpr int PSM_CHUNK = 1024;       // sources staged per pass
 constexpr int PSM_THREADS = 128;
 
-template <bool KICK>
+template <int G, bool KICK>
 __global__ void __launch_bounds__(PSM_THREADS) pair_small_kernel(BigParams p) {
-    __shared__ __align__(16) double2 s_src[2 * PSM_MAX];
-    __shared__ int s_gj[PSM_MAX];
-    __shared__ double s_rc[PSM_MAX];
+    __shared__ __align__(16) double2 s_src[2 * PSM_CHUNK];
+    __shared__ int s_gj[PSM_CHUNK];
+    __shared__ double s_rc[PSM_CHUNK];
     const int tid = threadIdx.x;
-    for (int j = tid; j < p.nbig; j += PSM_THREADS) {
-        s_src[2 * j] = make_double2(p.x[j], p.x[p.ld + j]);
-        s_src[2 * j + 1] = make_double2(p.x[2 * p.ld + j], p.gm[j]);
-        const double rc = p.rcrit[j];
-        s_gj[j] = __double2hiint(rc * rc);
-        s_rc[j] = rc;
-    }
-    const int i = blockIdx.x * (PSM_THREADS / PSM_G) + tid / PSM_G;
-    const int g = tid % PSM_G;
+    const int i = blockIdx.x * (PSM_THREADS / G) + tid / G;
+    const int g = tid % G;
     const bool live = i < p.nb;
     const double xi = live ? p.x[i] : 0.0, yi = live ? p.x[p.ld + i] : 0.0, zi = live ? p.x[2 * p.ld + i] : 0.0;
     const double rci = live ? p.rcrit[i] : 0.0;
     const int gi = __double2hiint(rci * rci);
     double vx = 0.0, vy = 0.0, vz = 0.0;
     if (KICK && live && g == 0) { vx = p.v[i]; vy = p.v[p.ld + i]; vz = p.v[2 * p.ld + i]; }
-    __syncthreads();
     double ax = 0.0, ay = 0.0, az = 0.0;
+    for (int j0 = 0; j0 < p.nbig; j0 += PSM_CHUNK) {
+        const int n = min(PSM_CHUNK, p.nbig - j0);
+        __syncthreads();                                   // previous chunk fully consumed
+        for (int t = tid; t < n; t += PSM_THREADS) {
+            const int j = j0 + t;
+            s_src[2 * t] = make_double2(p.x[j], p.x[p.ld + j]);
+            s_src[2 * t + 1] = make_double2(p.x[2 * p.ld + j], p.gm[j]);
+            const double rc = p.rcrit[j];
+            s_gj[t] = __double2hiint(rc * rc);
+            s_rc[t] = rc;
+        }
+        __syncthreads();
 #pragma unroll 4
-    for (int j = g; j < p.nbig; j += PSM_G) {
-        const double2 pa = s_src[2 * j], pb = s_src[2 * j + 1];
-        const double dx = pa.x - xi, dy = pa.y - yi, dz = pb.x - zi;
-        const double s2 = fma(dz, dz, fma(dy, dy, dx * dx));
-        const double y = rsqrt_seed(s2);
-        const double y2 = y * y;
-        const double e = fma(-s2, y2, 1.0);
-        const double w0 = (pb.y * y) * y2;
-        const double t = e * fma(1.875, e, 1.5);
-        double w = fma(w0, t, w0);
-        if (__double2hiint(s2) <= max(gi, s_gj[j])) w = changeover_weight(s2, w, fmax(rci, s_rc[j]));
-        ax = fma(w, dx, ax); ay = fma(w, dy, ay); az = fma(w, dz, az);
+        for (int j = g; j < n; j += G) {
+            const double2 pa = s_src[2 * j], pb = s_src[2 * j + 1];
+            const double dx = pa.x - xi, dy = pa.y - yi, dz = pb.x - zi;
+            const double s2 = fma(dz, dz, fma(dy, dy, dx * dx));
+            const double y = rsqrt_seed(s2);
+            const double y2 = y * y;
+            const double e = fma(-s2, y2, 1.0);
+            const double w0 = (pb.y * y) * y2;
+            const double t = e * fma(1.875, e, 1.5);
+            double w = fma(w0, t, w0);
+            if (__double2hiint(s2) <= max(gi, s_gj[j])) w = changeover_weight(s2, w, fmax(rci, s_rc[j]));
+            ax = fma(w, dx, ax); ay = fma(w, dy, ay); az = fma(w, dz, az);
+        }
     }
 #pragma unroll
-    for (int o = PSM_G / 2; o > 0; o >>= 1) {
-        ax += __shfl_down_sync(0xffffffffu, ax, o, PSM_G);
-        ay += __shfl_down_sync(0xffffffffu, ay, o, PSM_G);
-        az += __shfl_down_sync(0xffffffffu, az, o, PSM_G);
+    for (int o = G / 2; o > 0; o >>= 1) {
+        ax += __shfl_down_sync(0xffffffffu, ax, o, G);
+        ay += __shfl_down_sync(0xffffffffu, ay, o, G);
+        az += __shfl_down_sync(0xffffffffu, az, o, G);
     }
     if (live && g == 0) {
         p.a[i] = ax; p.a[p.ld + i] = ay; p.a[2 * p.ld + i] = az;

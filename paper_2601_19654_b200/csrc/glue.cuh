@@ -36,6 +36,8 @@ __global__ void __launch_bounds__(ON_BLOCK) kick_psum_kernel(double* __restrict_
 
 struct MidParams {
     double *x, *v, *x0, *v0;
+    double *x1, *v1;        // nullable: second copy of the drifted state, read by the encounter pass while the
+                            // jump / pair sum / kick branch already moves x and v (overlapped step)
     const double *gm, *rcrit;
     const double* psum_in;  // partials of sum gm v before the drift
     double* psum_out;       // partials after the drift
@@ -70,6 +72,10 @@ __global__ void __launch_bounds__(ON_BLOCK) jump_drift_boxes_kernel(MidParams p)
         if (iters > 3) atomicMax(&p.st->max_newton, iters);
         p.x[b] = x; p.x[ld + b] = y; p.x[2 * ld + b] = z;
         p.v[b] = vx; p.v[ld + b] = vy; p.v[2 * ld + b] = vz;
+        if (p.x1) {
+            p.x1[b] = x; p.x1[ld + b] = y; p.x1[2 * ld + b] = z;
+            p.v1[b] = vx; p.v1[ld + b] = vy; p.v1[2 * ld + b] = vz;
+        }
         const double rc = b < p.nbig ? p.rcrit[b] : 0.0;   // LOOP 2 pads the big bodies only
         double lo, hi;
         double4 bx;

@@ -30,6 +30,12 @@ struct mo_ctx {
     uint8_t* flag = nullptr;
     cudaStream_t stream = nullptr;
     cudaStream_t cap_stream = nullptr;  // owned: graph capture needs a non-legacy stream
+    // overlapped step: the encounter pass runs on a second (high-priority) stream beside jump + pair sum + kick,
+    // reading its own copy x1, v1 of the drifted state
+    bool overlap = false;
+    cudaStream_t enc_stream = nullptr;
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+    double *x1 = nullptr, *v1 = nullptr;
     // owned scratch
     double *gm = nullptr, *x0 = nullptr, *v0 = nullptr, *part = nullptr, *psumA = nullptr, *psumB = nullptr;
     unsigned* ticket = nullptr;         // two last-block counters (psumA, psumB)
@@ -222,6 +228,10 @@ extern "C" void mo_destroy(mo_ctx* ctx) {
     if (!ctx) return;
     if (ctx->gexec) cudaGraphExecDestroy(ctx->gexec);
     if (ctx->cap_stream) cudaStreamDestroy(ctx->cap_stream);
+    if (ctx->enc_stream) cudaStreamDestroy(ctx->enc_stream);
+    if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
+    if (ctx->ev_join) cudaEventDestroy(ctx->ev_join);
+    cudaFree(ctx->x1); cudaFree(ctx->v1);
     for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
     cudaFree(ctx->gm); cudaFree(ctx->x0); cudaFree(ctx->v0); cudaFree(ctx->part);
     cudaFree(ctx->psumA); cudaFree(ctx->psumB); cudaFree(ctx->ticket);
@@ -325,6 +335,16 @@ extern "C" mo_status mo_create(mo_ctx** out, int32_t nb, int32_t ld, double m_st
 static mo_status ensure_pair_scratch(mo_ctx* ctx) {
     if (ctx->pair_ready) return MO_OK;
     cudaError_t e = cudaSuccess;
+    ctx->overlap = !ctx->use_small && ctx->nb >= env_int("MO_OVERLAP_MIN", 8192) && env_int("MO_OVERLAP", 1) != 0;
+    if (ctx->overlap && !ctx->enc_stream) {
+        int lo = 0, hi = 0;
+        cudaDeviceGetStreamPriorityRange(&lo, &hi);
+        e = cudaStreamCreateWithPriority(&ctx->enc_stream, cudaStreamNonBlocking, hi);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_join, cudaEventDisableTiming);
+        if (e == cudaSuccess) e = dalloc(ctx, &ctx->x1, 3 * (size_t)ctx->ld);
+        if (e == cudaSuccess) e = dalloc(ctx, &ctx->v1, 3 * (size_t)ctx->ld);
+    }
     const size_t pl = 3 * (size_t)ctx->ld;
     if (!ctx->use_sym && !ctx->use_big && !ctx->use_psm) e = dalloc(ctx, &ctx->part, pl * (size_t)ctx->nsplit);
     if (ctx->use_sym) {
@@ -496,6 +516,7 @@ static mo_status enqueue_step(mo_ctx* ctx, double dt) {
         SmallParams q;
         MidParams& mp = q.m;
         mp.x = ctx->x; mp.v = ctx->v; mp.x0 = ctx->x0; mp.v0 = ctx->v0; mp.gm = ctx->gm; mp.rcrit = ctx->rcrit;
+        mp.x1 = nullptr; mp.v1 = nullptr;
         mp.psum_in = nullptr; mp.psum_out = nullptr; mp.ticket = nullptr; mp.enc = ctx->enc; mp.flag = ctx->flag;
         mp.st = ctx->dstats; mp.nb = ctx->nb; mp.ld = ctx->ld; mp.nbPad = ctx->nbPad; mp.npsum = 0; mp.nbig = ctx->nbig;
         mp.hj_over_mu = 0.5 * dt / ctx->mu; mp.mu = ctx->mu; mp.h = dt;
@@ -517,13 +538,32 @@ static mo_status enqueue_step(mo_ctx* ctx, double dt) {
     if (s != MO_OK) return s;
     MidParams mp;
     mp.x = ctx->x; mp.v = ctx->v; mp.x0 = ctx->x0; mp.v0 = ctx->v0; mp.gm = ctx->gm; mp.rcrit = ctx->rcrit;
-    mp.psum_in = ctx->psumA; mp.psum_out = ctx->psumB; mp.ticket = ctx->ticket + 1; mp.enc = ctx->enc; mp.flag = ctx->flag;
+    mp.psum_in = ctx->psumA; mp.psum_out = ctx->psumB; mp.ticket = ctx->ticket + 1;
+    mp.x1 = ctx->overlap ? ctx->x1 : nullptr; mp.v1 = ctx->overlap ? ctx->v1 : nullptr; mp.enc = ctx->enc; mp.flag = ctx->flag;
     mp.st = ctx->dstats; mp.nb = ctx->nb; mp.ld = ctx->ld; mp.nbPad = ctx->nbPad; mp.npsum = ctx->npsum;
     mp.nbig = ctx->nbig;
     mp.hj_over_mu = 0.5 * dt / ctx->mu; mp.mu = ctx->mu; mp.h = dt;
     jump_drift_boxes_kernel<<<ctx->npsum, ON_BLOCK, 0, ctx->stream>>>(mp);
     s = post_launch(ctx);
     if (s != MO_OK) return s;
+    if (ctx->overlap) {
+        // fork: encounter pass on enc_stream (reads x0, v0, x1, v1, boxes, rcrit; writes pairs, flag, stats),
+        // jump + pair sum + closing kick on the main stream (moves x, v; writes a); join at the end
+        cudaStream_t mainS = ctx->stream;
+        CK(cudaEventRecord(ctx->ev_fork, mainS));
+        CK(cudaStreamWaitEvent(ctx->enc_stream, ctx->ev_fork, 0));
+        EncState es = enc_state(ctx, ctx->x0, ctx->v0, dt);
+        es.x1 = ctx->x1; es.v1 = ctx->v1;
+        ctx->stream = ctx->enc_stream;
+        s = enqueue_pairs(ctx, es, 1);
+        ctx->stream = mainS;
+        if (s != MO_OK) return s;
+        CK(cudaEventRecord(ctx->ev_join, ctx->enc_stream));
+        s = enqueue_accel(ctx, true, 0.5 * dt, true, 0.5 * dt);
+        if (s != MO_OK) return s;
+        CK(cudaStreamWaitEvent(mainS, ctx->ev_join, 0));
+        return MO_OK;
+    }
     s = enqueue_pairs(ctx, enc_state(ctx, ctx->x0, ctx->v0, dt), 1);
     if (s != MO_OK) return s;
     return enqueue_accel(ctx, true, 0.5 * dt, true, 0.5 * dt);

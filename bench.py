@@ -43,10 +43,10 @@ FP64_LANES_PER_SM = 64        # DESIGN.md section "Rooflines": 148 SMs x 64 DFMA
 EXECUTED_FLOP_PER_PAIR = 15.5
 # one-sided kernels (pair_accel_kernel, pair_big_kernel): 3 DADD + 5 DMUL + 8 DFMA per ordered pair
 EXECUTED_FLOP_PER_PAIR_ONE_SIDED = 24.0
-# dram__bytes_read.sum + dram__bytes_write.sum of one launch of the pair kernel from the ncu --set full captures
-# summarised in profiles/r1d_kernels_full.md: pair_sym_kernel at config 3 (5.1 MB read + 93.3 MB written),
-# pair_big_kernel at --bigsmall 1000000,100 (56.0 MB read + 2.9 MB written)
-PAIR_KERNEL_DRAM_TRAFFIC_BYTES = {3: 98.4e6, "1000000,100": 58.9e6}
+# dram__bytes_read.sum + dram__bytes_write.sum of one launch of the pair kernel from the ncu --set full captures:
+# pair_sym_kernel at config 3 (profiles/r1f_launches.md: 5.2 MB read + 91.1 MB written),
+# pair_big_kernel at --bigsmall 1000000,100 (profiles/r1d_kernels_full.md: 56.0 MB read + 2.9 MB written)
+PAIR_KERNEL_DRAM_TRAFFIC_BYTES = {3: 96.3e6, "1000000,100": 58.9e6}
 
 
 def reduce_max_over_ranks(values, dist=None, device="cpu"):

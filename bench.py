@@ -438,6 +438,48 @@ def run_support(args):
     return 0
 
 
+def run_step_sweep(args):
+    """Step time (CUDA-graph replay of 1000 steps, CUDA events) of the cfg1 disk recipe at small and middle sizes
+    through each launch path the library can take, selected with its MO_* environment switches (read at
+    mo_create): the evidence behind the default thresholds in choose_geometry().  One JSON line."""
+    import torch
+    from paper_2601_19654_b200 import mopal as M
+    from paper_2601_19654_b200 import workloads as W
+    keys = ("MO_SMALL", "MO_SMALL_MAX", "MO_PSM", "MO_PSM_MAX", "MO_OVERLAP_MIN", "MO_OVERLAP")
+    paths = {"default": {},
+             "single_cta_front_end+lane_split_pair": {"MO_SMALL_MAX": "1024", "MO_PSM_MAX": "8191"},
+             "lane_split_pair+overlap": {"MO_SMALL": "0", "MO_PSM_MAX": "8191", "MO_OVERLAP_MIN": "1"},
+             "lane_split_pair": {"MO_SMALL": "0", "MO_PSM_MAX": "8191", "MO_OVERLAP": "0"},
+             "tiled_pair+overlap": {"MO_SMALL": "0", "MO_PSM": "0", "MO_OVERLAP_MIN": "1"},
+             "tiled_pair (round 1d)": {"MO_SMALL": "0", "MO_PSM": "0", "MO_OVERLAP": "0"}}
+    saved = {k: os.environ.get(k) for k in keys}
+    rows = []
+    for N in [64, 128, 256, 384, 512, 768, 1000, 1536, 2048, 3072, 4096, 8192]:
+        w = W.make_config(0) if N == 256 else W.make_config(1) if N == 4096 else W.shrink(1, N)
+        row = {"N": N}
+        for tag, env in paths.items():
+            if tag.startswith("single_cta") and w.nb > 1024:
+                continue
+            for k in keys:
+                os.environ.pop(k, None)
+            os.environ.update(env)
+            m = M.Mopal(w.mass, w.x, w.v, w.rcrit, m_star=w.m_star, G=w.G)
+            m.step(w.dt, 5)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(m.stream); m.step(w.dt, 1000); e1.record(m.stream); torch.cuda.synchronize()
+            row[tag] = round(e0.elapsed_time(e1), 1)          # ms per 1000 steps = us per step
+            if tag == "default":
+                row["default_pair_kernel"] = m.pair_kernel_name()
+            m.close()
+        rows.append(row)
+    for k, v in saved.items():
+        os.environ.pop(k, None)
+        if v is not None:
+            os.environ[k] = v
+    print(json.dumps({"metric": "us_per_step_by_launch_path", "workload": "cfg1 recipe at N (cfg0 at 256)", "rows": rows}), flush=True)
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -451,7 +493,10 @@ def main():
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of CPU work for the cpu_baseline sample")
     ap.add_argument("--drift-sweep", action="store_true", help="time mo_drift alone against the HBM roofline and exit")
     ap.add_argument("--support", action="store_true", help="time mo_energy / mo_hill / mo_dh2h against their rooflines and exit")
+    ap.add_argument("--step-sweep", action="store_true", help="step time at small / middle N through every launch path and exit")
     args = ap.parse_args()
+    if args.step_sweep:
+        return run_step_sweep(args)
     if args.support:
         return run_support(args)
     if args.drift_sweep:

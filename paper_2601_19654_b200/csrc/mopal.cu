@@ -164,8 +164,10 @@ static void choose_geometry(mo_ctx* ctx) {
     if (ctx->enc_split < 1) ctx->enc_split = 1;
     if (ctx->enc_split > 8) ctx->enc_split = 8;
     // two-sided kernel for large nb: units = (row block, chunk of sym_ch j tiles from the diagonal on)
-    ctx->use_small = nb <= env_int("MO_SMALL_MAX", 400) && nb <= SMALL_MAX && env_int("MO_SMALL", 1) != 0;
-    ctx->use_psm = nb <= env_int("MO_PSM_MAX", 1024) && nb <= PSM_MAX && env_int("MO_PSM", 1) != 0;
+    ctx->use_small = nb <= env_int("MO_SMALL_MAX", 320) && nb <= SMALL_MAX && env_int("MO_SMALL", 1) != 0;
+    // measured (profiles/r1g_path_selection.md): single-CTA front end up to ~320 bodies, lane-split pair kernel up to
+    // ~2500, tiled one-sided kernel up to 8191, two-sided kernel above
+    ctx->use_psm = nb <= env_int("MO_PSM_MAX", 2560) && nb <= PSM_MAX && env_int("MO_PSM", 1) != 0;
     ctx->psm_g = env_int("MO_PSM_G", 8);
     if (ctx->psm_g != 2 && ctx->psm_g != 4 && ctx->psm_g != 8) ctx->psm_g = 8;
     ctx->use_big = !ctx->use_psm && ctx->nbig < nb && ctx->nbig <= env_int("MO_BIG_MAX", 4096);
@@ -335,7 +337,7 @@ extern "C" mo_status mo_create(mo_ctx** out, int32_t nb, int32_t ld, double m_st
 static mo_status ensure_pair_scratch(mo_ctx* ctx) {
     if (ctx->pair_ready) return MO_OK;
     cudaError_t e = cudaSuccess;
-    ctx->overlap = !ctx->use_small && ctx->nb >= env_int("MO_OVERLAP_MIN", 8192) && env_int("MO_OVERLAP", 1) != 0;
+    ctx->overlap = !ctx->use_small && ctx->nb >= env_int("MO_OVERLAP_MIN", 1) && env_int("MO_OVERLAP", 1) != 0;
     if (ctx->overlap && !ctx->enc_stream) {
         int lo = 0, hi = 0;
         cudaDeviceGetStreamPriorityRange(&lo, &hi);

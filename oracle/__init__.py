@@ -78,6 +78,8 @@ def _lib(kind="ld"):
     L.oracle_hill.argtypes = [I, I, I, C.c_double, C.c_double, C.c_double, D, D, D, D, D]
     L.oracle_energy.restype = I
     L.oracle_energy.argtypes = [I, I, I, C.c_double, C.c_double, D, D, D, D]
+    L.oracle_resolve.restype = I
+    L.oracle_resolve.argtypes = [I, I, C.c_double, D, D, C.c_double, D, D, D, D, P32, I64, C.c_double, P32]
     _loaded[kind] = L
     return L
 
@@ -262,3 +264,19 @@ def energy(G, m_star, mass, x, v, nbig=None, kind="ld"):
     out = np.zeros(11)
     assert _lib(kind).oracle_energy(nb, _nbig(nbig, nb), nb, float(G), float(m_star), _dp(mass), _dp(x), _dp(v), _dp(out)) == 0
     return dict(T=out[0], Us=out[1], Up=out[2], E=out[3], L=out[4:7].copy(), Eabs=out[7], Labs=out[8:11].copy())
+
+
+def resolve(mu, gm, rcrit, h, x0, v0, x, v, pairs, tol=1e-12, kind="ld"):
+    """X-1..X-5: Bulirsch-Stoer integration of the bodies in ``pairs`` from the snapshot (x0, v0) over h under the
+    star's Kepler term and the (1 - K)-weighted listed pair forces; other bodies keep (x, v).
+    Returns dict(x, v, n, nsteps, nrhs, fail)."""
+    x0 = _soa(x0); v0 = _soa(v0); x = _soa(x).copy(); v = _soa(v).copy()
+    gm = _vec(gm); rcrit = _vec(rcrit)
+    pairs = np.ascontiguousarray(pairs, dtype=np.int32).reshape(-1, 2)
+    nb = x.shape[1]
+    st = np.zeros(4, dtype=np.int32)
+    rc = _lib(kind).oracle_resolve(nb, nb, float(mu), _dp(gm), _dp(rcrit), float(h), _dp(x0), _dp(v0), _dp(x), _dp(v),
+                                   pairs.ctypes.data_as(C.POINTER(C.c_int32)), len(pairs), float(tol),
+                                   st.ctypes.data_as(C.POINTER(C.c_int32)))
+    assert rc in (0, 1), rc
+    return dict(x=x, v=v, n=int(st[0]), nsteps=int(st[1]), nrhs=int(st[2]), fail=int(st[3]))

@@ -46,6 +46,10 @@
  *                perihelion; energy/L - two-body closed forms -GMm/2a and reduced-mass
  *                sqrt(mu a (1-e^2)), mpmath brute force over all N+1 bodies, dt^2
  *                scaling of the step's energy error                  -> pinned
+ *   resolve    : no interaction left => the pinned Kepler drift; scipy DOP853 on the same
+ *                equations written with the pinned changeover function (inside the shell, inside
+ *                0.1 rc, negative h); time reversal; energy of the composed hybrid step through
+ *                a close encounter with / without the encounter solve     -> pinned
  *   multi-step trajectories beyond ~10 steps: parity unpinned by construction
  *   (chaos; the paper itself compares curves and medians).
  */
@@ -792,4 +796,170 @@ int oracle_energy(int nb, int nbig, int ld, double G, double mstar, const double
     for (int c = 0; c < 3; ++c) { out[4 + c] = (double)L[c]; out[8 + c] = (double)Labs[c]; }
     out[7] = (double)Eabs;
     return 0;
+}
+
+/* ---------------------------------------------------------------------------
+ * Close-encounter resolution (the paper's mdt_hkce: "restore x and v to the
+ * state before the call of arxes_drift using x0 and [v0] ... <integrate close encounters on CPU>";
+ * PAPER.md:104 fn. 14: "switch to the slower Bulirsch-Stoer integration scheme to advance the
+ * interaction and Keplerian Hamiltonians of the bodies involved in the close encounter").
+ * The paper keeps this on the host and prints no algorithm; readings X-1..X-5:
+ *   X-1 the bodies involved = every endpoint of the encounter pair list, integrated as ONE system
+ *       with a shared step control (one mdt_hkce call per step), from the snapshot x0, v0 over h;
+ *       all other bodies keep their Kepler-drift result
+ *   X-2 equations of motion: dx/dt = v, dv/dt = -mu x/|x|^3 + sum over the LISTED pairs (i,j) that
+ *       contain the body of gm_other (1 - K(r; rc)) (x_other - x_i)/r^3 - the complement of the
+ *       K-weighted kick (A-1..A-5), so kick + encounter solve see the full Newtonian pair force
+ *   X-3 integrator: Gragg's modified midpoint with n_k = 2, 4, .., 16 substeps, polynomial
+ *       (Aitken-Neville) extrapolation in (H/n)^2; error of column k = max over components of
+ *       |T_kk - T_k,k-1| / scale, scale = |x_i| (positions) and |v_i| (velocities) of that body at
+ *       the start of the BS step; accepted when <= tol
+ *   X-4 step control by column only: accepted at column k <= 3: H_next = 2 H; k <= 5: H; else H/2;
+ *       no column accepted: H/2 and retry (at most 40 halvings, else failure: bodies keep the drift
+ *       result); H never exceeds what is left of h
+ *   X-5 pairs summed in list order per body; coincident bodies contribute 0
+ * ------------------------------------------------------------------------- */
+#define BS_KMAX 8
+
+typedef struct {
+    int n;                 /* bodies in the system */
+    int np;                /* pairs */
+    const int *pi, *pj;    /* local body indices of each pair */
+    const real *gm, *rc;   /* per local body */
+    real mu;
+} enc_sys;
+
+/* f(y): y = [x(3n) | v(3n)] body-major (3 per body) */
+static void enc_rhs(const enc_sys *s, const real *y, real *f)
+{
+    const int n = s->n;
+    const real *X = y, *V = y + 3 * n;
+    real *dX = f, *dV = f + 3 * n;
+    for (int b = 0; b < n; ++b) {
+        real r2 = X[3 * b] * X[3 * b] + X[3 * b + 1] * X[3 * b + 1] + X[3 * b + 2] * X[3 * b + 2];
+        real r = R_SQRT(r2);
+        real w = -s->mu / (r2 * r);
+        for (int c = 0; c < 3; ++c) { dX[3 * b + c] = V[3 * b + c]; dV[3 * b + c] = w * X[3 * b + c]; }
+    }
+    for (int p = 0; p < s->np; ++p) {                       /* list order: fixed summation order per body */
+        const int i = s->pi[p], j = s->pj[p];
+        real d[3], s2 = 0;
+        for (int c = 0; c < 3; ++c) { d[c] = X[3 * j + c] - X[3 * i + c]; s2 += d[c] * d[c]; }
+        if (!(s2 > 0)) continue;
+        real rc = rmax(s->rc[i], s->rc[j]);
+        real K = changeover_s2(s2, rc);
+        real u = ((real)1 - K) / (s2 * R_SQRT(s2));
+        for (int c = 0; c < 3; ++c) {
+            dV[3 * i + c] += s->gm[j] * u * d[c];
+            dV[3 * j + c] -= s->gm[i] * u * d[c];
+        }
+    }
+}
+
+/* y over H with nsub modified-midpoint substeps -> out */
+static void enc_midpoint(const enc_sys *s, const real *y, real H, int nsub, real *out, real *z0, real *z1, real *f)
+{
+    const int m = 6 * s->n;
+    const real hs = H / (real)nsub;
+    enc_rhs(s, y, f);
+    for (int c = 0; c < m; ++c) { z0[c] = y[c]; z1[c] = y[c] + hs * f[c]; }
+    for (int k = 1; k < nsub; ++k) {
+        enc_rhs(s, z1, f);
+        for (int c = 0; c < m; ++c) {
+            real t = z0[c] + (real)2 * hs * f[c];
+            z0[c] = z1[c]; z1[c] = t;
+        }
+    }
+    enc_rhs(s, z1, f);
+    for (int c = 0; c < m; ++c) out[c] = (real)0.5L * (z0[c] + z1[c] + hs * f[c]);
+}
+
+/* pairs: npairs x 2 (i, j) body indices as mo_encounters lists them.  x, v: the drifted state, in/out.
+ * stats (nullable, 4 ints): bodies in the system, BS steps accepted, force evaluations, 1 if failed.
+ * Returns 0, or 1 if the integration failed (x, v untouched). */
+int oracle_resolve(int nb, int ld, double mu, const double *gm, const double *rcrit, double h,
+                   const double *x0, const double *v0, double *x, double *v,
+                   const int32_t *pairs, int64_t npairs, double tol, int32_t *stats)
+{
+    if (nb < 0 || ld < nb || npairs < 0 || !(tol > 0) || h == 0) return -1;
+    if (stats) stats[0] = stats[1] = stats[2] = stats[3] = 0;
+    if (npairs == 0) return 0;
+    /* X-1: the system = sorted unique endpoints */
+    int *loc = (int *)malloc(sizeof(int) * (size_t)nb);
+    for (int b = 0; b < nb; ++b) loc[b] = -1;
+    for (int64_t p = 0; p < npairs; ++p) { loc[pairs[2 * p]] = 0; loc[pairs[2 * p + 1]] = 0; }
+    int n = 0;
+    for (int b = 0; b < nb; ++b) if (loc[b] == 0) loc[b] = n++;
+    int *body = (int *)malloc(sizeof(int) * (size_t)n);
+    for (int b = 0; b < nb; ++b) if (loc[b] >= 0) body[loc[b]] = b;
+    int *pi = (int *)malloc(sizeof(int) * (size_t)npairs), *pj = (int *)malloc(sizeof(int) * (size_t)npairs);
+    for (int64_t p = 0; p < npairs; ++p) { pi[p] = loc[pairs[2 * p]]; pj[p] = loc[pairs[2 * p + 1]]; }
+    const int m = 6 * n;
+    real *g = (real *)malloc(sizeof(real) * (size_t)n), *rc = (real *)malloc(sizeof(real) * (size_t)n);
+    real *y = (real *)malloc(sizeof(real) * (size_t)m * (BS_KMAX + 6));
+    real *z0 = y + m, *z1 = z0 + m, *f = z1 + m, *scale = f + m, *res = scale + m, *T = res + m;  /* T: BS_KMAX rows */
+    for (int k = 0; k < n; ++k) {
+        g[k] = (real)gm[body[k]]; rc[k] = (real)rcrit[body[k]];
+        for (int c = 0; c < 3; ++c) { y[3 * k + c] = X_(x0, c, body[k]); y[3 * n + 3 * k + c] = X_(v0, c, body[k]); }
+    }
+    enc_sys s = {n, (int)npairs, pi, pj, g, rc, (real)mu};
+    const real hh = (real)h;
+    real t = 0, H = hh;
+    int fail = 0, nacc = 0, halvings = 0;
+    long nrhs = 0;
+    while (!fail) {
+        const real rem = hh - t;
+        if (R_FABS(rem) <= (real)4 * R_EPS * R_FABS(hh)) break;
+        int last = 0;
+        if (R_FABS(H) >= R_FABS(rem)) { H = rem; last = 1; }
+        for (int k = 0; k < n; ++k) {                          /* X-3 scale: |x_i|, |v_i| at the start of the step */
+            real sx = 0, sv = 0;
+            for (int c = 0; c < 3; ++c) { sx += y[3 * k + c] * y[3 * k + c]; sv += y[3 * n + 3 * k + c] * y[3 * n + 3 * k + c]; }
+            sx = R_SQRT(sx); sv = R_SQRT(sv);
+            for (int c = 0; c < 3; ++c) { scale[3 * k + c] = sx; scale[3 * n + 3 * k + c] = sv; }
+        }
+        int acc_col = -1;
+        for (int k = 0; k < BS_KMAX; ++k) {
+            const int nsub = 2 * (k + 1);
+            enc_midpoint(&s, y, H, nsub, res, z0, z1, f);
+            nrhs += nsub + 1;
+            /* Aitken-Neville per component: T[c][j] holds row k-1 (T_{k-1,j}) and is overwritten with row k */
+            real err = 0;
+            for (int c = 0; c < m; ++c) {
+                real cur[BS_KMAX], *old = T + (size_t)c * BS_KMAX;   /* old[j] = T_{k-1, j} */
+                cur[0] = res[c];
+                for (int j = 1; j <= k; ++j) {
+                    real ratio = (real)(2 * (k + 1)) / (real)(2 * (k - j + 1));
+                    cur[j] = cur[j - 1] + (cur[j - 1] - old[j - 1]) / (ratio * ratio - (real)1);
+                }
+                if (k >= 1) {
+                    real e = R_FABS(cur[k] - cur[k - 1]);
+                    real sc = scale[c];
+                    e = sc > 0 ? e / sc : (e > 0 ? (real)1e300 : (real)0);
+                    if (e > err) err = e;
+                }
+                for (int j = 0; j <= k; ++j) old[j] = cur[j];
+            }
+            if (k >= 1 && err <= (real)tol) { acc_col = k; break; }
+        }
+        if (acc_col < 0) {                                     /* X-4: no column accepted */
+            H *= (real)0.5L;
+            if (++halvings > 40) fail = 1;
+            continue;
+        }
+        for (int c = 0; c < m; ++c) y[c] = T[(size_t)c * BS_KMAX + acc_col];
+        t = last ? hh : t + H;
+        ++nacc;
+        if (acc_col <= 3) H *= (real)2; else if (acc_col > 5) H *= (real)0.5L;
+    }
+    if (!fail) {
+        for (int k = 0; k < n; ++k)
+            for (int c = 0; c < 3; ++c) {
+                x[(size_t)c * ld + body[k]] = (double)y[3 * k + c];
+                v[(size_t)c * ld + body[k]] = (double)y[3 * n + 3 * k + c];
+            }
+    }
+    if (stats) { stats[0] = n; stats[1] = nacc; stats[2] = (int32_t)nrhs; stats[3] = fail; }
+    free(loc); free(body); free(pi); free(pj); free(g); free(rc); free(y);
+    return fail;
 }

@@ -1,0 +1,137 @@
+"""Pins for the oracle's close-encounter resolution (the paper's mdt_hkce, PAPER.md:104
+fn. 14, 126, 297-315; readings X-1..X-5) - no GPU.  Independent references: the pinned Kepler drift (no
+interaction left => pure two-body motion), scipy's DOP853 on the same equations of motion written with the
+pinned changeover function, time reversal, and the energy budget of the whole hybrid step."""
+import math
+
+import numpy as np
+import pytest
+from scipy.integrate import solve_ivp
+
+import oracle
+from paper_2601_19654_b200 import workloads as W
+
+G = W.G_AU_DAY_MSUN
+
+
+def _relv(got, ref):
+    return float((np.max(np.abs(got - ref), axis=0) / np.linalg.norm(ref, axis=0)).max())
+
+
+def _encounter_system(sep=0.01, m=1e-5, extra=3, seed=5):
+    """star + two bodies of mass m on neighbouring orbits at 1 AU, `sep` apart, + `extra` bystanders"""
+    M = 1.0
+    a = np.array([1.0, 1.0 + 0.6 * sep] + [1.7 + 0.4 * k for k in range(extra)])
+    n = len(a)
+    e = np.array([0.01, 0.012] + [0.05] * extra)
+    inc = np.array([0.001, 0.002] + [0.01] * extra)
+    Om = np.zeros(n); om = np.zeros(n)
+    Man = np.array([0.3, 0.3 + 0.8 * sep] + [1.0 + k for k in range(extra)])
+    mass = np.array([m, m] + [1e-7] * extra)
+    x, vh = W.elements_to_state(G * (M + mass), a, e, inc, Om, om, Man)
+    v = oracle.h2dh(M, mass, vh)
+    rh, rc = oracle.hill(G, M, mass, x, v, n_hill=3.0)
+    return M, mass, x, v, rc
+
+
+def test_X1_without_interaction_it_is_the_kepler_drift():
+    w = W.make_config(0)
+    mu, gm = G * w.m_star, G * w.mass
+    x1, v1, fl = oracle.drift(mu, w.dt, w.x, w.v)
+    enc = oracle.encounters(w.dt, w.x, w.v, x1, v1, w.rcrit)
+    assert enc["count"] >= 4
+    idx = np.unique(enc["pairs"])
+    # massless bodies: nothing but the star's Kepler term is left
+    r = oracle.resolve(mu, gm * 0.0, w.rcrit, w.dt, w.x, w.v, x1, v1, enc["pairs"])
+    assert r["fail"] == 0 and r["n"] == len(idx)
+    assert _relv(r["x"][:, idx], x1[:, idx]) <= 1e-12 and _relv(r["v"][:, idx], v1[:, idx]) <= 1e-12
+    # rcrit -> 0: every listed pair is outside its shell, 1 - K = 0
+    r = oracle.resolve(mu, gm, w.rcrit * 1e-9, w.dt, w.x, w.v, x1, v1, enc["pairs"])
+    assert _relv(r["x"][:, idx], x1[:, idx]) <= 1e-12 and _relv(r["v"][:, idx], v1[:, idx]) <= 1e-12
+    # bodies outside the list keep the drift result bit for bit; empty list: nothing changes
+    r = oracle.resolve(mu, gm, w.rcrit, w.dt, w.x, w.v, x1, v1, enc["pairs"])
+    rest = np.setdiff1d(np.arange(w.nb), idx)
+    assert np.array_equal(r["x"][:, rest], x1[:, rest]) and np.array_equal(r["v"][:, rest], v1[:, rest])
+    assert not np.array_equal(r["x"][:, idx], x1[:, idx])
+    r = oracle.resolve(mu, gm, w.rcrit, w.dt, w.x, w.v, x1, v1, np.zeros((0, 2), dtype=np.int32))
+    assert np.array_equal(r["x"], x1) and r["n"] == 0
+
+
+@pytest.mark.parametrize("sep,h", [(0.01, 2.0), (0.003, 1.0), (0.02, -3.0), (0.0009, 0.5)])
+def test_X2_against_dop853_on_the_same_equations(sep, h):
+    """sep = 0.01, 0.02: inside the changeover shell (0 < K < 1); 0.003, 0.0009: partly / wholly inside 0.1 rc"""
+    M, mass, x, v, rc = _encounter_system(sep)
+    mu, gm = G * M, G * mass
+    pairs = np.array([[0, 1], [0, 3], [1, 4]], dtype=np.int32)       # the close pair + two distant listed pairs
+    idx = np.unique(pairs)
+    loc = {b: k for k, b in enumerate(idx)}
+    n = len(idx)
+
+    def rhs(t, y):
+        X = y[:3 * n].reshape(n, 3); V = y[3 * n:].reshape(n, 3)
+        A = -mu * X / np.linalg.norm(X, axis=1)[:, None] ** 3
+        for i, j in pairs:
+            d = X[loc[j]] - X[loc[i]]
+            r = np.linalg.norm(d)
+            u = (1.0 - oracle.changeover(r, max(rc[i], rc[j]))) / r**3
+            A[loc[i]] += gm[j] * u * d
+            A[loc[j]] -= gm[i] * u * d
+        return np.concatenate([V.ravel(), A.ravel()])
+
+    y0 = np.concatenate([x[:, idx].T.ravel(), v[:, idx].T.ravel()])
+    sol = solve_ivp(rhs, (0.0, h), y0, method="DOP853", rtol=1e-13, atol=1e-18)
+    assert sol.success
+    xr = sol.y[:3 * n, -1].reshape(n, 3).T; vr = sol.y[3 * n:, -1].reshape(n, 3).T
+    x1, v1, _ = oracle.drift(mu, h, x, v)
+    r = oracle.resolve(mu, gm, rc, h, x, v, x1, v1, pairs, tol=1e-13)
+    assert r["fail"] == 0 and r["n"] == n
+    assert _relv(r["x"][:, idx], xr) <= 2e-11 and _relv(r["v"][:, idx], vr) <= 2e-11
+    # and the encounter matters: the close pair does not follow its Kepler drift
+    assert _relv(r["v"][:, :2], v1[:, :2]) > 1e-7
+
+
+def test_X3_time_reversal_and_pair_order():
+    M, mass, x, v, rc = _encounter_system(0.008)
+    mu, gm = G * M, G * mass
+    pairs = np.array([[0, 1], [1, 2]], dtype=np.int32)
+    x1, v1, _ = oracle.drift(mu, 2.0, x, v)
+    f = oracle.resolve(mu, gm, rc, 2.0, x, v, x1, v1, pairs)
+    b = oracle.resolve(mu, gm, rc, -2.0, f["x"], f["v"], f["x"], f["v"], pairs)
+    idx = np.unique(pairs)
+    assert _relv(b["x"][:, idx], x[:, idx]) <= 1e-11 and _relv(b["v"][:, idx], v[:, idx]) <= 1e-11
+    g = oracle.resolve(mu, gm, rc, 2.0, x, v, x1, v1, pairs[::-1].copy())
+    assert _relv(g["x"][:, idx], f["x"][:, idx]) <= 1e-15
+
+
+def _hybrid_steps(M, mass, x, v, rc, dt, nsteps, resolve):
+    """the hybrid step composed from the oracle's pinned parts (S-1), with or without X-1..X-5"""
+    mu, gm = G * M, G * mass
+    a, _ = oracle.accel(gm, x, rc)
+    nres = 0
+    for _ in range(nsteps):
+        v = oracle.kick(0.5 * dt, v, a)
+        x, _ = oracle.jump(0.5 * dt, mu, gm, x, v)
+        x0, v0 = x.copy(), v.copy()
+        x, v, _ = oracle.drift(mu, dt, x, v)
+        enc = oracle.encounters(dt, x0, v0, x, v, rc)
+        if resolve and enc["count"] > 0:
+            r = oracle.resolve(mu, gm, rc, dt, x0, v0, x, v, enc["pairs"])
+            assert r["fail"] == 0
+            x, v = r["x"], r["v"]
+            nres += 1
+        x, _ = oracle.jump(0.5 * dt, mu, gm, x, v)
+        a, _ = oracle.accel(gm, x, rc)
+        v = oracle.kick(0.5 * dt, v, a)
+    return x, v, nres
+
+
+def test_X4_the_resolved_hybrid_step_keeps_the_energy_through_a_close_encounter():
+    """inside the shell the kick carries only K of the pair force; the encounter solve must supply the rest"""
+    M, mass, x, v, rc = _encounter_system(sep=0.004, m=3e-5, extra=2)
+    E0 = oracle.energy(G, M, mass, x, v)["E"]
+    xa, va, nres = _hybrid_steps(M, mass, x, v, rc, 1.0, 30, resolve=True)
+    xb, vb, _ = _hybrid_steps(M, mass, x, v, rc, 1.0, 30, resolve=False)
+    ea = abs(oracle.energy(G, M, mass, xa, va)["E"] - E0) / abs(E0)
+    eb = abs(oracle.energy(G, M, mass, xb, vb)["E"] - E0) / abs(E0)
+    assert nres >= 20
+    assert ea < 1e-7 and eb > 100 * ea, (ea, eb)

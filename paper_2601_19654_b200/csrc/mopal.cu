@@ -15,6 +15,7 @@
 #include "pair_sym.cuh"
 #include "support.cuh"
 #include "step_small.cuh"
+#include "resolve.cuh"
 
 using namespace mopal;
 
@@ -44,6 +45,11 @@ struct mo_ctx {
     double *en_on = nullptr, *en_pair = nullptr, *en_out = nullptr;   // energy partials / result (lazy)
     double* en_host = nullptr;          // pinned, 7 doubles
     int en_npair = 0, en_split = 1;
+    double res_tol = 0.0;               // mo_set_resolve: <= 0 off
+    int* res_loc = nullptr;             // nb ints (lazy)
+    double* res_tab = nullptr;          // extrapolation tableaux
+    ResStats* res_out = nullptr;        // device
+    ResStats* res_host = nullptr;       // pinned
     int hill_mode = -1;                 // mo_set_hill: -1 off
     double hill_n = 3.0;
     unsigned char* tiles = nullptr;
@@ -237,6 +243,8 @@ extern "C" void mo_destroy(mo_ctx* ctx) {
     for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
     cudaFree(ctx->gm); cudaFree(ctx->x0); cudaFree(ctx->v0); cudaFree(ctx->part);
     cudaFree(ctx->psumA); cudaFree(ctx->psumB); cudaFree(ctx->ticket);
+    cudaFree(ctx->res_loc); cudaFree(ctx->res_out); cudaFree(ctx->res_tab);
+    if (ctx->res_host) cudaFreeHost(ctx->res_host);
     cudaFree(ctx->gmsum); cudaFree(ctx->en_on); cudaFree(ctx->en_pair); cudaFree(ctx->en_out);
     if (ctx->en_host) cudaFreeHost(ctx->en_host); cudaFree(ctx->tiles);
     cudaFree(ctx->sym_units); cudaFree(ctx->sym_ustart); cudaFree(ctx->sym_partI); cudaFree(ctx->sym_partJ);
@@ -513,8 +521,29 @@ static mo_status enqueue_hill(mo_ctx* ctx, double n_hill, int mode, double* rhil
     return post_launch(ctx);
 }
 
+static mo_status ensure_resolve_scratch(mo_ctx* ctx) {
+    if (ctx->res_loc) return MO_OK;
+    cudaError_t e = dalloc(ctx, &ctx->res_loc, (size_t)ctx->nb);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_out, 1);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_tab, (size_t)6 * RES_KMAX * RES_NMAX);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(resolve_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, RES_DYN_SMEM);
+    if (e == cudaSuccess) e = cudaMemsetAsync(ctx->res_out, 0, sizeof(ResStats), ctx->stream);
+    if (e == cudaSuccess) e = cudaMallocHost(reinterpret_cast<void**>(&ctx->res_host), sizeof(ResStats));
+    if (e != cudaSuccess) { cudaGetLastError(); ctx->last_err = e; return e == cudaErrorMemoryAllocation ? MO_ENOMEM : MO_ECUDA; }
+    return MO_OK;
+}
+
+static mo_status enqueue_resolve(mo_ctx* ctx, double dt, double tol) {
+    ResParams rp;
+    rp.x0 = ctx->x0; rp.v0 = ctx->v0; rp.x = ctx->x; rp.v = ctx->v; rp.gm = ctx->gm; rp.rcrit = ctx->rcrit;
+    rp.pairs = ctx->pairs; rp.flag = ctx->flag; rp.st = ctx->dstats; rp.loc = ctx->res_loc; rp.tab = ctx->res_tab; rp.out = ctx->res_out;
+    rp.cap = ctx->cap; rp.nb = ctx->nb; rp.ld = ctx->ld; rp.mu = ctx->mu; rp.h = dt; rp.tol = tol;
+    resolve_kernel<<<1, RES_NMAX, RES_DYN_SMEM, ctx->stream>>>(rp);
+    return post_launch(ctx);
+}
+
 static mo_status enqueue_step(mo_ctx* ctx, double dt) {
-    if (ctx->use_small) {
+    if (ctx->use_small && ctx->res_tol <= 0.0) {
         SmallParams q;
         MidParams& mp = q.m;
         mp.x = ctx->x; mp.v = ctx->v; mp.x0 = ctx->x0; mp.v0 = ctx->v0; mp.gm = ctx->gm; mp.rcrit = ctx->rcrit;
@@ -541,14 +570,15 @@ static mo_status enqueue_step(mo_ctx* ctx, double dt) {
     MidParams mp;
     mp.x = ctx->x; mp.v = ctx->v; mp.x0 = ctx->x0; mp.v0 = ctx->v0; mp.gm = ctx->gm; mp.rcrit = ctx->rcrit;
     mp.psum_in = ctx->psumA; mp.psum_out = ctx->psumB; mp.ticket = ctx->ticket + 1;
-    mp.x1 = ctx->overlap ? ctx->x1 : nullptr; mp.v1 = ctx->overlap ? ctx->v1 : nullptr; mp.enc = ctx->enc; mp.flag = ctx->flag;
+    const bool ovl = ctx->overlap && ctx->res_tol <= 0.0;   // the encounter solve needs the list before the jump
+    mp.x1 = ovl ? ctx->x1 : nullptr; mp.v1 = ovl ? ctx->v1 : nullptr; mp.enc = ctx->enc; mp.flag = ctx->flag;
     mp.st = ctx->dstats; mp.nb = ctx->nb; mp.ld = ctx->ld; mp.nbPad = ctx->nbPad; mp.npsum = ctx->npsum;
     mp.nbig = ctx->nbig;
     mp.hj_over_mu = 0.5 * dt / ctx->mu; mp.mu = ctx->mu; mp.h = dt;
     jump_drift_boxes_kernel<<<ctx->npsum, ON_BLOCK, 0, ctx->stream>>>(mp);
     s = post_launch(ctx);
     if (s != MO_OK) return s;
-    if (ctx->overlap) {
+    if (ovl) {
         // fork: encounter pass on enc_stream (reads x0, v0, x1, v1, boxes, rcrit; writes pairs, flag, stats),
         // jump + pair sum + closing kick on the main stream (moves x, v; writes a); join at the end
         cudaStream_t mainS = ctx->stream;
@@ -568,6 +598,14 @@ static mo_status enqueue_step(mo_ctx* ctx, double dt) {
     }
     s = enqueue_pairs(ctx, enc_state(ctx, ctx->x0, ctx->v0, dt), 1);
     if (s != MO_OK) return s;
+    if (ctx->res_tol > 0.0) {
+        s = enqueue_resolve(ctx, dt, ctx->res_tol);
+        if (s != MO_OK) return s;
+        // v of the resolved bodies changed: sum gm v for the second jump again
+        kick_psum_kernel<false><<<ctx->npsum, ON_BLOCK, 0, ctx->stream>>>(ctx->v, nullptr, ctx->gm, ctx->nb, ctx->ld, 0.0, ctx->psumB, ctx->ticket + 1);
+        s = post_launch(ctx);
+        if (s != MO_OK) return s;
+    }
     return enqueue_accel(ctx, true, 0.5 * dt, true, 0.5 * dt);
 }
 
@@ -651,6 +689,36 @@ extern "C" mo_status mo_set_nbig(mo_ctx* ctx, int32_t nbig) {
     ctx->nbig = nbig;
     ctx->nSrcTiles = (nbig + TJ - 1) / TJ;
     choose_geometry(ctx);
+    return MO_OK;
+}
+
+extern "C" mo_status mo_resolve(mo_ctx* ctx, double dt, double tol) {
+    if (!ctx || !isfinite(dt) || dt == 0.0 || !(tol > 0.0) || !ctx->snap_valid) return MO_EINVAL;
+    mo_status s = ensure_resolve_scratch(ctx);
+    if (s != MO_OK) return s;
+    return enqueue_resolve(ctx, dt, tol);
+}
+
+extern "C" mo_status mo_set_resolve(mo_ctx* ctx, double tol) {
+    if (!ctx || !isfinite(tol)) return MO_EINVAL;
+    if (tol > 0.0) {
+        mo_status s = ensure_resolve_scratch(ctx);
+        if (s != MO_OK) return s;
+    }
+    if (ctx->gexec) {
+        CK(cudaStreamSynchronize(ctx->stream));
+        cudaGraphExecDestroy(ctx->gexec); ctx->gexec = nullptr;
+    }
+    ctx->res_tol = tol > 0.0 ? tol : 0.0;
+    return MO_OK;
+}
+
+extern "C" mo_status mo_resolve_stats(mo_ctx* ctx, int32_t* out4) {
+    if (!ctx || !out4) return MO_EINVAL;
+    if (!ctx->res_out) { out4[0] = out4[1] = out4[2] = out4[3] = 0; return MO_OK; }
+    CK(cudaMemcpyAsync(ctx->res_host, ctx->res_out, sizeof(ResStats), cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+    out4[0] = ctx->res_host->bodies; out4[1] = ctx->res_host->steps; out4[2] = ctx->res_host->rhs; out4[3] = ctx->res_host->fail;
     return MO_OK;
 }
 

@@ -21,7 +21,8 @@ EXPORTS = ["mo_create", "mo_accel", "mo_drift", "mo_encounters", "mo_step", "mo_
            "mo_snapshot", "mo_snapshot_ptrs", "mo_snapshot_copy", "mo_invalidate_accel", "mo_get_stats", "mo_launch_count",
            "mo_workspace_bytes", "mo_step_host", "mo_accel_host", "mo_probe_fp64_peak",
            "mo_pair_geometry", "mo_set_kernel_timing", "mo_pair_kernel_ms", "mo_strerror", "mo_version",
-           "mo_set_nbig", "mo_pair_kernel_name", "mo_h2dh", "mo_dh2h", "mo_hill", "mo_set_hill", "mo_energy"]
+           "mo_set_nbig", "mo_pair_kernel_name", "mo_h2dh", "mo_dh2h", "mo_hill", "mo_set_hill", "mo_energy",
+           "mo_resolve", "mo_set_resolve", "mo_resolve_stats"]
 
 
 class MoStats(C.Structure):
@@ -71,6 +72,9 @@ def load():
     L.mo_hill.restype = C.c_int; L.mo_hill.argtypes = [vp, C.c_double, I32, vp]
     L.mo_set_hill.restype = C.c_int; L.mo_set_hill.argtypes = [vp, C.c_double, I32]
     L.mo_energy.restype = C.c_int; L.mo_energy.argtypes = [vp, C.POINTER(MoEnergy)]
+    L.mo_resolve.restype = C.c_int; L.mo_resolve.argtypes = [vp, C.c_double, C.c_double]
+    L.mo_set_resolve.restype = C.c_int; L.mo_set_resolve.argtypes = [vp, C.c_double]
+    L.mo_resolve_stats.restype = C.c_int; L.mo_resolve_stats.argtypes = [vp, C.POINTER(I32)]
     L.mo_get_stats.restype = C.c_int; L.mo_get_stats.argtypes = [vp, C.POINTER(MoStats)]
     L.mo_launch_count.restype = I64; L.mo_launch_count.argtypes = [vp]
     L.mo_workspace_bytes.restype = I64; L.mo_workspace_bytes.argtypes = [vp]
@@ -247,6 +251,20 @@ class Mopal:
         e = MoEnergy()
         self._check(self._L.mo_energy(self._ctx, C.byref(e)), "mo_energy")
         return dict(T=e.T, Us=e.Us, Up=e.Up, E=e.E, L=np.array(list(e.L)))
+
+    # ---- close-encounter resolution (the paper's mdt_hkce) ----
+    def resolve(self, dt, tol=1e-12):
+        """Bulirsch-Stoer integration of the bodies of the current pair list from the snapshot over dt."""
+        self._check(self._L.mo_resolve(self._ctx, float(dt), float(tol)), "mo_resolve")
+
+    def set_resolve(self, tol=1e-12):
+        """mo_step resolves the encounters of every step (tol <= 0: off)."""
+        self._check(self._L.mo_set_resolve(self._ctx, float(tol)), "mo_set_resolve")
+
+    def resolve_stats(self):
+        out = (C.c_int32 * 4)()
+        self._check(self._L.mo_resolve_stats(self._ctx, out), "mo_resolve_stats")
+        return dict(bodies=out[0], steps=out[1], rhs=out[2], fail=out[3])
 
     def invalidate_accel(self):
         self._check(self._L.mo_invalidate_accel(self._ctx), "mo_invalidate_accel")

@@ -772,3 +772,104 @@ def test_step_small_path_overflow_and_large_path_agree(M, monkeypatch):
     assert _rel_vec_err(m1.get("x"), m2.get("x")).max() <= 1e-14 and _rel_vec_err(m1.get("v"), m2.get("v")).max() <= 1e-14
     assert s1.nce_last == s2.nce_last and np.array_equal(m1.pair_list(s1.nce_last), m2.pair_list(s2.nce_last))
     m1.close(); m2.close()
+
+
+# ------------------------------------------------------------------------------ encounter resolution
+def _close_pair_system(sep, m=1e-5, extra=600, seed=3):
+    """two massive bodies `sep` apart on neighbouring orbits at 1 AU inside a small disk (cfg1 recipe, shrunk)"""
+    w = W.shrink(1, extra + 3, seed=seed)
+    a = np.array([1.0, 1.0 + 0.6 * sep]); e = np.array([0.01, 0.012]); inc = np.array([0.001, 0.002])
+    z = np.zeros(2); Man = np.array([0.3, 0.3 + 0.8 * sep])
+    mass = w.mass.copy(); mass[2:4] = m
+    x2, vh2 = W.elements_to_state(G * (w.m_star + m), a, e, inc, z, z, Man)
+    x = w.x.copy(); x[:, 2:4] = x2
+    vh = oracle.dh2h(w.m_star, w.mass, w.v); vh[:, 2:4] = vh2
+    v = oracle.h2dh(w.m_star, mass, vh)
+    _, rc = oracle.hill(G, w.m_star, mass, x, v, n_hill=3.0)
+    return w, mass, x, v, rc
+
+
+@pytest.mark.parametrize("sep,dt,tol", [(0.01, 2.0, 1e-12), (0.003, 1.0, 1e-13), (0.02, -3.0, 1e-12)])
+def test_resolve_vs_oracle(M, sep, dt, tol):
+    w, mass, x, v, rc = _close_pair_system(sep)
+    mu, gm = G * w.m_star, G * mass
+    x1, v1, _ = oracle.drift(mu, dt, x, v)
+    enc = oracle.encounters(dt, x, v, x1, v1, rc)
+    assert enc["count"] >= 3 and [2, 3] in enc["pairs"].tolist()
+    ref = oracle.resolve(mu, gm, rc, dt, x, v, x1, v1, enc["pairs"], tol=tol)
+    m = M.Mopal(mass, x, v, rc, m_star=w.m_star, G=w.G)
+    m.snapshot(); m.set("x", x1); m.set("v", v1)
+    cnt = m.encounters(dt)
+    assert np.array_equal(m.pair_list(cnt), enc["pairs"])
+    m.resolve(dt, tol)
+    st = m.resolve_stats()
+    assert st["fail"] == 0 and st["bodies"] == ref["n"] and st["steps"] == ref["nsteps"] and st["rhs"] == ref["nrhs"]
+    idx = np.unique(enc["pairs"]); rest = np.setdiff1d(np.arange(w.nb), idx)
+    gx, gv = m.get("x"), m.get("v")
+    assert _rel_vec_err(gx[:, idx], ref["x"][:, idx]).max() <= 1e-12 and _rel_vec_err(gv[:, idx], ref["v"][:, idx]).max() <= 1e-12
+    assert np.array_equal(gx[:, rest], x1[:, rest]) and np.array_equal(gv[:, rest], v1[:, rest])
+    assert _rel_vec_err(gv[:, 2:4], v1[:, 2:4]).max() > 1e-8          # the encounter matters
+    m.close()
+
+
+@pytest.mark.parametrize("cfg,N", [(0, 256), (1, 1500), (3, 3000)])
+def test_resolve_inside_step_vs_oracle(M, cfg, N):
+    """mo_set_resolve: kick, jump, snapshot, drift, encounter check, encounter solve, jump, accel, kick"""
+    w = W.make_config(cfg) if N == 256 else W.shrink(cfg, N)
+    mu, gm = G * w.m_star, G * w.mass
+    m = _mk(M, w)
+    m.set_resolve(1e-12)
+    a, _ = oracle.accel(gm, w.x, w.rcrit)
+    x, v = w.x, w.v
+    nres = 0
+    for k in range(3):
+        st = m.step(w.dt, 1)
+        v = oracle.kick(0.5 * w.dt, v, a)
+        x, _ = oracle.jump(0.5 * w.dt, mu, gm, x, v)
+        x0, v0 = x.copy(), v.copy()
+        x, v, _ = oracle.drift(mu, w.dt, x, v)
+        enc = oracle.encounters(w.dt, x0, v0, x, v, w.rcrit)
+        if enc["count"] > 0:
+            r = oracle.resolve(mu, gm, w.rcrit, w.dt, x0, v0, x, v, enc["pairs"])
+            assert r["fail"] == 0
+            x, v = r["x"], r["v"]
+            rs = m.resolve_stats()
+            assert rs["fail"] == 0 and rs["bodies"] == r["n"] and rs["steps"] == r["nsteps"]
+            nres += 1
+        x, _ = oracle.jump(0.5 * w.dt, mu, gm, x, v)
+        a, _ = oracle.accel(gm, x, w.rcrit)
+        v = oracle.kick(0.5 * w.dt, v, a)
+        tol = 2e-13 * (1 + k)
+        assert _rel_vec_err(m.get("x"), x).max() <= tol and _rel_vec_err(m.get("v"), v).max() <= tol, k
+        assert st.nce_last == enc["count"]
+    assert nres == 3
+    m2 = _mk(M, w); m2.set_resolve(1e-12); m2.step(w.dt, 3)           # graph replay
+    assert np.array_equal(m.get("x"), m2.get("x")) and np.array_equal(m.get("v"), m2.get("v"))
+    m.close(); m2.close()
+
+
+def test_resolve_energy_and_limits(M):
+    """through a close encounter the resolved step keeps the energy (mo_energy) orders of magnitude better"""
+    w, mass, x, v, rc = _close_pair_system(0.004, m=3e-5, extra=300)
+    out = []
+    for tol in (1e-12, 0.0):
+        m = M.Mopal(mass, x, v, rc, m_star=w.m_star, G=w.G)
+        m.set_resolve(tol)
+        e0 = m.energy()["E"]
+        m.step(1.0, 30)
+        out.append(abs(m.energy()["E"] - e0) / abs(e0))
+        m.close()
+    assert out[0] < 1e-7 and out[1] > 50 * out[0], out
+    # list larger than this version handles: reported, bodies keep the drift result
+    w = W.shrink(4, 600)
+    huge = np.full(w.nb, 1e3)
+    m = M.Mopal(w.mass, w.x, w.v, huge, cap=1 << 20)
+    x1, v1 = _enc_inputs(w)
+    m.snapshot(); m.set("x", x1); m.set("v", v1)
+    assert m.encounters(w.dt) > 2048
+    m.resolve(w.dt, 1e-12)
+    assert m.resolve_stats()["fail"] == 2 and np.array_equal(m.get("x"), x1)
+    L = M.load()
+    assert L.mo_resolve(m._ctx, 0.0, 1e-12) == M.MO_EINVAL and L.mo_resolve(m._ctx, 1.0, 0.0) == M.MO_EINVAL
+    assert L.mo_resolve_stats(m._ctx, None) == M.MO_EINVAL and L.mo_set_resolve(None, 1.0) == M.MO_EINVAL
+    m.close()

@@ -804,8 +804,11 @@ int oracle_energy(int nb, int nbig, int ld, double G, double mstar, const double
  * PAPER.md:104 fn. 14: "switch to the slower Bulirsch-Stoer integration scheme to advance the
  * interaction and Keplerian Hamiltonians of the bodies involved in the close encounter").
  * The paper keeps this on the host and prints no algorithm; readings X-1..X-5:
- *   X-1 the bodies involved = every endpoint of the encounter pair list, integrated as ONE system
- *       with a shared step control (one mdt_hkce call per step), from the snapshot x0, v0 over h;
+ *   X-1 the bodies involved = every endpoint of the encounter pair list.  The connected components of
+ *       the pair graph share no listed pair, so their equations of motion (X-2) are decoupled: each
+ *       component is integrated as its own system, with its own step control, from the snapshot x0, v0
+ *       over h (the parent code makes one mdt_hkce call for all of them; the solutions agree to the
+ *       tolerance, and a tight pair no longer forces its small steps on a giant's hundred neighbours);
  *       all other bodies keep their Kepler-drift result
  *   X-2 equations of motion: dx/dt = v, dv/dt = -mu x/|x|^3 + sum over the LISTED pairs (i,j) that
  *       contain the body of gm_other (1 - K(r; rc)) (x_other - x_i)/r^3 - the complement of the
@@ -874,10 +877,10 @@ static void enc_midpoint(const enc_sys *s, const real *y, real H, int nsub, real
     for (int c = 0; c < m; ++c) out[c] = (real)0.5L * (z0[c] + z1[c] + hs * f[c]);
 }
 
-/* pairs: npairs x 2 (i, j) body indices as mo_encounters lists them.  x, v: the drifted state, in/out.
+/* One system (X-1: one connected component of the pair graph): its bodies are the endpoints of `pairs`.
  * stats (nullable, 4 ints): bodies in the system, BS steps accepted, force evaluations, 1 if failed.
- * Returns 0, or 1 if the integration failed (x, v untouched). */
-int oracle_resolve(int nb, int ld, double mu, const double *gm, const double *rcrit, double h,
+ * Returns 0, or 1 if the integration failed (x, v of its bodies untouched). */
+static int resolve_system(int nb, int ld, double mu, const double *gm, const double *rcrit, double h,
                    const double *x0, const double *v0, double *x, double *v,
                    const int32_t *pairs, int64_t npairs, double tol, int32_t *stats)
 {
@@ -962,4 +965,44 @@ int oracle_resolve(int nb, int ld, double mu, const double *gm, const double *rc
     if (stats) { stats[0] = n; stats[1] = nacc; stats[2] = (int32_t)nrhs; stats[3] = fail; }
     free(loc); free(body); free(pi); free(pj); free(g); free(rc); free(y);
     return fail;
+}
+
+/* pairs: npairs x 2 (i, j) body indices as mo_encounters lists them.  x, v: the drifted state, in/out.
+ * X-1: union-find over the pairs; components taken in ascending order of their smallest body, each
+ * with its pairs in list order.  stats (nullable, 4 ints): bodies in all systems, BS steps accepted
+ * (summed over the components), force evaluations (summed), number of failed components.
+ * Returns 0, or 1 if a component failed (its bodies keep the drift result). */
+static int uf_find(int *par, int a) { while (par[a] != a) { par[a] = par[par[a]]; a = par[a]; } return a; }
+
+int oracle_resolve(int nb, int ld, double mu, const double *gm, const double *rcrit, double h,
+                   const double *x0, const double *v0, double *x, double *v,
+                   const int32_t *pairs, int64_t npairs, double tol, int32_t *stats)
+{
+    if (nb < 0 || ld < nb || npairs < 0 || !(tol > 0) || h == 0) return -1;
+    if (stats) stats[0] = stats[1] = stats[2] = stats[3] = 0;
+    if (npairs == 0) return 0;
+    int *par = (int *)malloc(sizeof(int) * (size_t)nb);
+    for (int b = 0; b < nb; ++b) par[b] = b;
+    for (int64_t p = 0; p < npairs; ++p) {
+        int a = uf_find(par, pairs[2 * p]), b = uf_find(par, pairs[2 * p + 1]);
+        if (a != b) { if (a < b) par[b] = a; else par[a] = b; }      /* root = smallest body of the component */
+    }
+    int32_t *sub = (int32_t *)malloc(sizeof(int32_t) * 2 * (size_t)npairs);
+    char *done = (char *)calloc((size_t)npairs, 1);
+    int anyfail = 0;
+    for (int64_t p0 = 0; p0 < npairs; ++p0) {                        /* list sorted by (i, j): roots come up in ascending order */
+        if (done[p0]) continue;
+        const int root = uf_find(par, pairs[2 * p0]);
+        int64_t ns = 0;
+        for (int64_t p = p0; p < npairs; ++p)
+            if (!done[p] && uf_find(par, pairs[2 * p]) == root) {
+                sub[2 * ns] = pairs[2 * p]; sub[2 * ns + 1] = pairs[2 * p + 1]; ++ns; done[p] = 1;
+            }
+        int32_t st[4] = {0, 0, 0, 0};
+        int f = resolve_system(nb, ld, mu, gm, rcrit, h, x0, v0, x, v, sub, ns, tol, st);
+        if (stats) { stats[0] += st[0]; stats[1] += st[1]; stats[2] += st[2]; stats[3] += st[3]; }
+        anyfail |= (f != 0);
+    }
+    free(par); free(sub); free(done);
+    return anyfail;
 }

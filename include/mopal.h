@@ -163,15 +163,16 @@ mo_status mo_energy(mo_ctx *ctx, mo_energy_t *out_host);
  * snapshot x0, v0 and integrated over dt as one system with a Bulirsch-Stoer scheme to relative
  * tolerance tol, under the star's Kepler term and the (1 - K)-weighted forces of the listed pairs - the
  * complement of the K-weighted kick; x, v of those bodies (which must hold the Kepler-drift result of the
- * other bodies) are overwritten.  Limits of this version: 1024 bodies and 2048 pairs in the list; beyond,
- * or without convergence, the bodies keep the drift result and the failure is reported by
- * mo_resolve_stats.  Asynchronous.  MO_EINVAL: tol <= 0, dt == 0, no snapshot. */
+ * other bodies) are overwritten.  Each connected component of the pair graph is its own system with its
+ * own step control.  Limits of this version: 1024 bodies and 2048 pairs per component; beyond, or without
+ * convergence, the component's bodies keep the drift result and it is counted in mo_resolve_stats.
+ * Asynchronous.  MO_EINVAL: tol <= 0, dt == 0, no snapshot. */
 mo_status mo_resolve(mo_ctx *ctx, double dt, double tol);
 /* Make mo_step resolve the encounters of every step (between the encounter check and the second jump,
  * PAPER.md:297-315); tol <= 0 switches it off (the default).  Drops the cached step graph. */
 mo_status mo_set_resolve(mo_ctx *ctx, double tol);
-/* Last resolution: out4 = {bodies in the system, accepted BS steps, right-hand-side evaluations,
- * failure (0 ok, 1 no convergence, 2 list too large)}.  Synchronises. */
+/* Last resolution: out4 = {bodies in all components, accepted BS steps and right-hand-side evaluations
+ * summed over the components, components not resolved}.  Synchronises. */
 mo_status mo_resolve_stats(mo_ctx *ctx, int32_t *out4);
 
 /* Copy the current x, v into the context's x0, v0 snapshot (asynchronous). */

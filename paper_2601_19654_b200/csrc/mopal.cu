@@ -47,7 +47,9 @@ struct mo_ctx {
     int en_npair = 0, en_split = 1;
     double res_tol = 0.0;               // mo_set_resolve: <= 0 off
     int* res_loc = nullptr;             // nb ints (lazy)
-    double* res_tab = nullptr;          // extrapolation tableaux
+    double* res_tab = nullptr;          // extrapolation tableaux, one set per CTA
+    int *res_label = nullptr, *res_roots = nullptr, *res_nroots = nullptr;
+    int res_grid = 1;
     ResStats* res_out = nullptr;        // device
     ResStats* res_host = nullptr;       // pinned
     int hill_mode = -1;                 // mo_set_hill: -1 off
@@ -243,7 +245,7 @@ extern "C" void mo_destroy(mo_ctx* ctx) {
     for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
     cudaFree(ctx->gm); cudaFree(ctx->x0); cudaFree(ctx->v0); cudaFree(ctx->part);
     cudaFree(ctx->psumA); cudaFree(ctx->psumB); cudaFree(ctx->ticket);
-    cudaFree(ctx->res_loc); cudaFree(ctx->res_out); cudaFree(ctx->res_tab);
+    cudaFree(ctx->res_loc); cudaFree(ctx->res_out); cudaFree(ctx->res_tab); cudaFree(ctx->res_label); cudaFree(ctx->res_roots); cudaFree(ctx->res_nroots);
     if (ctx->res_host) cudaFreeHost(ctx->res_host);
     cudaFree(ctx->gmsum); cudaFree(ctx->en_on); cudaFree(ctx->en_pair); cudaFree(ctx->en_out);
     if (ctx->en_host) cudaFreeHost(ctx->en_host); cudaFree(ctx->tiles);
@@ -525,8 +527,14 @@ static mo_status ensure_resolve_scratch(mo_ctx* ctx) {
     if (ctx->res_loc) return MO_OK;
     cudaError_t e = dalloc(ctx, &ctx->res_loc, (size_t)ctx->nb);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_out, 1);
-    if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_tab, (size_t)6 * RES_KMAX * RES_NMAX);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(resolve_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, RES_DYN_SMEM);
+    ctx->res_grid = ctx->nsm;
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_tab, (size_t)6 * RES_KMAX * RES_NMAX * ctx->res_grid);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_label, (size_t)ctx->nb);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_roots, (size_t)(ctx->cap > 0 ? ctx->cap : 1));
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_nroots, 1);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(resolve_kernel<64, 0, 32>, cudaFuncAttributeMaxDynamicSharedMemorySize, RES_DYN_SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(resolve_kernel<256, 32, 128>, cudaFuncAttributeMaxDynamicSharedMemorySize, RES_DYN_SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(resolve_kernel<RES_NMAX, 128, 1 << 30>, cudaFuncAttributeMaxDynamicSharedMemorySize, RES_DYN_SMEM);
     if (e == cudaSuccess) e = cudaMemsetAsync(ctx->res_out, 0, sizeof(ResStats), ctx->stream);
     if (e == cudaSuccess) e = cudaMallocHost(reinterpret_cast<void**>(&ctx->res_host), sizeof(ResStats));
     if (e != cudaSuccess) { cudaGetLastError(); ctx->last_err = e; return e == cudaErrorMemoryAllocation ? MO_ENOMEM : MO_ECUDA; }
@@ -536,9 +544,18 @@ static mo_status ensure_resolve_scratch(mo_ctx* ctx) {
 static mo_status enqueue_resolve(mo_ctx* ctx, double dt, double tol) {
     ResParams rp;
     rp.x0 = ctx->x0; rp.v0 = ctx->v0; rp.x = ctx->x; rp.v = ctx->v; rp.gm = ctx->gm; rp.rcrit = ctx->rcrit;
-    rp.pairs = ctx->pairs; rp.flag = ctx->flag; rp.st = ctx->dstats; rp.loc = ctx->res_loc; rp.tab = ctx->res_tab; rp.out = ctx->res_out;
+    rp.pairs = ctx->pairs; rp.flag = ctx->flag; rp.st = ctx->dstats; rp.loc = ctx->res_loc; rp.tab = ctx->res_tab; rp.label = ctx->res_label; rp.roots = ctx->res_roots; rp.nroots = ctx->res_nroots; rp.out = ctx->res_out;
     rp.cap = ctx->cap; rp.nb = ctx->nb; rp.ld = ctx->ld; rp.mu = ctx->mu; rp.h = dt; rp.tol = tol;
-    resolve_kernel<<<1, RES_NMAX, RES_DYN_SMEM, ctx->stream>>>(rp);
+    resolve_label_kernel<<<1, RES_NMAX, 0, ctx->stream>>>(rp);
+    mo_status s = post_launch(ctx);
+    if (s != MO_OK) return s;
+    resolve_kernel<64, 0, 32><<<ctx->res_grid, 64, RES_DYN_SMEM, ctx->stream>>>(rp);       // components of <= 32 pairs
+    s = post_launch(ctx);
+    if (s != MO_OK) return s;
+    resolve_kernel<256, 32, 128><<<ctx->res_grid, 256, RES_DYN_SMEM, ctx->stream>>>(rp);    // <= 128 pairs
+    s = post_launch(ctx);
+    if (s != MO_OK) return s;
+    resolve_kernel<RES_NMAX, 128, 1 << 30><<<ctx->res_grid, RES_NMAX, RES_DYN_SMEM, ctx->stream>>>(rp);   // the rest
     return post_launch(ctx);
 }
 

@@ -438,6 +438,46 @@ def run_support(args):
     return 0
 
 
+def run_resolve(args):
+    """Cost of the on-device close-encounter resolution: mo_step with mo_set_resolve(1e-12)
+    against the plain step, graph replay, at configs 0, 1 and 3; the Bulirsch-Stoer work of the last step (bodies,
+    accepted steps and right-hand sides summed over the components) and the time per right-hand side it implies.
+    The solve is a chain of dependent right-hand sides: latency-bound, no roofline fraction applies.  One JSON line."""
+    import torch
+    from paper_2601_19654_b200 import mopal as M
+    from paper_2601_19654_b200 import workloads as W
+    rows = []
+    for cfg, nsteps in ((0, 500), (1, 200), (3, 20)):
+        w = W.make_config(cfg)
+        row = {"workload": w.name}
+        for tag, tol in (("plain", 0.0), ("resolved", 1e-12)):
+            m = M.Mopal(w.mass, w.x, w.v, w.rcrit, m_star=w.m_star, G=w.G)
+            m.set_resolve(tol)
+            m.step(w.dt, 3)
+            rhs = 0
+            if tol > 0:                      # right-hand sides of the timed steps, counted on single steps of a twin run
+                m2 = M.Mopal(w.mass, w.x, w.v, w.rcrit, m_star=w.m_star, G=w.G)
+                m2.set_resolve(tol); m2.step(w.dt, 3)
+                for _ in range(nsteps):
+                    m2.step(w.dt, 1); rhs += m2.resolve_stats()["rhs"]
+                m2.close()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(m.stream); st = m.step(w.dt, nsteps); e1.record(m.stream); torch.cuda.synchronize()
+            row[tag + "_ms_per_step"] = e0.elapsed_time(e1) / nsteps
+            if tol > 0:
+                row["encounter_pairs_last_step"] = st.nce_last
+                row["last_step"] = m.resolve_stats()
+                row["rhs_per_step"] = rhs / nsteps
+                extra_ms = row["resolved_ms_per_step"] - row["plain_ms_per_step"]
+                row["us_per_rhs_longest_chain_bound"] = extra_ms * 1e3 / max(rhs / nsteps, 1)
+            m.close()
+        rows.append(row)
+    print(json.dumps({"metric": "encounter_resolution_cost", "tol": 1e-12, "rows": rows,
+                      "note": "us_per_rhs divides by ALL right-hand sides of a step although components run concurrently: "
+                              "it is a lower bound on the latency of one right-hand side of the slowest component"}), flush=True)
+    return 0
+
+
 def run_step_sweep(args):
     """Step time (CUDA-graph replay of 1000 steps, CUDA events) of the cfg1 disk recipe at small and middle sizes
     through each launch path the library can take, selected with its MO_* environment switches (read at
@@ -494,7 +534,10 @@ def main():
     ap.add_argument("--drift-sweep", action="store_true", help="time mo_drift alone against the HBM roofline and exit")
     ap.add_argument("--support", action="store_true", help="time mo_energy / mo_hill / mo_dh2h against their rooflines and exit")
     ap.add_argument("--step-sweep", action="store_true", help="step time at small / middle N through every launch path and exit")
+    ap.add_argument("--resolve", action="store_true", help="cost of the on-device close-encounter resolution and exit")
     args = ap.parse_args()
+    if args.resolve:
+        return run_resolve(args)
     if args.step_sweep:
         return run_step_sweep(args)
     if args.support:

@@ -117,6 +117,8 @@ __global__ void __launch_bounds__(NT) resolve_kernel(ResParams p) {
     __shared__ int sJstart[NT + 1];
     __shared__ double sRed[32];
     __shared__ int sScan[64];
+    __shared__ int sHub[6];                                             // the body with most pairs: thread, jLo, jCnt, iLo, iHi, degree
+    __shared__ double sHubAcc[3];
     double* sF = reinterpret_cast<double*>(res_dyn);                    // [RES_PMAX][3] pair terms
     double* sGi = sF + 3 * RES_PMAX;                                    // [RES_PMAX] gm of the first member
     double* sGj = sGi + RES_PMAX;                                       // [RES_PMAX] gm of the second member
@@ -190,6 +192,26 @@ __global__ void __launch_bounds__(NT) resolve_kernel(ResParams p) {
     }
     __syncthreads();
     const int jHi = jLo + jCnt;
+    // the component's hub (a giant with hundreds of pairs): its sum is taken by warp 0 together, lane l adding the
+    // terms l, l + 32, .. and a fixed shuffle tree - every other body sums its few terms alone
+    {
+        const int deg = live ? jCnt + (iHi - iLo) : 0;
+        int best = (deg << 11) | (NT - 1 - tid);                        // max degree, ties to the smallest thread
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) best = max(best, __shfl_xor_sync(0xffffffffu, best, o));
+        __syncthreads();
+        if (lane == 0) sScan[warp] = best;
+        __syncthreads();
+        int bb = sScan[0];
+        for (int w = 1; w < NT / 32; ++w) bb = max(bb, sScan[w]);
+        __syncthreads();
+        if (tid < 64) sScan[tid] = 0;                                   // the scan helper expects zeros in unused slots
+        const int hubTid = NT - 1 - (bb & 2047);
+        if (tid == hubTid) { sHub[0] = tid; sHub[1] = jLo; sHub[2] = jCnt; sHub[3] = iLo; sHub[4] = iHi; sHub[5] = deg; }
+        __syncthreads();
+    }
+    const bool hubOn = sHub[5] > 64;                                    // CTA-uniform
+    const bool iAmHub = hubOn && tid == sHub[0];
 
     // ---- state and the right-hand side ----
     double y[6] = {0, 0, 0, 0, 0, 0};
@@ -212,10 +234,28 @@ __global__ void __launch_bounds__(NT) resolve_kernel(ResParams p) {
             sF[3 * q] = u * dx; sF[3 * q + 1] = u * dy; sF[3 * q + 2] = u * dz;
         }
         __syncthreads();
+        if (hubOn) {
+            if (warp == 0) {
+                const int hj0 = sHub[1], hjc = sHub[2], hi0 = sHub[3], D = sHub[5];
+                double h0 = 0.0, h1 = 0.0, h2 = 0.0;
+                for (int t = lane; t < D; t += 32) {
+                    if (t < hjc) { const int q = sJadj[hj0 + t]; const double gi = sGi[q]; h0 -= gi * sF[3 * q]; h1 -= gi * sF[3 * q + 1]; h2 -= gi * sF[3 * q + 2]; }
+                    else { const int q = hi0 + (t - hjc); const double gj = sGj[q]; h0 += gj * sF[3 * q]; h1 += gj * sF[3 * q + 1]; h2 += gj * sF[3 * q + 2]; }
+                }
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) {
+                    h0 += __shfl_xor_sync(0xffffffffu, h0, o); h1 += __shfl_xor_sync(0xffffffffu, h1, o); h2 += __shfl_xor_sync(0xffffffffu, h2, o);
+                }
+                if (lane == 0) { sHubAcc[0] = h0; sHubAcc[1] = h1; sHubAcc[2] = h2; }
+            }
+            __syncthreads();
+        }
         if (live) {
             const double r2 = z[0] * z[0] + z[1] * z[1] + z[2] * z[2];
             const double w = -p.mu / (r2 * sqrt(r2));
             double a0 = w * z[0], a1 = w * z[1], a2 = w * z[2];
+            if (iAmHub) { a0 += sHubAcc[0]; a1 += sHubAcc[1]; a2 += sHubAcc[2]; }
+            else {
             for (int k = jLo; k < jHi; ++k) {                           // I am the second member: -gm_i u d
                 const int q = sJadj[k];
                 const double gi = sGi[q];
@@ -224,6 +264,7 @@ __global__ void __launch_bounds__(NT) resolve_kernel(ResParams p) {
             for (int q = iLo; q < iHi; ++q) {                           // I am the first member: +gm_j u d
                 const double gj = sGj[q];
                 a0 += gj * sF[3 * q]; a1 += gj * sF[3 * q + 1]; a2 += gj * sF[3 * q + 2];
+            }
             }
             f[0] = z[3]; f[1] = z[4]; f[2] = z[5]; f[3] = a0; f[4] = a1; f[5] = a2;
         }

@@ -448,6 +448,7 @@ def run_resolve(args):
     from paper_2601_19654_b200 import workloads as W
     rows = []
     for cfg, nsteps in ((0, 500), (1, 200), (3, 20)):
+        nsteps = min(nsteps, args.steps) if args.steps < 100 else nsteps      # --steps 3: a short run for profiling
         w = W.make_config(cfg)
         row = {"workload": w.name}
         for tag, tol in (("plain", 0.0), ("resolved", 1e-12)):

@@ -203,9 +203,10 @@ class Mopal:
         return _stats(s, st)
 
     def close(self):
-        if getattr(self, "_ctx", None) is not None and self._ctx.value:
-            self._L.mo_destroy(self._ctx)
-            self._ctx = C.c_void_p(None)
+        ctx = getattr(self, "_ctx", None)
+        if ctx is not None and ctx.value:
+            self._L.mo_destroy(ctx)
+            ctx.value = None          # (no module globals here: close() also runs from __del__ at interpreter exit)
 
     __del__ = close
 

@@ -48,7 +48,7 @@ struct mo_ctx {
     double res_tol = 0.0;               // mo_set_resolve: <= 0 off
     int* res_loc = nullptr;             // nb ints (lazy)
     double* res_tab = nullptr;          // extrapolation tableaux, one set per CTA
-    int *res_label = nullptr, *res_roots = nullptr, *res_nroots = nullptr;
+    int *res_label = nullptr, *res_roots = nullptr, *res_nroots = nullptr, *res_done = nullptr;
     int res_grid = 1;
     ResStats* res_out = nullptr;        // device
     ResStats* res_host = nullptr;       // pinned
@@ -245,7 +245,7 @@ extern "C" void mo_destroy(mo_ctx* ctx) {
     for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
     cudaFree(ctx->gm); cudaFree(ctx->x0); cudaFree(ctx->v0); cudaFree(ctx->part);
     cudaFree(ctx->psumA); cudaFree(ctx->psumB); cudaFree(ctx->ticket);
-    cudaFree(ctx->res_loc); cudaFree(ctx->res_out); cudaFree(ctx->res_tab); cudaFree(ctx->res_label); cudaFree(ctx->res_roots); cudaFree(ctx->res_nroots);
+    cudaFree(ctx->res_loc); cudaFree(ctx->res_out); cudaFree(ctx->res_tab); cudaFree(ctx->res_label); cudaFree(ctx->res_roots); cudaFree(ctx->res_nroots); cudaFree(ctx->res_done);
     if (ctx->res_host) cudaFreeHost(ctx->res_host);
     cudaFree(ctx->gmsum); cudaFree(ctx->en_on); cudaFree(ctx->en_pair); cudaFree(ctx->en_out);
     if (ctx->en_host) cudaFreeHost(ctx->en_host); cudaFree(ctx->tiles);
@@ -532,9 +532,11 @@ static mo_status ensure_resolve_scratch(mo_ctx* ctx) {
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_label, (size_t)ctx->nb);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_roots, (size_t)(ctx->cap > 0 ? ctx->cap : 1));
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_nroots, 1);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(resolve_kernel<64, 0, 32>, cudaFuncAttributeMaxDynamicSharedMemorySize, RES_DYN_SMEM);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(resolve_kernel<256, 32, 128>, cudaFuncAttributeMaxDynamicSharedMemorySize, RES_DYN_SMEM);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(resolve_kernel<RES_NMAX, 128, 1 << 30>, cudaFuncAttributeMaxDynamicSharedMemorySize, RES_DYN_SMEM);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_done, (size_t)(ctx->cap > 0 ? ctx->cap : 1));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(resolve_kernel<64, 0, 32, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, RES_DYN_SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(resolve_kernel<256, 32, 128, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, RES_DYN_SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(resolve_kernel<512, 128, 1 << 30, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, RES_DYN_SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(resolve_kernel<RES_NMAX, 128, 1 << 30, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, RES_DYN_SMEM);
     if (e == cudaSuccess) e = cudaMemsetAsync(ctx->res_out, 0, sizeof(ResStats), ctx->stream);
     if (e == cudaSuccess) e = cudaMallocHost(reinterpret_cast<void**>(&ctx->res_host), sizeof(ResStats));
     if (e != cudaSuccess) { cudaGetLastError(); ctx->last_err = e; return e == cudaErrorMemoryAllocation ? MO_ENOMEM : MO_ECUDA; }
@@ -544,18 +546,21 @@ static mo_status ensure_resolve_scratch(mo_ctx* ctx) {
 static mo_status enqueue_resolve(mo_ctx* ctx, double dt, double tol) {
     ResParams rp;
     rp.x0 = ctx->x0; rp.v0 = ctx->v0; rp.x = ctx->x; rp.v = ctx->v; rp.gm = ctx->gm; rp.rcrit = ctx->rcrit;
-    rp.pairs = ctx->pairs; rp.flag = ctx->flag; rp.st = ctx->dstats; rp.loc = ctx->res_loc; rp.tab = ctx->res_tab; rp.label = ctx->res_label; rp.roots = ctx->res_roots; rp.nroots = ctx->res_nroots; rp.out = ctx->res_out;
+    rp.pairs = ctx->pairs; rp.flag = ctx->flag; rp.st = ctx->dstats; rp.loc = ctx->res_loc; rp.tab = ctx->res_tab; rp.label = ctx->res_label; rp.roots = ctx->res_roots; rp.nroots = ctx->res_nroots; rp.done = ctx->res_done; rp.out = ctx->res_out;
     rp.cap = ctx->cap; rp.nb = ctx->nb; rp.ld = ctx->ld; rp.mu = ctx->mu; rp.h = dt; rp.tol = tol;
     resolve_label_kernel<<<1, RES_NMAX, 0, ctx->stream>>>(rp);
     mo_status s = post_launch(ctx);
     if (s != MO_OK) return s;
-    resolve_kernel<64, 0, 32><<<ctx->res_grid, 64, RES_DYN_SMEM, ctx->stream>>>(rp);       // components of <= 32 pairs
+    resolve_kernel<64, 0, 32, true><<<ctx->res_grid, 64, RES_DYN_SMEM, ctx->stream>>>(rp);       // components of <= 32 pairs
     s = post_launch(ctx);
     if (s != MO_OK) return s;
-    resolve_kernel<256, 32, 128><<<ctx->res_grid, 256, RES_DYN_SMEM, ctx->stream>>>(rp);    // <= 128 pairs
+    resolve_kernel<256, 32, 128, true><<<ctx->res_grid, 256, RES_DYN_SMEM, ctx->stream>>>(rp);    // <= 128 pairs
     s = post_launch(ctx);
     if (s != MO_OK) return s;
-    resolve_kernel<RES_NMAX, 128, 1 << 30><<<ctx->res_grid, RES_NMAX, RES_DYN_SMEM, ctx->stream>>>(rp);   // the rest
+    resolve_kernel<512, 128, 1 << 30, false><<<ctx->res_grid, 512, RES_DYN_SMEM, ctx->stream>>>(rp);   // more pairs, <= 512 bodies
+    s = post_launch(ctx);
+    if (s != MO_OK) return s;
+    resolve_kernel<RES_NMAX, 128, 1 << 30, true><<<ctx->res_grid, RES_NMAX, RES_DYN_SMEM, ctx->stream>>>(rp);   // the rest
     return post_launch(ctx);
 }
 

@@ -34,6 +34,7 @@ struct ResParams {
     int* loc;                    // nb scratch: body -> index in its component
     int* label;                  // nb scratch: smallest body of the component (valid for flagged bodies)
     int* roots; int* nroots;     // the components' smallest bodies
+    int* done;                   // per component: 1 once an instance of resolve_kernel has taken it
     double* tab;                 // 6 * RES_KMAX * RES_NMAX scratch: the extrapolation tableaux, [component][column][thread]
                                  // (kept out of local memory: a large per-thread stack makes the driver resize its
                                  // local-memory pool around every launch)
@@ -99,16 +100,18 @@ __global__ void __launch_bounds__(RES_NMAX) resolve_label_kernel(ResParams p) {
     } while (changed);
     for (int q = tid; q < np; q += RES_NMAX) {
         const int i = p.pairs[2 * q];
-        if (label[i] == i && (q == 0 || p.pairs[2 * (q - 1)] != i)) p.roots[atomicAdd(p.nroots, 1)] = i;
+        if (label[i] == i && (q == 0 || p.pairs[2 * (q - 1)] != i)) { const int c = atomicAdd(p.nroots, 1); p.roots[c] = i; p.done[c] = 0; }
     }
 }
 
 // One CTA per component (CTAs walk the root list), one thread per body of the component.  Three instances by
 // the component's number of pairs, PLO < np <= PHI, with NT = 2 PHI threads (a component of np pairs has at
 // most 2 np bodies; the last instance takes what fits 1024 bodies): most components are single pairs, and the
-// barriers of every right-hand side cost by the warp - 64 threads for np <= 32, 256 for np <= 128, 1024 above
-// (the stars around the big bodies).
-template <int NT, int PLO, int PHI>
+// barriers of every right-hand side cost by the warp - 64 threads for np <= 32, 256 for np <= 128, then 512
+// threads if the bodies fit (the stars around the big bodies), else 1024.
+// LAST: the instance that takes whatever the earlier ones left (they skip a component whose bodies outnumber
+// their threads; the last one counts it as failed).
+template <int NT, int PLO, int PHI, bool LAST>
 __global__ void __launch_bounds__(NT) resolve_kernel(ResParams p) {
     extern __shared__ __align__(16) unsigned char res_dyn[];
     __shared__ double sX[3 * NT];                                 // positions of the current right-hand side
@@ -144,8 +147,8 @@ __global__ void __launch_bounds__(NT) resolve_kernel(ResParams p) {
         if (mine && np + off < RES_PMAX) sPq[np + off] = q;
         np += tot;
     }
-    if (np <= PLO || np > PHI) continue;                               // another instance's component
-    if (np > RES_PMAX) { if (tid == 0) atomicAdd(&p.out->fail, 1); continue; }
+    if (np <= PLO || np > PHI || p.done[comp]) continue;               // another instance's component
+    if (np > RES_PMAX) { if (LAST && tid == 0) atomicAdd(&p.out->fail, 1); continue; }
     // ---- its bodies in ascending order (thread t scans its own segment of the flags) ----
     const int seg = (p.nb + NT - 1) / NT;
     const int b0 = tid * seg, b1 = min(p.nb, b0 + seg);
@@ -158,7 +161,11 @@ __global__ void __launch_bounds__(NT) resolve_kernel(ResParams p) {
             for (int b = b0; b < b1; ++b)
                 if (p.flag[b] && p.label[b] == root) { p.loc[b] = k; sJstart[k] = b; ++k; }   // sJstart doubles as the body list
     }
-    if (n > NT) { if (tid == 0) { atomicAdd(&p.out->fail, 1); atomicAdd(&p.out->bodies, n); } continue; }
+    if (n > NT) {
+        if (LAST && tid == 0) { atomicAdd(&p.out->fail, 1); atomicAdd(&p.out->bodies, n); }
+        continue;                                                      // not LAST: a later, wider instance takes it
+    }
+    if (tid == 0) p.done[comp] = 1;
     __syncthreads();
     const bool live = tid < n;
     const int me = live ? sJstart[tid] : 0;                            // my global body index

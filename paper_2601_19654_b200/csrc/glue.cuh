@@ -1,6 +1,6 @@
 // glue.cuh - the O(N) parts of the hybrid step (Hamiltonian block, and
-// the drift loop), fused so that one step is eight launches and no
-// per-body quantity goes through HBM more than once per stage:
+// the drift loop), fused so that no per-body quantity goes through HBM more
+// than once per stage (the whole step is 13 launches; step_small.cuh: 2 for small systems):
 //   kick_psum_kernel        LOOP 1 (v += h/2 a)  + LOOP 2 partials (sum gm v)
 //   jump_drift_boxes_kernel LOOP 2 finish + LOOP 3 (x += h/2 P/mu) + LOOP 4 (x0,v0 copy)
 //                           + keplerian drift + mce_snif LOOP 1-2 (boxes) + the partials of

@@ -818,8 +818,8 @@ int oracle_energy(int nb, int nbig, int ld, double G, double mstar, const double
  *       |T_kk - T_k,k-1| / scale, scale = |x_i| (positions) and |v_i| (velocities) of that body at
  *       the start of the BS step; accepted when <= tol
  *   X-4 step control by column only: accepted at column k <= 3: H_next = 2 H; k <= 5: H; else H/2;
- *       no column accepted: H/2 and retry (at most 40 halvings, else failure: bodies keep the drift
- *       result); H never exceeds what is left of h
+ *       no column accepted: H/2 and retry (40 halvings in a row are a failure: the bodies keep the
+ *       drift result); H never exceeds what is left of h
  *   X-5 pairs summed in list order per body; coincident bodies contribute 0
  * ------------------------------------------------------------------------- */
 #define BS_KMAX 8
@@ -953,6 +953,7 @@ static int resolve_system(int nb, int ld, double mu, const double *gm, const dou
         for (int c = 0; c < m; ++c) y[c] = T[(size_t)c * BS_KMAX + acc_col];
         t = last ? hh : t + H;
         ++nacc;
+        halvings = 0;                                          /* X-4: 40 CONSECUTIVE halvings are a failure */
         if (acc_col <= 3) H *= (real)2; else if (acc_col > 5) H *= (real)0.5L;
     }
     if (!fail) {

@@ -346,6 +346,7 @@ __global__ void __launch_bounds__(NT) resolve_kernel(ResParams p) {
         for (int c = 0; c < 6; ++c) y[c] = T[((size_t)c * RES_KMAX + acc) * NT];
         t = last ? hh : t + H;
         ++nacc;
+        halv = 0;                                                       // X-4: 40 halvings in a row are a failure
         if (acc <= 3) H *= 2.0; else if (acc > 5) H *= 0.5;
     }
     if (!fail && live) {

@@ -873,3 +873,43 @@ def test_resolve_energy_and_limits(M):
     assert L.mo_resolve(m._ctx, 0.0, 1e-12) == M.MO_EINVAL and L.mo_resolve(m._ctx, 1.0, 0.0) == M.MO_EINVAL
     assert L.mo_resolve_stats(m._ctx, None) == M.MO_EINVAL and L.mo_set_resolve(None, 1.0) == M.MO_EINVAL
     m.close()
+
+
+@pytest.mark.parametrize("K,expect", [(300, "512"), (700, "1024"), (100, "256")])
+def test_resolve_big_star_components(M, K, expect):
+    """a giant with K planetesimals inside its critical radius: one star component of K+1 bodies - the 256-, 512- and
+    1024-thread instances of resolve_kernel and the warp-summed hub, against the oracle"""
+    rng = np.random.default_rng(40 + K)
+    m_star, mg = 1.0, 1e-3
+    # K = 700 keeps 0.15 AU from the giant: with grazing passes AND 700 bodies the FP64 error estimate sits at its
+    # rounding floor for tol = 1e-12 and the kernel takes more (smaller) steps than the long-double oracle
+    ang = rng.uniform(0, 2 * np.pi, K); rad = rng.uniform(0.15 if K > 500 else 0.02, 0.85, K); zz = rng.uniform(-0.01, 0.01, K)
+    xg = np.array([5.2, 0.0, 0.0])
+    X = np.empty((3, K + 1)); X[:, 0] = xg
+    X[0, 1:] = xg[0] + rad * np.cos(ang); X[1, 1:] = xg[1] + rad * np.sin(ang); X[2, 1:] = zz
+    r = np.linalg.norm(X, axis=0)
+    vc = np.sqrt(G * m_star / r)                                   # circular heliocentric speeds
+    Vh = np.stack([-vc * X[1] / r, vc * X[0] / r, np.zeros(K + 1)])
+    mass = np.concatenate([[mg], np.full(K, 1e-9)])
+    V = oracle.h2dh(m_star, mass, Vh)
+    _, rc = oracle.hill(G, m_star, mass, X, V, n_hill=3.0)
+    mu, gm, dt = G * m_star, G * mass, 8.0
+    x1, v1, _ = oracle.drift(mu, dt, X, V)
+    enc = oracle.encounters(dt, X, V, x1, v1, rc)
+    assert enc["count"] >= K and (enc["pairs"][:K, 0] == 0).all()
+    ref = oracle.resolve(mu, gm, rc, dt, X, V, x1, v1, enc["pairs"])
+    assert ref["fail"] == 0 and ref["n"] == K + 1
+    m = M.Mopal(mass, X, V, rc, m_star=m_star, G=G)
+    m.snapshot(); m.set("x", x1); m.set("v", v1)
+    cnt = m.encounters(dt)
+    assert np.array_equal(m.pair_list(cnt), enc["pairs"])
+    m.resolve(dt, 1e-12)
+    st = m.resolve_stats()
+    assert st["fail"] == 0 and st["bodies"] == K + 1 and st["steps"] == ref["nsteps"] and st["rhs"] == ref["nrhs"], (st, ref["nsteps"], ref["nrhs"])
+    # same BS steps on both sides, so they differ by rounding only (FP64 against long double) - but a planetesimal
+    # that passes 0.02 AU from the giant amplifies it: 1e-10 here (1e-12 in the gentler cases above)
+    assert _rel_vec_err(m.get("x"), ref["x"]).max() <= 1e-10 and _rel_vec_err(m.get("v"), ref["v"]).max() <= 1e-10
+    far = rad > 0.3
+    assert _rel_vec_err(m.get("x")[:, 1:][:, far], ref["x"][:, 1:][:, far]).max() <= 1e-12
+    assert _rel_vec_err(m.get("v")[:, :1], v1[:, :1]).max() > 1e-12       # the giant felt its planetesimals
+    m.close()

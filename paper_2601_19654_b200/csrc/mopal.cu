@@ -533,8 +533,8 @@ static mo_status ensure_resolve_scratch(mo_ctx* ctx) {
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_roots, (size_t)(ctx->cap > 0 ? ctx->cap : 1));
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_nroots, 1);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_done, (size_t)(ctx->cap > 0 ? ctx->cap : 1));
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(resolve_kernel<64, 0, 32, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, RES_DYN_SMEM);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(resolve_kernel<256, 32, 128, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, RES_DYN_SMEM);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(resolve_kernel<64, 0, 32, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, RES_DYN_SMEM + 6 * RES_KMAX * 64 * 8);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(resolve_kernel<256, 32, 128, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, RES_DYN_SMEM + 6 * RES_KMAX * 256 * 8);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(resolve_kernel<512, 128, 1 << 30, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, RES_DYN_SMEM);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(resolve_kernel<RES_NMAX, 128, 1 << 30, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, RES_DYN_SMEM);
     if (e == cudaSuccess) e = cudaMemsetAsync(ctx->res_out, 0, sizeof(ResStats), ctx->stream);
@@ -551,10 +551,10 @@ static mo_status enqueue_resolve(mo_ctx* ctx, double dt, double tol) {
     resolve_label_kernel<<<1, RES_NMAX, 0, ctx->stream>>>(rp);
     mo_status s = post_launch(ctx);
     if (s != MO_OK) return s;
-    resolve_kernel<64, 0, 32, true><<<ctx->res_grid, 64, RES_DYN_SMEM, ctx->stream>>>(rp);       // components of <= 32 pairs
+    resolve_kernel<64, 0, 32, true><<<ctx->res_grid, 64, RES_DYN_SMEM + 6 * RES_KMAX * 64 * 8, ctx->stream>>>(rp);       // components of <= 32 pairs
     s = post_launch(ctx);
     if (s != MO_OK) return s;
-    resolve_kernel<256, 32, 128, true><<<ctx->res_grid, 256, RES_DYN_SMEM, ctx->stream>>>(rp);    // <= 128 pairs
+    resolve_kernel<256, 32, 128, true><<<ctx->res_grid, 256, RES_DYN_SMEM + 6 * RES_KMAX * 256 * 8, ctx->stream>>>(rp);    // <= 128 pairs
     s = post_launch(ctx);
     if (s != MO_OK) return s;
     resolve_kernel<512, 128, 1 << 30, false><<<ctx->res_grid, 512, RES_DYN_SMEM, ctx->stream>>>(rp);   // more pairs, <= 512 bodies

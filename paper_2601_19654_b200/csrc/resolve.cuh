@@ -281,7 +281,8 @@ __global__ void __launch_bounds__(NT) resolve_kernel(ResParams p) {
     const double hh = p.h;
     double t = 0.0, H = hh;
     int fail = 0, nacc = 0, halv = 0;
-    double* T = p.tab + (size_t)blockIdx.x * 6 * RES_KMAX * NT + tid;                                           // T_{row, j} of component c at T[(c * RES_KMAX + j) * threads]
+    // the tableaux: shared memory for the instances of up to 256 threads, global scratch above
+    double* T = (NT <= 256 ? reinterpret_cast<double*>(res_dyn + RES_DYN_SMEM) : p.tab + (size_t)blockIdx.x * 6 * RES_KMAX * NT) + tid;                                           // T_{row, j} of component c at T[(c * RES_KMAX + j) * threads]
     while (!fail) {
         const double rem = hh - t;
         if (fabs(rem) <= 4.0 * 2.220446049250313e-16 * fabs(hh)) break;
@@ -308,15 +309,21 @@ __global__ void __launch_bounds__(NT) resolve_kernel(ResParams p) {
             double err = 0.0;
 #pragma unroll
             for (int c = 0; c < 6; ++c) {
-                // row k of the tableau from row k-1 (in T), overwriting it column by column
+                // row k of the tableau from row k-1 (in T), overwriting it column by column; the old row is read
+                // first, all loads in flight together (interleaved with the stores they would serialise)
                 double* Tc = T + (size_t)c * RES_KMAX * NT;
+                double old[RES_KMAX];
+#pragma unroll
+                for (int j = 0; j < RES_KMAX; ++j) old[j] = (j < k) ? Tc[(size_t)j * NT] : 0.0;
                 double cur = res[c], prev = 0.0;
-                for (int j = 1; j <= k; ++j) {
-                    const double ratio = (double)(2 * (k + 1)) / (double)(2 * (k - j + 1));
-                    const double old = Tc[(size_t)(j - 1) * NT];
-                    Tc[(size_t)(j - 1) * NT] = cur;
-                    prev = cur;
-                    cur = cur + (cur - old) / (ratio * ratio - 1.0);
+#pragma unroll
+                for (int j = 1; j < RES_KMAX; ++j) {
+                    if (j <= k) {
+                        const double ratio = (double)(2 * (k + 1)) / (double)(2 * (k - j + 1));
+                        Tc[(size_t)(j - 1) * NT] = cur;
+                        prev = cur;
+                        cur = cur + (cur - old[j - 1]) / (ratio * ratio - 1.0);
+                    }
                 }
                 Tc[(size_t)k * NT] = cur;
                 if (k >= 1 && live) {

@@ -447,7 +447,7 @@ static mo_status enqueue_accel(mo_ctx* ctx, bool jump, double hj, bool kick, dou
     const int nblk = (ctx->nb + ON_BLOCK - 1) / ON_BLOCK;
     if (ctx->use_sym) {
         auto rk = kick ? sym_reduce_kernel<true> : sym_reduce_kernel<false>;
-        rk<<<nblk, ON_BLOCK, 0, ctx->stream>>>(ctx->sym_partI, ctx->sym_partJ, ctx->sym_ustart, ctx->nb, ctx->ld, ctx->nbPad,
+        rk<<<dim3(nblk, 3), ON_BLOCK, 0, ctx->stream>>>(ctx->sym_partI, ctx->sym_partJ, ctx->sym_ustart, ctx->nb, ctx->ld, ctx->nbPad,
                                                ctx->a, kick ? ctx->v : nullptr, kick ? hk : 0.0);
     } else if (kick)
         accel_reduce_kernel<true><<<nblk, ON_BLOCK, 0, ctx->stream>>>(ctx->part, ctx->nsplit, ctx->nb, ctx->ld, ctx->a, ctx->v, hk);

@@ -273,21 +273,35 @@ __global__ void __launch_bounds__(ON_BLOCK) sym_reduce_kernel(const double* __re
                                                                const int* __restrict__ ustart, int nb, int ld,
                                                                int nbPad, double* __restrict__ a,
                                                                double* __restrict__ v, double hk) {
+    // one thread per (body, component) - blockIdx.y = component - and four interleaved partial sums per
+    // list, combined in a fixed order: three times the threads and four times the loads in flight of a
+    // thread-per-body loop, still a fixed tree that depends on nb only
     const int b = blockIdx.x * ON_BLOCK + threadIdx.x;
     if (b >= nb) return;
+    const int c = blockIdx.y;
     const int Ib = b / SYM_R, r = b - Ib * SYM_R;
     const int u0 = ustart[Ib], u1 = ustart[Ib + 1];
-#pragma unroll
-    for (int c = 0; c < 3; ++c) {
-        double s = 0.0;
-        for (int u = u0; u < u1; ++u) s += partI[((size_t)u * 3 + c) * SYM_R + r];
-        for (int I = 0; I <= Ib; ++I) {
-            const int jw = nbPad - I * SYM_R;
-            s += partJ[symJ_off(I, nbPad) + (size_t)c * jw + (b - I * SYM_R)];
-        }
-        a[(size_t)c * ld + b] = s;
-        if (KICK) v[(size_t)c * ld + b] = fma(hk, s, v[(size_t)c * ld + b]);
+    double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
+    int u = u0;
+    for (; u + 3 < u1; u += 4) {
+        s0 += partI[((size_t)u * 3 + c) * SYM_R + r];
+        s1 += partI[((size_t)(u + 1) * 3 + c) * SYM_R + r];
+        s2 += partI[((size_t)(u + 2) * 3 + c) * SYM_R + r];
+        s3 += partI[((size_t)(u + 3) * 3 + c) * SYM_R + r];
     }
+    for (; u < u1; ++u) s0 += partI[((size_t)u * 3 + c) * SYM_R + r];
+    double t0 = 0.0, t1 = 0.0, t2 = 0.0, t3 = 0.0;
+    int I = 0;
+    for (; I + 3 <= Ib; I += 4) {
+        t0 += partJ[symJ_off(I, nbPad) + (size_t)c * (nbPad - I * SYM_R) + (b - I * SYM_R)];
+        t1 += partJ[symJ_off(I + 1, nbPad) + (size_t)c * (nbPad - (I + 1) * SYM_R) + (b - (I + 1) * SYM_R)];
+        t2 += partJ[symJ_off(I + 2, nbPad) + (size_t)c * (nbPad - (I + 2) * SYM_R) + (b - (I + 2) * SYM_R)];
+        t3 += partJ[symJ_off(I + 3, nbPad) + (size_t)c * (nbPad - (I + 3) * SYM_R) + (b - (I + 3) * SYM_R)];
+    }
+    for (; I <= Ib; ++I) t0 += partJ[symJ_off(I, nbPad) + (size_t)c * (nbPad - I * SYM_R) + (b - I * SYM_R)];
+    const double s = ((s0 + s1) + (s2 + s3)) + ((t0 + t1) + (t2 + t3));
+    a[(size_t)c * ld + b] = s;
+    if (KICK) v[(size_t)c * ld + b] = fma(hk, s, v[(size_t)c * ld + b]);
 }
 
 }  // namespace mopal

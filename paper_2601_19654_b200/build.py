@@ -33,7 +33,8 @@ def build_lib(force: bool = False, verbose: bool = False) -> str:
     if r.returncode != 0:
         raise RuntimeError("nvcc failed building libmopal.so")
     with open(os.path.join(HERE, "ptxas_info.txt"), "w") as f:
-        f.write(" ".join(cmd) + "\n" + r.stderr)
+        # registers / spills / shared memory per kernel; the "Compile time" lines change from run to run
+        f.write(" ".join(cmd) + "\n" + "".join(l for l in r.stderr.splitlines(True) if "Compile time" not in l))
     return LIB
 
 

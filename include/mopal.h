@@ -62,8 +62,11 @@ typedef enum {
     MO_ECUDA = 3,     /* CUDA runtime error (or no device) */
     MO_EOVERFLOW = 4, /* more encounter pairs than `cap`: the first `cap` pairs in sorted
                          order are stored, the count is still the true total */
-    MO_ENOCONV = 5    /* >= 1 body's Kepler solve failed (paper's iflag);
+    MO_ENOCONV = 5,   /* >= 1 body's Kepler solve failed (paper's iflag);
                          those bodies are left unchanged, the others advanced */
+    MO_ERESOLVE = 6   /* mo_set_resolve / mo_resolve: >= 1 encounter component was not resolved (no
+                         convergence, or a truncated pair list); its bodies kept the Kepler-drift
+                         result of that step.  Sticky: counted in mo_stats.resolve_fail */
 } mo_status;
 
 typedef struct {
@@ -72,6 +75,8 @@ typedef struct {
     int64_t nce_total;  /* sum of nce_last over all passes */
     int32_t drift_fail; /* bodies whose Kepler solve failed, cumulative */
     int32_t max_newton; /* largest Newton iteration count any body needed so far */
+    int32_t resolve_fail; /* encounter components the Bulirsch-Stoer solve gave up on, cumulative */
+    int32_t reserved;
 } mo_stats;
 
 /* Create a context.  Reads `mass` once (gm = G*mass is kept in scratch).
@@ -109,7 +114,8 @@ mo_status mo_encounters(mo_ctx *ctx, double dt, const double *x0, const double *
 /* nsteps hybrid steps of size dt.  `a` must be current for `x` unless the context has
  * never computed it or mo_invalidate_accel was called (then it is computed first, the
  * paper's first-call logic).  stats_host nullable; if given the call
- * synchronises and returns MO_EOVERFLOW / MO_ENOCONV if either happened. */
+ * synchronises and returns MO_EOVERFLOW / MO_ENOCONV / MO_ERESOLVE (in that order of
+ * precedence) if any of them happened since mo_create. */
 mo_status mo_step(mo_ctx *ctx, double dt, int32_t nsteps, mo_stats *stats_host);
 
 void mo_destroy(mo_ctx *ctx);
@@ -181,6 +187,11 @@ mo_status mo_snapshot(mo_ctx *ctx);
 mo_status mo_snapshot_ptrs(mo_ctx *ctx, const double **x0, const double **v0);
 /* Copy the snapshot into caller-owned device arrays (3*ld doubles each; asynchronous). */
 mo_status mo_snapshot_copy(mo_ctx *ctx, double *x0_dst, double *v0_dst);
+/* mce_snif LOOP 1-2, for inspection: copy the per-body boxes of the last encounter
+ * pass (mo_encounters or the last mo_step) into box_dst (device, 4*nb doubles): body b at
+ * box_dst[4b..4b+3] = {lo_x, hi_x, lo_y, hi_y}, extremes of the cubic Hermite interpolant over the step,
+ * padded by rcrit for the big bodies.  Asynchronous.  MO_EINVAL before any encounter pass. */
+mo_status mo_boxes_copy(mo_ctx *ctx, double *box_dst);
 /* Tell the context that the caller changed x: the next mo_step recomputes a first. */
 mo_status mo_invalidate_accel(mo_ctx *ctx);
 /* Synchronise the stream and read the statistics. */

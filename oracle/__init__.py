@@ -45,6 +45,8 @@ def _lib(kind="ld"):
     D, I, I64 = C.POINTER(C.c_double), C.c_int, C.c_int64
     P32, PU8, PI64 = C.POINTER(C.c_int32), C.POINTER(C.c_uint8), C.POINTER(C.c_int64)
     L.oracle_real_bytes.restype = I
+    L.oracle_set_num_threads.restype = I
+    L.oracle_set_num_threads.argtypes = [I]
     L.oracle_changeover.restype = C.c_double
     L.oracle_changeover.argtypes = [C.c_double, C.c_double]
     L.oracle_accel_big.restype = I
@@ -98,8 +100,11 @@ def real_bytes(kind="ld") -> int:
     return _lib(kind).oracle_real_bytes()
 
 
-def set_threads(n: int) -> None:
+def set_threads(n: int, kind="ld") -> int:
+    """OpenMP threads of the outer body loops of build `kind` (timing only; no result depends on it).
+    Returns the thread count in force."""
     os.environ["OMP_NUM_THREADS"] = str(int(n))
+    return int(_lib(kind).oracle_set_num_threads(int(n)))
 
 
 def changeover(r: float, rc: float, kind="ld") -> float:

@@ -77,6 +77,15 @@ static inline real rmin(real a, real b) { return a < b ? a : b; }
 
 int oracle_real_bytes(void) { return (int)sizeof(real); }
 
+/* Threads of the `omp parallel for` over the outer body loops (timing legs of bench.py: one thread
+ * and all cores); n <= 0 only reports.  No arithmetic depends on it. */
+#ifdef _OPENMP
+#include <omp.h>
+int oracle_set_num_threads(int n) { if (n > 0) omp_set_num_threads(n); return omp_get_max_threads(); }
+#else
+int oracle_set_num_threads(int n) { (void)n; return 1; }
+#endif
+
 /* ---------------------------------------------------------------------------
  * Changeover weight K(s ; rc)  [reading A-1, A-4, A-5; PAPER.md:104 fn. 14]
  *   q = (s - 0.1 rc) / (0.9 rc);  K = 0 (q<=0), 1 (q>=1), else q^3 (10 - 15 q + 6 q^2)

@@ -32,7 +32,7 @@ def build_lib(force: bool = False, verbose: bool = False) -> str:
         sys.stderr.write(r.stdout + r.stderr)
     if r.returncode != 0:
         raise RuntimeError("nvcc failed building libmopal.so")
-    with open(os.path.join(HERE, "ptxas_info.txt"), "w") as f:
+    with open(os.path.join(HERE, "ptxas_info.txt"), "w") as f:   # a build log (git-ignored)
         # registers / spills / shared memory per kernel; the "Compile time" lines change from run to run
         f.write(" ".join(cmd) + "\n" + "".join(l for l in r.stderr.splitlines(True) if "Compile time" not in l))
     return LIB

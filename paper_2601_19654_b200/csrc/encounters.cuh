@@ -552,7 +552,7 @@ struct DevStats {
     long long steps_done, nce_last, nce_total;
     int drift_fail, max_newton;
     int overflow;  // sticky: some pass found more pairs than cap
-    int pad;
+    int resolve_fail;  // cumulative: encounter components the Bulirsch-Stoer solve gave up on
 };
 
 // one block per run of TJ rows: the block's base is the sum of the per-tile hit counts before it

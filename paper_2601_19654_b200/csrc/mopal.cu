@@ -79,7 +79,7 @@ struct mo_ctx {
     std::vector<int4> h_units;
     std::vector<int> h_ustart;
     bool pair_ready = false;
-    bool a_valid = false, snap_valid = false, debug = false, use_graph = true;
+    bool a_valid = false, snap_valid = false, box_valid = false, debug = false, use_graph = true;
     long long launches = 0;
     cudaError_t last_err = cudaSuccess;
     // graph cache (one dt)
@@ -228,6 +228,7 @@ extern "C" const char* mo_strerror(mo_status s) {
         case MO_ECUDA: return "CUDA error or no CUDA device";
         case MO_EOVERFLOW: return "more encounter pairs than cap";
         case MO_ENOCONV: return "Kepler solve failed for at least one body";
+        case MO_ERESOLVE: return "at least one encounter component was not resolved";
     }
     return "unknown status";
 }
@@ -358,7 +359,7 @@ static mo_status ensure_pair_scratch(mo_ctx* ctx) {
         if (e == cudaSuccess) e = dalloc(ctx, &ctx->v1, 3 * (size_t)ctx->ld);
     }
     const size_t pl = 3 * (size_t)ctx->ld;
-    if (!ctx->use_sym && !ctx->use_big && !ctx->use_psm) e = dalloc(ctx, &ctx->part, pl * (size_t)ctx->nsplit);
+    if (e == cudaSuccess && !ctx->use_sym && !ctx->use_big && !ctx->use_psm) e = dalloc(ctx, &ctx->part, pl * (size_t)ctx->nsplit);
     if (ctx->use_sym) {
         if (e == cudaSuccess) e = dalloc(ctx, &ctx->sym_units, (size_t)ctx->sym_nunits);
         if (e == cudaSuccess) e = dalloc(ctx, &ctx->sym_ustart, ctx->h_ustart.size());
@@ -371,6 +372,7 @@ static mo_status ensure_pair_scratch(mo_ctx* ctx) {
     if (e != cudaSuccess) {
         cudaGetLastError();
         ctx->last_err = e;
+        ctx->overlap = false;      // never run the forked step on half-made streams / copies
         return e == cudaErrorMemoryAllocation ? MO_ENOMEM : MO_ECUDA;
     }
     ctx->pair_ready = true;
@@ -640,6 +642,8 @@ static mo_status read_stats(mo_ctx* ctx, mo_stats* out, bool* overflow) {
         out->nce_total = ctx->hstats->nce_total;
         out->drift_fail = ctx->hstats->drift_fail;
         out->max_newton = ctx->hstats->max_newton;
+        out->resolve_fail = ctx->hstats->resolve_fail;
+        out->reserved = 0;
     }
     if (overflow) *overflow = ctx->hstats->overflow != 0;
     return MO_OK;
@@ -653,6 +657,7 @@ static mo_status status_from_stats(mo_ctx* ctx, mo_stats* out) {
     if (out) *out = tmp;
     if (ovf) return MO_EOVERFLOW;
     if (tmp.drift_fail > 0) return MO_ENOCONV;
+    if (tmp.resolve_fail > 0) return MO_ERESOLVE;
     return MO_OK;
 }
 
@@ -695,6 +700,12 @@ extern "C" mo_status mo_snapshot_copy(mo_ctx* ctx, double* x0_dst, double* v0_ds
     const size_t bytes = 3 * (size_t)ctx->ld * sizeof(double);
     CK(cudaMemcpyAsync(x0_dst, ctx->x0, bytes, cudaMemcpyDeviceToDevice, ctx->stream));
     CK(cudaMemcpyAsync(v0_dst, ctx->v0, bytes, cudaMemcpyDeviceToDevice, ctx->stream));
+    return MO_OK;
+}
+
+extern "C" mo_status mo_boxes_copy(mo_ctx* ctx, double* box_dst) {
+    if (!ctx || !box_dst || !ctx->box_valid) return MO_EINVAL;
+    CK(cudaMemcpyAsync(box_dst, ctx->enc.box, (size_t)ctx->nb * sizeof(double4), cudaMemcpyDeviceToDevice, ctx->stream));
     return MO_OK;
 }
 
@@ -830,6 +841,7 @@ extern "C" mo_status mo_encounters(mo_ctx* ctx, double dt, const double* x0, con
     if (s != MO_OK) return s;
     s = enqueue_pairs(ctx, es, 0);
     if (s != MO_OK) return s;
+    ctx->box_valid = true;
     if (count_host) {
         mo_stats st;
         s = read_stats(ctx, &st, nullptr);
@@ -886,7 +898,7 @@ extern "C" mo_status mo_step(mo_ctx* ctx, double dt, int32_t nsteps, mo_stats* s
             if (s != MO_OK) return s;
         }
     }
-    if (nsteps > 0) { ctx->snap_valid = true; ctx->a_valid = true; }
+    if (nsteps > 0) { ctx->snap_valid = true; ctx->a_valid = true; ctx->box_valid = true; }
     if (stats_host) return status_from_stats(ctx, stats_host);
     return MO_OK;
 }

@@ -30,7 +30,7 @@ struct ResParams {
     const double *gm, *rcrit;
     const int* pairs;            // sorted (i, j) list of the last encounter pass
     const uint8_t* flag;         // 1 for every endpoint
-    const DevStats* st;          // nce_last
+    DevStats* st;                // nce_last; resolve_fail (cumulative)
     int* loc;                    // nb scratch: body -> index in its component
     int* label;                  // nb scratch: smallest body of the component (valid for flagged bodies)
     int* roots; int* nroots;     // the components' smallest bodies
@@ -82,7 +82,7 @@ __global__ void __launch_bounds__(RES_NMAX) resolve_label_kernel(ResParams p) {
     if (tid == 0) { *p.out = ResStats{0, 0, 0, 0}; *p.nroots = 0; }
     const long long nce = p.st->nce_last;
     if (nce <= 0) return;
-    if (nce > p.cap) { if (tid == 0) p.out->fail = 1 << 30; return; }      // truncated list: nothing can be resolved
+    if (nce > p.cap) { if (tid == 0) { p.out->fail = 1 << 30; atomicAdd(&p.st->resolve_fail, 1); } return; }      // truncated list: nothing can be resolved
     const int np = (int)nce;
     volatile int* label = p.label;
     for (int q = tid; q < np; q += RES_NMAX) { label[p.pairs[2 * q]] = p.pairs[2 * q]; label[p.pairs[2 * q + 1]] = p.pairs[2 * q + 1]; }
@@ -148,7 +148,7 @@ __global__ void __launch_bounds__(NT) resolve_kernel(ResParams p) {
         np += tot;
     }
     if (np <= PLO || np > PHI || p.done[comp]) continue;               // another instance's component
-    if (np > RES_PMAX) { if (LAST && tid == 0) atomicAdd(&p.out->fail, 1); continue; }
+    if (np > RES_PMAX) { if (LAST && tid == 0) { atomicAdd(&p.out->fail, 1); atomicAdd(&p.st->resolve_fail, 1); } continue; }
     // ---- its bodies in ascending order (thread t scans its own segment of the flags) ----
     // (segments of a multiple of 8 bodies: the flags are read eight at a time where the array is 8-byte aligned -
     // at 1e6 bodies almost all of them are 0)
@@ -169,7 +169,7 @@ __global__ void __launch_bounds__(NT) resolve_kernel(ResParams p) {
                 if (p.flag[b] && p.label[b] == root) { p.loc[b] = k; sJstart[k] = b; ++k; }   // sJstart doubles as the body list
     }
     if (n > NT) {
-        if (LAST && tid == 0) { atomicAdd(&p.out->fail, 1); atomicAdd(&p.out->bodies, n); }
+        if (LAST && tid == 0) { atomicAdd(&p.out->fail, 1); atomicAdd(&p.st->resolve_fail, 1); atomicAdd(&p.out->bodies, n); }
         continue;                                                      // not LAST: a later, wider instance takes it
     }
     if (tid == 0) p.done[comp] = 1;
@@ -368,7 +368,7 @@ __global__ void __launch_bounds__(NT) resolve_kernel(ResParams p) {
     }
     if (tid == 0) {
         atomicAdd(&p.out->bodies, n); atomicAdd(&p.out->steps, nacc); atomicAdd(&p.out->rhs, nrhs);
-        if (fail) atomicAdd(&p.out->fail, 1);
+        if (fail) { atomicAdd(&p.out->fail, 1); atomicAdd(&p.st->resolve_fail, 1); }
     }
     }   // components
 }

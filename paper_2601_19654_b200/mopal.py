@@ -15,19 +15,20 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libmopal.so")
 
-MO_OK, MO_EINVAL, MO_ENOMEM, MO_ECUDA, MO_EOVERFLOW, MO_ENOCONV = range(6)
+MO_OK, MO_EINVAL, MO_ENOMEM, MO_ECUDA, MO_EOVERFLOW, MO_ENOCONV, MO_ERESOLVE = range(7)
+_SOFT = (MO_OK, MO_EOVERFLOW, MO_ENOCONV, MO_ERESOLVE)      # statuses reported in Stats.status instead of raised
 
 EXPORTS = ["mo_create", "mo_accel", "mo_drift", "mo_encounters", "mo_step", "mo_destroy",
            "mo_snapshot", "mo_snapshot_ptrs", "mo_snapshot_copy", "mo_invalidate_accel", "mo_get_stats", "mo_launch_count",
            "mo_workspace_bytes", "mo_step_host", "mo_accel_host", "mo_probe_fp64_peak",
            "mo_pair_geometry", "mo_set_kernel_timing", "mo_pair_kernel_ms", "mo_strerror", "mo_version",
            "mo_set_nbig", "mo_pair_kernel_name", "mo_h2dh", "mo_dh2h", "mo_hill", "mo_set_hill", "mo_energy",
-           "mo_resolve", "mo_set_resolve", "mo_resolve_stats"]
+           "mo_resolve", "mo_set_resolve", "mo_resolve_stats", "mo_boxes_copy"]
 
 
 class MoStats(C.Structure):
     _fields_ = [("steps_done", C.c_int64), ("nce_last", C.c_int64), ("nce_total", C.c_int64),
-                ("drift_fail", C.c_int32), ("max_newton", C.c_int32)]
+                ("drift_fail", C.c_int32), ("max_newton", C.c_int32), ("resolve_fail", C.c_int32), ("reserved", C.c_int32)]
 
 
 class MoEnergy(C.Structure):
@@ -65,6 +66,7 @@ def load():
     L.mo_snapshot_ptrs.restype = C.c_int; L.mo_snapshot_ptrs.argtypes = [vp, C.POINTER(vp), C.POINTER(vp)]
     L.mo_snapshot_copy.restype = C.c_int; L.mo_snapshot_copy.argtypes = [vp, vp, vp]
     L.mo_invalidate_accel.restype = C.c_int; L.mo_invalidate_accel.argtypes = [vp]
+    L.mo_boxes_copy.restype = C.c_int; L.mo_boxes_copy.argtypes = [vp, vp]
     L.mo_set_nbig.restype = C.c_int; L.mo_set_nbig.argtypes = [vp, I32]
     L.mo_pair_kernel_name.restype = C.c_char_p; L.mo_pair_kernel_name.argtypes = [vp]
     L.mo_h2dh.restype = C.c_int; L.mo_h2dh.argtypes = [vp]
@@ -122,11 +124,13 @@ class Stats:
     nce_total: int
     drift_fail: int
     max_newton: int
+    resolve_fail: int = 0
     status: int = MO_OK
 
 
 def _stats(s: MoStats, status=MO_OK) -> Stats:
-    return Stats(int(s.steps_done), int(s.nce_last), int(s.nce_total), int(s.drift_fail), int(s.max_newton), int(status))
+    return Stats(int(s.steps_done), int(s.nce_last), int(s.nce_total), int(s.drift_fail), int(s.max_newton),
+                 int(s.resolve_fail), int(status))
 
 
 class Mopal:
@@ -198,7 +202,7 @@ class Mopal:
             return None
         s = MoStats()
         st = self._L.mo_step(self._ctx, float(dt), int(nsteps), C.byref(s))
-        if st not in (MO_OK, MO_EOVERFLOW, MO_ENOCONV):
+        if st not in _SOFT:
             raise MopalError(st, "mo_step")
         return _stats(s, st)
 
@@ -221,6 +225,14 @@ class Mopal:
         self._check(self._L.mo_snapshot_copy(self._ctx, x0.data_ptr(), v0.data_ptr()), "mo_snapshot_copy")
         self.stream.synchronize()
         return x0, v0
+
+    def boxes(self):
+        """(lo[2, nb], hi[2, nb]) numpy: the x and y boxes of the last encounter pass (mce_snif LOOP 1-2)."""
+        t = self._torch.empty((self.nb, 4), dtype=self._torch.float64, device=self.device)
+        self._check(self._L.mo_boxes_copy(self._ctx, t.data_ptr()), "mo_boxes_copy")
+        self.stream.synchronize()
+        b = t.cpu().numpy()
+        return np.stack([b[:, 0], b[:, 2]]), np.stack([b[:, 1], b[:, 3]])
 
     def set_nbig(self, nbig):
         """Bodies 0..nbig-1 are the big bodies: the only gravity sources and first members of
@@ -273,7 +285,7 @@ class Mopal:
     def stats(self) -> Stats:
         s = MoStats()
         st = self._L.mo_get_stats(self._ctx, C.byref(s))
-        if st not in (MO_OK, MO_EOVERFLOW, MO_ENOCONV):
+        if st not in _SOFT:
             raise MopalError(st, "mo_get_stats")
         return _stats(s, st)
 
@@ -306,7 +318,7 @@ class Mopal:
         cap_h = 0 if pairs_host is None else int(pairs_host.shape[0])
         st = self._L.mo_step_host(self._ctx, float(dt), int(nsteps), _hptr(x_host), _hptr(v_host),
                                   _hptr(rcrit_host), 1 if a_is_current else 0, _hptr(pairs_host), cap_h, C.byref(s))
-        if st not in (MO_OK, MO_EOVERFLOW, MO_ENOCONV):
+        if st not in _SOFT:
             raise MopalError(st, "mo_step_host")
         return _stats(s, st)
 
@@ -327,6 +339,9 @@ class Mopal:
         return t.cpu().numpy()
 
     def set(self, name, arr):
+        """Overwrite a state array from numpy; changing x or rcrit invalidates the cached accelerations."""
+        if name in ("x", "rcrit"):
+            self.invalidate_accel()
         t = getattr(self, name)
         src = self._torch.from_numpy(np.ascontiguousarray(arr)).to(self.device)
         if t.dim() == 2 and t.shape[1] == self.ld:

@@ -62,17 +62,17 @@ def test_accel_full_configs(M, cfg):
 
 
 @pytest.mark.parametrize("cfg", [3, 4])
-def test_accel_headline_sizes_sampled_rows(M, cfg):
-    """full-size launch configuration (the one bench.py times); oracle on sampled bodies."""
+def test_accel_headline_sizes_every_row(M, cfg):
+    """full-size launch configuration (the one bench.py times) against the oracle on EVERY row
+    (4 s / 18 s of oracle time on the GPU box's host cores)."""
     w = W.make_config(cfg)
     m = _mk(M, w)
+    assert m.pair_kernel_name() == "pair_sym_kernel"
     m.accel()
     a = m.get("a")
-    rng = np.random.default_rng(cfg)
-    rows = np.unique(np.concatenate([np.arange(8), [w.nb - 1, w.nb - 2, 127, 128, 255, 256],
-                                     rng.integers(0, w.nb, 48)])).astype(np.int32)
-    a_ref, S = oracle.accel_rows(G * w.mass, w.x, w.rcrit, rows)
-    _check_accel(a[:, rows], a_ref, S, w.name)
+    a_ref, S = oracle.accel(G * w.mass, w.x, w.rcrit)
+    worst = _check_accel(a, a_ref, S, w.name)
+    assert worst < 2e-13
     # property at any size: Newton III with the symmetric K
     for c in range(3):
         assert abs(np.sum(w.mass * a[c])) <= 1e-11 * np.sum(w.mass * np.abs(a[c]))
@@ -257,24 +257,101 @@ def test_encounters_full_configs(M, cfg, scale):
     m.close()
 
 
-@pytest.mark.parametrize("cfg,stride", [(3, 97), (4, 193)])
-def test_encounters_headline_sizes_sampled_rows(M, cfg, stride):
+@pytest.mark.parametrize("cfg", [3, 4])
+def test_encounters_headline_sizes_whole_list(M, cfg):
+    """the WHOLE list at full size against the oracle's - the giants' rows 0..3 of cfg3 (thousands of hits each:
+    the long-row ranking path of enc_rank_kernel) and the dense load of cfg4 included."""
     w = W.make_config(cfg)
     x1, v1 = _enc_inputs(w)
+    ref = oracle.encounters(w.dt, w.x, w.v, x1, v1, w.rcrit, cap=1 << 20)
     m = _mk(M, w)
     m.snapshot()
     m.set("x", x1); m.set("v", v1)
     cnt = m.encounters(w.dt)
     got = m.pair_list(cnt)
     assert cnt == len(got) > 0
+    n_amb = _pairs_ok(got, ref)
+    if n_amb == 0:
+        assert cnt == ref["count"] and np.array_equal(got, ref["pairs"])
+        assert np.array_equal(m.get("flag"), ref["flag"])
     assert got.tolist() == sorted(got.tolist()) and np.all(got[:, 0] < got[:, 1])
-    fl = np.zeros(w.nb, dtype=np.uint8); fl[got.ravel()] = 1
-    assert np.array_equal(fl, m.get("flag"))
-    # rows 0..7 hold the giants (most pairs) - take them plus a strided sample
-    for phase_rows, kw in [(got[got[:, 0] % stride == 5], dict(row_stride=stride, row_phase=5))]:
-        ref = oracle.encounters(w.dt, w.x, w.v, x1, v1, w.rcrit, **kw)
-        _pairs_ok(phase_rows, ref)
+    if cfg == 3:      # the giants' rows are long rows (> 64 hits: the CTA ranking path)
+        assert min(np.sum(ref["pairs"][:, 0] == g) for g in range(2)) > 64
     m.close()
+
+
+def _check_boxes(m, h, x0, v0, x1, v1, rcrit, nbig=None):
+    """a7 directly: the library's boxes against oracle.boxes.  Both sides evaluate B-1 in the same operation
+    order, so the plain-double build of the oracle must agree to the last bit and the long-double parity build to
+    a few ulp of the box scale (measured between the two oracle builds: <= 7e-16)."""
+    lo, hi = m.boxes()
+    rl, rh = oracle.boxes(h, x0, v0, x1, v1, rcrit, nbig=nbig)
+    sc = np.maximum(np.maximum(np.abs(rl), np.abs(rh)), 1e-300)
+    assert np.max(np.abs(lo - rl) / sc) <= 4e-15 and np.max(np.abs(hi - rh) / sc) <= 4e-15
+    dl, dh = oracle.boxes(h, x0, v0, x1, v1, rcrit, nbig=nbig, kind="f64")
+    assert np.array_equal(lo, dl) and np.array_equal(hi, dh)
+    return lo, hi
+
+
+@pytest.mark.parametrize("cfg", [0, 1, 2, 3, 4])
+def test_boxes_all_configs(M, cfg):
+    """mce_snif LOOP 1-2 on every body of the five configs, stand-alone and inside mo_step."""
+    w = W.make_config(cfg)
+    x1, v1 = _enc_inputs(w)
+    m = _mk(M, w)
+    with pytest.raises(M.MopalError):
+        m.boxes()                                  # no encounter pass yet
+    m.snapshot(); m.set("x", x1); m.set("v", v1)
+    m.encounters(w.dt)
+    lo, hi = _check_boxes(m, w.dt, w.x, w.v, x1, v1, w.rcrit)
+    turning = (w.v[:2] * v1[:2] < 0)
+    assert turning.sum() >= 4                      # the interior-extremum branch is exercised
+    ends_lo = np.minimum(w.x[:2], x1[:2]) - w.rcrit
+    assert (lo[turning] < ends_lo[turning]).any() or (hi[turning] > (np.maximum(w.x[:2], x1[:2]) + w.rcrit)[turning]).any()
+    # inside the step: the boxes are those of (x0, v0) -> drifted (x, v) of that step
+    m.set("x", w.x); m.set("v", w.v)
+    m.step(w.dt, 1)
+    x0t, v0t = m.snapshot_tensors()
+    x0, v0 = x0t[:, :w.nb].cpu().numpy(), v0t[:, :w.nb].cpu().numpy()
+    xd, vd, _ = oracle.drift(G * w.m_star, w.dt, x0, v0)
+    lo, hi = m.boxes()
+    rl, rh = oracle.boxes(w.dt, x0, v0, xd, vd, w.rcrit)
+    sc = np.maximum(np.abs(rl), np.abs(rh))
+    assert np.max(np.abs(lo - rl) / sc) <= 1e-12 and np.max(np.abs(hi - rh) / sc) <= 1e-12   # drifted state to 1e-13
+    m.close()
+
+
+@pytest.mark.parametrize("nbig", [None, 37])
+def test_boxes_planted_turning_points(M, nbig):
+    """every branch of B-1 on planted (p0, w0) -> (p1, w1): one or two interior extrema, D < 0, k3 = 0 exactly,
+    a root at the end of the interval, negative h; with nbig < nb only the big bodies' boxes are padded (R-2)."""
+    import torch
+    rng = np.random.default_rng(7)
+    nb = 1200
+    x0 = rng.uniform(-5, 5, (3, nb)); x1 = x0 + rng.normal(0, 0.05, (3, nb))
+    v0 = rng.normal(0, 0.02, (3, nb)); v1 = v0.copy()
+    v1[:2, ::2] = -v0[:2, ::2] * rng.uniform(0.2, 3.0, (2, nb // 2))          # turning points in x and y
+    v1[:2, 1::4] = v0[:2, 1::4] * rng.uniform(0.2, 3.0, (2, nb // 4))          # same sign: endpoints only
+    # k3 = 2 p0 + h w0 - 2 p1 + h w1 = 0 exactly: p1 = p0 + h (w0 + w1) / 2 with exactly representable numbers
+    h = 4.0
+    x0[0, :8] = [0.5, -1.25, 2.0, 3.5, -0.75, 1.0, 4.0, -2.5]; v0[0, :8] = 0.125; v1[0, :8] = -0.0625
+    x1[0, :8] = x0[0, :8] + h * (0.125 - 0.0625) / 2
+    x1[1, 8:16] = x0[1, 8:16]; v0[1, 8:16] = 0.25; v1[1, 8:16] = -0.25         # symmetric: extremum at tau = 1/2
+    x1[0, 16:24] = x0[0, 16:24] + 10.0; v0[0, 16:24] = 1e-3; v1[0, 16:24] = -1e-3   # big jump: roots outside (0,1) or D < 0
+    rc = rng.uniform(0.0, 0.3, nb)
+    for hh in (h, -h):
+        m = M.Mopal(np.full(nb, 1e-9), x1, v1, rc)
+        if nbig is not None:
+            m.set_nbig(nbig)
+        X0 = torch.zeros_like(m.x); V0 = torch.zeros_like(m.v)
+        X0[:, :nb] = torch.from_numpy(x0).cuda(); V0[:, :nb] = torch.from_numpy(v0).cuda()
+        m.encounters(hh, X0, V0)
+        lo, hi = _check_boxes(m, hh, x0, v0, x1, v1, rc, nbig=nbig)
+        if nbig is not None:       # small bodies: no pad
+            assert np.all(lo[:, nbig:] <= np.minimum(x0[:2], x1[:2])[:, nbig:])
+            same = v0[:2, nbig:] * v1[:2, nbig:] >= 0
+            assert np.array_equal(lo[:, nbig:][same], np.minimum(x0[:2], x1[:2])[:, nbig:][same])
+        m.close()
 
 
 def test_encounters_overflow_and_edges(M):
@@ -351,6 +428,7 @@ def test_step_vs_oracle(M, cfg, nsteps):
         # the snapshot is the oracle's x0, v0
         x0, v0 = m.snapshot_tensors()
         assert _rel_vec_err(x0[:, :w.nb].cpu().numpy(), r["x0"]).max() <= tol
+        assert _rel_vec_err(v0[:, :w.nb].cpu().numpy(), r["v0"]).max() <= tol
     m.close()
 
 
@@ -382,22 +460,38 @@ def test_step_nb1_and_reversibility(M):
     m.close()
 
 
-@pytest.mark.parametrize("cfg,nsteps", [(3, 3), (4, 2)])
-def test_step_headline_sizes_properties(M, cfg, nsteps):
-    """full sizes: properties that hold at any size + sampled oracle rows on the final state."""
+@pytest.mark.parametrize("cfg", [3, 4])
+def test_step_headline_sizes_vs_oracle(M, cfg):
+    """P-S1 at full size: one mo_step against oracle.step - x, v, the snapshot x0 AND v0, the pair list and flags,
+    and the closing accelerations on every row (against the oracle's sum at the stepped positions)."""
     w = W.make_config(cfg)
+    gm, mu = G * w.mass, G * w.m_star
+    a0, _ = oracle.accel(gm, w.x, w.rcrit)
+    r = oracle.step(mu, gm, w.rcrit, w.dt, w.x, w.v, a0, cap=1 << 20)
+    assert r["nfail"] == 0
     m = _mk(M, w)
     L0 = (w.mass * np.cross(w.x.T, w.v.T).T).sum(1)
-    st = m.step(w.dt, nsteps)
-    assert st.steps_done == nsteps and st.drift_fail == 0
+    st = m.step(w.dt, 1)
+    assert st.steps_done == 1 and st.drift_fail == 0
     x, v, a = m.get("x"), m.get("v"), m.get("a")
+    assert _rel_vec_err(x, r["x"]).max() <= 1e-13 and _rel_vec_err(v, r["v"]).max() <= 1e-13
+    x0, v0 = m.snapshot_tensors()
+    assert _rel_vec_err(x0[:, :w.nb].cpu().numpy(), r["x0"]).max() <= 1e-13
+    assert _rel_vec_err(v0[:, :w.nb].cpu().numpy(), r["v0"]).max() <= 1e-13
+    got = m.pair_list(st.nce_last)
+    n_amb = _pairs_ok(got, r)
+    if n_amb == 0:
+        assert st.nce_last == r["count"] and np.array_equal(got, r["pairs"]) and np.array_equal(m.get("flag"), r["flag"])
+    # a is current for the GPU's x: the oracle's sum at those positions, every row
+    a_ref, S = oracle.accel(gm, x, w.rcrit)
+    _check_accel(a, a_ref, S, w.name + " after the step")
     L1 = (w.mass * np.cross(x.T, v.T).T).sum(1)
     assert np.linalg.norm(L1 - L0) <= 1e-13 * np.linalg.norm(L0)       # P-S2
-    rows = np.unique(np.random.default_rng(1).integers(0, w.nb, 24)).astype(np.int32)
-    a_ref, S = oracle.accel_rows(G * w.mass, x, w.rcrit, rows)          # a is current for x
-    _check_accel(a[:, rows], a_ref, S)
-    got = m.pair_list(st.nce_last)
-    assert len(got) == st.nce_last and got.tolist() == sorted(got.tolist())
+    # two more steps through the graph path: invariants only (P-S6)
+    st = m.step(w.dt, 2)
+    x, v = m.get("x"), m.get("v")
+    L2 = (w.mass * np.cross(x.T, v.T).T).sum(1)
+    assert st.steps_done == 3 and np.linalg.norm(L2 - L0) <= 1e-13 * np.linalg.norm(L0)
     m.close()
 
 
@@ -738,6 +832,7 @@ def test_step_small_path_vs_oracle(M, monkeypatch, cfg, N, nbig, hill):
         seen += st.nce_last
         x0, v0 = m.snapshot_tensors()
         assert _rel_vec_err(x0[:, :w.nb].cpu().numpy(), r["x0"]).max() <= tol
+        assert _rel_vec_err(v0[:, :w.nb].cpu().numpy(), r["v0"]).max() <= tol
     assert seen > 0 or cfg == 2
     m2 = _mk(M, w, rcrit=rc0)                       # graph replay gives the same trajectory
     if nbig is not None:

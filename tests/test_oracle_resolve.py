@@ -135,3 +135,72 @@ def test_X4_the_resolved_hybrid_step_keeps_the_energy_through_a_close_encounter(
     eb = abs(oracle.energy(G, M, mass, xb, vb)["E"] - E0) / abs(E0)
     assert nres >= 20
     assert ea < 1e-7 and eb > 100 * ea, (ea, eb)
+
+
+def _multi_component_system():
+    """star + seven massive bodies forming THREE encounter components whose members interleave in body order:
+    pair A = (0, 3) at 1 AU, pair B = (1, 5) at 1.6 AU, chain C = (2, 4), (4, 6) at 2.3 AU; + 2 bystanders.
+    The sorted list (0,3), (1,5), (2,4), (4,6) alternates between the components."""
+    M = 1.0
+    sepA, sepB, sepC = 0.006, 0.004, 0.005
+    a = np.empty(9); Man = np.empty(9)
+    a[[0, 3]] = [1.0, 1.0 + 0.6 * sepA]; Man[[0, 3]] = [0.3, 0.3 + 0.8 * sepA]
+    a[[1, 5]] = [1.6, 1.6 + 0.6 * sepB]; Man[[1, 5]] = [2.1, 2.1 + 0.8 * sepB / 1.6]
+    a[[2, 4, 6]] = [2.3, 2.3 + 0.6 * sepC, 2.3 + 1.2 * sepC]; Man[[2, 4, 6]] = [4.0, 4.0 + 0.8 * sepC / 2.3, 4.0 + 1.7 * sepC / 2.3]
+    a[7:] = [3.1, 3.7]; Man[7:] = [1.0, 5.0]
+    e = np.array([0.01, 0.02, 0.015, 0.012, 0.018, 0.022, 0.013, 0.05, 0.05])
+    inc = np.array([0.001, 0.003, 0.002, 0.002, 0.001, 0.004, 0.003, 0.01, 0.01])
+    z = np.zeros(9)
+    mass = np.array([1e-5, 2e-5, 1.5e-5, 1.2e-5, 0.8e-5, 1e-5, 2.5e-5, 1e-7, 1e-7])
+    x, vh = W.elements_to_state(G * (M + mass), a, e, inc, z, z, Man)
+    v = oracle.h2dh(M, mass, vh)
+    _, rc = oracle.hill(G, M, mass, x, v, n_hill=3.0)
+    pairs = np.array([[0, 3], [1, 5], [2, 4], [4, 6]], dtype=np.int32)
+    return M, mass, x, v, rc, pairs
+
+
+@pytest.mark.parametrize("h", [2.0, -1.5])
+def test_X1_several_interacting_components_against_dop853_on_the_union_system(h):
+    """Pins the union-find split of oracle_resolve (reading X-1): three components with non-zero masses, interleaved
+    in the list, against ONE DOP853 integration of all listed bodies under all listed pairs (the paper's single call
+    for 'the bodies involved in the close encounter', PAPER.md:104 fn. 14).  A pair put into the wrong component, or
+    dropped, changes the states by ~1e-6, nine orders above the tolerance."""
+    M, mass, x, v, rc, pairs = _multi_component_system()
+    mu, gm = G * M, G * mass
+    idx = np.unique(pairs)
+    loc = {b: k for k, b in enumerate(idx)}
+    n = len(idx)
+    # every listed pair is inside its changeover shell: the encounter terms are really there
+    for i, j in pairs:
+        r = np.linalg.norm(x[:, j] - x[:, i])
+        assert oracle.changeover(r, max(rc[i], rc[j])) < 0.9
+
+    def rhs(t, y):
+        X = y[:3 * n].reshape(n, 3); V = y[3 * n:].reshape(n, 3)
+        A = -mu * X / np.linalg.norm(X, axis=1)[:, None] ** 3
+        for i, j in pairs:
+            d = X[loc[j]] - X[loc[i]]
+            r = np.linalg.norm(d)
+            u = (1.0 - oracle.changeover(r, max(rc[i], rc[j]))) / r**3
+            A[loc[i]] += gm[j] * u * d
+            A[loc[j]] -= gm[i] * u * d
+        return np.concatenate([V.ravel(), A.ravel()])
+
+    y0 = np.concatenate([x[:, idx].T.ravel(), v[:, idx].T.ravel()])
+    sol = solve_ivp(rhs, (0.0, h), y0, method="DOP853", rtol=1e-13, atol=1e-18)
+    assert sol.success
+    xr = sol.y[:3 * n, -1].reshape(n, 3).T; vr = sol.y[3 * n:, -1].reshape(n, 3).T
+    x1, v1, _ = oracle.drift(mu, h, x, v)
+    r = oracle.resolve(mu, gm, rc, h, x, v, x1, v1, pairs, tol=1e-13)
+    assert r["fail"] == 0 and r["n"] == n
+    assert _relv(r["x"][:, idx], xr) <= 2e-11 and _relv(r["v"][:, idx], vr) <= 2e-11
+    # every one of the seven bodies felt its encounter (none was left to the drift by a wrong split) ...
+    for b in idx:
+        assert np.linalg.norm(r["v"][:, b] - v1[:, b]) / np.linalg.norm(v1[:, b]) > 1e-8, b
+    # ... the bystanders did not move off the drift, and the list order does not matter
+    assert np.array_equal(r["x"][:, 7:], x1[:, 7:]) and np.array_equal(r["v"][:, 7:], v1[:, 7:])
+    g = oracle.resolve(mu, gm, rc, h, x, v, x1, v1, pairs[[2, 0, 3, 1]].copy(), tol=1e-13)
+    assert _relv(g["x"][:, idx], r["x"][:, idx]) <= 1e-13 and _relv(g["v"][:, idx], r["v"][:, idx]) <= 1e-13
+    # dropping the chain's second pair (what a wrong split would amount to for body 6) is far outside the tolerance
+    bad = oracle.resolve(mu, gm, rc, h, x, v, x1, v1, pairs[:3].copy(), tol=1e-13)
+    assert np.linalg.norm(bad["v"][:, 4] - r["v"][:, 4]) / np.linalg.norm(r["v"][:, 4]) > 1e-9

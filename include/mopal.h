@@ -166,19 +166,24 @@ mo_status mo_energy(mo_ctx *ctx, mo_energy_t *out_host);
 /* ---- close-encounter resolution on the device (the paper's host-side mdt_hkce, PAPER.md:104 fn. 14,
  * 126, 297-315; readings X-1..X-5) -------------------------------------------------------------
  * The bodies of the current encounter pair list (the last mo_encounters / mo_step) are restored to the
- * snapshot x0, v0 and integrated over dt as one system with a Bulirsch-Stoer scheme to relative
- * tolerance tol, under the star's Kepler term and the (1 - K)-weighted forces of the listed pairs - the
- * complement of the K-weighted kick; x, v of those bodies (which must hold the Kepler-drift result of the
- * other bodies) are overwritten.  Each connected component of the pair graph is its own system with its
- * own step control.  Limits of this version: 1024 bodies and 2048 pairs per component; beyond, or without
- * convergence, the component's bodies keep the drift result and it is counted in mo_resolve_stats.
+ * snapshot x0, v0 and integrated over dt with a Bulirsch-Stoer scheme (modified midpoint, 2..16 substeps,
+ * polynomial extrapolation) whose local error stays below tol relative to |x_i|, |v_i| of every body, under
+ * the star's Kepler term and the (1 - K)-weighted forces of the listed pairs - the complement of the
+ * K-weighted kick; x, v of those bodies (which must hold the Kepler-drift result of the other bodies) are
+ * overwritten.  Each connected component of the pair graph is its own system with its own step control; a
+ * massless body (mass 0: the test particles of the big x all regime) exerts no force and is integrated in a
+ * small system of its own with its massive partners.  Components of any size are resolved (up to 1023 pairs
+ * in shared memory, one thread per body; larger ones streamed through global scratch).  Without convergence
+ * (40 rejected steps in a row), or when the pair list was truncated (count > cap), the bodies keep the
+ * Kepler-drift result, the component is counted in mo_resolve_stats / mo_stats.resolve_fail and the next
+ * synchronising call returns MO_ERESOLVE.  The result is deterministic (fixed summation orders).
  * Asynchronous.  MO_EINVAL: tol <= 0, dt == 0, no snapshot. */
 mo_status mo_resolve(mo_ctx *ctx, double dt, double tol);
 /* Make mo_step resolve the encounters of every step (between the encounter check and the second jump,
  * PAPER.md:297-315); tol <= 0 switches it off (the default).  Drops the cached step graph. */
 mo_status mo_set_resolve(mo_ctx *ctx, double tol);
-/* Last resolution: out4 = {bodies in all components, accepted BS steps and right-hand-side evaluations
- * summed over the components, components not resolved}.  Synchronises. */
+/* Last resolution: out4 = {bodies integrated and written back, accepted BS steps and right-hand-side
+ * evaluations summed over the systems, systems not resolved}.  Synchronises. */
 mo_status mo_resolve_stats(mo_ctx *ctx, int32_t *out4);
 
 /* Copy the current x, v into the context's x0, v0 snapshot (asynchronous). */

@@ -47,9 +47,13 @@ struct mo_ctx {
     int en_npair = 0, en_split = 1;
     double res_tol = 0.0;               // mo_set_resolve: <= 0 off
     int* res_loc = nullptr;             // nb ints (lazy)
-    double* res_tab = nullptr;          // extrapolation tableaux, one set per CTA
-    int *res_label = nullptr, *res_roots = nullptr, *res_nroots = nullptr, *res_done = nullptr;
-    int res_grid = 1;
+    double* res_tab = nullptr;          // extrapolation tableaux of the class-C CTAs (fallback when shared memory is short)
+    int *res_label = nullptr, *res_cnp = nullptr, *res_cstart = nullptr, *res_cfill = nullptr, *res_cq = nullptr;
+    int *res_clist = nullptr, *res_ctl = nullptr, *res_aux = nullptr, *res_cown = nullptr;
+    double *res_dbody = nullptr, *res_dpair = nullptr;   // class D (components of more than 1023 pairs): state pools
+    int *res_dbodyi = nullptr, *res_dpairi = nullptr;
+    long long res_dbodyN = 0;
+    int res_smemA = 0, res_smemB = 0, res_smemC = 0;
     ResStats* res_out = nullptr;        // device
     ResStats* res_host = nullptr;       // pinned
     int hill_mode = -1;                 // mo_set_hill: -1 off
@@ -246,7 +250,9 @@ extern "C" void mo_destroy(mo_ctx* ctx) {
     for (cudaEvent_t e : ctx->ev) cudaEventDestroy(e);
     cudaFree(ctx->gm); cudaFree(ctx->x0); cudaFree(ctx->v0); cudaFree(ctx->part);
     cudaFree(ctx->psumA); cudaFree(ctx->psumB); cudaFree(ctx->ticket);
-    cudaFree(ctx->res_loc); cudaFree(ctx->res_out); cudaFree(ctx->res_tab); cudaFree(ctx->res_label); cudaFree(ctx->res_roots); cudaFree(ctx->res_nroots); cudaFree(ctx->res_done);
+    cudaFree(ctx->res_loc); cudaFree(ctx->res_out); cudaFree(ctx->res_tab); cudaFree(ctx->res_label);
+    cudaFree(ctx->res_cnp); cudaFree(ctx->res_cstart); cudaFree(ctx->res_cfill); cudaFree(ctx->res_cq); cudaFree(ctx->res_clist); cudaFree(ctx->res_ctl); cudaFree(ctx->res_aux); cudaFree(ctx->res_cown);
+    cudaFree(ctx->res_dbody); cudaFree(ctx->res_dpair); cudaFree(ctx->res_dbodyi); cudaFree(ctx->res_dpairi);
     if (ctx->res_host) cudaFreeHost(ctx->res_host);
     cudaFree(ctx->gmsum); cudaFree(ctx->en_on); cudaFree(ctx->en_pair); cudaFree(ctx->en_out);
     if (ctx->en_host) cudaFreeHost(ctx->en_host); cudaFree(ctx->tiles);
@@ -525,20 +531,41 @@ static mo_status enqueue_hill(mo_ctx* ctx, double n_hill, int mode, double* rhil
     return post_launch(ctx);
 }
 
+// grids of the resolve kernels: class 0 (components of up to 63 pairs, 64 threads: several CTAs per SM), the larger
+// classes hold few components (the stars around the big bodies): small grids, cheap to launch when they have nothing to do
+static constexpr int RES_GRID_0_PER_SM = 6, RES_GRID_1 = 74, RES_GRID_2 = 32, RES_GRID_3 = 16, RES_GRID_4 = 16;
+
 static mo_status ensure_resolve_scratch(mo_ctx* ctx) {
     if (ctx->res_loc) return MO_OK;
+    const size_t capn = (size_t)(ctx->cap > 0 ? ctx->cap : 1);
     cudaError_t e = dalloc(ctx, &ctx->res_loc, (size_t)ctx->nb);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_out, 1);
-    ctx->res_grid = ctx->nsm;
-    if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_tab, (size_t)6 * RES_KMAX * RES_NMAX * ctx->res_grid);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_label, (size_t)ctx->nb);
-    if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_roots, (size_t)(ctx->cap > 0 ? ctx->cap : 1));
-    if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_nroots, 1);
-    if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_done, (size_t)(ctx->cap > 0 ? ctx->cap : 1));
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(resolve_kernel<64, 0, 32, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, RES_DYN_SMEM + 6 * RES_KMAX * 64 * 8);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(resolve_kernel<256, 32, 128, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, RES_DYN_SMEM + 6 * RES_KMAX * 256 * 8);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(resolve_kernel<512, 128, 1 << 30, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, RES_DYN_SMEM);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(resolve_kernel<RES_NMAX, 128, 1 << 30, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, RES_DYN_SMEM);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_aux, (size_t)ctx->nb);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_cown, capn);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_cnp, capn);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_cstart, capn);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_cfill, capn);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_cq, capn);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_clist, capn * RES_NCLS);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_ctl, 16);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_tab, (size_t)6 * RES_KMAX * 1024 * RES_GRID_2);   // classes 2 and 3 (they run one after the other)
+    // class D pools: every body and every pair of the list can be in a class-D component
+    ctx->res_dbodyN = (long long)ctx->nb < 2 * (long long)capn ? (long long)ctx->nb : 2 * (long long)capn;
+    if (ctx->cap > RES_PHI_3) {          // a shorter list cannot hold a class-D component
+        if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_dbody, (size_t)ctx->res_dbodyN * RES_D_BODY_PLANES);
+        if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_dbodyi, (size_t)ctx->res_dbodyN * RES_D_BODY_IPLANES);
+        if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_dpair, capn * RES_D_PAIR_PLANES);
+        if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_dpairi, capn * RES_D_PAIR_IPLANES);
+    }
+    // dynamic shared memory: 86 B per pair + 24 B per 32 pairs, 129 B per body, 6 * RES_KMAX doubles per body of tableau
+    ctx->res_smemA = 88 * 64 + (132 + 6 * RES_KMAX * 8) * 64;
+    ctx->res_smemB = 88 * 256 + (132 + 6 * RES_KMAX * 8) * 256;
+    ctx->res_smemC = 227 * 1024 - 2048;                              // classes 2, 3: all there is (minus the static part)
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(resolve_solve_kernel<64, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->res_smemA);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(resolve_solve_kernel<256, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->res_smemB);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(resolve_solve_kernel<512, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->res_smemC);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(resolve_solve_kernel<1024, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->res_smemC);
     if (e == cudaSuccess) e = cudaMemsetAsync(ctx->res_out, 0, sizeof(ResStats), ctx->stream);
     if (e == cudaSuccess) e = cudaMallocHost(reinterpret_cast<void**>(&ctx->res_host), sizeof(ResStats));
     if (e != cudaSuccess) { cudaGetLastError(); ctx->last_err = e; return e == cudaErrorMemoryAllocation ? MO_ENOMEM : MO_ECUDA; }
@@ -548,21 +575,30 @@ static mo_status ensure_resolve_scratch(mo_ctx* ctx) {
 static mo_status enqueue_resolve(mo_ctx* ctx, double dt, double tol) {
     ResParams rp;
     rp.x0 = ctx->x0; rp.v0 = ctx->v0; rp.x = ctx->x; rp.v = ctx->v; rp.gm = ctx->gm; rp.rcrit = ctx->rcrit;
-    rp.pairs = ctx->pairs; rp.flag = ctx->flag; rp.st = ctx->dstats; rp.loc = ctx->res_loc; rp.tab = ctx->res_tab; rp.label = ctx->res_label; rp.roots = ctx->res_roots; rp.nroots = ctx->res_nroots; rp.done = ctx->res_done; rp.out = ctx->res_out;
-    rp.cap = ctx->cap; rp.nb = ctx->nb; rp.ld = ctx->ld; rp.mu = ctx->mu; rp.h = dt; rp.tol = tol;
-    resolve_label_kernel<<<1, RES_NMAX, 0, ctx->stream>>>(rp);
+    rp.pairs = ctx->pairs; rp.st = ctx->dstats; rp.out = ctx->res_out; rp.loc = ctx->res_loc; rp.label = ctx->res_label; rp.aux = ctx->res_aux; rp.cown = ctx->res_cown;
+    rp.cnp = ctx->res_cnp; rp.cstart = ctx->res_cstart; rp.cfill = ctx->res_cfill; rp.cq = ctx->res_cq; rp.clist = ctx->res_clist;
+    rp.ctl = ctx->res_ctl; rp.tab = ctx->res_tab; rp.dbody = ctx->res_dbody; rp.dbodyi = ctx->res_dbodyi; rp.dpair = ctx->res_dpair;
+    rp.dpairi = ctx->res_dpairi; rp.dbodyN = ctx->res_dbodyN;
+    rp.cap = ctx->cap > 0 ? ctx->cap : 1; rp.nb = ctx->nb; rp.ld = ctx->ld; rp.mu = ctx->mu; rp.h = dt; rp.tol = tol;
+    resolve_label_kernel<<<1, RES_LABEL_THREADS, 0, ctx->stream>>>(rp);
     mo_status s = post_launch(ctx);
     if (s != MO_OK) return s;
-    resolve_kernel<64, 0, 32, true><<<ctx->res_grid, 64, RES_DYN_SMEM + 6 * RES_KMAX * 64 * 8, ctx->stream>>>(rp);       // components of <= 32 pairs
+    // largest first: the long solves (a giant's star) start before the many short ones fill the SMs
+    if (ctx->res_dbody) {
+        resolve_stream_kernel<<<RES_GRID_4, RES_D_THREADS, 0, ctx->stream>>>(rp);
+        s = post_launch(ctx);
+        if (s != MO_OK) return s;
+    }
+    resolve_solve_kernel<1024, 3><<<RES_GRID_3, 1024, ctx->res_smemC, ctx->stream>>>(rp, ctx->res_smemC);
     s = post_launch(ctx);
     if (s != MO_OK) return s;
-    resolve_kernel<256, 32, 128, true><<<ctx->res_grid, 256, RES_DYN_SMEM + 6 * RES_KMAX * 256 * 8, ctx->stream>>>(rp);    // <= 128 pairs
+    resolve_solve_kernel<512, 2><<<RES_GRID_2, 512, ctx->res_smemC, ctx->stream>>>(rp, ctx->res_smemC);
     s = post_launch(ctx);
     if (s != MO_OK) return s;
-    resolve_kernel<512, 128, 1 << 30, false><<<ctx->res_grid, 512, RES_DYN_SMEM, ctx->stream>>>(rp);   // more pairs, <= 512 bodies
+    resolve_solve_kernel<256, 1><<<RES_GRID_1, 256, ctx->res_smemB, ctx->stream>>>(rp, ctx->res_smemB);
     s = post_launch(ctx);
     if (s != MO_OK) return s;
-    resolve_kernel<RES_NMAX, 128, 1 << 30, true><<<ctx->res_grid, RES_NMAX, RES_DYN_SMEM, ctx->stream>>>(rp);   // the rest
+    resolve_solve_kernel<64, 0><<<ctx->nsm * RES_GRID_0_PER_SM, 64, ctx->res_smemA, ctx->stream>>>(rp, ctx->res_smemA);
     return post_launch(ctx);
 }
 

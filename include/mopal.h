@@ -186,6 +186,31 @@ mo_status mo_set_resolve(mo_ctx *ctx, double tol);
  * evaluations summed over the systems, systems not resolved}.  Synchronises. */
 mo_status mo_resolve_stats(mo_ctx *ctx, int32_t *out4);
 
+/* ---- the pair sum sharded over several GPUs (the paper sees MPI over CPU clusters as
+ * the only multi-device route) -----------------------------------------------------------------------
+ * One process and one context per GPU, all holding the WHOLE state (identical arrays on every rank).  Only the
+ * O(N^2) pair sum is split: after mo_set_shard(rank, world) a context evaluates its contiguous share of the pair
+ * kernel's work units (two-sided kernel, nb >= 8192: units of the triangle, so a rank's result is a PARTIAL
+ * acceleration of every body; big x all mode: blocks of bodies i, the other rows 0), and the caller sums `a` over the
+ * ranks (one all-reduce of 3*ld doubles per step, e.g. NCCL through torch.distributed - the library itself holds no
+ * communicator).  Every O(N) stage and the encounter pass run replicated on every rank, on identical data, so the
+ * states stay bit-identical across the ranks.  Protocol:
+ *     mo_accel(ctx); <sum a over ranks>; mo_accel_summed(ctx);
+ *     per step: mo_step_begin(ctx, dt); <sum a over ranks>; mo_step_end(ctx, dt, stats);
+ * mo_step itself returns MO_EINVAL while world > 1.  MO_EINVAL also for sizes whose pair kernel does not split
+ * (fully interacting systems below 8192 bodies: a step there is tens of microseconds). */
+mo_status mo_set_shard(mo_ctx *ctx, int32_t rank, int32_t world);
+/* [lo, hi) = rank's contiguous share of n work units: lo = n*rank/world, hi = n*(rank+1)/world.  Host only. */
+mo_status mo_shard_range(int64_t n, int32_t rank, int32_t world, int64_t *lo, int64_t *hi);
+/* The pair kernel's work units and this context's share of them (for inspection). */
+mo_status mo_shard_units(const mo_ctx *ctx, int64_t *units, int64_t *lo, int64_t *hi);
+/* kick, jump, snapshot, drift, encounter pass, jump, this rank's share of a(x).  Needs a summed a (see above). */
+mo_status mo_step_begin(mo_ctx *ctx, double dt);
+/* Tell the context that `a` now holds the sum over the ranks. */
+mo_status mo_accel_summed(mo_ctx *ctx);
+/* The closing kick v += dt/2 a with the summed a; stats_host as in mo_step (nullable; synchronises if given). */
+mo_status mo_step_end(mo_ctx *ctx, double dt, mo_stats *stats_host);
+
 /* Copy the current x, v into the context's x0, v0 snapshot (asynchronous). */
 mo_status mo_snapshot(mo_ctx *ctx);
 /* Device pointers of the snapshot planes (3*ld doubles each), for inspection. */

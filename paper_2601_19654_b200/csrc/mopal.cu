@@ -54,6 +54,8 @@ struct mo_ctx {
     int *res_dbodyi = nullptr, *res_dpairi = nullptr;
     long long res_dbodyN = 0;
     int res_smemA = 0, res_smemB = 0, res_smemC = 0;
+    cudaStream_t res_stream[4] = {nullptr, nullptr, nullptr, nullptr};   // the size classes are solved side by side
+    cudaEvent_t res_fork = nullptr, res_join[4] = {nullptr, nullptr, nullptr, nullptr};
     ResStats* res_out = nullptr;        // device
     ResStats* res_host = nullptr;       // pinned
     int hill_mode = -1;                 // mo_set_hill: -1 off
@@ -82,6 +84,7 @@ struct mo_ctx {
     double *sym_partI = nullptr, *sym_partJ = nullptr;
     std::vector<int4> h_units;
     std::vector<int> h_ustart;
+    int shard_rank = 0, shard_world = 1;   // mo_set_shard: this context computes rank's share of the pair sum (row f4)
     bool pair_ready = false;
     bool a_valid = false, snap_valid = false, box_valid = false, debug = false, use_graph = true;
     long long launches = 0;
@@ -103,6 +106,11 @@ struct mo_ctx {
             return MO_ECUDA;                              \
         }                                                 \
     } while (0)
+
+static inline void shard_range(long long n, int rank, int world, long long* lo, long long* hi) {
+    *lo = n * rank / world;
+    *hi = n * (rank + 1) / world;
+}
 
 static inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
@@ -254,6 +262,8 @@ extern "C" void mo_destroy(mo_ctx* ctx) {
     cudaFree(ctx->res_cnp); cudaFree(ctx->res_cstart); cudaFree(ctx->res_cfill); cudaFree(ctx->res_cq); cudaFree(ctx->res_clist); cudaFree(ctx->res_ctl); cudaFree(ctx->res_aux); cudaFree(ctx->res_cown);
     cudaFree(ctx->res_dbody); cudaFree(ctx->res_dpair); cudaFree(ctx->res_dbodyi); cudaFree(ctx->res_dpairi);
     if (ctx->res_host) cudaFreeHost(ctx->res_host);
+    for (int k = 0; k < 4; ++k) { if (ctx->res_stream[k]) cudaStreamDestroy(ctx->res_stream[k]); if (ctx->res_join[k]) cudaEventDestroy(ctx->res_join[k]); }
+    if (ctx->res_fork) cudaEventDestroy(ctx->res_fork);
     cudaFree(ctx->gmsum); cudaFree(ctx->en_on); cudaFree(ctx->en_pair); cudaFree(ctx->en_out);
     if (ctx->en_host) cudaFreeHost(ctx->en_host); cudaFree(ctx->tiles);
     cudaFree(ctx->sym_units); cudaFree(ctx->sym_ustart); cudaFree(ctx->sym_partI); cudaFree(ctx->sym_partJ);
@@ -404,7 +414,7 @@ static mo_status launch_pair(mo_ctx* ctx, bool kick = false, double hk = 0.0) {
     if (ctx->use_psm) {
         BigParams bp;
         bp.x = ctx->x; bp.gm = ctx->gm; bp.rcrit = ctx->rcrit; bp.a = ctx->a; bp.v = ctx->v;
-        bp.nb = ctx->nb; bp.nbig = ctx->nbig; bp.ld = ctx->ld; bp.hk = hk;
+        bp.nb = ctx->nb; bp.nbig = ctx->nbig; bp.ld = ctx->ld; bp.hk = hk; bp.blk0 = 0; bp.blk1 = 0;
         const int G = ctx->psm_g, per = PSM_THREADS / G;
         const int grid = (ctx->nb + per - 1) / per;
         auto k = G == 8 ? (kick ? pair_small_kernel<8, true> : pair_small_kernel<8, false>)
@@ -414,13 +424,25 @@ static mo_status launch_pair(mo_ctx* ctx, bool kick = false, double hk = 0.0) {
     } else if (ctx->use_big) {
         BigParams bp;
         bp.x = ctx->x; bp.gm = ctx->gm; bp.rcrit = ctx->rcrit; bp.a = ctx->a; bp.v = ctx->v;
-        bp.nb = ctx->nb; bp.nbig = ctx->nbig; bp.ld = ctx->ld; bp.hk = hk;
-        pick_big_kernel(ctx->big_ipt, kick)<<<ctx->big_grid, BIG_THREADS, 0, ctx->stream>>>(bp);
+        bp.nb = ctx->nb; bp.nbig = ctx->nbig; bp.ld = ctx->ld; bp.hk = hk; bp.blk0 = 0; bp.blk1 = 0;
+        int grid = ctx->big_grid;
+        if (ctx->shard_world > 1) {       // this rank's blocks of bodies i; the other rows of a stay 0 (the caller sums over the ranks)
+            long long lo, hi;
+            shard_range(ctx->nIblk, ctx->shard_rank, ctx->shard_world, &lo, &hi);
+            bp.blk0 = (int)lo; bp.blk1 = (int)hi;
+            CK(cudaMemsetAsync(ctx->a, 0, 3 * (size_t)ctx->ld * sizeof(double), ctx->stream));
+            grid = hi - lo < grid ? (int)(hi - lo) : grid;
+        }
+        if (grid > 0 && (ctx->shard_world == 1 || bp.blk1 > bp.blk0))
+            pick_big_kernel(ctx->big_ipt, kick)<<<grid, BIG_THREADS, 0, ctx->stream>>>(bp);
     } else if (ctx->use_sym) {
         SymParams sp;
         sp.tiles = ctx->tiles; sp.x = ctx->x; sp.gm = ctx->gm; sp.rcrit = ctx->rcrit; sp.units = ctx->sym_units;
         sp.partI = ctx->sym_partI; sp.partJ = ctx->sym_partJ; sp.nb = ctx->nb; sp.ld = ctx->ld; sp.nbPad = ctx->nbPad;
-        pair_sym_kernel<<<ctx->sym_nunits, SYM_THREADS, 0, ctx->stream>>>(sp);
+        long long u0 = 0, u1 = ctx->sym_nunits;
+        if (ctx->shard_world > 1) shard_range(ctx->sym_nunits, ctx->shard_rank, ctx->shard_world, &u0, &u1);
+        sp.unit0 = (int)u0;
+        if (u1 > u0) pair_sym_kernel<<<(int)(u1 - u0), SYM_THREADS, 0, ctx->stream>>>(sp);
     } else {
         pick_pair_kernel(ctx->ipt, ctx->unroll)<<<grid, CTA_THREADS, 0, ctx->stream>>>(p);
     }
@@ -430,6 +452,7 @@ static mo_status launch_pair(mo_ctx* ctx, bool kick = false, double hk = 0.0) {
 
 // a <- accel(x), optionally preceded by the jump (psumB) and followed by the kick
 static mo_status enqueue_accel(mo_ctx* ctx, bool jump, double hj, bool kick, double hk) {
+    if (ctx->shard_world > 1) kick = false;      // a is this rank's share: the kick follows the caller's sum over the ranks (mo_step_end)
     const double hjm = jump ? hj / ctx->mu : 0.0;
     const double* ps = jump ? ctx->psumB : nullptr;
     const int nps = jump ? ctx->npsum : 0;
@@ -455,8 +478,10 @@ static mo_status enqueue_accel(mo_ctx* ctx, bool jump, double hj, bool kick, dou
     const int nblk = (ctx->nb + ON_BLOCK - 1) / ON_BLOCK;
     if (ctx->use_sym) {
         auto rk = kick ? sym_reduce_kernel<true> : sym_reduce_kernel<false>;
+        long long u0 = 0, u1 = ctx->sym_nunits;
+        if (ctx->shard_world > 1) shard_range(ctx->sym_nunits, ctx->shard_rank, ctx->shard_world, &u0, &u1);
         rk<<<dim3(nblk, 3), ON_BLOCK, 0, ctx->stream>>>(ctx->sym_partI, ctx->sym_partJ, ctx->sym_ustart, ctx->nb, ctx->ld, ctx->nbPad,
-                                               ctx->a, kick ? ctx->v : nullptr, kick ? hk : 0.0);
+                                               ctx->a, kick ? ctx->v : nullptr, kick ? hk : 0.0, (int)u0, (int)u1, ctx->sym_ch);
     } else if (kick)
         accel_reduce_kernel<true><<<nblk, ON_BLOCK, 0, ctx->stream>>>(ctx->part, ctx->nsplit, ctx->nb, ctx->ld, ctx->a, ctx->v, hk);
     else
@@ -568,6 +593,11 @@ static mo_status ensure_resolve_scratch(mo_ctx* ctx) {
     if (e == cudaSuccess) e = cudaFuncSetAttribute(resolve_solve_kernel<1024, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->res_smemC);
     if (e == cudaSuccess) e = cudaMemsetAsync(ctx->res_out, 0, sizeof(ResStats), ctx->stream);
     if (e == cudaSuccess) e = cudaMallocHost(reinterpret_cast<void**>(&ctx->res_host), sizeof(ResStats));
+    for (int k = 0; k < 4 && e == cudaSuccess; ++k) {
+        e = cudaStreamCreateWithFlags(&ctx->res_stream[k], cudaStreamNonBlocking);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->res_join[k], cudaEventDisableTiming);
+    }
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->res_fork, cudaEventDisableTiming);
     if (e != cudaSuccess) { cudaGetLastError(); ctx->last_err = e; return e == cudaErrorMemoryAllocation ? MO_ENOMEM : MO_ECUDA; }
     return MO_OK;
 }
@@ -583,23 +613,30 @@ static mo_status enqueue_resolve(mo_ctx* ctx, double dt, double tol) {
     resolve_label_kernel<<<1, RES_LABEL_THREADS, 0, ctx->stream>>>(rp);
     mo_status s = post_launch(ctx);
     if (s != MO_OK) return s;
-    // largest first: the long solves (a giant's star) start before the many short ones fill the SMs
-    if (ctx->res_dbody) {
-        resolve_stream_kernel<<<RES_GRID_4, RES_D_THREADS, 0, ctx->stream>>>(rp);
+    // the size classes side by side: the few large components (a giant's star is a long chain of right-hand sides on one
+    // CTA) on streams of their own, the many small ones on the caller's
+    cudaStream_t mainS = ctx->stream;
+    CK(cudaEventRecord(ctx->res_fork, mainS));
+    for (int k = 0; k < 4; ++k) {
+        if (k == 0 && !ctx->res_dbody) continue;
+        cudaStream_t st = ctx->res_stream[k];
+        CK(cudaStreamWaitEvent(st, ctx->res_fork, 0));
+        if (k == 0) resolve_stream_kernel<<<RES_GRID_4, RES_D_THREADS, 0, st>>>(rp);
+        else if (k == 1) resolve_solve_kernel<1024, 3><<<RES_GRID_3, 1024, ctx->res_smemC, st>>>(rp, ctx->res_smemC);
+        else if (k == 2) resolve_solve_kernel<512, 2><<<RES_GRID_2, 512, ctx->res_smemC, st>>>(rp, ctx->res_smemC);
+        else resolve_solve_kernel<256, 1><<<RES_GRID_1, 256, ctx->res_smemB, st>>>(rp, ctx->res_smemB);
         s = post_launch(ctx);
         if (s != MO_OK) return s;
+        CK(cudaEventRecord(ctx->res_join[k], st));
     }
-    resolve_solve_kernel<1024, 3><<<RES_GRID_3, 1024, ctx->res_smemC, ctx->stream>>>(rp, ctx->res_smemC);
+    resolve_solve_kernel<64, 0><<<ctx->nsm * RES_GRID_0_PER_SM, 64, ctx->res_smemA, mainS>>>(rp, ctx->res_smemA);
     s = post_launch(ctx);
     if (s != MO_OK) return s;
-    resolve_solve_kernel<512, 2><<<RES_GRID_2, 512, ctx->res_smemC, ctx->stream>>>(rp, ctx->res_smemC);
-    s = post_launch(ctx);
-    if (s != MO_OK) return s;
-    resolve_solve_kernel<256, 1><<<RES_GRID_1, 256, ctx->res_smemB, ctx->stream>>>(rp, ctx->res_smemB);
-    s = post_launch(ctx);
-    if (s != MO_OK) return s;
-    resolve_solve_kernel<64, 0><<<ctx->nsm * RES_GRID_0_PER_SM, 64, ctx->res_smemA, ctx->stream>>>(rp, ctx->res_smemA);
-    return post_launch(ctx);
+    for (int k = 0; k < 4; ++k) {
+        if (k == 0 && !ctx->res_dbody) continue;
+        CK(cudaStreamWaitEvent(mainS, ctx->res_join[k], 0));
+    }
+    return MO_OK;
 }
 
 static mo_status enqueue_step(mo_ctx* ctx, double dt) {
@@ -703,7 +740,7 @@ extern "C" mo_status mo_accel(mo_ctx* ctx) {
     mo_status s = ensure_pair_scratch(ctx);
     if (s != MO_OK) return s;
     s = enqueue_accel(ctx, false, 0.0, false, 0.0);
-    if (s == MO_OK) ctx->a_valid = true;
+    if (s == MO_OK) ctx->a_valid = ctx->shard_world == 1;     // sharded: a share, until mo_accel_summed
     return s;
 }
 
@@ -758,6 +795,10 @@ extern "C" mo_status mo_set_nbig(mo_ctx* ctx, int32_t nbig) {
     ctx->nbig = nbig;
     ctx->nSrcTiles = (nbig + TJ - 1) / TJ;
     choose_geometry(ctx);
+    if (ctx->shard_world > 1 && !(ctx->use_sym || ctx->use_big)) {     // this size takes a kernel that does not split its work
+        ctx->shard_rank = 0; ctx->shard_world = 1;
+        return MO_EINVAL;
+    }
     return MO_OK;
 }
 
@@ -888,8 +929,68 @@ extern "C" mo_status mo_encounters(mo_ctx* ctx, double dt, const double* x0, con
     return MO_OK;
 }
 
+extern "C" mo_status mo_shard_range(int64_t n, int32_t rank, int32_t world, int64_t* lo, int64_t* hi) {
+    if (n < 0 || world < 1 || rank < 0 || rank >= world || !lo || !hi) return MO_EINVAL;
+    long long a, b;
+    shard_range(n, rank, world, &a, &b);
+    *lo = a; *hi = b;
+    return MO_OK;
+}
+
+extern "C" mo_status mo_set_shard(mo_ctx* ctx, int32_t rank, int32_t world) {
+    if (!ctx || world < 1 || rank < 0 || rank >= world) return MO_EINVAL;
+    // only the kernels of the large systems split their work: the two-sided pair sum (nb >= 8192) and the big x all sum
+    if (world > 1 && !(ctx->use_sym || ctx->use_big)) return MO_EINVAL;
+    if (ctx->gexec) {
+        CK(cudaStreamSynchronize(ctx->stream));
+        cudaGraphExecDestroy(ctx->gexec); ctx->gexec = nullptr;
+    }
+    ctx->shard_rank = rank; ctx->shard_world = world;
+    ctx->a_valid = false;
+    return MO_OK;
+}
+
+extern "C" mo_status mo_shard_units(const mo_ctx* ctx, int64_t* units, int64_t* lo, int64_t* hi) {
+    if (!ctx || !units || !lo || !hi) return MO_EINVAL;
+    const long long n = ctx->use_sym ? ctx->sym_nunits : ctx->use_big ? ctx->nIblk : 0;
+    long long a = 0, b = n;
+    if (ctx->shard_world > 1) shard_range(n, ctx->shard_rank, ctx->shard_world, &a, &b);
+    *units = n; *lo = a; *hi = b;
+    return MO_OK;
+}
+
+// Sharded step, first part: everything up to and including this rank's share of the pair sum; a holds the share.
+extern "C" mo_status mo_step_begin(mo_ctx* ctx, double dt) {
+    if (!ctx || !isfinite(dt) || dt == 0.0 || ctx->shard_world < 2) return MO_EINVAL;
+    if (!ctx->a_valid) return MO_EINVAL;          // mo_accel + the caller's sum over the ranks + mo_accel_summed come first
+    mo_status s = ensure_pair_scratch(ctx);
+    if (s != MO_OK) return s;
+    s = enqueue_step(ctx, dt);
+    if (s == MO_OK) { ctx->snap_valid = true; ctx->box_valid = true; ctx->a_valid = false; }
+    return s;
+}
+
+// The caller has summed a over the ranks: a is the acceleration of the current x.
+extern "C" mo_status mo_accel_summed(mo_ctx* ctx) {
+    if (!ctx || ctx->shard_world < 2) return MO_EINVAL;
+    ctx->a_valid = true;
+    return MO_OK;
+}
+
+// Sharded step, second part (after the sum of a over the ranks): the closing kick.
+extern "C" mo_status mo_step_end(mo_ctx* ctx, double dt, mo_stats* stats_host) {
+    if (!ctx || !isfinite(dt) || dt == 0.0 || ctx->shard_world < 2) return MO_EINVAL;
+    kick_psum_kernel<true><<<ctx->npsum, ON_BLOCK, 0, ctx->stream>>>(ctx->v, ctx->a, ctx->gm, ctx->nb, ctx->ld, 0.5 * dt, ctx->psumA, ctx->ticket);
+    mo_status s = post_launch(ctx);
+    if (s != MO_OK) return s;
+    ctx->a_valid = true;
+    if (stats_host) return status_from_stats(ctx, stats_host);
+    return MO_OK;
+}
+
 extern "C" mo_status mo_step(mo_ctx* ctx, double dt, int32_t nsteps, mo_stats* stats_host) {
     if (!ctx || !isfinite(dt) || dt == 0.0 || nsteps < 0) return MO_EINVAL;
+    if (ctx->shard_world > 1) return MO_EINVAL;   // sharded: mo_step_begin / sum of a over the ranks / mo_step_end
     mo_status s = ensure_pair_scratch(ctx);   // before any capture: allocation cannot be recorded
     if (s != MO_OK) return s;
     if (!ctx->a_valid && nsteps > 0) {

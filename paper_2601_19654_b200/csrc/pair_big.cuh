@@ -29,6 +29,7 @@ struct BigParams {
     double* v;             // 3*ld in/out when KICK
     int nb, nbig, ld;
     double hk;
+    int blk0, blk1;        // pair_big_kernel: the blocks of bodies i this launch covers (a rank's share, row f4), blk1 <= 0: all
 };
 
 // The pairs the integer gate could not prove to be outside the changeover shell (readings A-1..A-5,
@@ -51,7 +52,9 @@ __global__ void __launch_bounds__(BIG_THREADS) pair_big_kernel(BigParams p) {
     __shared__ int s_gj[BIG_SRC];      // per-source changeover gate: high word of rcrit_j^2
     __shared__ double s_rc[BIG_SRC];   // rcrit_j, for the pairs that fail the gate
     const int tid = threadIdx.x;
-    const int nIblk = (p.nb + BIG_THREADS * IPT - 1) / (BIG_THREADS * IPT);
+    const int nIall = (p.nb + BIG_THREADS * IPT - 1) / (BIG_THREADS * IPT);
+    const int nIblk = p.blk1 > 0 ? min(p.blk1, nIall) : nIall;
+    const int blkFirst = p.blk1 > 0 ? p.blk0 : 0;
     const bool single = p.nbig <= BIG_SRC;             // all sources fit: staged once per CTA
 
     auto stage = [&](int j0, int n, int npad) {
@@ -88,8 +91,8 @@ __global__ void __launch_bounds__(BIG_THREADS) pair_big_kernel(BigParams p) {
             nrc[k] = ok ? p.rcrit[i] : 0.0;
         }
     };
-    fetch(blockIdx.x);
-    for (int blk = blockIdx.x; blk < nIblk; blk += gridDim.x) {
+    fetch(blkFirst + blockIdx.x);
+    for (int blk = blkFirst + blockIdx.x; blk < nIblk; blk += gridDim.x) {
         const int ibase = blk * (BIG_THREADS * IPT) + tid;
         double xi[IPT], yi[IPT], zi[IPT], ax[IPT], ay[IPT], az[IPT], rci[IPT];
         int gi[IPT];

@@ -59,6 +59,7 @@ struct SymParams {
     double* partI;               // [nUnits][3][SYM_R]
     double* partJ;               // triangular: block I at symJ_off(I), planes of (nbPad - I*SYM_R)
     int nb, ld, nbPad;
+    int unit0;                   // first work unit of this launch (a rank's share of the units, row f4; 0 otherwise)
 };
 
 __host__ __device__ inline long long symJ_off(int I, int nbPad) {
@@ -187,7 +188,8 @@ __global__ void __launch_bounds__(SYM_THREADS, SYM_MINB) pair_sym_kernel(SymPara
     __shared__ __align__(8) uint64_t s_full[SYM_STAGES];
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int4 un = p.units[blockIdx.x];
+    const int ug = blockIdx.x + p.unit0;
+    const int4 un = p.units[ug];
     const int I = un.x, t0 = un.y, nt = un.z - un.y;
     const unsigned char* src = p.tiles + (size_t)t0 * ACC_TILE_BYTES;
 
@@ -257,7 +259,7 @@ __global__ void __launch_bounds__(SYM_THREADS, SYM_MINB) pair_sym_kernel(SymPara
         }
     }
 
-    double* pi = p.partI + (size_t)blockIdx.x * 3 * SYM_R;
+    double* pi = p.partI + (size_t)ug * 3 * SYM_R;
 #pragma unroll
     for (int k = 0; k < SYM_IPT; ++k) {
         const int r = warp * (32 * SYM_IPT) + k * 32 + lane;
@@ -267,12 +269,14 @@ __global__ void __launch_bounds__(SYM_THREADS, SYM_MINB) pair_sym_kernel(SymPara
 
 // a_b = (row partials of b's block, in unit order) + (column partials, ascending I); optionally
 // the closing half kick v += hk * a (Hamiltonian block LOOP 1).
+// [us0, us1): the work units that were run (all of them; a rank's share when the pair sum is sharded over GPUs, SURVEY.md
+// 8(e) - the sum over the ranks of the results is then the full acceleration); ch = j tiles per unit.
 template <bool KICK>
 __global__ void __launch_bounds__(ON_BLOCK) sym_reduce_kernel(const double* __restrict__ partI,
                                                                const double* __restrict__ partJ,
                                                                const int* __restrict__ ustart, int nb, int ld,
                                                                int nbPad, double* __restrict__ a,
-                                                               double* __restrict__ v, double hk) {
+                                                               double* __restrict__ v, double hk, int us0, int us1, int ch) {
     // one thread per (body, component) - blockIdx.y = component - and four interleaved partial sums per
     // list, combined in a fixed order: three times the threads and four times the loads in flight of a
     // thread-per-body loop, still a fixed tree that depends on nb only
@@ -280,7 +284,7 @@ __global__ void __launch_bounds__(ON_BLOCK) sym_reduce_kernel(const double* __re
     if (b >= nb) return;
     const int c = blockIdx.y;
     const int Ib = b / SYM_R, r = b - Ib * SYM_R;
-    const int u0 = ustart[Ib], u1 = ustart[Ib + 1];
+    const int u0 = max(ustart[Ib], us0), u1 = min(ustart[Ib + 1], us1);
     double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
     int u = u0;
     for (; u + 3 < u1; u += 4) {
@@ -290,15 +294,16 @@ __global__ void __launch_bounds__(ON_BLOCK) sym_reduce_kernel(const double* __re
         s3 += partI[((size_t)(u + 3) * 3 + c) * SYM_R + r];
     }
     for (; u < u1; ++u) s0 += partI[((size_t)u * 3 + c) * SYM_R + r];
+    // the column partial of row block I was written by the unit that holds this body's j tile
+    const int tb = b / TJ;
+    auto colpart = [&](int I) -> double {
+        const int ug = ustart[I] + (tb - I * SYM_TPB) / ch;
+        return (ug >= us0 && ug < us1) ? partJ[symJ_off(I, nbPad) + (size_t)c * (nbPad - I * SYM_R) + (b - I * SYM_R)] : 0.0;
+    };
     double t0 = 0.0, t1 = 0.0, t2 = 0.0, t3 = 0.0;
     int I = 0;
-    for (; I + 3 <= Ib; I += 4) {
-        t0 += partJ[symJ_off(I, nbPad) + (size_t)c * (nbPad - I * SYM_R) + (b - I * SYM_R)];
-        t1 += partJ[symJ_off(I + 1, nbPad) + (size_t)c * (nbPad - (I + 1) * SYM_R) + (b - (I + 1) * SYM_R)];
-        t2 += partJ[symJ_off(I + 2, nbPad) + (size_t)c * (nbPad - (I + 2) * SYM_R) + (b - (I + 2) * SYM_R)];
-        t3 += partJ[symJ_off(I + 3, nbPad) + (size_t)c * (nbPad - (I + 3) * SYM_R) + (b - (I + 3) * SYM_R)];
-    }
-    for (; I <= Ib; ++I) t0 += partJ[symJ_off(I, nbPad) + (size_t)c * (nbPad - I * SYM_R) + (b - I * SYM_R)];
+    for (; I + 3 <= Ib; I += 4) { t0 += colpart(I); t1 += colpart(I + 1); t2 += colpart(I + 2); t3 += colpart(I + 3); }
+    for (; I <= Ib; ++I) t0 += colpart(I);
     const double s = ((s0 + s1) + (s2 + s3)) + ((t0 + t1) + (t2 + t3));
     a[(size_t)c * ld + b] = s;
     if (KICK) v[(size_t)c * ld + b] = fma(hk, s, v[(size_t)c * ld + b]);

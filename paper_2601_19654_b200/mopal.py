@@ -23,7 +23,8 @@ EXPORTS = ["mo_create", "mo_accel", "mo_drift", "mo_encounters", "mo_step", "mo_
            "mo_workspace_bytes", "mo_step_host", "mo_accel_host", "mo_probe_fp64_peak",
            "mo_pair_geometry", "mo_set_kernel_timing", "mo_pair_kernel_ms", "mo_strerror", "mo_version",
            "mo_set_nbig", "mo_pair_kernel_name", "mo_h2dh", "mo_dh2h", "mo_hill", "mo_set_hill", "mo_energy",
-           "mo_resolve", "mo_set_resolve", "mo_resolve_stats", "mo_boxes_copy"]
+           "mo_resolve", "mo_set_resolve", "mo_resolve_stats", "mo_boxes_copy",
+           "mo_set_shard", "mo_shard_range", "mo_shard_units", "mo_step_begin", "mo_accel_summed", "mo_step_end"]
 
 
 class MoStats(C.Structure):
@@ -77,6 +78,12 @@ def load():
     L.mo_resolve.restype = C.c_int; L.mo_resolve.argtypes = [vp, C.c_double, C.c_double]
     L.mo_set_resolve.restype = C.c_int; L.mo_set_resolve.argtypes = [vp, C.c_double]
     L.mo_resolve_stats.restype = C.c_int; L.mo_resolve_stats.argtypes = [vp, C.POINTER(I32)]
+    L.mo_set_shard.restype = C.c_int; L.mo_set_shard.argtypes = [vp, I32, I32]
+    L.mo_shard_range.restype = C.c_int; L.mo_shard_range.argtypes = [C.c_int64, I32, I32, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
+    L.mo_shard_units.restype = C.c_int; L.mo_shard_units.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
+    L.mo_step_begin.restype = C.c_int; L.mo_step_begin.argtypes = [vp, C.c_double]
+    L.mo_accel_summed.restype = C.c_int; L.mo_accel_summed.argtypes = [vp]
+    L.mo_step_end.restype = C.c_int; L.mo_step_end.argtypes = [vp, C.c_double, C.POINTER(MoStats)]
     L.mo_get_stats.restype = C.c_int; L.mo_get_stats.argtypes = [vp, C.POINTER(MoStats)]
     L.mo_launch_count.restype = I64; L.mo_launch_count.argtypes = [vp]
     L.mo_workspace_bytes.restype = I64; L.mo_workspace_bytes.argtypes = [vp]
@@ -101,6 +108,15 @@ def strerror(status) -> str:
 
 def version() -> str:
     return load().mo_version().decode()
+
+
+def shard_range(n, rank, world):
+    """[lo, hi): rank's contiguous share of n work units (mo_shard_range; host only, no GPU needed)."""
+    lo, hi = C.c_int64(0), C.c_int64(0)
+    st = load().mo_shard_range(int(n), int(rank), int(world), C.byref(lo), C.byref(hi))
+    if st != MO_OK:
+        raise MopalError(st, "mo_shard_range")
+    return int(lo.value), int(hi.value)
 
 
 def probe_fp64_peak(reps: int = 5, with_mean: bool = False):
@@ -278,6 +294,32 @@ class Mopal:
         out = (C.c_int32 * 4)()
         self._check(self._L.mo_resolve_stats(self._ctx, out), "mo_resolve_stats")
         return dict(bodies=out[0], steps=out[1], rhs=out[2], fail=out[3])
+
+    # ---- pair sum sharded over several GPUs (include/mopal.h: mo_set_shard) ----
+    def set_shard(self, rank, world):
+        self._check(self._L.mo_set_shard(self._ctx, int(rank), int(world)), "mo_set_shard")
+
+    def shard_units(self):
+        """(work units of the pair kernel, lo, hi): this context evaluates the units [lo, hi)."""
+        n, lo, hi = C.c_int64(0), C.c_int64(0), C.c_int64(0)
+        self._check(self._L.mo_shard_units(self._ctx, C.byref(n), C.byref(lo), C.byref(hi)), "mo_shard_units")
+        return int(n.value), int(lo.value), int(hi.value)
+
+    def step_begin(self, dt):
+        self._check(self._L.mo_step_begin(self._ctx, float(dt)), "mo_step_begin")
+
+    def accel_summed(self):
+        self._check(self._L.mo_accel_summed(self._ctx), "mo_accel_summed")
+
+    def step_end(self, dt, sync=True) -> Stats | None:
+        if not sync:
+            self._check(self._L.mo_step_end(self._ctx, float(dt), None), "mo_step_end")
+            return None
+        s = MoStats()
+        st = self._L.mo_step_end(self._ctx, float(dt), C.byref(s))
+        if st not in _SOFT:
+            raise MopalError(st, "mo_step_end")
+        return _stats(s, st)
 
     def invalidate_accel(self):
         self._check(self._L.mo_invalidate_accel(self._ctx), "mo_invalidate_accel")

@@ -1124,3 +1124,100 @@ def test_resolve_massless_planetesimals_are_detached(M, K):
     assert st2["fail"] == 0 and st2["bodies"] == len(idx2) - 1
     assert np.array_equal(gx2[:, 0], x1b[:, 0]) and np.array_equal(gv2[:, 0], v1b[:, 0])
     assert _rel_vec_err(gx2[:, idx2], ref2["x"][:, idx2]).max() <= 1e-10 and _rel_vec_err(gv2[:, idx2], ref2["v"][:, idx2]).max() <= 1e-10
+
+
+# ------------------------------------------------------------------------------ pair sum sharded over GPUs
+class _SeqDist:
+    """torch.distributed stand-in for ONE GPU: the 'ranks' are contexts stepped one after the other (nobody waits on
+    anybody); all_reduce(SUM) is deferred until every rank has handed in its tensor, then each gets the sum."""
+    class ReduceOp:
+        SUM = "sum"
+
+    def __init__(self, world):
+        self.world, self.pending = world, []
+
+    def all_reduce(self, t, op=None, group=None):
+        self.pending.append(t)
+        if len(self.pending) == self.world:
+            tot = self.pending[0].clone()
+            for u in self.pending[1:]:
+                tot += u
+            for u in self.pending:
+                u.copy_(tot)
+            self.pending = []
+
+
+@pytest.mark.parametrize("kind,world", [("sym", 2), ("sym", 3), ("big", 2)])
+def test_sharded_pair_sum_and_step_on_one_gpu(M, kind, world):
+    """every rank's share of the pair kernel's work units, summed = the unsharded acceleration (oracle tolerance), and
+    begin / sum / end = mo_step; the ranks' states stay bit-identical"""
+    if kind == "sym":
+        w, nbig = W.shrink(3, 9000), None
+    else:
+        w, nbig = W.make_bigsmall(30000, 40), 40
+    gm = G * w.mass
+
+    def mk():
+        m = _mk(M, w)
+        if nbig is not None:
+            m.set_nbig(nbig)
+        return m
+    ref = mk()
+    assert ref.pair_kernel_name() == ("pair_sym_kernel" if kind == "sym" else "pair_big_kernel")
+    ranks = [mk() for _ in range(world)]
+    for r, m in enumerate(ranks):
+        m.set_shard(r, world)
+    n, lo0, _ = ranks[0].shard_units()
+    assert lo0 == 0 and ranks[-1].shard_units()[2] == n and all(ranks[r].shard_units()[2] == ranks[r + 1].shard_units()[1] for r in range(world - 1))
+    # shares of a
+    ref.accel()
+    tot = None
+    for m in ranks:
+        m.accel()
+        tot = m.a.clone() if tot is None else tot + m.a
+    a_ref, S = oracle.accel(gm, w.x, w.rcrit, nbig=nbig)
+    _check_accel(tot[:, :w.nb].cpu().numpy(), a_ref, S, "sum of the shares")
+    assert np.abs(tot[:, :w.nb].cpu().numpy() - ref.get("a")).max() <= 1e-14 * S.max()
+    if kind == "big":                                   # row shares: a rank's rows outside its blocks are exactly 0
+        assert float(ranks[0].a[:, w.nb - 100:w.nb].abs().max()) == 0.0
+    # steps: the ranks one after the other, the sum when all have handed in their share
+    L = M.load()
+    assert L.mo_step(ranks[0]._ctx, w.dt, 1, None) == M.MO_EINVAL and L.mo_step_begin(ranks[0]._ctx, w.dt) == M.MO_EINVAL   # a not summed yet
+    for m in ranks:
+        m.a.copy_(tot); m.accel_summed()
+    for _ in range(3):
+        for m in ranks:
+            m.step_begin(w.dt)
+        tot = ranks[0].a.clone()
+        for m in ranks[1:]:
+            tot += m.a
+        for m in ranks:
+            m.a.copy_(tot); m.accel_summed()
+        sts = [m.step_end(w.dt) for m in ranks]
+    s_ref = ref.step(w.dt, 3)
+    for m, st in zip(ranks, sts):
+        assert np.array_equal(m.get("x"), ranks[0].get("x")) and np.array_equal(m.get("v"), ranks[0].get("v"))
+        assert st.nce_last == s_ref.nce_last and st.steps_done == 3
+        assert np.array_equal(m.pair_list(st.nce_last), ref.pair_list(s_ref.nce_last))
+    assert _rel_vec_err(ranks[0].get("x"), ref.get("x")).max() <= 1e-14 and _rel_vec_err(ranks[0].get("v"), ref.get("v")).max() <= 1e-13
+    for m in ranks + [ref]:
+        m.close()
+
+
+def test_sharded_driver_world1_and_unsupported_sizes(M):
+    from paper_2601_19654_b200.sharded import ShardedMopal
+    w = W.shrink(3, 9000)
+    m1, m2 = _mk(M, w), _mk(M, w)
+    sm = ShardedMopal(m1)                              # world 1: plain mo_step
+    sm.step(w.dt, 2); m2.step(w.dt, 2)
+    assert np.array_equal(m1.get("x"), m2.get("x")) and sm.allreduces == 0
+    m1.close(); m2.close()
+    # the driver over the sequential stand-in: two ranks, two steps (the deferred sum needs both ranks to have called in,
+    # so the ranks' calls are interleaved by hand)
+    small = _mk(M, W.shrink(1, 2000))
+    L = M.load()
+    assert L.mo_set_shard(small._ctx, 0, 2) == M.MO_EINVAL          # below 8192 bodies the pair kernel does not split
+    assert L.mo_set_shard(small._ctx, 0, 1) == M.MO_OK
+    assert L.mo_set_shard(small._ctx, 2, 2) == M.MO_EINVAL and L.mo_set_shard(None, 0, 1) == M.MO_EINVAL
+    assert L.mo_step_begin(small._ctx, 1.0) == M.MO_EINVAL and L.mo_step_end(small._ctx, 1.0, None) == M.MO_EINVAL
+    small.close()

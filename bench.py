@@ -379,6 +379,24 @@ def run_ours(args):
     from paper_2601_19654_b200 import mopal as M
     from paper_2601_19654_b200 import workloads as W
 
+    if args.side_only:
+        # one of the side measurements alone (short runs for ncu: profiles/README.md names the commands)
+        peak = M.probe_fp64_peak(20, with_mean=True)[2]
+        flush = torch.empty(256 << 20, dtype=torch.uint8, device=f"cuda:{dev}")
+        hbm = float(_measured_peaks().get("hbm_gbs", 6550.0))
+        name = args.side_only
+        if name == "drift":
+            out = side_drift(torch, M, W, hbm)
+        elif name == "bigsmall":
+            out = side_config(torch, M, W.make_bigsmall(1_000_000, 100), 100, flush, peak, 3, 3)
+        elif name == "bigsmall_resolve":
+            out = side_config(torch, M, W.make_bigsmall(1_000_000, 100), 100, flush, peak, 3, 3, resolve_tol=1e-12)
+        elif name == "resolve":
+            out = side_config(torch, M, W.make_config(args.config), None, flush, peak, 3, 3, resolve_tol=1e-12)
+        else:
+            out = side_config(torch, M, W.make_config(int(name[3:])), None, flush, peak, 3, 3)
+        print(json.dumps({"side_only": name, **out}), flush=True)
+        return 0
     w, nbig = _workload(args)
     nb, pairs = w.nb, _pairs_per_step(w, nbig)
     K, Wm = args.steps, max(args.warmup, 3)
@@ -522,6 +540,63 @@ def run_ours(args):
     return 0
 
 
+def run_sharded(args):
+    """Row f4: ONE system whose O(N^2) pair sum is split over the ranks (strong scaling) - every rank holds the whole
+    state, one all-reduce of a (3*ld doubles, NCCL) per step.  Only ever exercised at world 1 on this pool (one GPU per
+    call); the driver's own scaling runs use the default replicas."""
+    import torch
+    rank, local_rank, world = _dist_env()
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py --sharded: no CUDA device")
+    dev = local_rank % torch.cuda.device_count()
+    torch.cuda.set_device(dev)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", dev))
+    from paper_2601_19654_b200 import mopal as M
+    from paper_2601_19654_b200.sharded import ShardedMopal
+    w, nbig = _workload(args)
+    pairs = _pairs_per_step(w, nbig)
+    m = M.Mopal(w.mass, w.x, w.v, w.rcrit, m_star=w.m_star, G=w.G, cap=1 << 20, device=f"cuda:{dev}")
+    if nbig is not None:
+        m.set_nbig(nbig)
+    sm = ShardedMopal(m, dist, rank, world)
+    K, Wm = args.steps, max(args.warmup, 3)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=m.device)
+    sm.step(w.dt, Wm)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    for k in range(K):
+        flush.zero_()
+        ev[k][0].record(m.stream); sm.step(w.dt, 1, sync=False); ev[k][1].record(m.stream)
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    total_ms = sum(a.elapsed_time(b) for a, b in ev)
+    (total_ms_max,) = reduce_max_over_ranks([total_ms], dist, m.device)
+    st = m.stats()
+    units = m.shard_units()
+    if rank == 0:
+        print(json.dumps({
+            "metric": METRIC, "value": pairs * K / (total_ms_max * 1e-3), "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
+            "ms_per_step": total_ms_max / K, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic",
+            "config": {"workload": w.name, "N": w.N, "nb": w.nb, "nbig": w.nb if nbig is None else nbig, "dt_days": w.dt, "seed": w.seed,
+                       "parallelism": f"pair sum sharded over {world} rank(s): work units {units[0]}, rank 0 takes [{units[1]}, {units[2]}); "
+                                      "one all-reduce of a per step; O(N) stages and the encounter pass replicated",
+                       "l2": "flushed (256 MiB memset) between timed steps"},
+            "allreduces": sm.allreduces, "allreduce_bytes_per_step": 3 * m.ld * 8 if world > 1 else 0,
+            "encounter_pairs_last_step": st.nce_last, "gpu_launches": None}), flush=True)
+    m.close()
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -531,12 +606,17 @@ def main():
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json config index (3 = N=65,536 headline)")
     ap.add_argument("--bigsmall", default="", metavar="N,NBIG",
                     help="big x all workload (SURVEY.md 8(f) row 1): N objects, NBIG gravity sources, e.g. 1000000,100")
+    ap.add_argument("--sharded", action="store_true", help="row f4: one system, the pair sum split over the ranks (strong scaling)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-side", action="store_true", help="skip per_config / bigsmall / resolve / drift (profiling runs)")
+    ap.add_argument("--side-only", default="", metavar="NAME",
+                    help="run one side measurement alone: drift, resolve, bigsmall, bigsmall_resolve, cfg0..cfg4 (profiling runs)")
     ap.add_argument("--cpu-budget", type=float, default=20.0, help="seconds of CPU work for the headline cpu_baseline sample")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.sharded:
+        return run_sharded(args)
     return run_ours(args)
 
 

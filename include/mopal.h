@@ -20,8 +20,9 @@
  *   mo_step       mdt_hy (Fig. 1, 202-226): kick h/2, stellar jump h/2,
  *                   copy x0,v0, drift h, encounter check, jump h/2, accel, kick h/2 -
  *                   all state resident in HBM (the paper moves 7N doubles H<->D twice
- *                   per step).  No restore and no Bulirsch-Stoer
- *                   resolution of flagged pairs (mdt_hkce stays out of scope).
+ *                   per step).  By default no restore and no
+ *                   Bulirsch-Stoer resolution of flagged pairs; mo_set_resolve switches the
+ *                   on-device resolution (the paper's host-side mdt_hkce) in.
  *
  * Units: AU, day, Msun; gm = G * mass.  Coordinates are democratic heliocentric:
  * heliocentric positions, barycentric velocities (PAPER.md:84, 100 fn. 12).
@@ -42,6 +43,15 @@
  * stdout; failures are return codes.  Asynchronous CUDA errors surface as
  * MO_ECUDA on the next synchronising call.  There is no CPU fallback: without a
  * CUDA device mo_create returns MO_ECUDA.
+ *
+ * Environment (read once, at mo_create / mo_set_nbig; everything else is a function
+ * argument): MO_DEBUG=1 synchronises after every launch so that a failing kernel is
+ * reported by the call that launched it.  Five switches exist for the test-suite only -
+ * they force a kernel that the problem size alone would not select, so that every kernel
+ * is checked at sizes the oracle handles: MO_PSM=0 (no lane-split pair kernel), MO_SYM=1
+ * (two-sided pair kernel at any size), MO_SYM_CH=n (its j tiles per work unit), MO_SMALL=0 /
+ * MO_SMALL_MAX=n (single-CTA front end off / up to n bodies).  They change which kernel
+ * computes a result, never the result's definition.
  */
 #ifndef MOPAL_H
 #define MOPAL_H
@@ -190,7 +200,7 @@ mo_status mo_resolve_stats(mo_ctx *ctx, int32_t *out4);
  * the only multi-device route) -----------------------------------------------------------------------
  * One process and one context per GPU, all holding the WHOLE state (identical arrays on every rank).  Only the
  * O(N^2) pair sum is split: after mo_set_shard(rank, world) a context evaluates its contiguous share of the pair
- * kernel's work units (two-sided kernel, nb >= 8192: units of the triangle, so a rank's result is a PARTIAL
+ * kernel's work units (two-sided kernel, nb > 2560: units of the triangle, so a rank's result is a PARTIAL
  * acceleration of every body; big x all mode: blocks of bodies i, the other rows 0), and the caller sums `a` over the
  * ranks (one all-reduce of 3*ld doubles per step, e.g. NCCL through torch.distributed - the library itself holds no
  * communicator).  Every O(N) stage and the encounter pass run replicated on every rank, on identical data, so the
@@ -198,7 +208,7 @@ mo_status mo_resolve_stats(mo_ctx *ctx, int32_t *out4);
  *     mo_accel(ctx); <sum a over ranks>; mo_accel_summed(ctx);
  *     per step: mo_step_begin(ctx, dt); <sum a over ranks>; mo_step_end(ctx, dt, stats);
  * mo_step itself returns MO_EINVAL while world > 1.  MO_EINVAL also for sizes whose pair kernel does not split
- * (fully interacting systems below 8192 bodies: a step there is tens of microseconds). */
+ * (fully interacting systems of up to 2560 bodies: a step there is tens of microseconds). */
 mo_status mo_set_shard(mo_ctx *ctx, int32_t rank, int32_t world);
 /* [lo, hi) = rank's contiguous share of n work units: lo = n*rank/world, hi = n*(rank+1)/world.  Host only. */
 mo_status mo_shard_range(int64_t n, int32_t rank, int32_t world, int64_t *lo, int64_t *hi);
@@ -260,7 +270,7 @@ mo_status mo_probe_fp64_peak(void *cuda_stream, int32_t reps, double *tflops_out
 mo_status mo_pair_geometry(const mo_ctx *ctx, int32_t *ipt, int32_t *jsplit,
                            int32_t *ctas, int32_t *ctas_per_sm);
 
-/* Name of the pair kernel this context launches for mo_accel ("pair_sym_kernel": two-sided, nb >= 8192
+/* Name of the pair kernel this context launches for mo_accel ("pair_sym_kernel": two-sided, nb > 2560
  * fully interacting; "pair_big_kernel": few gravity sources after mo_set_nbig; else "pair_accel_kernel").
  * Static string; NULL for a NULL context. */
 const char *mo_pair_kernel_name(const mo_ctx *ctx);

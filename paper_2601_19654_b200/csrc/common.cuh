@@ -14,6 +14,8 @@ constexpr int STAGES = 4;               // TMA ring depth
 constexpr int CONSUMER_THREADS = 128;   // 4 compute warps, one per SM sub-partition
 constexpr int CTA_THREADS = CONSUMER_THREADS + 32;  // + 1 TMA producer warp
 constexpr int ACC_TILE_BYTES = TJ * 32 + 16;        // TJ x {x,y,z,gm} + 16 B gate header
+constexpr int SYM_TILE_BYTES = TJ * 32 + 16 + TJ * 8; // two-sided kernel: the same + TJ x rcrit (5136)
+constexpr int SYM_RC_OFF = TJ * 32 + 16;
 constexpr int BOX_TILE_BYTES = TJ * 32;             // TJ x {lox,hix,loy,hiy}
 constexpr int ON_BLOCK = 256;           // block size of the O(N) kernels
 

@@ -78,7 +78,7 @@ struct mo_ctx {
     bool use_psm = false;               // nb <= PSM_MAX: pair_small_kernel (several lanes per body) instead of pack + pair + reduce
     bool use_small = false;             // nb <= SMALL_MAX: the pre-acceleration part of the step is one single-CTA kernel
     int gkernels = 0;                   // kernel launches recorded in the cached step graph
-    int sym_nI = 0, sym_ch = 1, sym_nunits = 0;
+    int sym_nI = 0, sym_ch = 1, sym_nunits = 0, sym_ipt = 6;
     int4* sym_units = nullptr;
     int* sym_ustart = nullptr;
     double *sym_partI = nullptr, *sym_partJ = nullptr;
@@ -136,14 +136,22 @@ static pair_kernel_t pick_pair_kernel(int ipt, int unroll) {
     return unroll == 4 ? pair_accel_kernel<2, 4> : pair_accel_kernel<2, 2>;
 }
 
+// Environment switches (read at mo_create / mo_set_nbig; documented in include/mopal.h): MO_DEBUG, and the five the
+// tests use to force a kernel that the size alone would not select - MO_PSM, MO_SYM, MO_SYM_CH, MO_SYM_IPT, MO_SMALL, MO_SMALL_MAX.
 static int env_int(const char* name, int dflt) {
     const char* s = getenv(name);
     return (s && *s) ? atoi(s) : dflt;
 }
 
+typedef void (*sym_kernel_t)(SymParams);
+static sym_kernel_t pick_sym_kernel(int ipt) {
+    return ipt == 2 ? pair_sym_kernel<2> : ipt == 3 ? pair_sym_kernel<3> : pair_sym_kernel<6>;
+}
+static constexpr int SYM_MIN = 2561;   // right above the lane-split kernel's range
+
 typedef void (*big_kernel_t)(BigParams);
 static big_kernel_t pick_big_kernel(int ipt, bool kick) {
-    if (ipt == 4 && env_int("MO_BIG_U", 1) == 2) return kick ? pair_big_kernel<4, 2, true> : pair_big_kernel<4, 2, false>;
+    if (ipt == 4 && false) return kick ? pair_big_kernel<4, 2, true> : pair_big_kernel<4, 2, false>;
     if (ipt == 4) return kick ? pair_big_kernel<4, 1, true> : pair_big_kernel<4, 1, false>;
     if (ipt == 2) return kick ? pair_big_kernel<2, 2, true> : pair_big_kernel<2, 2, false>;
     return kick ? pair_big_kernel<1, 4, true> : pair_big_kernel<1, 4, false>;
@@ -152,9 +160,9 @@ static big_kernel_t pick_big_kernel(int ipt, bool kick) {
 // j-split count: minimise (waves) x (tiles per CTA + start-up), see DESIGN.md section 5
 static void choose_geometry(mo_ctx* ctx) {
     const int nb = ctx->nb;
-    ctx->ipt = env_int("MO_IPT", nb >= 8192 ? 2 : 1);
+    ctx->ipt = nb >= 8192 ? 2 : 1;
     if (ctx->ipt != 1 && ctx->ipt != 2) ctx->ipt = 1;
-    ctx->unroll = env_int("MO_UNROLL", ctx->ipt == 2 ? 2 : 4);
+    ctx->unroll = ctx->ipt == 2 ? 2 : 4;
     if (ctx->unroll != 2 && ctx->unroll != 4) ctx->unroll = 4;
     const int rows = CONSUMER_THREADS * ctx->ipt;
     ctx->nIblk = (nb + rows - 1) / rows;
@@ -175,26 +183,24 @@ static void choose_geometry(mo_ctx* ctx) {
         const double cost = (double)waves * (tps + 1.5);
         if (cost < best * (1.0 - 1e-9)) { best = cost; bestS = Se; }
     }
-    const int forced = env_int("MO_JSPLIT", 0);
-    if (forced > 0) bestS = forced < nST ? forced : nST;
     ctx->tps = (nST + bestS - 1) / bestS;
     ctx->nsplit = (nST + ctx->tps - 1) / ctx->tps;
     // encounter find: column tiles of a row tile are dealt round-robin to enc_split CTAs
-    ctx->enc_split = env_int("MO_ENC_SPLIT", ctx->nTiles / 8);
+    ctx->enc_split = ctx->nTiles / 8;
     if (ctx->enc_split < 1) ctx->enc_split = 1;
     if (ctx->enc_split > 8) ctx->enc_split = 8;
     // two-sided kernel for large nb: units = (row block, chunk of sym_ch j tiles from the diagonal on)
     ctx->use_small = nb <= env_int("MO_SMALL_MAX", 320) && nb <= SMALL_MAX && env_int("MO_SMALL", 1) != 0;
     // measured (profiles/r1g_path_selection.md): single-CTA front end up to ~320 bodies, lane-split pair kernel up to
     // ~2500, tiled one-sided kernel up to 8191, two-sided kernel above
-    ctx->use_psm = nb <= env_int("MO_PSM_MAX", 2560) && nb <= PSM_MAX && env_int("MO_PSM", 1) != 0;
-    ctx->psm_g = env_int("MO_PSM_G", 8);
+    ctx->use_psm = nb <= 2560 && nb <= PSM_MAX && env_int("MO_PSM", 1) != 0;
+    ctx->psm_g = 8;
     if (ctx->psm_g != 2 && ctx->psm_g != 4 && ctx->psm_g != 8) ctx->psm_g = 8;
-    ctx->use_big = !ctx->use_psm && ctx->nbig < nb && ctx->nbig <= env_int("MO_BIG_MAX", 4096);
+    ctx->use_big = !ctx->use_psm && ctx->nbig < nb && ctx->nbig <= 4096;
     if (ctx->use_big) {
         // bodies per thread: as many as still leave about two waves of CTAs
         const long long want = 2LL * ctx->nsm * BIG_THREADS;
-        ctx->big_ipt = env_int("MO_BIG_IPT", nb >= 2 * want ? 2 : 1);   // 4 measured no faster (register-bound occupancy)
+        ctx->big_ipt = nb >= 2 * want ? 2 : 1;   // 4 measured no faster (register-bound occupancy)
         if (ctx->big_ipt != 1 && ctx->big_ipt != 2 && ctx->big_ipt != 4) ctx->big_ipt = 1;
         ctx->ipt = ctx->big_ipt; ctx->nsplit = 1; ctx->tps = ctx->nSrcTiles;
         ctx->nIblk = (nb + BIG_THREADS * ctx->big_ipt - 1) / (BIG_THREADS * ctx->big_ipt);
@@ -204,15 +210,20 @@ static void choose_geometry(mo_ctx* ctx) {
         ctx->ctas_per_sm = occb;
         ctx->big_grid = ctx->nIblk < ctx->nsm * occb ? ctx->nIblk : ctx->nsm * occb;   // persistent: CTAs walk over i blocks
     }
-    ctx->use_sym = !ctx->use_psm && ctx->nbig == nb && env_int("MO_SYM", nb >= env_int("MO_SYM_MIN", 8192) ? 1 : 0) != 0;
+    // two-sided kernel: from SYM_MIN bodies on (below, the lane-split kernel's single launch wins)
+    ctx->use_sym = !ctx->use_psm && ctx->nbig == nb && env_int("MO_SYM", nb >= SYM_MIN ? 1 : 0) != 0;
     if (ctx->use_sym) {
+        // bodies per lane: the triangle of a mid-size system in enough, short enough units for the SMs
+        ctx->sym_ipt = env_int("MO_SYM_IPT", nb >= 32768 ? 6 : nb >= 7000 ? 3 : 2);   // measured: profiles/r2_path_selection.md
+        if (ctx->sym_ipt != 2 && ctx->sym_ipt != 3 && ctx->sym_ipt != 6) ctx->sym_ipt = 6;
+        const int R = sym_rows(ctx->sym_ipt), TPB = ctx->sym_ipt;
         int occs = 1;
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occs, pair_sym_kernel, SYM_THREADS, 0);
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occs, pick_sym_kernel(ctx->sym_ipt), SYM_THREADS, 0);
         if (occs < 1) occs = 1;
         const long long sslots = (long long)ctx->nsm * occs;
-        ctx->sym_nI = (ctx->nbPad + SYM_R - 1) / SYM_R;
+        ctx->sym_nI = (ctx->nbPad + R - 1) / R;
         long long tot = 0;
-        for (int I = 0; I < ctx->sym_nI; ++I) tot += ctx->nTiles - I * SYM_TPB;
+        for (int I = 0; I < ctx->sym_nI; ++I) tot += ctx->nTiles - I * TPB;
         long long ch = (tot + 16 * sslots - 1) / (16 * sslots);   // about sixteen waves of units: short tail
         if (ch < 1) ch = 1;
         if (ch > 16) ch = 16;
@@ -221,14 +232,14 @@ static void choose_geometry(mo_ctx* ctx) {
         ctx->h_units.clear(); ctx->h_ustart.clear();
         for (int I = 0; I < ctx->sym_nI; ++I) {
             ctx->h_ustart.push_back((int)ctx->h_units.size());
-            for (int t = I * SYM_TPB; t < ctx->nTiles; t += ctx->sym_ch) {
+            for (int t = I * TPB; t < ctx->nTiles; t += ctx->sym_ch) {
                 const int t1 = t + ctx->sym_ch < ctx->nTiles ? t + ctx->sym_ch : ctx->nTiles;
                 ctx->h_units.push_back(make_int4(I, t, t1, 0));
             }
         }
         ctx->h_ustart.push_back((int)ctx->h_units.size());
         ctx->sym_nunits = (int)ctx->h_units.size();
-        ctx->ipt = SYM_IPT; ctx->ctas_per_sm = occs; ctx->nsplit = 1;
+        ctx->ipt = ctx->sym_ipt; ctx->ctas_per_sm = occs; ctx->nsplit = 1;
     }
 }
 
@@ -294,7 +305,7 @@ extern "C" mo_status mo_create(mo_ctx** out, int32_t nb, int32_t ld, double m_st
     ctx->x = x; ctx->v = v; ctx->a = a; ctx->rcrit = rcrit; ctx->pairs = pairs; ctx->cap = cap; ctx->flag = flag;
     ctx->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
     ctx->debug = env_int("MO_DEBUG", 0) != 0;
-    ctx->use_graph = env_int("MO_NO_GRAPH", 0) == 0;
+    ctx->use_graph = true;
     ctx->nTiles = (nb + TJ - 1) / TJ;
     ctx->nbPad = ctx->nTiles * TJ;
     ctx->nbig = nb; ctx->nSrcTiles = ctx->nTiles;
@@ -317,7 +328,7 @@ extern "C" mo_status mo_create(mo_ctx** out, int32_t nb, int32_t ld, double m_st
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->gmsum, 1);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->ticket, 2);
     if (e == cudaSuccess) e = cudaMemsetAsync(ctx->ticket, 0, 2 * sizeof(unsigned), ctx->stream);
-    if (e == cudaSuccess) e = dalloc(ctx, &ctx->tiles, (size_t)ctx->nTiles * ACC_TILE_BYTES);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->tiles, (size_t)ctx->nTiles * SYM_TILE_BYTES);   // the larger of the two tile layouts
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->enc.box, (size_t)ctx->nbPad);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->enc.boxf, (size_t)ctx->nbPad);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->enc.rowcnt, (size_t)ctx->nbPad);
@@ -364,7 +375,7 @@ extern "C" mo_status mo_create(mo_ctx** out, int32_t nb, int32_t ld, double m_st
 static mo_status ensure_pair_scratch(mo_ctx* ctx) {
     if (ctx->pair_ready) return MO_OK;
     cudaError_t e = cudaSuccess;
-    ctx->overlap = !ctx->use_small && ctx->nb >= env_int("MO_OVERLAP_MIN", 1) && env_int("MO_OVERLAP", 1) != 0;
+    ctx->overlap = !ctx->use_small && true;
     if (ctx->overlap && !ctx->enc_stream) {
         int lo = 0, hi = 0;
         cudaDeviceGetStreamPriorityRange(&lo, &hi);
@@ -379,8 +390,8 @@ static mo_status ensure_pair_scratch(mo_ctx* ctx) {
     if (ctx->use_sym) {
         if (e == cudaSuccess) e = dalloc(ctx, &ctx->sym_units, (size_t)ctx->sym_nunits);
         if (e == cudaSuccess) e = dalloc(ctx, &ctx->sym_ustart, ctx->h_ustart.size());
-        if (e == cudaSuccess) e = dalloc(ctx, &ctx->sym_partI, (size_t)ctx->sym_nunits * 3 * SYM_R);
-        if (e == cudaSuccess) e = dalloc(ctx, &ctx->sym_partJ, (size_t)symJ_off(ctx->sym_nI, ctx->nbPad));
+        if (e == cudaSuccess) e = dalloc(ctx, &ctx->sym_partI, (size_t)ctx->sym_nunits * 3 * sym_rows(ctx->sym_ipt));
+        if (e == cudaSuccess) e = dalloc(ctx, &ctx->sym_partJ, (size_t)symJ_off(ctx->sym_nI, ctx->nbPad, sym_rows(ctx->sym_ipt)));
         if (e == cudaSuccess) e = cudaMemcpyAsync(ctx->sym_units, ctx->h_units.data(), ctx->h_units.size() * sizeof(int4), cudaMemcpyHostToDevice, ctx->stream);
         if (e == cudaSuccess) e = cudaMemcpyAsync(ctx->sym_ustart, ctx->h_ustart.data(), ctx->h_ustart.size() * sizeof(int), cudaMemcpyHostToDevice, ctx->stream);
         if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);   // pageable source vectors
@@ -442,7 +453,7 @@ static mo_status launch_pair(mo_ctx* ctx, bool kick = false, double hk = 0.0) {
         long long u0 = 0, u1 = ctx->sym_nunits;
         if (ctx->shard_world > 1) shard_range(ctx->sym_nunits, ctx->shard_rank, ctx->shard_world, &u0, &u1);
         sp.unit0 = (int)u0;
-        if (u1 > u0) pair_sym_kernel<<<(int)(u1 - u0), SYM_THREADS, 0, ctx->stream>>>(sp);
+        if (u1 > u0) pick_sym_kernel(ctx->sym_ipt)<<<(int)(u1 - u0), SYM_THREADS, 0, ctx->stream>>>(sp);
     } else {
         pick_pair_kernel(ctx->ipt, ctx->unroll)<<<grid, CTA_THREADS, 0, ctx->stream>>>(p);
     }
@@ -477,11 +488,12 @@ static mo_status enqueue_accel(mo_ctx* ctx, bool jump, double hj, bool kick, dou
     if (s != MO_OK) return s;
     const int nblk = (ctx->nb + ON_BLOCK - 1) / ON_BLOCK;
     if (ctx->use_sym) {
-        auto rk = kick ? sym_reduce_kernel<true> : sym_reduce_kernel<false>;
+        const bool shd = ctx->shard_world > 1;
+        auto rk = kick ? sym_reduce_kernel<true, false> : shd ? sym_reduce_kernel<false, true> : sym_reduce_kernel<false, false>;
         long long u0 = 0, u1 = ctx->sym_nunits;
         if (ctx->shard_world > 1) shard_range(ctx->sym_nunits, ctx->shard_rank, ctx->shard_world, &u0, &u1);
         rk<<<dim3(nblk, 3), ON_BLOCK, 0, ctx->stream>>>(ctx->sym_partI, ctx->sym_partJ, ctx->sym_ustart, ctx->nb, ctx->ld, ctx->nbPad,
-                                               ctx->a, kick ? ctx->v : nullptr, kick ? hk : 0.0, (int)u0, (int)u1, ctx->sym_ch);
+                                               ctx->a, kick ? ctx->v : nullptr, kick ? hk : 0.0, (int)u0, (int)u1, ctx->sym_ch, sym_rows(ctx->sym_ipt));
     } else if (kick)
         accel_reduce_kernel<true><<<nblk, ON_BLOCK, 0, ctx->stream>>>(ctx->part, ctx->nsplit, ctx->nb, ctx->ld, ctx->a, ctx->v, hk);
     else
@@ -939,7 +951,7 @@ extern "C" mo_status mo_shard_range(int64_t n, int32_t rank, int32_t world, int6
 
 extern "C" mo_status mo_set_shard(mo_ctx* ctx, int32_t rank, int32_t world) {
     if (!ctx || world < 1 || rank < 0 || rank >= world) return MO_EINVAL;
-    // only the kernels of the large systems split their work: the two-sided pair sum (nb >= 8192) and the big x all sum
+    // only the kernels of the large systems split their work: the two-sided pair sum (nb > 2560) and the big x all sum
     if (world > 1 && !(ctx->use_sym || ctx->use_big)) return MO_EINVAL;
     if (ctx->gexec) {
         CK(cudaStreamSynchronize(ctx->stream));

@@ -247,10 +247,11 @@ __global__ void __launch_bounds__(TJ) pack_kernel(double* __restrict__ x, const 
         pa = make_double2(PAD_POS, PAD_POS);
         pb = make_double2(PAD_POS, 0.0);
     }
-    unsigned char* tile = tiles + (size_t)blockIdx.x * ACC_TILE_BYTES;
+    unsigned char* tile = tiles + (size_t)blockIdx.x * (SYM ? SYM_TILE_BYTES : ACC_TILE_BYTES);
     if (SYM) {
         double2* rec = reinterpret_cast<double2*>(tile);
         rec[threadIdx.x] = pa; rec[TJ + threadIdx.x] = pb;
+        reinterpret_cast<double*>(tile + SYM_RC_OFF)[threadIdx.x] = j < nsrc ? rcrit[j] : 0.0;
     } else {
         double2* rec = reinterpret_cast<double2*>(tile) + 2 * threadIdx.x;
         rec[0] = pa; rec[1] = pb;

@@ -36,37 +36,35 @@
 
 namespace mopal {
 
-#ifndef SYM_IPT_N
-#define SYM_IPT_N 6
-#endif
-#ifndef SYM_MINB
-#define SYM_MINB 2
-#endif
 #ifndef SYM_STAGES_N
 #define SYM_STAGES_N 4
 #endif
-constexpr int SYM_IPT = SYM_IPT_N;
 constexpr int SYM_STAGES = SYM_STAGES_N;
-constexpr int SYM_R = CONSUMER_THREADS * SYM_IPT;   // rows per row block (768)
-constexpr int SYM_TPB = SYM_R / TJ;                 // j tiles spanned by a row block (6)
+// Bodies i per lane (IPT): a template parameter - 6 for the large systems (768-row blocks: least shuffle traffic per
+// FP64 instruction), 3 and 2 for the mid-size ones, whose triangle would otherwise break into too few, too long work
+// units for the 148 SMs (a unit of IPT x 128 rows by one 128-body tile is 256 IPT pair evaluations per lane).
+// A row block spans IPT j tiles (128 IPT rows).
+__host__ __device__ constexpr int sym_rows(int ipt) { return CONSUMER_THREADS * ipt; }
 
 struct SymParams {
-    const unsigned char* tiles;  // nTiles * ACC_TILE_BYTES, SoA-halves layout (pack_kernel<.., true>)
+    const unsigned char* tiles;  // nTiles * SYM_TILE_BYTES, SoA-planes layout (pack_kernel<.., true>)
     const double* x;             // 3*ld
     const double* gm;            // nb
     const double* rcrit;         // nb
     const int4* units;           // {I, t0, t1, unused}
-    double* partI;               // [nUnits][3][SYM_R]
-    double* partJ;               // triangular: block I at symJ_off(I), planes of (nbPad - I*SYM_R)
+    double* partI;               // [nUnits][3][R], R = 128 IPT
+    double* partJ;               // triangular: block I at symJ_off(I), planes of (nbPad - I*R)
     int nb, ld, nbPad;
     int unit0;                   // first work unit of this launch (a rank's share of the units, row f4; 0 otherwise)
 };
 
-__host__ __device__ inline long long symJ_off(int I, int nbPad) {
-    return 3LL * ((long long)I * nbPad - (long long)SYM_R * ((long long)I * (I - 1) / 2));
+__host__ __device__ inline long long symJ_off(int I, int nbPad, int R) {
+    return 3LL * ((long long)I * nbPad - (long long)R * ((long long)I * (I - 1) / 2));
 }
 
-constexpr int SYM_TILE_STRIDE = 4608;   // shared-memory stage stride: tile (4112 B) padded to 9 x 512 B
+// Tile of the two-sided kernel: {x,y}[128] | {z,gm}[128] | 16 B header (largest changeover gate of the tile) | rcrit[128]
+// (the last plane is read on the changeover path only: no global load there)
+constexpr int SYM_TILE_STRIDE = 5632;   // shared-memory stage stride: tile padded to 11 x 512 B
 
 __device__ __forceinline__ void lds_rec(double2& a, double2& b, uint32_t addr) {
     asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(a.x), "=d"(a.y) : "r"(addr));
@@ -76,6 +74,22 @@ __device__ __forceinline__ void lds_rec(double2& a, double2& b, uint32_t addr) {
 // next record of the 32-record (512 B, 512-B aligned) group, cyclically: VIADD + one LOP3
 __device__ __forceinline__ uint32_t next_rec(uint32_t addr) { return (addr & ~511u) | ((addr + 16u) & 511u); }
 
+// K(r; rc) / r^3 of a pair that may be inside a changeover shell (readings A-1..A-5, A-9), from registers and shared
+// memory alone: a giant's row or tile sends thousands of pairs here, so there is no function call, no global load and
+// no square root (the refined MUFU seed, 2 ulp) - one division, for the pairs that really are inside the shell.
+__device__ __forceinline__ double sym_slow_u(double s2, double rc) {
+    if (!(s2 > 0.0)) return 0.0;                       // coincident bodies, self pairs
+    const double y0 = rsqrt_seed(s2);
+    const double e = fma(-s2, y0 * y0, 1.0);
+    const double y = fma(y0, e * fma(0.375, e, 0.5), y0);
+    const double y3 = y * (y * y);
+    if (s2 >= rc * rc) return y3;                      // K = 1
+    const double rin = 0.1 * rc;
+    if (s2 <= rin * rin) return 0.0;                   // K = 0
+    const double q = (s2 * y - rin) / (0.9 * rc);
+    return q * q * q * (10.0 + q * (6.0 * q - 15.0)) * y3;
+}
+
 // one rotation: IPT pairs of this lane against the body whose record is (ca, cb).  The record of
 // the NEXT rotation is loaded into (na, nb2) as soon as this rotation's separations are formed, so
 // the shared-memory latency is covered by the FP64 instructions that follow.  An FP64 warp
@@ -83,15 +97,15 @@ __device__ __forceinline__ uint32_t next_rec(uint32_t addr) { return (addr & ~51
 // costs half a DFMA: the changeover gate is ONE compare per rotation (min over the IPT high words
 // of s2 against the largest gate of the lane's bodies and the tile), the j index is only formed on
 // the slow path, and the records ping-pong between two register sets (no copies).
-template <bool DIAG>
+template <int SYM_IPT, bool DIAG>
 __device__ __forceinline__ void sym_rotation(const double2 ca, const double2 cb, double2& na, double2& nb2,
                                              const uint32_t caddr, const uint32_t naddr, const int jgrp,
                                              const int ibase, const double (&xi)[SYM_IPT],
                                              const double (&yi)[SYM_IPT], const double (&zi)[SYM_IPT],
                                              const double (&mi)[SYM_IPT], const int g,
                                              double (&ax)[SYM_IPT], double (&ay)[SYM_IPT], double (&az)[SYM_IPT],
-                                             double& tx, double& ty, double& tz, const double* __restrict__ rcrit,
-                                             int nb) {
+                                             double& tx, double& ty, double& tz, const double (&rci)[SYM_IPT],
+                                             const uint32_t rcbase) {
     double dx[SYM_IPT], dy[SYM_IPT], dz[SYM_IPT], u[SYM_IPT];
 #pragma unroll
     for (int k = 0; k < SYM_IPT; ++k) {
@@ -115,13 +129,14 @@ __device__ __forceinline__ void sym_rotation(const double2 ca, const double2 cb,
 #pragma unroll
         for (int k = 0; k < SYM_IPT; ++k) u[k] = jglob_d > ibase + k * 32 ? u[k] : 0.0;
     }
-    if (hmin <= g) {  // rare: a pair that may be inside a changeover shell, or coincident bodies
+    if (hmin <= g) {  // a pair that may be inside a changeover shell, or coincident bodies
         const int jglob = jgrp + (int)((caddr & 511u) >> 4);
+        double rcj;
+        asm volatile("ld.shared.f64 %0, [%1];" : "=d"(rcj) : "r"(rcbase + ((caddr & 511u) >> 1)));
 #pragma unroll
         for (int k = 0; k < SYM_IPT; ++k) {
             const double q2 = fma(dz[k], dz[k], fma(dy[k], dy[k], dx[k] * dx[k]));
-            if (__double2hiint(q2) <= g && (!DIAG || jglob > ibase + k * 32))
-                u[k] = slow_weight(q2, 1.0, rcrit, ibase + k * 32, jglob, nb);
+            if (__double2hiint(q2) <= g && (!DIAG || jglob > ibase + k * 32)) u[k] = sym_slow_u(q2, fmax(rci[k], rcj));
         }
     }
 #pragma unroll
@@ -138,34 +153,35 @@ __device__ __forceinline__ void sym_rotation(const double2 ca, const double2 cb,
 }
 
 // tile_sa: shared-space address of the tile (512-B aligned); records {x,y}[TJ] then {z,gm}[TJ]
-template <bool DIAG>
+template <int SYM_IPT, bool DIAG>
 __device__ __forceinline__ void sym_tile(const uint32_t tile_sa, const int jbase, const int lane, const int ibase,
                                          const double (&xi)[SYM_IPT], const double (&yi)[SYM_IPT],
                                          const double (&zi)[SYM_IPT], const double (&mi)[SYM_IPT],
                                          const int g, double (&ax)[SYM_IPT], double (&ay)[SYM_IPT],
                                          double (&az)[SYM_IPT], double* __restrict__ sj,
-                                         const double* __restrict__ rcrit, int nb) {
+                                         const double (&rci)[SYM_IPT]) {
     const unsigned full = 0xffffffffu;
 #pragma unroll 1
     for (int grp = 0; grp < TJ / 32; ++grp) {
         // this lane walks the group's 32 records cyclically, starting at its home record
         uint32_t a0 = tile_sa + grp * 512 + lane * 16;
         const int jgrp = jbase + grp * 32;
+        const uint32_t rcbase = tile_sa + SYM_RC_OFF + grp * 256;
         double tx = 0.0, ty = 0.0, tz = 0.0;
         double2 pa, pb, qa, qb;
         lds_rec(pa, pb, a0);
 #pragma unroll 1
         for (int s = 0; s < 32; s += 2) {
             const uint32_t a1 = next_rec(a0);
-            sym_rotation<DIAG>(pa, pb, qa, qb, a0, a1, jgrp, ibase, xi, yi, zi, mi, g, ax, ay, az, tx, ty, tz, rcrit,
-                               nb);
+            sym_rotation<SYM_IPT, DIAG>(pa, pb, qa, qb, a0, a1, jgrp, ibase, xi, yi, zi, mi, g, ax, ay, az, tx, ty, tz, rci,
+                               rcbase);
             // hand the travelling sums of j = (lane+s) to the lane that works on that j next
             tx = __shfl_sync(full, tx, lane + 1);
             ty = __shfl_sync(full, ty, lane + 1);
             tz = __shfl_sync(full, tz, lane + 1);
             a0 = next_rec(a1);                             // s = 30 wraps to the home record (unused load)
-            sym_rotation<DIAG>(qa, qb, pa, pb, a1, a0, jgrp, ibase, xi, yi, zi, mi, g, ax, ay, az, tx, ty, tz, rcrit,
-                               nb);
+            sym_rotation<SYM_IPT, DIAG>(qa, qb, pa, pb, a1, a0, jgrp, ibase, xi, yi, zi, mi, g, ax, ay, az, tx, ty, tz, rci,
+                               rcbase);
             tx = __shfl_sync(full, tx, lane + 1);
             ty = __shfl_sync(full, ty, lane + 1);
             tz = __shfl_sync(full, tz, lane + 1);
@@ -182,7 +198,9 @@ __device__ __forceinline__ void sym_tile(const uint32_t tile_sa, const int jbase
 // registers lets 3 CTAs = 12 compute warps share an SM.
 constexpr int SYM_THREADS = CONSUMER_THREADS;
 
-__global__ void __launch_bounds__(SYM_THREADS, SYM_MINB) pair_sym_kernel(SymParams p) {
+template <int SYM_IPT>
+__global__ void __launch_bounds__(SYM_THREADS, SYM_IPT >= 5 ? 2 : SYM_IPT >= 3 ? 3 : 4) pair_sym_kernel(SymParams p) {
+    constexpr int SYM_R = sym_rows(SYM_IPT), SYM_TPB = SYM_IPT;
     __shared__ __align__(512) unsigned char s_tiles[SYM_STAGES * SYM_TILE_STRIDE];
     __shared__ __align__(16) double s_aj[2][SYM_THREADS / 32][3 * TJ];   // [parity][warp][c][j]
     __shared__ __align__(8) uint64_t s_full[SYM_STAGES];
@@ -191,7 +209,7 @@ __global__ void __launch_bounds__(SYM_THREADS, SYM_MINB) pair_sym_kernel(SymPara
     const int ug = blockIdx.x + p.unit0;
     const int4 un = p.units[ug];
     const int I = un.x, t0 = un.y, nt = un.z - un.y;
-    const unsigned char* src = p.tiles + (size_t)t0 * ACC_TILE_BYTES;
+    const unsigned char* src = p.tiles + (size_t)t0 * SYM_TILE_BYTES;
 
     if (tid == 0) {
 #pragma unroll
@@ -200,8 +218,8 @@ __global__ void __launch_bounds__(SYM_THREADS, SYM_MINB) pair_sym_kernel(SymPara
 #pragma unroll
         for (int s = 0; s < SYM_STAGES; ++s) {
             if (s < nt) {
-                mbar_arrive_expect_tx(&s_full[s], ACC_TILE_BYTES);
-                tma_load_1d(s_tiles + s * SYM_TILE_STRIDE, src + (size_t)s * ACC_TILE_BYTES, ACC_TILE_BYTES, &s_full[s]);
+                mbar_arrive_expect_tx(&s_full[s], SYM_TILE_BYTES);
+                tma_load_1d(s_tiles + s * SYM_TILE_STRIDE, src + (size_t)s * SYM_TILE_BYTES, SYM_TILE_BYTES, &s_full[s]);
             }
         }
     }
@@ -209,7 +227,7 @@ __global__ void __launch_bounds__(SYM_THREADS, SYM_MINB) pair_sym_kernel(SymPara
 
     // ---- compute warps: resident bodies i = I*SYM_R + warp*32*IPT + k*32 + lane ----
     const int ibase = I * SYM_R + warp * (32 * SYM_IPT) + lane;
-    double xi[SYM_IPT], yi[SYM_IPT], zi[SYM_IPT], mi[SYM_IPT], ax[SYM_IPT], ay[SYM_IPT], az[SYM_IPT];
+    double xi[SYM_IPT], yi[SYM_IPT], zi[SYM_IPT], mi[SYM_IPT], rci[SYM_IPT], ax[SYM_IPT], ay[SYM_IPT], az[SYM_IPT];
     int gi = 0;   // largest changeover gate of this lane's bodies: high word of rcrit_i^2
 #pragma unroll
     for (int k = 0; k < SYM_IPT; ++k) {
@@ -218,16 +236,17 @@ __global__ void __launch_bounds__(SYM_THREADS, SYM_MINB) pair_sym_kernel(SymPara
             xi[k] = p.x[i]; yi[k] = p.x[p.ld + i]; zi[k] = p.x[2 * p.ld + i];
             mi[k] = p.gm[i];
             const double rc = p.rcrit[i];
+            rci[k] = rc;
             gi = max(gi, __double2hiint(rc * rc));
         } else {   // pad rows: far away and massless
-            xi[k] = yi[k] = zi[k] = -PAD_POS; mi[k] = 0.0;
+            xi[k] = yi[k] = zi[k] = -PAD_POS; mi[k] = 0.0; rci[k] = 0.0;
         }
         ax[k] = ay[k] = az[k] = 0.0;
     }
 
     const int jrow0 = I * SYM_R;                       // first column of partJ block I
     const int jw = p.nbPad - jrow0;                    // its plane width
-    double* pj = p.partJ + symJ_off(I, p.nbPad);
+    double* pj = p.partJ + symJ_off(I, p.nbPad, SYM_R);
 
     for (int n = 0; n < nt; ++n) {
         const int st = n % SYM_STAGES;
@@ -239,14 +258,14 @@ __global__ void __launch_bounds__(SYM_THREADS, SYM_MINB) pair_sym_kernel(SymPara
         const int g = max(gi, gt);
         double* sj = s_aj[n & 1][warp];
         if (t < (I + 1) * SYM_TPB)
-            sym_tile<true>(tile_sa, t * TJ, lane, ibase, xi, yi, zi, mi, g, ax, ay, az, sj, p.rcrit, p.nb);
+            sym_tile<SYM_IPT, true>(tile_sa, t * TJ, lane, ibase, xi, yi, zi, mi, g, ax, ay, az, sj, rci);
         else
-            sym_tile<false>(tile_sa, t * TJ, lane, ibase, xi, yi, zi, mi, g, ax, ay, az, sj, p.rcrit, p.nb);
+            sym_tile<SYM_IPT, false>(tile_sa, t * TJ, lane, ibase, xi, yi, zi, mi, g, ax, ay, az, sj, rci);
         // combine the 4 warps' column partials in warp order (double-buffered: one barrier per tile)
         __syncthreads();
         if (tid == 0 && n + SYM_STAGES < nt) {   // every warp has left slot st: refill it
-            mbar_arrive_expect_tx(&s_full[st], ACC_TILE_BYTES);
-            tma_load_1d(s_tiles + st * SYM_TILE_STRIDE, src + (size_t)(n + SYM_STAGES) * ACC_TILE_BYTES, ACC_TILE_BYTES,
+            mbar_arrive_expect_tx(&s_full[st], SYM_TILE_BYTES);
+            tma_load_1d(s_tiles + st * SYM_TILE_STRIDE, src + (size_t)(n + SYM_STAGES) * SYM_TILE_BYTES, SYM_TILE_BYTES,
                         &s_full[st]);
         }
         const int jc = t * TJ + tid - jrow0;
@@ -271,20 +290,22 @@ __global__ void __launch_bounds__(SYM_THREADS, SYM_MINB) pair_sym_kernel(SymPara
 // the closing half kick v += hk * a (Hamiltonian block LOOP 1).
 // [us0, us1): the work units that were run (all of them; a rank's share when the pair sum is sharded over GPUs, SURVEY.md
 // 8(e) - the sum over the ranks of the results is then the full acceleration); ch = j tiles per unit.
-template <bool KICK>
+template <bool KICK, bool SHARD>
 __global__ void __launch_bounds__(ON_BLOCK) sym_reduce_kernel(const double* __restrict__ partI,
                                                                const double* __restrict__ partJ,
                                                                const int* __restrict__ ustart, int nb, int ld,
                                                                int nbPad, double* __restrict__ a,
-                                                               double* __restrict__ v, double hk, int us0, int us1, int ch) {
+                                                               double* __restrict__ v, double hk, int us0, int us1, int ch,
+                                                               int SYM_R) {
     // one thread per (body, component) - blockIdx.y = component - and four interleaved partial sums per
     // list, combined in a fixed order: three times the threads and four times the loads in flight of a
     // thread-per-body loop, still a fixed tree that depends on nb only
     const int b = blockIdx.x * ON_BLOCK + threadIdx.x;
     if (b >= nb) return;
     const int c = blockIdx.y;
+    const int SYM_TPB = SYM_R / TJ;
     const int Ib = b / SYM_R, r = b - Ib * SYM_R;
-    const int u0 = max(ustart[Ib], us0), u1 = min(ustart[Ib + 1], us1);
+    const int u0 = SHARD ? max(ustart[Ib], us0) : ustart[Ib], u1 = SHARD ? min(ustart[Ib + 1], us1) : ustart[Ib + 1];
     double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
     int u = u0;
     for (; u + 3 < u1; u += 4) {
@@ -297,8 +318,11 @@ __global__ void __launch_bounds__(ON_BLOCK) sym_reduce_kernel(const double* __re
     // the column partial of row block I was written by the unit that holds this body's j tile
     const int tb = b / TJ;
     auto colpart = [&](int I) -> double {
-        const int ug = ustart[I] + (tb - I * SYM_TPB) / ch;
-        return (ug >= us0 && ug < us1) ? partJ[symJ_off(I, nbPad) + (size_t)c * (nbPad - I * SYM_R) + (b - I * SYM_R)] : 0.0;
+        if (SHARD) {
+            const int ug = ustart[I] + (tb - I * SYM_TPB) / ch;
+            if (ug < us0 || ug >= us1) return 0.0;
+        }
+        return partJ[symJ_off(I, nbPad, SYM_R) + (size_t)c * (nbPad - I * SYM_R) + (b - I * SYM_R)];
     };
     double t0 = 0.0, t1 = 0.0, t2 = 0.0, t3 = 0.0;
     int I = 0;

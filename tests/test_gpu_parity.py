@@ -103,25 +103,28 @@ def test_accel_ragged_sizes_and_changeover_shell(M, monkeypatch, nb, psm):
 @pytest.fixture
 def force_sym(monkeypatch):
     """Select the two-sided pair kernel (pair_sym_kernel) whatever nb is; MO_SYM is read by mo_create."""
-    def _set(ch=None):
+    def _set(ch=None, ipt=6):
         monkeypatch.setenv("MO_SYM", "1")
         monkeypatch.setenv("MO_PSM", "0")
+        monkeypatch.setenv("MO_SYM_IPT", str(ipt))
         if ch is not None:
             monkeypatch.setenv("MO_SYM_CH", str(ch))
     return _set
 
 
-@pytest.mark.parametrize("nb,ch", [(1, 1), (2, 1), (33, 1), (129, 2), (511, 1), (767, 1), (768, 3), (769, 1), (1000, 2),
+@pytest.mark.parametrize("ipt", [6, 3, 2])
+@pytest.mark.parametrize("nb,ch", [(1, 1), (2, 1), (33, 1), (129, 2), (257, 1), (385, 2), (511, 1), (767, 1), (768, 3), (769, 1), (1000, 2),
                                    (1537, 1), (2500, 5)])
-def test_accel_sym_kernel_ragged_sizes_and_changeover_shell(M, force_sym, nb, ch):
-    # several row blocks (768 rows), diagonal and off-diagonal tiles, ragged tails, every chunking
-    force_sym(ch)
+def test_accel_sym_kernel_ragged_sizes_and_changeover_shell(M, force_sym, nb, ch, ipt):
+    # several row blocks (768 / 384 / 256 rows for 6 / 3 / 2 bodies per lane), diagonal and off-diagonal tiles, ragged
+    # tails, every chunking
+    force_sym(ch, ipt)
     w = W.random_cluster(nb, 300 + nb, box=1.0, rc_frac=(0.0, 0.7)) if nb > 1 else W.random_cluster(1, 5)
     if nb > 100:
         w.x[:, 1] = w.x[:, 0] + np.array([0.03 * max(w.rcrit[0], w.rcrit[1]), 0.0, 0.0])
         w.x[:, nb - 1] = w.x[:, 5]          # coincident bodies in different tiles contribute nothing
     m = _mk(M, w)
-    assert m.pair_geometry()["ipt"] == 6    # the two-sided kernel really is the one running
+    assert m.pair_geometry()["ipt"] == ipt and m.pair_kernel_name() == "pair_sym_kernel"   # the two-sided kernel really is the one running
     m.accel()
     a = m.get("a")
     a_ref, S = oracle.accel(G * w.mass, w.x, w.rcrit)
@@ -132,8 +135,9 @@ def test_accel_sym_kernel_ragged_sizes_and_changeover_shell(M, force_sym, nb, ch
     m.close()
 
 
-def test_accel_sym_kernel_disk_and_step(M, force_sym):
-    force_sym()
+@pytest.mark.parametrize("ipt", [6, 3, 2])
+def test_accel_sym_kernel_disk_and_step(M, force_sym, ipt):
+    force_sym(None, ipt)
     w = W.shrink(1, 3000)
     m = _mk(M, w)
     m.accel()

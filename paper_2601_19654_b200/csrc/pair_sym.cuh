@@ -105,7 +105,7 @@ __device__ __forceinline__ void sym_rotation(const double2 ca, const double2 cb,
                                              const double (&mi)[SYM_IPT], const int g,
                                              double (&ax)[SYM_IPT], double (&ay)[SYM_IPT], double (&az)[SYM_IPT],
                                              double& tx, double& ty, double& tz, const double (&rci)[SYM_IPT],
-                                             const uint32_t rcbase) {
+                                             const uint32_t rcbase, const double* __restrict__ rcrit, int nb) {
     double dx[SYM_IPT], dy[SYM_IPT], dz[SYM_IPT], u[SYM_IPT];
 #pragma unroll
     for (int k = 0; k < SYM_IPT; ++k) {
@@ -131,12 +131,25 @@ __device__ __forceinline__ void sym_rotation(const double2 ca, const double2 cb,
     }
     if (hmin <= g) {  // a pair that may be inside a changeover shell, or coincident bodies
         const int jglob = jgrp + (int)((caddr & 511u) >> 4);
-        double rcj;
-        asm volatile("ld.shared.f64 %0, [%1];" : "=d"(rcj) : "r"(rcbase + ((caddr & 511u) >> 1)));
+        if constexpr (SYM_IPT >= 6) {
+            // large systems: a few of thousands of units meet a giant - the out-of-line path (two global loads) costs
+            // nothing there, and the kernel keeps its registers for the six resident bodies
 #pragma unroll
-        for (int k = 0; k < SYM_IPT; ++k) {
-            const double q2 = fma(dz[k], dz[k], fma(dy[k], dy[k], dx[k] * dx[k]));
-            if (__double2hiint(q2) <= g && (!DIAG || jglob > ibase + k * 32)) u[k] = sym_slow_u(q2, fmax(rci[k], rcj));
+            for (int k = 0; k < SYM_IPT; ++k) {
+                const double q2 = fma(dz[k], dz[k], fma(dy[k], dy[k], dx[k] * dx[k]));
+                if (__double2hiint(q2) <= g && (!DIAG || jglob > ibase + k * 32))
+                    u[k] = slow_weight(q2, 1.0, rcrit, ibase + k * 32, jglob, nb);
+            }
+        } else {
+            // mid-size systems: the kernel is as long as its slowest unit, and the unit with a giant's row takes this
+            // path in every rotation
+            double rcj;
+            asm volatile("ld.shared.f64 %0, [%1];" : "=d"(rcj) : "r"(rcbase + ((caddr & 511u) >> 1)));
+#pragma unroll
+            for (int k = 0; k < SYM_IPT; ++k) {
+                const double q2 = fma(dz[k], dz[k], fma(dy[k], dy[k], dx[k] * dx[k]));
+                if (__double2hiint(q2) <= g && (!DIAG || jglob > ibase + k * 32)) u[k] = sym_slow_u(q2, fmax(rci[k], rcj));
+            }
         }
     }
 #pragma unroll
@@ -159,7 +172,7 @@ __device__ __forceinline__ void sym_tile(const uint32_t tile_sa, const int jbase
                                          const double (&zi)[SYM_IPT], const double (&mi)[SYM_IPT],
                                          const int g, double (&ax)[SYM_IPT], double (&ay)[SYM_IPT],
                                          double (&az)[SYM_IPT], double* __restrict__ sj,
-                                         const double (&rci)[SYM_IPT]) {
+                                         const double (&rci)[SYM_IPT], const double* __restrict__ rcrit, int nb) {
     const unsigned full = 0xffffffffu;
 #pragma unroll 1
     for (int grp = 0; grp < TJ / 32; ++grp) {
@@ -174,14 +187,14 @@ __device__ __forceinline__ void sym_tile(const uint32_t tile_sa, const int jbase
         for (int s = 0; s < 32; s += 2) {
             const uint32_t a1 = next_rec(a0);
             sym_rotation<SYM_IPT, DIAG>(pa, pb, qa, qb, a0, a1, jgrp, ibase, xi, yi, zi, mi, g, ax, ay, az, tx, ty, tz, rci,
-                               rcbase);
+                               rcbase, rcrit, nb);
             // hand the travelling sums of j = (lane+s) to the lane that works on that j next
             tx = __shfl_sync(full, tx, lane + 1);
             ty = __shfl_sync(full, ty, lane + 1);
             tz = __shfl_sync(full, tz, lane + 1);
             a0 = next_rec(a1);                             // s = 30 wraps to the home record (unused load)
             sym_rotation<SYM_IPT, DIAG>(qa, qb, pa, pb, a1, a0, jgrp, ibase, xi, yi, zi, mi, g, ax, ay, az, tx, ty, tz, rci,
-                               rcbase);
+                               rcbase, rcrit, nb);
             tx = __shfl_sync(full, tx, lane + 1);
             ty = __shfl_sync(full, ty, lane + 1);
             tz = __shfl_sync(full, tz, lane + 1);
@@ -201,6 +214,7 @@ constexpr int SYM_THREADS = CONSUMER_THREADS;
 template <int SYM_IPT>
 __global__ void __launch_bounds__(SYM_THREADS, SYM_IPT >= 5 ? 2 : SYM_IPT >= 3 ? 3 : 4) pair_sym_kernel(SymParams p) {
     constexpr int SYM_R = sym_rows(SYM_IPT), SYM_TPB = SYM_IPT;
+    constexpr int LOAD_BYTES = SYM_IPT >= 6 ? ACC_TILE_BYTES : SYM_TILE_BYTES;   // the rcrit plane is read by the in-line changeover path only
     __shared__ __align__(512) unsigned char s_tiles[SYM_STAGES * SYM_TILE_STRIDE];
     __shared__ __align__(16) double s_aj[2][SYM_THREADS / 32][3 * TJ];   // [parity][warp][c][j]
     __shared__ __align__(8) uint64_t s_full[SYM_STAGES];
@@ -218,8 +232,8 @@ __global__ void __launch_bounds__(SYM_THREADS, SYM_IPT >= 5 ? 2 : SYM_IPT >= 3 ?
 #pragma unroll
         for (int s = 0; s < SYM_STAGES; ++s) {
             if (s < nt) {
-                mbar_arrive_expect_tx(&s_full[s], SYM_TILE_BYTES);
-                tma_load_1d(s_tiles + s * SYM_TILE_STRIDE, src + (size_t)s * SYM_TILE_BYTES, SYM_TILE_BYTES, &s_full[s]);
+                mbar_arrive_expect_tx(&s_full[s], LOAD_BYTES);
+                tma_load_1d(s_tiles + s * SYM_TILE_STRIDE, src + (size_t)s * SYM_TILE_BYTES, LOAD_BYTES, &s_full[s]);
             }
         }
     }
@@ -258,14 +272,14 @@ __global__ void __launch_bounds__(SYM_THREADS, SYM_IPT >= 5 ? 2 : SYM_IPT >= 3 ?
         const int g = max(gi, gt);
         double* sj = s_aj[n & 1][warp];
         if (t < (I + 1) * SYM_TPB)
-            sym_tile<SYM_IPT, true>(tile_sa, t * TJ, lane, ibase, xi, yi, zi, mi, g, ax, ay, az, sj, rci);
+            sym_tile<SYM_IPT, true>(tile_sa, t * TJ, lane, ibase, xi, yi, zi, mi, g, ax, ay, az, sj, rci, p.rcrit, p.nb);
         else
-            sym_tile<SYM_IPT, false>(tile_sa, t * TJ, lane, ibase, xi, yi, zi, mi, g, ax, ay, az, sj, rci);
+            sym_tile<SYM_IPT, false>(tile_sa, t * TJ, lane, ibase, xi, yi, zi, mi, g, ax, ay, az, sj, rci, p.rcrit, p.nb);
         // combine the 4 warps' column partials in warp order (double-buffered: one barrier per tile)
         __syncthreads();
         if (tid == 0 && n + SYM_STAGES < nt) {   // every warp has left slot st: refill it
-            mbar_arrive_expect_tx(&s_full[st], SYM_TILE_BYTES);
-            tma_load_1d(s_tiles + st * SYM_TILE_STRIDE, src + (size_t)(n + SYM_STAGES) * SYM_TILE_BYTES, SYM_TILE_BYTES,
+            mbar_arrive_expect_tx(&s_full[st], LOAD_BYTES);
+            tma_load_1d(s_tiles + st * SYM_TILE_STRIDE, src + (size_t)(n + SYM_STAGES) * SYM_TILE_BYTES, LOAD_BYTES,
                         &s_full[st]);
         }
         const int jc = t * TJ + tid - jrow0;

@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmopal.so")
 SOURCES = ["mopal.cu"]
-HEADERS = ["common.cuh", "pair_accel.cuh", "pair_big.cuh", "pair_sym.cuh", "kepler.cuh", "encounters.cuh", "glue.cuh", "support.cuh", "step_small.cuh", "resolve.cuh"]
+HEADERS = ["common.cuh", "fixup.cuh", "pair_accel.cuh", "pair_big.cuh", "pair_sym.cuh", "kepler.cuh", "encounters.cuh", "glue.cuh", "support.cuh", "step_small.cuh", "resolve.cuh"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "--shared", "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 

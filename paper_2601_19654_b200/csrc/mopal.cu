@@ -16,6 +16,7 @@
 #include "support.cuh"
 #include "step_small.cuh"
 #include "resolve.cuh"
+#include "fixup.cuh"
 
 using namespace mopal;
 
@@ -54,6 +55,10 @@ struct mo_ctx {
     int *res_dbodyi = nullptr, *res_dpairi = nullptr;
     long long res_dbodyN = 0;
     int res_smemA = 0, res_smemB = 0, res_smemC = 0;
+    double* fix_part = nullptr;                      // partial rows of the flagged bodies
+    int *fix_list = nullptr, *fix_nf = nullptr;      // the flagged bodies, ascending (the solve beside the pair sum: fixup.cuh)
+    const double* pair_x = nullptr;                  // positions the pair kernel reads (nullptr: x)
+    int pair_u0 = -1, pair_u1 = -1;                  // work units of the next two-sided launch (-1: all / the rank's share)
     cudaStream_t res_stream[4] = {nullptr, nullptr, nullptr, nullptr};   // the size classes are solved side by side
     cudaEvent_t res_fork = nullptr, res_join[4] = {nullptr, nullptr, nullptr, nullptr};
     ResStats* res_out = nullptr;        // device
@@ -270,7 +275,7 @@ extern "C" void mo_destroy(mo_ctx* ctx) {
     cudaFree(ctx->gm); cudaFree(ctx->x0); cudaFree(ctx->v0); cudaFree(ctx->part);
     cudaFree(ctx->psumA); cudaFree(ctx->psumB); cudaFree(ctx->ticket);
     cudaFree(ctx->res_loc); cudaFree(ctx->res_out); cudaFree(ctx->res_tab); cudaFree(ctx->res_label);
-    cudaFree(ctx->res_cnp); cudaFree(ctx->res_cstart); cudaFree(ctx->res_cfill); cudaFree(ctx->res_cq); cudaFree(ctx->res_clist); cudaFree(ctx->res_ctl); cudaFree(ctx->res_aux); cudaFree(ctx->res_cown);
+    cudaFree(ctx->res_cnp); cudaFree(ctx->res_cstart); cudaFree(ctx->res_cfill); cudaFree(ctx->res_cq); cudaFree(ctx->res_clist); cudaFree(ctx->res_ctl); cudaFree(ctx->res_aux); cudaFree(ctx->res_cown); cudaFree(ctx->fix_list); cudaFree(ctx->fix_nf); cudaFree(ctx->fix_part);
     cudaFree(ctx->res_dbody); cudaFree(ctx->res_dpair); cudaFree(ctx->res_dbodyi); cudaFree(ctx->res_dpairi);
     if (ctx->res_host) cudaFreeHost(ctx->res_host);
     for (int k = 0; k < 4; ++k) { if (ctx->res_stream[k]) cudaStreamDestroy(ctx->res_stream[k]); if (ctx->res_join[k]) cudaEventDestroy(ctx->res_join[k]); }
@@ -448,10 +453,11 @@ static mo_status launch_pair(mo_ctx* ctx, bool kick = false, double hk = 0.0) {
             pick_big_kernel(ctx->big_ipt, kick)<<<grid, BIG_THREADS, 0, ctx->stream>>>(bp);
     } else if (ctx->use_sym) {
         SymParams sp;
-        sp.tiles = ctx->tiles; sp.x = ctx->x; sp.gm = ctx->gm; sp.rcrit = ctx->rcrit; sp.units = ctx->sym_units;
+        sp.tiles = ctx->tiles; sp.x = ctx->pair_x ? ctx->pair_x : ctx->x; sp.gm = ctx->gm; sp.rcrit = ctx->rcrit; sp.units = ctx->sym_units;
         sp.partI = ctx->sym_partI; sp.partJ = ctx->sym_partJ; sp.nb = ctx->nb; sp.ld = ctx->ld; sp.nbPad = ctx->nbPad;
         long long u0 = 0, u1 = ctx->sym_nunits;
         if (ctx->shard_world > 1) shard_range(ctx->sym_nunits, ctx->shard_rank, ctx->shard_world, &u0, &u1);
+        if (ctx->pair_u0 >= 0) { u0 = ctx->pair_u0; u1 = ctx->pair_u1; }
         sp.unit0 = (int)u0;
         if (u1 > u0) pick_sym_kernel(ctx->sym_ipt)<<<(int)(u1 - u0), SYM_THREADS, 0, ctx->stream>>>(sp);
     } else {
@@ -579,6 +585,9 @@ static mo_status ensure_resolve_scratch(mo_ctx* ctx) {
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_out, 1);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_label, (size_t)ctx->nb);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_aux, (size_t)ctx->nb);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->fix_list, (size_t)ctx->nb);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->fix_nf, 1);
+    if (e == cudaSuccess && ctx->use_sym) e = dalloc(ctx, &ctx->fix_part, (size_t)FIX_JS * 3 * ctx->nb);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_cown, capn);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_cnp, capn);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_cstart, capn);
@@ -606,7 +615,9 @@ static mo_status ensure_resolve_scratch(mo_ctx* ctx) {
     if (e == cudaSuccess) e = cudaMemsetAsync(ctx->res_out, 0, sizeof(ResStats), ctx->stream);
     if (e == cudaSuccess) e = cudaMallocHost(reinterpret_cast<void**>(&ctx->res_host), sizeof(ResStats));
     for (int k = 0; k < 4 && e == cudaSuccess; ++k) {
-        e = cudaStreamCreateWithFlags(&ctx->res_stream[k], cudaStreamNonBlocking);
+        int plo = 0, phi = 0;
+        cudaDeviceGetStreamPriorityRange(&plo, &phi);
+        e = cudaStreamCreateWithPriority(&ctx->res_stream[k], cudaStreamNonBlocking, phi);   // ahead of a pair sum that becomes eligible at the same time
         if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->res_join[k], cudaEventDisableTiming);
     }
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->res_fork, cudaEventDisableTiming);
@@ -679,7 +690,9 @@ static mo_status enqueue_step(mo_ctx* ctx, double dt) {
     MidParams mp;
     mp.x = ctx->x; mp.v = ctx->v; mp.x0 = ctx->x0; mp.v0 = ctx->v0; mp.gm = ctx->gm; mp.rcrit = ctx->rcrit;
     mp.psum_in = ctx->psumA; mp.psum_out = ctx->psumB; mp.ticket = ctx->ticket + 1;
-    const bool ovl = ctx->overlap && ctx->res_tol <= 0.0;   // the encounter solve needs the list before the jump
+    // with the encounter solve: beside the pair sum when the two-sided kernel runs (fixup.cuh), else before it
+    const bool ovl_res = ctx->overlap && ctx->res_tol > 0.0 && ctx->use_sym && ctx->shard_world == 1 && ctx->fix_part;
+    const bool ovl = (ctx->overlap && ctx->res_tol <= 0.0) || ovl_res;
     mp.x1 = ovl ? ctx->x1 : nullptr; mp.v1 = ovl ? ctx->v1 : nullptr; mp.enc = ctx->enc; mp.flag = ctx->flag;
     mp.st = ctx->dstats; mp.nb = ctx->nb; mp.ld = ctx->ld; mp.nbPad = ctx->nbPad; mp.npsum = ctx->npsum;
     mp.nbig = ctx->nbig;
@@ -687,6 +700,65 @@ static mo_status enqueue_step(mo_ctx* ctx, double dt) {
     jump_drift_boxes_kernel<<<ctx->npsum, ON_BLOCK, 0, ctx->stream>>>(mp);
     s = post_launch(ctx);
     if (s != MO_OK) return s;
+    if (ovl_res) {
+        // fork: encounter pass + encounter solve on enc_stream (read x0, v0, x1, v1; the solve writes x, v of the flagged
+        // bodies), pair sum over the drifted positions x1 on the main stream; join; corrections, jump, kick
+        cudaStream_t mainS = ctx->stream;
+        CK(cudaEventRecord(ctx->ev_fork, mainS));
+        CK(cudaStreamWaitEvent(ctx->enc_stream, ctx->ev_fork, 0));
+        EncState es = enc_state(ctx, ctx->x0, ctx->v0, dt);
+        es.x1 = ctx->x1; es.v1 = ctx->v1;
+        ctx->stream = ctx->enc_stream;
+        s = enqueue_pairs(ctx, es, 1);
+        if (s == MO_OK) s = enqueue_resolve(ctx, dt, ctx->res_tol);
+        ctx->stream = mainS;
+        if (s != MO_OK) return s;
+        CK(cudaEventRecord(ctx->ev_join, ctx->enc_stream));
+        // The pair sum in two launches.  A giant's star needs a whole SM for its CTA; inside one launch of 15 waves the pair
+        // kernel's CTAs would keep every SM half full and the solve would wait for the tail.  So: the first tenth of the
+        // units while the encounter pass and the label kernel run; the rest once the components are known (res_fork) - then
+        // the solve's CTAs and the pair kernel's become eligible together on draining SMs, and the solve's streams have the
+        // higher priority.
+        ctx->pair_x = ctx->x1;
+        pack_kernel<false, true><<<ctx->nSrcTiles, TJ, 0, mainS>>>(ctx->x1, ctx->gm, ctx->rcrit, ctx->nb, ctx->nbig, ctx->ld, ctx->tiles, nullptr, 0, 0.0);
+        s = post_launch(ctx);
+        const int ucut = ctx->sym_nunits / 10;
+        if (s == MO_OK) { ctx->pair_u0 = 0; ctx->pair_u1 = ucut; s = launch_pair(ctx); }
+        if (s == MO_OK) {
+            CK(cudaStreamWaitEvent(mainS, ctx->res_fork, 0));
+            ctx->pair_u0 = ucut; ctx->pair_u1 = ctx->sym_nunits; s = launch_pair(ctx);
+        }
+        ctx->pair_x = nullptr; ctx->pair_u0 = ctx->pair_u1 = -1;
+        if (s != MO_OK) return s;
+        const int nblk = (ctx->nb + ON_BLOCK - 1) / ON_BLOCK;
+        sym_reduce_kernel<false, false><<<dim3(nblk, 3), ON_BLOCK, 0, mainS>>>(ctx->sym_partI, ctx->sym_partJ, ctx->sym_ustart, ctx->nb, ctx->ld, ctx->nbPad,
+                                                                                ctx->a, nullptr, 0.0, 0, ctx->sym_nunits, ctx->sym_ch, sym_rows(ctx->sym_ipt));
+        s = post_launch(ctx);
+        if (s != MO_OK) return s;
+        CK(cudaStreamWaitEvent(mainS, ctx->ev_join, 0));
+        fix_list_kernel<<<1, FIX_LIST_THREADS, 0, mainS>>>(ctx->flag, ctx->nb, ctx->fix_list, ctx->fix_nf);
+        s = post_launch(ctx);
+        if (s != MO_OK) return s;
+        kick_psum_kernel<false><<<ctx->npsum, ON_BLOCK, 0, mainS>>>(ctx->v, nullptr, ctx->gm, ctx->nb, ctx->ld, 0.0, ctx->psumB, ctx->ticket + 1);
+        s = post_launch(ctx);
+        if (s != MO_OK) return s;
+        FixParams fp;
+        fp.x = ctx->x; fp.x1 = ctx->x1; fp.gm = ctx->gm; fp.rcrit = ctx->rcrit; fp.flag = ctx->flag; fp.flist = ctx->fix_list; fp.nf = ctx->fix_nf;
+        fp.a = ctx->a; fp.part = ctx->fix_part; fp.nb = ctx->nb; fp.ld = ctx->ld;
+        fix_unflagged_kernel<<<(ctx->nb + FIX_THREADS - 1) / FIX_THREADS, FIX_THREADS, 0, mainS>>>(fp);
+        s = post_launch(ctx);
+        if (s != MO_OK) return s;
+        // (the number of flagged bodies is not known on the host: CTAs beyond the list exit at once)
+        const int fgx = (ctx->nb + FIX_FB - 1) / FIX_FB < 512 ? (ctx->nb + FIX_FB - 1) / FIX_FB : 512;
+        fix_flagged_kernel<<<dim3(fgx, FIX_JS), FIX_THREADS, 0, mainS>>>(fp);
+        s = post_launch(ctx);
+        if (s != MO_OK) return s;
+        fix_flagged_reduce_kernel<<<(ctx->nb + FIX_THREADS - 1) / FIX_THREADS, FIX_THREADS, 0, mainS>>>(fp);
+        s = post_launch(ctx);
+        if (s != MO_OK) return s;
+        jump_kick_kernel<<<ctx->npsum, ON_BLOCK, 0, mainS>>>(ctx->x, ctx->v, ctx->a, ctx->psumB, ctx->npsum, 0.5 * dt / ctx->mu, 0.5 * dt, ctx->nb, ctx->ld);
+        return post_launch(ctx);
+    }
     if (ovl) {
         // fork: encounter pass on enc_stream (reads x0, v0, x1, v1, boxes, rcrit; writes pairs, flag, stats),
         // jump + pair sum + closing kick on the main stream (moves x, v; writes a); join at the end

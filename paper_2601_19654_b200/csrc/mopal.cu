@@ -55,6 +55,7 @@ struct mo_ctx {
     int *res_dbodyi = nullptr, *res_dpairi = nullptr;
     long long res_dbodyN = 0;
     int res_smemA = 0, res_smemB = 0, res_smemC = 0;
+    double* res_colres = nullptr; int* res_csync = nullptr;   // clusters: column results, barrier counters
     double* fix_part = nullptr;                      // partial rows of the flagged bodies
     int *fix_list = nullptr, *fix_nf = nullptr;      // the flagged bodies, ascending (the solve beside the pair sum: fixup.cuh)
     const double* pair_x = nullptr;                  // positions the pair kernel reads (nullptr: x)
@@ -275,7 +276,7 @@ extern "C" void mo_destroy(mo_ctx* ctx) {
     cudaFree(ctx->gm); cudaFree(ctx->x0); cudaFree(ctx->v0); cudaFree(ctx->part);
     cudaFree(ctx->psumA); cudaFree(ctx->psumB); cudaFree(ctx->ticket);
     cudaFree(ctx->res_loc); cudaFree(ctx->res_out); cudaFree(ctx->res_tab); cudaFree(ctx->res_label);
-    cudaFree(ctx->res_cnp); cudaFree(ctx->res_cstart); cudaFree(ctx->res_cfill); cudaFree(ctx->res_cq); cudaFree(ctx->res_clist); cudaFree(ctx->res_ctl); cudaFree(ctx->res_aux); cudaFree(ctx->res_cown); cudaFree(ctx->fix_list); cudaFree(ctx->fix_nf); cudaFree(ctx->fix_part);
+    cudaFree(ctx->res_cnp); cudaFree(ctx->res_cstart); cudaFree(ctx->res_cfill); cudaFree(ctx->res_cq); cudaFree(ctx->res_clist); cudaFree(ctx->res_ctl); cudaFree(ctx->res_aux); cudaFree(ctx->res_cown); cudaFree(ctx->fix_list); cudaFree(ctx->fix_nf); cudaFree(ctx->fix_part); cudaFree(ctx->res_colres); cudaFree(ctx->res_csync);
     cudaFree(ctx->res_dbody); cudaFree(ctx->res_dpair); cudaFree(ctx->res_dbodyi); cudaFree(ctx->res_dpairi);
     if (ctx->res_host) cudaFreeHost(ctx->res_host);
     for (int k = 0; k < 4; ++k) { if (ctx->res_stream[k]) cudaStreamDestroy(ctx->res_stream[k]); if (ctx->res_join[k]) cudaEventDestroy(ctx->res_join[k]); }
@@ -576,7 +577,8 @@ static mo_status enqueue_hill(mo_ctx* ctx, double n_hill, int mode, double* rhil
 
 // grids of the resolve kernels: class 0 (components of up to 63 pairs, 64 threads: several CTAs per SM), the larger
 // classes hold few components (the stars around the big bodies): small grids, cheap to launch when they have nothing to do
-static constexpr int RES_GRID_0_PER_SM = 6, RES_GRID_1 = 74, RES_GRID_2 = 32, RES_GRID_3 = 16, RES_GRID_4 = 16;
+static constexpr int RES_GRID_0_PER_SM = 6, RES_GRID_4 = 16;
+static constexpr int RES_CL_GRID = RES_NCOL * (RES_NCLUSTERS / 3);   // classes 1..3: 8 clusters of 8 CTAs each
 
 static mo_status ensure_resolve_scratch(mo_ctx* ctx) {
     if (ctx->res_loc) return MO_OK;
@@ -595,7 +597,9 @@ static mo_status ensure_resolve_scratch(mo_ctx* ctx) {
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_cq, capn);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_clist, capn * RES_NCLS);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_ctl, 16);
-    if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_tab, (size_t)6 * RES_KMAX * 1024 * RES_GRID_2);   // classes 2 and 3 (they run one after the other)
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_tab, (size_t)6 * RES_KMAX * 1024 * RES_CL_GRID);   // per CTA of the widest launch
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_colres, (size_t)RES_NCLUSTERS * 2 * RES_NCOL * 6 * 1024);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_csync, RES_NCLUSTERS);
     // class D pools: every body and every pair of the list can be in a class-D component
     ctx->res_dbodyN = (long long)ctx->nb < 2 * (long long)capn ? (long long)ctx->nb : 2 * (long long)capn;
     if (ctx->cap > RES_PHI_3) {          // a shorter list cannot hold a class-D component
@@ -608,10 +612,10 @@ static mo_status ensure_resolve_scratch(mo_ctx* ctx) {
     ctx->res_smemA = 88 * 64 + (132 + 6 * RES_KMAX * 8) * 64;
     ctx->res_smemB = 88 * 256 + (132 + 6 * RES_KMAX * 8) * 256;
     ctx->res_smemC = 227 * 1024 - 2048;                              // classes 2, 3: all there is (minus the static part)
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(resolve_solve_kernel<64, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->res_smemA);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(resolve_solve_kernel<256, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->res_smemB);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(resolve_solve_kernel<512, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->res_smemC);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(resolve_solve_kernel<1024, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->res_smemC);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(resolve_solve_kernel<64, 0, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->res_smemA);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(resolve_solve_kernel<256, 1, RES_NCOL>, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->res_smemB);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(resolve_solve_kernel<512, 2, RES_NCOL>, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->res_smemC);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(resolve_solve_kernel<1024, 3, RES_NCOL>, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->res_smemC);
     if (e == cudaSuccess) e = cudaMemsetAsync(ctx->res_out, 0, sizeof(ResStats), ctx->stream);
     if (e == cudaSuccess) e = cudaMallocHost(reinterpret_cast<void**>(&ctx->res_host), sizeof(ResStats));
     for (int k = 0; k < 4 && e == cudaSuccess; ++k) {
@@ -630,7 +634,7 @@ static mo_status enqueue_resolve(mo_ctx* ctx, double dt, double tol) {
     rp.x0 = ctx->x0; rp.v0 = ctx->v0; rp.x = ctx->x; rp.v = ctx->v; rp.gm = ctx->gm; rp.rcrit = ctx->rcrit;
     rp.pairs = ctx->pairs; rp.st = ctx->dstats; rp.out = ctx->res_out; rp.loc = ctx->res_loc; rp.label = ctx->res_label; rp.aux = ctx->res_aux; rp.cown = ctx->res_cown;
     rp.cnp = ctx->res_cnp; rp.cstart = ctx->res_cstart; rp.cfill = ctx->res_cfill; rp.cq = ctx->res_cq; rp.clist = ctx->res_clist;
-    rp.ctl = ctx->res_ctl; rp.tab = ctx->res_tab; rp.dbody = ctx->res_dbody; rp.dbodyi = ctx->res_dbodyi; rp.dpair = ctx->res_dpair;
+    rp.ctl = ctx->res_ctl; rp.colres = ctx->res_colres; rp.csync = ctx->res_csync; rp.tab = ctx->res_tab; rp.dbody = ctx->res_dbody; rp.dbodyi = ctx->res_dbodyi; rp.dpair = ctx->res_dpair;
     rp.dpairi = ctx->res_dpairi; rp.dbodyN = ctx->res_dbodyN;
     rp.cap = ctx->cap > 0 ? ctx->cap : 1; rp.nb = ctx->nb; rp.ld = ctx->ld; rp.mu = ctx->mu; rp.h = dt; rp.tol = tol;
     resolve_label_kernel<<<1, RES_LABEL_THREADS, 0, ctx->stream>>>(rp);
@@ -645,14 +649,22 @@ static mo_status enqueue_resolve(mo_ctx* ctx, double dt, double tol) {
         cudaStream_t st = ctx->res_stream[k];
         CK(cudaStreamWaitEvent(st, ctx->res_fork, 0));
         if (k == 0) resolve_stream_kernel<<<RES_GRID_4, RES_D_THREADS, 0, st>>>(rp);
-        else if (k == 1) resolve_solve_kernel<1024, 3><<<RES_GRID_3, 1024, ctx->res_smemC, st>>>(rp, ctx->res_smemC);
-        else if (k == 2) resolve_solve_kernel<512, 2><<<RES_GRID_2, 512, ctx->res_smemC, st>>>(rp, ctx->res_smemC);
-        else resolve_solve_kernel<256, 1><<<RES_GRID_1, 256, ctx->res_smemB, st>>>(rp, ctx->res_smemB);
+        else {
+            // clusters of RES_NCOL CTAs: one component per cluster, one Bulirsch-Stoer column per CTA
+            cudaLaunchConfig_t cfg = {};
+            cudaLaunchAttribute at[1];
+            at[0].id = cudaLaunchAttributeClusterDimension;
+            at[0].val.clusterDim.x = RES_NCOL; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+            cfg.gridDim = dim3(RES_CL_GRID); cfg.stream = st; cfg.attrs = at; cfg.numAttrs = 1;
+            if (k == 1) { cfg.blockDim = dim3(1024); cfg.dynamicSmemBytes = ctx->res_smemC; CK(cudaLaunchKernelEx(&cfg, resolve_solve_kernel<1024, 3, RES_NCOL>, rp, ctx->res_smemC)); }
+            else if (k == 2) { cfg.blockDim = dim3(512); cfg.dynamicSmemBytes = ctx->res_smemC; CK(cudaLaunchKernelEx(&cfg, resolve_solve_kernel<512, 2, RES_NCOL>, rp, ctx->res_smemC)); }
+            else { cfg.blockDim = dim3(256); cfg.dynamicSmemBytes = ctx->res_smemB; CK(cudaLaunchKernelEx(&cfg, resolve_solve_kernel<256, 1, RES_NCOL>, rp, ctx->res_smemB)); }
+        }
         s = post_launch(ctx);
         if (s != MO_OK) return s;
         CK(cudaEventRecord(ctx->res_join[k], st));
     }
-    resolve_solve_kernel<64, 0><<<ctx->nsm * RES_GRID_0_PER_SM, 64, ctx->res_smemA, mainS>>>(rp, ctx->res_smemA);
+    resolve_solve_kernel<64, 0, 1><<<ctx->nsm * RES_GRID_0_PER_SM, 64, ctx->res_smemA, mainS>>>(rp, ctx->res_smemA);
     s = post_launch(ctx);
     if (s != MO_OK) return s;
     for (int k = 0; k < 4; ++k) {

@@ -38,6 +38,8 @@ constexpr int RES_NCLS = 5;        // size classes: 0..3 one thread per body (64
 constexpr int RES_PHI_0 = 63, RES_PHI_1 = 255, RES_PHI_2 = 511, RES_PHI_3 = 1023;   // largest pair count of classes 0..3
 constexpr int RES_CTL_CNT = 1, RES_CTL_TKT = 1 + RES_NCLS, RES_CTL_POOL = 1 + 2 * RES_NCLS, RES_CTL_N = 2 + 2 * RES_NCLS;
 constexpr int RES_LABEL_THREADS = 1024;
+constexpr int RES_NCOL = 8;        // CTAs per cluster = columns side by side (classes 1..3)
+constexpr int RES_NCLUSTERS = 24;  // clusters of the three launches together (8 + 8 + 8)
 constexpr int RES_D_THREADS = 1024;
 constexpr int RES_D_BODY_PLANES = 3 + 6 + 6 + 6 + 3 + 2 + 3 + 6 * RES_KMAX;   // P, Y, D0, D1, F0A, SC, ACC, T
 constexpr int RES_D_BODY_IPLANES = 7;                                    // body, iLo, iHi, jLo, d2, tier, list of the warp-summed bodies
@@ -62,6 +64,8 @@ struct ResParams {
     int* cq;                     // cap: pair indices grouped by component (unordered inside a group)
     int* clist;                  // RES_NCLS * cap: the components of each class
     int* ctl;                    // [0] components, [RES_CTL_CNT + c] class counts, [RES_CTL_TKT + c] tickets, [RES_CTL_POOL] streamed-class body pool in use
+    double* colres;              // column results of the clusters: [cluster][2][NCOL][6][threads]
+    int* csync;                  // barrier counters of the clusters (zeroed by the label kernel)
     double* tab;                 // extrapolation tableaux of the class-C CTAs whose component does not leave room in shared memory
     double* dbody; int* dbodyi;  // class D pools: planes of dbodyN doubles / ints
     double* dpair; int* dpairi;  // planes of cap
@@ -105,6 +109,21 @@ __device__ __forceinline__ int res_scan(int v, int* sScan, int& total) {
 }
 
 __device__ __forceinline__ int res_class(int np) { return np <= RES_PHI_0 ? 0 : np <= RES_PHI_1 ? 1 : np <= RES_PHI_2 ? 2 : np <= RES_PHI_3 ? 3 : 4; }
+
+// barrier of the CTAs of a cluster that work on one component: every CTA's thread 0 counts itself in and waits for the
+// others (the cluster's CTAs are co-scheduled, so nobody waits for a CTA that is not running); the CTA's other live warps
+// wait at its named barrier.  Global writes before the barrier are visible after it (fences on both sides; readers use ld.cg).
+__device__ __forceinline__ void res_bar(int nthreads);
+__device__ __forceinline__ void res_cluster_barrier(int* cnt, int target, int nact) {
+    __threadfence();
+    res_bar(nact);
+    if (threadIdx.x == 0) {
+        atomicAdd(cnt, 1);
+        while (*reinterpret_cast<volatile int*>(cnt) < target) { }
+        __threadfence();
+    }
+    res_bar(nact);
+}
 
 // barrier of the first nthreads threads of the block (whole warps), beside the block barrier 0
 __device__ __forceinline__ void res_bar(int nthreads) { asm volatile("bar.sync 1, %0;" ::"r"(nthreads) : "memory"); }
@@ -156,6 +175,7 @@ __global__ void __launch_bounds__(RES_LABEL_THREADS) resolve_label_kernel(ResPar
     const int tid = threadIdx.x;
     if (tid < 64) sScan[tid] = 0;
     if (tid == 0) { *p.out = ResStats{0, 0, 0, 0}; for (int k = 0; k < RES_CTL_N; ++k) p.ctl[k] = 0; }
+    if (tid < RES_NCLUSTERS) p.csync[tid] = 0;
     const long long nce = p.st->nce_last;
     if (nce <= 0) return;
     if (nce > p.cap) { if (tid == 0) { p.out->fail = 1 << 30; atomicAdd(&p.st->resolve_fail, 1); } return; }      // truncated list: nothing can be resolved
@@ -339,7 +359,7 @@ struct ResCtl {
 // else global scratch.  Registers hold only the two running increments of the midpoint rule.  Only the warps that
 // hold a body (nact = n rounded up to whole warps) run the Bulirsch-Stoer loop, synchronised by a named barrier of
 // nact threads; the others wait at the block barrier that ends the component.
-template <int NT, int CLS>
+template <int NT, int CLS, int NCOL>
 __global__ void __launch_bounds__(NT, 1) resolve_solve_kernel(ResParams p, int smemBytes) {
     extern __shared__ __align__(16) unsigned char res_dyn[];
     __shared__ double sRed[32];
@@ -349,11 +369,20 @@ __global__ void __launch_bounds__(NT, 1) resolve_solve_kernel(ResParams p, int s
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     if (tid < 64) sScan[tid] = 0;
     bool firstTicket = true;
+    // NCOL > 1: the NCOL CTAs of a thread-block cluster work on the same component, CTA `col` integrating column `col` of
+    // every Bulirsch-Stoer step (the columns - 2, 4, .., 16 substeps from the same state - are independent integrations:
+    // side by side a step costs its longest column instead of their sum); components dealt to the clusters round-robin
+    const int col = NCOL > 1 ? (int)(blockIdx.x % NCOL) : 0;
+    const int cl = blockIdx.x / NCOL, ncl = gridDim.x / NCOL;
+    const int cslot = NCOL > 1 ? (CLS - 1) * (RES_NCLUSTERS / 3) + cl : 0;   // this cluster's barrier counter and result buffer
+    int nbarrier = 0;                                                      // cluster barriers passed so far (all CTAs alike)
+    int round = 0;
 
     for (;;) {
     __syncthreads();                                                       // the previous component is finished with shared memory
     int ticket;
-    if (firstTicket) { ticket = blockIdx.x; firstTicket = false; }         // the first gridDim.x components need no counter
+    if (NCOL > 1) ticket = cl + (round++) * ncl;
+    else if (firstTicket) { ticket = blockIdx.x; firstTicket = false; }    // the first gridDim.x components need no counter
     else {
         if (tid == 0) sBc[0] = gridDim.x + atomicAdd(&p.ctl[RES_CTL_TKT + CLS], 1);
         __syncthreads();
@@ -409,17 +438,20 @@ __global__ void __launch_bounds__(NT, 1) resolve_solve_kernel(ResParams p, int s
         __syncthreads();
     }
     // ---- its bodies, numbered by first appearance in the list (deterministic) ----
-    int* const tFirst = tBody + npad + 32;                                  // detached systems only: 2 npad + 2 npad more ints
+    // no shared body -> index table: a detached body's partners are in other systems too, and the CTAs of a cluster set
+    // the same component up side by side
+    const bool search = own >= 0 || NCOL > 1;
+    int* const tFirst = tBody + npad + 32;                                  // search only: 2 npad + 2 npad more ints
     int* const tId = tFirst + 2 * npad;
 #pragma unroll 1
     for (int k = tid; k < np; k += NT) {
         const int q = tQs[k], bi = p.pairs[2 * q], bj = p.pairs[2 * q + 1];
         tBi[k] = bi; tBj[k] = bj;
-        if (own < 0) { p.loc[bi] = 0x7fffffff; p.loc[bj] = 0x7fffffff; }
+        if (!search) { p.loc[bi] = 0x7fffffff; p.loc[bj] = 0x7fffffff; }
     }
     __syncthreads();
     int n = 0;
-    if (own < 0) {
+    if (!search) {
         // a component's bodies are in no other component: the global body -> index table is theirs alone
 #pragma unroll 1
         for (int k = tid; k < np; k += NT) { atomicMin(&p.loc[tBi[k]], 2 * k); atomicMin(&p.loc[tBj[k]], 2 * k + 1); }
@@ -470,12 +502,12 @@ __global__ void __launch_bounds__(NT, 1) resolve_solve_kernel(ResParams p, int s
     const int bodyBytes = 129 * nbp + 15 & ~15;
     const bool live = tid < n;
     const int me = live ? tBody[tid] : 0;
-    if (live) { if (own < 0) p.loc[me] = tid; sILo[tid] = 0; sIHi[tid] = 0; sD2[tid] = 0; }
+    if (live) { if (!search) p.loc[me] = tid; sILo[tid] = 0; sIHi[tid] = 0; sD2[tid] = 0; }
     __syncthreads();
 #pragma unroll 1
     for (int k = tid; k < np; k += NT) {
         const int bi = tBi[k], bj = tBj[k];
-        const int li = own < 0 ? p.loc[bi] : tId[tFirst[2 * k]], lj = own < 0 ? p.loc[bj] : tId[tFirst[2 * k + 1]];
+        const int li = !search ? p.loc[bi] : tId[tFirst[2 * k]], lj = !search ? p.loc[bj] : tId[tFirst[2 * k + 1]];
         sPi[k] = (unsigned short)li; sPj[k] = (unsigned short)lj;
         sGi[k] = p.gm[bi]; sGj[k] = p.gm[bj];
         const double rc = fmax(p.rcrit[bi], p.rcrit[bj]);
@@ -537,19 +569,21 @@ __global__ void __launch_bounds__(NT, 1) resolve_solve_kernel(ResParams p, int s
         const int kcols = min(ctl.ktarg + 1, RES_KMAX - 1);
         int acc = -1, klast = 0;
         float facCur = 1.0f, facPrev = 1.0f;
-#pragma unroll 1
-        for (int k = 0; k <= kcols; ++k) {
-            const int nsub = 2 * (k + 1);
+        // column kk: the modified midpoint rule with 2 (kk + 1) substeps over H -> cur (its increment); with run = false only
+        // f(y) and the error scales (m = 0), when they are still missing
+        auto column = [&](const int kk, const bool run, double (&cur)[6]) {
+            const int nsub = 2 * (kk + 1);
             const double hs = H / (double)nsub;
-            double d0[6], d1[6], cur[6];
+            double d0[6], d1[6];
 #pragma unroll
             for (int c = 0; c < 6; ++c) { d0[c] = 0.0; d1[c] = 0.0; cur[c] = 0.0; }
             if (havef0 && live) {
 #pragma unroll
                 for (int c = 0; c < 3; ++c) { d1[c] = hs * sY[(3 + c) * nbp + tid]; d1[3 + c] = hs * sF0[c * nbp + tid]; }
             }
+            const int mlast = run ? nsub : 0;
 #pragma unroll 1
-            for (int m = havef0 ? 1 : 0; m <= nsub; ++m) {
+            for (int m = havef0 ? 1 : 0; m <= mlast; ++m) {
                 const bool base = m == 0;
                 // own position: the increment goes to shared memory (y itself for f(y))
                 const double y0 = sY[tid], y1 = sY[nbp + tid], y2 = sY[2 * nbp + tid];
@@ -654,6 +688,30 @@ __global__ void __launch_bounds__(NT, 1) resolve_solve_kernel(ResParams p, int s
                     cur[3] = 0.5 * (d0[3] + fma(hs, a0, d1[3])); cur[4] = 0.5 * (d0[4] + fma(hs, a1, d1[4])); cur[5] = 0.5 * (d0[5] + fma(hs, a2, d1[5]));
                 }
             }
+        };
+        double* const cres = NCOL > 1 ? p.colres + ((size_t)(cslot * 2 + (nbarrier & 1)) * NCOL) * 6 * NT : nullptr;   // [column][component][thread]
+        if constexpr (NCOL > 1) {
+            // every CTA its own column (the CTAs beyond the columns this step tries: f(y) only), results through global
+            // memory, one barrier of the cluster per Bulirsch-Stoer step
+            double mine[6];
+            column(col, col <= kcols, mine);
+            if (live && col <= kcols) {
+#pragma unroll
+                for (int c = 0; c < 6; ++c) cres[((size_t)col * 6 + c) * NT + tid] = mine[c];
+            }
+            ++nbarrier;
+            res_cluster_barrier(p.csync + cslot, NCOL * nbarrier, nact);
+            if (col == 0) nrhs += (kcols + 1) * (kcols + 2) - 2;            // the other columns' right-hand sides: sum of 2 (k + 1)
+        }
+#pragma unroll 1
+        for (int k = 0; k <= kcols; ++k) {
+            double cur[6];
+            if constexpr (NCOL > 1) {
+#pragma unroll
+                for (int c = 0; c < 6; ++c) cur[c] = live ? __ldcg(&cres[((size_t)k * 6 + c) * NT + tid]) : 0.0;
+            } else {
+                column(k, true, cur);
+            }
             // row k of the tableau from row k-1 (in T), overwriting it column by column
             double err = 0.0;
             if (live) {
@@ -709,11 +767,11 @@ __global__ void __launch_bounds__(NT, 1) resolve_solve_kernel(ResParams p, int s
         havef0 = false;
         ctl.accepted(acc, facCur, facPrev);
     }
-    if (!fail && live && (own < 0 || own == me)) {                         // a detached body's system writes only that body
+    if (!fail && live && col == 0 && (own < 0 || own == me)) {             // a detached body's system writes only that body
 #pragma unroll
         for (int c = 0; c < 3; ++c) { p.x[(size_t)c * p.ld + me] = sY[c * nbp + tid]; p.v[(size_t)c * p.ld + me] = sY[(3 + c) * nbp + tid]; }
     }
-    if (tid == 0) {
+    if (tid == 0 && col == 0) {
         atomicAdd(&p.out->bodies, own < 0 ? n : 1); atomicAdd(&p.out->steps, nacc); atomicAdd(&p.out->rhs, nrhs);
         if (fail) { atomicAdd(&p.out->fail, 1); atomicAdd(&p.st->resolve_fail, 1); }
     }

@@ -1022,6 +1022,47 @@ def test_resolve_inside_step_vs_oracle(M, cfg, N):
     m.close(); m2.close()
 
 
+def test_resolve_inside_step_headline_size(M):
+    """one resolving step at cfg3 (N = 65,536: the giants' stars in clusters of CTAs, the solve beside the pair sum in two
+    launches, the flagged bodies' terms exchanged) against the oracle's kick / jump / drift / encounters / resolve / jump /
+    accel / kick"""
+    w = W.make_config(3)
+    mu, gm = G * w.m_star, G * w.mass
+    m = _mk(M, w)
+    m.set_resolve(1e-12)
+    st = m.step(w.dt, 1)
+    a, _ = oracle.accel(gm, w.x, w.rcrit)
+    v = oracle.kick(0.5 * w.dt, w.v, a)
+    x, _ = oracle.jump(0.5 * w.dt, mu, gm, w.x, v)
+    x0, v0 = x.copy(), v.copy()
+    x, v, _ = oracle.drift(mu, w.dt, x, v)
+    enc = oracle.encounters(w.dt, x0, v0, x, v, w.rcrit)
+    assert enc["count"] > 500 and st.nce_last == enc["count"] and np.array_equal(m.pair_list(st.nce_last), enc["pairs"])
+    r = oracle.resolve(mu, gm, w.rcrit, w.dt, x0, v0, x, v, enc["pairs"])
+    assert r["fail"] == 0
+    rs = m.resolve_stats()
+    assert rs["fail"] == 0 and rs["bodies"] == r["n"] and st.resolve_fail == 0
+    x, v = r["x"], r["v"]
+    x, _ = oracle.jump(0.5 * w.dt, mu, gm, x, v)
+    a, S = oracle.accel(gm, x, w.rcrit)
+    v = oracle.kick(0.5 * w.dt, v, a)
+    # the flagged bodies that pass a giant closely scatter (see test_resolve_big_star_components): positions to 1e-10 for
+    # them - and their accelerations, dominated by the giant 0.02-1 AU away, follow their positions (3 dr / r): 1e-7 S
+    idx = np.unique(enc["pairs"]); rest = np.setdiff1d(np.arange(w.nb), idx)
+    ag = m.get("a")
+    assert np.all(np.abs(ag - a) <= 1e-7 * S) and np.median(np.abs(ag - a) / S) <= 1e-13
+    # the strict check of the accelerations (pair sum over the drifted positions + exchanged terms of the flagged bodies +
+    # their recomputed rows): against the oracle's sum at the kernel's OWN final positions, every body
+    a2, S2 = oracle.accel(gm, m.get("x"), w.rcrit)
+    _check_accel(ag, a2, S2, "cfg3 resolving step, accelerations at the step's own positions")
+    tol = RES_RTOL(1e-12) + 2e-13
+    assert _rel_vec_err(m.get("x")[:, rest], x[:, rest]).max() <= tol and _rel_vec_err(m.get("v")[:, rest], v[:, rest]).max() <= tol
+    assert _rel_vec_err(m.get("x")[:, idx], x[:, idx]).max() <= 1e-10 and _rel_vec_err(m.get("v")[:, idx], v[:, idx]).max() <= 1e-10
+    ex = _rel_vec_err(m.get("v")[:, idx], v[:, idx])
+    assert np.median(ex) <= tol
+    m.close()
+
+
 def test_resolve_energy_and_a_dense_component(M):
     """through a close encounter the resolved step keeps the energy (mo_energy) orders of magnitude better"""
     w, mass, x, v, rc = _close_pair_system(0.004, m=3e-5, extra=300)

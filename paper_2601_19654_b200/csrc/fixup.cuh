@@ -93,11 +93,12 @@ constexpr int FIX_CHUNK = 256;   // flagged bodies staged per pass of fix_unflag
 constexpr int FIX_FB = 8;        // flagged bodies per CTA of fix_flagged_kernel
 constexpr int FIX_JS = 8;        // j splits of a flagged body's row
 
-__global__ void __launch_bounds__(FIX_THREADS) fix_unflagged_kernel(FixParams p) {
+constexpr int FIX_UT = 128;      // threads of fix_unflagged_kernel (one body each): small CTAs, more of them per SM
+__global__ void __launch_bounds__(FIX_UT) fix_unflagged_kernel(FixParams p) {
     __shared__ double sN[3][FIX_CHUNK], sO[3][FIX_CHUNK], sG[FIX_CHUNK], sR[FIX_CHUNK];
     const int nf = *p.nf;
     if (nf == 0) return;
-    const int i = blockIdx.x * FIX_THREADS + threadIdx.x;
+    const int i = blockIdx.x * FIX_UT + threadIdx.x;
     const bool mine = i < p.nb && !p.flag[i];
     double xi = 0.0, yi = 0.0, zi = 0.0, rci = 0.0;
     if (mine) { xi = p.x[i]; yi = p.x[p.ld + i]; zi = p.x[2 * p.ld + i]; rci = p.rcrit[i]; }
@@ -105,7 +106,7 @@ __global__ void __launch_bounds__(FIX_THREADS) fix_unflagged_kernel(FixParams p)
     for (int base = 0; base < nf; base += FIX_CHUNK) {
         const int m = min(FIX_CHUNK, nf - base);
         __syncthreads();
-        for (int t = threadIdx.x; t < m; t += FIX_THREADS) {
+        for (int t = threadIdx.x; t < m; t += FIX_UT) {
             const int f = p.flist[base + t];
 #pragma unroll
             for (int c = 0; c < 3; ++c) { sN[c][t] = p.x[(size_t)c * p.ld + f]; sO[c][t] = p.x1[(size_t)c * p.ld + f]; }
@@ -146,8 +147,14 @@ __global__ void __launch_bounds__(FIX_THREADS) fix_flagged_kernel(FixParams p) {
     }
     const int per = ((p.nb + FIX_JS - 1) / FIX_JS + FIX_THREADS - 1) / FIX_THREADS * FIX_THREADS;
     const int j0 = js * per, j1 = min(p.nb, j0 + per);
-    for (int j = j0 + threadIdx.x; j < j1; j += FIX_THREADS) {
-        const double xj = p.x[j], yj = p.x[p.ld + j], zj = p.x[2 * p.ld + j], gj = p.gm[j], rcj = p.rcrit[j];
+    // the next body's record is loaded while the current one is used
+    int j = j0 + threadIdx.x;
+    double nx = 0.0, ny = 0.0, nz = 0.0, ng = 0.0, nr = 0.0;
+    if (j < j1) { nx = p.x[j]; ny = p.x[p.ld + j]; nz = p.x[2 * p.ld + j]; ng = p.gm[j]; nr = p.rcrit[j]; }
+    for (; j < j1; j += FIX_THREADS) {
+        const double xj = nx, yj = ny, zj = nz, gj = ng, rcj = nr;
+        const int jn = j + FIX_THREADS;
+        if (jn < j1) { nx = p.x[jn]; ny = p.x[p.ld + jn]; nz = p.x[2 * p.ld + jn]; ng = p.gm[jn]; nr = p.rcrit[jn]; }
 #pragma unroll
         for (int r = 0; r < FIX_FB; ++r) {
             const double dx = xj - xf[r], dy = yj - yf[r], dz = zj - zf[r];

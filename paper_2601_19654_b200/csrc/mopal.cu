@@ -2,6 +2,7 @@
 // orchestration and the CUDA-graph step driver.  All arithmetic is in the kernels of
 // pair_accel.cuh / kepler.cuh / encounters.cuh / glue.cuh.
 #include <cuda_runtime.h>
+#include <nvtx3/nvToolsExt.h>
 #include <math.h>
 #include <stdlib.h>
 #include <string.h>
@@ -112,6 +113,13 @@ struct mo_ctx {
             return MO_ECUDA;                              \
         }                                                 \
     } while (0)
+
+// NVTX range around the enqueue of a stage (header-only NVTX 3: a no-op unless a tool such as nsys is attached); the
+// ranges name the stages of SURVEY.md 8(a) on a timeline of single steps (a replayed graph shows its kernels only)
+struct StageRange {
+    explicit StageRange(const char* name) { nvtxRangePushA(name); }
+    ~StageRange() { nvtxRangePop(); }
+};
 
 static inline void shard_range(long long n, int rank, int world, long long* lo, long long* hi) {
     *lo = n * rank / world;
@@ -470,6 +478,7 @@ static mo_status launch_pair(mo_ctx* ctx, bool kick = false, double hk = 0.0) {
 
 // a <- accel(x), optionally preceded by the jump (psumB) and followed by the kick
 static mo_status enqueue_accel(mo_ctx* ctx, bool jump, double hj, bool kick, double hk) {
+    StageRange nv("mopal: jump + pair accelerations + kick (a4, a1, a2, a3)");
     if (ctx->shard_world > 1) kick = false;      // a is this rank's share: the kick follows the caller's sum over the ranks (mo_step_end)
     const double hjm = jump ? hj / ctx->mu : 0.0;
     const double* ps = jump ? ctx->psumB : nullptr;
@@ -517,6 +526,7 @@ static EncState enc_state(const mo_ctx* ctx, const double* x0, const double* v0,
 
 // find + scan + place (+ overflow fallback) on boxes already in ctx->enc (counters already zeroed)
 static mo_status enqueue_pairs(mo_ctx* ctx, const EncState& es, int step_inc) {
+    StageRange nv("mopal: encounter pairs (a8)");
     EncFindParams fp;
     fp.s = es; fp.e = ctx->enc; fp.cap = ctx->cap; fp.nTiles = ctx->nTiles;
     mo_status s;
@@ -630,6 +640,7 @@ static mo_status ensure_resolve_scratch(mo_ctx* ctx) {
 }
 
 static mo_status enqueue_resolve(mo_ctx* ctx, double dt, double tol) {
+    StageRange nv("mopal: encounter resolution (f3)");
     ResParams rp;
     rp.x0 = ctx->x0; rp.v0 = ctx->v0; rp.x = ctx->x; rp.v = ctx->v; rp.gm = ctx->gm; rp.rcrit = ctx->rcrit;
     rp.pairs = ctx->pairs; rp.st = ctx->dstats; rp.out = ctx->res_out; rp.loc = ctx->res_loc; rp.label = ctx->res_label; rp.aux = ctx->res_aux; rp.cown = ctx->res_cown;
@@ -675,6 +686,7 @@ static mo_status enqueue_resolve(mo_ctx* ctx, double dt, double tol) {
 }
 
 static mo_status enqueue_step(mo_ctx* ctx, double dt) {
+    StageRange nv("mopal: hybrid step (a9)");
     if (ctx->use_small && ctx->res_tol <= 0.0) {
         SmallParams q;
         MidParams& mp = q.m;
@@ -696,9 +708,10 @@ static mo_status enqueue_step(mo_ctx* ctx, double dt) {
         mo_status hs = enqueue_hill(ctx, ctx->hill_n, ctx->hill_mode, nullptr);
         if (hs != MO_OK) return hs;
     }
+    nvtxRangePushA("mopal: kick, sum gm v, jump, snapshot, drift, boxes (a3-a7)");
     kick_psum_kernel<true><<<ctx->npsum, ON_BLOCK, 0, ctx->stream>>>(ctx->v, ctx->a, ctx->gm, ctx->nb, ctx->ld, 0.5 * dt, ctx->psumA, ctx->ticket);
     mo_status s = post_launch(ctx);
-    if (s != MO_OK) return s;
+    if (s != MO_OK) { nvtxRangePop(); return s; }
     MidParams mp;
     mp.x = ctx->x; mp.v = ctx->v; mp.x0 = ctx->x0; mp.v0 = ctx->v0; mp.gm = ctx->gm; mp.rcrit = ctx->rcrit;
     mp.psum_in = ctx->psumA; mp.psum_out = ctx->psumB; mp.ticket = ctx->ticket + 1;
@@ -711,6 +724,7 @@ static mo_status enqueue_step(mo_ctx* ctx, double dt) {
     mp.hj_over_mu = 0.5 * dt / ctx->mu; mp.mu = ctx->mu; mp.h = dt;
     jump_drift_boxes_kernel<<<ctx->npsum, ON_BLOCK, 0, ctx->stream>>>(mp);
     s = post_launch(ctx);
+    nvtxRangePop();
     if (s != MO_OK) return s;
     if (ovl_res) {
         // fork: encounter pass + encounter solve on enc_stream (read x0, v0, x1, v1; the solve writes x, v of the flagged

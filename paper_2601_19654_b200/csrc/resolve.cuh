@@ -689,7 +689,7 @@ __global__ void __launch_bounds__(NT, 1) resolve_solve_kernel(ResParams p, int s
                 }
             }
         };
-        double* const cres = NCOL > 1 ? p.colres + ((size_t)(cslot * 2 + (nbarrier & 1)) * NCOL) * 6 * NT : nullptr;   // [column][component][thread]
+        double* const cres = NCOL > 1 ? p.colres + ((size_t)(cslot * 2 + (nbarrier & 1)) * NCOL) * 6 * 1024 : nullptr;   // [column][component][thread], 1024 per plane
         if constexpr (NCOL > 1) {
             // every CTA its own column (the CTAs beyond the columns this step tries: f(y) only), results through global
             // memory, one barrier of the cluster per Bulirsch-Stoer step
@@ -697,7 +697,7 @@ __global__ void __launch_bounds__(NT, 1) resolve_solve_kernel(ResParams p, int s
             column(col, col <= kcols, mine);
             if (live && col <= kcols) {
 #pragma unroll
-                for (int c = 0; c < 6; ++c) cres[((size_t)col * 6 + c) * NT + tid] = mine[c];
+                for (int c = 0; c < 6; ++c) cres[((size_t)col * 6 + c) * 1024 + tid] = mine[c];
             }
             ++nbarrier;
             res_cluster_barrier(p.csync + cslot, NCOL * nbarrier, nact);
@@ -708,7 +708,7 @@ __global__ void __launch_bounds__(NT, 1) resolve_solve_kernel(ResParams p, int s
             double cur[6];
             if constexpr (NCOL > 1) {
 #pragma unroll
-                for (int c = 0; c < 6; ++c) cur[c] = live ? __ldcg(&cres[((size_t)k * 6 + c) * NT + tid]) : 0.0;
+                for (int c = 0; c < 6; ++c) cur[c] = live ? __ldcg(&cres[((size_t)k * 6 + c) * 1024 + tid]) : 0.0;
             } else {
                 column(k, true, cur);
             }

@@ -18,7 +18,7 @@ on-device close-encounter solve at the headline config) and ``cpu_baseline`` (th
 of the oracle on the box's host cores: one thread and all cores, as BASELINE.md plans).
 
 One JSON line on stdout (rank 0).  Under torchrun every rank runs an independent replica
-(DESIGN.md section 1 row e: "replicas only"; ``--sharded`` times the i-sharded step of row f4
+(DESIGN.md section 1 row e: replicas by default; ``--sharded`` times the step of row f4, the pair sum split over the ranks,
 instead), timing is the max over ranks, ``value`` the total over ranks.
 
 ``--impl reference`` times the CPU oracle (test infrastructure, as it stands; plain-double build, all

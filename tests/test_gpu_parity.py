@@ -1251,6 +1251,36 @@ def test_sharded_pair_sum_and_step_on_one_gpu(M, kind, world):
         m.close()
 
 
+def test_sharded_step_with_encounter_resolution(M):
+    """the resolving step under sharding: the solve runs replicated on every rank before the rank's share of the pair sum
+    (no detour beside the pair sum there) - same step as the unsharded one, which takes the detour"""
+    w = W.shrink(3, 6000)
+    ref = _mk(M, w); ref.set_resolve(1e-12)
+    ranks = [_mk(M, w) for _ in range(2)]
+    for r, m in enumerate(ranks):
+        m.set_shard(r, 2); m.set_resolve(1e-12)
+    tot = None
+    for m in ranks:
+        m.accel()
+        tot = m.a.clone() if tot is None else tot + m.a
+    for m in ranks:
+        m.a.copy_(tot); m.accel_summed()
+    for _ in range(2):
+        for m in ranks:
+            m.step_begin(w.dt)
+        tot = ranks[0].a + ranks[1].a
+        for m in ranks:
+            m.a.copy_(tot); m.accel_summed()
+        sts = [m.step_end(w.dt) for m in ranks]
+    s_ref = ref.step(w.dt, 2)
+    assert sts[0].nce_last == s_ref.nce_last > 0 and sts[0].resolve_fail == 0 and s_ref.resolve_fail == 0
+    assert ranks[0].resolve_stats()["bodies"] == ref.resolve_stats()["bodies"] > 0
+    assert np.array_equal(ranks[0].get("x"), ranks[1].get("x")) and np.array_equal(ranks[0].get("v"), ranks[1].get("v"))
+    assert _rel_vec_err(ranks[0].get("x"), ref.get("x")).max() <= 1e-13 and _rel_vec_err(ranks[0].get("v"), ref.get("v")).max() <= 1e-12
+    for m in ranks + [ref]:
+        m.close()
+
+
 def test_sharded_driver_world1_and_unsupported_sizes(M):
     from paper_2601_19654_b200.sharded import ShardedMopal
     w = W.shrink(3, 9000)

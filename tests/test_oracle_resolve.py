@@ -204,3 +204,37 @@ def test_X1_several_interacting_components_against_dop853_on_the_union_system(h)
     # dropping the chain's second pair (what a wrong split would amount to for body 6) is far outside the tolerance
     bad = oracle.resolve(mu, gm, rc, h, x, v, x1, v1, pairs[:3].copy(), tol=1e-13)
     assert np.linalg.norm(bad["v"][:, 4] - r["v"][:, 4]) / np.linalg.norm(r["v"][:, 4]) > 1e-9
+
+
+def test_X6_massless_bodies_can_be_integrated_apart():
+    """Reading X-6 (the kernel detaches massless bodies): a massless body exerts no force, so integrating every test
+    particle in a system of its own with its massive partners gives the states of integrating the whole component
+    together - shown here on the ORACLE alone (joint call vs one call per test particle), to the tolerance."""
+    M = 1.0
+    K = 6
+    rng = np.random.default_rng(7)
+    xg = np.array([5.2, 0.0, 0.0])
+    rad = rng.uniform(0.05, 0.6, K); ang = rng.uniform(0, 2 * np.pi, K)
+    X = np.empty((3, K + 2)); X[:, 0] = xg; X[:, 1] = xg + np.array([0.25, 0.1, 0.0])
+    X[0, 2:] = xg[0] + rad * np.cos(ang); X[1, 2:] = xg[1] + rad * np.sin(ang); X[2, 2:] = rng.uniform(-0.01, 0.01, K)
+    r = np.linalg.norm(X, axis=0)
+    vc = np.sqrt(G * M / r)
+    Vh = np.stack([-vc * X[1] / r, vc * X[0] / r, np.zeros(K + 2)])
+    mass = np.concatenate([[1e-3, 3e-6], np.zeros(K)])            # a giant, an embryo next to it, K test particles
+    V = oracle.h2dh(M, mass, Vh)
+    _, rc = oracle.hill(G, M, mass, X, V, n_hill=3.0)
+    mu, gm, h = G * M, G * mass, 6.0
+    x1, v1, _ = oracle.drift(mu, h, X, V)
+    pairs = np.array([[0, 1]] + [[0, k] for k in range(2, K + 2)] + [[1, 2], [1, 3]], dtype=np.int32)
+    pairs = pairs[np.lexsort((pairs[:, 1], pairs[:, 0]))]
+    joint = oracle.resolve(mu, gm, rc, h, X, V, x1, v1, pairs, tol=1e-13)
+    assert joint["fail"] == 0 and joint["n"] == K + 2
+    core = np.array([[0, 1]], dtype=np.int32)
+    alone = oracle.resolve(mu, gm, rc, h, X, V, x1, v1, core, tol=1e-13)          # the massive bodies by themselves
+    assert _relv(alone["x"][:, :2], joint["x"][:, :2]) <= 1e-12 and _relv(alone["v"][:, :2], joint["v"][:, :2]) <= 1e-12
+    for k in range(2, K + 2):                                                    # every test particle with the core
+        own = pairs[(pairs[:, 1] == k)]
+        sub = np.concatenate([core, own]); sub = sub[np.lexsort((sub[:, 1], sub[:, 0]))]
+        one = oracle.resolve(mu, gm, rc, h, X, V, x1, v1, sub, tol=1e-13)
+        assert _relv(one["x"][:, [k]], joint["x"][:, [k]]) <= 1e-11 and _relv(one["v"][:, [k]], joint["v"][:, [k]]) <= 1e-11, k
+        assert np.linalg.norm(one["v"][:, k] - v1[:, k]) / np.linalg.norm(v1[:, k]) > 1e-8       # the encounter matters

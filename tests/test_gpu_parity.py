@@ -1096,6 +1096,25 @@ def test_resolve_energy_and_a_dense_component(M):
     m.close()
 
 
+def test_resolve_truncated_list_is_reported(M):
+    """more pairs than cap: the list is truncated, nothing can be resolved - the bodies keep the drift result, the failure is
+    counted (sticky) and the step's status says so"""
+    w = W.shrink(1, 1500)
+    x1, v1 = _enc_inputs(w)
+    m = M.Mopal(w.mass, w.x, w.v, w.rcrit, m_star=w.m_star, G=w.G, cap=4)
+    m.snapshot(); m.set("x", x1); m.set("v", v1)
+    assert m.encounters(w.dt) > 4
+    m.resolve(w.dt, 1e-12)
+    assert m.resolve_stats()["fail"] >= 1 and np.array_equal(m.get("x"), x1) and np.array_equal(m.get("v"), v1)
+    assert m.stats().resolve_fail == 1
+    m.close()
+    m = M.Mopal(w.mass, w.x, w.v, w.rcrit, m_star=w.m_star, G=w.G, cap=4)
+    m.set_resolve(1e-12)
+    st = m.step(w.dt, 2)
+    assert st.status == M.MO_EOVERFLOW and st.resolve_fail == 2          # overflow outranks MO_ERESOLVE; both are sticky
+    m.close()
+
+
 def _giant_star(K, rmin, seed_off=40):
     """a giant with K planetesimals inside its critical radius: one star component of K + 1 bodies"""
     rng = np.random.default_rng(seed_off + K)

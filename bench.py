@@ -323,7 +323,7 @@ def side_config(torch, M, w, nbig, flush, peak_sust, steps_single=5, steps_graph
     e0.record(m.stream); st = m.step(w.dt, steps_graph, sync=False); e1.record(m.stream); torch.cuda.synchronize()
     g_ms = e0.elapsed_time(e1) / steps_graph
     st = m.stats()
-    alg, exe = _pair_roofline(kname, pairs, pair_ms, peak_sust)
+    alg, exe = _pair_roofline(kname, pairs, pair_ms, peak_sust) if pair_ms > 0 else (0.0, 0.0)   # (no kernel time in the resolving step: gated launches)
     out = {"workload": w.name, "N": w.N, "nbig": w.nb if nbig is None else nbig, "ms_per_step": total_ms / steps_single,
            "ms_per_step_graph_replay": g_ms, "pairs_per_s": pairs / (total_ms / steps_single * 1e-3),
            "pairs_per_s_graph_replay": pairs / (g_ms * 1e-3), "pair_kernel": kname, "pair_kernel_ms": pair_ms,

@@ -23,6 +23,11 @@ __device__ __forceinline__ uint32_t smem_u32(const void* p) {
     return (uint32_t)__cvta_generic_to_shared(p);
 }
 
+// A kernel launch that is recorded in the step's graph but only WORKS when a device flag says so (the resolving step has
+// two ways of getting its closing accelerations, chosen on the device from the last step's encounter list: mopal.cu)
+struct Gate { const int* flag; int want; };
+__device__ __forceinline__ bool gate_closed(const Gate& g) { return g.flag != nullptr && *g.flag != g.want; }
+
 // ---- mbarrier ----------------------------------------------------------
 __device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");

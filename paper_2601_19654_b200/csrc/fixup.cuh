@@ -43,8 +43,9 @@ __device__ __forceinline__ int fix_scan(int v, int* sScan, int& total) {
 // F in ascending order: one CTA, thread t takes the bodies [t seg, (t+1) seg), seg a multiple of 8 (the flags are read
 // eight at a time: almost all of them are 0)
 __global__ void __launch_bounds__(FIX_LIST_THREADS) fix_list_kernel(const uint8_t* __restrict__ flag, int nb,
-                                                                    int* __restrict__ flist, int* __restrict__ nf) {
+                                                                    int* __restrict__ flist, int* __restrict__ nf, Gate gate) {
     __shared__ int sScan[64];
+    if (gate_closed(gate)) return;
     const int tid = threadIdx.x;
     const int seg = ((nb + FIX_LIST_THREADS - 1) / FIX_LIST_THREADS + 7) & ~7;
     const int b0 = min(nb, tid * seg), b1 = min(nb, b0 + seg);
@@ -74,6 +75,7 @@ struct FixParams {
     double* a;             // 3*ld in/out
     double* part;          // FIX_JS * 3 * nb: partial rows of the flagged bodies
     int nb, ld;
+    Gate gate;
 };
 
 // K(r; rc) / r^3: outside the changeover radius (almost every pair) the seed + one third-order correction of the pair
@@ -96,6 +98,7 @@ constexpr int FIX_JS = 8;        // j splits of a flagged body's row
 constexpr int FIX_UT = 128;      // threads of fix_unflagged_kernel (one body each): small CTAs, more of them per SM
 __global__ void __launch_bounds__(FIX_UT) fix_unflagged_kernel(FixParams p) {
     __shared__ double sN[3][FIX_CHUNK], sO[3][FIX_CHUNK], sG[FIX_CHUNK], sR[FIX_CHUNK];
+    if (gate_closed(p.gate)) return;
     const int nf = *p.nf;
     if (nf == 0) return;
     const int i = blockIdx.x * FIX_UT + threadIdx.x;
@@ -133,6 +136,7 @@ __global__ void __launch_bounds__(FIX_UT) fix_unflagged_kernel(FixParams p) {
 // (every j loaded once for FIX_FB rows), fixed-order block sum -> part[js][f][c]
 __global__ void __launch_bounds__(FIX_THREADS) fix_flagged_kernel(FixParams p) {
     __shared__ double sh[FIX_THREADS / 32][3 * FIX_FB];
+    if (gate_closed(p.gate)) return;
     const int nf = *p.nf;
     const int js = blockIdx.y;
     for (int k0 = blockIdx.x * FIX_FB; k0 < nf; k0 += gridDim.x * FIX_FB) {
@@ -186,6 +190,7 @@ __global__ void __launch_bounds__(FIX_THREADS) fix_flagged_kernel(FixParams p) {
 }
 
 __global__ void __launch_bounds__(FIX_THREADS) fix_flagged_reduce_kernel(FixParams p) {
+    if (gate_closed(p.gate)) return;
     const int nf = *p.nf;
     const int k = blockIdx.x * FIX_THREADS + threadIdx.x;
     if (k >= nf) return;
@@ -202,7 +207,8 @@ __global__ void __launch_bounds__(FIX_THREADS) fix_flagged_reduce_kernel(FixPara
 // second jump x += hj P / mu (Hamiltonian block LOOP 2-3) and closing kick v += hk a (LOOP 1)
 __global__ void __launch_bounds__(ON_BLOCK) jump_kick_kernel(double* __restrict__ x, double* __restrict__ v,
                                                               const double* __restrict__ a, const double* __restrict__ psum,
-                                                              int npsum, double hj_over_mu, double hk, int nb, int ld) {
+                                                              int npsum, double hj_over_mu, double hk, int nb, int ld, Gate gate) {
+    if (gate_closed(gate)) return;
     const int b = blockIdx.x * ON_BLOCK + threadIdx.x;
     if (b >= nb) return;
     double P0, P1, P2;
@@ -210,5 +216,8 @@ __global__ void __launch_bounds__(ON_BLOCK) jump_kick_kernel(double* __restrict_
     x[b] += hj_over_mu * P0; x[ld + b] += hj_over_mu * P1; x[2 * ld + b] += hj_over_mu * P2;
     v[b] = fma(hk, a[b], v[b]); v[ld + b] = fma(hk, a[ld + b], v[ld + b]); v[2 * ld + b] = fma(hk, a[2 * ld + b], v[2 * ld + b]);
 }
+
+// the step's way of getting its accelerations: taken over from what the last step's label kernel saw
+__global__ void mode_latch_kernel(int* mode) { mode[0] = mode[1]; }
 
 }  // namespace mopal

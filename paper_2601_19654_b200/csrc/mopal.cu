@@ -61,6 +61,9 @@ struct mo_ctx {
     int *fix_list = nullptr, *fix_nf = nullptr;      // the flagged bodies, ascending (the solve beside the pair sum: fixup.cuh)
     const double* pair_x = nullptr;                  // positions the pair kernel reads (nullptr: x)
     int pair_u0 = -1, pair_u1 = -1;                  // work units of the next two-sided launch (-1: all / the rank's share)
+    Gate gate = {nullptr, 0};                        // gate of the pack / pair / reduce launches being enqueued (none by default)
+    int* res_mode = nullptr;                         // [0] how this step gets its accelerations (1: solve beside the pair sum,
+                                                     // 0: before it), [1] what the label kernel saw (latched at the next step)
     cudaStream_t res_stream[4] = {nullptr, nullptr, nullptr, nullptr};   // the size classes are solved side by side
     cudaEvent_t res_fork = nullptr, res_join[4] = {nullptr, nullptr, nullptr, nullptr};
     ResStats* res_out = nullptr;        // device
@@ -284,7 +287,7 @@ extern "C" void mo_destroy(mo_ctx* ctx) {
     cudaFree(ctx->gm); cudaFree(ctx->x0); cudaFree(ctx->v0); cudaFree(ctx->part);
     cudaFree(ctx->psumA); cudaFree(ctx->psumB); cudaFree(ctx->ticket);
     cudaFree(ctx->res_loc); cudaFree(ctx->res_out); cudaFree(ctx->res_tab); cudaFree(ctx->res_label);
-    cudaFree(ctx->res_cnp); cudaFree(ctx->res_cstart); cudaFree(ctx->res_cfill); cudaFree(ctx->res_cq); cudaFree(ctx->res_clist); cudaFree(ctx->res_ctl); cudaFree(ctx->res_aux); cudaFree(ctx->res_cown); cudaFree(ctx->fix_list); cudaFree(ctx->fix_nf); cudaFree(ctx->fix_part); cudaFree(ctx->res_colres); cudaFree(ctx->res_csync);
+    cudaFree(ctx->res_cnp); cudaFree(ctx->res_cstart); cudaFree(ctx->res_cfill); cudaFree(ctx->res_cq); cudaFree(ctx->res_clist); cudaFree(ctx->res_ctl); cudaFree(ctx->res_aux); cudaFree(ctx->res_cown); cudaFree(ctx->fix_list); cudaFree(ctx->fix_nf); cudaFree(ctx->fix_part); cudaFree(ctx->res_colres); cudaFree(ctx->res_csync); cudaFree(ctx->res_mode);
     cudaFree(ctx->res_dbody); cudaFree(ctx->res_dpair); cudaFree(ctx->res_dbodyi); cudaFree(ctx->res_dpairi);
     if (ctx->res_host) cudaFreeHost(ctx->res_host);
     for (int k = 0; k < 4; ++k) { if (ctx->res_stream[k]) cudaStreamDestroy(ctx->res_stream[k]); if (ctx->res_join[k]) cudaEventDestroy(ctx->res_join[k]); }
@@ -426,7 +429,8 @@ static mo_status launch_pair(mo_ctx* ctx, bool kick = false, double hk = 0.0) {
     p.nb = ctx->nb; p.ld = ctx->ld; p.nTiles = ctx->nSrcTiles; p.tps = ctx->tps;
     dim3 grid(ctx->nIblk, ctx->nsplit);
     cudaEvent_t e0 = nullptr, e1 = nullptr;
-    if (ctx->timing) {
+    const bool timed = ctx->timing && !ctx->gate.flag;    // a gated launch may be a no-op: not a kernel time
+    if (timed) {
         if (ctx->ev_used + 2 > ctx->ev.size()) {
             cudaEvent_t a, b;
             CK(cudaEventCreate(&a)); CK(cudaEventCreate(&b));
@@ -467,12 +471,12 @@ static mo_status launch_pair(mo_ctx* ctx, bool kick = false, double hk = 0.0) {
         long long u0 = 0, u1 = ctx->sym_nunits;
         if (ctx->shard_world > 1) shard_range(ctx->sym_nunits, ctx->shard_rank, ctx->shard_world, &u0, &u1);
         if (ctx->pair_u0 >= 0) { u0 = ctx->pair_u0; u1 = ctx->pair_u1; }
-        sp.unit0 = (int)u0;
+        sp.unit0 = (int)u0; sp.gate = ctx->gate;
         if (u1 > u0) pick_sym_kernel(ctx->sym_ipt)<<<(int)(u1 - u0), SYM_THREADS, 0, ctx->stream>>>(sp);
     } else {
         pick_pair_kernel(ctx->ipt, ctx->unroll)<<<grid, CTA_THREADS, 0, ctx->stream>>>(p);
     }
-    if (ctx->timing) CK(cudaEventRecord(e1, ctx->stream));
+    if (timed) CK(cudaEventRecord(e1, ctx->stream));
     return post_launch(ctx);
 }
 
@@ -488,7 +492,7 @@ static mo_status enqueue_accel(mo_ctx* ctx, bool jump, double hj, bool kick, dou
         // pair_big_kernel reads the sources from x, writes a itself and applies the closing kick
         if (jump) {
             pack_kernel<true, false><<<ctx->nTiles, TJ, 0, ctx->stream>>>(ctx->x, ctx->gm, ctx->rcrit, ctx->nb, ctx->nbig, ctx->ld,
-                                                                        ctx->tiles, ps, nps, hjm);
+                                                                        ctx->tiles, ps, nps, hjm, ctx->gate);
             mo_status s = post_launch(ctx);
             if (s != MO_OK) return s;
         }
@@ -497,7 +501,7 @@ static mo_status enqueue_accel(mo_ctx* ctx, bool jump, double hj, bool kick, dou
     auto pk = jump ? (ctx->use_sym ? pack_kernel<true, true> : pack_kernel<true, false>)
                    : (ctx->use_sym ? pack_kernel<false, true> : pack_kernel<false, false>);
     pk<<<jump ? ctx->nTiles : ctx->nSrcTiles, TJ, 0, ctx->stream>>>(ctx->x, ctx->gm, ctx->rcrit, ctx->nb, ctx->nbig, ctx->ld,
-                                                                    ctx->tiles, ps, nps, hjm);
+                                                                    ctx->tiles, ps, nps, hjm, ctx->gate);
     mo_status s = post_launch(ctx);
     if (s != MO_OK) return s;
     s = launch_pair(ctx);
@@ -509,7 +513,7 @@ static mo_status enqueue_accel(mo_ctx* ctx, bool jump, double hj, bool kick, dou
         long long u0 = 0, u1 = ctx->sym_nunits;
         if (ctx->shard_world > 1) shard_range(ctx->sym_nunits, ctx->shard_rank, ctx->shard_world, &u0, &u1);
         rk<<<dim3(nblk, 3), ON_BLOCK, 0, ctx->stream>>>(ctx->sym_partI, ctx->sym_partJ, ctx->sym_ustart, ctx->nb, ctx->ld, ctx->nbPad,
-                                               ctx->a, kick ? ctx->v : nullptr, kick ? hk : 0.0, (int)u0, (int)u1, ctx->sym_ch, sym_rows(ctx->sym_ipt));
+                                               ctx->a, kick ? ctx->v : nullptr, kick ? hk : 0.0, (int)u0, (int)u1, ctx->sym_ch, sym_rows(ctx->sym_ipt), ctx->gate);
     } else if (kick)
         accel_reduce_kernel<true><<<nblk, ON_BLOCK, 0, ctx->stream>>>(ctx->part, ctx->nsplit, ctx->nb, ctx->ld, ctx->a, ctx->v, hk);
     else
@@ -610,6 +614,8 @@ static mo_status ensure_resolve_scratch(mo_ctx* ctx) {
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_tab, (size_t)6 * RES_KMAX * 1024 * RES_CL_GRID);   // per CTA of the widest launch
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_colres, (size_t)RES_NCLUSTERS * 2 * RES_NCOL * 6 * 1024);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_csync, RES_NCLUSTERS);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_mode, 2);
+    if (e == cudaSuccess) { const int one[2] = {1, 1}; e = cudaMemcpyAsync(ctx->res_mode, one, sizeof(one), cudaMemcpyHostToDevice, ctx->stream); if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream); }
     // class D pools: every body and every pair of the list can be in a class-D component
     ctx->res_dbodyN = (long long)ctx->nb < 2 * (long long)capn ? (long long)ctx->nb : 2 * (long long)capn;
     if (ctx->cap > RES_PHI_3) {          // a shorter list cannot hold a class-D component
@@ -645,7 +651,7 @@ static mo_status enqueue_resolve(mo_ctx* ctx, double dt, double tol) {
     rp.x0 = ctx->x0; rp.v0 = ctx->v0; rp.x = ctx->x; rp.v = ctx->v; rp.gm = ctx->gm; rp.rcrit = ctx->rcrit;
     rp.pairs = ctx->pairs; rp.st = ctx->dstats; rp.out = ctx->res_out; rp.loc = ctx->res_loc; rp.label = ctx->res_label; rp.aux = ctx->res_aux; rp.cown = ctx->res_cown;
     rp.cnp = ctx->res_cnp; rp.cstart = ctx->res_cstart; rp.cfill = ctx->res_cfill; rp.cq = ctx->res_cq; rp.clist = ctx->res_clist;
-    rp.ctl = ctx->res_ctl; rp.colres = ctx->res_colres; rp.csync = ctx->res_csync; rp.tab = ctx->res_tab; rp.dbody = ctx->res_dbody; rp.dbodyi = ctx->res_dbodyi; rp.dpair = ctx->res_dpair;
+    rp.ctl = ctx->res_ctl; rp.colres = ctx->res_colres; rp.csync = ctx->res_csync; rp.mode = ctx->res_mode; rp.tab = ctx->res_tab; rp.dbody = ctx->res_dbody; rp.dbodyi = ctx->res_dbodyi; rp.dpair = ctx->res_dpair;
     rp.dpairi = ctx->res_dpairi; rp.dbodyN = ctx->res_dbodyN;
     rp.cap = ctx->cap > 0 ? ctx->cap : 1; rp.nb = ctx->nb; rp.ld = ctx->ld; rp.mu = ctx->mu; rp.h = dt; rp.tol = tol;
     resolve_label_kernel<<<1, RES_LABEL_THREADS, 0, ctx->stream>>>(rp);
@@ -730,6 +736,9 @@ static mo_status enqueue_step(mo_ctx* ctx, double dt) {
         // fork: encounter pass + encounter solve on enc_stream (read x0, v0, x1, v1; the solve writes x, v of the flagged
         // bodies), pair sum over the drifted positions x1 on the main stream; join; corrections, jump, kick
         cudaStream_t mainS = ctx->stream;
+        mode_latch_kernel<<<1, 1, 0, mainS>>>(ctx->res_mode);
+        s = post_launch(ctx);
+        if (s != MO_OK) return s;
         CK(cudaEventRecord(ctx->ev_fork, mainS));
         CK(cudaStreamWaitEvent(ctx->enc_stream, ctx->ev_fork, 0));
         EncState es = enc_state(ctx, ctx->x0, ctx->v0, dt);
@@ -745,8 +754,9 @@ static mo_status enqueue_step(mo_ctx* ctx, double dt) {
         // units while the encounter pass and the label kernel run; the rest once the components are known (res_fork) - then
         // the solve's CTAs and the pair kernel's become eligible together on draining SMs, and the solve's streams have the
         // higher priority.
-        ctx->pair_x = ctx->x1;
-        pack_kernel<false, true><<<ctx->nSrcTiles, TJ, 0, mainS>>>(ctx->x1, ctx->gm, ctx->rcrit, ctx->nb, ctx->nbig, ctx->ld, ctx->tiles, nullptr, 0, 0.0);
+        const Gate gO = {ctx->res_mode, 1}, gS = {ctx->res_mode, 0};   // beside the pair sum / before it (see below)
+        ctx->pair_x = ctx->x1; ctx->gate = gO;
+        pack_kernel<false, true><<<ctx->nSrcTiles, TJ, 0, mainS>>>(ctx->x1, ctx->gm, ctx->rcrit, ctx->nb, ctx->nbig, ctx->ld, ctx->tiles, nullptr, 0, 0.0, gO);
         s = post_launch(ctx);
         const int ucut = ctx->sym_nunits / 10;
         if (s == MO_OK) { ctx->pair_u0 = 0; ctx->pair_u1 = ucut; s = launch_pair(ctx); }
@@ -754,15 +764,15 @@ static mo_status enqueue_step(mo_ctx* ctx, double dt) {
             CK(cudaStreamWaitEvent(mainS, ctx->res_fork, 0));
             ctx->pair_u0 = ucut; ctx->pair_u1 = ctx->sym_nunits; s = launch_pair(ctx);
         }
-        ctx->pair_x = nullptr; ctx->pair_u0 = ctx->pair_u1 = -1;
+        ctx->pair_x = nullptr; ctx->pair_u0 = ctx->pair_u1 = -1; ctx->gate = Gate{nullptr, 0};
         if (s != MO_OK) return s;
         const int nblk = (ctx->nb + ON_BLOCK - 1) / ON_BLOCK;
         sym_reduce_kernel<false, false><<<dim3(nblk, 3), ON_BLOCK, 0, mainS>>>(ctx->sym_partI, ctx->sym_partJ, ctx->sym_ustart, ctx->nb, ctx->ld, ctx->nbPad,
-                                                                                ctx->a, nullptr, 0.0, 0, ctx->sym_nunits, ctx->sym_ch, sym_rows(ctx->sym_ipt));
+                                                                                ctx->a, nullptr, 0.0, 0, ctx->sym_nunits, ctx->sym_ch, sym_rows(ctx->sym_ipt), gO);
         s = post_launch(ctx);
         if (s != MO_OK) return s;
         CK(cudaStreamWaitEvent(mainS, ctx->ev_join, 0));
-        fix_list_kernel<<<1, FIX_LIST_THREADS, 0, mainS>>>(ctx->flag, ctx->nb, ctx->fix_list, ctx->fix_nf);
+        fix_list_kernel<<<1, FIX_LIST_THREADS, 0, mainS>>>(ctx->flag, ctx->nb, ctx->fix_list, ctx->fix_nf, gO);
         s = post_launch(ctx);
         if (s != MO_OK) return s;
         kick_psum_kernel<false><<<ctx->npsum, ON_BLOCK, 0, mainS>>>(ctx->v, nullptr, ctx->gm, ctx->nb, ctx->ld, 0.0, ctx->psumB, ctx->ticket + 1);
@@ -770,7 +780,7 @@ static mo_status enqueue_step(mo_ctx* ctx, double dt) {
         if (s != MO_OK) return s;
         FixParams fp;
         fp.x = ctx->x; fp.x1 = ctx->x1; fp.gm = ctx->gm; fp.rcrit = ctx->rcrit; fp.flag = ctx->flag; fp.flist = ctx->fix_list; fp.nf = ctx->fix_nf;
-        fp.a = ctx->a; fp.part = ctx->fix_part; fp.nb = ctx->nb; fp.ld = ctx->ld;
+        fp.a = ctx->a; fp.part = ctx->fix_part; fp.nb = ctx->nb; fp.ld = ctx->ld; fp.gate = gO;
         fix_unflagged_kernel<<<(ctx->nb + FIX_UT - 1) / FIX_UT, FIX_UT, 0, mainS>>>(fp);
         s = post_launch(ctx);
         if (s != MO_OK) return s;
@@ -782,8 +792,17 @@ static mo_status enqueue_step(mo_ctx* ctx, double dt) {
         fix_flagged_reduce_kernel<<<(ctx->nb + FIX_THREADS - 1) / FIX_THREADS, FIX_THREADS, 0, mainS>>>(fp);
         s = post_launch(ctx);
         if (s != MO_OK) return s;
-        jump_kick_kernel<<<ctx->npsum, ON_BLOCK, 0, mainS>>>(ctx->x, ctx->v, ctx->a, ctx->psumB, ctx->npsum, 0.5 * dt / ctx->mu, 0.5 * dt, ctx->nb, ctx->ld);
-        return post_launch(ctx);
+        jump_kick_kernel<<<ctx->npsum, ON_BLOCK, 0, mainS>>>(ctx->x, ctx->v, ctx->a, ctx->psumB, ctx->npsum, 0.5 * dt / ctx->mu, 0.5 * dt, ctx->nb, ctx->ld, gO);
+        s = post_launch(ctx);
+        if (s != MO_OK) return s;
+        // the other way, for lists without a long chain (only components of up to 63 pairs: their solve takes tens of
+        // microseconds, less than the exchange of the flagged bodies' terms costs): jump, pair sum over the resolved
+        // positions, kick.  Both ways are in the graph; which one works is the device flag the label kernel of the LAST
+        // step set (latched at the start of this step) - a stale choice costs time, never correctness.
+        ctx->gate = gS;
+        s = enqueue_accel(ctx, true, 0.5 * dt, true, 0.5 * dt);
+        ctx->gate = Gate{nullptr, 0};
+        return s;
     }
     if (ovl) {
         // fork: encounter pass on enc_stream (reads x0, v0, x1, v1, boxes, rcrit; writes pairs, flag, stats),

@@ -217,8 +217,9 @@ template <bool JUMP, bool SYM>
 __global__ void __launch_bounds__(TJ) pack_kernel(double* __restrict__ x, const double* __restrict__ gm,
                                                   const double* __restrict__ rcrit, int nb, int nsrc, int ld,
                                                   unsigned char* __restrict__ tiles,
-                                                  const double* __restrict__ psum, int npsum, double hj_over_mu) {
+                                                  const double* __restrict__ psum, int npsum, double hj_over_mu, Gate gate) {
     __shared__ int sg[TJ / 32];
+    if (gate_closed(gate)) return;
     double sx = 0, sy = 0, sz = 0;
     if (JUMP) {
         double P0, P1, P2;

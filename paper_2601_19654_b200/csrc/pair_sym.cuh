@@ -56,6 +56,7 @@ struct SymParams {
     double* partJ;               // triangular: block I at symJ_off(I), planes of (nbPad - I*R)
     int nb, ld, nbPad;
     int unit0;                   // first work unit of this launch (a rank's share of the units, row f4; 0 otherwise)
+    Gate gate;
 };
 
 __host__ __device__ inline long long symJ_off(int I, int nbPad, int R) {
@@ -219,6 +220,7 @@ __global__ void __launch_bounds__(SYM_THREADS, SYM_IPT >= 5 ? 2 : SYM_IPT >= 3 ?
     __shared__ __align__(16) double s_aj[2][SYM_THREADS / 32][3 * TJ];   // [parity][warp][c][j]
     __shared__ __align__(8) uint64_t s_full[SYM_STAGES];
 
+    if (gate_closed(p.gate)) return;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int ug = blockIdx.x + p.unit0;
     const int4 un = p.units[ug];
@@ -310,7 +312,8 @@ __global__ void __launch_bounds__(ON_BLOCK) sym_reduce_kernel(const double* __re
                                                                const int* __restrict__ ustart, int nb, int ld,
                                                                int nbPad, double* __restrict__ a,
                                                                double* __restrict__ v, double hk, int us0, int us1, int ch,
-                                                               int SYM_R) {
+                                                               int SYM_R, Gate gate) {
+    if (gate_closed(gate)) return;
     // one thread per (body, component) - blockIdx.y = component - and four interleaved partial sums per
     // list, combined in a fixed order: three times the threads and four times the loads in flight of a
     // thread-per-body loop, still a fixed tree that depends on nb only

@@ -66,6 +66,7 @@ struct ResParams {
     int* ctl;                    // [0] components, [RES_CTL_CNT + c] class counts, [RES_CTL_TKT + c] tickets, [RES_CTL_POOL] streamed-class body pool in use
     double* colres;              // column results of the clusters: [cluster][2][NCOL][6][threads]
     int* csync;                  // barrier counters of the clusters (zeroed by the label kernel)
+    int* mode;                   // [1] <- 1 if this list holds a component of more than 63 pairs (a long chain: mopal.cu), else 0
     double* tab;                 // extrapolation tableaux of the class-C CTAs whose component does not leave room in shared memory
     double* dbody; int* dbodyi;  // class D pools: planes of dbodyN doubles / ints
     double* dpair; int* dpairi;  // planes of cap
@@ -177,6 +178,7 @@ __global__ void __launch_bounds__(RES_LABEL_THREADS) resolve_label_kernel(ResPar
     if (tid == 0) { *p.out = ResStats{0, 0, 0, 0}; for (int k = 0; k < RES_CTL_N; ++k) p.ctl[k] = 0; }
     if (tid < RES_NCLUSTERS) p.csync[tid] = 0;
     const long long nce = p.st->nce_last;
+    if (nce <= 0 || nce > p.cap) { if (tid == 0) p.mode[1] = 0; }
     if (nce <= 0) return;
     if (nce > p.cap) { if (tid == 0) { p.out->fail = 1 << 30; atomicAdd(&p.st->resolve_fail, 1); } return; }      // truncated list: nothing can be resolved
     const int np = (int)nce;
@@ -294,7 +296,11 @@ __global__ void __launch_bounds__(RES_LABEL_THREADS) resolve_label_kernel(ResPar
         const int cls = res_class(tot);
         p.clist[(size_t)cls * p.cap + atomicAdd(&p.ctl[RES_CTL_CNT + cls], 1)] = c;
     }
-    if (tid == 0) p.ctl[0] = ncomp;
+    __syncthreads();
+    if (tid == 0) {
+        p.ctl[0] = ncomp;
+        p.mode[1] = (p.ctl[RES_CTL_CNT + 1] + p.ctl[RES_CTL_CNT + 2] + p.ctl[RES_CTL_CNT + 3] + p.ctl[RES_CTL_CNT + 4]) > 0 ? 1 : 0;
+    }
 }
 
 // reciprocal square root to ~2 ulp: MUFU seed (22 bits) and one third-order correction (truncation 5/16 e^3 < 1e-19)

@@ -984,11 +984,12 @@ def test_resolve_several_components_interleaved(M):
         assert np.linalg.norm(gv[:, b] - v1[:, b]) / np.linalg.norm(v1[:, b]) > 1e-8, b
 
 
-@pytest.mark.parametrize("cfg,N", [(0, 256), (1, 1500), (3, 3000), (3, 9000)])
+@pytest.mark.parametrize("cfg,N", [(0, 256), (1, 1500), (3, 3000), (3, 9000), (4, 24000)])
 def test_resolve_inside_step_vs_oracle(M, cfg, N):
     """mo_set_resolve: kick, jump, snapshot, drift, encounter check, encounter solve, jump, accel, kick.  From 2561 bodies
     on the solve runs BESIDE the pair sum (fixup.cuh: the sum over the drifted positions, then the flagged bodies' terms
-    exchanged and their own rows recomputed) - the result is the same step."""
+    exchanged and their own rows recomputed) - the result is the same step.  (4, 24000): planetesimal pairs only, no long
+    chain - after the first step the device flag sends the step the other way (solve, then the pair sum), both in the graph."""
     w = W.make_config(cfg) if N == 256 else W.shrink(cfg, N)
     mu, gm = G * w.m_star, G * w.mass
     m = _mk(M, w)
@@ -1016,7 +1017,7 @@ def test_resolve_inside_step_vs_oracle(M, cfg, N):
         tol = (RES_RTOL(1e-12) + 2e-13) * (1 + k)
         assert _rel_vec_err(m.get("x"), x).max() <= tol and _rel_vec_err(m.get("v"), v).max() <= tol, k
         assert st.nce_last == enc["count"] and st.resolve_fail == 0
-    assert nres == 3
+    assert nres == 3 or cfg == 4
     m2 = _mk(M, w); m2.set_resolve(1e-12); m2.step(w.dt, 3)           # graph replay: bit for bit the same
     assert np.array_equal(m.get("x"), m2.get("x")) and np.array_equal(m.get("v"), m2.get("v"))
     m.close(); m2.close()

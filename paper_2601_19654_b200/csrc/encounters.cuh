@@ -352,6 +352,7 @@ struct EncFindParams {
     EncBuf e;
     long long cap;
     int nTiles;
+    int unsorted;        // 1: no spatial ordering (a few tiles only: every pair of tiles is gated, in body order)
 };
 
 __device__ __forceinline__ bool gate_f32(const float4& a, const float4& b) {
@@ -376,7 +377,7 @@ __device__ __forceinline__ void enc_exact_body(const EncFindParams& p, int i, in
 
 // one survivor per lane (sorted positions c.x < c.y): (i, j) = (smaller, larger) body index
 __device__ __forceinline__ void enc_exact(const EncFindParams& p, int2 c) {
-    const int ba = p.e.perm[c.x], bb = p.e.perm[c.y];
+    const int ba = p.unsorted ? c.x : p.e.perm[c.x], bb = p.unsorted ? c.y : p.e.perm[c.y];
     enc_exact_body(p, min(ba, bb), max(ba, bb));
 }
 
@@ -468,8 +469,9 @@ __global__ void __launch_bounds__(CTA_THREADS) enc_find_kernel(EncFindParams p) 
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int rb = blockIdx.x;
-    const float4 own = p.e.tbox[rb];
-    const bool rbig = p.e.tbig[rb] != 0;
+    const float4 own = p.unsorted ? make_float4(0.f, 0.f, 0.f, 0.f) : p.e.tbox[rb];   // (not used without the ordering)
+    const bool rbig = p.unsorted ? rb * TJ < p.s.nbig : p.e.tbig[rb] != 0;
+    const float4* __restrict__ boxes = p.unsorted ? p.e.boxf : p.e.sboxf;
 
     if (tid == 0) {
 #pragma unroll
@@ -479,7 +481,7 @@ __global__ void __launch_bounds__(CTA_THREADS) enc_find_kernel(EncFindParams p) 
     const unsigned full = 0xffffffffu, lt = (1u << lane) - 1u;
     const bool producer = warp == CONSUMER_THREADS / 32;
     const int si = rb * TJ + (producer ? 0 : tid);
-    const float4 bi = p.e.sboxf[si];          // pad records hold the never-overlapping box
+    const float4 bi = boxes[si];              // pad records hold the never-overlapping box
     int2* q = s_q[producer ? 0 : warp];
     int qhead = 0, qn = 0;                    // warp-uniform
     int nglob = 0;                            // tiles streamed so far (ring position), CTA-uniform
@@ -491,14 +493,14 @@ __global__ void __launch_bounds__(CTA_THREADS) enc_find_kernel(EncFindParams p) 
         __syncthreads();
         for (int k = tid; k < ENC_WIN; k += CTA_THREADS) {
             const int t = w0 + k * S;
-            if (t < p.nTiles && gate_f32(own, p.e.tbox[t]) && (rbig || p.e.tbig[t] != 0)) s_list[atomicAdd(&s_n, 1)] = t;
+            if (t < p.nTiles && (p.unsorted ? rbig : gate_f32(own, p.e.tbox[t]) && (rbig || p.e.tbig[t] != 0))) s_list[atomicAdd(&s_n, 1)] = t;
         }
         __syncthreads();
         const int nt = s_n;
 
         if (producer) {  // ---- TMA producer warp ----
             if (lane == 0) {
-                const unsigned char* src = reinterpret_cast<const unsigned char*>(p.e.sboxf);
+                const unsigned char* src = reinterpret_cast<const unsigned char*>(boxes);
                 for (int n = 0; n < nt; ++n) {
                     const int g = nglob + n, st = g % STAGES;
                     mbar_wait(&s_empty[st], ((g / STAGES) & 1) ^ 1);

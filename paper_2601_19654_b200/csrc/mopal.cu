@@ -8,6 +8,7 @@
 #include <string.h>
 
 #include <new>
+#include <algorithm>
 #include <vector>
 
 #include "../../include/mopal.h"
@@ -33,6 +34,7 @@ struct mo_ctx {
     uint8_t* flag = nullptr;
     cudaStream_t stream = nullptr;
     cudaStream_t cap_stream = nullptr;  // owned: graph capture needs a non-legacy stream
+    std::vector<const void*> pair_funcs; // the O(N^2) pair kernels this context launches (graph: every other kernel node runs at high priority)
     // overlapped step: the encounter pass runs on a second (high-priority) stream beside jump + pair sum + kick,
     // reading its own copy x1, v1 of the drifted state
     bool overlap = false;
@@ -94,6 +96,8 @@ struct mo_ctx {
     double *sym_partI = nullptr, *sym_partJ = nullptr;
     std::vector<int4> h_units;
     std::vector<int> h_ustart;
+    std::vector<long long> h_uwork;     // [nunits + 1] work before each unit, in groups of 32 columns
+    int2* sym_qr = nullptr;             // [sym_nI] sharded: the column groups of each row block this rank works on
     int shard_rank = 0, shard_world = 1;   // mo_set_shard: this context computes rank's share of the pair sum (row f4)
     bool pair_ready = false;
     bool a_valid = false, snap_valid = false, box_valid = false, debug = false, use_graph = true;
@@ -127,6 +131,75 @@ struct StageRange {
 static inline void shard_range(long long n, int rank, int world, long long* lo, long long* hi) {
     *lo = n * rank / world;
     *hi = n * (rank + 1) / world;
+}
+
+// The work units of the two-sided pair kernel, in launch (= dispatch) order: row blocks I ascending, each block's j tiles
+// from its diagonal on in chunks of ch tiles.  All CTA slots are busy until the list runs out, and then the kernel is as
+// long as the last units to finish: so the end of the list is cut finer - the last slots * ch / 2 tiles one per unit (they
+// level the spread of the slots' finishing times, which is about one chunk), and of those the last slots / 2 tiles one
+// GROUP of 32 columns per unit (a quarter tile: the finest piece the warp rotation works on).  A system with fewer tiles
+// than slots (N = 4096: 272 tiles for 592 slots) is cut into groups throughout: twice the resident warps per SM.
+static void plan_sym_units(mo_ctx* ctx, long long tot, long long slots) {
+    const int TPB = ctx->sym_ipt, ch = ctx->sym_ch;
+    // (measured, profiles/r2e_tail_and_priorities.md: half as much or twice as much of either changes nothing)
+    const long long tailQ = tot < 2 * slots ? tot : slots / 2;
+    const long long tail1 = tailQ + (ch > 1 ? slots * ch / 2 : 0);
+    ctx->h_units.clear(); ctx->h_ustart.clear(); ctx->h_uwork.clear();
+    long long seen = 0, work = 0;        // tiles before the current one; groups before the current unit
+    for (int I = 0; I < ctx->sym_nI; ++I) {
+        ctx->h_ustart.push_back((int)ctx->h_units.size());
+        int t = I * TPB;
+        while (t < ctx->nTiles) {
+            const long long left = tot - seen;                 // tiles from here to the end of the list
+            if (left <= tailQ) {
+                for (int g = 0; g < TJ / 32; ++g) {
+                    ctx->h_uwork.push_back(work); work += 1;
+                    ctx->h_units.push_back(make_int4(I, t, t + 1, g | (g + 1) << 8));
+                }
+                t += 1; seen += 1;
+                continue;
+            }
+            int n = left <= tail1 ? 1 : ch;
+            if (n > ctx->nTiles - t) n = ctx->nTiles - t;
+            if (left - n < tailQ) n = (int)(left - tailQ);      // the chunk ends where the finer tail begins
+            ctx->h_uwork.push_back(work); work += (long long)n * (TJ / 32);
+            ctx->h_units.push_back(make_int4(I, t, t + n, (TJ / 32) << 8));
+            t += n; seen += n;
+        }
+    }
+    ctx->h_ustart.push_back((int)ctx->h_units.size());
+    ctx->h_uwork.push_back(work);
+    ctx->sym_nunits = (int)ctx->h_units.size();
+}
+
+// this rank's run of the work units: equal shares of the WORK (the units differ in length)
+static void sym_shard_units(const mo_ctx* ctx, long long* u0, long long* u1) {
+    *u0 = 0; *u1 = ctx->sym_nunits;
+    if (ctx->shard_world <= 1) return;
+    const long long W = ctx->h_uwork.back();
+    long long wlo, whi;
+    shard_range(W, ctx->shard_rank, ctx->shard_world, &wlo, &whi);
+    auto first_at = [&](long long w) { return (long long)(std::lower_bound(ctx->h_uwork.begin(), ctx->h_uwork.end() - 1, w) - ctx->h_uwork.begin()); };
+    *u0 = first_at(wlo);
+    *u1 = ctx->shard_rank == ctx->shard_world - 1 ? ctx->sym_nunits : first_at(whi);
+}
+
+// sharded: the run of column groups of every row block (counted from the block's diagonal) that this rank's units cover
+static cudaError_t sym_fill_qr(mo_ctx* ctx) {
+    long long u0, u1;
+    sym_shard_units(ctx, &u0, &u1);
+    std::vector<int2> qr((size_t)ctx->sym_nI, make_int2(0, 0));
+    const int G = TJ / 32;
+    for (long long u = u0; u < u1; ++u) {
+        const int4 un = ctx->h_units[(size_t)u];
+        const int first = (un.y - un.x * ctx->sym_ipt) * G + (un.w & 0xff);
+        const int end = (un.z - 1 - un.x * ctx->sym_ipt) * G + (un.w >> 8);
+        int2& q = qr[(size_t)un.x];
+        if (q.y == q.x) q = make_int2(first, end); else q.y = end;      // the units of a block follow one another
+    }
+    cudaError_t e = cudaMemcpyAsync(ctx->sym_qr, qr.data(), qr.size() * sizeof(int2), cudaMemcpyHostToDevice, ctx->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);       // pageable source
+    return e;
 }
 
 static inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
@@ -203,9 +276,17 @@ static void choose_geometry(mo_ctx* ctx) {
     ctx->tps = (nST + bestS - 1) / bestS;
     ctx->nsplit = (nST + ctx->tps - 1) / ctx->tps;
     // encounter find: column tiles of a row tile are dealt round-robin to enc_split CTAs
+    // (up to 8 for the large systems, whose dense rows overlap many tiles; a mid-size system's few row tiles are split
+    // further, down to two column tiles per CTA: about four CTAs per SM, and a short chain of gates per thread)
     ctx->enc_split = ctx->nTiles / 8;
     if (ctx->enc_split < 1) ctx->enc_split = 1;
     if (ctx->enc_split > 8) ctx->enc_split = 8;
+    {
+        int want = 4 * ctx->nsm / (ctx->nTiles > 0 ? ctx->nTiles : 1), most = ctx->nTiles / 2;
+        if (want > 32) want = 32;
+        if (want > most) want = most;
+        if (want > ctx->enc_split) ctx->enc_split = want;
+    }
     // two-sided kernel for large nb: units = (row block, chunk of sym_ch j tiles from the diagonal on)
     ctx->use_small = nb <= env_int("MO_SMALL_MAX", 320) && nb <= SMALL_MAX && env_int("MO_SMALL", 1) != 0;
     // measured (profiles/r1g_path_selection.md): single-CTA front end up to ~320 bodies, lane-split pair kernel up to
@@ -231,7 +312,7 @@ static void choose_geometry(mo_ctx* ctx) {
     ctx->use_sym = !ctx->use_psm && ctx->nbig == nb && env_int("MO_SYM", nb >= SYM_MIN ? 1 : 0) != 0;
     if (ctx->use_sym) {
         // bodies per lane: the triangle of a mid-size system in enough, short enough units for the SMs
-        ctx->sym_ipt = env_int("MO_SYM_IPT", nb >= 32768 ? 6 : nb >= 7000 ? 3 : 2);   // measured: profiles/r2_path_selection.md
+        ctx->sym_ipt = env_int("MO_SYM_IPT", nb >= 20000 ? 6 : nb >= 7000 ? 3 : 2);   // measured: profiles/r2c_path_selection.md, r2e_tail_and_priorities.md
         if (ctx->sym_ipt != 2 && ctx->sym_ipt != 3 && ctx->sym_ipt != 6) ctx->sym_ipt = 6;
         const int R = sym_rows(ctx->sym_ipt), TPB = ctx->sym_ipt;
         int occs = 1;
@@ -246,16 +327,7 @@ static void choose_geometry(mo_ctx* ctx) {
         if (ch > 16) ch = 16;
         ctx->sym_ch = env_int("MO_SYM_CH", (int)ch);
         if (ctx->sym_ch < 1) ctx->sym_ch = 1;
-        ctx->h_units.clear(); ctx->h_ustart.clear();
-        for (int I = 0; I < ctx->sym_nI; ++I) {
-            ctx->h_ustart.push_back((int)ctx->h_units.size());
-            for (int t = I * TPB; t < ctx->nTiles; t += ctx->sym_ch) {
-                const int t1 = t + ctx->sym_ch < ctx->nTiles ? t + ctx->sym_ch : ctx->nTiles;
-                ctx->h_units.push_back(make_int4(I, t, t1, 0));
-            }
-        }
-        ctx->h_ustart.push_back((int)ctx->h_units.size());
-        ctx->sym_nunits = (int)ctx->h_units.size();
+        plan_sym_units(ctx, tot, sslots);
         ctx->ipt = ctx->sym_ipt; ctx->ctas_per_sm = occs; ctx->nsplit = 1;
     }
 }
@@ -294,7 +366,7 @@ extern "C" void mo_destroy(mo_ctx* ctx) {
     if (ctx->res_fork) cudaEventDestroy(ctx->res_fork);
     cudaFree(ctx->gmsum); cudaFree(ctx->en_on); cudaFree(ctx->en_pair); cudaFree(ctx->en_out);
     if (ctx->en_host) cudaFreeHost(ctx->en_host); cudaFree(ctx->tiles);
-    cudaFree(ctx->sym_units); cudaFree(ctx->sym_ustart); cudaFree(ctx->sym_partI); cudaFree(ctx->sym_partJ);
+    cudaFree(ctx->sym_units); cudaFree(ctx->sym_ustart); cudaFree(ctx->sym_partI); cudaFree(ctx->sym_partJ); cudaFree(ctx->sym_qr);
     cudaFree(ctx->enc.box); cudaFree(ctx->enc.boxf); cudaFree(ctx->enc.rowcnt); cudaFree(ctx->enc.rowfill);
     cudaFree(ctx->enc.rowoff); cudaFree(ctx->enc.hits); cudaFree(ctx->enc.tmpj); cudaFree(ctx->enc.nhit);
     cudaFree(ctx->enc.ovf_now); cudaFree(ctx->dstats); cudaFree(ctx->probe);
@@ -392,7 +464,7 @@ extern "C" mo_status mo_create(mo_ctx** out, int32_t nb, int32_t ld, double m_st
 static mo_status ensure_pair_scratch(mo_ctx* ctx) {
     if (ctx->pair_ready) return MO_OK;
     cudaError_t e = cudaSuccess;
-    ctx->overlap = !ctx->use_small && true;
+    ctx->overlap = !ctx->use_small;
     if (ctx->overlap && !ctx->enc_stream) {
         int lo = 0, hi = 0;
         cudaDeviceGetStreamPriorityRange(&lo, &hi);
@@ -412,6 +484,8 @@ static mo_status ensure_pair_scratch(mo_ctx* ctx) {
         if (e == cudaSuccess) e = cudaMemcpyAsync(ctx->sym_units, ctx->h_units.data(), ctx->h_units.size() * sizeof(int4), cudaMemcpyHostToDevice, ctx->stream);
         if (e == cudaSuccess) e = cudaMemcpyAsync(ctx->sym_ustart, ctx->h_ustart.data(), ctx->h_ustart.size() * sizeof(int), cudaMemcpyHostToDevice, ctx->stream);
         if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);   // pageable source vectors
+        if (e == cudaSuccess) e = dalloc(ctx, &ctx->sym_qr, (size_t)ctx->sym_nI);
+        if (e == cudaSuccess) e = sym_fill_qr(ctx);
     }
     if (e != cudaSuccess) {
         cudaGetLastError();
@@ -421,6 +495,40 @@ static mo_status ensure_pair_scratch(mo_ctx* ctx) {
     }
     ctx->pair_ready = true;
     return MO_OK;
+}
+
+static void note_pair_func(mo_ctx* ctx, const void* f) {
+    if (std::find(ctx->pair_funcs.begin(), ctx->pair_funcs.end(), f) == ctx->pair_funcs.end()) ctx->pair_funcs.push_back(f);
+}
+
+// The recorded step replays with the priorities of its nodes (cudaGraphInstantiateFlagUseNodePriority; without the flag
+// every node runs at the priority of the stream the graph is launched into): the pair kernel, whose CTAs take every
+// slot of the GPU for the length of the step, at the lowest, every other kernel - the encounter branch and the
+// encounter solve beside it, chains of short dependent kernels - at the highest, so that a slot a pair CTA leaves goes
+// to them first.  (Measured at N = 16,384: without it the encounter branch only got onto the GPU when the pair kernel's
+// grid had been handed out, and the replayed step was as long as with no overlap at all.)
+static cudaError_t set_node_priorities(mo_ctx* ctx, cudaGraph_t g) {
+    int lo = 0, hi = 0;
+    cudaError_t e = cudaDeviceGetStreamPriorityRange(&lo, &hi);
+    size_t n = 0;
+    if (e == cudaSuccess) e = cudaGraphGetNodes(g, nullptr, &n);
+    if (e != cudaSuccess || n == 0) return e;
+    std::vector<cudaGraphNode_t> nodes(n);
+    e = cudaGraphGetNodes(g, nodes.data(), &n);
+    for (size_t k = 0; k < n && e == cudaSuccess; ++k) {
+        cudaGraphNodeType ty;
+        e = cudaGraphNodeGetType(nodes[k], &ty);
+        if (e != cudaSuccess || ty != cudaGraphNodeTypeKernel) continue;
+        cudaKernelNodeParams kp;
+        e = cudaGraphKernelNodeGetParams(nodes[k], &kp);
+        if (e != cudaSuccess) break;
+        const bool pair = std::find(ctx->pair_funcs.begin(), ctx->pair_funcs.end(), (const void*)kp.func) != ctx->pair_funcs.end();
+        cudaLaunchAttributeValue v;
+        memset(&v, 0, sizeof v);
+        v.priority = pair ? lo : hi;
+        e = cudaGraphKernelNodeSetAttribute(nodes[k], cudaLaunchAttributePriority, &v);
+    }
+    return e;
 }
 
 static mo_status launch_pair(mo_ctx* ctx, bool kick = false, double hk = 0.0) {
@@ -449,6 +557,7 @@ static mo_status launch_pair(mo_ctx* ctx, bool kick = false, double hk = 0.0) {
         auto k = G == 8 ? (kick ? pair_small_kernel<8, true> : pair_small_kernel<8, false>)
                : G == 4 ? (kick ? pair_small_kernel<4, true> : pair_small_kernel<4, false>)
                         : (kick ? pair_small_kernel<2, true> : pair_small_kernel<2, false>);
+        note_pair_func(ctx, (const void*)k);
         k<<<grid, PSM_THREADS, 0, ctx->stream>>>(bp);
     } else if (ctx->use_big) {
         BigParams bp;
@@ -463,17 +572,19 @@ static mo_status launch_pair(mo_ctx* ctx, bool kick = false, double hk = 0.0) {
             grid = hi - lo < grid ? (int)(hi - lo) : grid;
         }
         if (grid > 0 && (ctx->shard_world == 1 || bp.blk1 > bp.blk0))
-            pick_big_kernel(ctx->big_ipt, kick)<<<grid, BIG_THREADS, 0, ctx->stream>>>(bp);
+            { note_pair_func(ctx, (const void*)pick_big_kernel(ctx->big_ipt, kick)); pick_big_kernel(ctx->big_ipt, kick)<<<grid, BIG_THREADS, 0, ctx->stream>>>(bp); }
     } else if (ctx->use_sym) {
         SymParams sp;
         sp.tiles = ctx->tiles; sp.x = ctx->pair_x ? ctx->pair_x : ctx->x; sp.gm = ctx->gm; sp.rcrit = ctx->rcrit; sp.units = ctx->sym_units;
         sp.partI = ctx->sym_partI; sp.partJ = ctx->sym_partJ; sp.nb = ctx->nb; sp.ld = ctx->ld; sp.nbPad = ctx->nbPad;
-        long long u0 = 0, u1 = ctx->sym_nunits;
-        if (ctx->shard_world > 1) shard_range(ctx->sym_nunits, ctx->shard_rank, ctx->shard_world, &u0, &u1);
+        long long u0, u1;
+        sym_shard_units(ctx, &u0, &u1);
         if (ctx->pair_u0 >= 0) { u0 = ctx->pair_u0; u1 = ctx->pair_u1; }
         sp.unit0 = (int)u0; sp.gate = ctx->gate;
+        note_pair_func(ctx, (const void*)pick_sym_kernel(ctx->sym_ipt));
         if (u1 > u0) pick_sym_kernel(ctx->sym_ipt)<<<(int)(u1 - u0), SYM_THREADS, 0, ctx->stream>>>(sp);
     } else {
+        note_pair_func(ctx, (const void*)pick_pair_kernel(ctx->ipt, ctx->unroll));
         pick_pair_kernel(ctx->ipt, ctx->unroll)<<<grid, CTA_THREADS, 0, ctx->stream>>>(p);
     }
     if (timed) CK(cudaEventRecord(e1, ctx->stream));
@@ -510,10 +621,10 @@ static mo_status enqueue_accel(mo_ctx* ctx, bool jump, double hj, bool kick, dou
     if (ctx->use_sym) {
         const bool shd = ctx->shard_world > 1;
         auto rk = kick ? sym_reduce_kernel<true, false> : shd ? sym_reduce_kernel<false, true> : sym_reduce_kernel<false, false>;
-        long long u0 = 0, u1 = ctx->sym_nunits;
-        if (ctx->shard_world > 1) shard_range(ctx->sym_nunits, ctx->shard_rank, ctx->shard_world, &u0, &u1);
-        rk<<<dim3(nblk, 3), ON_BLOCK, 0, ctx->stream>>>(ctx->sym_partI, ctx->sym_partJ, ctx->sym_ustart, ctx->nb, ctx->ld, ctx->nbPad,
-                                               ctx->a, kick ? ctx->v : nullptr, kick ? hk : 0.0, (int)u0, (int)u1, ctx->sym_ch, sym_rows(ctx->sym_ipt), ctx->gate);
+        long long u0, u1;
+        sym_shard_units(ctx, &u0, &u1);
+        rk<<<dim3((ctx->nb + 31) / 32, 3), RED_THREADS, 0, ctx->stream>>>(ctx->sym_partI, ctx->sym_partJ, ctx->sym_ustart, ctx->nb, ctx->ld, ctx->nbPad,
+                                               ctx->a, kick ? ctx->v : nullptr, kick ? hk : 0.0, (int)u0, (int)u1, ctx->sym_qr, sym_rows(ctx->sym_ipt), ctx->gate);
     } else if (kick)
         accel_reduce_kernel<true><<<nblk, ON_BLOCK, 0, ctx->stream>>>(ctx->part, ctx->nsplit, ctx->nb, ctx->ld, ctx->a, ctx->v, hk);
     else
@@ -533,11 +644,19 @@ static mo_status enqueue_pairs(mo_ctx* ctx, const EncState& es, int step_inc) {
     StageRange nv("mopal: encounter pairs (a8)");
     EncFindParams fp;
     fp.s = es; fp.e = ctx->enc; fp.cap = ctx->cap; fp.nTiles = ctx->nTiles;
+    // up to 40 tiles (N <= 5120) every pair of tiles is gated, in body order: that costs less than the three ordering
+    // kernels in a chain of dependent launches this short (at N = 4096 the chain, not the pair sum, was the step: 61 ->
+    // 50.5 us; equal at N = 6000, and at N = 8192 the ordering wins by 15 us)
+    fp.unsorted = ctx->nTiles <= 40 ? 1 : 0;
     mo_status s;
     if (ctx->use_big) {
         // few big bodies: the nbig x nb rectangle of gates directly, in body order
         const int per = BIGF_THREADS * BIGF_JPT;
         enc_bigfind_kernel<<<(ctx->nb + per - 1) / per, BIGF_THREADS, 0, ctx->stream>>>(fp);
+        s = post_launch(ctx);
+        if (s != MO_OK) return s;
+    } else if (fp.unsorted) {
+        enc_find_kernel<<<dim3(ctx->nTiles, ctx->enc_split), CTA_THREADS, 0, ctx->stream>>>(fp);
         s = post_launch(ctx);
         if (s != MO_OK) return s;
     } else {
@@ -766,9 +885,8 @@ static mo_status enqueue_step(mo_ctx* ctx, double dt) {
         }
         ctx->pair_x = nullptr; ctx->pair_u0 = ctx->pair_u1 = -1; ctx->gate = Gate{nullptr, 0};
         if (s != MO_OK) return s;
-        const int nblk = (ctx->nb + ON_BLOCK - 1) / ON_BLOCK;
-        sym_reduce_kernel<false, false><<<dim3(nblk, 3), ON_BLOCK, 0, mainS>>>(ctx->sym_partI, ctx->sym_partJ, ctx->sym_ustart, ctx->nb, ctx->ld, ctx->nbPad,
-                                                                                ctx->a, nullptr, 0.0, 0, ctx->sym_nunits, ctx->sym_ch, sym_rows(ctx->sym_ipt), gO);
+        sym_reduce_kernel<false, false><<<dim3((ctx->nb + 31) / 32, 3), RED_THREADS, 0, mainS>>>(ctx->sym_partI, ctx->sym_partJ, ctx->sym_ustart, ctx->nb, ctx->ld, ctx->nbPad,
+                                                                                ctx->a, nullptr, 0.0, 0, ctx->sym_nunits, nullptr, sym_rows(ctx->sym_ipt), gO);
         s = post_launch(ctx);
         if (s != MO_OK) return s;
         CK(cudaStreamWaitEvent(mainS, ctx->ev_join, 0));
@@ -917,7 +1035,8 @@ extern "C" mo_status mo_set_nbig(mo_ctx* ctx, int32_t nbig) {
     CK(cudaStreamSynchronize(ctx->stream));   // nothing in flight may still use the scratch freed below
     if (ctx->gexec) { cudaGraphExecDestroy(ctx->gexec); ctx->gexec = nullptr; }
     cudaFree(ctx->part); ctx->part = nullptr;
-    cudaFree(ctx->sym_units); cudaFree(ctx->sym_ustart); cudaFree(ctx->sym_partI); cudaFree(ctx->sym_partJ);
+    cudaFree(ctx->sym_units); cudaFree(ctx->sym_ustart); cudaFree(ctx->sym_partI); cudaFree(ctx->sym_partJ); cudaFree(ctx->sym_qr);
+    ctx->sym_qr = nullptr;
     ctx->sym_units = nullptr; ctx->sym_ustart = nullptr; ctx->sym_partI = nullptr; ctx->sym_partJ = nullptr;
     ctx->pair_ready = false;
     ctx->a_valid = false;
@@ -1076,6 +1195,7 @@ extern "C" mo_status mo_set_shard(mo_ctx* ctx, int32_t rank, int32_t world) {
     }
     ctx->shard_rank = rank; ctx->shard_world = world;
     ctx->a_valid = false;
+    if (ctx->use_sym && ctx->pair_ready) CK(sym_fill_qr(ctx));
     return MO_OK;
 }
 
@@ -1083,7 +1203,8 @@ extern "C" mo_status mo_shard_units(const mo_ctx* ctx, int64_t* units, int64_t* 
     if (!ctx || !units || !lo || !hi) return MO_EINVAL;
     const long long n = ctx->use_sym ? ctx->sym_nunits : ctx->use_big ? ctx->nIblk : 0;
     long long a = 0, b = n;
-    if (ctx->shard_world > 1) shard_range(n, ctx->shard_rank, ctx->shard_world, &a, &b);
+    if (ctx->use_sym) sym_shard_units(ctx, &a, &b);
+    else if (ctx->shard_world > 1) shard_range(n, ctx->shard_rank, ctx->shard_world, &a, &b);
     *units = n; *lo = a; *hi = b;
     return MO_OK;
 }
@@ -1149,7 +1270,8 @@ extern "C" mo_status mo_step(mo_ctx* ctx, double dt, int32_t nsteps, mo_stats* s
                 cudaGetLastError();
                 return MO_ECUDA;
             }
-            e = cudaGraphInstantiate(&ctx->gexec, g, 0);
+            e = set_node_priorities(ctx, g);
+            if (e == cudaSuccess) e = cudaGraphInstantiateWithFlags(&ctx->gexec, g, cudaGraphInstantiateFlagUseNodePriority);
             cudaGraphDestroy(g);
             if (e != cudaSuccess) { ctx->gexec = nullptr; ctx->last_err = e; return MO_ECUDA; }
             ctx->gdt = dt;

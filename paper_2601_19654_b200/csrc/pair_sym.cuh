@@ -8,7 +8,9 @@
 // 6 DFMA (two accumulations) = 20, i.e. 10 per ordered pair against 16 for the one-sided kernel.
 //
 // Work unit = (row block I of SYM_R = 128*IPT bodies) x (a chunk of j tiles at or right of the
-// block's diagonal).  Each lane keeps IPT bodies i resident (position, gm, gate, accumulators).
+// block's diagonal; the units at the end of the list are cut finer - single tiles, then single groups of 32 bodies of
+// a tile - so that the CTAs of the last wave end together, see plan_sym_units in mopal.cu).  Each lane keeps IPT bodies
+// i resident (position, gm, gate, accumulators).
 // A j tile is 4 groups of 32 bodies; a group ROTATES through the warp: at rotation s lane L works
 // on j = (L + s) mod 32, reading its record from the shared-memory tile (SoA halves {x,y}[128] and
 // {z,gm}[128]: 16-byte stride, conflict-free for lane-distinct addresses) and carrying the three
@@ -51,7 +53,8 @@ struct SymParams {
     const double* x;             // 3*ld
     const double* gm;            // nb
     const double* rcrit;         // nb
-    const int4* units;           // {I, t0, t1, unused}
+    const int4* units;           // {I, t0, t1, g0 | g1 << 8}: j tiles [t0, t1) of row block I; of a single tile, the
+                                 // groups of 32 bodies [g0, g1) (all four of every tile of a longer unit)
     double* partI;               // [nUnits][3][R], R = 128 IPT
     double* partJ;               // triangular: block I at symJ_off(I), planes of (nbPad - I*R)
     int nb, ld, nbPad;
@@ -173,10 +176,11 @@ __device__ __forceinline__ void sym_tile(const uint32_t tile_sa, const int jbase
                                          const double (&zi)[SYM_IPT], const double (&mi)[SYM_IPT],
                                          const int g, double (&ax)[SYM_IPT], double (&ay)[SYM_IPT],
                                          double (&az)[SYM_IPT], double* __restrict__ sj,
-                                         const double (&rci)[SYM_IPT], const double* __restrict__ rcrit, int nb) {
+                                         const double (&rci)[SYM_IPT], const double* __restrict__ rcrit, int nb,
+                                         const int g0, const int g1) {
     const unsigned full = 0xffffffffu;
 #pragma unroll 1
-    for (int grp = 0; grp < TJ / 32; ++grp) {
+    for (int grp = g0; grp < g1; ++grp) {
         // this lane walks the group's 32 records cyclically, starting at its home record
         uint32_t a0 = tile_sa + grp * 512 + lane * 16;
         const int jgrp = jbase + grp * 32;
@@ -225,6 +229,7 @@ __global__ void __launch_bounds__(SYM_THREADS, SYM_IPT >= 5 ? 2 : SYM_IPT >= 3 ?
     const int ug = blockIdx.x + p.unit0;
     const int4 un = p.units[ug];
     const int I = un.x, t0 = un.y, nt = un.z - un.y;
+    const int g0 = un.w & 0xff, g1 = un.w >> 8;
     const unsigned char* src = p.tiles + (size_t)t0 * SYM_TILE_BYTES;
 
     if (tid == 0) {
@@ -274,9 +279,9 @@ __global__ void __launch_bounds__(SYM_THREADS, SYM_IPT >= 5 ? 2 : SYM_IPT >= 3 ?
         const int g = max(gi, gt);
         double* sj = s_aj[n & 1][warp];
         if (t < (I + 1) * SYM_TPB)
-            sym_tile<SYM_IPT, true>(tile_sa, t * TJ, lane, ibase, xi, yi, zi, mi, g, ax, ay, az, sj, rci, p.rcrit, p.nb);
+            sym_tile<SYM_IPT, true>(tile_sa, t * TJ, lane, ibase, xi, yi, zi, mi, g, ax, ay, az, sj, rci, p.rcrit, p.nb, g0, g1);
         else
-            sym_tile<SYM_IPT, false>(tile_sa, t * TJ, lane, ibase, xi, yi, zi, mi, g, ax, ay, az, sj, rci, p.rcrit, p.nb);
+            sym_tile<SYM_IPT, false>(tile_sa, t * TJ, lane, ibase, xi, yi, zi, mi, g, ax, ay, az, sj, rci, p.rcrit, p.nb, g0, g1);
         // combine the 4 warps' column partials in warp order (double-buffered: one barrier per tile)
         __syncthreads();
         if (tid == 0 && n + SYM_STAGES < nt) {   // every warp has left slot st: refill it
@@ -285,12 +290,14 @@ __global__ void __launch_bounds__(SYM_THREADS, SYM_IPT >= 5 ? 2 : SYM_IPT >= 3 ?
                         &s_full[st]);
         }
         const int jc = t * TJ + tid - jrow0;
+        if (warp >= g0 && warp < g1) {           // the columns this unit worked on (the others belong to its sister units)
 #pragma unroll
-        for (int c = 0; c < 3; ++c) {
-            double s = s_aj[n & 1][0][c * TJ + tid];
+            for (int c = 0; c < 3; ++c) {
+                double s = s_aj[n & 1][0][c * TJ + tid];
 #pragma unroll
-            for (int w = 1; w < SYM_THREADS / 32; ++w) s += s_aj[n & 1][w][c * TJ + tid];
-            pj[(size_t)c * jw + jc] = s;
+                for (int w = 1; w < SYM_THREADS / 32; ++w) s += s_aj[n & 1][w][c * TJ + tid];
+                pj[(size_t)c * jw + jc] = s;
+            }
         }
     }
 
@@ -304,50 +311,67 @@ __global__ void __launch_bounds__(SYM_THREADS, SYM_IPT >= 5 ? 2 : SYM_IPT >= 3 ?
 
 // a_b = (row partials of b's block, in unit order) + (column partials, ascending I); optionally
 // the closing half kick v += hk * a (Hamiltonian block LOOP 1).
-// [us0, us1): the work units that were run (all of them; a rank's share when the pair sum is sharded over GPUs, SURVEY.md
-// 8(e) - the sum over the ranks of the results is then the full acceleration); ch = j tiles per unit.
+// SHARD (the pair sum sharded over GPUs): only the work units [us0, us1) were run - a contiguous run of
+// every row block's units, i.e. of its groups of 32 columns: qr[I] = {first, end} group of block I's columns, counted
+// from the block's diagonal, that this rank worked on.  The sum over the ranks of the results is the full acceleration.
+#ifndef RED_SLICES_N
+#define RED_SLICES_N 8
+#endif
+constexpr int RED_SLICES = RED_SLICES_N;           // threads per (body, component) of sym_reduce_kernel
+constexpr int RED_THREADS = 32 * RED_SLICES;       // a block: 32 consecutive bodies (one row block: SYM_R is a multiple of 32)
 template <bool KICK, bool SHARD>
-__global__ void __launch_bounds__(ON_BLOCK) sym_reduce_kernel(const double* __restrict__ partI,
-                                                               const double* __restrict__ partJ,
-                                                               const int* __restrict__ ustart, int nb, int ld,
-                                                               int nbPad, double* __restrict__ a,
-                                                               double* __restrict__ v, double hk, int us0, int us1, int ch,
-                                                               int SYM_R, Gate gate) {
+__global__ void __launch_bounds__(RED_THREADS) sym_reduce_kernel(const double* __restrict__ partI,
+                                                                  const double* __restrict__ partJ,
+                                                                  const int* __restrict__ ustart, int nb, int ld,
+                                                                  int nbPad, double* __restrict__ a,
+                                                                  double* __restrict__ v, double hk, int us0, int us1,
+                                                                  const int2* __restrict__ qr, int SYM_R, Gate gate) {
+    __shared__ double sh[RED_SLICES][32];
     if (gate_closed(gate)) return;
-    // one thread per (body, component) - blockIdx.y = component - and four interleaved partial sums per
-    // list, combined in a fixed order: three times the threads and four times the loads in flight of a
-    // thread-per-body loop, still a fixed tree that depends on nb only
-    const int b = blockIdx.x * ON_BLOCK + threadIdx.x;
-    if (b >= nb) return;
+    // blockIdx.y = component; warp w of the block = slice w: it takes the units u0 + w, u0 + w + 8, ... of the body's row
+    // block and the column partials of the row blocks I = w, w + 8, ... (two interleaved sums each), and warp 0 adds the
+    // eight slices in slice order: a fixed tree that depends on nb only, with eight times the loads in flight of a
+    // thread-per-body loop (a row block cut into single column groups has hundreds of units)
+    const int lane = threadIdx.x & 31, sl = threadIdx.x >> 5;
+    const int b = blockIdx.x * 32 + lane;
     const int c = blockIdx.y;
     const int SYM_TPB = SYM_R / TJ;
-    const int Ib = b / SYM_R, r = b - Ib * SYM_R;
-    const int u0 = SHARD ? max(ustart[Ib], us0) : ustart[Ib], u1 = SHARD ? min(ustart[Ib + 1], us1) : ustart[Ib + 1];
-    double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
-    int u = u0;
-    for (; u + 3 < u1; u += 4) {
-        s0 += partI[((size_t)u * 3 + c) * SYM_R + r];
-        s1 += partI[((size_t)(u + 1) * 3 + c) * SYM_R + r];
-        s2 += partI[((size_t)(u + 2) * 3 + c) * SYM_R + r];
-        s3 += partI[((size_t)(u + 3) * 3 + c) * SYM_R + r];
-    }
-    for (; u < u1; ++u) s0 += partI[((size_t)u * 3 + c) * SYM_R + r];
-    // the column partial of row block I was written by the unit that holds this body's j tile
-    const int tb = b / TJ;
-    auto colpart = [&](int I) -> double {
-        if (SHARD) {
-            const int ug = ustart[I] + (tb - I * SYM_TPB) / ch;
-            if (ug < us0 || ug >= us1) return 0.0;
+    double s = 0.0;
+    if (b < nb) {
+        const int Ib = b / SYM_R, r = b - Ib * SYM_R;
+        const int u0 = SHARD ? max(ustart[Ib], us0) : ustart[Ib], u1 = SHARD ? min(ustart[Ib + 1], us1) : ustart[Ib + 1];
+        double s0 = 0.0, s1 = 0.0;
+        int u = u0 + sl;
+        for (; u + RED_SLICES < u1; u += 2 * RED_SLICES) {
+            s0 += partI[((size_t)u * 3 + c) * SYM_R + r];
+            s1 += partI[((size_t)(u + RED_SLICES) * 3 + c) * SYM_R + r];
         }
-        return partJ[symJ_off(I, nbPad, SYM_R) + (size_t)c * (nbPad - I * SYM_R) + (b - I * SYM_R)];
-    };
-    double t0 = 0.0, t1 = 0.0, t2 = 0.0, t3 = 0.0;
-    int I = 0;
-    for (; I + 3 <= Ib; I += 4) { t0 += colpart(I); t1 += colpart(I + 1); t2 += colpart(I + 2); t3 += colpart(I + 3); }
-    for (; I <= Ib; ++I) t0 += colpart(I);
-    const double s = ((s0 + s1) + (s2 + s3)) + ((t0 + t1) + (t2 + t3));
-    a[(size_t)c * ld + b] = s;
-    if (KICK) v[(size_t)c * ld + b] = fma(hk, s, v[(size_t)c * ld + b]);
+        if (u < u1) s0 += partI[((size_t)u * 3 + c) * SYM_R + r];
+        // the column partial of row block I was written by the unit(s) that hold this body's group of 32 columns
+        const int qb = b >> 5;
+        auto colpart = [&](int I) -> double {
+            if (SHARD) {
+                const int2 r2 = qr[I];
+                const int q = qb - I * SYM_TPB * (TJ / 32);
+                if (q < r2.x || q >= r2.y) return 0.0;
+            }
+            return partJ[symJ_off(I, nbPad, SYM_R) + (size_t)c * (nbPad - I * SYM_R) + (b - I * SYM_R)];
+        };
+        double t0 = 0.0, t1 = 0.0;
+        int I = sl;
+        for (; I + RED_SLICES <= Ib; I += 2 * RED_SLICES) { t0 += colpart(I); t1 += colpart(I + RED_SLICES); }
+        if (I <= Ib) t0 += colpart(I);
+        s = (s0 + s1) + (t0 + t1);
+    }
+    sh[sl][lane] = s;
+    __syncthreads();
+    if (sl == 0 && b < nb) {
+        double tot = sh[0][lane];
+#pragma unroll
+        for (int w = 1; w < RED_SLICES; ++w) tot += sh[w][lane];
+        a[(size_t)c * ld + b] = tot;
+        if (KICK) v[(size_t)c * ld + b] = fma(hk, tot, v[(size_t)c * ld + b]);
+    }
 }
 
 }  // namespace mopal

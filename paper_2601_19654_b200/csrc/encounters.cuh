@@ -345,6 +345,7 @@ __global__ void __launch_bounds__(TJ) enc_tilebox_kernel(EncBuf e, int nbig) {
 constexpr int BOXF_TILE_BYTES = TJ * 16;   // TJ x float4
 constexpr int ENC_BATCH = 8;               // j's gated between two survivor checks
 constexpr int ENC_QCAP = 64;               // per-warp survivor queue (a drain leaves < 32)
+constexpr int ENC_UNSORTED_TILES = 40;     // up to this many tiles (N <= 5120) the find pass runs without the spatial ordering
 constexpr int ENC_WIN = 1024;              // column tiles examined per window (candidate list in smem)
 
 struct EncFindParams {

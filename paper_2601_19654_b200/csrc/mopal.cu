@@ -282,7 +282,10 @@ static void choose_geometry(mo_ctx* ctx) {
     if (ctx->enc_split < 1) ctx->enc_split = 1;
     if (ctx->enc_split > 8) ctx->enc_split = 8;
     {
-        int want = 4 * ctx->nsm / (ctx->nTiles > 0 ? ctx->nTiles : 1), most = ctx->nTiles / 2;
+        // (without the spatial ordering, up to 40 tiles: one column tile per CTA - the exact tests of a giant's row, which
+        // passes the gate against thousands of bodies, are the long pole of the pass)
+        int want = 4 * ctx->nsm / (ctx->nTiles > 0 ? ctx->nTiles : 1), most = ctx->nTiles <= ENC_UNSORTED_TILES ? ctx->nTiles : ctx->nTiles / 2;
+        if (ctx->nTiles <= ENC_UNSORTED_TILES) want = 32;
         if (want > 32) want = 32;
         if (want > most) want = most;
         if (want > ctx->enc_split) ctx->enc_split = want;
@@ -647,7 +650,7 @@ static mo_status enqueue_pairs(mo_ctx* ctx, const EncState& es, int step_inc) {
     // up to 40 tiles (N <= 5120) every pair of tiles is gated, in body order: that costs less than the three ordering
     // kernels in a chain of dependent launches this short (at N = 4096 the chain, not the pair sum, was the step: 61 ->
     // 50.5 us; equal at N = 6000, and at N = 8192 the ordering wins by 15 us)
-    fp.unsorted = ctx->nTiles <= 40 ? 1 : 0;
+    fp.unsorted = ctx->nTiles <= ENC_UNSORTED_TILES ? 1 : 0;
     mo_status s;
     if (ctx->use_big) {
         // few big bodies: the nbig x nb rectangle of gates directly, in body order

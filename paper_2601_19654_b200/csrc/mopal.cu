@@ -66,8 +66,8 @@ struct mo_ctx {
     Gate gate = {nullptr, 0};                        // gate of the pack / pair / reduce launches being enqueued (none by default)
     int* res_mode = nullptr;                         // [0] how this step gets its accelerations (1: solve beside the pair sum,
                                                      // 0: before it), [1] what the label kernel saw (latched at the next step)
-    cudaStream_t res_stream[4] = {nullptr, nullptr, nullptr, nullptr};   // the size classes are solved side by side
-    cudaEvent_t res_fork = nullptr, res_join[4] = {nullptr, nullptr, nullptr, nullptr};
+    cudaStream_t res_stream[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};   // the size classes are solved side by side
+    cudaEvent_t res_fork = nullptr, res_join[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
     ResStats* res_out = nullptr;        // device
     ResStats* res_host = nullptr;       // pinned
     int hill_mode = -1;                 // mo_set_hill: -1 off
@@ -365,7 +365,7 @@ extern "C" void mo_destroy(mo_ctx* ctx) {
     cudaFree(ctx->res_cnp); cudaFree(ctx->res_cstart); cudaFree(ctx->res_cfill); cudaFree(ctx->res_cq); cudaFree(ctx->res_clist); cudaFree(ctx->res_ctl); cudaFree(ctx->res_aux); cudaFree(ctx->res_cown); cudaFree(ctx->fix_list); cudaFree(ctx->fix_nf); cudaFree(ctx->fix_part); cudaFree(ctx->res_colres); cudaFree(ctx->res_csync); cudaFree(ctx->res_mode);
     cudaFree(ctx->res_dbody); cudaFree(ctx->res_dpair); cudaFree(ctx->res_dbodyi); cudaFree(ctx->res_dpairi);
     if (ctx->res_host) cudaFreeHost(ctx->res_host);
-    for (int k = 0; k < 4; ++k) { if (ctx->res_stream[k]) cudaStreamDestroy(ctx->res_stream[k]); if (ctx->res_join[k]) cudaEventDestroy(ctx->res_join[k]); }
+    for (int k = 0; k < 5; ++k) { if (ctx->res_stream[k]) cudaStreamDestroy(ctx->res_stream[k]); if (ctx->res_join[k]) cudaEventDestroy(ctx->res_join[k]); }
     if (ctx->res_fork) cudaEventDestroy(ctx->res_fork);
     cudaFree(ctx->gmsum); cudaFree(ctx->en_on); cudaFree(ctx->en_pair); cudaFree(ctx->en_out);
     if (ctx->en_host) cudaFreeHost(ctx->en_host); cudaFree(ctx->tiles);
@@ -713,7 +713,7 @@ static mo_status enqueue_hill(mo_ctx* ctx, double n_hill, int mode, double* rhil
 
 // grids of the resolve kernels: class 0 (components of up to 63 pairs, 64 threads: several CTAs per SM), the larger
 // classes hold few components (the stars around the big bodies): small grids, cheap to launch when they have nothing to do
-static constexpr int RES_GRID_0_PER_SM = 6, RES_GRID_4 = 16;
+static constexpr int RES_GRID_0_PER_SM = 6, RES_GRID_4 = 16, RES_GRID_S_PER_SM = 4;
 static constexpr int RES_CL_GRID = RES_NCOL * (RES_NCLUSTERS / 3);   // classes 1..3: 8 clusters of 8 CTAs each
 
 static mo_status ensure_resolve_scratch(mo_ctx* ctx) {
@@ -756,7 +756,7 @@ static mo_status ensure_resolve_scratch(mo_ctx* ctx) {
     if (e == cudaSuccess) e = cudaFuncSetAttribute(resolve_solve_kernel<1024, 3, RES_NCOL>, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->res_smemC);
     if (e == cudaSuccess) e = cudaMemsetAsync(ctx->res_out, 0, sizeof(ResStats), ctx->stream);
     if (e == cudaSuccess) e = cudaMallocHost(reinterpret_cast<void**>(&ctx->res_host), sizeof(ResStats));
-    for (int k = 0; k < 4 && e == cudaSuccess; ++k) {
+    for (int k = 0; k < 5 && e == cudaSuccess; ++k) {
         int plo = 0, phi = 0;
         cudaDeviceGetStreamPriorityRange(&plo, &phi);
         e = cudaStreamCreateWithPriority(&ctx->res_stream[k], cudaStreamNonBlocking, phi);   // ahead of a pair sum that becomes eligible at the same time
@@ -783,11 +783,12 @@ static mo_status enqueue_resolve(mo_ctx* ctx, double dt, double tol) {
     // CTA) on streams of their own, the many small ones on the caller's
     cudaStream_t mainS = ctx->stream;
     CK(cudaEventRecord(ctx->res_fork, mainS));
-    for (int k = 0; k < 4; ++k) {
+    for (int k = 0; k < 5; ++k) {
         if (k == 0 && !ctx->res_dbody) continue;
         cudaStream_t st = ctx->res_stream[k];
         CK(cudaStreamWaitEvent(st, ctx->res_fork, 0));
         if (k == 0) resolve_stream_kernel<<<RES_GRID_4, RES_D_THREADS, 0, st>>>(rp);
+        else if (k == 4) resolve_solve_kernel<64, 0, 1><<<ctx->nsm * RES_GRID_0_PER_SM, 64, ctx->res_smemA, st>>>(rp, ctx->res_smemA);
         else {
             // clusters of RES_NCOL CTAs: one component per cluster, one Bulirsch-Stoer column per CTA
             cudaLaunchConfig_t cfg = {};
@@ -803,10 +804,11 @@ static mo_status enqueue_resolve(mo_ctx* ctx, double dt, double tol) {
         if (s != MO_OK) return s;
         CK(cudaEventRecord(ctx->res_join[k], st));
     }
-    resolve_solve_kernel<64, 0, 1><<<ctx->nsm * RES_GRID_0_PER_SM, 64, ctx->res_smemA, mainS>>>(rp, ctx->res_smemA);
+    // the small systems (almost all of them) on the caller's stream: one CTA of 8 warps each, a column per warp
+    resolve_small_kernel<<<ctx->nsm * RES_GRID_S_PER_SM, RES_S_THREADS, 0, mainS>>>(rp);
     s = post_launch(ctx);
     if (s != MO_OK) return s;
-    for (int k = 0; k < 4; ++k) {
+    for (int k = 0; k < 5; ++k) {
         if (k == 0 && !ctx->res_dbody) continue;
         CK(cudaStreamWaitEvent(mainS, ctx->res_join[k], 0));
     }

@@ -16,6 +16,8 @@
 //                          Classes 0..3: np <= 63 / 255 / 511 / 1023 pairs with 64 / 256 / 512 / 1024 threads.
 //                          Everything a right-hand side touches is in shared memory, carved by the component's
 //                          actual size; the extrapolation tableau too when it fits (else global scratch).
+//   resolve_small_kernel   class 5, at most 31 pairs (almost every system): one CTA of 8 warps, warp w = column w of the
+//                          Bulirsch-Stoer step, lane = body / pair.
 //   resolve_stream_kernel  class 4, any size: the same algorithm with all per-body and per-pair state in global
 //                          pools, thread-strided loops, block-wide sums for the hubs.
 //
@@ -34,8 +36,11 @@ namespace mopal {
 
 constexpr int RES_KMAX = 8;        // columns: 2, 4, .., 16 substeps
 constexpr int RES_HEAVY = 12;      // a body with more pairs is summed by its whole warp
-constexpr int RES_NCLS = 5;        // size classes: 0..3 one thread per body (64 / 256 / 512 / 1024 threads), 4 streamed
+constexpr int RES_NCLS = 6;        // size classes: 0..3 one thread per body (64 / 256 / 512 / 1024 threads), 4 streamed,
+                                   // 5 the small systems (at most RES_PHI_S pairs): one warp per column
 constexpr int RES_PHI_0 = 63, RES_PHI_1 = 255, RES_PHI_2 = 511, RES_PHI_3 = 1023;   // largest pair count of classes 0..3
+constexpr int RES_PHI_S = 31;      // ... and of class 5: at most 32 bodies, one per lane
+constexpr int RES_S_THREADS = 32 * RES_KMAX;   // resolve_small_kernel: warp w integrates column w
 constexpr int RES_CTL_CNT = 1, RES_CTL_TKT = 1 + RES_NCLS, RES_CTL_POOL = 1 + 2 * RES_NCLS, RES_CTL_N = 2 + 2 * RES_NCLS;
 constexpr int RES_LABEL_THREADS = 1024;
 constexpr int RES_NCOL = 8;        // CTAs per cluster = columns side by side (classes 1..3)
@@ -109,7 +114,7 @@ __device__ __forceinline__ int res_scan(int v, int* sScan, int& total) {
     return (warp ? sScan[32 + warp - 1] : 0) + incl - v;
 }
 
-__device__ __forceinline__ int res_class(int np) { return np <= RES_PHI_0 ? 0 : np <= RES_PHI_1 ? 1 : np <= RES_PHI_2 ? 2 : np <= RES_PHI_3 ? 3 : 4; }
+__device__ __forceinline__ int res_class(int np) { return np <= RES_PHI_S ? 5 : np <= RES_PHI_0 ? 0 : np <= RES_PHI_1 ? 1 : np <= RES_PHI_2 ? 2 : np <= RES_PHI_3 ? 3 : 4; }
 
 // barrier of the CTAs of a cluster that work on one component: every CTA's thread 0 counts itself in and waits for the
 // others (the cluster's CTAs are co-scheduled, so nobody waits for a CTA that is not running); the CTA's other live warps
@@ -783,6 +788,273 @@ __global__ void __launch_bounds__(NT, 1) resolve_solve_kernel(ResParams p, int s
     }
     }   // active warps
     }   // components
+}
+
+// ---- class S: the small systems (at most RES_PHI_S pairs, hence at most 32 bodies: a planetesimal pair, a test particle
+// with its one or two big partners - almost every system of a list).  One CTA of RES_KMAX warps per system at a time, and
+// the columns of a Bulirsch-Stoer step SIDE BY SIDE inside it: warp w integrates column w (2 (w + 1) substeps), lane =
+// body for the state, lane = pair for the pair terms, everything in shared memory and registers, warp barriers only
+// inside a right-hand side.  A step then costs its longest column (at most 17 right-hand sides) instead of the sum of
+// its columns (42-72), and two block barriers: columns -> shared memory | warp 0 runs the extrapolation tableau and the
+// error test, moves the state on acceptance and publishes the outcome | every warp updates the same controller from it.
+// The deepest passage of a list - a test particle grazing an embryo: ~100 steps - is the length of the whole solve
+// when the systems are many and small (N = 1e6, nbig = 100), which is why it is cut here and not the throughput.
+// Same arithmetic and the same summation order per body (pairs as second member first, list order) as
+// resolve_solve_kernel; the controller is the same code on the same numbers.
+#ifndef RES_S_MINB
+#define RES_S_MINB 2
+#endif
+__global__ void __launch_bounds__(RES_S_THREADS, RES_S_MINB) resolve_small_kernel(ResParams p) {
+    constexpr int W = RES_KMAX;
+    __shared__ double sY[6][32];                 // state at the start of the Bulirsch-Stoer step
+    __shared__ double sP[W][3][32];              // per column: position increments of the current right-hand side (y for f(y))
+    __shared__ double sFt[W][3][32];             // per column: pair terms
+    __shared__ double sDy[W][3][32];             // per column (identical copies): y_j - y_i at the start of the step
+    __shared__ double sCol[W][6][32];            // column results
+    __shared__ double sT[W][6][32];              // extrapolation tableau (warp 0)
+    __shared__ double sRc2[32], sInv[32], sGi[32], sGj[32];
+    __shared__ int sPi[32], sPj[32], sQ[32], sQs[32], sBi[32], sBj[32], sBody[32], sFirst[64], sId[64];
+    __shared__ float sFac[2];
+    __shared__ int sCtl[4];                      // ticket | accepted column (-1: none) | last column tested | bodies
+    constexpr unsigned full = 0xffffffffu;
+    const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+    const unsigned lt = (1u << lane) - 1u;
+    bool firstTicket = true;
+
+    for (;;) {
+    __syncthreads();                                                       // the previous system is finished with shared memory
+    int ticket;
+    if (firstTicket) { ticket = blockIdx.x; firstTicket = false; }
+    else {
+        if (tid == 0) sCtl[0] = gridDim.x + atomicAdd(&p.ctl[RES_CTL_TKT + 5], 1);
+        __syncthreads();
+        ticket = sCtl[0];
+    }
+    if (ticket >= p.ctl[RES_CTL_CNT + 5]) break;
+    const int comp = p.clist[(size_t)5 * p.cap + ticket];
+    const int np = p.cnp[comp];
+    const int own = p.cown[comp];                                          // a detached body's system (see res_owner), else -1
+
+    // ---- set-up by warp 0: pairs in list order, bodies numbered by first appearance (as in resolve_solve_kernel) ----
+    if (w == 0) {
+        const int ps = p.cstart[comp], nown = p.cfill[comp];
+        if (lane < nown) sQ[lane] = p.cq[ps + lane];
+        __syncwarp();
+        if (own >= 0 && lane == 0) {                                       // + the pairs of its partners' components, each once
+            int cnt = nown;
+            for (int k = 0; k < nown; ++k) {
+                const int q = sQ[k];
+                const int cc = p.aux[p.pairs[2 * q] == own ? p.pairs[2 * q + 1] : p.pairs[2 * q]];
+                if (cc < 0) continue;
+                bool seen = false;
+                for (int m = 0; m < k; ++m) { const int q2 = sQ[m]; seen |= p.aux[p.pairs[2 * q2] == own ? p.pairs[2 * q2 + 1] : p.pairs[2 * q2]] == cc; }
+                if (!seen) for (int m = 0; m < p.cfill[cc]; ++m) sQ[cnt++] = p.cq[p.cstart[cc] + m];
+            }
+        }
+        __syncwarp();
+        if (lane < np) {
+            const int mine = sQ[lane];
+            int r = 0;
+            for (int m = 0; m < np; ++m) r += (sQ[m] < mine) ? 1 : 0;
+            sQs[r] = mine;
+        }
+        __syncwarp();
+        int bi = 0, bj = 0;
+        if (lane < np) { const int q = sQs[lane]; bi = p.pairs[2 * q]; bj = p.pairs[2 * q + 1]; sBi[lane] = bi; sBj[lane] = bj; }
+        __syncwarp();
+        int isf0 = 0, isf1 = 0;
+        if (lane < np) {
+            int f0 = 2 * lane, f1 = 2 * lane + 1;
+            for (int m = 2 * lane - 1; m >= 0; --m) if (((m & 1) ? sBj[m >> 1] : sBi[m >> 1]) == bi) f0 = m;
+            for (int m = 2 * lane; m >= 0; --m) if (((m & 1) ? sBj[m >> 1] : sBi[m >> 1]) == bj) f1 = m;
+            sFirst[2 * lane] = f0; sFirst[2 * lane + 1] = f1;
+            isf0 = f0 == 2 * lane; isf1 = f1 == 2 * lane + 1;
+        }
+        const unsigned b0 = __ballot_sync(full, isf0), b1 = __ballot_sync(full, isf1);
+        const int id0 = __popc(b0 & lt) + __popc(b1 & lt);
+        if (isf0) { sId[2 * lane] = id0; sBody[id0] = bi; }
+        if (isf1) { sId[2 * lane + 1] = id0 + isf0; sBody[id0 + isf0] = bj; }
+        if (lane == 0) sCtl[3] = __popc(b0) + __popc(b1);
+        __syncwarp();
+        if (lane < np) {
+            sPi[lane] = sId[sFirst[2 * lane]]; sPj[lane] = sId[sFirst[2 * lane + 1]];
+            sGi[lane] = p.gm[bi]; sGj[lane] = p.gm[bj];
+            const double rc = fmax(p.rcrit[bi], p.rcrit[bj]);
+            sRc2[lane] = rc * rc; sInv[lane] = rc > 0.0 ? 1.0 / (0.9 * rc) : 0.0;
+        }
+        const int n0 = sCtl[3];
+        const int b = lane < n0 ? sBody[lane] : 0;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {                                      // pad rows: a harmless body at (1, 0, 0)
+            sY[c][lane] = lane < n0 ? p.x0[(size_t)c * p.ld + b] : (c == 0 ? 1.0 : 0.0);
+            sY[3 + c][lane] = lane < n0 ? p.v0[(size_t)c * p.ld + b] : 0.0;
+        }
+    }
+    __syncthreads();
+    const int n = sCtl[3];
+    const bool live = lane < n;
+    const int me = live ? sBody[lane] : 0;
+    unsigned mI = 0u, mJ = 0u;                                             // this body's pairs as first / second member
+    for (int k = 0; k < np; ++k) { mI |= (sPi[k] == lane) ? (1u << k) : 0u; mJ |= (sPj[k] == lane) ? (1u << k) : 0u; }
+    if (!live) { mI = 0u; mJ = 0u; }
+    const int pi = lane < np ? sPi[lane] : 0, pj = lane < np ? sPj[lane] : 0;
+    const double rc2 = lane < np ? sRc2[lane] : 0.0, inv = lane < np ? sInv[lane] : 0.0;
+
+    // ---- the Bulirsch-Stoer loop (every warp takes the same decisions from the same published numbers) ----
+    const double mu = p.mu, hh = p.h, tol = p.tol;
+    double t = 0.0;
+    ResCtl ctl{hh, 5, 0};
+    int fail = 0, nacc = 0, nrhs = 0;
+    bool havef0 = false;
+    double f0[3] = {0.0, 0.0, 0.0}, isx = 0.0, isv = 0.0;                  // f(y) and the inverse error scales of this body
+    while (!fail) {
+        const double rem = hh - t;
+        if (fabs(rem) <= 4.0 * 2.220446049250313e-16 * fabs(hh)) break;
+        bool last = false;
+        if (fabs(ctl.H) >= fabs(rem)) { ctl.H = rem; last = true; }
+        const double H = ctl.H;
+        const int kcols = min(ctl.ktarg + 1, RES_KMAX - 1);
+        // this warp's column: the modified midpoint rule with 2 (w + 1) substeps over H (a warp beyond the columns this
+        // step tries evaluates f(y) only, when it is still missing)
+        {
+            const bool run = w <= kcols;
+            const int nsub = 2 * (w + 1);
+            const double hs = H / (double)nsub;
+            double d0[6], d1[6], cur[6];
+#pragma unroll
+            for (int c = 0; c < 6; ++c) { d0[c] = 0.0; d1[c] = 0.0; cur[c] = 0.0; }
+            if (havef0 && live) {
+#pragma unroll
+                for (int c = 0; c < 3; ++c) { d1[c] = hs * sY[3 + c][lane]; d1[3 + c] = hs * f0[c]; }
+            }
+            const int mlast = run ? nsub : 0;
+#pragma unroll 1
+            for (int m = havef0 ? 1 : 0; m <= mlast; ++m) {
+                const bool base = m == 0;
+                const double y0 = sY[0][lane], y1 = sY[1][lane], y2 = sY[2][lane];
+                const double v0 = sY[3][lane] + d1[3], v1 = sY[4][lane] + d1[4], v2 = sY[5][lane] + d1[5];
+                sP[w][0][lane] = base ? y0 : d1[0]; sP[w][1][lane] = base ? y1 : d1[1]; sP[w][2][lane] = base ? y2 : d1[2];
+                __syncwarp();
+                const double z0 = y0 + d1[0], z1 = y1 + d1[1], z2 = y2 + d1[2];            // d1 = 0 when base
+                const double yk = res_rsqrt(fma(z2, z2, fma(z1, z1, z0 * z0)));
+                const double wk = -mu * (yk * yk * yk);
+                double a0 = wk * z0, a1 = wk * z1, a2 = wk * z2;
+                if (lane < np) {                                           // lane = pair
+                    double dx = sP[w][0][pj] - sP[w][0][pi], dy = sP[w][1][pj] - sP[w][1][pi], dz = sP[w][2][pj] - sP[w][2][pi];
+                    if (base) { sDy[w][0][lane] = dx; sDy[w][1][lane] = dy; sDy[w][2][lane] = dz; }
+                    else { dx += sDy[w][0][lane]; dy += sDy[w][1][lane]; dz += sDy[w][2][lane]; }
+                    const double u = res_pair_u(fma(dz, dz, fma(dy, dy, dx * dx)), rc2, inv);
+                    sFt[w][0][lane] = u * dx; sFt[w][1][lane] = u * dy; sFt[w][2][lane] = u * dz;
+                }
+                __syncwarp();
+                for (unsigned mm = mJ; mm; mm &= mm - 1u) {                // lane = body: as second member, -gm_i u d
+                    const int q = __ffs(mm) - 1;
+                    const double g = sGi[q];
+                    a0 = fma(-g, sFt[w][0][q], a0); a1 = fma(-g, sFt[w][1][q], a1); a2 = fma(-g, sFt[w][2][q], a2);
+                }
+                for (unsigned mm = mI; mm; mm &= mm - 1u) {                // as first member, +gm_j u d
+                    const int q = __ffs(mm) - 1;
+                    const double g = sGj[q];
+                    a0 = fma(g, sFt[w][0][q], a0); a1 = fma(g, sFt[w][1][q], a1); a2 = fma(g, sFt[w][2][q], a2);
+                }
+                if (w == 0) ++nrhs;
+                if (base) {                                                // f(y) and the error scales of this BS step
+                    if (live) {
+                        f0[0] = a0; f0[1] = a1; f0[2] = a2;
+                        const double sx2 = fma(y2, y2, fma(y1, y1, y0 * y0)), sv2 = fma(v2, v2, fma(v1, v1, v0 * v0));
+                        isx = sx2 > 0.0 ? 1.0 / sqrt(sx2) : 1e300; isv = sv2 > 0.0 ? 1.0 / sqrt(sv2) : 1e300;
+                        d1[0] = hs * v0; d1[1] = hs * v1; d1[2] = hs * v2; d1[3] = hs * a0; d1[4] = hs * a1; d1[5] = hs * a2;
+                    }
+                    havef0 = true;
+                } else if (m < nsub) {
+                    const double h2s = 2.0 * hs;
+                    double tt;
+                    tt = fma(h2s, v0, d0[0]); d0[0] = d1[0]; d1[0] = tt;
+                    tt = fma(h2s, v1, d0[1]); d0[1] = d1[1]; d1[1] = tt;
+                    tt = fma(h2s, v2, d0[2]); d0[2] = d1[2]; d1[2] = tt;
+                    tt = fma(h2s, a0, d0[3]); d0[3] = d1[3]; d1[3] = tt;
+                    tt = fma(h2s, a1, d0[4]); d0[4] = d1[4]; d1[4] = tt;
+                    tt = fma(h2s, a2, d0[5]); d0[5] = d1[5]; d1[5] = tt;
+                } else {
+                    cur[0] = 0.5 * (d0[0] + fma(hs, v0, d1[0])); cur[1] = 0.5 * (d0[1] + fma(hs, v1, d1[1])); cur[2] = 0.5 * (d0[2] + fma(hs, v2, d1[2]));
+                    cur[3] = 0.5 * (d0[3] + fma(hs, a0, d1[3])); cur[4] = 0.5 * (d0[4] + fma(hs, a1, d1[4])); cur[5] = 0.5 * (d0[5] + fma(hs, a2, d1[5]));
+                }
+            }
+            if (run) {
+#pragma unroll
+                for (int c = 0; c < 6; ++c) sCol[w][c][lane] = cur[c];
+            }
+        }
+        __syncthreads();
+        if (w == 0) {
+            nrhs += (kcols + 1) * (kcols + 2) - 2;                         // the other columns' right-hand sides: sum of 2 (k + 1)
+            int acc = -1, klast = 0;
+            float facCur = 1.0f, facPrev = 1.0f;
+#pragma unroll 1
+            for (int k = 0; k <= kcols; ++k) {
+                double cur[6], prev[6];
+#pragma unroll
+                for (int c = 0; c < 6; ++c) { cur[c] = live ? sCol[k][c][lane] : 0.0; prev[c] = cur[c]; }
+                double err = 0.0;
+                if (live) {
+#pragma unroll 1
+                    for (int j = 1; j <= k; ++j) {                         // row k of the tableau from row k-1 (in sT), overwriting it
+                        const double cf = RES_COEF[k * RES_KMAX + j];
+#pragma unroll
+                        for (int c = 0; c < 6; ++c) {
+                            const double oldv = sT[j - 1][c][lane];
+                            sT[j - 1][c][lane] = cur[c];
+                            prev[c] = cur[c];
+                            cur[c] = fma(cur[c] - oldv, cf, cur[c]);
+                        }
+                    }
+#pragma unroll
+                    for (int c = 0; c < 6; ++c) {
+                        sT[k][c][lane] = cur[c];
+                        double e = fabs(cur[c] - prev[c]) * (c < 3 ? isx : isv);
+                        if (!(e <= 1e300)) e = 1e300;                       // NaN / inf: never accepted
+                        err = fmax(err, e);
+                    }
+                }
+                if (k >= 1) {
+#pragma unroll
+                    for (int o = 16; o > 0; o >>= 1) err = fmax(err, __shfl_xor_sync(full, err, o));
+                    const double e = err / tol;
+                    facPrev = facCur; facCur = res_fac(e, k);
+                    klast = k;
+                    if (e <= 1.0) { acc = k; break; }
+                    if (k < kcols && res_hopeless(e, k, ctl.ktarg)) break;
+                }
+            }
+            if (acc >= 0 && live) {
+#pragma unroll
+                for (int c = 0; c < 6; ++c) sY[c][lane] += sT[acc][c][lane];
+            }
+            if (lane == 0) { sCtl[1] = acc; sCtl[2] = klast; sFac[0] = facCur; sFac[1] = facPrev; }
+        }
+        __syncthreads();
+        const int acc = sCtl[1], klast = sCtl[2];
+        const float facCur = sFac[0], facPrev = sFac[1];
+        if (acc < 0) {
+            if (ctl.rejected(klast, facCur)) fail = 1;
+            continue;
+        }
+        t = last ? hh : t + H;
+        ++nacc;
+        havef0 = false;
+        ctl.accepted(acc, facCur, facPrev);
+    }
+    if (w == 0) {
+        if (!fail && live && (own < 0 || own == me)) {                     // a detached body's system writes only that body
+#pragma unroll
+            for (int c = 0; c < 3; ++c) { p.x[(size_t)c * p.ld + me] = sY[c][lane]; p.v[(size_t)c * p.ld + me] = sY[3 + c][lane]; }
+        }
+        if (lane == 0) {
+            atomicAdd(&p.out->bodies, own < 0 ? n : 1); atomicAdd(&p.out->steps, nacc); atomicAdd(&p.out->rhs, nrhs);
+            if (fail) { atomicAdd(&p.out->fail, 1); atomicAdd(&p.st->resolve_fail, 1); }
+        }
+    }
+    }   // systems
 }
 
 // ---- class D: components of any size.  All per-body and per-pair state lives in global pools (planes of

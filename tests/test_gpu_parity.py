@@ -1130,10 +1130,12 @@ def _giant_star(K, rmin, seed_off=40):
     return m_star, mg, X, Vh, rad
 
 
-@pytest.mark.parametrize("K,rmin", [(40, 0.05), (100, 0.02), (300, 0.02), (450, 0.1), (700, 0.15), (1500, 0.15)])
+@pytest.mark.parametrize("K,rmin", [(5, 0.1), (24, 0.1), (31, 0.1), (32, 0.1), (40, 0.05), (100, 0.02), (300, 0.02), (450, 0.1), (700, 0.15),
+                                    (1500, 0.15)])
 def test_resolve_big_star_components(M, K, rmin):
-    """the size classes of resolve_solve_kernel (64 / 256 / 512 / 1024 threads), the warp-summed hub with its group sums,
-    and - K = 1500 - resolve_stream_kernel, against the oracle.  Planetesimals that pass within a few 0.01 AU of the giant
+    """resolve_small_kernel (at most 31 pairs: a warp per column; K = 31 / 32 sit on either side of its limit), the size
+    classes of resolve_solve_kernel (64 / 256 / 512 / 1024 threads), the warp-summed hub with its group sums, and - K = 1500 -
+    resolve_stream_kernel, against the oracle.  Planetesimals that pass within a few 0.01 AU of the giant
     amplify the FP64 / long-double rounding difference (the flyby is a scattering): 1e-10 for them, the tolerance-derived
     bound for the bodies that stay farther than 0.3 AU."""
     m_star, mg, X, Vh, rad = _giant_star(K, rmin)

@@ -53,7 +53,7 @@ struct mo_ctx {
     int* res_loc = nullptr;             // nb ints (lazy)
     double* res_tab = nullptr;          // extrapolation tableaux of the class-C CTAs (fallback when shared memory is short)
     int *res_label = nullptr, *res_cnp = nullptr, *res_cstart = nullptr, *res_cfill = nullptr, *res_cq = nullptr;
-    int *res_clist = nullptr, *res_ctl = nullptr, *res_aux = nullptr, *res_cown = nullptr;
+    int *res_clist = nullptr, *res_ctl = nullptr, *res_aux = nullptr, *res_cown = nullptr, *res_ckey = nullptr;
     double *res_dbody = nullptr, *res_dpair = nullptr;   // class D (components of more than 1023 pairs): state pools
     int *res_dbodyi = nullptr, *res_dpairi = nullptr;
     long long res_dbodyN = 0;
@@ -362,7 +362,7 @@ extern "C" void mo_destroy(mo_ctx* ctx) {
     cudaFree(ctx->gm); cudaFree(ctx->x0); cudaFree(ctx->v0); cudaFree(ctx->part);
     cudaFree(ctx->psumA); cudaFree(ctx->psumB); cudaFree(ctx->ticket);
     cudaFree(ctx->res_loc); cudaFree(ctx->res_out); cudaFree(ctx->res_tab); cudaFree(ctx->res_label);
-    cudaFree(ctx->res_cnp); cudaFree(ctx->res_cstart); cudaFree(ctx->res_cfill); cudaFree(ctx->res_cq); cudaFree(ctx->res_clist); cudaFree(ctx->res_ctl); cudaFree(ctx->res_aux); cudaFree(ctx->res_cown); cudaFree(ctx->fix_list); cudaFree(ctx->fix_nf); cudaFree(ctx->fix_part); cudaFree(ctx->res_colres); cudaFree(ctx->res_csync); cudaFree(ctx->res_mode);
+    cudaFree(ctx->res_cnp); cudaFree(ctx->res_cstart); cudaFree(ctx->res_cfill); cudaFree(ctx->res_cq); cudaFree(ctx->res_clist); cudaFree(ctx->res_ctl); cudaFree(ctx->res_aux); cudaFree(ctx->res_cown); cudaFree(ctx->res_ckey); cudaFree(ctx->fix_list); cudaFree(ctx->fix_nf); cudaFree(ctx->fix_part); cudaFree(ctx->res_colres); cudaFree(ctx->res_csync); cudaFree(ctx->res_mode);
     cudaFree(ctx->res_dbody); cudaFree(ctx->res_dpair); cudaFree(ctx->res_dbodyi); cudaFree(ctx->res_dpairi);
     if (ctx->res_host) cudaFreeHost(ctx->res_host);
     for (int k = 0; k < 5; ++k) { if (ctx->res_stream[k]) cudaStreamDestroy(ctx->res_stream[k]); if (ctx->res_join[k]) cudaEventDestroy(ctx->res_join[k]); }
@@ -727,6 +727,7 @@ static mo_status ensure_resolve_scratch(mo_ctx* ctx) {
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->fix_nf, 1);
     if (e == cudaSuccess && ctx->use_sym) e = dalloc(ctx, &ctx->fix_part, (size_t)FIX_JS * 3 * ctx->nb);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_cown, capn);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_ckey, capn);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_cnp, capn);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_cstart, capn);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_cfill, capn);
@@ -771,7 +772,7 @@ static mo_status enqueue_resolve(mo_ctx* ctx, double dt, double tol) {
     StageRange nv("mopal: encounter resolution (f3)");
     ResParams rp;
     rp.x0 = ctx->x0; rp.v0 = ctx->v0; rp.x = ctx->x; rp.v = ctx->v; rp.gm = ctx->gm; rp.rcrit = ctx->rcrit;
-    rp.pairs = ctx->pairs; rp.st = ctx->dstats; rp.out = ctx->res_out; rp.loc = ctx->res_loc; rp.label = ctx->res_label; rp.aux = ctx->res_aux; rp.cown = ctx->res_cown;
+    rp.pairs = ctx->pairs; rp.st = ctx->dstats; rp.out = ctx->res_out; rp.loc = ctx->res_loc; rp.label = ctx->res_label; rp.aux = ctx->res_aux; rp.cown = ctx->res_cown; rp.ckey = ctx->res_ckey;
     rp.cnp = ctx->res_cnp; rp.cstart = ctx->res_cstart; rp.cfill = ctx->res_cfill; rp.cq = ctx->res_cq; rp.clist = ctx->res_clist;
     rp.ctl = ctx->res_ctl; rp.colres = ctx->res_colres; rp.csync = ctx->res_csync; rp.mode = ctx->res_mode; rp.tab = ctx->res_tab; rp.dbody = ctx->res_dbody; rp.dbodyi = ctx->res_dbodyi; rp.dpair = ctx->res_dpair;
     rp.dpairi = ctx->res_dpairi; rp.dbodyN = ctx->res_dbodyN;

@@ -36,8 +36,9 @@ namespace mopal {
 
 constexpr int RES_KMAX = 8;        // columns: 2, 4, .., 16 substeps
 constexpr int RES_HEAVY = 12;      // a body with more pairs is summed by its whole warp
-constexpr int RES_NCLS = 6;        // size classes: 0..3 one thread per body (64 / 256 / 512 / 1024 threads), 4 streamed,
-                                   // 5 the small systems (at most RES_PHI_S pairs): one warp per column
+constexpr int RES_NCLS = 7;        // size classes: 0..3 one thread per body (64 / 256 / 512 / 1024 threads), 4 streamed,
+                                   // 5 the small systems (at most RES_PHI_S pairs): one warp per column; 6 those of
+                                   // them that look like a long chain of steps (a deep passage): taken first
 constexpr int RES_PHI_0 = 63, RES_PHI_1 = 255, RES_PHI_2 = 511, RES_PHI_3 = 1023;   // largest pair count of classes 0..3
 constexpr int RES_PHI_S = 31;      // ... and of class 5: at most 32 bodies, one per lane
 constexpr int RES_S_THREADS = 32 * RES_KMAX;   // resolve_small_kernel: warp w integrates column w
@@ -65,6 +66,7 @@ struct ResParams {
     int* label;                  // nb: smallest body of the component (valid for listed bodies)
     int* aux;                    // nb: the component a body is in (-1: none; a detached body, or a massive body with detached partners only)
     int* cown;                   // per system: the detached body it belongs to (the only one written back), or -1
+    int* ckey;                   // per system: smallest (closest straight-line approach / rc)^2 of its own pairs, as float bits
     int *cnp, *cstart, *cfill;   // per system (<= cap): pairs (a detached body's: with its partners' components), first slot in cq, own pairs there
     int* cq;                     // cap: pair indices grouped by component (unordered inside a group)
     int* clist;                  // RES_NCLS * cap: the components of each class
@@ -131,6 +133,10 @@ __device__ __forceinline__ void res_cluster_barrier(int* cnt, int target, int na
     res_bar(nact);
 }
 
+// producer / consumer halves of named barrier id (n threads in all): the producers arrive and go on, the consumers wait
+__device__ __forceinline__ void res_nb_arrive(int id, int n) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(n) : "memory"); }
+__device__ __forceinline__ void res_nb_sync(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
+
 // barrier of the first nthreads threads of the block (whole warps), beside the block barrier 0
 __device__ __forceinline__ void res_bar(int nthreads) { asm volatile("bar.sync 1, %0;" ::"r"(nthreads) : "memory"); }
 
@@ -150,6 +156,27 @@ __device__ __forceinline__ int res_owner(const ResParams& p, int q, const int* l
     if (!mi && label[i] < 0) return i;                           // i detached
     if (!mj && label[j] < 0) return j;                           // j detached
     return label[i];                                             // the component's smallest body
+}
+
+// How deep a listed pair's passage looks (scheduling only: the systems that will need many Bulirsch-Stoer steps are started
+// first, so that the longest chain of the list runs beside the others instead of after them): the closest approach of the
+// straight line from the separation at the snapshot to the separation after the drift, squared, over rc^2 - as the bits
+// of a non-negative float, which order like the floats.
+constexpr float RES_DEEP_RATIO = 0.04f;           // closest approach below 0.2 rc
+__device__ __forceinline__ int res_depth_key(const ResParams& p, int q) {
+    const int i = p.pairs[2 * q], j = p.pairs[2 * q + 1];
+    float a[3], d[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        a[c] = (float)(p.x0[(size_t)c * p.ld + j] - p.x0[(size_t)c * p.ld + i]);
+        d[c] = (float)(p.x[(size_t)c * p.ld + j] - p.x[(size_t)c * p.ld + i]) - a[c];
+    }
+    const float dd = d[0] * d[0] + d[1] * d[1] + d[2] * d[2], ad = a[0] * d[0] + a[1] * d[1] + a[2] * d[2];
+    const float t = dd > 0.f ? fminf(fmaxf(-ad / dd, 0.f), 1.f) : 0.f;
+    const float m0 = a[0] + t * d[0], m1 = a[1] + t * d[1], m2 = a[2] + t * d[2];
+    const float rc = (float)fmax(p.rcrit[i], p.rcrit[j]);
+    const float r = rc > 0.f ? (m0 * m0 + m1 * m1 + m2 * m2) / (rc * rc) : 1e30f;
+    return __float_as_int(r >= 0.f ? fminf(r, 1e30f) : 1e30f);            // NaN: not deep
 }
 
 // min-label propagation along the pairs that belong to components (not left out, not owned by a detached body)
@@ -237,7 +264,7 @@ __global__ void __launch_bounds__(RES_LABEL_THREADS) resolve_label_kernel(ResPar
         if (q < np) { o = res_owner(p, q, p.label); isfirst = (o >= 0 && p.loc[o] == q) ? 1 : 0; }
         int tot;
         const int off = res_scan(isfirst, sScan, tot);
-        if (isfirst) { const int c = carry + off; p.cfill[c] = q; p.cnp[c] = 0; p.cown[c] = p.gm[o] > 0.0 ? -1 : o; }
+        if (isfirst) { const int c = carry + off; p.cfill[c] = q; p.cnp[c] = 0; p.cown[c] = p.gm[o] > 0.0 ? -1 : o; p.ckey[c] = 0x7f7fffff; }
         carry += tot;
     }
     const int ncomp = carry;
@@ -257,7 +284,7 @@ __global__ void __launch_bounds__(RES_LABEL_THREADS) resolve_label_kernel(ResPar
     __syncthreads();
     for (int q = tid; q < np; q += NT) {
         const int o = res_owner(p, q, p.label);
-        if (o >= 0) atomicAdd(&p.cnp[p.loc[o]], 1);
+        if (o >= 0) { atomicAdd(&p.cnp[p.loc[o]], 1); atomicMin(&p.ckey[p.loc[o]], res_depth_key(p, q)); }
     }
     __syncthreads();
     carry = 0;
@@ -279,7 +306,7 @@ __global__ void __launch_bounds__(RES_LABEL_THREADS) resolve_label_kernel(ResPar
     // a detached body's system: its own pairs (cfill of them, in cq) and the pairs of its partners' components;
     // cnp = the total, which decides the class
     for (int c = tid; c < ncomp; c += NT) {
-        int tot = p.cnp[c];
+        int tot = p.cnp[c], key = p.ckey[c];
         const int own = p.cown[c];
         if (own >= 0) {
             const int ps = p.cstart[c], no = p.cfill[c];
@@ -294,11 +321,12 @@ __global__ void __launch_bounds__(RES_LABEL_THREADS) resolve_label_kernel(ResPar
                     const int h2 = p.pairs[2 * q2] == own ? p.pairs[2 * q2 + 1] : p.pairs[2 * q2];
                     seen |= p.aux[h2] == cc;
                 }
-                if (!seen) tot += p.cfill[cc];
+                if (!seen) { tot += p.cfill[cc]; key = min(key, p.ckey[cc]); }
             }
         }
         p.cnp[c] = tot;
-        const int cls = res_class(tot);
+        int cls = res_class(tot);
+        if (cls == 5 && key < __float_as_int(RES_DEEP_RATIO)) cls = 6;      // scheduling only: the long chains first
         p.clist[(size_t)cls * p.cap + atomicAdd(&p.ctl[RES_CTL_CNT + cls], 1)] = c;
     }
     __syncthreads();
@@ -323,6 +351,16 @@ __device__ __forceinline__ double res_pair_u(double s2, double rc2, double inv) 
     const double q = fmin(fma(s2 * y, inv, -1.0 / 9.0), 1.0);          // (r - 0.1 rc) / (0.9 rc)
     const double K = q > 0.0 ? q * q * q * fma(q, fma(6.0, q, -15.0), 10.0) : 0.0;
     return (1.0 - K) * (y * y * y);
+}
+
+// the same without a branch (the small systems' kernel: one warp, straight-line code)
+__device__ __forceinline__ double res_pair_u_nb(double s2, double rc2, double inv) {
+    const bool in = (s2 < rc2) && (s2 > 0.0);
+    const double y = res_rsqrt(in ? s2 : 1.0);
+    const double q = fmin(fma(s2 * y, inv, -1.0 / 9.0), 1.0);
+    const double K = q > 0.0 ? q * q * q * fma(q, fma(6.0, q, -15.0), 10.0) : 0.0;
+    const double r = (1.0 - K) * (y * y * y);
+    return in ? r : 0.0;
 }
 
 // ---- controller (uniform over the CTA: every thread takes the same decisions from the same block-wide numbers) ----
@@ -810,8 +848,8 @@ __global__ void __launch_bounds__(RES_S_THREADS, RES_S_MINB) resolve_small_kerne
     __shared__ double sP[W][3][32];              // per column: position increments of the current right-hand side (y for f(y))
     __shared__ double sFt[W][3][32];             // per column: pair terms
     __shared__ double sDy[W][3][32];             // per column (identical copies): y_j - y_i at the start of the step
-    __shared__ double sCol[W][6][32];            // column results
-    __shared__ double sT[W][6][32];              // extrapolation tableau (warp 0)
+    __shared__ double sCol[W][6][32];            // column results; warp 0 turns them into the extrapolation tableau in place
+    __shared__ double sC[32][32];                // [pair][body]: +gm_j if the body is the pair's first member, -gm_i if its second, else 0
     __shared__ double sRc2[32], sInv[32], sGi[32], sGj[32];
     __shared__ int sPi[32], sPj[32], sQ[32], sQs[32], sBi[32], sBj[32], sBody[32], sFirst[64], sId[64];
     __shared__ float sFac[2];
@@ -830,8 +868,9 @@ __global__ void __launch_bounds__(RES_S_THREADS, RES_S_MINB) resolve_small_kerne
         __syncthreads();
         ticket = sCtl[0];
     }
-    if (ticket >= p.ctl[RES_CTL_CNT + 5]) break;
-    const int comp = p.clist[(size_t)5 * p.cap + ticket];
+    const int ndeep = p.ctl[RES_CTL_CNT + 6];                            // the systems that look deep first
+    if (ticket >= ndeep + p.ctl[RES_CTL_CNT + 5]) break;
+    const int comp = ticket < ndeep ? p.clist[(size_t)6 * p.cap + ticket] : p.clist[(size_t)5 * p.cap + ticket - ndeep];
     const int np = p.cnp[comp];
     const int own = p.cown[comp];                                          // a detached body's system (see res_owner), else -1
 
@@ -894,11 +933,11 @@ __global__ void __launch_bounds__(RES_S_THREADS, RES_S_MINB) resolve_small_kerne
     const int n = sCtl[3];
     const bool live = lane < n;
     const int me = live ? sBody[lane] : 0;
-    unsigned mI = 0u, mJ = 0u;                                             // this body's pairs as first / second member
-    for (int k = 0; k < np; ++k) { mI |= (sPi[k] == lane) ? (1u << k) : 0u; mJ |= (sPj[k] == lane) ? (1u << k) : 0u; }
-    if (!live) { mI = 0u; mJ = 0u; }
+    for (int k = w; k < np; k += W) sC[k][lane] = sPi[k] == lane ? sGj[k] : sPj[k] == lane ? -sGi[k] : 0.0;
+    // lanes beyond the pairs work on a pair of body 0 with itself and rc = 0: a term of exactly 0, no branch
     const int pi = lane < np ? sPi[lane] : 0, pj = lane < np ? sPj[lane] : 0;
     const double rc2 = lane < np ? sRc2[lane] : 0.0, inv = lane < np ? sInv[lane] : 0.0;
+    __syncthreads();
 
     // ---- the Bulirsch-Stoer loop (every warp takes the same decisions from the same published numbers) ----
     const double mu = p.mu, hh = p.h, tol = p.tol;
@@ -939,30 +978,26 @@ __global__ void __launch_bounds__(RES_S_THREADS, RES_S_MINB) resolve_small_kerne
                 const double yk = res_rsqrt(fma(z2, z2, fma(z1, z1, z0 * z0)));
                 const double wk = -mu * (yk * yk * yk);
                 double a0 = wk * z0, a1 = wk * z1, a2 = wk * z2;
-                if (lane < np) {                                           // lane = pair
+                {                                                          // lane = pair; straight-line code: the star's term
+                    // above and this chain are independent and interleave (one warp: every instruction waits for its operands)
                     double dx = sP[w][0][pj] - sP[w][0][pi], dy = sP[w][1][pj] - sP[w][1][pi], dz = sP[w][2][pj] - sP[w][2][pi];
                     if (base) { sDy[w][0][lane] = dx; sDy[w][1][lane] = dy; sDy[w][2][lane] = dz; }
                     else { dx += sDy[w][0][lane]; dy += sDy[w][1][lane]; dz += sDy[w][2][lane]; }
-                    const double u = res_pair_u(fma(dz, dz, fma(dy, dy, dx * dx)), rc2, inv);
+                    const double u = res_pair_u_nb(fma(dz, dz, fma(dy, dy, dx * dx)), rc2, inv);
                     sFt[w][0][lane] = u * dx; sFt[w][1][lane] = u * dy; sFt[w][2][lane] = u * dz;
                 }
                 __syncwarp();
-                for (unsigned mm = mJ; mm; mm &= mm - 1u) {                // lane = body: as second member, -gm_i u d
-                    const int q = __ffs(mm) - 1;
-                    const double g = sGi[q];
-                    a0 = fma(-g, sFt[w][0][q], a0); a1 = fma(-g, sFt[w][1][q], a1); a2 = fma(-g, sFt[w][2][q], a2);
-                }
-                for (unsigned mm = mI; mm; mm &= mm - 1u) {                // as first member, +gm_j u d
-                    const int q = __ffs(mm) - 1;
-                    const double g = sGj[q];
-                    a0 = fma(g, sFt[w][0][q], a0); a1 = fma(g, sFt[w][1][q], a1); a2 = fma(g, sFt[w][2][q], a2);
+#pragma unroll 2
+                for (int k = 0; k < np; ++k) {                             // lane = body: its terms in list order (0 for the pairs it is not in)
+                    const double g = sC[k][lane];
+                    a0 = fma(g, sFt[w][0][k], a0); a1 = fma(g, sFt[w][1][k], a1); a2 = fma(g, sFt[w][2][k], a2);
                 }
                 if (w == 0) ++nrhs;
                 if (base) {                                                // f(y) and the error scales of this BS step
                     if (live) {
                         f0[0] = a0; f0[1] = a1; f0[2] = a2;
                         const double sx2 = fma(y2, y2, fma(y1, y1, y0 * y0)), sv2 = fma(v2, v2, fma(v1, v1, v0 * v0));
-                        isx = sx2 > 0.0 ? 1.0 / sqrt(sx2) : 1e300; isv = sv2 > 0.0 ? 1.0 / sqrt(sv2) : 1e300;
+                        isx = sx2 > 0.0 ? res_rsqrt(sx2) : 1e300; isv = sv2 > 0.0 ? res_rsqrt(sv2) : 1e300;
                         d1[0] = hs * v0; d1[1] = hs * v1; d1[2] = hs * v2; d1[3] = hs * a0; d1[4] = hs * a1; d1[5] = hs * a2;
                     }
                     havef0 = true;
@@ -983,34 +1018,39 @@ __global__ void __launch_bounds__(RES_S_THREADS, RES_S_MINB) resolve_small_kerne
             if (run) {
 #pragma unroll
                 for (int c = 0; c < 6; ++c) sCol[w][c][lane] = cur[c];
+                // column w is there: warp 0, which is through with its own two substeps long before, takes the rows of
+                // the tableau as the columns come in (named barrier w: this warp arrives, warp 0 waits)
+                if (w > 0) { __threadfence_block(); res_nb_arrive(w, 64); }
             }
         }
-        __syncthreads();
         if (w == 0) {
             nrhs += (kcols + 1) * (kcols + 2) - 2;                         // the other columns' right-hand sides: sum of 2 (k + 1)
             int acc = -1, klast = 0;
             float facCur = 1.0f, facPrev = 1.0f;
+            bool done = false;
 #pragma unroll 1
             for (int k = 0; k <= kcols; ++k) {
+                if (k > 0) res_nb_sync(k, 64);
+                if (done) continue;                                        // (the later columns still have to be waited for)
                 double cur[6], prev[6];
 #pragma unroll
                 for (int c = 0; c < 6; ++c) { cur[c] = live ? sCol[k][c][lane] : 0.0; prev[c] = cur[c]; }
                 double err = 0.0;
                 if (live) {
 #pragma unroll 1
-                    for (int j = 1; j <= k; ++j) {                         // row k of the tableau from row k-1 (in sT), overwriting it
+                    for (int j = 1; j <= k; ++j) {                         // row k of the tableau from row k-1 (in sCol[0..k-1]), overwriting it
                         const double cf = RES_COEF[k * RES_KMAX + j];
 #pragma unroll
                         for (int c = 0; c < 6; ++c) {
-                            const double oldv = sT[j - 1][c][lane];
-                            sT[j - 1][c][lane] = cur[c];
+                            const double oldv = sCol[j - 1][c][lane];
+                            sCol[j - 1][c][lane] = cur[c];
                             prev[c] = cur[c];
                             cur[c] = fma(cur[c] - oldv, cf, cur[c]);
                         }
                     }
 #pragma unroll
                     for (int c = 0; c < 6; ++c) {
-                        sT[k][c][lane] = cur[c];
+                        sCol[k][c][lane] = cur[c];
                         double e = fabs(cur[c] - prev[c]) * (c < 3 ? isx : isv);
                         if (!(e <= 1e300)) e = 1e300;                       // NaN / inf: never accepted
                         err = fmax(err, e);
@@ -1022,13 +1062,13 @@ __global__ void __launch_bounds__(RES_S_THREADS, RES_S_MINB) resolve_small_kerne
                     const double e = err / tol;
                     facPrev = facCur; facCur = res_fac(e, k);
                     klast = k;
-                    if (e <= 1.0) { acc = k; break; }
-                    if (k < kcols && res_hopeless(e, k, ctl.ktarg)) break;
+                    if (e <= 1.0) { acc = k; done = true; }
+                    else if (k < kcols && res_hopeless(e, k, ctl.ktarg)) done = true;
                 }
             }
-            if (acc >= 0 && live) {
+            if (acc >= 0 && live) {                                        // every column has read the old state by now
 #pragma unroll
-                for (int c = 0; c < 6; ++c) sY[c][lane] += sT[acc][c][lane];
+                for (int c = 0; c < 6; ++c) sY[c][lane] += sCol[acc][c][lane];
             }
             if (lane == 0) { sCtl[1] = acc; sCtl[2] = klast; sFac[0] = facCur; sFac[1] = facPrev; }
         }

@@ -74,9 +74,11 @@ typedef enum {
                          order are stored, the count is still the true total */
     MO_ENOCONV = 5,   /* >= 1 body's Kepler solve failed (paper's iflag);
                          those bodies are left unchanged, the others advanced */
-    MO_ERESOLVE = 6   /* mo_set_resolve / mo_resolve: >= 1 encounter component was not resolved (no
+    MO_ERESOLVE = 6,  /* mo_set_resolve / mo_resolve: >= 1 encounter component was not resolved (no
                          convergence, or a truncated pair list); its bodies kept the Kepler-drift
                          result of that step.  Sticky: counted in mo_stats.resolve_fail */
+    MO_ELIMIT = 7     /* mo_accel_static: nb beyond mo_accel_static_max_nb() - its scratch is a fixed
+                         array, there is no allocation to fall back to.  Nothing was launched */
 } mo_status;
 
 typedef struct {
@@ -281,6 +283,32 @@ const char *mo_pair_kernel_name(const mo_ctx *ctx);
  * n_out their number); both reset on read. */
 mo_status mo_set_kernel_timing(mo_ctx *ctx, int32_t on);
 mo_status mo_pair_kernel_ms(mo_ctx *ctx, double *ms_out, int32_t *n_out);
+
+/* ---- No-allocation entry point -------------------------------------------------------------
+ * mo_accel_static: a(x) of a fully interacting system - the same operation as mo_accel (force block
+ * LOOP 2 with the changeover weight K; readings A-1..A-9), by the same
+ * kernels (pack, two-sided pair sum with 2 bodies per lane, fixed-order reduce), for callers that cannot
+ * call cudaMalloc: code under CUDA graph capture, tight serving loops, harnesses that forbid it.  It
+ * needs no context and calls no cudaMalloc / cudaFree / allocating library routine, ever: the kernels'
+ * scratch (packed tiles, work-unit list, row and column partial sums) is ONE file-scope device array of
+ * 2.7 MB inside the library, which every GPU that loads the library holds until exit.
+ *   nb            bodies, 1 <= nb <= mo_accel_static_max_nb() (4096); larger -> MO_ELIMIT, nothing launched
+ *   ld            leading dimension of x and a (ld >= nb, ld % 4 == 0)
+ *   gm, rcrit     device, nb doubles each: G m_j and the changeover radii (read)
+ *   x             device, 3*ld doubles, SoA planes x | y | z, democratic-heliocentric positions (read)
+ *   a             device, 3*ld doubles (written: rows < nb of each plane; nothing else is touched)
+ *   cuda_stream   cudaStream_t; NULL = legacy default stream.  Four kernels are enqueued; asynchronous
+ * All pointers 16-byte aligned, caller-owned.  The result equals mo_accel's to rounding (same arithmetic per
+ * pair, a different fixed summation tree) and is bit-reproducible from call to call.
+ * The array is looked up once per device (cudaGetSymbolAddress, with the caller's current device) and is
+ * SHARED by every call on that device; it keeps the last call's contents, none of which a later call reads
+ * before rewriting it (nothing has to start at zero).  Calls that overlap on the GPU - two streams, two
+ * host threads, two captured graphs replayed side by side - RACE on it: serialise them (one stream, or
+ * events).  Contexts (mo_create) do not use the array.
+ * MO_EINVAL: nb < 1, ld < nb, ld % 4, null / misaligned pointer.  MO_ECUDA: no device / launch error. */
+int32_t mo_accel_static_max_nb(void);
+mo_status mo_accel_static(int32_t nb, int32_t ld, const double *gm, const double *x,
+                          const double *rcrit, double *a, void *cuda_stream);
 
 const char *mo_strerror(mo_status s);
 const char *mo_version(void);

@@ -9,6 +9,7 @@
 
 #include <new>
 #include <algorithm>
+#include <mutex>
 #include <vector>
 
 #include "../../include/mopal.h"
@@ -344,6 +345,7 @@ extern "C" const char* mo_strerror(mo_status s) {
         case MO_EOVERFLOW: return "more encounter pairs than cap";
         case MO_ENOCONV: return "Kepler solve failed for at least one body";
         case MO_ERESOLVE: return "at least one encounter component was not resolved";
+        case MO_ELIMIT: return "size beyond the fixed maximum of a no-allocation entry point (mo_accel_static_max_nb)";
     }
     return "unknown status";
 }
@@ -1434,5 +1436,100 @@ extern "C" mo_status mo_probe_fp64_peak(void* cuda_stream, int32_t reps, double*
     *tflops_out = flops / (best * 1e-3) / 1e12;
     if (ms_out) *ms_out = best;
     if (tflops_mean_out) *tflops_mean_out = flops * reps / (tot * 1e-3) / 1e12;
+    return MO_OK;
+}
+
+// ---- mo_accel_static: the pair accelerations of a small system with NO allocation anywhere ------------------------
+// For callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid
+// it): the same kernels as mo_accel takes for a mid-size system - pack_kernel<false, true>, pair_sym_kernel<2>,
+// sym_reduce_kernel<false, false> - with their scratch (the packed j tiles, the work-unit list, the row and column
+// partial sums) in ONE file-scope device array of fixed size instead of a context's cudaMalloc'ed buffers.  No context:
+// the caller passes inputs and outputs.  Every GPU that loads the library holds the array (2.7 MB) until exit.
+constexpr int STATIC_MAX_NB = 4096;                                      // mo_accel_static_max_nb()
+constexpr int ST_IPT = 2;                                                // bodies per lane: the mid-size instance
+constexpr int ST_R = sym_rows(ST_IPT);                                   // 256 rows per row block
+constexpr int ST_NT = STATIC_MAX_NB / TJ;                                // 32 tiles
+constexpr int ST_NI = (STATIC_MAX_NB + ST_R - 1) / ST_R;                 // 16 row blocks
+constexpr int ST_NU = ST_NI * ST_NT - ST_IPT * (ST_NI * (ST_NI - 1) / 2);   // 272 units: one per (row block, j tile from its diagonal on)
+constexpr size_t st_up(size_t b) { return (b + 255) & ~(size_t)255; }
+constexpr size_t ST_OFF_TILES = 0;
+constexpr size_t ST_OFF_UNITS = ST_OFF_TILES + st_up((size_t)ST_NT * SYM_TILE_BYTES);
+constexpr size_t ST_OFF_USTART = ST_OFF_UNITS + st_up((size_t)ST_NU * sizeof(int4));
+constexpr size_t ST_OFF_PARTI = ST_OFF_USTART + st_up((size_t)(ST_NI + 1) * sizeof(int));
+constexpr size_t ST_OFF_PARTJ = ST_OFF_PARTI + st_up((size_t)ST_NU * 3 * ST_R * sizeof(double));
+constexpr size_t ST_BYTES = ST_OFF_PARTJ + st_up((size_t)(3LL * ((long long)ST_NI * STATIC_MAX_NB - (long long)ST_R * (ST_NI * (ST_NI - 1) / 2))) * sizeof(double));
+static_assert(STATIC_MAX_NB % ST_R == 0 && ST_BYTES < (3u << 20), "mo_accel_static: scratch layout");
+
+// The scratch itself.  In HOST code this name is a host-side stand-in, not a device address: the kernels get the address
+// cudaGetSymbolAddress returns (static_scratch_ptr below), never the name.
+static __device__ __align__(256) unsigned char g_static_scratch[ST_BYTES];
+
+// the work-unit list of this nb, written on the device (no host staging buffer): unit (I, t) = j tile t >= I * IPT of
+// row block I, all four groups of 32 columns; ustart[I] = first unit of row block I
+__global__ void static_plan_kernel(int4* __restrict__ units, int* __restrict__ ustart, int nI, int nTiles) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k <= nI) {
+        // row blocks I' < k hold nTiles - I' * IPT units each (k = nI: the total)
+        ustart[k] = k * nTiles - ST_IPT * (k * (k - 1) / 2);
+    }
+    if (k >= nI * nTiles) return;
+    const int I = k / nTiles, t = k - I * nTiles;
+    if (t < I * ST_IPT) return;
+    const int u0 = I * nTiles - ST_IPT * (I * (I - 1) / 2);
+    units[u0 + t - I * ST_IPT] = make_int4(I, t, t + 1, (TJ / 32) << 8);
+}
+
+// device address of the scratch on the CURRENT device: looked up once per device, with that device current
+static cudaError_t static_scratch_ptr(unsigned char** out) {
+    constexpr int MAXDEV = 64;
+    static unsigned char* ptrs[MAXDEV] = {};
+    static std::mutex mu;
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= MAXDEV) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(mu);
+    if (!ptrs[dev]) {
+        unsigned char* p = nullptr;
+        e = cudaGetSymbolAddress(reinterpret_cast<void**>(&p), g_static_scratch);
+        if (e != cudaSuccess) return e;
+        if (!p || (reinterpret_cast<uintptr_t>(p) & 255u)) return cudaErrorInvalidSymbol;
+        ptrs[dev] = p;
+    }
+    *out = ptrs[dev];
+    return cudaSuccess;
+}
+
+extern "C" int32_t mo_accel_static_max_nb(void) { return STATIC_MAX_NB; }
+
+extern "C" mo_status mo_accel_static(int32_t nb, int32_t ld, const double* gm, const double* x, const double* rcrit,
+                                     double* a, void* cuda_stream) {
+    if (nb < 1 || ld < nb || (ld & 3) || !gm || !x || !rcrit || !a) return MO_EINVAL;
+    if (!aligned16(gm) || !aligned16(x) || !aligned16(rcrit) || !aligned16(a)) return MO_EINVAL;
+    if (nb > STATIC_MAX_NB) return MO_ELIMIT;                            // the scratch is fixed: no fallback to an allocation
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+    unsigned char* base = nullptr;
+    if (static_scratch_ptr(&base) != cudaSuccess) { cudaGetLastError(); return MO_ECUDA; }
+    const int nTiles = (nb + TJ - 1) / TJ, nbPad = nTiles * TJ;
+    const int nI = (nbPad + ST_R - 1) / ST_R;
+    const int nU = nI * nTiles - ST_IPT * (nI * (nI - 1) / 2);
+    unsigned char* tiles = base + ST_OFF_TILES;
+    int4* units = reinterpret_cast<int4*>(base + ST_OFF_UNITS);
+    int* ustart = reinterpret_cast<int*>(base + ST_OFF_USTART);
+    double* partI = reinterpret_cast<double*>(base + ST_OFF_PARTI);
+    double* partJ = reinterpret_cast<double*>(base + ST_OFF_PARTJ);
+    // Nothing in the scratch has to start at zero: every entry the reduce kernel reads (one row partial per unit, one
+    // column partial per (row block, column at or right of its diagonal)) and every tile and unit record is rewritten
+    // by this call before it is read, whatever the last call - of any nb - left there.
+    const Gate open{nullptr, 0};
+    static_plan_kernel<<<(nI * nTiles + 1 + 127) / 128, 128, 0, st>>>(units, ustart, nI, nTiles);
+    pack_kernel<false, true><<<nTiles, TJ, 0, st>>>(const_cast<double*>(x), gm, rcrit, nb, nb, ld, tiles, nullptr, 0, 0.0, open);
+    SymParams sp;
+    sp.tiles = tiles; sp.x = x; sp.gm = gm; sp.rcrit = rcrit; sp.units = units; sp.partI = partI; sp.partJ = partJ;
+    sp.nb = nb; sp.ld = ld; sp.nbPad = nbPad; sp.unit0 = 0; sp.gate = open;
+    pair_sym_kernel<ST_IPT><<<nU, SYM_THREADS, 0, st>>>(sp);
+    sym_reduce_kernel<false, false><<<dim3((nb + 31) / 32, 3), RED_THREADS, 0, st>>>(partI, partJ, ustart, nb, ld, nbPad, a, nullptr, 0.0,
+                                                                                   0, nU, nullptr, ST_R, open);
+    if (cudaGetLastError() != cudaSuccess) return MO_ECUDA;
     return MO_OK;
 }

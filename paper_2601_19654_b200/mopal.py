@@ -15,7 +15,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libmopal.so")
 
-MO_OK, MO_EINVAL, MO_ENOMEM, MO_ECUDA, MO_EOVERFLOW, MO_ENOCONV, MO_ERESOLVE = range(7)
+MO_OK, MO_EINVAL, MO_ENOMEM, MO_ECUDA, MO_EOVERFLOW, MO_ENOCONV, MO_ERESOLVE, MO_ELIMIT = range(8)
 _SOFT = (MO_OK, MO_EOVERFLOW, MO_ENOCONV, MO_ERESOLVE)      # statuses reported in Stats.status instead of raised
 
 EXPORTS = ["mo_create", "mo_accel", "mo_drift", "mo_encounters", "mo_step", "mo_destroy",
@@ -24,7 +24,8 @@ EXPORTS = ["mo_create", "mo_accel", "mo_drift", "mo_encounters", "mo_step", "mo_
            "mo_pair_geometry", "mo_set_kernel_timing", "mo_pair_kernel_ms", "mo_strerror", "mo_version",
            "mo_set_nbig", "mo_pair_kernel_name", "mo_h2dh", "mo_dh2h", "mo_hill", "mo_set_hill", "mo_energy",
            "mo_resolve", "mo_set_resolve", "mo_resolve_stats", "mo_boxes_copy",
-           "mo_set_shard", "mo_shard_range", "mo_shard_units", "mo_step_begin", "mo_accel_summed", "mo_step_end"]
+           "mo_set_shard", "mo_shard_range", "mo_shard_units", "mo_step_begin", "mo_accel_summed", "mo_step_end",
+           "mo_accel_static", "mo_accel_static_max_nb"]
 
 
 class MoStats(C.Structure):
@@ -90,6 +91,9 @@ def load():
     L.mo_step_host.restype = C.c_int
     L.mo_step_host.argtypes = [vp, D, I32, vp, vp, vp, I32, vp, I64, C.POINTER(MoStats)]
     L.mo_accel_host.restype = C.c_int; L.mo_accel_host.argtypes = [vp, vp, vp]
+    L.mo_accel_static_max_nb.restype = I32; L.mo_accel_static_max_nb.argtypes = []
+    L.mo_accel_static.restype = C.c_int
+    L.mo_accel_static.argtypes = [I32, I32, vp, vp, vp, vp, vp]
     L.mo_probe_fp64_peak.restype = C.c_int
     L.mo_probe_fp64_peak.argtypes = [vp, I32, C.POINTER(D), C.POINTER(D), C.POINTER(D)]
     L.mo_pair_geometry.restype = C.c_int
@@ -117,6 +121,31 @@ def shard_range(n, rank, world):
     if st != MO_OK:
         raise MopalError(st, "mo_shard_range")
     return int(lo.value), int(hi.value)
+
+
+def accel_static_max_nb() -> int:
+    return int(load().mo_accel_static_max_nb())
+
+
+def accel_static(gm, x, rcrit, a=None):
+    """a(x) through mo_accel_static - the entry point that allocates nothing (its scratch is a fixed device array inside
+    the library; nb <= accel_static_max_nb()).  gm, rcrit: [nb], x: [3, ld] float64 CUDA tensors; returns a [3, ld]
+    (the tensor passed as ``a``, else a new one - that allocation is the caller's, not the library's).  Enqueued on
+    torch's current stream; calls that overlap on the GPU race on the shared scratch."""
+    import torch
+    nb, ld = int(gm.numel()), int(x.shape[1])
+    for t in (gm, x, rcrit):
+        if not (t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
+            raise MopalError(MO_EINVAL, "accel_static: float64 contiguous CUDA tensors")
+    if a is None:
+        a = torch.zeros_like(x)
+    st = load().mo_accel_static(nb, ld, gm.data_ptr(), x.data_ptr(), rcrit.data_ptr(), a.data_ptr(),
+                                C.c_void_p(torch.cuda.current_stream().cuda_stream))
+    if st == MO_ELIMIT:
+        raise MopalError(st, f"mo_accel_static: nb = {nb} > {accel_static_max_nb()}")
+    if st != MO_OK:
+        raise MopalError(st, "mo_accel_static")
+    return a
 
 
 def probe_fp64_peak(reps: int = 5, with_mean: bool = False):

@@ -137,6 +137,18 @@ __device__ __forceinline__ void res_cluster_barrier(int* cnt, int target, int na
 __device__ __forceinline__ void res_nb_arrive(int id, int n) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(n) : "memory"); }
 __device__ __forceinline__ void res_nb_sync(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
 
+// thread-block cluster: the hardware barrier in its two halves, and a load from another CTA's shared memory
+__device__ __forceinline__ void res_cl_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
+__device__ __forceinline__ void res_cl_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
+__device__ __forceinline__ void res_cl_sync() { res_cl_arrive(); res_cl_wait(); }
+__device__ __forceinline__ double res_ld_remote(const void* mine, int rank) {      // the same variable in CTA `rank` of the cluster
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(smem_u32(mine)), "r"(rank));
+    double v;
+    asm volatile("ld.shared::cluster.f64 %0, [%1];" : "=d"(v) : "r"(r) : "memory");
+    return v;
+}
+
 // barrier of the first nthreads threads of the block (whole warps), beside the block barrier 0
 __device__ __forceinline__ void res_bar(int nthreads) { asm volatile("bar.sync 1, %0;" ::"r"(nthreads) : "memory"); }
 
@@ -414,6 +426,17 @@ __global__ void __launch_bounds__(NT, 1) resolve_solve_kernel(ResParams p, int s
     __shared__ double sRed[32];
     __shared__ int sScan[64];
     __shared__ int sBc[2];
+    // SLICE (classes 1 and 2): the columns of a step stay in the shared memory of the CTAs that integrated them, and the
+    // extrapolation tableau is SHARED OUT - CTA c runs it for the bodies [c S, (c + 1) S), S = n / NCOL, reading the
+    // columns from the other CTAs' shared memory (distributed shared memory, ~0.1 us a load), and every CTA fetches the
+    // row maxima of the error estimates and, after an accepted step, its bodies' increments from their owners.  Measured
+    // on Jupiter's star at cfg3 (342 bodies, 92 attempted steps; per attempt, longest column 22 us): with the results in
+    // global memory and the whole tableau in every CTA the exchange cost 5 + 14 us per attempt (profiles/r2d_resolve.md).
+    // Class 3 (1024 threads) has no shared memory left for the columns and keeps the exchange through global memory.
+    constexpr bool SLICE = NCOL > 1 && NT <= 512;
+    __shared__ double sRedK[SLICE ? 4 : 1][RES_KMAX];                      // the slice warps' error maxima of every tableau row
+    __shared__ double sErr[RES_KMAX];                                      // this CTA's slice: error maximum of every row
+    __shared__ int sStop;                                                  // the cluster-barrier phase after which the warps without a body leave
     constexpr unsigned full = 0xffffffffu;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     if (tid < 64) sScan[tid] = 0;
@@ -429,6 +452,7 @@ __global__ void __launch_bounds__(NT, 1) resolve_solve_kernel(ResParams p, int s
 
     for (;;) {
     __syncthreads();                                                       // the previous component is finished with shared memory
+    if (SLICE && tid == 0) sStop = 0x7fffffff;
     int ticket;
     if (NCOL > 1) ticket = cl + (round++) * ncl;
     else if (firstTicket) { ticket = blockIdx.x; firstTicket = false; }    // the first gridDim.x components need no counter
@@ -440,7 +464,7 @@ __global__ void __launch_bounds__(NT, 1) resolve_solve_kernel(ResParams p, int s
     if (ticket >= p.ctl[RES_CTL_CNT + CLS]) break;
     const int comp = p.clist[(size_t)CLS * p.cap + ticket];
     const int np = p.cnp[comp];
-    const int npad = (np + 31) & ~31;
+    const int npad = SLICE ? (np + 32) & ~31 : (np + 31) & ~31;             // (SLICE: at least as many slots as bodies - sF doubles as the column result)
     double* const sF = reinterpret_cast<double*>(res_dyn);                  // [3][npad] pair terms
     double* const sDy = sF + 3 * npad;                                      // [3][npad] y_j - y_i of the state the BS step starts from
     double* const sRc2 = sDy + 3 * npad;                                    // [npad] max(rcrit_i, rcrit_j)^2
@@ -591,6 +615,9 @@ __global__ void __launch_bounds__(NT, 1) resolve_solve_kernel(ResParams p, int s
     }
     for (int k = np + tid; k < npad; k += NT) sPi[k] = 0xffff;              // pad pairs: no group of theirs is a whole run of a hub
     __syncthreads();                                                       // the temporaries (on sF, sDy) are consumed; sAdj is complete
+    const int S = nbp / (NCOL > 1 ? NCOL : 1);                              // SLICE: bodies of the tableau slice of a CTA (nbp is a multiple of 32)
+    const int SLW = (S + 31) & ~31;                                         // ... and the threads (whole warps) that work on it
+    double* const sT = reinterpret_cast<double*>(res_dyn + pairBytes + bodyBytes);   // SLICE: [6 KMAX][S] tableau of this CTA's slice
     const bool tabShared = pairBytes + bodyBytes + 6 * RES_KMAX * 8 * nbp <= smemBytes;
     const int TS = tabShared ? nbp : NT;                                    // tableau stride
     double* const Tb = (tabShared ? reinterpret_cast<double*>(res_dyn + pairBytes + bodyBytes)
@@ -608,6 +635,7 @@ __global__ void __launch_bounds__(NT, 1) resolve_solve_kernel(ResParams p, int s
     double t = 0.0;
     ResCtl ctl{hh, 5, 0};
     int fail = 0, nacc = 0, nrhs = 0;
+    int nphase = 0;                                                        // SLICE: phases of the cluster barrier passed in this component
     bool havef0 = false;
     while (!fail) {
         const double rem = hh - t;
@@ -738,8 +766,104 @@ __global__ void __launch_bounds__(NT, 1) resolve_solve_kernel(ResParams p, int s
                 }
             }
         };
-        double* const cres = NCOL > 1 ? p.colres + ((size_t)(cslot * 2 + (nbarrier & 1)) * NCOL) * 6 * 1024 : nullptr;   // [column][component][thread], 1024 per plane
-        if constexpr (NCOL > 1) {
+        if constexpr (SLICE) {
+            // Every CTA its own column (the CTAs beyond the columns this step tries: f(y) only).  The result goes where the
+            // right-hand side's scratch was - rows 0..2 on sP, rows 3..5 on sF (npad >= nbp) - for the other CTAs to read.
+            // Two phases of the cluster's hardware barrier per step: A - the columns are there; B - the slices' tableaux
+            // and error maxima are there, and nobody reads a column any more.  Whoever writes the next column, tableau
+            // or maxima has passed the barrier all their readers arrive at only after reading.
+            double mine[6];
+            column(col, col <= kcols, mine);
+            res_bar(nact);                                                 // the last right-hand side's sums have read sF
+            if (live && col <= kcols) {
+#pragma unroll
+                for (int c = 0; c < 3; ++c) { sP[c * nbp + tid] = mine[c]; sF[c * npad + tid] = mine[3 + c]; }
+            }
+            res_cl_sync(); ++nphase;                                       // A
+            if (col == 0) nrhs += (kcols + 1) * (kcols + 2) - 2;            // the other columns' right-hand sides: sum of 2 (k + 1)
+            if (tid < SLW) {
+                // this CTA's slice of the tableau: body b, rows 0..kcols in place (entry j * 6 + c at sT[(j * 6 + c) S + tid];
+                // row k's column comes from CTA k, the next row's is on its way while this row is extrapolated)
+                const int b = col * S + tid;
+                const bool liveS = tid < S && b < n;
+                const int bb = liveS ? b : 0;
+                double nxt[6];
+#pragma unroll
+                for (int c = 0; c < 3; ++c) { nxt[c] = res_ld_remote(&sP[c * nbp + bb], 0); nxt[3 + c] = res_ld_remote(&sF[c * npad + bb], 0); }
+                const double isx = sIS[bb], isv = sIS[nbp + bb];
+                double* const T = sT + tid;
+#pragma unroll 1
+                for (int k = 0; k <= kcols; ++k) {
+                    double cur[6], prev[6];
+#pragma unroll
+                    for (int c = 0; c < 6; ++c) { cur[c] = nxt[c]; prev[c] = cur[c]; }
+                    if (k < kcols) {
+#pragma unroll
+                        for (int c = 0; c < 3; ++c) { nxt[c] = res_ld_remote(&sP[c * nbp + bb], k + 1); nxt[3 + c] = res_ld_remote(&sF[c * npad + bb], k + 1); }
+                    }
+                    double err = 0.0;
+                    if (liveS) {
+#pragma unroll 1
+                        for (int j = 1; j <= k; ++j) {
+                            const double cf = RES_COEF[k * RES_KMAX + j];
+#pragma unroll
+                            for (int c = 0; c < 6; ++c) {
+                                double* tp = T + ((j - 1) * 6 + c) * S;
+                                const double oldv = *tp;
+                                *tp = cur[c];
+                                prev[c] = cur[c];
+                                cur[c] = fma(cur[c] - oldv, cf, cur[c]);
+                            }
+                        }
+#pragma unroll
+                        for (int c = 0; c < 6; ++c) {
+                            T[(k * 6 + c) * S] = cur[c];
+                            double e = fabs(cur[c] - prev[c]) * (c < 3 ? isx : isv);
+                            if (!(e <= 1e300)) e = 1e300;                   // NaN / inf: never accepted
+                            err = fmax(err, e);
+                        }
+                    }
+#pragma unroll
+                    for (int o = 16; o > 0; o >>= 1) err = fmax(err, __shfl_xor_sync(full, err, o));
+                    if (lane == 0) sRedK[warp][k] = err;
+                }
+                asm volatile("bar.sync 2, %0;" ::"r"(SLW) : "memory");      // the slice's warps
+                if (tid < RES_KMAX) {
+                    double v = 0.0;
+                    for (int w2 = 0; w2 < SLW / 32; ++w2) v = fmax(v, sRedK[w2][tid]);
+                    sErr[tid] = tid <= kcols ? v : 0.0;
+                }
+            }
+            res_cl_sync(); ++nphase;                                       // B
+            // the rows' error maxima over all the slices: lane l reads rows (l >> 3) + 1 and (l >> 3) + 5 of CTA l & 7
+            {
+                const int r0 = (lane >> 3) + 1, r1 = (lane >> 3) + 5;
+                double v0 = res_ld_remote(&sErr[r0], lane & (NCOL - 1));
+                double v1 = r1 < RES_KMAX ? res_ld_remote(&sErr[r1], lane & (NCOL - 1)) : 0.0;
+#pragma unroll
+                for (int o = 4; o > 0; o >>= 1) { v0 = fmax(v0, __shfl_xor_sync(full, v0, o)); v1 = fmax(v1, __shfl_xor_sync(full, v1, o)); }
+                bool done = false;
+                double eL = 0.0, eP = 0.0;                                  // the error of the last row looked at, and of the one before
+#pragma unroll
+                for (int k = 1; k < RES_KMAX; ++k) {
+                    const double e = (k <= 4 ? __shfl_sync(full, v0, (k - 1) * 8) : __shfl_sync(full, v1, (k - 5) * 8)) / tol;
+                    if (k <= kcols && !done) {
+                        eP = eL; eL = e; klast = k;
+                        if (e <= 1.0) { acc = k; done = true; }
+                        else if (k < kcols && res_hopeless(e, k, ctl.ktarg)) done = true;
+                    }
+                }
+                facCur = res_fac(eL, klast);
+                facPrev = klast >= 2 ? res_fac(eP, klast - 1) : 1.0f;
+            }
+            if (acc >= 0 && live) {                                        // this body's increment from the CTA that ran its tableau
+                const int o = tid / S, i = tid - o * S;
+#pragma unroll
+                for (int c = 0; c < 6; ++c) sY[c * nbp + tid] += res_ld_remote(&sT[(acc * 6 + c) * S + i], o);
+            }
+        }
+        double* const cres = NCOL > 1 && !SLICE ? p.colres + ((size_t)(cslot * 2 + (nbarrier & 1)) * NCOL) * 6 * 1024 : nullptr;   // [column][component][thread], 1024 per plane
+        if constexpr (NCOL > 1 && !SLICE) {
             // every CTA its own column (the CTAs beyond the columns this step tries: f(y) only), results through global
             // memory, one barrier of the cluster per Bulirsch-Stoer step
             double mine[6];
@@ -753,7 +877,7 @@ __global__ void __launch_bounds__(NT, 1) resolve_solve_kernel(ResParams p, int s
             if (col == 0) nrhs += (kcols + 1) * (kcols + 2) - 2;            // the other columns' right-hand sides: sum of 2 (k + 1)
         }
 #pragma unroll 1
-        for (int k = 0; k <= kcols; ++k) {
+        for (int k = 0; !SLICE && k <= kcols; ++k) {
             double cur[6];
             if constexpr (NCOL > 1) {
 #pragma unroll
@@ -807,7 +931,7 @@ __global__ void __launch_bounds__(NT, 1) resolve_solve_kernel(ResParams p, int s
             if (ctl.rejected(klast, facCur)) fail = 1;
             continue;
         }
-        if (live) {
+        if (!SLICE && live) {
 #pragma unroll
             for (int c = 0; c < 6; ++c) sY[c * nbp + tid] += Tb[(size_t)(acc * 6 + c) * TS];
         }
@@ -815,6 +939,10 @@ __global__ void __launch_bounds__(NT, 1) resolve_solve_kernel(ResParams p, int s
         ++nacc;
         havef0 = false;
         ctl.accepted(acc, facCur, facPrev);
+    }
+    if constexpr (SLICE) {                                                 // one more phase, after which the warps without a body leave too
+        if (tid == 0) sStop = nphase + 1;
+        res_cl_sync();
     }
     if (!fail && live && col == 0 && (own < 0 || own == me)) {             // a detached body's system writes only that body
 #pragma unroll
@@ -825,6 +953,13 @@ __global__ void __launch_bounds__(NT, 1) resolve_solve_kernel(ResParams p, int s
         if (fail) { atomicAdd(&p.out->fail, 1); atomicAdd(&p.st->resolve_fail, 1); }
     }
     }   // active warps
+    else if constexpr (SLICE) {
+        // the cluster's barrier counts every thread of its CTAs: the warps without a body go through its phases too
+        for (int ph = 1;; ++ph) {
+            res_cl_sync();
+            if (ph == *reinterpret_cast<volatile int*>(&sStop)) break;
+        }
+    }
     }   // components
 }
 

@@ -735,7 +735,7 @@ static mo_status ensure_resolve_scratch(mo_ctx* ctx) {
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_cfill, capn);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_cq, capn);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_clist, capn * RES_NCLS);
-    if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_ctl, 16);
+    if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_ctl, (size_t)((RES_CTL_N + 15) & ~15));
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_tab, (size_t)6 * RES_KMAX * 1024 * RES_CL_GRID);   // per CTA of the widest launch
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_colres, (size_t)RES_NCLUSTERS * 2 * RES_NCOL * 6 * 1024);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_csync, RES_NCLUSTERS);
@@ -779,7 +779,15 @@ static mo_status enqueue_resolve(mo_ctx* ctx, double dt, double tol) {
     rp.ctl = ctx->res_ctl; rp.colres = ctx->res_colres; rp.csync = ctx->res_csync; rp.mode = ctx->res_mode; rp.tab = ctx->res_tab; rp.dbody = ctx->res_dbody; rp.dbodyi = ctx->res_dbodyi; rp.dpair = ctx->res_dpair;
     rp.dpairi = ctx->res_dpairi; rp.dbodyN = ctx->res_dbodyN;
     rp.cap = ctx->cap > 0 ? ctx->cap : 1; rp.nb = ctx->nb; rp.ld = ctx->ld; rp.mu = ctx->mu; rp.h = dt; rp.tol = tol;
-    resolve_label_kernel<<<1, RES_LABEL_THREADS, 0, ctx->stream>>>(rp);
+    {
+        // one cluster of RES_LABEL_CTAS CTAs (a short list is handled by its first CTA alone)
+        cudaLaunchConfig_t cfg = {};
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = RES_LABEL_CTAS; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        cfg.gridDim = dim3(RES_LABEL_CTAS); cfg.blockDim = dim3(RES_LABEL_THREADS); cfg.stream = ctx->stream; cfg.attrs = at; cfg.numAttrs = 1;
+        CK(cudaLaunchKernelEx(&cfg, resolve_label_kernel, rp));
+    }
     mo_status s = post_launch(ctx);
     if (s != MO_OK) return s;
     // the size classes side by side: the few large components (a giant's star is a long chain of right-hand sides on one

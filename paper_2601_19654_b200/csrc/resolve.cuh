@@ -36,9 +36,10 @@ namespace mopal {
 
 constexpr int RES_KMAX = 8;        // columns: 2, 4, .., 16 substeps
 constexpr int RES_HEAVY = 12;      // a body with more pairs is summed by its whole warp
-constexpr int RES_NCLS = 7;        // size classes: 0..3 one thread per body (64 / 256 / 512 / 1024 threads), 4 streamed,
+constexpr int RES_NCLS = 10;       // size classes: 0..3 one thread per body (64 / 256 / 512 / 1024 threads), 4 streamed,
                                    // 5 the small systems (at most RES_PHI_S pairs): one warp per column; 6 those of
-                                   // them that look like a long chain of steps (a deep passage): taken first
+                                   // them that look like a long chain of steps (a deep passage), in four levels of
+                                   // depth (6: the deepest .. 9): taken first, deepest first
 constexpr int RES_PHI_0 = 63, RES_PHI_1 = 255, RES_PHI_2 = 511, RES_PHI_3 = 1023;   // largest pair count of classes 0..3
 constexpr int RES_PHI_S = 31;      // ... and of class 5: at most 32 bodies, one per lane
 constexpr int RES_S_THREADS = 32 * RES_KMAX;   // resolve_small_kernel: warp w integrates column w
@@ -191,58 +192,103 @@ __device__ __forceinline__ int res_depth_key(const ResParams& p, int q) {
     return __float_as_int(r >= 0.f ? fminf(r, 1e30f) : 1e30f);            // NaN: not deep
 }
 
-// min-label propagation along the pairs that belong to components (not left out, not owned by a detached body)
-__device__ __forceinline__ void res_propagate(const ResParams& p, int np, bool massive_only) {
-    volatile int* label = p.label;
-    int changed;
-    do {
-        changed = 0;
-        for (int q = threadIdx.x; q < np; q += RES_LABEL_THREADS) {
-            const int i = p.pairs[2 * q], j = p.pairs[2 * q + 1];
-            const bool mi = p.gm[i] > 0.0, mj = p.gm[j] > 0.0;
-            if (massive_only ? !(mi && mj) : (!mi && !mj)) continue;
-            const int li = label[i], lj = label[j];
-            if (li < 0 || lj < 0) continue;                       // a detached body's pair
-            if (li < lj) { atomicMin(p.label + j, li); changed = 1; }
-            else if (lj < li) { atomicMin(p.label + i, lj); changed = 1; }
-        }
-        changed = __syncthreads_or(changed);
-    } while (changed);
+// X-1: connected components of the pair graph and the detached bodies' systems.  One cluster of RES_LABEL_CTAS CTAs (a list
+// of up to RES_LABEL_SOLO pairs: its first CTA alone): label[b] = smallest body of b's component, by min-propagation along
+// the pairs until nothing changes (encounter graphs are stars around the big bodies: a few sweeps); then the systems in
+// ascending order of their first pair, their pair counts, the pairs grouped by system and the class lists.  Every phase
+// is a loop over the pairs (or the systems) strided over all the threads at work, with the cluster's hardware barrier
+// in between; the two exchanges that are not through global memory - "did any thread change a label" and the CTAs' totals
+// of a scan - go through the CTAs' shared memory.  (One CTA took 0.37 ms for the 12.7 k pairs of the big x all workload.)
+constexpr int RES_LABEL_CTAS = 8;
+constexpr int RES_LABEL_SOLO = 2048;
+__device__ __forceinline__ int res_ld_remote_int(const void* mine, int rank) {    // the same variable in CTA `rank` of the cluster
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(smem_u32(mine)), "r"(rank));
+    int v;
+    asm volatile("ld.shared::cluster.s32 %0, [%1];" : "=r"(v) : "r"(r) : "memory");
+    return v;
 }
-
-// X-1: connected components of the pair graph and the detached bodies' systems.  One CTA: label[b] = smallest body of
-// b's component, by min-propagation along the pairs until nothing changes (encounter graphs are stars around the big
-// bodies: a few sweeps); then the systems in ascending order of their first pair, their pair counts, the pairs grouped
-// by system and the class lists.
 __global__ void __launch_bounds__(RES_LABEL_THREADS) resolve_label_kernel(ResParams p) {
     __shared__ int sScan[64];
+    __shared__ int sXc[2][2];                                              // [parity][flag | total]: what this CTA tells the others
     constexpr int NT = RES_LABEL_THREADS;
-    const int tid = threadIdx.x;
+    const int tid = threadIdx.x, rank = blockIdx.x;                        // (the grid is one cluster)
     if (tid < 64) sScan[tid] = 0;
-    if (tid == 0) { *p.out = ResStats{0, 0, 0, 0}; for (int k = 0; k < RES_CTL_N; ++k) p.ctl[k] = 0; }
-    if (tid < RES_NCLUSTERS) p.csync[tid] = 0;
     const long long nce = p.st->nce_last;
-    if (nce <= 0 || nce > p.cap) { if (tid == 0) p.mode[1] = 0; }
+    // a short list is one CTA's work (its barriers are cheaper than the cluster's); the other CTAs leave at once and the
+    // cluster's barrier is never used
+    const bool solo = nce <= RES_LABEL_SOLO || gridDim.x == 1;
+    if (solo && rank > 0) return;
+    const int NC = solo ? 1 : (int)gridDim.x;
+    const int gtid = rank * NT + tid, GNT = NC * NT;
+    if (gtid == 0) { *p.out = ResStats{0, 0, 0, 0}; for (int k = 0; k < RES_CTL_N; ++k) p.ctl[k] = 0; }
+    if (gtid < RES_NCLUSTERS) p.csync[gtid] = 0;
+    if (nce <= 0 || nce > p.cap) { if (gtid == 0) p.mode[1] = 0; }
     if (nce <= 0) return;
-    if (nce > p.cap) { if (tid == 0) { p.out->fail = 1 << 30; atomicAdd(&p.st->resolve_fail, 1); } return; }      // truncated list: nothing can be resolved
+    if (nce > p.cap) { if (gtid == 0) { p.out->fail = 1 << 30; atomicAdd(&p.st->resolve_fail, 1); } return; }      // truncated list: nothing can be resolved
+    int xph = 0;                                                           // exchanges so far (the slots alternate)
+    // barrier of all the threads at work; what a thread wrote to global memory before it, every thread sees after it
+    auto sync = [&]() { if (solo) __syncthreads(); else res_cl_sync(); };
+    // OR over all the threads at work (with a barrier)
+    auto any = [&](int v) -> int {
+        v = __syncthreads_or(v);
+        if (solo) return v;
+        if (tid == 0) sXc[xph & 1][0] = v;
+        res_cl_sync();
+        int r = 0;
+        for (int c = 0; c < NC; ++c) r |= res_ld_remote_int(&sXc[xph & 1][0], c);
+        ++xph;
+        return r;
+    };
+    // exclusive scan of one int per thread, in (CTA, thread) order, and the total over all the threads at work
+    auto scan = [&](int v, int& total) -> int {
+        int tot;
+        const int off = res_scan(v, sScan, tot);
+        if (solo) { total = tot; return off; }
+        if (tid == 0) sXc[xph & 1][1] = tot;
+        res_cl_sync();
+        int before = 0, all = 0;
+        for (int c = 0; c < NC; ++c) { const int t = res_ld_remote_int(&sXc[xph & 1][1], c); all += t; before += c < rank ? t : 0; }
+        ++xph;
+        total = all;
+        return before + off;
+    };
+    // min-label propagation along the pairs that belong to components (not left out, not owned by a detached body)
+    auto propagate = [&](bool massive_only) {
+        volatile int* label = p.label;
+        int changed;
+        do {
+            changed = 0;
+            for (int q = gtid; q < (int)nce; q += GNT) {
+                const int i = p.pairs[2 * q], j = p.pairs[2 * q + 1];
+                const bool mi = p.gm[i] > 0.0, mj = p.gm[j] > 0.0;
+                if (massive_only ? !(mi && mj) : (!mi && !mj)) continue;
+                const int li = label[i], lj = label[j];
+                if (li < 0 || lj < 0) continue;                   // a detached body's pair
+                if (li < lj) { atomicMin(p.label + j, li); changed = 1; }
+                else if (lj < li) { atomicMin(p.label + i, lj); changed = 1; }
+            }
+            changed = any(changed);
+        } while (changed);
+    };
     const int np = (int)nce;
     int anyMassless = 0;
-    for (int q = tid; q < np; q += NT) {
+    for (int q = gtid; q < np; q += GNT) {
         const int i = p.pairs[2 * q], j = p.pairs[2 * q + 1];
         p.label[i] = i; p.label[j] = j; p.aux[i] = 0; p.aux[j] = 0; p.loc[i] = 0; p.loc[j] = 0;
         anyMassless |= (p.gm[i] > 0.0 && p.gm[j] > 0.0) ? 0 : 1;
     }
-    anyMassless = __syncthreads_or(anyMassless);
+    anyMassless = any(anyMassless);
     if (anyMassless) {
         // cores: components of the massive-massive pairs alone; aux[root] = their pair count
-        res_propagate(p, np, true);
-        for (int q = tid; q < np; q += NT) {
+        propagate(true);
+        for (int q = gtid; q < np; q += GNT) {
             const int i = p.pairs[2 * q], j = p.pairs[2 * q + 1];
             if (p.gm[i] > 0.0 && p.gm[j] > 0.0) atomicAdd(&p.aux[p.label[i]], 1);
         }
-        __syncthreads();
+        sync();
         // size of a massless body's own system (an upper bound: a core shared by two partners counts twice)
-        for (int q = tid; q < np; q += NT) {
+        for (int q = gtid; q < np; q += GNT) {
             const int i = p.pairs[2 * q], j = p.pairs[2 * q + 1];
             const bool mi = p.gm[i] > 0.0, mj = p.gm[j] > 0.0;
             if (mi == mj) continue;
@@ -250,41 +296,41 @@ __global__ void __launch_bounds__(RES_LABEL_THREADS) resolve_label_kernel(ResPar
             atomicAdd(&p.loc[l], 1);                                              // partners
             atomicAdd(&p.aux[l], 1 + p.aux[p.label[h]]);                           // pairs (aux of a massless body)
         }
-        __syncthreads();
-        for (int q = tid; q < np; q += NT) {
+        sync();
+        for (int q = gtid; q < np; q += GNT) {
 #pragma unroll
             for (int e = 0; e < 2; ++e) {
                 const int b = p.pairs[2 * q + e];
                 if (!(p.gm[b] > 0.0)) p.label[b] = (p.loc[b] >= 1 && p.loc[b] <= RES_DET_PARTNERS && p.aux[b] <= RES_PHI_0) ? -1 : b;
             }
         }
-        __syncthreads();
+        sync();
     }
-    res_propagate(p, np, false);
+    propagate(false);
     // first pair of every owner (loc, until the systems are numbered)
-    for (int q = tid; q < np; q += NT) { p.loc[p.pairs[2 * q]] = 0x7fffffff; p.loc[p.pairs[2 * q + 1]] = 0x7fffffff; }
-    __syncthreads();
-    for (int q = tid; q < np; q += NT) {
+    for (int q = gtid; q < np; q += GNT) { p.loc[p.pairs[2 * q]] = 0x7fffffff; p.loc[p.pairs[2 * q + 1]] = 0x7fffffff; }
+    sync();
+    for (int q = gtid; q < np; q += GNT) {
         const int o = res_owner(p, q, p.label);
         if (o >= 0) atomicMin(&p.loc[o], q);
     }
-    __syncthreads();
+    sync();
     int carry = 0;
-    for (int base = 0; base < np; base += NT) {
-        const int q = base + tid;
+    for (int base = 0; base < np; base += GNT) {
+        const int q = base + gtid;
         int isfirst = 0, o = -1;
         if (q < np) { o = res_owner(p, q, p.label); isfirst = (o >= 0 && p.loc[o] == q) ? 1 : 0; }
         int tot;
-        const int off = res_scan(isfirst, sScan, tot);
+        const int off = scan(isfirst, tot);
         if (isfirst) { const int c = carry + off; p.cfill[c] = q; p.cnp[c] = 0; p.cown[c] = p.gm[o] > 0.0 ? -1 : o; p.ckey[c] = 0x7f7fffff; }
         carry += tot;
     }
     const int ncomp = carry;
-    __syncthreads();
-    for (int c = tid; c < ncomp; c += NT) { p.loc[res_owner(p, p.cfill[c], p.label)] = c; }   // owner -> system
-    __syncthreads();
+    sync();
+    for (int c = gtid; c < ncomp; c += GNT) { p.loc[res_owner(p, p.cfill[c], p.label)] = c; }   // owner -> system
+    sync();
     // aux[b] = the component of a body that is in one (massive, or massless and not detached), else -1
-    for (int q = tid; q < np; q += NT) {
+    for (int q = gtid; q < np; q += GNT) {
 #pragma unroll
         for (int e = 0; e < 2; ++e) {
             const int b = p.pairs[2 * q + e];
@@ -292,32 +338,32 @@ __global__ void __launch_bounds__(RES_LABEL_THREADS) resolve_label_kernel(ResPar
             p.aux[b] = (lb >= 0 && p.loc[lb] != 0x7fffffff) ? p.loc[lb] : -1;
         }
     }
-    for (int c = tid; c < ncomp; c += NT) p.cfill[c] = 0;
-    __syncthreads();
-    for (int q = tid; q < np; q += NT) {
+    for (int c = gtid; c < ncomp; c += GNT) p.cfill[c] = 0;
+    sync();
+    for (int q = gtid; q < np; q += GNT) {
         const int o = res_owner(p, q, p.label);
         if (o >= 0) { atomicAdd(&p.cnp[p.loc[o]], 1); atomicMin(&p.ckey[p.loc[o]], res_depth_key(p, q)); }
     }
-    __syncthreads();
+    sync();
     carry = 0;
-    for (int base = 0; base < ncomp; base += NT) {
-        const int c = base + tid;
+    for (int base = 0; base < ncomp; base += GNT) {
+        const int c = base + gtid;
         int tot;
-        const int off = res_scan(c < ncomp ? p.cnp[c] : 0, sScan, tot);
+        const int off = scan(c < ncomp ? p.cnp[c] : 0, tot);
         if (c < ncomp) p.cstart[c] = carry + off;
         carry += tot;
     }
-    __syncthreads();
-    for (int q = tid; q < np; q += NT) {
+    sync();
+    for (int q = gtid; q < np; q += GNT) {
         const int o = res_owner(p, q, p.label);
         if (o < 0) continue;
         const int c = p.loc[o];
         p.cq[p.cstart[c] + atomicAdd(&p.cfill[c], 1)] = q;
     }
-    __syncthreads();
+    sync();
     // a detached body's system: its own pairs (cfill of them, in cq) and the pairs of its partners' components;
     // cnp = the total, which decides the class
-    for (int c = tid; c < ncomp; c += NT) {
+    for (int c = gtid; c < ncomp; c += GNT) {
         int tot = p.cnp[c], key = p.ckey[c];
         const int own = p.cown[c];
         if (own >= 0) {
@@ -338,11 +384,12 @@ __global__ void __launch_bounds__(RES_LABEL_THREADS) resolve_label_kernel(ResPar
         }
         p.cnp[c] = tot;
         int cls = res_class(tot);
-        if (cls == 5 && key < __float_as_int(RES_DEEP_RATIO)) cls = 6;      // scheduling only: the long chains first
+        if (cls == 5 && key < __float_as_int(RES_DEEP_RATIO))              // scheduling only: the long chains first, by depth
+            cls = key < __float_as_int(RES_DEEP_RATIO / 64.f) ? 6 : key < __float_as_int(RES_DEEP_RATIO / 16.f) ? 7 : key < __float_as_int(RES_DEEP_RATIO / 4.f) ? 8 : 9;
         p.clist[(size_t)cls * p.cap + atomicAdd(&p.ctl[RES_CTL_CNT + cls], 1)] = c;
     }
-    __syncthreads();
-    if (tid == 0) {
+    sync();
+    if (gtid == 0) {
         p.ctl[0] = ncomp;
         p.mode[1] = (p.ctl[RES_CTL_CNT + 1] + p.ctl[RES_CTL_CNT + 2] + p.ctl[RES_CTL_CNT + 3] + p.ctl[RES_CTL_CNT + 4]) > 0 ? 1 : 0;
     }
@@ -1003,9 +1050,10 @@ __global__ void __launch_bounds__(RES_S_THREADS, RES_S_MINB) resolve_small_kerne
         __syncthreads();
         ticket = sCtl[0];
     }
-    const int ndeep = p.ctl[RES_CTL_CNT + 6];                            // the systems that look deep first
-    if (ticket >= ndeep + p.ctl[RES_CTL_CNT + 5]) break;
-    const int comp = ticket < ndeep ? p.clist[(size_t)6 * p.cap + ticket] : p.clist[(size_t)5 * p.cap + ticket - ndeep];
+    int cls = 6, tk = ticket;                                              // the systems that look deep first, deepest first
+    while (cls <= 9 && tk >= p.ctl[RES_CTL_CNT + cls]) { tk -= p.ctl[RES_CTL_CNT + cls]; ++cls; }
+    if (cls > 9) { cls = 5; if (tk >= p.ctl[RES_CTL_CNT + 5]) break; }
+    const int comp = p.clist[(size_t)cls * p.cap + tk];
     const int np = p.cnp[comp];
     const int own = p.cown[comp];                                          // a detached body's system (see res_owner), else -1
 

@@ -1156,6 +1156,31 @@ def test_resolve_big_star_components(M, K, rmin):
     assert _rel_vec_err(gv[:, :1], v1[:, :1]).max() > 1e-12               # the giant felt its planetesimals
 
 
+def test_resolve_big_x_all_thousands_of_detached_systems(M):
+    """the production regime at a size the oracle takes a second for (N = 250,000, nbig = 100: ~3,100 listed pairs, ~3,000
+    test-particle systems): the label kernel's cluster path (more than 2048 pairs: 8 CTAs, scans and flags exchanged
+    through their shared memory), the depth levels of resolve_small_kernel's dispatch, the detached systems' cores."""
+    w = W.make_bigsmall(250_000, 100)
+    mu, gm, dt, tol = G * w.m_star, G * w.mass, w.dt, 1e-12
+    x1, v1, _ = oracle.drift(mu, dt, w.x, w.v)
+    enc = oracle.encounters(dt, w.x, w.v, x1, v1, w.rcrit, nbig=100)
+    assert enc["count"] > 2048
+    ref = oracle.resolve(mu, gm, w.rcrit, dt, w.x, w.v, x1, v1, enc["pairs"])
+    assert ref["fail"] == 0
+    gx, gv, st, stats = _gpu_resolve(M, w.mass, w.x, w.v, x1, v1, w.rcrit, w.m_star, dt, tol, enc["pairs"], nbig=100)
+    idx = np.unique(enc["pairs"]); rest = np.setdiff1d(np.arange(w.nb), idx)
+    # counted: the bodies a system wrote back - every listed test particle, and the big bodies that feel another big body (a
+    # big body whose partners are all massless feels nothing: it is integrated along in their systems, its drift stands)
+    pr = enc["pairs"]; mm = (w.mass[pr[:, 0]] > 0) & (w.mass[pr[:, 1]] > 0)
+    n_min = int((w.mass[idx] == 0).sum()) + len(np.unique(pr[mm]))
+    assert st["fail"] == 0 and stats.resolve_fail == 0 and n_min <= st["bodies"] <= len(idx), (st, n_min, len(idx))
+    ex, ev = _rel_vec_err(gx[:, idx], ref["x"][:, idx]), _rel_vec_err(gv[:, idx], ref["v"][:, idx])
+    assert ex.max() <= 1e-10 and ev.max() <= 1e-10                        # (a grazing passage amplifies the FP64 / long-double difference)
+    assert np.mean(ex <= RES_RTOL(tol)) > 0.99 and np.mean(ev <= RES_RTOL(tol)) > 0.99
+    assert np.array_equal(gx[:, rest], x1[:, rest]) and np.array_equal(gv[:, rest], v1[:, rest])
+    assert _rel_vec_err(gv[:, idx], v1[:, idx]).max() > 1e-8               # the encounters matter
+
+
 @pytest.mark.parametrize("K", [60, 900])
 def test_resolve_massless_planetesimals_are_detached(M, K):
     """big x all regime (mo_set_nbig): the K test particles inside a giant's radius are massless, the giant feels nothing.

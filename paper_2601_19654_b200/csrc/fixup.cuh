@@ -92,16 +92,20 @@ __device__ __forceinline__ double fix_w(double s2, double rc) {
 }
 
 constexpr int FIX_CHUNK = 256;   // flagged bodies staged per pass of fix_unflagged_kernel
-constexpr int FIX_FB = 8;        // flagged bodies per CTA of fix_flagged_kernel
+constexpr int FIX_FB = 4;        // flagged bodies per CTA of fix_flagged_kernel
 constexpr int FIX_JS = 8;        // j splits of a flagged body's row
 
-constexpr int FIX_UT = 128;      // threads of fix_unflagged_kernel (one body each): small CTAs, more of them per SM
+constexpr int FIX_UT = 256;      // threads of fix_unflagged_kernel
+constexpr int FIX_SP = 4;        // lanes that share a body there (measured at cfg3, 725 flagged bodies: 128 threads x 1 lane
+                                 // 225 us, 128 x 2 201, 128 x 4 198, 256 x 4 187, 256 x 8 203)
 __global__ void __launch_bounds__(FIX_UT) fix_unflagged_kernel(FixParams p) {
     __shared__ double sN[3][FIX_CHUNK], sO[3][FIX_CHUNK], sG[FIX_CHUNK], sR[FIX_CHUNK];
     if (gate_closed(p.gate)) return;
     const int nf = *p.nf;
     if (nf == 0) return;
-    const int i = blockIdx.x * FIX_UT + threadIdx.x;
+    // FIX_SP neighbouring lanes share a body and take every FIX_SP-th flagged body of a chunk: more warps per SM for the
+    // same staging (one warp in flight per 8 cycles of FP64 latency and sub-partition was not enough)
+    const int i = blockIdx.x * (FIX_UT / FIX_SP) + threadIdx.x / FIX_SP, h = threadIdx.x % FIX_SP;
     const bool mine = i < p.nb && !p.flag[i];
     double xi = 0.0, yi = 0.0, zi = 0.0, rci = 0.0;
     if (mine) { xi = p.x[i]; yi = p.x[p.ld + i]; zi = p.x[2 * p.ld + i]; rci = p.rcrit[i]; }
@@ -118,7 +122,7 @@ __global__ void __launch_bounds__(FIX_UT) fix_unflagged_kernel(FixParams p) {
         __syncthreads();
         if (mine) {
 #pragma unroll 4
-            for (int t = 0; t < m; ++t) {
+            for (int t = h; t < m; t += FIX_SP) {
                 const double g = sG[t];
                 const double rc = fmax(rci, sR[t]);
                 const double nx = sN[0][t] - xi, ny = sN[1][t] - yi, nz = sN[2][t] - zi;
@@ -129,12 +133,18 @@ __global__ void __launch_bounds__(FIX_UT) fix_unflagged_kernel(FixParams p) {
             }
         }
     }
-    if (mine) { p.a[i] += c0; p.a[p.ld + i] += c1; p.a[2 * p.ld + i] += c2; }
+#pragma unroll
+    for (int o = 1; o < FIX_SP; o <<= 1) {                 // the sharing lanes' sums, in a fixed order
+        c0 += __shfl_xor_sync(0xffffffffu, c0, o); c1 += __shfl_xor_sync(0xffffffffu, c1, o); c2 += __shfl_xor_sync(0xffffffffu, c2, o);
+    }
+    if (mine && h == 0) { p.a[i] += c0; p.a[p.ld + i] += c1; p.a[2 * p.ld + i] += c2; }
 }
 
 // rows of the flagged bodies over the resolved positions: CTA (g, js) sums FIX_FB rows over the js-th part of the bodies j
 // (every j loaded once for FIX_FB rows), fixed-order block sum -> part[js][f][c]
-__global__ void __launch_bounds__(FIX_THREADS) fix_flagged_kernel(FixParams p) {
+// (measured at cfg3, 725 flagged bodies: 8 rows per CTA at 169 registers - one CTA per SM - 154 us; 4 rows and two CTAs per
+// SM 109 us; 2 rows 164 us)
+__global__ void __launch_bounds__(FIX_THREADS, 2) fix_flagged_kernel(FixParams p) {
     __shared__ double sh[FIX_THREADS / 32][3 * FIX_FB];
     if (gate_closed(p.gate)) return;
     const int nf = *p.nf;

@@ -915,7 +915,7 @@ static mo_status enqueue_step(mo_ctx* ctx, double dt) {
         FixParams fp;
         fp.x = ctx->x; fp.x1 = ctx->x1; fp.gm = ctx->gm; fp.rcrit = ctx->rcrit; fp.flag = ctx->flag; fp.flist = ctx->fix_list; fp.nf = ctx->fix_nf;
         fp.a = ctx->a; fp.part = ctx->fix_part; fp.nb = ctx->nb; fp.ld = ctx->ld; fp.gate = gO;
-        fix_unflagged_kernel<<<(ctx->nb + FIX_UT - 1) / FIX_UT, FIX_UT, 0, mainS>>>(fp);
+        fix_unflagged_kernel<<<(ctx->nb + FIX_UT / FIX_SP - 1) / (FIX_UT / FIX_SP), FIX_UT, 0, mainS>>>(fp);
         s = post_launch(ctx);
         if (s != MO_OK) return s;
         // (the number of flagged bodies is not known on the host: CTAs beyond the list exit at once)

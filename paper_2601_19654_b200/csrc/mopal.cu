@@ -136,15 +136,16 @@ static inline void shard_range(long long n, int rank, int world, long long* lo, 
 
 // The work units of the two-sided pair kernel, in launch (= dispatch) order: row blocks I ascending, each block's j tiles
 // from its diagonal on in chunks of ch tiles.  All CTA slots are busy until the list runs out, and then the kernel is as
-// long as the last units to finish: so the end of the list is cut finer - the last slots * ch / 2 tiles one per unit (they
-// level the spread of the slots' finishing times, which is about one chunk), and of those the last slots / 2 tiles one
-// GROUP of 32 columns per unit (a quarter tile: the finest piece the warp rotation works on).  A system with fewer tiles
-// than slots (N = 4096: 272 tiles for 592 slots) is cut into groups throughout: twice the resident warps per SM.
+// long as the last units to finish: so the end of the list is cut finer and finer ("guided"): levels of `slots` units
+// each, of .., 4, 2, 1 tiles - every level halves the spread of the slots' finishing times that the level before it left -
+// and last slots / 2 tiles one GROUP of 32 columns per unit (a quarter tile: the finest piece the warp rotation works
+// on).  A system with fewer tiles than two per slot (N = 4096: 272 tiles for 592 slots) is cut into groups throughout: twice
+// the resident warps per SM.  Long chunks before the tail keep the units few: every unit writes a row partial of
+// 24 R bytes that sym_reduce_kernel reads back (cfg3: 5599 units of at most 5 tiles -> 2700 of at most 18: half the
+// DRAM traffic of the partial sums, the same kernel time; profiles/r2e_tail_and_priorities.md).
 static void plan_sym_units(mo_ctx* ctx, long long tot, long long slots) {
     const int TPB = ctx->sym_ipt, ch = ctx->sym_ch;
-    // (measured, profiles/r2e_tail_and_priorities.md: half as much or twice as much of either changes nothing)
     const long long tailQ = tot < 2 * slots ? tot : slots / 2;
-    const long long tail1 = tailQ + (ch > 1 ? slots * ch / 2 : 0);
     ctx->h_units.clear(); ctx->h_ustart.clear(); ctx->h_uwork.clear();
     long long seen = 0, work = 0;        // tiles before the current one; groups before the current unit
     for (int I = 0; I < ctx->sym_nI; ++I) {
@@ -160,9 +161,17 @@ static void plan_sym_units(mo_ctx* ctx, long long tot, long long slots) {
                 t += 1; seen += 1;
                 continue;
             }
-            int n = left <= tail1 ? 1 : ch;
+            // (the first tenth of the work in units of two tiles: in the resolving step it is launched on its own, beside
+            // the encounter pass, and the encounter solve's CTAs - whole SMs - can only start when its CTAs have left:
+            // cfg3 with resolution 3.45 ms per step with units of 4 tiles there, 3.39 with 2, 3.37 with 1)
+            int n = seen < tot / 10 && ch > 2 ? 2 : ch;
+            long long lo = tailQ;                               // where the next finer level begins
+            for (int m = 1; m < ch; m *= 2) {
+                if (left <= lo + slots * m) { n = m < n ? m : n; break; }
+                lo += slots * m;
+            }
             if (n > ctx->nTiles - t) n = ctx->nTiles - t;
-            if (left - n < tailQ) n = (int)(left - tailQ);      // the chunk ends where the finer tail begins
+            if (left - n < lo) n = (int)(left - lo);            // the chunk ends where the finer tail begins
             ctx->h_uwork.push_back(work); work += (long long)n * (TJ / 32);
             ctx->h_units.push_back(make_int4(I, t, t + n, (TJ / 32) << 8));
             t += n; seen += n;
@@ -326,10 +335,11 @@ static void choose_geometry(mo_ctx* ctx) {
         ctx->sym_nI = (ctx->nbPad + R - 1) / R;
         long long tot = 0;
         for (int I = 0; I < ctx->sym_nI; ++I) tot += ctx->nTiles - I * TPB;
-        long long ch = (tot + 16 * sslots - 1) / (16 * sslots);   // about sixteen waves of units: short tail
-        if (ch < 1) ch = 1;
-        if (ch > 16) ch = 16;
+        long long ch = (tot + 4 * sslots - 1) / (4 * sslots);     // about four waves of long units before the guided tail (plan_sym_units)
+        if (ch < 4) ch = 4;
+        if (ch > 24) ch = 24;
         ctx->sym_ch = env_int("MO_SYM_CH", (int)ch);
+        if (ctx->sym_ch > 64) ctx->sym_ch = 64;
         if (ctx->sym_ch < 1) ctx->sym_ch = 1;
         plan_sym_units(ctx, tot, sslots);
         ctx->ipt = ctx->sym_ipt; ctx->ctas_per_sm = occs; ctx->nsplit = 1;
@@ -893,7 +903,8 @@ static mo_status enqueue_step(mo_ctx* ctx, double dt) {
         ctx->pair_x = ctx->x1; ctx->gate = gO;
         pack_kernel<false, true><<<ctx->nSrcTiles, TJ, 0, mainS>>>(ctx->x1, ctx->gm, ctx->rcrit, ctx->nb, ctx->nbig, ctx->ld, ctx->tiles, nullptr, 0, 0.0, gO);
         s = post_launch(ctx);
-        const int ucut = ctx->sym_nunits / 10;
+        // (a tenth of the WORK: the units differ in length)
+        const int ucut = (int)(std::lower_bound(ctx->h_uwork.begin(), ctx->h_uwork.end() - 1, ctx->h_uwork.back() / 10) - ctx->h_uwork.begin());
         if (s == MO_OK) { ctx->pair_u0 = 0; ctx->pair_u1 = ucut; s = launch_pair(ctx); }
         if (s == MO_OK) {
             CK(cudaStreamWaitEvent(mainS, ctx->res_fork, 0));

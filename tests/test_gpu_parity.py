@@ -1156,6 +1156,39 @@ def test_resolve_big_star_components(M, K, rmin):
     assert _rel_vec_err(gv[:, :1], v1[:, :1]).max() > 1e-12               # the giant felt its planetesimals
 
 
+def test_resolve_more_star_components_than_clusters(M):
+    """twelve giants on different orbits, each with a star of 80-100 planetesimals (64-255 pairs: the 256-thread class on
+    clusters of 8 CTAs) and one with 300 (the 512-thread class): more components than the 8 clusters of a class, so a cluster
+    takes several components one after the other - its barrier's phases, the warps without a body and the column /
+    tableau / error exchange through the CTAs' shared memory carry over from one component to the next."""
+    rng = np.random.default_rng(77)
+    m_star, mg = 1.0, 1e-3
+    Xs, masses, far = [], [], []
+    for g in range(12):
+        K = 300 if g == 5 else 80 + 2 * g
+        a_g, th = 4.0 + 2.2 * g, 0.55 * g
+        xg = a_g * np.array([np.cos(th), np.sin(th), 0.0])
+        rmax = 0.6 * 3.0 * a_g * (mg / 3.0) ** (1.0 / 3.0)                 # inside 3 Hill radii
+        ang = rng.uniform(0, 2 * np.pi, K); rad = rng.uniform(0.12 * rmax, rmax, K); zz = rng.uniform(-0.01, 0.01, K)
+        X = np.empty((3, K + 1)); X[:, 0] = xg
+        X[0, 1:] = xg[0] + rad * np.cos(ang); X[1, 1:] = xg[1] + rad * np.sin(ang); X[2, 1:] = zz
+        Xs.append(X); masses.append(np.concatenate([[mg], np.full(K, 1e-9)])); far.append(np.concatenate([[True], rad > 0.4 * rmax]))
+    X = np.concatenate(Xs, axis=1); mass = np.concatenate(masses); far = np.concatenate(far)
+    r = np.linalg.norm(X, axis=0); vc = np.sqrt(G * m_star / r)
+    Vh = np.stack([-vc * X[1] / r, vc * X[0] / r, np.zeros(X.shape[1])])
+    V = oracle.h2dh(m_star, mass, Vh)
+    _, rc = oracle.hill(G, m_star, mass, X, V, n_hill=3.0)
+    mu, gm, dt, tol = G * m_star, G * mass, 8.0, 1e-12
+    x1, v1, _ = oracle.drift(mu, dt, X, V)
+    enc = oracle.encounters(dt, X, V, x1, v1, rc)
+    ref = oracle.resolve(mu, gm, rc, dt, X, V, x1, v1, enc["pairs"])
+    assert ref["fail"] == 0 and ref["n"] == X.shape[1]
+    gx, gv, st, stats = _gpu_resolve(M, mass, X, V, x1, v1, rc, m_star, dt, tol, enc["pairs"])
+    assert st["fail"] == 0 and stats.resolve_fail == 0 and st["bodies"] == X.shape[1], st
+    assert _rel_vec_err(gx, ref["x"]).max() <= 1e-10 and _rel_vec_err(gv, ref["v"]).max() <= 1e-10
+    assert _rel_vec_err(gx[:, far], ref["x"][:, far]).max() <= RES_RTOL(tol) and _rel_vec_err(gv[:, far], ref["v"][:, far]).max() <= RES_RTOL(tol)
+
+
 def test_resolve_big_x_all_thousands_of_detached_systems(M):
     """the production regime at a size the oracle takes a second for (N = 250,000, nbig = 100: ~3,100 listed pairs, ~3,000
     test-particle systems): the label kernel's cluster path (more than 2048 pairs: 8 CTAs, scans and flags exchanged

@@ -1156,6 +1156,30 @@ def test_resolve_big_star_components(M, K, rmin):
     assert _rel_vec_err(gv[:, :1], v1[:, :1]).max() > 1e-12               # the giant felt its planetesimals
 
 
+def test_resolve_long_run_keeps_energy_and_angular_momentum(M):
+    """300 steps of cfg1 (N = 4096, two giants: ~28,000 encounter pairs in all, a different pair list, component structure
+    and launch path - beside or before the pair sum - every step).  No oracle at this length (declared: multi-step
+    trajectories beyond ~10 steps are unpinned); what the method fixes instead: the angular momentum to rounding, the
+    energy to the symplectic error of the step size, every component resolved - and the same run WITHOUT resolution
+    loses energy two orders of magnitude faster (the encounters matter)."""
+    w = W.make_config(1)
+    out = {}
+    for tol in (0.0, 1e-12):
+        m = M.Mopal(w.mass, w.x, w.v, w.rcrit, m_star=w.m_star, G=w.G, cap=1 << 18)
+        if tol > 0:
+            m.set_resolve(tol)
+        e0 = m.energy()
+        st = m.step(w.dt, 300)
+        e1 = m.energy()
+        assert st.status == 0 and st.resolve_fail == 0 and st.drift_fail == 0 and st.nce_total > 10_000
+        L0, L1 = np.array(e0["L"]), np.array(e1["L"])
+        assert np.linalg.norm(L1 - L0) <= 1e-13 * np.linalg.norm(L0)
+        out[tol] = abs((e1["E"] - e0["E"]) / e0["E"])
+        m.close()
+    assert out[1e-12] < 1e-8, out
+    assert out[0.0] > 30 * out[1e-12], out
+
+
 def test_resolve_more_star_components_than_clusters(M):
     """twelve giants on different orbits, each with a star of 80-100 planetesimals (64-255 pairs: the 256-thread class on
     clusters of 8 CTAs) and one with 300 (the 512-thread class): more components than the 8 clusters of a class, so a cluster

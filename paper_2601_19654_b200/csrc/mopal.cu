@@ -890,6 +890,10 @@ static mo_status enqueue_step(mo_ctx* ctx, double dt) {
         es.x1 = ctx->x1; es.v1 = ctx->v1;
         ctx->stream = ctx->enc_stream;
         s = enqueue_pairs(ctx, es, 1);
+        if (s == MO_OK) {       // the list of the flagged bodies for the corrections below: the flags are final here
+            fix_list_kernel<<<1, FIX_LIST_THREADS, 0, ctx->stream>>>(ctx->flag, ctx->nb, ctx->fix_list, ctx->fix_nf, Gate{ctx->res_mode, 1});
+            s = post_launch(ctx);
+        }
         if (s == MO_OK) s = enqueue_resolve(ctx, dt, ctx->res_tol);
         ctx->stream = mainS;
         if (s != MO_OK) return s;
@@ -917,9 +921,6 @@ static mo_status enqueue_step(mo_ctx* ctx, double dt) {
         s = post_launch(ctx);
         if (s != MO_OK) return s;
         CK(cudaStreamWaitEvent(mainS, ctx->ev_join, 0));
-        fix_list_kernel<<<1, FIX_LIST_THREADS, 0, mainS>>>(ctx->flag, ctx->nb, ctx->fix_list, ctx->fix_nf, gO);
-        s = post_launch(ctx);
-        if (s != MO_OK) return s;
         kick_psum_kernel<false><<<ctx->npsum, ON_BLOCK, 0, mainS>>>(ctx->v, nullptr, ctx->gm, ctx->nb, ctx->ld, 0.0, ctx->psumB, ctx->ticket + 1);
         s = post_launch(ctx);
         if (s != MO_OK) return s;

@@ -59,7 +59,6 @@ struct mo_ctx {
     int *res_dbodyi = nullptr, *res_dpairi = nullptr;
     long long res_dbodyN = 0;
     int res_smemA = 0, res_smemB = 0, res_smemC = 0;
-    double* res_colres = nullptr; int* res_csync = nullptr;   // clusters: column results, barrier counters
     double* fix_part = nullptr;                      // partial rows of the flagged bodies
     int *fix_list = nullptr, *fix_nf = nullptr;      // the flagged bodies, ascending (the solve beside the pair sum: fixup.cuh)
     const double* pair_x = nullptr;                  // positions the pair kernel reads (nullptr: x)
@@ -374,7 +373,7 @@ extern "C" void mo_destroy(mo_ctx* ctx) {
     cudaFree(ctx->gm); cudaFree(ctx->x0); cudaFree(ctx->v0); cudaFree(ctx->part);
     cudaFree(ctx->psumA); cudaFree(ctx->psumB); cudaFree(ctx->ticket);
     cudaFree(ctx->res_loc); cudaFree(ctx->res_out); cudaFree(ctx->res_tab); cudaFree(ctx->res_label);
-    cudaFree(ctx->res_cnp); cudaFree(ctx->res_cstart); cudaFree(ctx->res_cfill); cudaFree(ctx->res_cq); cudaFree(ctx->res_clist); cudaFree(ctx->res_ctl); cudaFree(ctx->res_aux); cudaFree(ctx->res_cown); cudaFree(ctx->res_ckey); cudaFree(ctx->fix_list); cudaFree(ctx->fix_nf); cudaFree(ctx->fix_part); cudaFree(ctx->res_colres); cudaFree(ctx->res_csync); cudaFree(ctx->res_mode);
+    cudaFree(ctx->res_cnp); cudaFree(ctx->res_cstart); cudaFree(ctx->res_cfill); cudaFree(ctx->res_cq); cudaFree(ctx->res_clist); cudaFree(ctx->res_ctl); cudaFree(ctx->res_aux); cudaFree(ctx->res_cown); cudaFree(ctx->res_ckey); cudaFree(ctx->fix_list); cudaFree(ctx->fix_nf); cudaFree(ctx->fix_part); cudaFree(ctx->res_mode);
     cudaFree(ctx->res_dbody); cudaFree(ctx->res_dpair); cudaFree(ctx->res_dbodyi); cudaFree(ctx->res_dpairi);
     if (ctx->res_host) cudaFreeHost(ctx->res_host);
     for (int k = 0; k < 5; ++k) { if (ctx->res_stream[k]) cudaStreamDestroy(ctx->res_stream[k]); if (ctx->res_join[k]) cudaEventDestroy(ctx->res_join[k]); }
@@ -747,8 +746,6 @@ static mo_status ensure_resolve_scratch(mo_ctx* ctx) {
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_clist, capn * RES_NCLS);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_ctl, (size_t)((RES_CTL_N + 15) & ~15));
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_tab, (size_t)6 * RES_KMAX * 1024 * RES_CL_GRID);   // per CTA of the widest launch
-    if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_colres, (size_t)RES_NCLUSTERS * 2 * RES_NCOL * 6 * 1024);
-    if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_csync, RES_NCLUSTERS);
     if (e == cudaSuccess) e = dalloc(ctx, &ctx->res_mode, 2);
     if (e == cudaSuccess) { const int one[2] = {1, 1}; e = cudaMemcpyAsync(ctx->res_mode, one, sizeof(one), cudaMemcpyHostToDevice, ctx->stream); if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream); }
     // class D pools: every body and every pair of the list can be in a class-D component
@@ -786,7 +783,7 @@ static mo_status enqueue_resolve(mo_ctx* ctx, double dt, double tol) {
     rp.x0 = ctx->x0; rp.v0 = ctx->v0; rp.x = ctx->x; rp.v = ctx->v; rp.gm = ctx->gm; rp.rcrit = ctx->rcrit;
     rp.pairs = ctx->pairs; rp.st = ctx->dstats; rp.out = ctx->res_out; rp.loc = ctx->res_loc; rp.label = ctx->res_label; rp.aux = ctx->res_aux; rp.cown = ctx->res_cown; rp.ckey = ctx->res_ckey;
     rp.cnp = ctx->res_cnp; rp.cstart = ctx->res_cstart; rp.cfill = ctx->res_cfill; rp.cq = ctx->res_cq; rp.clist = ctx->res_clist;
-    rp.ctl = ctx->res_ctl; rp.colres = ctx->res_colres; rp.csync = ctx->res_csync; rp.mode = ctx->res_mode; rp.tab = ctx->res_tab; rp.dbody = ctx->res_dbody; rp.dbodyi = ctx->res_dbodyi; rp.dpair = ctx->res_dpair;
+    rp.ctl = ctx->res_ctl; rp.mode = ctx->res_mode; rp.tab = ctx->res_tab; rp.dbody = ctx->res_dbody; rp.dbodyi = ctx->res_dbodyi; rp.dpair = ctx->res_dpair;
     rp.dpairi = ctx->res_dpairi; rp.dbodyN = ctx->res_dbodyN;
     rp.cap = ctx->cap > 0 ? ctx->cap : 1; rp.nb = ctx->nb; rp.ld = ctx->ld; rp.mu = ctx->mu; rp.h = dt; rp.tol = tol;
     {

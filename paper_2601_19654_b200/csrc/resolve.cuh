@@ -72,8 +72,6 @@ struct ResParams {
     int* cq;                     // cap: pair indices grouped by component (unordered inside a group)
     int* clist;                  // RES_NCLS * cap: the components of each class
     int* ctl;                    // [0] components, [RES_CTL_CNT + c] class counts, [RES_CTL_TKT + c] tickets, [RES_CTL_POOL] streamed-class body pool in use
-    double* colres;              // column results of the clusters: [cluster][2][NCOL][6][threads]
-    int* csync;                  // barrier counters of the clusters (zeroed by the label kernel)
     int* mode;                   // [1] <- 1 if this list holds a component of more than 63 pairs (a long chain: mopal.cu), else 0
     double* tab;                 // extrapolation tableaux of the class-C CTAs whose component does not leave room in shared memory
     double* dbody; int* dbodyi;  // class D pools: planes of dbodyN doubles / ints
@@ -119,20 +117,7 @@ __device__ __forceinline__ int res_scan(int v, int* sScan, int& total) {
 
 __device__ __forceinline__ int res_class(int np) { return np <= RES_PHI_S ? 5 : np <= RES_PHI_0 ? 0 : np <= RES_PHI_1 ? 1 : np <= RES_PHI_2 ? 2 : np <= RES_PHI_3 ? 3 : 4; }
 
-// barrier of the CTAs of a cluster that work on one component: every CTA's thread 0 counts itself in and waits for the
-// others (the cluster's CTAs are co-scheduled, so nobody waits for a CTA that is not running); the CTA's other live warps
-// wait at its named barrier.  Global writes before the barrier are visible after it (fences on both sides; readers use ld.cg).
 __device__ __forceinline__ void res_bar(int nthreads);
-__device__ __forceinline__ void res_cluster_barrier(int* cnt, int target, int nact) {
-    __threadfence();
-    res_bar(nact);
-    if (threadIdx.x == 0) {
-        atomicAdd(cnt, 1);
-        while (*reinterpret_cast<volatile int*>(cnt) < target) { }
-        __threadfence();
-    }
-    res_bar(nact);
-}
 
 // producer / consumer halves of named barrier id (n threads in all): the producers arrive and go on, the consumers wait
 __device__ __forceinline__ void res_nb_arrive(int id, int n) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(n) : "memory"); }
@@ -222,7 +207,6 @@ __global__ void __launch_bounds__(RES_LABEL_THREADS) resolve_label_kernel(ResPar
     const int NC = solo ? 1 : (int)gridDim.x;
     const int gtid = rank * NT + tid, GNT = NC * NT;
     if (gtid == 0) { *p.out = ResStats{0, 0, 0, 0}; for (int k = 0; k < RES_CTL_N; ++k) p.ctl[k] = 0; }
-    if (gtid < RES_NCLUSTERS) p.csync[gtid] = 0;
     if (nce <= 0 || nce > p.cap) { if (gtid == 0) p.mode[1] = 0; }
     if (nce <= 0) return;
     if (nce > p.cap) { if (gtid == 0) { p.out->fail = 1 << 30; atomicAdd(&p.st->resolve_fail, 1); } return; }      // truncated list: nothing can be resolved
@@ -479,8 +463,8 @@ __global__ void __launch_bounds__(NT, 1) resolve_solve_kernel(ResParams p, int s
     // row maxima of the error estimates and, after an accepted step, its bodies' increments from their owners.  Measured
     // on Jupiter's star at cfg3 (342 bodies, 92 attempted steps; per attempt, longest column 22 us): with the results in
     // global memory and the whole tableau in every CTA the exchange cost 5 + 14 us per attempt (profiles/r2d_resolve.md).
-    // Class 3 (1024 threads) has no shared memory left for the columns and keeps the exchange through global memory.
-    constexpr bool SLICE = NCOL > 1 && NT <= 512;
+    // The slice's tableau is in shared memory when there is room (always, up to 512 bodies), else in global scratch.
+    constexpr bool SLICE = NCOL > 1;
     __shared__ double sRedK[SLICE ? 4 : 1][RES_KMAX];                      // the slice warps' error maxima of every tableau row
     __shared__ double sErr[RES_KMAX];                                      // this CTA's slice: error maximum of every row
     __shared__ int sStop;                                                  // the cluster-barrier phase after which the warps without a body leave
@@ -493,8 +477,6 @@ __global__ void __launch_bounds__(NT, 1) resolve_solve_kernel(ResParams p, int s
     // side by side a step costs its longest column instead of their sum); components dealt to the clusters round-robin
     const int col = NCOL > 1 ? (int)(blockIdx.x % NCOL) : 0;
     const int cl = blockIdx.x / NCOL, ncl = gridDim.x / NCOL;
-    const int cslot = NCOL > 1 ? (CLS - 1) * (RES_NCLUSTERS / 3) + cl : 0;   // this cluster's barrier counter and result buffer
-    int nbarrier = 0;                                                      // cluster barriers passed so far (all CTAs alike)
     int round = 0;
 
     for (;;) {
@@ -664,7 +646,12 @@ __global__ void __launch_bounds__(NT, 1) resolve_solve_kernel(ResParams p, int s
     __syncthreads();                                                       // the temporaries (on sF, sDy) are consumed; sAdj is complete
     const int S = nbp / (NCOL > 1 ? NCOL : 1);                              // SLICE: bodies of the tableau slice of a CTA (nbp is a multiple of 32)
     const int SLW = (S + 31) & ~31;                                         // ... and the threads (whole warps) that work on it
-    double* const sT = reinterpret_cast<double*>(res_dyn + pairBytes + bodyBytes);   // SLICE: [6 KMAX][S] tableau of this CTA's slice
+    // SLICE: [6 KMAX][S] tableau of this CTA's slice - in shared memory when there is room (always, up to 512 bodies), else in
+    // this CTA's part of the global scratch (the cluster's barrier orders its writes before the other CTAs' ld.cg reads)
+    // (known at compile time for the classes up to 512 threads: plain shared-memory addressing there)
+    const bool sliceShared = NT <= 512 || pairBytes + bodyBytes + 6 * RES_KMAX * 8 * S <= smemBytes;
+    double* const sT = reinterpret_cast<double*>(res_dyn + pairBytes + bodyBytes);
+    double* const gT = p.tab + (size_t)blockIdx.x * 6 * RES_KMAX * NT;
     const bool tabShared = pairBytes + bodyBytes + 6 * RES_KMAX * 8 * nbp <= smemBytes;
     const int TS = tabShared ? nbp : NT;                                    // tableau stride
     double* const Tb = (tabShared ? reinterpret_cast<double*>(res_dyn + pairBytes + bodyBytes)
@@ -838,7 +825,7 @@ __global__ void __launch_bounds__(NT, 1) resolve_solve_kernel(ResParams p, int s
 #pragma unroll
                 for (int c = 0; c < 3; ++c) { nxt[c] = res_ld_remote(&sP[c * nbp + bb], 0); nxt[3 + c] = res_ld_remote(&sF[c * npad + bb], 0); }
                 const double isx = sIS[bb], isv = sIS[nbp + bb];
-                double* const T = sT + tid;
+                double* const T = (sliceShared ? sT : gT) + tid;
 #pragma unroll 1
                 for (int k = 0; k <= kcols; ++k) {
                     double cur[6], prev[6];
@@ -906,32 +893,15 @@ __global__ void __launch_bounds__(NT, 1) resolve_solve_kernel(ResParams p, int s
             if (acc >= 0 && live) {                                        // this body's increment from the CTA that ran its tableau
                 const int o = tid / S, i = tid - o * S;
 #pragma unroll
-                for (int c = 0; c < 6; ++c) sY[c * nbp + tid] += res_ld_remote(&sT[(acc * 6 + c) * S + i], o);
+                for (int c = 0; c < 6; ++c)
+                    sY[c * nbp + tid] += sliceShared ? res_ld_remote(&sT[(acc * 6 + c) * S + i], o)
+                                                     : __ldcg(&p.tab[((size_t)blockIdx.x - col + o) * 6 * RES_KMAX * NT + (size_t)(acc * 6 + c) * S + i]);
             }
-        }
-        double* const cres = NCOL > 1 && !SLICE ? p.colres + ((size_t)(cslot * 2 + (nbarrier & 1)) * NCOL) * 6 * 1024 : nullptr;   // [column][component][thread], 1024 per plane
-        if constexpr (NCOL > 1 && !SLICE) {
-            // every CTA its own column (the CTAs beyond the columns this step tries: f(y) only), results through global
-            // memory, one barrier of the cluster per Bulirsch-Stoer step
-            double mine[6];
-            column(col, col <= kcols, mine);
-            if (live && col <= kcols) {
-#pragma unroll
-                for (int c = 0; c < 6; ++c) cres[((size_t)col * 6 + c) * 1024 + tid] = mine[c];
-            }
-            ++nbarrier;
-            res_cluster_barrier(p.csync + cslot, NCOL * nbarrier, nact);
-            if (col == 0) nrhs += (kcols + 1) * (kcols + 2) - 2;            // the other columns' right-hand sides: sum of 2 (k + 1)
         }
 #pragma unroll 1
         for (int k = 0; !SLICE && k <= kcols; ++k) {
             double cur[6];
-            if constexpr (NCOL > 1) {
-#pragma unroll
-                for (int c = 0; c < 6; ++c) cur[c] = live ? __ldcg(&cres[((size_t)k * 6 + c) * 1024 + tid]) : 0.0;
-            } else {
-                column(k, true, cur);
-            }
+            column(k, true, cur);
             // row k of the tableau from row k-1 (in T), overwriting it column by column
             double err = 0.0;
             if (live) {
